@@ -1,0 +1,191 @@
+"""ctypes loader + stage-by-stage driver for the CPU oracle (oracle/tpc_oracle.cpp).
+
+TEST INFRASTRUCTURE, NOT PRODUCT: only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+--impl reference legs may import this.  It never imports paper_2502_09138_b200.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import time
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libtpc_oracle.so")
+_SRC = [os.path.join(_HERE, "tpc_oracle.cpp"), os.path.join(_HERE, "tpc_oracle.h")]
+
+
+class Params(C.Structure):
+    _fields_ = [
+        ("w_y", C.c_int32), ("w_z", C.c_int32), ("cost_wy", C.c_int32), ("cost_wz", C.c_int32),
+        ("c_max", C.c_int32), ("l_min", C.c_int32),
+        ("units_per_cm", C.c_double), ("sigma_y", C.c_double), ("sigma_z", C.c_double),
+        ("sinphi_max", C.c_double), ("max_miss", C.c_int32), ("n_min_tracklet", C.c_int32),
+        ("gate_d", C.c_double), ("gate_y_cm", C.c_double), ("gate_z_cm", C.c_double),
+        ("c_reset", C.c_double * 5), ("cq_per_tesla", C.c_double), ("n_min_owned", C.c_int32),
+    ]
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with g++ -O2 -fopenmp if missing or stale."""
+    stale = (not os.path.exists(_SO)) or any(os.path.getmtime(s) > os.path.getmtime(_SO) for s in _SRC)
+    if force or stale:
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fopenmp", "-fPIC", "-shared", "-Wall",
+                               _SRC[0], "-o", _SO])
+    return _SO
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_find_seeds.restype = C.c_int64
+        _lib.orc_select.restype = C.c_int64
+        _lib.orc_update.restype = C.c_double
+        _lib.orc_transport.restype = C.c_int
+        _lib.orc_num_threads.restype = C.c_int
+    return _lib
+
+
+def default_params() -> Params:
+    p = Params()
+    lib().orc_default_params(C.byref(p))
+    return p
+
+
+def _p(a, t):
+    return a.ctypes.data_as(C.POINTER(t))
+
+
+def _i32(a):
+    return _p(a, C.c_int32)
+
+
+def _u32(a):
+    return _p(a, C.c_uint32)
+
+
+def _f64(a):
+    return _p(a, C.c_double)
+
+
+def neighbours(y, z, row_offsets, n_sectors, n_rows, params=None, brute=False):
+    p = params or default_params()
+    n = y.shape[0]
+    up = np.empty(n, dtype=np.int32)
+    dn = np.empty(n, dtype=np.int32)
+    f = lib().orc_neighbours_brute if brute else lib().orc_neighbours_pruned
+    f(C.byref(p), C.c_int32(n_sectors), C.c_int32(n_rows), _i32(y), _i32(z), _u32(row_offsets), _i32(up), _i32(dn))
+    return up, dn
+
+
+def clean_links(up, dn):
+    n = up.shape[0]
+    upc = np.empty(n, dtype=np.int32)
+    dnc = np.empty(n, dtype=np.int32)
+    lib().orc_clean_links(C.c_int64(n), _i32(up), _i32(dn), _i32(upc), _i32(dnc))
+    return upc, dnc
+
+
+def find_seeds(upc, dnc, params=None):
+    p = params or default_params()
+    n = upc.shape[0]
+    cap = n // max(1, p.l_min) + 1
+    start = np.empty(cap, dtype=np.int32)
+    length = np.empty(cap, dtype=np.int32)
+    ns = lib().orc_find_seeds(C.byref(p), C.c_int64(n), _i32(upc), _i32(dnc), _i32(start), _i32(length))
+    return start[:ns].copy(), length[:ns].copy()
+
+
+def transport(state, cov, dx, cq, sinphi_max=0.95):
+    st = np.array(state, dtype=np.float64)
+    cv = None if cov is None else np.array(cov, dtype=np.float64).reshape(25)
+    ok = lib().orc_transport(C.c_double(cq), C.c_double(sinphi_max), C.c_double(dx), _f64(st),
+                             _f64(cv) if cv is not None else None)
+    return bool(ok), st, (None if cv is None else cv.reshape(5, 5))
+
+
+def jacobian(state, dx, cq):
+    st = np.array(state, dtype=np.float64)
+    F = np.empty(25, dtype=np.float64)
+    lib().orc_jacobian(C.c_double(cq), C.c_double(dx), _f64(st), _f64(F))
+    return F.reshape(5, 5)
+
+
+def update(state, cov, ym, zm, sy2, sz2):
+    st = np.array(state, dtype=np.float64)
+    cv = np.array(cov, dtype=np.float64).reshape(25)
+    chi2 = lib().orc_update(_f64(st), _f64(cv), C.c_double(ym), C.c_double(zm), C.c_double(sy2), C.c_double(sz2))
+    return st, cv.reshape(5, 5), float(chi2)
+
+
+def follow(y_cm, z_cm, row_offsets, n_sectors, n_rows, row_x, bz, upc, seed_start, seed_len, params=None,
+           search_mode=1):
+    p = params or default_params()
+    ns = seed_start.shape[0]
+    par = np.zeros((ns, 6), dtype=np.float64)
+    cov = np.zeros((ns, 15), dtype=np.float64)
+    chi2 = np.zeros(ns, dtype=np.float64)
+    n_hits = np.zeros(ns, dtype=np.int32)
+    hits = np.full((ns, n_rows), -1, dtype=np.int32)
+    y_cm = np.ascontiguousarray(y_cm, dtype=np.float64)
+    z_cm = np.ascontiguousarray(z_cm, dtype=np.float64)
+    row_x = np.ascontiguousarray(row_x, dtype=np.float64)
+    lib().orc_follow(C.byref(p), C.c_double(bz), C.c_int32(n_sectors), C.c_int32(n_rows), _f64(row_x), _f64(y_cm),
+                     _f64(z_cm), _u32(row_offsets), _i32(upc), C.c_int64(ns), _i32(seed_start), _i32(seed_len),
+                     C.c_int(search_mode), _f64(par), _f64(cov), _f64(chi2), _i32(n_hits), _i32(hits))
+    return par, cov, chi2, n_hits, hits
+
+
+def select(n, n_rows, seed_start, n_hits, hits, params=None):
+    p = params or default_params()
+    ns = seed_start.shape[0]
+    owner = np.empty(n, dtype=np.int32)
+    trk_seed = np.empty(ns, dtype=np.int32)
+    trk_n = np.empty(ns, dtype=np.int32)
+    trk_off = np.empty(ns, dtype=np.int32)
+    hit_ids = np.empty(int(np.maximum(n_hits, 0).sum()) + 1, dtype=np.int32)
+    nh = C.c_int64(0)
+    hits = np.ascontiguousarray(hits, dtype=np.int32)
+    nt = lib().orc_select(C.byref(p), C.c_int64(n), C.c_int32(n_rows), C.c_int64(ns), _i32(seed_start), _i32(n_hits),
+                          _i32(hits), _i32(owner), _i32(trk_seed), _i32(trk_n), _i32(trk_off), _i32(hit_ids),
+                          C.byref(nh))
+    return owner, trk_seed[:nt].copy(), trk_n[:nt].copy(), trk_off[:nt].copy(), hit_ids[:nh.value].copy()
+
+
+def track(ev, params=None, *, brute=False, search_mode=1, exact_coords=False, timings=None):
+    """Whole path on one generated event (gen.events.Event).  Returns a dict with every stage's output.
+
+    exact_coords=True feeds the follower the un-smeared, un-quantised doubles (y_exact/z_exact) instead of
+    int/units_per_cm: the oracle-internal entry that bypasses quantisation (SURVEY 8c pin table)."""
+    p = params or default_params()
+    t = [time.perf_counter()]
+    up, dn = neighbours(ev.y, ev.z, ev.row_offsets, ev.n_sectors, ev.n_rows, p, brute=brute)
+    t.append(time.perf_counter())
+    upc, dnc = clean_links(up, dn)
+    ss, sl = find_seeds(upc, dnc, p)
+    t.append(time.perf_counter())
+    if exact_coords:
+        y_cm, z_cm = ev.y_exact, ev.z_exact
+    else:
+        y_cm, z_cm = ev.y / p.units_per_cm, ev.z / p.units_per_cm
+    par, cov, chi2, n_hits, hits = follow(y_cm, z_cm, ev.row_offsets, ev.n_sectors, ev.n_rows, ev.row_x, ev.cfg.bz,
+                                          upc, ss, sl, p, search_mode)
+    t.append(time.perf_counter())
+    owner, trk_seed, trk_n, trk_off, hit_ids = select(ev.n, ev.n_rows, ss, n_hits, hits, p)
+    t.append(time.perf_counter())
+    if timings is not None:
+        timings.update(neighbours=t[1] - t[0], clean_seeds=t[2] - t[1], follow=t[3] - t[2], select=t[4] - t[3],
+                       total=t[4] - t[0])
+    return dict(link_up=up, link_dn=dn, up_c=upc, dn_c=dnc, seed_start=ss, seed_len=sl, par=par, cov=cov,
+                chi2=chi2, n_hits=n_hits, hits=hits, owner=owner, trk_seed=trk_seed, trk_n_owned=trk_n,
+                trk_hit_offset=trk_off, hit_ids=hit_ids)
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())

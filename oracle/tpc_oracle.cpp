@@ -1,0 +1,523 @@
+// tpc_oracle.cpp -- CPU oracle (fp64) for TPC sector track finding.  TEST INFRASTRUCTURE, NOT PRODUCT.
+// See tpc_oracle.h for the contract.  Follows SURVEY.md section 8(c) / Appendix C step by step
+// (PAPER.md:29, :40 name the task only; BASELINE.json north_star names the five stages).
+// Independent of the CUDA path: no shared code, headers, tables or constants.
+//
+// Pins (tests/test_oracle_*.py): grid == brute force; mutual links; chain partition invariants;
+// transport == closed-form circle/helix and reversibility; Jacobian == central finite differences and
+// == long-double closed form; straight-line limit == weighted least squares (numpy lstsq); exact helices
+// reconstructed to 1e-4; <=1 owner per hit.  Unpinned by the paper: the free constants of orc_params_t and
+// the efficiency / fake-rate values themselves ("parity unpinned" beyond the 100 % zero-smearing case).
+#include "tpc_oracle.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <limits>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+extern "C" void orc_default_params(orc_params_t* p) {
+  p->w_y = 1280;  // P7: 2.0 cm
+  p->w_z = 1600;  // P7: 2.5 cm
+  p->cost_wy = 9; // P8
+  p->cost_wz = 4;
+  p->c_max = 3538944;  // P10 = 16 * 221184
+  p->l_min = 5;        // P13
+  p->units_per_cm = 640.0;  // P3
+  p->sigma_y = 0.1;         // P15
+  p->sigma_z = 0.15;
+  p->sinphi_max = 0.95;  // P18
+  p->max_miss = 5;       // P20
+  p->n_min_tracklet = 10;  // P24
+  p->gate_d = 15.0;        // P21
+  p->gate_y_cm = 2.0;
+  p->gate_z_cm = 2.5;
+  p->c_reset[0] = 0.25;  // P22
+  p->c_reset[1] = 0.25;
+  p->c_reset[2] = 0.05;
+  p->c_reset[3] = 0.05;
+  p->c_reset[4] = 25.0;
+  p->cq_per_tesla = -0.00299792458;  // P4
+  p->n_min_owned = 10;               // P27
+}
+
+extern "C" int orc_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+// ------------------------------------------------------------------------------------------------
+// Stage 1-2: neighbours.  SURVEY 8(c): for cluster h in row r (1 <= r <= n_rows-2, P5), candidates
+// U in row r+1 and D in row r-1 of the same sector inside the inclusive window (P7); choose the pair
+// minimising (cost, id_u, id_d) lexicographically (P8, P9); accept iff cost <= c_max (P10).
+// ------------------------------------------------------------------------------------------------
+static inline bool in_window(const orc_params_t* p, int32_t yh, int32_t zh, int32_t yc, int32_t zc) {
+  int64_t dy = (int64_t)yc - yh, dz = (int64_t)zc - zh;
+  return std::llabs(dy) <= p->w_y && std::llabs(dz) <= p->w_z;
+}
+
+static inline int64_t pair_cost(const orc_params_t* p, int32_t yh, int32_t zh, int32_t yu, int32_t zu, int32_t yd,
+                                int32_t zd) {
+  int64_t ddy = (int64_t)yu + yd - 2 * (int64_t)yh;
+  int64_t ddz = (int64_t)zu + zd - 2 * (int64_t)zh;
+  return p->cost_wy * ddy * ddy + p->cost_wz * ddz * ddz;
+}
+
+static void best_pair(const orc_params_t* p, const int32_t* y, const int32_t* z, int32_t h,
+                      const std::vector<int32_t>& U, const std::vector<int32_t>& D, int32_t* up, int32_t* dn) {
+  int64_t best_cost = std::numeric_limits<int64_t>::max();
+  int32_t bu = -1, bd = -1;
+  for (int32_t u : U)
+    for (int32_t d : D) {
+      int64_t c = pair_cost(p, y[h], z[h], y[u], z[u], y[d], z[d]);
+      bool better = c < best_cost || (c == best_cost && (u < bu || (u == bu && d < bd)));
+      if (better) {
+        best_cost = c;
+        bu = u;
+        bd = d;
+      }
+    }
+  if (bu >= 0 && best_cost <= p->c_max) {
+    *up = bu;
+    *dn = bd;
+  } else {
+    *up = -1;
+    *dn = -1;
+  }
+}
+
+extern "C" void orc_neighbours_brute(const orc_params_t* p, int32_t n_sectors, int32_t n_rows, const int32_t* y,
+                                     const int32_t* z, const uint32_t* ro, int32_t* link_up, int32_t* link_dn) {
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int32_t s = 0; s < n_sectors; ++s) {
+    std::vector<int32_t> U, D;
+    for (int32_t r = 0; r < n_rows; ++r) {
+      const uint32_t* o = ro + (int64_t)s * n_rows + r;
+      for (uint32_t h = o[0]; h < o[1]; ++h) {
+        link_up[h] = -1;
+        link_dn[h] = -1;
+        if (r < 1 || r > n_rows - 2) continue;
+        U.clear();
+        D.clear();
+        for (uint32_t c = o[1]; c < o[2]; ++c)
+          if (in_window(p, y[h], z[h], y[c], z[c])) U.push_back((int32_t)c);
+        for (uint32_t c = o[-1]; c < o[0]; ++c)
+          if (in_window(p, y[h], z[h], y[c], z[c])) D.push_back((int32_t)c);
+        best_pair(p, y, z, (int32_t)h, U, D, &link_up[h], &link_dn[h]);
+      }
+    }
+  }
+}
+
+// z-sorted index per row: the oracle's own pruning structure (not the GPU's (y,z) bin grid).
+template <typename T>
+static void build_zorder(int64_t n_sr, const uint32_t* ro, const T* z, std::vector<int32_t>& idx) {
+  idx.resize(ro[n_sr]);
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t sr = 0; sr < n_sr; ++sr) {
+    for (uint32_t h = ro[sr]; h < ro[sr + 1]; ++h) idx[h] = (int32_t)h;
+    std::sort(idx.begin() + ro[sr], idx.begin() + ro[sr + 1],
+              [&](int32_t a, int32_t b) { return z[a] < z[b] || (z[a] == z[b] && a < b); });
+  }
+}
+
+extern "C" void orc_neighbours_pruned(const orc_params_t* p, int32_t n_sectors, int32_t n_rows, const int32_t* y,
+                                      const int32_t* z, const uint32_t* ro, int32_t* link_up, int32_t* link_dn) {
+  std::vector<int32_t> zo;
+  build_zorder<int32_t>((int64_t)n_sectors * n_rows, ro, z, zo);
+  auto collect = [&](uint32_t a, uint32_t b, int32_t yh, int32_t zh, std::vector<int32_t>& out) {
+    out.clear();
+    int64_t zlo = (int64_t)zh - p->w_z;
+    auto first = std::lower_bound(zo.begin() + a, zo.begin() + b, zlo,
+                                  [&](int32_t c, int64_t v) { return (int64_t)z[c] < v; });
+    for (auto it = first; it != zo.begin() + b; ++it) {
+      if ((int64_t)z[*it] > (int64_t)zh + p->w_z) break;
+      if (in_window(p, yh, zh, y[*it], z[*it])) out.push_back(*it);
+    }
+  };
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int32_t s = 0; s < n_sectors; ++s) {
+    std::vector<int32_t> U, D;
+    for (int32_t r = 0; r < n_rows; ++r) {
+      const uint32_t* o = ro + (int64_t)s * n_rows + r;
+      for (uint32_t h = o[0]; h < o[1]; ++h) {
+        link_up[h] = -1;
+        link_dn[h] = -1;
+        if (r < 1 || r > n_rows - 2) continue;
+        collect(o[1], o[2], y[h], z[h], U);
+        collect(o[-1], o[0], y[h], z[h], D);
+        best_pair(p, y, z, (int32_t)h, U, D, &link_up[h], &link_dn[h]);
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Stage 3.  SURVEY 8(c): one synchronous step from the raw tables (P11); chain start = no down link,
+// has up link (P12); length counts clusters; seed iff L >= l_min (P13); seeds ascend by start id (P14).
+// ------------------------------------------------------------------------------------------------
+extern "C" void orc_clean_links(int64_t n, const int32_t* up, const int32_t* dn, int32_t* up_c, int32_t* dn_c) {
+  for (int64_t h = 0; h < n; ++h) {
+    up_c[h] = (up[h] >= 0 && dn[up[h]] == (int32_t)h) ? up[h] : -1;
+    dn_c[h] = (dn[h] >= 0 && up[dn[h]] == (int32_t)h) ? dn[h] : -1;
+  }
+}
+
+extern "C" int64_t orc_find_seeds(const orc_params_t* p, int64_t n, const int32_t* up_c, const int32_t* dn_c,
+                                  int32_t* seed_start, int32_t* seed_len) {
+  int64_t ns = 0;
+  for (int64_t h = 0; h < n; ++h) {
+    if (dn_c[h] >= 0 || up_c[h] < 0) continue;
+    int32_t len = 1;
+    for (int32_t c = up_c[h]; c >= 0; c = up_c[c]) ++len;
+    if (len >= p->l_min) {
+      seed_start[ns] = (int32_t)h;
+      seed_len[ns] = len;
+      ++ns;
+    }
+  }
+  return ns;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Stage 4 building blocks.  SURVEY Appendix C (textbook circle/helix geometry in the sector frame).
+// State (y, z, s = sin phi, t = tan lambda = dz/ds_xy, q = q/pT) at x; k = cq * q is the signed curvature:
+// s(x + dx) = s + k dx exactly on a circle.
+// ------------------------------------------------------------------------------------------------
+struct Step {
+  double s1, c0, c1, tau, dy, dS, m, dSdk;
+};
+
+// Geometry of one step.  dy = dx (s+s1)/(c0+c1) [= (c0-c1)/k]; chord = sign(dx) sqrt(dx^2+dy^2);
+// u = k chord / 2; dS = chord asin(u)/u [= (asin s1 - asin s)/k].
+// d(dS)/dk = (dx/c1 - dS)/k, evaluated without the 0/0 at k -> 0: with phi_m = (phi0+phi1)/2 (tan phi_m = tau)
+// and delta = k dS / 2 = (phi1-phi0)/2,
+//   dx/c1 - dS = (2/(k c1)) [cos phi_m (sin d - d cos d) + d sin phi_m sin d]
+//   => d(dS)/dk = [ (dS^2/2) sin phi_m sinc(d) + (k dS^3/4) cos phi_m g(d) ] / c1,  g(d) = (sin d - d cos d)/d^3.
+static bool step_geometry(double k, double s, double dx, double smax, Step* g) {
+  double s1 = s + k * dx;
+  if (std::fabs(s) >= smax || std::fabs(s1) >= smax) return false;
+  double c0 = std::sqrt(1.0 - s * s), c1 = std::sqrt(1.0 - s1 * s1);
+  double tau = (s + s1) / (c0 + c1);
+  double dy = dx * tau;
+  double chord = std::copysign(std::sqrt(dx * dx + dy * dy), dx);
+  double u = 0.5 * k * chord;
+  double dS = (std::fabs(u) < 1e-6) ? chord * (1.0 + u * u / 6.0) : chord * std::asin(u) / u;
+  double d = 0.5 * k * dS;
+  double sinc = (std::fabs(d) < 1e-6) ? 1.0 - d * d / 6.0 : std::sin(d) / d;
+  double gg = (std::fabs(d) < 1e-2) ? 1.0 / 3.0 - d * d / 30.0 + d * d * d * d / 840.0
+                                   : (std::sin(d) - d * std::cos(d)) / (d * d * d);
+  double cm = 1.0 / std::sqrt(1.0 + tau * tau), sm = tau * cm;
+  g->s1 = s1;
+  g->c0 = c0;
+  g->c1 = c1;
+  g->tau = tau;
+  g->dy = dy;
+  g->dS = dS;
+  g->m = c0 + s * tau;  // = sin(phi1-phi0)/(k dx)
+  g->dSdk = (0.5 * dS * dS * sm * sinc + 0.25 * k * dS * dS * dS * cm * gg) / c1;
+  return true;
+}
+
+static void jacobian_from(const Step& g, double cq, double dx, double t, double F[25]) {
+  for (int i = 0; i < 25; ++i) F[i] = 0.0;
+  for (int i = 0; i < 5; ++i) F[i * 5 + i] = 1.0;
+  F[0 * 5 + 2] = dx * g.m / (g.c0 * g.c1);                      // dy1/ds
+  F[0 * 5 + 4] = cq * dx * dx * g.m / (g.c1 * (g.c0 + g.c1));   // dy1/dq
+  F[1 * 5 + 2] = t * g.dy / (g.c0 * g.c1);                      // dz1/ds
+  F[1 * 5 + 3] = g.dS;                                          // dz1/dt
+  F[1 * 5 + 4] = t * cq * g.dSdk;                               // dz1/dq
+  F[2 * 5 + 4] = cq * dx;                                       // ds1/dq
+}
+
+extern "C" void orc_jacobian(double cq, double dx, const double* st, double* F) {
+  Step g;
+  if (!step_geometry(cq * st[4], st[2], dx, 1.0, &g)) {
+    for (int i = 0; i < 25; ++i) F[i] = std::numeric_limits<double>::quiet_NaN();
+    return;
+  }
+  jacobian_from(g, cq, dx, st[3], F);
+}
+
+extern "C" int orc_transport(double cq, double smax, double dx, double* st, double* C) {
+  Step g;
+  if (!step_geometry(cq * st[4], st[2], dx, smax, &g)) return 0;
+  if (C) {
+    double F[25], FC[25];
+    jacobian_from(g, cq, dx, st[3], F);
+    for (int i = 0; i < 5; ++i)
+      for (int j = 0; j < 5; ++j) {
+        double a = 0.0;
+        for (int l = 0; l < 5; ++l) a += F[i * 5 + l] * C[l * 5 + j];
+        FC[i * 5 + j] = a;
+      }
+    for (int i = 0; i < 5; ++i)
+      for (int j = 0; j < 5; ++j) {
+        double a = 0.0;
+        for (int l = 0; l < 5; ++l) a += FC[i * 5 + l] * F[j * 5 + l];
+        C[i * 5 + j] = a;
+      }
+  }
+  st[0] += g.dy;
+  st[1] += st[3] * g.dS;
+  st[2] = g.s1;
+  return 1;
+}
+
+// Standard Kalman update with H = [I2 | 0], V = diag(sy2, sz2) (Appendix C):
+// S = C[0:2,0:2] + V; K = C[:,0:2] S^-1; p += K r; C -= K C[0:2,:]; symmetrise; chi2 = r^T S^-1 r.
+extern "C" double orc_update(double* st, double* C, double ym, double zm, double sy2, double sz2) {
+  double S00 = C[0] + sy2, S01 = C[1], S10 = C[5], S11 = C[6] + sz2;
+  double det = S00 * S11 - S01 * S10;
+  double I00 = S11 / det, I01 = -S01 / det, I10 = -S10 / det, I11 = S00 / det;
+  double r0 = ym - st[0], r1 = zm - st[1];
+  double K[5][2];
+  for (int i = 0; i < 5; ++i) {
+    K[i][0] = C[i * 5 + 0] * I00 + C[i * 5 + 1] * I10;
+    K[i][1] = C[i * 5 + 0] * I01 + C[i * 5 + 1] * I11;
+  }
+  double HC[2][5];
+  for (int j = 0; j < 5; ++j) {
+    HC[0][j] = C[0 * 5 + j];
+    HC[1][j] = C[1 * 5 + j];
+  }
+  for (int i = 0; i < 5; ++i) st[i] += K[i][0] * r0 + K[i][1] * r1;
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j < 5; ++j) C[i * 5 + j] -= K[i][0] * HC[0][j] + K[i][1] * HC[1][j];
+  for (int i = 0; i < 5; ++i)
+    for (int j = i + 1; j < 5; ++j) {
+      double a = 0.5 * (C[i * 5 + j] + C[j * 5 + i]);
+      C[i * 5 + j] = a;
+      C[j * 5 + i] = a;
+    }
+  return r0 * (I00 * r0 + I01 * r1) + r1 * (I10 * r0 + I11 * r1);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Stage 4: follower.  SURVEY 8(c) "Stage 4" (P15..P24).
+// ------------------------------------------------------------------------------------------------
+struct FollowCtx {
+  const orc_params_t* p;
+  double cq;  // cq_per_tesla * Bz
+  int32_t n_rows;
+  int64_t n_sr;  // n_sectors * n_rows
+  const double* row_x;
+  const double* y;
+  const double* z;
+  const uint32_t* ro;
+  const int32_t* zorder;  // NULL in search_mode 0
+  double sy2, sz2;
+};
+
+// P17/P21: among all clusters of the sector-row inside |dy| <= gate_y, |dz| <= gate_z, minimise (d, id),
+// d = dy^2/(Cyy + sy2) + dz^2/(Czz + sz2); accept iff d < gate_d.
+static int32_t search_row(const FollowCtx& c, int64_t sr, const double* st, const double* C) {
+  const orc_params_t* p = c.p;
+  double wy = 1.0 / (C[0] + c.sy2), wz = 1.0 / (C[6] + c.sz2);
+  double bestd = std::numeric_limits<double>::infinity();
+  int32_t best = -1;
+  auto consider = [&](int32_t id) {
+    double dy = c.y[id] - st[0], dz = c.z[id] - st[1];
+    if (std::fabs(dy) > p->gate_y_cm || std::fabs(dz) > p->gate_z_cm) return;
+    double d = dy * dy * wy + dz * dz * wz;
+    if (d < bestd || (d == bestd && id < best)) {
+      bestd = d;
+      best = id;
+    }
+  };
+  uint32_t a = c.ro[sr], b = c.ro[sr + 1];
+  if (!c.zorder) {
+    for (uint32_t h = a; h < b; ++h) consider((int32_t)h);
+  } else {
+    double zlo = st[1] - p->gate_z_cm - 1e-9, zhi = st[1] + p->gate_z_cm + 1e-9;  // pruning only, superset
+    const int32_t* first = std::lower_bound(c.zorder + a, c.zorder + b, zlo,
+                                            [&](int32_t id, double v) { return c.z[id] < v; });
+    for (const int32_t* it = first; it != c.zorder + b && c.z[*it] <= zhi; ++it) consider(*it);
+  }
+  return (best >= 0 && bestd < p->gate_d) ? best : -1;
+}
+
+static void reset_cov(const orc_params_t* p, double* C) {
+  for (int i = 0; i < 25; ++i) C[i] = 0.0;
+  for (int i = 0; i < 5; ++i) C[i * 5 + i] = p->c_reset[i];
+}
+
+static void follow_one(const FollowCtx& c, int32_t h0, int32_t L, const int32_t* up_c, double* par, double* cov,
+                       double* chi2_out, int32_t* n_hits_out, int32_t* hits) {
+  const orc_params_t* p = c.p;
+  const int32_t nr = c.n_rows;
+  // locate (sector,row) of h0 by binary search over the CSR offsets: ro[lo] <= h0 < ro[lo+1]
+  int64_t lo = 0, hi = c.n_sr;
+  while (hi - lo > 1) {
+    int64_t mid = (lo + hi) / 2;
+    if (c.ro[mid] <= (uint32_t)h0) lo = mid; else hi = mid;
+  }
+  const int64_t sec_base = (lo / nr) * nr;
+  const int32_t r0 = (int32_t)(lo % nr);
+  for (int32_t r = 0; r < nr; ++r) hits[r] = -1;
+
+  // P19 init from the first two chain hits
+  int32_t c0 = h0, c1 = up_c[h0];
+  double x = c.row_x[r0];
+  double dxr = c.row_x[r0 + 1] - c.row_x[r0];
+  double dy = c.y[c1] - c.y[c0], dz = c.z[c1] - c.z[c0];
+  double chord = std::sqrt(dxr * dxr + dy * dy);
+  double st[5] = {c.y[c0], c.z[c0], dy / chord, dz / chord, 0.0};
+  double C[25];
+  reset_cov(p, C);
+  orc_update(st, C, c.y[c0], c.z[c0], c.sy2, c.sz2);
+  hits[r0] = c0;
+  int32_t row = r0;
+  bool fail_up = false;
+
+  // Phase A: fit up the chain, no gate
+  int32_t h = c0;
+  for (int32_t i = 1; i < L; ++i) {
+    h = up_c[h];
+    if (!orc_transport(c.cq, p->sinphi_max, c.row_x[r0 + i] - x, st, C)) {
+      fail_up = true;
+      break;
+    }
+    row = r0 + i;
+    x = c.row_x[row];
+    orc_update(st, C, c.y[h], c.z[h], c.sy2, c.sz2);
+    hits[row] = h;
+  }
+  // Phase B: extend up with gated nearest-hit search (P20: stop after max_miss consecutive empty rows)
+  if (!fail_up) {
+    int32_t miss = 0;
+    while (row + 1 <= nr - 1 && miss < p->max_miss) {
+      if (!orc_transport(c.cq, p->sinphi_max, c.row_x[row + 1] - x, st, C)) break;
+      ++row;
+      x = c.row_x[row];
+      int32_t f = search_row(c, sec_base + row, st, C);
+      if (f >= 0) {
+        orc_update(st, C, c.y[f], c.z[f], c.sy2, c.sz2);
+        hits[row] = f;
+        miss = 0;
+      } else {
+        ++miss;
+      }
+    }
+  }
+  // Phase C: keep the state, reset the covariance (P22), refit downwards over the recorded hits;
+  // Phase D: below the seed's first row, search as in B.
+  reset_cov(p, C);
+  double chi2 = 0.0;
+  if (hits[row] >= 0) chi2 += orc_update(st, C, c.y[hits[row]], c.z[hits[row]], c.sy2, c.sz2);
+  bool fail_dn = false;
+  int32_t miss = 0;
+  while (row > 0) {
+    if (row - 1 < r0 && miss >= p->max_miss) break;
+    if (!orc_transport(c.cq, p->sinphi_max, c.row_x[row - 1] - x, st, C)) {
+      fail_dn = true;
+      break;
+    }
+    --row;
+    x = c.row_x[row];
+    if (row >= r0) {
+      if (hits[row] >= 0) chi2 += orc_update(st, C, c.y[hits[row]], c.z[hits[row]], c.sy2, c.sz2);
+    } else {
+      int32_t f = search_row(c, sec_base + row, st, C);
+      if (f >= 0) {
+        chi2 += orc_update(st, C, c.y[f], c.z[f], c.sy2, c.sz2);
+        hits[row] = f;
+        miss = 0;
+      } else {
+        ++miss;
+      }
+    }
+  }
+  // P23: transport (no update) back to the lowest-row hit
+  int32_t lowest = 0, nh = 0;
+  for (int32_t r = nr - 1; r >= 0; --r)
+    if (hits[r] >= 0) {
+      lowest = r;
+      ++nh;
+    }
+  if (!fail_dn && lowest != row) {
+    if (orc_transport(c.cq, p->sinphi_max, c.row_x[lowest] - x, st, C)) x = c.row_x[lowest];
+  }
+  par[0] = x;
+  for (int i = 0; i < 5; ++i) par[1 + i] = st[i];
+  int q = 0;
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j <= i; ++j) cov[q++] = C[i * 5 + j];
+  *chi2_out = chi2;
+  *n_hits_out = nh;
+}
+
+extern "C" void orc_follow(const orc_params_t* p, double bz, int32_t n_sectors, int32_t n_rows, const double* row_x,
+                           const double* y_cm, const double* z_cm, const uint32_t* ro, const int32_t* up_c,
+                           int64_t n_seeds, const int32_t* seed_start, const int32_t* seed_len, int search_mode,
+                           double* par, double* cov, double* chi2, int32_t* n_hits, int32_t* hits) {
+  std::vector<int32_t> zo;
+  if (search_mode == 1) build_zorder<double>((int64_t)n_sectors * n_rows, ro, z_cm, zo);
+  FollowCtx c;
+  c.p = p;
+  c.cq = p->cq_per_tesla * bz;
+  c.n_rows = n_rows;
+  c.n_sr = (int64_t)n_sectors * n_rows;
+  c.row_x = row_x;
+  c.y = y_cm;
+  c.z = z_cm;
+  c.ro = ro;
+  c.zorder = search_mode == 1 ? zo.data() : nullptr;
+  c.sy2 = p->sigma_y * p->sigma_y;
+  c.sz2 = p->sigma_z * p->sigma_z;
+#pragma omp parallel for schedule(dynamic, 16)
+  for (int64_t i = 0; i < n_seeds; ++i) {
+    follow_one(c, seed_start[i], seed_len[i], up_c, par + i * 6, cov + i * 15, chi2 + i, n_hits + i,
+               hits + i * (int64_t)n_rows);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Stage 5.  SURVEY 8(c): surviving tracklets have n_hits >= n_min_tracklet (P24); owner(h) = surviving
+// tracklet containing h with the largest n_hits, ties -> smallest seed start id (P26); output iff owned
+// >= n_min_owned (P27); hit list = owned hits ascending row; output order = ascending seed start id (P29).
+// ------------------------------------------------------------------------------------------------
+extern "C" int64_t orc_select(const orc_params_t* p, int64_t n, int32_t n_rows, int64_t n_seeds,
+                              const int32_t* seed_start, const int32_t* n_hits, const int32_t* hits, int32_t* owner,
+                              int32_t* trk_seed, int32_t* trk_n_owned, int32_t* trk_hit_offset, int32_t* hit_ids,
+                              int64_t* n_out_hits) {
+  for (int64_t h = 0; h < n; ++h) owner[h] = -1;
+  for (int64_t i = 0; i < n_seeds; ++i) {
+    if (n_hits[i] < p->n_min_tracklet) continue;
+    for (int32_t r = 0; r < n_rows; ++r) {
+      int32_t h = hits[i * n_rows + r];
+      if (h < 0) continue;
+      int32_t o = owner[h];
+      // seeds ascend by start id, so "smaller start id" == "smaller rank"
+      if (o < 0 || n_hits[i] > n_hits[o] || (n_hits[i] == n_hits[o] && seed_start[i] < seed_start[o]))
+        owner[h] = (int32_t)i;
+    }
+  }
+  int64_t nt = 0, nh = 0;
+  for (int64_t i = 0; i < n_seeds; ++i) {
+    if (n_hits[i] < p->n_min_tracklet) continue;
+    int32_t owned = 0;
+    for (int32_t r = 0; r < n_rows; ++r) {
+      int32_t h = hits[i * n_rows + r];
+      if (h >= 0 && owner[h] == (int32_t)i) ++owned;
+    }
+    if (owned < p->n_min_owned) continue;
+    trk_seed[nt] = (int32_t)i;
+    trk_n_owned[nt] = owned;
+    trk_hit_offset[nt] = (int32_t)nh;
+    for (int32_t r = 0; r < n_rows; ++r) {
+      int32_t h = hits[i * n_rows + r];
+      if (h >= 0 && owner[h] == (int32_t)i) hit_ids[nh++] = h;
+    }
+    ++nt;
+  }
+  *n_out_hits = nh;
+  return nt;
+}

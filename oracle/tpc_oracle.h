@@ -1,0 +1,89 @@
+/* tpc_oracle.h -- CPU oracle for TPC sector track finding.  TEST INFRASTRUCTURE, NOT PRODUCT.
+ *
+ * Plain, slow, fp64, obviously-correct restatement of the five-stage path that BASELINE.json's
+ * north_star names (the paper, Table 1 / PAPER.md:40, only says "TPC tracking"; it gives no
+ * algorithm).  Every stage follows SURVEY.md section 8(c) step by step, in that order and notation;
+ * readings P1..P40 are listed in DESIGN.md.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may load this library.  It shares no code, header, table or
+ * constant generator with paper_2502_09138_b200/ (the CUDA path); neither includes the other.
+ *
+ * All pointers are host pointers.  Cluster ids are indices into the event arrays; -1 = none.
+ * Clusters of one (sector,row) are contiguous: row_offsets[s*n_rows + r] .. row_offsets[s*n_rows+r+1].
+ */
+#ifndef TPC_ORACLE_H
+#define TPC_ORACLE_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct {
+  /* stage 2 (integer) -- SURVEY 8(c) P7, P8, P10 */
+  int32_t w_y, w_z;            /* search window half-widths in fixed-point units, inclusive: 1280, 1600 */
+  int32_t cost_wy, cost_wz;    /* cost = cost_wy*ddy^2 + cost_wz*ddz^2 : 9, 4 */
+  int32_t c_max;               /* accept iff cost <= c_max : 3538944 */
+  /* stage 3 -- P13 */
+  int32_t l_min;               /* seed iff chain length >= l_min : 5 */
+  /* stage 4 -- P15..P24 */
+  double units_per_cm;         /* 640 */
+  double sigma_y, sigma_z;     /* 0.1, 0.15 cm */
+  double sinphi_max;           /* 0.95 */
+  int32_t max_miss;            /* 5 consecutive rows */
+  int32_t n_min_tracklet;      /* 10 */
+  double gate_d;               /* accept iff d < 15 */
+  double gate_y_cm, gate_z_cm; /* |dy| <= 2.0, |dz| <= 2.5 */
+  double c_reset[5];           /* variances 0.25, 0.25, 0.05, 0.05, 25 */
+  double cq_per_tesla;         /* k = cq_per_tesla * Bz * q/pT : -0.00299792458 (P4) */
+  /* stage 5 -- P27 */
+  int32_t n_min_owned;         /* 10 */
+} orc_params_t;
+
+void orc_default_params(orc_params_t* p);
+
+/* ---- stage 1-2: neighbour finding (integer, bit-exact) -- SURVEY 8(c) "Stage 1-2" ---- */
+/* definition: all pairs over the two adjacent rows */
+void orc_neighbours_brute(const orc_params_t* p, int32_t n_sectors, int32_t n_rows, const int32_t* y,
+                          const int32_t* z, const uint32_t* row_offsets, int32_t* link_up, int32_t* link_dn);
+/* same result through the oracle's own pruning structure (per-row z-sorted index + binary search) */
+void orc_neighbours_pruned(const orc_params_t* p, int32_t n_sectors, int32_t n_rows, const int32_t* y,
+                           const int32_t* z, const uint32_t* row_offsets, int32_t* link_up, int32_t* link_dn);
+
+/* ---- stage 3: cleaner, chains, seeds (integer, bit-exact) -- SURVEY 8(c) "Stage 3" ---- */
+void orc_clean_links(int64_t n, const int32_t* up, const int32_t* dn, int32_t* up_c, int32_t* dn_c);
+/* returns number of seeds; seeds ascend by start id; seed_start/seed_len need capacity n / l_min + 1 */
+int64_t orc_find_seeds(const orc_params_t* p, int64_t n, const int32_t* up_c, const int32_t* dn_c,
+                       int32_t* seed_start, int32_t* seed_len);
+
+/* ---- stage 4 building blocks (exported for the pins) -- SURVEY Appendix C ---- */
+/* state = (y, z, sin phi, tan lambda, q/pT); cov = full 5x5 row-major (may be NULL); k = cq*q/pT.
+ * Returns 1 on success, 0 on transport failure (|sin phi| >= sinphi_max before or after). */
+int orc_transport(double cq, double sinphi_max, double dx, double* state, double* cov);
+void orc_jacobian(double cq, double dx, const double* state, double* F /* 5x5 row-major */);
+/* joint (y,z) Kalman update, V = diag(sy2, sz2); returns the chi2 increment */
+double orc_update(double* state, double* cov, double ym, double zm, double sy2, double sz2);
+
+/* ---- stage 4: follower ---- */
+/* Inputs: y_cm/z_cm are cluster coordinates in cm as doubles (normally int/units_per_cm; tests may pass
+ * exact doubles).  search_mode 0 = full-row scan (the definition, P17), 1 = z-sorted pruning (same result).
+ * Outputs per seed i: par[i*6 + 0..5] = (x_ref, y, z, sin phi, tan lambda, q/pT); cov[i*15 ..] packed lower
+ * triangle (00,10,11,20,21,22,...); chi2[i]; n_hits[i]; hits[i*n_rows + r] = cluster id in row r or -1. */
+void orc_follow(const orc_params_t* p, double bz, int32_t n_sectors, int32_t n_rows, const double* row_x,
+                const double* y_cm, const double* z_cm, const uint32_t* row_offsets, const int32_t* up_c,
+                int64_t n_seeds, const int32_t* seed_start, const int32_t* seed_len, int search_mode,
+                double* par, double* cov, double* chi2, int32_t* n_hits, int32_t* hits);
+
+/* ---- stage 5: ownership, selection, output -- SURVEY 8(c) "Stage 5" ---- */
+/* owner[h] = seed rank owning cluster h or -1.  Outputs tracks in ascending seed start id:
+ * trk_seed[t] = seed rank; trk_n_owned[t]; trk_hit_offset[t]; hit_ids = owned hits ascending row.
+ * Returns number of output tracks; *n_out_hits = total hits written. */
+int64_t orc_select(const orc_params_t* p, int64_t n, int32_t n_rows, int64_t n_seeds, const int32_t* seed_start,
+                   const int32_t* n_hits, const int32_t* hits, int32_t* owner, int32_t* trk_seed,
+                   int32_t* trk_n_owned, int32_t* trk_hit_offset, int32_t* hit_ids, int64_t* n_out_hits);
+
+int orc_num_threads(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
