@@ -1,0 +1,162 @@
+/* tpc_track.h -- C ABI of libtpctrack.so: TPC sector track finding on one B200 (sm_100a).
+ *
+ * What it computes: the "TPC tracking" part of the line "TPC Processing (Tracking, Clustering, Compression)
+ * 99.37 %" of the paper's Table 1 ("fully dominated by the TPC tracking which can run on GPUs",
+ * PAPER.md:40), in the five stages BASELINE.json's north_star names:
+ *   a1 per-pad-row (y,z) grid binning, a2 neighbour finding (best up/down pair in the adjacent rows),
+ *   a3 cellular-automaton link cleaner + chain/seed extraction, a4 Kalman-filter tracklet following (helix,
+ *   constant Bz), a5 hit-ownership selection + output compaction.
+ * The paper gives no algorithm; every stage is defined in SURVEY.md section 8(c) (readings P1..P40, restated in
+ * DESIGN.md).  The three entry points are the ones north_star lists; the handle argument of tpc_track and the
+ * host-buffer / debug entry points are additions.
+ *
+ * Conventions
+ *  - Every function returns an int status: TPC_OK (0) or a negative TPC_ERR_* code.  Nothing throws or aborts.
+ *  - Pointers are tagged [host] or [device] below.  The caller owns every buffer it passes; the handle owns
+ *    all scratch memory (grown on demand, released by tpc_tracker_destroy).
+ *  - tpc_track is asynchronous on `stream` (a cudaStream_t passed as void*; NULL = legacy default stream);
+ *    results are valid after the caller synchronises that stream.  One handle serves one stream at a time.
+ *  - Cluster ids are indices into the input arrays.  Clusters of one (sector,row) are contiguous:
+ *    row_offsets[s*n_rows + r] .. row_offsets[s*n_rows + r + 1]; the order inside a row is arbitrary.
+ *  - Coordinates are int32 fixed point, units_per_cm units per cm (640 = 1/64 mm, BASELINE.json configs[0]).
+ *    Sector-local frame: x along the sector's central radius (pad row r is the plane x = row_x[r]),
+ *    y across the sector, z along the beam.  Track state at x: (y, z, sin phi, tan lambda, q/pT [1/GeV]).
+ */
+#ifndef TPC_TRACK_H
+#define TPC_TRACK_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TPC_OK 0
+#define TPC_ERR_ARG (-1)       /* NULL pointer, negative size, parameter out of range */
+#define TPC_ERR_GEOMETRY (-2)  /* n_rows < 3, rows not equidistant (P6), non-positive extents */
+#define TPC_ERR_CUDA (-3)      /* a CUDA runtime call failed (tpc_last_cuda_error() tells which) */
+#define TPC_ERR_NOMEM (-4)     /* scratch allocation failed */
+#define TPC_ERR_CAPACITY (-5)  /* n too large for the packed ownership word (n/l_min >= 2^24) */
+
+/* device-side flags OR-ed into counts[2] */
+#define TPC_FLAG_TRACK_OVERFLOW 1u /* more output tracks than track_capacity: tracks beyond it not written */
+#define TPC_FLAG_HIT_OVERFLOW 2u   /* more output hits than hit_capacity: those tracks' hit lists not written */
+
+/* Free constants of the method.  tpc_default_params fills the defaults. */
+typedef struct {
+  int32_t w_y, w_z;          /* a2 window half-widths, fixed-point units, inclusive (P7): 1280, 1600 */
+  int32_t cost_wy, cost_wz;  /* a2 cost = cost_wy*(y_u+y_d-2y_h)^2 + cost_wz*(z_u+z_d-2z_h)^2 (P8): 9, 4 */
+  int32_t c_max;             /* a2 accept iff cost <= c_max (P10): 3538944 */
+  int32_t l_min;             /* a3 seed iff chain length >= l_min clusters (P13): 5 */
+  int32_t max_miss;          /* a4 stop after this many consecutive rows without a hit (P20): 5 */
+  int32_t n_min_tracklet;    /* a4/a5 tracklets with fewer hits are discarded (P24): 10 */
+  int32_t n_min_owned;       /* a5 output iff owned hits >= this (P27): 10 */
+  int32_t reserved;          /* must be 0 */
+  double sigma_y, sigma_z;   /* a4 hit errors in cm (P15): 0.1, 0.15 */
+  double sinphi_max;         /* a4 transport fails iff |sin phi| >= this before or after a step (P18): 0.95 */
+  double gate_d;             /* a4 accept a searched hit iff d < gate_d (P21): 15 */
+  double gate_y_cm, gate_z_cm; /* a4 search restricted to |dy| <= 2.0, |dz| <= 2.5 cm (P21) */
+  double c_reset[5];         /* a4 covariance reset, variances (P22): 0.25, 0.25, 0.05, 0.05, 25 */
+  double cq_per_tesla;       /* a4 curvature k = cq_per_tesla * Bz * q/pT, 1/cm (P4): -0.00299792458 */
+} tpc_params_t;
+
+typedef struct {
+  int32_t n_sectors;       /* independent sectors in one call (36; 1 for configs[0]; B*36 for a batch of B events) */
+  int32_t n_rows;          /* pad rows per sector (152), >= 3 */
+  const double* row_x;     /* [host] n_rows local x of the pad rows in cm, ascending, equidistant (P6) */
+  double units_per_cm;     /* fixed-point scale (640) */
+  double y_half_tan;       /* |y| <= row_x[r]*y_half_tan (tan 10 deg); used for grid sizing only */
+  double y_half_cm;        /* if > 0: |y| extent in cm for every row instead (open sector, configs[0]); grid sizing only */
+  double z_extent_cm;      /* z-length covered by one sector's clusters incl. drift offsets; grid sizing only */
+  const tpc_params_t* params; /* [host] NULL = defaults */
+} tpc_geometry_t;
+/* "grid sizing only": clusters outside these extents are still handled exactly (edge bins absorb them). */
+
+typedef struct {
+  double bz_tesla; /* constant field along z (0.5) */
+} tpc_field_t;
+
+typedef struct {
+  const int32_t* y;            /* [device] n fixed-point y */
+  const int32_t* z;            /* [device] n fixed-point z */
+  const uint32_t* row_offsets; /* [device] n_sectors*n_rows + 1 CSR offsets; row_offsets[last] == n */
+} tpc_clusters_t;
+
+/* One output track (112 bytes).  Parameters are the a4 fit over all the tracklet's hits at x (P23, P28). */
+typedef struct {
+  float x, y, z, sinphi, tanl, qpt;
+  float cov[15];       /* packed lower triangle 00,10,11,20,21,22,30,... in (y,z,sinphi,tanl,qpt) order */
+  float chi2;          /* accumulated over the downward pass (P22) */
+  int32_t sector;
+  int32_t first_row, last_row; /* of the owned hits */
+  int32_t n_hits;      /* owned hits = length of this track's hit list */
+  int32_t hit_offset;  /* start of the hit list in hit_ids */
+  int32_t seed_cluster; /* start cluster id of the seed; tracks ascend by it (P29) */
+} tpc_track_rec_t;
+
+typedef struct {
+  tpc_track_rec_t* tracks; /* [device] track_capacity records */
+  int32_t track_capacity;
+  int32_t hit_capacity;
+  int32_t* hit_ids;        /* [device] hit_capacity cluster ids; per track ascending row */
+  int32_t* counts;         /* [device] 4 x int32: [0] tracks found, [1] hits found (both may exceed the
+                              capacities: then the matching TPC_FLAG_* is set and the excess is not written),
+                              [2] flags, [3] number of seeds (tracklets followed) */
+} tpc_tracks_out_t;
+
+typedef struct tpc_tracker tpc_tracker_t;
+
+void tpc_default_params(tpc_params_t* p);
+
+/* Copies geometry, field and parameters into a new handle for the current CUDA device.  No cluster-sized
+ * allocation happens here.  Errors: TPC_ERR_ARG, TPC_ERR_GEOMETRY, TPC_ERR_CUDA, TPC_ERR_NOMEM. */
+int tpc_tracker_create(const tpc_geometry_t* geometry, const tpc_field_t* field, tpc_tracker_t** out);
+
+/* Runs a1..a5 on n clusters, enqueued on `stream`; no host synchronisation unless scratch must grow.
+ * clusters and out are [host] structs holding [device] pointers.  n may be 0.
+ * Errors: TPC_ERR_ARG, TPC_ERR_CAPACITY, TPC_ERR_NOMEM, TPC_ERR_CUDA. */
+int tpc_track(tpc_tracker_t* t, const tpc_clusters_t* clusters, int64_t n, void* stream, tpc_tracks_out_t* out);
+
+/* Same computation with HOST buffers: copies y, z, row_offsets to device staging owned by the handle, runs
+ * tpc_track, copies counts, tracks and hit_ids back into the [host] buffers of `out_host`, and synchronises
+ * `stream` before returning.  Pinned host memory makes the copies asynchronous but is not required. */
+int tpc_track_host(tpc_tracker_t* t, const tpc_clusters_t* clusters_host, int64_t n, void* stream,
+                   tpc_tracks_out_t* out_host);
+
+int tpc_tracker_destroy(tpc_tracker_t* t);
+
+const char* tpc_status_string(int status);
+const char* tpc_last_cuda_error(const tpc_tracker_t* t);
+
+/* Scratch bytes currently owned by the handle. */
+int64_t tpc_scratch_bytes(const tpc_tracker_t* t);
+
+/* Number of kernel launches one tpc_track call enqueues (for launch accounting in the bench). */
+int tpc_launches_per_call(const tpc_tracker_t* t);
+
+/* Per-stage device times in ms of the most recent tpc_track call made while stage timing was enabled
+ * (tpc_set_stage_timing(t, 1) inserts CUDA events between the stages).  ms[0..4] = a1..a5.  Synchronises. */
+int tpc_set_stage_timing(tpc_tracker_t* t, int enable);
+int tpc_get_stage_ms(tpc_tracker_t* t, float ms[5]);
+
+/* ---- test-only exports: intermediate results of the most recent tpc_track call on this handle ----
+ * All outputs are [device] buffers in id space (-1 = none), written asynchronously on `stream`. */
+/* which = 0: raw a2 link tables; 1: cleaned (a3).  up, dn: n int32 each. */
+int tpc_debug_copy_links(tpc_tracker_t* t, int which, int32_t* up, int32_t* dn, void* stream);
+/* start, len: capacity n/l_min + 1 each (seeds ascend by start id, P14). */
+int tpc_debug_copy_seeds(tpc_tracker_t* t, int32_t* start, int32_t* len, void* stream);
+/* Tracklets of all seeds, seed-major: par[s*6 + 0..5] = (x_ref, y, z, sin phi, tan lambda, q/pT),
+ * cov[s*15 + ..], chi2[s], n_hits[s], hits[s*n_rows + r] = cluster id in row r or -1.
+ * Any pointer may be NULL to skip it.  Sizes from counts[3]. */
+int tpc_debug_copy_tracklets(tpc_tracker_t* t, float* par, float* cov, float* chi2, int32_t* n_hits, int32_t* hits,
+                             void* stream);
+/* owner[h] = rank of the owning seed or -1; n int32. */
+int tpc_debug_copy_owner(tpc_tracker_t* t, int32_t* owner, void* stream);
+/* Sorted-grid view of a1: ids_sorted[n] (cluster id at each sorted position), bin_start [n_sectors*n_rows *
+ * bins_per_row_stride] ; returns the stride and per-row bin shape through the scalars (host). */
+int tpc_debug_grid_info(const tpc_tracker_t* t, int32_t* bins_stride, int32_t* nz, int32_t* shift_y, int32_t* shift_z);
+int tpc_debug_copy_grid(tpc_tracker_t* t, int32_t* ids_sorted, uint32_t* bin_start, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,108 @@
+// a2_neighbours.cu -- stage a2: neighbour finding (SURVEY 8(c) "Stage 1-2", P5, P7-P10; north_star
+// "each cluster links to the best pair of clusters in the adjacent rows").  Integer only -> bit-exact.
+//
+// For cluster h in row r (1 <= r <= n_rows-2): U = clusters of row r+1 with |dy| <= w_y and |dz| <= w_z,
+// D likewise in row r-1; pick the pair minimising (cost, id_u, id_d), cost = cost_wy*(yu+yd-2yh)^2 +
+// cost_wz*(zu+zd-2zh)^2; accept iff cost <= c_max.  Links are written in id space.
+// The a1 grid prunes the candidates: bins are at least 2*w wide, so a window touches at most 2 x 2 bins, and
+// with y-fastest bin order each z-bin contributes one contiguous range of sorted clusters.
+#include "tpc_internal.cuh"
+
+namespace {
+
+constexpr int A2_THREADS = 128;
+
+struct Ranges {
+  uint32_t a0, b0, a1, b1;   // up to two contiguous sorted ranges (second empty if the window is in one z-bin)
+};
+
+__device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
+
+__device__ __forceinline__ Ranges window_ranges(const DevGeom& g, int yh, int zh, int2 org, int ny,
+                                                const uint32_t* __restrict__ bs) {
+  const int iy_lo = clampi((yh - g.w_y - org.x) >> g.shift_y, 0, ny - 1);
+  const int iy_hi = clampi((yh + g.w_y - org.x) >> g.shift_y, 0, ny - 1);
+  const int iz_lo = clampi((zh - g.w_z - org.y) >> g.shift_z, 0, g.nz - 1);
+  const int iz_hi = clampi((zh + g.w_z - org.y) >> g.shift_z, 0, g.nz - 1);
+  Ranges q;
+  q.a0 = bs[iz_lo * ny + iy_lo];
+  q.b0 = bs[iz_lo * ny + iy_hi + 1];
+  if (iz_hi != iz_lo) {   // bins are >= 2*w_z wide, so iz_hi <= iz_lo + 1
+    q.a1 = bs[iz_hi * ny + iy_lo];
+    q.b1 = bs[iz_hi * ny + iy_hi + 1];
+  } else {
+    q.a1 = q.b1 = 0;
+  }
+  return q;
+}
+
+__global__ void __launch_bounds__(A2_THREADS)
+a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int32_t* __restrict__ ys,
+                     const int32_t* __restrict__ zs, const int32_t* __restrict__ ids,
+                     const int2* __restrict__ row_org, const uint32_t* __restrict__ bin_start,
+                     int32_t* __restrict__ link_up, int32_t* __restrict__ link_dn, uint32_t* __restrict__ owner) {
+  const int sr = blockIdx.x;
+  const int r = sr % g.n_rows;
+  const uint32_t a = ro[sr], b = ro[sr + 1];
+  const bool inner = r >= 1 && r <= g.n_rows - 2;   // P5
+  int2 org_u, org_d;
+  int ny_u = 1, ny_d = 1;
+  const uint32_t *bs_u = nullptr, *bs_d = nullptr;
+  if (inner) {
+    org_u = row_org[sr + 1];
+    org_d = row_org[sr - 1];
+    ny_u = g.ny_row[r + 1];
+    ny_d = g.ny_row[r - 1];
+    bs_u = bin_start + (size_t)(sr + 1) * g.nb_stride;
+    bs_d = bin_start + (size_t)(sr - 1) * g.nb_stride;
+  }
+  for (uint32_t j = a + threadIdx.x; j < b; j += A2_THREADS) {
+    const int yh = ys[j], zh = zs[j], hid = ids[j];
+    int best_u = -1, best_d = -1;
+    if (inner) {
+      const Ranges qu = window_ranges(g, yh, zh, org_u, ny_u, bs_u);
+      const Ranges qd = window_ranges(g, yh, zh, org_d, ny_d, bs_d);
+      int best_cost = INT32_MAX;
+#pragma unroll 1
+      for (int pu = 0; pu < 2; ++pu) {
+        const uint32_t ua = pu ? qu.a1 : qu.a0, ub = pu ? qu.b1 : qu.b0;
+        for (uint32_t u = ua; u < ub; ++u) {
+          const int dyu = ys[u] - yh, dzu = zs[u] - zh;
+          if (abs(dyu) > g.w_y || abs(dzu) > g.w_z) continue;
+          const int idu = ids[u];
+#pragma unroll 1
+          for (int pd = 0; pd < 2; ++pd) {
+            const uint32_t da = pd ? qd.a1 : qd.a0, db = pd ? qd.b1 : qd.b0;
+            for (uint32_t d = da; d < db; ++d) {
+              const int dyd = ys[d] - yh, dzd = zs[d] - zh;
+              if (abs(dyd) > g.w_y || abs(dzd) > g.w_z) continue;
+              const int ddy = dyu + dyd, ddz = dzu + dzd;
+              const int cost = g.cost_wy * ddy * ddy + g.cost_wz * ddz * ddz;
+              if (cost > best_cost) continue;
+              const int idd = ids[d];
+              if (cost < best_cost || idu < best_u || (idu == best_u && idd < best_d)) {   // P9
+                best_cost = cost;
+                best_u = idu;
+                best_d = idd;
+              }
+            }
+          }
+        }
+      }
+      if (best_u < 0 || best_cost > g.c_max) best_u = best_d = -1;   // P10
+    }
+    link_up[hid] = best_u;
+    link_dn[hid] = best_d;
+    owner[hid] = 0u;   // a5 ownership words start empty
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64_t n, cudaStream_t st) {
+  const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
+  if (R == 0) return cudaSuccess;
+  a2_neighbours_kernel<<<(unsigned)R, A2_THREADS, 0, st>>>(t->g, ro, t->s.ys, t->s.zs, t->s.ids, t->s.row_org,
+                                                          t->s.bin_start, t->s.link_up, t->s.link_dn, t->s.owner);
+  return cudaGetLastError();
+}

@@ -1,0 +1,340 @@
+// a4_follow.cu -- stage a4: Kalman-filter tracklet following with a helix model in constant Bz
+// (SURVEY 8(c) "Stage 4", P15-P24; Appendix C transport/Jacobian/update; north_star "one thread per seed ...
+// keeps the 5-parameter state and covariance in registers"), plus the a5 ownership vote
+// (atomicMax on packed (n_hits, rank) words, P26) fused at the end of each tracklet.
+//
+// fp32 on the device.  To keep fp32 residuals exact for long drift offsets (configs[2]: |z| up to ~5400 cm) the
+// filter runs in coordinates relative to the seed's first cluster: hit - origin is an exact integer difference,
+// and the model is translation invariant in y and z.  The origin is added back in double at the end.
+//
+// Thread per seed; seeds ascend by start id, so the lanes of a warp start in the same or adjacent rows of one
+// sector and step through the rows together.  Hit table layout [row][seed] makes those accesses coalesced.
+#include "tpc_internal.cuh"
+
+namespace {
+
+struct Cov {   // symmetric 5x5, lower triangle
+  float c00, c10, c11, c20, c21, c22, c30, c31, c32, c33, c40, c41, c42, c43, c44;
+};
+
+struct State {
+  float y, z, s, t, q;   // relative y, relative z, sin phi, tan lambda, q/pT
+};
+
+__device__ __forceinline__ void cov_reset(const DevGeom& g, Cov& C) {
+  C.c00 = g.c_reset[0]; C.c11 = g.c_reset[1]; C.c22 = g.c_reset[2]; C.c33 = g.c_reset[3]; C.c44 = g.c_reset[4];
+  C.c10 = C.c20 = C.c21 = C.c30 = C.c31 = C.c32 = C.c40 = C.c41 = C.c42 = C.c43 = 0.f;
+}
+
+// Appendix C.  One step of dx (either sign) along the helix; k = cq * q/pT.  Returns false (state untouched)
+// iff |sin phi| >= sinphi_max before or after (P18).  WITH_COV: C <- F C F^T with
+// F = I + [02]=a [04]=b [12]=c [13]=d [14]=e [24]=f.
+template <bool WITH_COV>
+__device__ __forceinline__ bool transport(const DevGeom& g, float dx, State& p, Cov& C) {
+  const float k = g.cq * p.q;
+  const float s0 = p.s;
+  const float s1 = fmaf(k, dx, s0);
+  if (!(fabsf(s0) < g.sinphi_max) || !(fabsf(s1) < g.sinphi_max)) return false;
+  const float c0 = sqrtf(fmaf(-s0, s0, 1.f)), c1 = sqrtf(fmaf(-s1, s1, 1.f));
+  const float tau = (s0 + s1) / (c0 + c1);
+  const float dy = dx * tau;
+  const float chord = copysignf(sqrtf(fmaf(dx, dx, dy * dy)), dx);
+  const float u = 0.5f * k * chord;
+  const float u2 = u * u;
+  // asin(u)/u = 1 + u^2/6 + 3u^4/40 + 15u^6/336 + 105 u^8/3456 ...
+  const float dS = (u2 < 0.01f) ? chord * fmaf(u2, fmaf(u2, fmaf(u2, fmaf(u2, 0.030381944f, 0.044642857f), 0.075f),
+                                                        0.16666667f), 1.f)
+                                : chord * asinf(u) / u;
+  if (WITH_COV) {
+    const float m = fmaf(s0, tau, c0);
+    const float ic0c1 = 1.f / (c0 * c1);
+    const float d_ = 0.5f * k * dS;
+    const float d2 = d_ * d_;
+    float sinc, gg;
+    if (d2 < 0.01f) {
+      sinc = fmaf(d2, fmaf(d2, 1.f / 120.f, -1.f / 6.f), 1.f);
+      gg = fmaf(d2, fmaf(d2, 1.f / 840.f, -1.f / 30.f), 1.f / 3.f);
+    } else {
+      float sn, cs;
+      sincosf(d_, &sn, &cs);
+      sinc = sn / d_;
+      gg = (sn - d_ * cs) / (d_ * d2);
+    }
+    const float cm = rsqrtf(fmaf(tau, tau, 1.f)), sm = tau * cm;
+    const float dSdk = (0.5f * dS * dS * sm * sinc + 0.25f * k * dS * dS * dS * cm * gg) / c1;
+    const float a = dx * m * ic0c1;                        // dy1/ds
+    const float b = g.cq * dx * dx * m / (c1 * (c0 + c1)); // dy1/dq
+    const float c = p.t * dy * ic0c1;                      // dz1/ds
+    const float d = dS;                                    // dz1/dt
+    const float e = p.t * g.cq * dSdk;                     // dz1/dq
+    const float f = g.cq * dx;                             // ds1/dq
+    // M = F C (rows 0..2 change), then C' = M F^T
+    const float m00 = C.c00 + a * C.c20 + b * C.c40;
+    const float m02 = C.c20 + a * C.c22 + b * C.c42;
+    const float m04 = C.c40 + a * C.c42 + b * C.c44;
+    const float m10 = C.c10 + c * C.c20 + d * C.c30 + e * C.c40;
+    const float m11 = C.c11 + c * C.c21 + d * C.c31 + e * C.c41;
+    const float m12 = C.c21 + c * C.c22 + d * C.c32 + e * C.c42;
+    const float m13 = C.c31 + c * C.c32 + d * C.c33 + e * C.c43;
+    const float m14 = C.c41 + c * C.c42 + d * C.c43 + e * C.c44;
+    const float m20 = C.c20 + f * C.c40;
+    const float m21 = C.c21 + f * C.c41;
+    const float m22 = C.c22 + f * C.c42;
+    const float m23 = C.c32 + f * C.c43;
+    const float m24 = C.c42 + f * C.c44;
+    Cov N;
+    N.c00 = m00 + a * m02 + b * m04;
+    N.c10 = m10 + a * m12 + b * m14;
+    N.c11 = m11 + c * m12 + d * m13 + e * m14;
+    N.c20 = m20 + a * m22 + b * m24;
+    N.c21 = m21 + c * m22 + d * m23 + e * m24;
+    N.c22 = m22 + f * m24;
+    N.c30 = C.c30 + a * C.c32 + b * C.c43;
+    N.c31 = C.c31 + c * C.c32 + d * C.c33 + e * C.c43;
+    N.c32 = C.c32 + f * C.c43;
+    N.c33 = C.c33;
+    N.c40 = C.c40 + a * C.c42 + b * C.c44;
+    N.c41 = C.c41 + c * C.c42 + d * C.c43 + e * C.c44;
+    N.c42 = C.c42 + f * C.c44;
+    N.c43 = C.c43;
+    N.c44 = C.c44;
+    C = N;
+  }
+  p.y += dy;
+  p.z = fmaf(p.t, dS, p.z);
+  p.s = s1;
+  return true;
+}
+
+// Appendix C update with H = [I2 | 0], V = diag(sy2, sz2).  Returns the chi2 increment.
+__device__ __forceinline__ float update(const DevGeom& g, State& p, Cov& C, float ym, float zm) {
+  const float S00 = C.c00 + g.sy2, S01 = C.c10, S11 = C.c11 + g.sz2;
+  const float idet = 1.f / (S00 * S11 - S01 * S01);
+  const float I00 = S11 * idet, I01 = -S01 * idet, I11 = S00 * idet;
+  const float r0 = ym - p.y, r1 = zm - p.z;
+  // K = C[:,0:2] S^-1
+  const float k00 = C.c00 * I00 + C.c10 * I01, k01 = C.c00 * I01 + C.c10 * I11;
+  const float k10 = C.c10 * I00 + C.c11 * I01, k11 = C.c10 * I01 + C.c11 * I11;
+  const float k20 = C.c20 * I00 + C.c21 * I01, k21 = C.c20 * I01 + C.c21 * I11;
+  const float k30 = C.c30 * I00 + C.c31 * I01, k31 = C.c30 * I01 + C.c31 * I11;
+  const float k40 = C.c40 * I00 + C.c41 * I01, k41 = C.c40 * I01 + C.c41 * I11;
+  p.y += k00 * r0 + k01 * r1;
+  p.z += k10 * r0 + k11 * r1;
+  p.s += k20 * r0 + k21 * r1;
+  p.t += k30 * r0 + k31 * r1;
+  p.q += k40 * r0 + k41 * r1;
+  // C <- C - K (H C), lower triangle: C_ij -= K_i0 C_0j + K_i1 C_1j
+  Cov N;
+  N.c00 = C.c00 - (k00 * C.c00 + k01 * C.c10);
+  N.c10 = C.c10 - (k10 * C.c00 + k11 * C.c10);
+  N.c11 = C.c11 - (k10 * C.c10 + k11 * C.c11);
+  N.c20 = C.c20 - (k20 * C.c00 + k21 * C.c10);
+  N.c21 = C.c21 - (k20 * C.c10 + k21 * C.c11);
+  N.c22 = C.c22 - (k20 * C.c20 + k21 * C.c21);
+  N.c30 = C.c30 - (k30 * C.c00 + k31 * C.c10);
+  N.c31 = C.c31 - (k30 * C.c10 + k31 * C.c11);
+  N.c32 = C.c32 - (k30 * C.c20 + k31 * C.c21);
+  N.c33 = C.c33 - (k30 * C.c30 + k31 * C.c31);
+  N.c40 = C.c40 - (k40 * C.c00 + k41 * C.c10);
+  N.c41 = C.c41 - (k40 * C.c10 + k41 * C.c11);
+  N.c42 = C.c42 - (k40 * C.c20 + k41 * C.c21);
+  N.c43 = C.c43 - (k40 * C.c30 + k41 * C.c31);
+  N.c44 = C.c44 - (k40 * C.c40 + k41 * C.c41);
+  C = N;
+  return r0 * (I00 * r0 + I01 * r1) + r1 * (I01 * r0 + I11 * r1);
+}
+
+__device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
+
+struct Found {
+  int id;
+  float y, z;   // relative coordinates of the accepted hit
+};
+
+// P17/P21: among the clusters of sector-row `sr` with |dy| <= gate_y and |dz| <= gate_z (cm) minimise (d, id),
+// d = dy^2/(Cyy + sy2) + dz^2/(Czz + sz2); accept iff d < gate_d.  The a1 grid only prunes.
+__device__ __forceinline__ Found search_row(const DevGeom& g, int sr, int row, const State& p, const Cov& C, int y0,
+                                            int z0, const int32_t* __restrict__ ys, const int32_t* __restrict__ zs,
+                                            const int32_t* __restrict__ ids, const int2* __restrict__ row_org,
+                                            const uint32_t* __restrict__ bin_start) {
+  Found f;
+  f.id = -1;
+  f.y = f.z = 0.f;
+  const int2 org = row_org[sr];
+  const int ny = g.ny_row[row];
+  const uint32_t* bs = bin_start + (size_t)sr * g.nb_stride;
+  // integer superset of the float window (+-1 unit of slack on each side), clamped against overflow
+  const float lim = 1.0e9f;
+  const int ylo = y0 + (int)fminf(fmaxf(floorf((p.y - g.gate_y) * g.units) - 1.f, -lim), lim);
+  const int yhi = y0 + (int)fminf(fmaxf(ceilf((p.y + g.gate_y) * g.units) + 1.f, -lim), lim);
+  const int zlo = z0 + (int)fminf(fmaxf(floorf((p.z - g.gate_z) * g.units) - 1.f, -lim), lim);
+  const int zhi = z0 + (int)fminf(fmaxf(ceilf((p.z + g.gate_z) * g.units) + 1.f, -lim), lim);
+  const int iy_lo = clampi((ylo - org.x) >> g.shift_y, 0, ny - 1);
+  const int iy_hi = clampi((yhi - org.x) >> g.shift_y, 0, ny - 1);
+  const int iz_lo = clampi((zlo - org.y) >> g.shift_z, 0, g.nz - 1);
+  const int iz_hi = clampi((zhi - org.y) >> g.shift_z, 0, g.nz - 1);
+  const float wy = 1.f / (C.c00 + g.sy2), wz = 1.f / (C.c11 + g.sz2);
+  float bestd = __int_as_float(0x7f800000);
+  for (int iz = iz_lo; iz <= iz_hi; ++iz) {
+    const uint32_t a = bs[iz * ny + iy_lo], b = bs[iz * ny + iy_hi + 1];
+    for (uint32_t j = a; j < b; ++j) {
+      const float cy = (float)(ys[j] - y0) * g.inv_units, cz = (float)(zs[j] - z0) * g.inv_units;
+      const float dy = cy - p.y, dz = cz - p.z;
+      if (fabsf(dy) > g.gate_y || fabsf(dz) > g.gate_z) continue;
+      const float d = dy * dy * wy + dz * dz * wz;
+      if (d > bestd) continue;
+      const int id = ids[j];
+      if (d < bestd || id < f.id) {
+        bestd = d;
+        f.id = id;
+        f.y = cy;
+        f.z = cz;
+      }
+    }
+  }
+  if (!(bestd < g.gate_d)) f.id = -1;
+  return f;
+}
+
+__global__ void __launch_bounds__(A4_BLOCK)
+a4_follow_kernel(const DevGeom g, int64_t s_cap, const DevCtl* __restrict__ ctl, const int32_t* __restrict__ y,
+                 const int32_t* __restrict__ z, const uint32_t* __restrict__ ro, const int32_t* __restrict__ ys,
+                 const int32_t* __restrict__ zs, const int32_t* __restrict__ ids, const int2* __restrict__ row_org,
+                 const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ up_c,
+                 const int32_t* __restrict__ seed_start, float* __restrict__ tl_par, float* __restrict__ tl_cov,
+                 float* __restrict__ tl_chi2, int32_t* __restrict__ tl_nhits, int32_t* __restrict__ tl_sr0,
+                 int32_t* __restrict__ tl_hits, uint32_t* __restrict__ owner) {
+  const int64_t i = (int64_t)blockIdx.x * A4_BLOCK + threadIdx.x;
+  if (i >= (int64_t)ctl->n_seeds) return;
+  const int nr = g.n_rows;
+  const int h0 = seed_start[i];
+  // (sector,row) of the seed: largest sr with ro[sr] <= h0
+  int lo = 0, hi = g.n_sectors * nr;
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (ro[mid] <= (uint32_t)h0) lo = mid; else hi = mid;
+  }
+  const int sec_base = (lo / nr) * nr;
+  const int r0 = lo - sec_base;
+  int32_t* hits = tl_hits + i;   // hits[row * s_cap]
+
+  // P19 init from the first two chain hits
+  const int y0 = y[h0], z0 = z[h0];
+  int h = up_c[h0];
+  State p;
+  Cov C;
+  {
+    const float dxr = g.row_dx[r0];
+    const float dy = (float)(y[h] - y0) * g.inv_units, dz = (float)(z[h] - z0) * g.inv_units;
+    const float ichord = rsqrtf(fmaf(dxr, dxr, dy * dy));
+    p.y = 0.f; p.z = 0.f; p.s = dy * ichord; p.t = dz * ichord; p.q = 0.f;
+  }
+  cov_reset(g, C);
+  update(g, p, C, 0.f, 0.f);
+  hits[(int64_t)r0 * s_cap] = h0;
+  int row = r0, nh = 1;
+  bool fail_up = false;
+
+  // Phase A: fit up the chain, no gate
+  while (h >= 0) {
+    if (!transport<true>(g, g.row_dx[row], p, C)) { fail_up = true; break; }
+    ++row;
+    update(g, p, C, (float)(y[h] - y0) * g.inv_units, (float)(z[h] - z0) * g.inv_units);
+    hits[(int64_t)row * s_cap] = h;
+    ++nh;
+    h = up_c[h];
+  }
+  // Phase B: extend up with the gated nearest-hit search (P20)
+  if (!fail_up) {
+    int miss = 0;
+    while (row + 1 <= nr - 1 && miss < g.max_miss) {
+      if (!transport<true>(g, g.row_dx[row], p, C)) break;
+      ++row;
+      const Found f = search_row(g, sec_base + row, row, p, C, y0, z0, ys, zs, ids, row_org, bin_start);
+      hits[(int64_t)row * s_cap] = f.id;
+      if (f.id >= 0) {
+        update(g, p, C, f.y, f.z);
+        ++nh;
+        miss = 0;
+      } else {
+        ++miss;
+      }
+    }
+  }
+  for (int r = row + 1; r < nr; ++r) hits[(int64_t)r * s_cap] = -1;
+
+  // Phase C: keep the state, reset the covariance (P22), refit down over the recorded hits;
+  // Phase D: below the seed's first row search as in B.
+  cov_reset(g, C);
+  float chi2 = 0.f;
+  {
+    const int hh = hits[(int64_t)row * s_cap];
+    if (hh >= 0) chi2 += update(g, p, C, (float)(y[hh] - y0) * g.inv_units, (float)(z[hh] - z0) * g.inv_units);
+  }
+  bool fail_dn = false;
+  int miss = 0, lowest = r0;
+  while (row > 0) {
+    if (row - 1 < r0 && miss >= g.max_miss) break;
+    if (!transport<true>(g, -g.row_dx[row - 1], p, C)) { fail_dn = true; break; }
+    --row;
+    if (row >= r0) {
+      const int hh = hits[(int64_t)row * s_cap];
+      if (hh >= 0) chi2 += update(g, p, C, (float)(y[hh] - y0) * g.inv_units, (float)(z[hh] - z0) * g.inv_units);
+    } else {
+      const Found f = search_row(g, sec_base + row, row, p, C, y0, z0, ys, zs, ids, row_org, bin_start);
+      hits[(int64_t)row * s_cap] = f.id;
+      if (f.id >= 0) {
+        chi2 += update(g, p, C, f.y, f.z);
+        ++nh;
+        lowest = row;
+        miss = 0;
+      } else {
+        ++miss;
+      }
+    }
+  }
+  // rows below the last visited one (rows < r0 only: rows >= r0 were all written in A/B)
+  for (int r = min(row, r0) - 1; r >= 0; --r) hits[(int64_t)r * s_cap] = -1;
+
+  // P23: transport (no update) back to the lowest-row hit
+  int xrow = row;
+  if (!fail_dn && lowest != row) {
+    const float dx = (float)(g.row_x[lowest] - g.row_x[row]);
+    if (transport<true>(g, dx, p, C)) xrow = lowest;
+  }
+  tl_par[0 * s_cap + i] = (float)g.row_x[xrow];
+  tl_par[1 * s_cap + i] = (float)((double)p.y + (double)y0 * g.inv_units_d);
+  tl_par[2 * s_cap + i] = (float)((double)p.z + (double)z0 * g.inv_units_d);
+  tl_par[3 * s_cap + i] = p.s;
+  tl_par[4 * s_cap + i] = p.t;
+  tl_par[5 * s_cap + i] = p.q;
+  const float cv[15] = {C.c00, C.c10, C.c11, C.c20, C.c21, C.c22, C.c30, C.c31, C.c32, C.c33,
+                        C.c40, C.c41, C.c42, C.c43, C.c44};
+#pragma unroll
+  for (int k = 0; k < 15; ++k) tl_cov[k * s_cap + i] = cv[k];
+  tl_chi2[i] = chi2;
+  tl_nhits[i] = nh;
+  tl_sr0[i] = sec_base + r0;
+
+  // a5 vote (P24, P26): owner(h) = surviving tracklet with the most hits, ties -> smallest rank
+  if (nh >= g.n_min_tracklet) {
+    const uint32_t word = ((uint32_t)nh << 24) | (0xFFFFFFu - (uint32_t)i);
+    for (int r = 0; r < nr; ++r) {
+      const int hh = hits[(int64_t)r * s_cap];
+      if (hh >= 0) atomicMax(&owner[hh], word);
+    }
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_a4_follow(const tpc_tracker* t, const int32_t* y, const int32_t* z, const uint32_t* ro, int64_t n,
+                             cudaStream_t st) {
+  if (n == 0 || t->s_cap == 0) return cudaSuccess;
+  const unsigned blocks = (unsigned)((t->s_cap + A4_BLOCK - 1) / A4_BLOCK);
+  a4_follow_kernel<<<blocks, A4_BLOCK, 0, st>>>(t->g, t->s_cap, t->s.ctl, y, z, ro, t->s.ys, t->s.zs, t->s.ids,
+                                               t->s.row_org, t->s.bin_start, t->s.up_c, t->s.seed_start, t->s.tl_par,
+                                               t->s.tl_cov, t->s.tl_chi2, t->s.tl_nhits, t->s.tl_sr0, t->s.tl_hits,
+                                               t->s.owner);
+  return cudaGetLastError();
+}

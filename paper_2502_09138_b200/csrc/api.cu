@@ -1,0 +1,428 @@
+// api.cu -- the C ABI of libtpctrack.so (include/tpc_track.h): handle, scratch arena, stage sequencing.
+// The five stages are enqueued back to back on the caller's stream; seed and track counts stay on the device
+// (grids are sized by upper bounds), so a call never synchronises unless the arena has to grow.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "tpc_internal.cuh"
+
+namespace {
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+int fail_cuda(tpc_tracker* t, cudaError_t e, const char* where) {
+  t->last_err = e;
+  snprintf(t->err_buf, sizeof(t->err_buf), "%s: %s", where, cudaGetErrorString(e));
+  return TPC_ERR_CUDA;
+}
+
+#define TPC_CUDA(t, call)                                   \
+  do {                                                      \
+    cudaError_t e_ = (call);                                \
+    if (e_ != cudaSuccess) return fail_cuda(t, e_, #call);  \
+  } while (0)
+
+int ceil_log2(int64_t v) {
+  int s = 0;
+  while (((int64_t)1 << s) < v) ++s;
+  return s;
+}
+
+// Lays the scratch arrays out inside one allocation; returns the total size.  base may be NULL (size query).
+size_t layout(tpc_tracker* t, char* base, int64_t n, int64_t R) {
+  size_t off = 0;
+  auto take = [&](size_t bytes) -> char* {
+    char* p = base ? base + off : nullptr;
+    off += align_up(bytes, 256);
+    return p;
+  };
+  const int64_t s_cap = n / t->params.l_min + 1;
+  const int64_t tiles_a3 = (n + A3_TILE - 1) / A3_TILE;
+  const int64_t tiles_a5 = (s_cap + A5_TILE - 1) / A5_TILE;
+  Scratch& s = t->s;
+  // zeroed per call: ctl + look-back status words (kept contiguous, first in the arena)
+  s.ctl = (DevCtl*)take(sizeof(DevCtl));
+  s.scan_a3 = (uint64_t*)take((size_t)tiles_a3 * 8);
+  s.scan_a5 = (uint64_t*)take((size_t)tiles_a5 * 16);
+  const size_t ctl_bytes = off;
+  s.ys = (int32_t*)take((size_t)n * 4 + 64);
+  s.zs = (int32_t*)take((size_t)n * 4 + 64);
+  s.ids = (int32_t*)take((size_t)n * 4 + 64);
+  s.row_org = (int2*)take((size_t)R * sizeof(int2));
+  s.bin_start = (uint32_t*)take((size_t)R * t->g.nb_stride * 4);
+  s.link_up = (int32_t*)take((size_t)n * 4);
+  s.link_dn = (int32_t*)take((size_t)n * 4);
+  s.up_c = (int32_t*)take((size_t)n * 4);
+  s.owner = (uint32_t*)take((size_t)n * 4);
+  s.seed_start = (int32_t*)take((size_t)s_cap * 4);
+  s.tl_par = (float*)take((size_t)s_cap * 6 * 4);
+  s.tl_cov = (float*)take((size_t)s_cap * 15 * 4);
+  s.tl_chi2 = (float*)take((size_t)s_cap * 4);
+  s.tl_nhits = (int32_t*)take((size_t)s_cap * 4);
+  s.tl_sr0 = (int32_t*)take((size_t)s_cap * 4);
+  s.tl_hits = (int32_t*)take((size_t)s_cap * t->g.n_rows * 4);
+  if (base) {
+    t->s_cap = s_cap;
+    t->tiles_a3 = tiles_a3;
+    t->tiles_a5 = tiles_a5;
+    t->ctl_bytes = ctl_bytes;
+  }
+  return off;
+}
+
+int ensure_arena(tpc_tracker* t, int64_t n, int64_t R) {
+  if (t->arena && n <= t->cap_n && R <= t->cap_rows) {
+    // same allocation, but s_cap / tile counts follow the actual n so that grids stay tight
+    layout(t, (char*)t->arena, n, R);
+    return TPC_OK;
+  }
+  int64_t cap_n = n, cap_r = R;
+  if (t->arena) {   // geometric growth
+    cap_n = n > t->cap_n ? n + n / 4 : t->cap_n;
+    cap_r = R > t->cap_rows ? R : t->cap_rows;
+    TPC_CUDA(t, cudaDeviceSynchronize());
+    TPC_CUDA(t, cudaFree(t->arena));
+    t->arena = nullptr;
+    t->arena_bytes = 0;
+  }
+  const size_t bytes = layout(t, nullptr, cap_n, cap_r);
+  void* p = nullptr;
+  cudaError_t e = cudaMalloc(&p, bytes);
+  if (e == cudaErrorMemoryAllocation) {
+    cudaGetLastError();
+    return TPC_ERR_NOMEM;
+  }
+  if (e != cudaSuccess) return fail_cuda(t, e, "cudaMalloc(arena)");
+  t->arena = p;
+  t->arena_bytes = bytes;
+  t->cap_n = cap_n;
+  t->cap_rows = cap_r;
+  layout(t, (char*)p, n, R);
+  return TPC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+#pragma GCC visibility push(default)
+
+void tpc_default_params(tpc_params_t* p) {
+  if (!p) return;
+  memset(p, 0, sizeof(*p));
+  p->w_y = 1280;
+  p->w_z = 1600;
+  p->cost_wy = 9;
+  p->cost_wz = 4;
+  p->c_max = 3538944;
+  p->l_min = 5;
+  p->max_miss = 5;
+  p->n_min_tracklet = 10;
+  p->n_min_owned = 10;
+  p->sigma_y = 0.1;
+  p->sigma_z = 0.15;
+  p->sinphi_max = 0.95;
+  p->gate_d = 15.0;
+  p->gate_y_cm = 2.0;
+  p->gate_z_cm = 2.5;
+  p->c_reset[0] = 0.25;
+  p->c_reset[1] = 0.25;
+  p->c_reset[2] = 0.05;
+  p->c_reset[3] = 0.05;
+  p->c_reset[4] = 25.0;
+  p->cq_per_tesla = -0.00299792458;
+}
+
+const char* tpc_status_string(int status) {
+  switch (status) {
+    case TPC_OK: return "ok";
+    case TPC_ERR_ARG: return "bad argument";
+    case TPC_ERR_GEOMETRY: return "bad geometry (n_rows < 3, rows not equidistant or extents not positive)";
+    case TPC_ERR_CUDA: return "CUDA runtime error";
+    case TPC_ERR_NOMEM: return "out of device memory";
+    case TPC_ERR_CAPACITY: return "too many clusters for one call";
+    default: return "unknown status";
+  }
+}
+
+const char* tpc_last_cuda_error(const tpc_tracker_t* t) { return t ? t->err_buf : ""; }
+
+int tpc_tracker_create(const tpc_geometry_t* geo, const tpc_field_t* field, tpc_tracker_t** out) {
+  if (!geo || !field || !out) return TPC_ERR_ARG;
+  *out = nullptr;
+  if (!geo->row_x || geo->n_sectors < 0) return TPC_ERR_ARG;
+  if (geo->n_rows < 3 || !(geo->units_per_cm > 0) || !(geo->z_extent_cm > 0)) return TPC_ERR_GEOMETRY;
+  if (!(geo->y_half_cm > 0) && !(geo->y_half_tan > 0)) return TPC_ERR_GEOMETRY;
+  const int nr = geo->n_rows;
+  const double pitch = (geo->row_x[nr - 1] - geo->row_x[0]) / (nr - 1);
+  if (!(pitch > 0)) return TPC_ERR_GEOMETRY;
+  for (int r = 0; r + 1 < nr; ++r)   // P6: the a2 cost is a second difference, valid for equidistant rows only
+    if (fabs((geo->row_x[r + 1] - geo->row_x[r]) - pitch) > 1e-6 * pitch) return TPC_ERR_GEOMETRY;
+
+  tpc_params_t prm;
+  if (geo->params) prm = *geo->params; else tpc_default_params(&prm);
+  if (prm.w_y < 0 || prm.w_z < 0 || prm.cost_wy < 0 || prm.cost_wz < 0 || prm.c_max < 0 || prm.l_min < 2 ||
+      prm.max_miss < 0 || prm.n_min_tracklet < 1 || prm.n_min_tracklet > 255 || prm.n_min_owned < 1 ||
+      nr > 255 || !(prm.sigma_y > 0) || !(prm.sigma_z > 0) || !(prm.sinphi_max > 0) || !(prm.sinphi_max < 1) ||
+      !(prm.gate_y_cm >= 0) || !(prm.gate_z_cm >= 0))
+    return TPC_ERR_ARG;
+  // the a2 cost must fit int32: |ddy| <= 2 w_y, |ddz| <= 2 w_z
+  {
+    const double cmaxv = (double)prm.cost_wy * 4.0 * prm.w_y * prm.w_y + (double)prm.cost_wz * 4.0 * prm.w_z * prm.w_z;
+    if (cmaxv >= 2147483647.0) return TPC_ERR_ARG;
+  }
+
+  tpc_tracker* t = new (std::nothrow) tpc_tracker();
+  if (!t) return TPC_ERR_NOMEM;
+  memset(t, 0, sizeof(*t));
+  t->params = prm;
+  t->bz = field->bz_tesla;
+  cudaError_t e = cudaGetDevice(&t->device);
+  if (e != cudaSuccess) {
+    delete t;
+    return TPC_ERR_CUDA;
+  }
+
+  DevGeom& g = t->g;
+  g.n_sectors = geo->n_sectors;
+  g.n_rows = nr;
+  const int64_t gy = (int64_t)ceil(prm.gate_y_cm * geo->units_per_cm) + 2, gz = (int64_t)ceil(prm.gate_z_cm * geo->units_per_cm) + 2;
+  g.shift_y = ceil_log2(2 * (prm.w_y > gy ? prm.w_y : gy) + 1);
+  g.shift_z = ceil_log2(2 * (prm.w_z > gz ? prm.w_z : gz) + 1);
+  const int64_t z_units = (int64_t)ceil(geo->z_extent_cm * geo->units_per_cm);
+  int* ny_host = new (std::nothrow) int[nr];
+  float* dx_host = new (std::nothrow) float[nr];
+  if (!ny_host || !dx_host) {
+    delete[] ny_host;
+    delete[] dx_host;
+    delete t;
+    return TPC_ERR_NOMEM;
+  }
+  int64_t nb;
+  for (;;) {   // shrink the bin count until one row's histogram fits the shared memory of a CTA
+    int ny_max = 1;
+    for (int r = 0; r < nr; ++r) {
+      const double yh = geo->y_half_cm > 0 ? geo->y_half_cm : geo->row_x[r] * geo->y_half_tan;
+      const int64_t span = (int64_t)ceil(2.0 * yh * geo->units_per_cm);
+      ny_host[r] = (int)((span >> g.shift_y) + 2);
+      if (ny_host[r] > ny_max) ny_max = ny_host[r];
+    }
+    g.nz = (int)((z_units >> g.shift_z) + 2);
+    nb = (int64_t)ny_max * g.nz;
+    if (nb + 1 <= 48 * 1024) break;
+    if (g.nz > ny_max) ++g.shift_z; else ++g.shift_y;
+  }
+  g.nb_stride = (int)align_up((size_t)nb + 1, 4);
+  for (int r = 0; r < nr; ++r) dx_host[r] = (float)(geo->row_x[r + 1 < nr ? r + 1 : r] - geo->row_x[r + 1 < nr ? r : r - 1]);
+  g.w_y = prm.w_y; g.w_z = prm.w_z; g.cost_wy = prm.cost_wy; g.cost_wz = prm.cost_wz; g.c_max = prm.c_max;
+  g.l_min = prm.l_min; g.max_miss = prm.max_miss; g.n_min_tracklet = prm.n_min_tracklet; g.n_min_owned = prm.n_min_owned;
+  g.sy2 = (float)(prm.sigma_y * prm.sigma_y);
+  g.sz2 = (float)(prm.sigma_z * prm.sigma_z);
+  g.sinphi_max = (float)prm.sinphi_max;
+  g.gate_d = (float)prm.gate_d;
+  g.gate_y = (float)prm.gate_y_cm;
+  g.gate_z = (float)prm.gate_z_cm;
+  g.inv_units = (float)(1.0 / geo->units_per_cm);
+  g.units = (float)geo->units_per_cm;
+  g.inv_units_d = 1.0 / geo->units_per_cm;
+  g.cq = (float)(prm.cq_per_tesla * field->bz_tesla);
+  for (int k = 0; k < 5; ++k) g.c_reset[k] = (float)prm.c_reset[k];
+
+  // geometry tables in one small device blob: row_x (double) | row_dx (float) | ny_row (int)
+  const size_t o_dx = align_up((size_t)nr * 8, 256), o_ny = o_dx + align_up((size_t)nr * 4, 256);
+  const size_t blob = o_ny + align_up((size_t)nr * 4, 256);
+  int rc = TPC_OK;
+  e = cudaMalloc(&t->geom_blob, blob);
+  if (e == cudaSuccess) e = cudaMemcpy(t->geom_blob, geo->row_x, (size_t)nr * 8, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy((char*)t->geom_blob + o_dx, dx_host, (size_t)nr * 4, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy((char*)t->geom_blob + o_ny, ny_host, (size_t)nr * 4, cudaMemcpyHostToDevice);
+  delete[] ny_host;
+  delete[] dx_host;
+  g.row_x = (const double*)t->geom_blob;
+  g.row_dx = (const float*)((char*)t->geom_blob + o_dx);
+  g.ny_row = (const int32_t*)((char*)t->geom_blob + o_ny);
+  if (e == cudaSuccess) e = setup_a1_attributes(t);
+  for (int k = 0; k < 6 && e == cudaSuccess; ++k) e = cudaEventCreate(&t->ev[k]);
+  if (e != cudaSuccess) {
+    rc = e == cudaErrorMemoryAllocation ? TPC_ERR_NOMEM : TPC_ERR_CUDA;
+    cudaGetLastError();
+    tpc_tracker_destroy(t);
+    return rc;
+  }
+  *out = t;
+  return TPC_OK;
+}
+
+int tpc_tracker_destroy(tpc_tracker_t* t) {
+  if (!t) return TPC_ERR_ARG;
+  cudaDeviceSynchronize();
+  if (t->arena) cudaFree(t->arena);
+  if (t->host_arena) cudaFree(t->host_arena);
+  if (t->geom_blob) cudaFree(t->geom_blob);
+  for (int k = 0; k < 6; ++k)
+    if (t->ev[k]) cudaEventDestroy(t->ev[k]);
+  delete t;
+  return TPC_OK;
+}
+
+int tpc_track(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* stream, tpc_tracks_out_t* out) {
+  if (!t || !cl || !out || n < 0) return TPC_ERR_ARG;
+  if (!out->counts || out->track_capacity < 0 || out->hit_capacity < 0) return TPC_ERR_ARG;
+  if ((out->track_capacity > 0 && !out->tracks) || (out->hit_capacity > 0 && !out->hit_ids)) return TPC_ERR_ARG;
+  if (n > 0 && (!cl->y || !cl->z)) return TPC_ERR_ARG;
+  if (!cl->row_offsets) return TPC_ERR_ARG;
+  if (n >= ((int64_t)1 << 31) || n / t->params.l_min + 1 >= 0xFFFFFF) return TPC_ERR_CAPACITY;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
+  int rc = ensure_arena(t, n, R);
+  if (rc != TPC_OK) return rc;
+  t->last_n = n;
+  t->last_ro = cl->row_offsets;
+  t->last_y = cl->y;
+  t->last_z = cl->z;
+  TPC_CUDA(t, cudaMemsetAsync(t->s.ctl, 0, t->ctl_bytes, st));
+  if (t->timing) TPC_CUDA(t, cudaEventRecord(t->ev[0], st));
+  TPC_CUDA(t, launch_a1_grid(t, cl->y, cl->z, cl->row_offsets, n, st));
+  if (t->timing) TPC_CUDA(t, cudaEventRecord(t->ev[1], st));
+  TPC_CUDA(t, launch_a2_neighbours(t, cl->row_offsets, n, st));
+  if (t->timing) TPC_CUDA(t, cudaEventRecord(t->ev[2], st));
+  TPC_CUDA(t, launch_a3_seeds(t, n, st));
+  if (t->timing) TPC_CUDA(t, cudaEventRecord(t->ev[3], st));
+  TPC_CUDA(t, launch_a4_follow(t, cl->y, cl->z, cl->row_offsets, n, st));
+  if (t->timing) TPC_CUDA(t, cudaEventRecord(t->ev[4], st));
+  TPC_CUDA(t, launch_a5_select(t, out, st));
+  if (t->timing) TPC_CUDA(t, cudaEventRecord(t->ev[5], st));
+  return TPC_OK;
+}
+
+int tpc_track_host(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* stream, tpc_tracks_out_t* out) {
+  if (!t || !cl || !out || n < 0) return TPC_ERR_ARG;
+  if (!out->counts || out->track_capacity < 0 || out->hit_capacity < 0) return TPC_ERR_ARG;
+  if ((out->track_capacity > 0 && !out->tracks) || (out->hit_capacity > 0 && !out->hit_ids)) return TPC_ERR_ARG;
+  if (!cl->row_offsets || (n > 0 && (!cl->y || !cl->z))) return TPC_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
+  // device staging for the caller's host buffers
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes, 256); return o; };
+  const size_t o_y = take((size_t)n * 4), o_z = take((size_t)n * 4), o_ro = take((size_t)(R + 1) * 4);
+  const size_t o_tr = take((size_t)out->track_capacity * sizeof(tpc_track_rec_t));
+  const size_t o_h = take((size_t)out->hit_capacity * 4), o_c = take(16);
+  if (off > t->host_arena_bytes) {
+    if (t->host_arena) {
+      TPC_CUDA(t, cudaDeviceSynchronize());
+      TPC_CUDA(t, cudaFree(t->host_arena));
+      t->host_arena = nullptr;
+      t->host_arena_bytes = 0;
+    }
+    cudaError_t e = cudaMalloc(&t->host_arena, off);
+    if (e == cudaErrorMemoryAllocation) {
+      cudaGetLastError();
+      return TPC_ERR_NOMEM;
+    }
+    if (e != cudaSuccess) return fail_cuda(t, e, "cudaMalloc(host staging)");
+    t->host_arena_bytes = off;
+  }
+  char* b = (char*)t->host_arena;
+  tpc_clusters_t dcl = {(const int32_t*)(b + o_y), (const int32_t*)(b + o_z), (const uint32_t*)(b + o_ro)};
+  tpc_tracks_out_t dout;
+  dout.tracks = (tpc_track_rec_t*)(b + o_tr);
+  dout.track_capacity = out->track_capacity;
+  dout.hit_capacity = out->hit_capacity;
+  dout.hit_ids = (int32_t*)(b + o_h);
+  dout.counts = (int32_t*)(b + o_c);
+  if (n > 0) {
+    TPC_CUDA(t, cudaMemcpyAsync(b + o_y, cl->y, (size_t)n * 4, cudaMemcpyHostToDevice, st));
+    TPC_CUDA(t, cudaMemcpyAsync(b + o_z, cl->z, (size_t)n * 4, cudaMemcpyHostToDevice, st));
+  }
+  TPC_CUDA(t, cudaMemcpyAsync(b + o_ro, cl->row_offsets, (size_t)(R + 1) * 4, cudaMemcpyHostToDevice, st));
+  int rc = tpc_track(t, &dcl, n, stream, &dout);
+  if (rc != TPC_OK) return rc;
+  TPC_CUDA(t, cudaMemcpyAsync(out->counts, dout.counts, 16, cudaMemcpyDeviceToHost, st));
+  TPC_CUDA(t, cudaStreamSynchronize(st));
+  const int64_t nt = out->counts[0] < out->track_capacity ? out->counts[0] : out->track_capacity;
+  const int64_t nh = out->counts[1] <= out->hit_capacity ? out->counts[1] : 0;
+  if (nt > 0)
+    TPC_CUDA(t, cudaMemcpyAsync(out->tracks, dout.tracks, (size_t)nt * sizeof(tpc_track_rec_t), cudaMemcpyDeviceToHost, st));
+  if (nh > 0) TPC_CUDA(t, cudaMemcpyAsync(out->hit_ids, dout.hit_ids, (size_t)nh * 4, cudaMemcpyDeviceToHost, st));
+  TPC_CUDA(t, cudaStreamSynchronize(st));
+  return TPC_OK;
+}
+
+int64_t tpc_scratch_bytes(const tpc_tracker_t* t) { return t ? (int64_t)(t->arena_bytes + t->host_arena_bytes) : 0; }
+
+int tpc_launches_per_call(const tpc_tracker_t* t) { return t ? 5 : 0; }
+
+int tpc_set_stage_timing(tpc_tracker_t* t, int enable) {
+  if (!t) return TPC_ERR_ARG;
+  t->timing = enable != 0;
+  return TPC_OK;
+}
+
+int tpc_get_stage_ms(tpc_tracker_t* t, float ms[5]) {
+  if (!t || !ms) return TPC_ERR_ARG;
+  TPC_CUDA(t, cudaEventSynchronize(t->ev[5]));
+  for (int k = 0; k < 5; ++k) TPC_CUDA(t, cudaEventElapsedTime(&ms[k], t->ev[k], t->ev[k + 1]));
+  return TPC_OK;
+}
+
+int tpc_debug_copy_links(tpc_tracker_t* t, int which, int32_t* up, int32_t* dn, void* stream) {
+  if (!t || !up || !dn || (which != 0 && which != 1)) return TPC_ERR_ARG;
+  if (!t->arena) return TPC_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (t->last_n == 0) return TPC_OK;
+  if (which == 0) {
+    TPC_CUDA(t, cudaMemcpyAsync(up, t->s.link_up, (size_t)t->last_n * 4, cudaMemcpyDeviceToDevice, st));
+    TPC_CUDA(t, cudaMemcpyAsync(dn, t->s.link_dn, (size_t)t->last_n * 4, cudaMemcpyDeviceToDevice, st));
+  } else {
+    TPC_CUDA(t, launch_dbg_clean(t, t->last_n, up, dn, st));
+  }
+  return TPC_OK;
+}
+
+int tpc_debug_copy_seeds(tpc_tracker_t* t, int32_t* start, int32_t* len, void* stream) {
+  if (!t || !start || !len || !t->arena) return TPC_ERR_ARG;
+  if (t->last_n == 0) return TPC_OK;
+  TPC_CUDA(t, launch_dbg_seed_len(t, start, len, (cudaStream_t)stream));
+  return TPC_OK;
+}
+
+int tpc_debug_copy_tracklets(tpc_tracker_t* t, float* par, float* cov, float* chi2, int32_t* n_hits, int32_t* hits,
+                             void* stream) {
+  if (!t || !t->arena) return TPC_ERR_ARG;
+  if (t->last_n == 0) return TPC_OK;
+  TPC_CUDA(t, launch_dbg_tracklets(t, par, cov, chi2, n_hits, hits, (cudaStream_t)stream));
+  return TPC_OK;
+}
+
+int tpc_debug_copy_owner(tpc_tracker_t* t, int32_t* owner, void* stream) {
+  if (!t || !owner || !t->arena) return TPC_ERR_ARG;
+  if (t->last_n == 0) return TPC_OK;
+  TPC_CUDA(t, launch_dbg_owner(t, t->last_n, owner, (cudaStream_t)stream));
+  return TPC_OK;
+}
+
+int tpc_debug_grid_info(const tpc_tracker_t* t, int32_t* bins_stride, int32_t* nz, int32_t* shift_y, int32_t* shift_z) {
+  if (!t) return TPC_ERR_ARG;
+  if (bins_stride) *bins_stride = t->g.nb_stride;
+  if (nz) *nz = t->g.nz;
+  if (shift_y) *shift_y = t->g.shift_y;
+  if (shift_z) *shift_z = t->g.shift_z;
+  return TPC_OK;
+}
+
+int tpc_debug_copy_grid(tpc_tracker_t* t, int32_t* ids_sorted, uint32_t* bin_start, void* stream) {
+  if (!t || !t->arena) return TPC_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
+  if (ids_sorted && t->last_n > 0)
+    TPC_CUDA(t, cudaMemcpyAsync(ids_sorted, t->s.ids, (size_t)t->last_n * 4, cudaMemcpyDeviceToDevice, st));
+  if (bin_start && R > 0)
+    TPC_CUDA(t, cudaMemcpyAsync(bin_start, t->s.bin_start, (size_t)R * t->g.nb_stride * 4, cudaMemcpyDeviceToDevice, st));
+  return TPC_OK;
+}
+
+#pragma GCC visibility pop
+}  // extern "C"

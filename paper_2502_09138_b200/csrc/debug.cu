@@ -1,0 +1,76 @@
+// debug.cu -- test-only exports of intermediate results (tpc_debug_* in include/tpc_track.h).
+// Not on the hot path: these kernels only re-shape what a1..a5 left in the handle's scratch so that the
+// parity tests can compare link tables, seeds and tracklets with the oracle element by element.
+#include "tpc_internal.cuh"
+
+namespace {
+
+__global__ void dbg_clean_kernel(int64_t n, const int32_t* __restrict__ up, const int32_t* __restrict__ dn,
+                                 int32_t* __restrict__ up_o, int32_t* __restrict__ dn_o) {
+  const int64_t h = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (h >= n) return;
+  const int u = up[h], d = dn[h];
+  up_o[h] = (u >= 0 && dn[u] == (int)h) ? u : -1;
+  dn_o[h] = (d >= 0 && up[d] == (int)h) ? d : -1;
+}
+
+__global__ void dbg_seed_len_kernel(const DevCtl* ctl, const int32_t* __restrict__ seed_start,
+                                    const int32_t* __restrict__ up_c, int32_t* __restrict__ start,
+                                    int32_t* __restrict__ len) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (int64_t)ctl->n_seeds) return;
+  const int h0 = seed_start[i];
+  int l = 1;
+  for (int c = up_c[h0]; c >= 0; c = up_c[c]) ++l;
+  start[i] = h0;
+  len[i] = l;
+}
+
+__global__ void dbg_tracklets_kernel(const DevCtl* ctl, int64_t s_cap, int n_rows, const float* __restrict__ tl_par,
+                                     const float* __restrict__ tl_cov, const float* __restrict__ tl_chi2,
+                                     const int32_t* __restrict__ tl_nhits, const int32_t* __restrict__ tl_hits,
+                                     float* par, float* cov, float* chi2, int32_t* n_hits, int32_t* hits) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (int64_t)ctl->n_seeds) return;
+  if (par)
+    for (int k = 0; k < 6; ++k) par[i * 6 + k] = tl_par[k * s_cap + i];
+  if (cov)
+    for (int k = 0; k < 15; ++k) cov[i * 15 + k] = tl_cov[k * s_cap + i];
+  if (chi2) chi2[i] = tl_chi2[i];
+  if (n_hits) n_hits[i] = tl_nhits[i];
+  if (hits)
+    for (int r = 0; r < n_rows; ++r) hits[i * n_rows + r] = tl_hits[(int64_t)r * s_cap + i];
+}
+
+__global__ void dbg_owner_kernel(int64_t n, const uint32_t* __restrict__ owner, int32_t* __restrict__ out) {
+  const int64_t h = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (h >= n) return;
+  const uint32_t w = owner[h];
+  out[h] = w ? (int32_t)(0xFFFFFFu - (w & 0xFFFFFFu)) : -1;
+}
+
+}  // namespace
+
+cudaError_t launch_dbg_clean(const tpc_tracker* t, int64_t n, int32_t* up, int32_t* dn, cudaStream_t st) {
+  if (n == 0) return cudaSuccess;
+  dbg_clean_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, t->s.link_up, t->s.link_dn, up, dn);
+  return cudaGetLastError();
+}
+cudaError_t launch_dbg_seed_len(const tpc_tracker* t, int32_t* start, int32_t* len, cudaStream_t st) {
+  if (t->s_cap == 0) return cudaSuccess;
+  dbg_seed_len_kernel<<<(unsigned)((t->s_cap + 255) / 256), 256, 0, st>>>(t->s.ctl, t->s.seed_start, t->s.up_c, start, len);
+  return cudaGetLastError();
+}
+cudaError_t launch_dbg_tracklets(const tpc_tracker* t, float* par, float* cov, float* chi2, int32_t* n_hits,
+                                 int32_t* hits, cudaStream_t st) {
+  if (t->s_cap == 0) return cudaSuccess;
+  dbg_tracklets_kernel<<<(unsigned)((t->s_cap + 127) / 128), 128, 0, st>>>(
+      t->s.ctl, t->s_cap, t->g.n_rows, t->s.tl_par, t->s.tl_cov, t->s.tl_chi2, t->s.tl_nhits, t->s.tl_hits, par, cov,
+      chi2, n_hits, hits);
+  return cudaGetLastError();
+}
+cudaError_t launch_dbg_owner(const tpc_tracker* t, int64_t n, int32_t* owner, cudaStream_t st) {
+  if (n == 0) return cudaSuccess;
+  dbg_owner_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, t->s.owner, owner);
+  return cudaGetLastError();
+}

@@ -1,0 +1,201 @@
+// tpc_internal.cuh -- shared declarations of the CUDA path (handle, device-side geometry, launchers).
+// Product code: shares nothing with oracle/.  Stage definitions: SURVEY.md 8(c) / DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/tpc_track.h"
+
+// Device view of geometry + parameters, passed by value to every kernel.
+struct DevGeom {
+  int32_t n_sectors, n_rows;
+  // a1 grid shape: bin = iz * ny_row[r] + iy, iy = (y - org.y) >> shift_y clamped to
+  // [0, ny-1], iz likewise with nz; org = per-row (min y, min z) of the data.
+  int32_t shift_y, shift_z, nz, nb_stride;
+  const int32_t* ny_row;   // [n_rows]
+  const double* row_x;     // [n_rows] cm
+  const float* row_dx;     // [n_rows] row_x[r+1] - row_x[r], rounded once from double (last entry repeats)
+  // a2 / a3
+  int32_t w_y, w_z, cost_wy, cost_wz, c_max, l_min;
+  // a4 / a5
+  int32_t max_miss, n_min_tracklet, n_min_owned;
+  float sy2, sz2, sinphi_max, gate_d, gate_y, gate_z, inv_units, units, cq;
+  float c_reset[5];
+  double inv_units_d;
+};
+
+// Counters living in device memory, zeroed at the start of every call.
+struct DevCtl {
+  uint32_t n_seeds;      // written by a3
+  uint32_t ticket_a3;    // dynamic tile ids for the a3 look-back scan
+  uint32_t ticket_a5;
+  uint32_t pad[13];
+};
+
+struct Scratch {
+  // a1
+  int32_t *ys, *zs, *ids;   // sorted (bin order inside each row) coordinates and cluster ids
+  int2* row_org;            // per (sector,row) grid origin
+  uint32_t* bin_start;      // [R * nb_stride] global sorted index of the first cluster of each bin (+ sentinel)
+  // a2 / a3 (id space)
+  int32_t *link_up, *link_dn, *up_c;
+  uint32_t* owner;          // packed (n_hits << 24 | 0xFFFFFF - rank), 0 = none
+  // a3 -> a4
+  int32_t* seed_start;      // [s_cap] start cluster id, ascending
+  // a4 tracklets, SoA over seeds
+  float* tl_par;            // [6][s_cap]  x_ref, y, z, sinphi, tanl, qpt
+  float* tl_cov;            // [15][s_cap]
+  float* tl_chi2;           // [s_cap]
+  int32_t* tl_nhits;        // [s_cap]
+  int32_t* tl_sr0;          // [s_cap] sector * n_rows + first row of the seed
+  int32_t* tl_hits;         // [n_rows][s_cap] cluster id or -1
+  // control
+  DevCtl* ctl;
+  uint64_t* scan_a3;        // look-back status words
+  uint64_t* scan_a5;        // two channels per tile
+  // host-buffer path staging
+  int32_t *st_y, *st_z; uint32_t* st_ro;
+  tpc_track_rec_t* st_tracks; int32_t* st_hits; int32_t* st_counts;
+};
+
+struct tpc_tracker {
+  int device;
+  DevGeom g;                 // device pointers inside point at geom_blob
+  void* geom_blob;
+  tpc_params_t params;
+  double bz;
+  // scratch arena
+  void* arena; size_t arena_bytes;
+  void* host_arena; size_t host_arena_bytes;   // staging for tpc_track_host
+  int64_t cap_n, cap_rows;   // sizes the arena was laid out for
+  int64_t s_cap;             // seed capacity of the current layout
+  int64_t tiles_a3, tiles_a5;
+  size_t ctl_bytes;          // bytes zeroed per call
+  Scratch s;
+  int64_t last_n; const uint32_t* last_ro; const int32_t* last_y; const int32_t* last_z;
+  // stage timing
+  int timing; cudaEvent_t ev[6];
+  cudaError_t last_err; char err_buf[256];
+};
+
+constexpr int A3_TILE = 1024;   // ids per a3 block (256 threads x 4)
+constexpr int A5_TILE = 128;    // tracklets per a5 block
+constexpr int A4_BLOCK = 64;
+
+// launchers (each in its own .cu)
+cudaError_t launch_a1_grid(const tpc_tracker* t, const int32_t* y, const int32_t* z, const uint32_t* ro, int64_t n, cudaStream_t st);
+cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64_t n, cudaStream_t st);
+cudaError_t launch_a3_seeds(const tpc_tracker* t, int64_t n, cudaStream_t st);
+cudaError_t launch_a4_follow(const tpc_tracker* t, const int32_t* y, const int32_t* z, const uint32_t* ro, int64_t n, cudaStream_t st);
+cudaError_t launch_a5_select(const tpc_tracker* t, const tpc_tracks_out_t* out, cudaStream_t st);
+cudaError_t setup_a1_attributes(const tpc_tracker* t);
+size_t a1_smem_bytes(const DevGeom& g);
+
+// debug.cu
+cudaError_t launch_dbg_clean(const tpc_tracker* t, int64_t n, int32_t* up, int32_t* dn, cudaStream_t st);
+cudaError_t launch_dbg_seed_len(const tpc_tracker* t, int32_t* start, int32_t* len, cudaStream_t st);
+cudaError_t launch_dbg_tracklets(const tpc_tracker* t, float* par, float* cov, float* chi2, int32_t* n_hits, int32_t* hits, cudaStream_t st);
+cudaError_t launch_dbg_owner(const tpc_tracker* t, int64_t n, int32_t* owner, cudaStream_t st);
+
+// ------------------------------------------------------------------------------------------------
+// Single-pass device-wide exclusive scan (decoupled look-back).  One 64-bit status word per tile and
+// channel: (state << 32) | value, state 0 = not ready, 1 = tile aggregate, 2 = inclusive prefix.
+// Tiles take their index from an atomic ticket so every predecessor is already running.
+// Called by all threads of the block; `tile_sum` must be valid in thread 0.  Returns the exclusive prefix
+// (sum over tiles < tile) to every thread through shared memory.
+// ------------------------------------------------------------------------------------------------
+template <int CH>
+__device__ __forceinline__ void lookback_scan(volatile uint64_t* status, uint32_t tile, const uint32_t (&tile_sum)[CH],
+                                              uint32_t (&excl)[CH], uint32_t* sh /* CH words of shared memory */) {
+  if (threadIdx.x < 32) {
+    const unsigned lane = threadIdx.x;
+    uint32_t sum[CH];
+#pragma unroll
+    for (int c = 0; c < CH; ++c) sum[c] = __shfl_sync(0xffffffffu, tile_sum[c], 0);
+    if (tile == 0) {
+      if (lane == 0) {
+#pragma unroll
+        for (int c = 0; c < CH; ++c) {
+          status[c] = (2ull << 32) | sum[c];
+          sh[c] = 0;
+        }
+      }
+    } else {
+      if (lane == 0) {
+#pragma unroll
+        for (int c = 0; c < CH; ++c) status[(size_t)tile * CH + c] = (1ull << 32) | sum[c];
+      }
+      uint32_t run[CH];
+#pragma unroll
+      for (int c = 0; c < CH; ++c) run[c] = 0;
+      int64_t base = (int64_t)tile - 1;   // window covers tiles base - lane
+      while (true) {
+        int64_t idx = base - lane;
+        uint64_t w[CH];
+        bool ready;
+        do {
+          ready = true;
+#pragma unroll
+          for (int c = 0; c < CH; ++c) {
+            w[c] = idx >= 0 ? status[(size_t)idx * CH + c] : (2ull << 32);
+            ready = ready && (w[c] >> 32) != 0;
+          }
+        } while (!__all_sync(0xffffffffu, ready));
+        // first lane (closest predecessor first) whose every channel holds an inclusive prefix
+        bool is_prefix = true;
+#pragma unroll
+        for (int c = 0; c < CH; ++c) is_prefix = is_prefix && (w[c] >> 32) == 2;
+        unsigned mask = __ballot_sync(0xffffffffu, is_prefix);
+        int stop = mask ? __ffs(mask) - 1 : 31;
+#pragma unroll
+        for (int c = 0; c < CH; ++c) {
+          uint32_t v = lane <= (unsigned)stop ? (uint32_t)w[c] : 0u;
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+          run[c] += v;
+        }
+        if (mask) break;
+        base -= 32;
+      }
+      if (lane == 0) {
+#pragma unroll
+        for (int c = 0; c < CH; ++c) {
+          status[(size_t)tile * CH + c] = (2ull << 32) | (uint32_t)(run[c] + sum[c]);
+          sh[c] = run[c];
+        }
+      }
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int c = 0; c < CH; ++c) excl[c] = sh[c];
+}
+
+// Block-wide exclusive scan of one uint32 per thread (blockDim.x multiple of 32, <= 1024).
+// Returns the exclusive prefix; *total (same in all threads) is the block sum.  `wsum` = 33 words of smem.
+__device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t* wsum, uint32_t* total) {
+  const unsigned lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  uint32_t inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= (unsigned)o) inc += t;
+  }
+  __syncthreads();   // protect wsum reuse
+  if (lane == 31) wsum[wid] = inc;
+  __syncthreads();
+  if (wid == 0) {
+    uint32_t s = lane < nw ? wsum[lane] : 0u;
+    uint32_t si = s;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      uint32_t t = __shfl_up_sync(0xffffffffu, si, o);
+      if (lane >= (unsigned)o) si += t;
+    }
+    wsum[lane] = si - s;            // exclusive warp offsets
+    if (lane == 31) wsum[32] = si;  // block total
+  }
+  __syncthreads();
+  *total = wsum[32];
+  return wsum[wid] + inc - v;
+}
