@@ -18,7 +18,8 @@ a3_seeds_kernel(const DevGeom g, int64_t n, const int32_t* __restrict__ up, cons
                 int32_t* __restrict__ up_c, int32_t* __restrict__ seed_start, DevCtl* __restrict__ ctl,
                 uint64_t* __restrict__ status, uint32_t n_tiles) {
   __shared__ uint32_t wsum[33];
-  __shared__ uint32_t sh_tile, sh_excl[1];
+  __shared__ uint32_t sh_tile;
+  __shared__ uint64_t sh_excl;
   if (threadIdx.x == 0) sh_tile = atomicAdd(&ctl->ticket_a3, 1u);
   __syncthreads();
   const uint32_t tile = sh_tile;
@@ -51,12 +52,11 @@ a3_seeds_kernel(const DevGeom g, int64_t n, const int32_t* __restrict__ up, cons
     pos[k] = running + block_excl_scan(seed[k] ? 1u : 0u, wsum, &tot);
     running += tot;
   }
-  uint32_t tsum[1] = {running}, excl[1];
-  lookback_scan<1>(status, tile, tsum, excl, sh_excl);
+  const uint32_t excl = (uint32_t)lookback_scan(status, tile, running, &sh_excl);
 #pragma unroll
   for (int k = 0; k < A3_ITEMS; ++k)
-    if (seed[k]) seed_start[excl[0] + pos[k]] = (int32_t)(base + k * A3_THREADS + threadIdx.x);
-  if (tile == n_tiles - 1 && threadIdx.x == 0) ctl->n_seeds = excl[0] + running;
+    if (seed[k]) seed_start[excl + pos[k]] = (int32_t)(base + k * A3_THREADS + threadIdx.x);
+  if (tile == n_tiles - 1 && threadIdx.x == 0) ctl->n_seeds = excl + running;
 }
 
 }  // namespace

@@ -13,12 +13,26 @@
 
 namespace {
 
+// Precision: state in fp32, covariance and gain in fp64.  With an fp32 covariance
+// 0.6 % (config 1) to 1.3 % (config 4) of the tracklets miss the 1e-4 bar on q/pT (cancellation in C - K H C
+// after the P22 reset); with the covariance in fp64 none does (measured: profiles/r01_a4_precision.md).
+#ifdef TPC_A4_COV32
+typedef float creal;
+#else
+typedef double creal;
+#endif
+#ifdef TPC_A4_STATE64
+typedef double sreal;
+#else
+typedef float sreal;
+#endif
+
 struct Cov {   // symmetric 5x5, lower triangle
-  float c00, c10, c11, c20, c21, c22, c30, c31, c32, c33, c40, c41, c42, c43, c44;
+  creal c00, c10, c11, c20, c21, c22, c30, c31, c32, c33, c40, c41, c42, c43, c44;
 };
 
 struct State {
-  float y, z, s, t, q;   // relative y, relative z, sin phi, tan lambda, q/pT
+  sreal y, z, s, t, q;   // relative y, relative z, sin phi, tan lambda, q/pT
 };
 
 __device__ __forceinline__ void cov_reset(const DevGeom& g, Cov& C) {
@@ -30,58 +44,61 @@ __device__ __forceinline__ void cov_reset(const DevGeom& g, Cov& C) {
 // iff |sin phi| >= sinphi_max before or after (P18).  WITH_COV: C <- F C F^T with
 // F = I + [02]=a [04]=b [12]=c [13]=d [14]=e [24]=f.
 template <bool WITH_COV>
-__device__ __forceinline__ bool transport(const DevGeom& g, float dx, State& p, Cov& C) {
-  const float k = g.cq * p.q;
-  const float s0 = p.s;
-  const float s1 = fmaf(k, dx, s0);
-  if (!(fabsf(s0) < g.sinphi_max) || !(fabsf(s1) < g.sinphi_max)) return false;
-  const float c0 = sqrtf(fmaf(-s0, s0, 1.f)), c1 = sqrtf(fmaf(-s1, s1, 1.f));
-  const float tau = (s0 + s1) / (c0 + c1);
-  const float dy = dx * tau;
-  const float chord = copysignf(sqrtf(fmaf(dx, dx, dy * dy)), dx);
-  const float u = 0.5f * k * chord;
-  const float u2 = u * u;
-  // asin(u)/u = 1 + u^2/6 + 3u^4/40 + 15u^6/336 + 105 u^8/3456 ...
-  const float dS = (u2 < 0.01f) ? chord * fmaf(u2, fmaf(u2, fmaf(u2, fmaf(u2, 0.030381944f, 0.044642857f), 0.075f),
-                                                        0.16666667f), 1.f)
-                                : chord * asinf(u) / u;
+__device__ __forceinline__ bool transport(const DevGeom& g, float dxf, State& p, Cov& C) {
+  const sreal dx = dxf;
+  const sreal cq = g.cq;
+  const sreal k = cq * p.q;
+  const sreal s0 = p.s;
+  const sreal s1 = fma(k, dx, s0);
+  if (!(fabs(s0) < (sreal)g.sinphi_max) || !(fabs(s1) < (sreal)g.sinphi_max)) return false;
+  const sreal c0 = sqrt(fma(-s0, s0, (sreal)1)), c1 = sqrt(fma(-s1, s1, (sreal)1));
+  const sreal tau = (s0 + s1) / (c0 + c1);
+  const sreal dy = dx * tau;
+  const sreal chord = copysign(sqrt(fma(dx, dx, dy * dy)), dx);
+  const sreal u = (sreal)0.5 * k * chord;
+  const sreal u2 = u * u;
+  // asin(u)/u = 1 + u^2/6 + 3u^4/40 + 15u^6/336 + 105 u^8/3456 + 945 u^10/42240 ...
+  const sreal dS = (u2 < (sreal)0.01)
+      ? chord * fma(u2, fma(u2, fma(u2, fma(u2, fma(u2, (sreal)0.022372159, (sreal)0.030381944), (sreal)0.044642857),
+                                   (sreal)0.075), (sreal)0.16666666666666666), (sreal)1)
+      : chord * asin(u) / u;
   if (WITH_COV) {
-    const float m = fmaf(s0, tau, c0);
-    const float ic0c1 = 1.f / (c0 * c1);
-    const float d_ = 0.5f * k * dS;
-    const float d2 = d_ * d_;
-    float sinc, gg;
-    if (d2 < 0.01f) {
-      sinc = fmaf(d2, fmaf(d2, 1.f / 120.f, -1.f / 6.f), 1.f);
-      gg = fmaf(d2, fmaf(d2, 1.f / 840.f, -1.f / 30.f), 1.f / 3.f);
+    const sreal m = fma(s0, tau, c0);
+    const sreal ic0c1 = (sreal)1 / (c0 * c1);
+    const sreal d_ = (sreal)0.5 * k * dS;
+    const sreal d2 = d_ * d_;
+    sreal sinc, gg;
+    if (d2 < (sreal)0.01) {
+      sinc = fma(d2, fma(d2, fma(d2, (sreal)(-1.0 / 5040.0), (sreal)(1.0 / 120.0)), (sreal)(-1.0 / 6.0)), (sreal)1);
+      gg = fma(d2, fma(d2, fma(d2, (sreal)(-1.0 / 45360.0), (sreal)(1.0 / 840.0)), (sreal)(-1.0 / 30.0)), (sreal)(1.0 / 3.0));
     } else {
-      float sn, cs;
-      sincosf(d_, &sn, &cs);
+      sreal sn, cs;
+      sincos(d_, &sn, &cs);
       sinc = sn / d_;
       gg = (sn - d_ * cs) / (d_ * d2);
     }
-    const float cm = rsqrtf(fmaf(tau, tau, 1.f)), sm = tau * cm;
-    const float dSdk = (0.5f * dS * dS * sm * sinc + 0.25f * k * dS * dS * dS * cm * gg) / c1;
-    const float a = dx * m * ic0c1;                        // dy1/ds
-    const float b = g.cq * dx * dx * m / (c1 * (c0 + c1)); // dy1/dq
-    const float c = p.t * dy * ic0c1;                      // dz1/ds
-    const float d = dS;                                    // dz1/dt
-    const float e = p.t * g.cq * dSdk;                     // dz1/dq
-    const float f = g.cq * dx;                             // ds1/dq
+    const sreal cm = rsqrt(fma(tau, tau, (sreal)1)), sm = tau * cm;
+    const sreal dSdk = ((sreal)0.5 * dS * dS * sm * sinc + (sreal)0.25 * k * dS * dS * dS * cm * gg) / c1;
+    const creal a = dx * m * ic0c1;                     // dy1/ds
+    const creal b = cq * dx * dx * m / (c1 * (c0 + c1)); // dy1/dq
+    const creal c = p.t * dy * ic0c1;                   // dz1/ds
+    const creal d = dS;                                 // dz1/dt
+    const creal e = p.t * cq * dSdk;                    // dz1/dq
+    const creal f = cq * dx;                            // ds1/dq
     // M = F C (rows 0..2 change), then C' = M F^T
-    const float m00 = C.c00 + a * C.c20 + b * C.c40;
-    const float m02 = C.c20 + a * C.c22 + b * C.c42;
-    const float m04 = C.c40 + a * C.c42 + b * C.c44;
-    const float m10 = C.c10 + c * C.c20 + d * C.c30 + e * C.c40;
-    const float m11 = C.c11 + c * C.c21 + d * C.c31 + e * C.c41;
-    const float m12 = C.c21 + c * C.c22 + d * C.c32 + e * C.c42;
-    const float m13 = C.c31 + c * C.c32 + d * C.c33 + e * C.c43;
-    const float m14 = C.c41 + c * C.c42 + d * C.c43 + e * C.c44;
-    const float m20 = C.c20 + f * C.c40;
-    const float m21 = C.c21 + f * C.c41;
-    const float m22 = C.c22 + f * C.c42;
-    const float m23 = C.c32 + f * C.c43;
-    const float m24 = C.c42 + f * C.c44;
+    const creal m00 = C.c00 + a * C.c20 + b * C.c40;
+    const creal m02 = C.c20 + a * C.c22 + b * C.c42;
+    const creal m04 = C.c40 + a * C.c42 + b * C.c44;
+    const creal m10 = C.c10 + c * C.c20 + d * C.c30 + e * C.c40;
+    const creal m11 = C.c11 + c * C.c21 + d * C.c31 + e * C.c41;
+    const creal m12 = C.c21 + c * C.c22 + d * C.c32 + e * C.c42;
+    const creal m13 = C.c31 + c * C.c32 + d * C.c33 + e * C.c43;
+    const creal m14 = C.c41 + c * C.c42 + d * C.c43 + e * C.c44;
+    const creal m20 = C.c20 + f * C.c40;
+    const creal m21 = C.c21 + f * C.c41;
+    const creal m22 = C.c22 + f * C.c42;
+    const creal m23 = C.c32 + f * C.c43;
+    const creal m24 = C.c42 + f * C.c44;
     Cov N;
     N.c00 = m00 + a * m02 + b * m04;
     N.c10 = m10 + a * m12 + b * m14;
@@ -101,28 +118,28 @@ __device__ __forceinline__ bool transport(const DevGeom& g, float dx, State& p, 
     C = N;
   }
   p.y += dy;
-  p.z = fmaf(p.t, dS, p.z);
+  p.z = fma(p.t, dS, p.z);
   p.s = s1;
   return true;
 }
 
 // Appendix C update with H = [I2 | 0], V = diag(sy2, sz2).  Returns the chi2 increment.
 __device__ __forceinline__ float update(const DevGeom& g, State& p, Cov& C, float ym, float zm) {
-  const float S00 = C.c00 + g.sy2, S01 = C.c10, S11 = C.c11 + g.sz2;
-  const float idet = 1.f / (S00 * S11 - S01 * S01);
-  const float I00 = S11 * idet, I01 = -S01 * idet, I11 = S00 * idet;
-  const float r0 = ym - p.y, r1 = zm - p.z;
+  const creal S00 = C.c00 + (creal)g.sy2, S01 = C.c10, S11 = C.c11 + (creal)g.sz2;
+  const creal idet = (creal)1 / (S00 * S11 - S01 * S01);
+  const creal I00 = S11 * idet, I01 = -S01 * idet, I11 = S00 * idet;
+  const creal r0 = (sreal)ym - p.y, r1 = (sreal)zm - p.z;
   // K = C[:,0:2] S^-1
-  const float k00 = C.c00 * I00 + C.c10 * I01, k01 = C.c00 * I01 + C.c10 * I11;
-  const float k10 = C.c10 * I00 + C.c11 * I01, k11 = C.c10 * I01 + C.c11 * I11;
-  const float k20 = C.c20 * I00 + C.c21 * I01, k21 = C.c20 * I01 + C.c21 * I11;
-  const float k30 = C.c30 * I00 + C.c31 * I01, k31 = C.c30 * I01 + C.c31 * I11;
-  const float k40 = C.c40 * I00 + C.c41 * I01, k41 = C.c40 * I01 + C.c41 * I11;
-  p.y += k00 * r0 + k01 * r1;
-  p.z += k10 * r0 + k11 * r1;
-  p.s += k20 * r0 + k21 * r1;
-  p.t += k30 * r0 + k31 * r1;
-  p.q += k40 * r0 + k41 * r1;
+  const creal k00 = C.c00 * I00 + C.c10 * I01, k01 = C.c00 * I01 + C.c10 * I11;
+  const creal k10 = C.c10 * I00 + C.c11 * I01, k11 = C.c10 * I01 + C.c11 * I11;
+  const creal k20 = C.c20 * I00 + C.c21 * I01, k21 = C.c20 * I01 + C.c21 * I11;
+  const creal k30 = C.c30 * I00 + C.c31 * I01, k31 = C.c30 * I01 + C.c31 * I11;
+  const creal k40 = C.c40 * I00 + C.c41 * I01, k41 = C.c40 * I01 + C.c41 * I11;
+  p.y += (sreal)(k00 * r0 + k01 * r1);
+  p.z += (sreal)(k10 * r0 + k11 * r1);
+  p.s += (sreal)(k20 * r0 + k21 * r1);
+  p.t += (sreal)(k30 * r0 + k31 * r1);
+  p.q += (sreal)(k40 * r0 + k41 * r1);
   // C <- C - K (H C), lower triangle: C_ij -= K_i0 C_0j + K_i1 C_1j
   Cov N;
   N.c00 = C.c00 - (k00 * C.c00 + k01 * C.c10);
@@ -141,7 +158,7 @@ __device__ __forceinline__ float update(const DevGeom& g, State& p, Cov& C, floa
   N.c43 = C.c43 - (k40 * C.c30 + k41 * C.c31);
   N.c44 = C.c44 - (k40 * C.c40 + k41 * C.c41);
   C = N;
-  return r0 * (I00 * r0 + I01 * r1) + r1 * (I01 * r0 + I11 * r1);
+  return (float)(r0 * (I00 * r0 + I01 * r1) + r1 * (I01 * r0 + I11 * r1));
 }
 
 __device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
@@ -165,21 +182,22 @@ __device__ __forceinline__ Found search_row(const DevGeom& g, int sr, int row, c
   const uint32_t* bs = bin_start + (size_t)sr * g.nb_stride;
   // integer superset of the float window (+-1 unit of slack on each side), clamped against overflow
   const float lim = 1.0e9f;
-  const int ylo = y0 + (int)fminf(fmaxf(floorf((p.y - g.gate_y) * g.units) - 1.f, -lim), lim);
-  const int yhi = y0 + (int)fminf(fmaxf(ceilf((p.y + g.gate_y) * g.units) + 1.f, -lim), lim);
-  const int zlo = z0 + (int)fminf(fmaxf(floorf((p.z - g.gate_z) * g.units) - 1.f, -lim), lim);
-  const int zhi = z0 + (int)fminf(fmaxf(ceilf((p.z + g.gate_z) * g.units) + 1.f, -lim), lim);
+  const float py = (float)p.y, pz = (float)p.z;
+  const int ylo = y0 + (int)fminf(fmaxf(floorf((py - g.gate_y) * g.units) - 1.f, -lim), lim);
+  const int yhi = y0 + (int)fminf(fmaxf(ceilf((py + g.gate_y) * g.units) + 1.f, -lim), lim);
+  const int zlo = z0 + (int)fminf(fmaxf(floorf((pz - g.gate_z) * g.units) - 1.f, -lim), lim);
+  const int zhi = z0 + (int)fminf(fmaxf(ceilf((pz + g.gate_z) * g.units) + 1.f, -lim), lim);
   const int iy_lo = clampi((ylo - org.x) >> g.shift_y, 0, ny - 1);
   const int iy_hi = clampi((yhi - org.x) >> g.shift_y, 0, ny - 1);
   const int iz_lo = clampi((zlo - org.y) >> g.shift_z, 0, g.nz - 1);
   const int iz_hi = clampi((zhi - org.y) >> g.shift_z, 0, g.nz - 1);
-  const float wy = 1.f / (C.c00 + g.sy2), wz = 1.f / (C.c11 + g.sz2);
+  const float wy = 1.f / ((float)C.c00 + g.sy2), wz = 1.f / ((float)C.c11 + g.sz2);
   float bestd = __int_as_float(0x7f800000);
   for (int iz = iz_lo; iz <= iz_hi; ++iz) {
     const uint32_t a = bs[iz * ny + iy_lo], b = bs[iz * ny + iy_hi + 1];
     for (uint32_t j = a; j < b; ++j) {
       const float cy = (float)(ys[j] - y0) * g.inv_units, cz = (float)(zs[j] - z0) * g.inv_units;
-      const float dy = cy - p.y, dz = cz - p.z;
+      const float dy = cy - py, dz = cz - pz;
       if (fabsf(dy) > g.gate_y || fabsf(dz) > g.gate_z) continue;
       const float d = dy * dy * wy + dz * dz * wz;
       if (d > bestd) continue;
@@ -227,7 +245,7 @@ a4_follow_kernel(const DevGeom g, int64_t s_cap, const DevCtl* __restrict__ ctl,
     const float dxr = g.row_dx[r0];
     const float dy = (float)(y[h] - y0) * g.inv_units, dz = (float)(z[h] - z0) * g.inv_units;
     const float ichord = rsqrtf(fmaf(dxr, dxr, dy * dy));
-    p.y = 0.f; p.z = 0.f; p.s = dy * ichord; p.t = dz * ichord; p.q = 0.f;
+    p.y = 0; p.z = 0; p.s = dy * ichord; p.t = dz * ichord; p.q = 0;
   }
   cov_reset(g, C);
   update(g, p, C, 0.f, 0.f);
@@ -305,11 +323,12 @@ a4_follow_kernel(const DevGeom g, int64_t s_cap, const DevCtl* __restrict__ ctl,
   tl_par[0 * s_cap + i] = (float)g.row_x[xrow];
   tl_par[1 * s_cap + i] = (float)((double)p.y + (double)y0 * g.inv_units_d);
   tl_par[2 * s_cap + i] = (float)((double)p.z + (double)z0 * g.inv_units_d);
-  tl_par[3 * s_cap + i] = p.s;
-  tl_par[4 * s_cap + i] = p.t;
-  tl_par[5 * s_cap + i] = p.q;
-  const float cv[15] = {C.c00, C.c10, C.c11, C.c20, C.c21, C.c22, C.c30, C.c31, C.c32, C.c33,
-                        C.c40, C.c41, C.c42, C.c43, C.c44};
+  tl_par[3 * s_cap + i] = (float)p.s;
+  tl_par[4 * s_cap + i] = (float)p.t;
+  tl_par[5 * s_cap + i] = (float)p.q;
+  const float cv[15] = {(float)C.c00, (float)C.c10, (float)C.c11, (float)C.c20, (float)C.c21, (float)C.c22, (float)C.c30,
+                        (float)C.c31, (float)C.c32, (float)C.c33, (float)C.c40, (float)C.c41, (float)C.c42, (float)C.c43,
+                        (float)C.c44};
 #pragma unroll
   for (int k = 0; k < 15; ++k) tl_cov[k * s_cap + i] = cv[k];
   tl_chi2[i] = chi2;

@@ -17,7 +17,8 @@ a5_select_kernel(const DevGeom g, int64_t s_cap, DevCtl* __restrict__ ctl, const
                  uint64_t* __restrict__ status, tpc_track_rec_t* __restrict__ tracks, int32_t track_capacity,
                  int32_t* __restrict__ hit_ids, int32_t hit_capacity, int32_t* __restrict__ counts) {
   __shared__ uint32_t wsum[33];
-  __shared__ uint32_t sh_tile, sh_excl[2];
+  __shared__ uint32_t sh_tile;
+  __shared__ uint64_t sh_excl;
   const uint32_t n_seeds = ctl->n_seeds;
   const uint32_t n_tiles = (n_seeds + A5_TILE - 1) / A5_TILE;
   if (n_seeds == 0) {
@@ -58,8 +59,9 @@ a5_select_kernel(const DevGeom g, int64_t s_cap, DevCtl* __restrict__ ctl, const
   uint32_t tot_k, tot_h;
   const uint32_t pos_k = block_excl_scan(keep ? 1u : 0u, wsum, &tot_k);
   const uint32_t pos_h = block_excl_scan(owned, wsum, &tot_h);
-  uint32_t tsum[2] = {tot_k, tot_h}, excl[2];
-  lookback_scan<2>(status, tile, tsum, excl, sh_excl);
+  // payload: tracks in bits 61..38 (s_cap < 2^24), hits in bits 37..0 (n < 2^31)
+  const uint64_t ex = lookback_scan(status, tile, ((uint64_t)tot_k << 38) | tot_h, &sh_excl);
+  const uint32_t excl[2] = {(uint32_t)(ex >> 38), (uint32_t)(ex & ((1ull << 38) - 1))};
 
   if (keep) {
     const uint32_t slot = excl[0] + pos_k;

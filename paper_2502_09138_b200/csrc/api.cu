@@ -46,7 +46,7 @@ size_t layout(tpc_tracker* t, char* base, int64_t n, int64_t R) {
   // zeroed per call: ctl + look-back status words (kept contiguous, first in the arena)
   s.ctl = (DevCtl*)take(sizeof(DevCtl));
   s.scan_a3 = (uint64_t*)take((size_t)tiles_a3 * 8);
-  s.scan_a5 = (uint64_t*)take((size_t)tiles_a5 * 16);
+  s.scan_a5 = (uint64_t*)take((size_t)tiles_a5 * 8);
   const size_t ctl_bytes = off;
   s.ys = (int32_t*)take((size_t)n * 4 + 64);
   s.zs = (int32_t*)take((size_t)n * 4 + 64);

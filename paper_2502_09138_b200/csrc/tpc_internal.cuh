@@ -98,77 +98,54 @@ cudaError_t launch_dbg_tracklets(const tpc_tracker* t, float* par, float* cov, f
 cudaError_t launch_dbg_owner(const tpc_tracker* t, int64_t n, int32_t* owner, cudaStream_t st);
 
 // ------------------------------------------------------------------------------------------------
-// Single-pass device-wide exclusive scan (decoupled look-back).  One 64-bit status word per tile and
-// channel: (state << 32) | value, state 0 = not ready, 1 = tile aggregate, 2 = inclusive prefix.
-// Tiles take their index from an atomic ticket so every predecessor is already running.
+// Single-pass device-wide exclusive scan (decoupled look-back).  One 64-bit status word per tile:
+// bits 63..62 = state (0 not ready, 1 tile aggregate, 2 inclusive prefix), bits 61..0 = payload, so state and
+// value always change together.  The payload may pack several counters in disjoint bit fields as long as no
+// field can overflow into the next (a5 packs tracks and hits).  Tiles take their index from an atomic ticket,
+// so every predecessor of a tile is already running.
 // Called by all threads of the block; `tile_sum` must be valid in thread 0.  Returns the exclusive prefix
 // (sum over tiles < tile) to every thread through shared memory.
 // ------------------------------------------------------------------------------------------------
-template <int CH>
-__device__ __forceinline__ void lookback_scan(volatile uint64_t* status, uint32_t tile, const uint32_t (&tile_sum)[CH],
-                                              uint32_t (&excl)[CH], uint32_t* sh /* CH words of shared memory */) {
+constexpr uint64_t LB_PAYLOAD = (1ull << 62) - 1;
+
+__device__ __forceinline__ uint64_t lookback_scan(volatile uint64_t* status, uint32_t tile, uint64_t tile_sum,
+                                                  uint64_t* sh /* one word of shared memory */) {
   if (threadIdx.x < 32) {
     const unsigned lane = threadIdx.x;
-    uint32_t sum[CH];
-#pragma unroll
-    for (int c = 0; c < CH; ++c) sum[c] = __shfl_sync(0xffffffffu, tile_sum[c], 0);
+    const uint64_t sum = __shfl_sync(0xffffffffu, tile_sum, 0);
     if (tile == 0) {
       if (lane == 0) {
-#pragma unroll
-        for (int c = 0; c < CH; ++c) {
-          status[c] = (2ull << 32) | sum[c];
-          sh[c] = 0;
-        }
+        status[0] = (2ull << 62) | sum;
+        *sh = 0;
       }
     } else {
-      if (lane == 0) {
-#pragma unroll
-        for (int c = 0; c < CH; ++c) status[(size_t)tile * CH + c] = (1ull << 32) | sum[c];
-      }
-      uint32_t run[CH];
-#pragma unroll
-      for (int c = 0; c < CH; ++c) run[c] = 0;
-      int64_t base = (int64_t)tile - 1;   // window covers tiles base - lane
+      if (lane == 0) status[tile] = (1ull << 62) | sum;
+      uint64_t run = 0;
+      int64_t base = (int64_t)tile - 1;   // lane l looks at tile base - l
       while (true) {
-        int64_t idx = base - lane;
-        uint64_t w[CH];
-        bool ready;
+        const int64_t idx = base - lane;
+        uint64_t w;
         do {
-          ready = true;
+          w = idx >= 0 ? status[idx] : (2ull << 62);
+        } while (!__all_sync(0xffffffffu, (w >> 62) != 0));
+        // nearest predecessor that already holds an inclusive prefix ends the walk
+        const unsigned mask = __ballot_sync(0xffffffffu, (w >> 62) == 2);
+        const int stop = mask ? __ffs(mask) - 1 : 31;
+        uint64_t v = lane <= (unsigned)stop ? (w & LB_PAYLOAD) : 0ull;
 #pragma unroll
-          for (int c = 0; c < CH; ++c) {
-            w[c] = idx >= 0 ? status[(size_t)idx * CH + c] : (2ull << 32);
-            ready = ready && (w[c] >> 32) != 0;
-          }
-        } while (!__all_sync(0xffffffffu, ready));
-        // first lane (closest predecessor first) whose every channel holds an inclusive prefix
-        bool is_prefix = true;
-#pragma unroll
-        for (int c = 0; c < CH; ++c) is_prefix = is_prefix && (w[c] >> 32) == 2;
-        unsigned mask = __ballot_sync(0xffffffffu, is_prefix);
-        int stop = mask ? __ffs(mask) - 1 : 31;
-#pragma unroll
-        for (int c = 0; c < CH; ++c) {
-          uint32_t v = lane <= (unsigned)stop ? (uint32_t)w[c] : 0u;
-#pragma unroll
-          for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-          run[c] += v;
-        }
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        run += v;
         if (mask) break;
         base -= 32;
       }
       if (lane == 0) {
-#pragma unroll
-        for (int c = 0; c < CH; ++c) {
-          status[(size_t)tile * CH + c] = (2ull << 32) | (uint32_t)(run[c] + sum[c]);
-          sh[c] = run[c];
-        }
+        status[tile] = (2ull << 62) | (run + sum);
+        *sh = run;
       }
     }
   }
   __syncthreads();
-#pragma unroll
-  for (int c = 0; c < CH; ++c) excl[c] = sh[c];
+  return *sh;
 }
 
 // Block-wide exclusive scan of one uint32 per thread (blockDim.x multiple of 32, <= 1024).
