@@ -1,0 +1,359 @@
+"""bench.py -- clusters tracked per second on B200 for BASELINE.json configs[1] (central Pb-Pb).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--batch-events B] [--impl ours|reference]
+
+One "step" = one tpc_track call = one pass of the whole hot path (a1 grid, a2 neighbours, a3 cleaner/seeds,
+a4 follower, a5 ownership/selection) over a batch of B distinct synthetic central Pb-Pb events, concatenated as
+B*36 independent sectors.  Prints ONE JSON line (rank 0).
+
+  value        clusters/s over all ranks, inputs resident in HBM, CUDA events on the launching stream
+  e2e          the same metric through tpc_track_host: pinned HOST buffers in, host buffers out, copies timed
+  roofline     the dominant kernel (a4 follower): algorithmic work / its mean launch duration, measured with
+               CUDA events recorded between the stages inside the timed region; plus roofline_path (whole step
+               against the HBM roofline, the figure BASELINE.json's metric names) and per-stage times
+  cpu_baseline the oracle (oracle/, fp64, OpenMP) timed on this box's host cores on a bounded sample
+
+--impl reference times the oracle itself (there is no reference implementation to install; the paper has no
+code), one bounded sample per step, rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "TPC clusters tracked/sec on 1 B200 (central Pb-Pb); % of HBM roofline"
+UNIT = "clusters/s"
+CFG_ID = 1
+# algorithmic work per unit: N clusters, N_b grid bins, T tracklet-hits, S seeds
+FLOP_PER_TRACKLET_HIT = 580.0      # a4: (transport + Jacobian + covariance transport + update) x 2 passes
+
+
+def stage_bytes(n, n_bins, t_hits, seeds):
+    """Algorithmic bytes per stage."""
+    return {
+        "a1": 20.0 * n + 4.0 * n_bins,
+        "a2": 20.0 * n + 4.0 * n_bins,
+        "a3": 24.0 * n + 8.0 * seeds,
+        "a4": 16.0 * t_hits + 100.0 * seeds,
+        "a5": 20.0 * t_hits,
+    }
+
+
+def read_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured", float(d.get("sm_max_mhz", 1965.0))
+    return 6650.0, "fallback", 1965.0
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.02):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        self._period = period_s
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nv = None
+
+    def _loop(self):
+        nv = self._nv
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
+                 "hw_power_brake_slowdown": 0x80, "applications_clocks_setting": 0x2, "sync_boost": 0x10}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self._h))
+                except Exception:
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(self._period)
+
+    def __enter__(self):
+        if self._nv is not None:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"], "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def shard_seeds(rank: int, world: int, batch_events: int) -> list[int]:
+    """Weak scaling: every rank tracks its own `batch_events` distinct events; seeds never repeat across ranks."""
+    return [1000 * CFG_ID + rank * batch_events + k for k in range(batch_events)]
+
+
+def aggregate(local_ms: float, local_units: float, dist=None, device=None):
+    """(max elapsed ms over ranks, total units over ranks).  Works on gloo (CPU tensors) and nccl."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return local_ms, local_units
+    import torch
+    t = torch.tensor([local_ms], dtype=torch.float64, device=device)
+    u = torch.tensor([local_units], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def make_batch(seeds, n_tracks=None):
+    from gen.events import make_event, concat_events
+    evs = [make_event(CFG_ID, s, n_tracks=n_tracks) for s in seeds]
+    return concat_events(evs), evs
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2502_09138_b200 import Tracker, load_library
+    from paper_2502_09138_b200.events import geometry_from_event, upload
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU path")
+    load_library()   # fails loudly if libtpctrack.so is missing
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    B = args.batch_events
+    ev, evs = make_batch(shard_seeds(rank, world, B))
+    n = ev.n
+    trk = Tracker(geometry_from_event(ev))
+    y, z, ro = upload(ev, dev)
+    out = trk.alloc_out(n, track_capacity=n // 40 + 1024, hit_capacity=n + 1024)
+    stream = torch.cuda.current_stream()
+
+    # ---- device-resident arm -----------------------------------------------------------------------------
+    for _ in range(args.warmup):
+        trk.track(y, z, ro, out, stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    trk.set_stage_timing(True)   # CUDA events between the stages, recorded on the launching stream
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clk:
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for _ in range(args.steps):
+            trk.track(y, z, ro, out, stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms_total = e0.elapsed_time(e1)
+    stage_ms, n_avg = trk.stage_ms_mean()
+    trk.set_stage_timing(False)
+    ms_max, units = aggregate(ms_total, float(n) * args.steps, dist if world > 1 else None, dev)
+    value = units / (ms_max * 1e-3)
+
+    tracks, hit_ids, n_seeds = out.to_host()
+    _, _, _, tl_nh, _ = trk.debug_tracklets(n_seeds)
+    t_hits = float(tl_nh.sum())
+    grid = trk.debug_grid(n)
+    n_bins = float(grid["stride"]) * trk.n_sectors * trk.n_rows
+
+    # ---- single-event latency (B = 1), for context -------------------------------------------------------
+    ev1 = evs[0]
+    trk1 = Tracker(geometry_from_event(ev1))
+    y1, z1, ro1 = upload(ev1, dev)
+    out1 = trk1.alloc_out(ev1.n)
+    for _ in range(3):
+        trk1.track(y1, z1, ro1, out1, stream)
+    torch.cuda.synchronize()
+    l0, l1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0.record(stream)
+    for _ in range(10):
+        trk1.track(y1, z1, ro1, out1, stream)
+    l1.record(stream)
+    torch.cuda.synchronize()
+    latency_ms = l0.elapsed_time(l1) / 10
+    trk1.close()
+
+    # ---- end to end through the host-buffer entry point --------------------------------------------------
+    hy = torch.from_numpy(ev.y.copy()).pin_memory()
+    hz = torch.from_numpy(ev.z.copy()).pin_memory()
+    hro = torch.from_numpy(ev.row_offsets.view(np.int32).copy()).pin_memory()
+    htr = torch.empty(out.tracks.shape[0], dtype=torch.uint8).pin_memory()
+    hhi = torch.empty(out.hit_ids.shape[0], dtype=torch.int32).pin_memory()
+    hcn = torch.zeros(4, dtype=torch.int32).pin_memory()
+    e2e_steps = max(3, min(args.steps, 20))
+    for _ in range(2):
+        trk.track_host(hy, hz, hro, htr, hhi, hcn, stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        trk.track_host(hy, hz, hro, htr, hhi, hcn, stream)   # returns after the results are in host memory
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    e2e_max, e2e_units = aggregate(e2e_ms, float(n) * e2e_steps, dist if world > 1 else None, dev)
+    h2d = int(hy.numel() * 4 + hz.numel() * 4 + hro.numel() * 4)
+    d2h = int(16 + int(hcn[0]) * 112 + int(hcn[1]) * 4)
+    assert int(hcn[0]) == len(tracks) and int(hcn[1]) == len(hit_ids), "host-buffer path disagrees with device path"
+
+    # ---- roofline ----------------------------------------------------------------------------------------
+    hbm_peak, peak_kind, sm_max = read_peaks()
+    sb = stage_bytes(float(n), n_bins, t_hits, float(n_seeds))
+    names = ["a1", "a2", "a3", "a4", "a5"]
+    stages = {k: {"ms": stage_ms[i], "alg_bytes": sb[k], "hbm_gbs": sb[k] / (stage_ms[i] * 1e-3) / 1e9}
+              for i, k in enumerate(names)}
+    dom = max(names, key=lambda k: stages[k]["ms"])
+    step_ms = ms_total / args.steps
+    path_bytes = sum(sb.values())
+    # a4 is plain-ALU bound (no dense contraction): fp32 FMA peak = 148 SMs x 128 lanes x 2 flop x max SM clock
+    alu_peak_tf = 148 * 128 * 2 * sm_max * 1e6 / 1e12
+    a4_tf = FLOP_PER_TRACKLET_HIT * t_hits / (stages["a4"]["ms"] * 1e-3) / 1e12
+    if dom == "a4":
+        roofline = {"kernel": "a4_follow_kernel", "bound": "alu", "achieved": a4_tf, "peak": alu_peak_tf,
+                    "unit": "TFLOP/s", "frac": a4_tf / alu_peak_tf, "traffic": None,
+                    "peak_kind": "derived: 148 SM x 128 fp32 lanes x 2 x %.0f MHz (DESIGN.md)" % sm_max,
+                    "hbm_achieved_gbs": stages["a4"]["hbm_gbs"], "hbm_frac": stages["a4"]["hbm_gbs"] / hbm_peak,
+                    "share_of_step": stages["a4"]["ms"] / sum(s["ms"] for s in stages.values())}
+    else:
+        roofline = {"kernel": dom, "bound": "hbm", "achieved": stages[dom]["hbm_gbs"], "peak": hbm_peak,
+                    "unit": "GB/s", "frac": stages[dom]["hbm_gbs"] / hbm_peak, "traffic": None,
+                    "peak_kind": peak_kind,
+                    "share_of_step": stages[dom]["ms"] / sum(s["ms"] for s in stages.values())}
+    path_gbs = path_bytes / (step_ms * 1e-3) / 1e9
+    roofline_path = {"bound": "hbm", "achieved": path_gbs, "peak": hbm_peak, "unit": "GB/s",
+                     "frac": path_gbs / hbm_peak, "peak_kind": peak_kind, "frac_of_8TBs_nominal": path_gbs / 8000.0,
+                     "alg_bytes_per_cluster": path_bytes / n}
+
+    # ---- oracle on the host cores (rank 0, N = 1 only) ----------------------------------------------------
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import oracle
+        oracle.build()
+        oracle.track(evs[0])   # warm the page cache / OpenMP pool
+        t0 = time.perf_counter()
+        done, k = 0, 0
+        while time.perf_counter() - t0 < 10.0 and k < 4 * len(evs):
+            oracle.track(evs[k % len(evs)])
+            done += evs[k % len(evs)].n
+            k += 1
+        dt = time.perf_counter() - t0
+        cpu = {"value": done / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"{k} single configs[1] events ({done} clusters) in {dt:.1f} s, g++ -O2 -fopenmp fp64"}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int32 (a1-a3, a5) / f32 state + f64 covariance (a4)", "data": "synthetic",
+            "config": {"workload": f"configs[1] central Pb-Pb (4000 tracks, 36 sectors, 5% noise), {B} distinct "
+                                   f"events per call as {B * 36} sectors", "batch_events": B,
+                       "clusters_per_step_per_gpu": n, "seeds_per_step": int(n_seeds), "tracks_per_step": len(tracks),
+                       "tracklet_hits_per_step": int(t_hits), "parallelism": "none (sectors independent; "
+                       "ranks = replicas on their own events)",
+                       "l2": f"working set {trk.scratch_bytes() / 1e6:.0f} MB scratch + {8 * n / 1e6:.0f} MB input "
+                             f"> 126 MB L2; no explicit flush"},
+            "tracks_per_s": len(tracks) * world * args.steps / (ms_max * 1e-3),
+            "single_event_latency_ms": latency_ms,
+            "e2e": {"value": e2e_units / (e2e_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "steps": e2e_steps, "ms_per_step": e2e_max / e2e_steps},
+            "gpu_launches": trk.launches_per_call() * args.steps,
+            "clocks": clk.summary(),
+            "roofline": roofline, "roofline_path": roofline_path, "stages": stages, "stage_calls_averaged": n_avg,
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(line))
+    trk.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_reference(args):
+    """The oracle as it stands, timed on the host cores: there is no reference implementation for this path (the
+    paper publishes no code), so the base contract's reference arm is the oracle.  Rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from gen.events import make_event
+    from oracle import oracle
+    oracle.build()
+    cores = oracle.num_threads()
+    # bounded sample: one configs[1] event per step; shrink it if the whole run would exceed ~3 minutes
+    total = args.steps + args.warmup
+    ev = make_event(CFG_ID)
+    t0 = time.perf_counter()
+    oracle.track(ev)
+    t_ev = time.perf_counter() - t0
+    n_tracks = None
+    if t_ev * total > 180.0:
+        n_tracks = max(50, int(4000 * 180.0 / (t_ev * total)))
+        ev = make_event(CFG_ID, n_tracks=n_tracks)
+    for _ in range(args.warmup):
+        oracle.track(ev)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.track(ev)
+    dt = time.perf_counter() - t0
+    value = ev.n * args.steps / dt
+    sample = (f"one configs[1] event per step ({ev.n} clusters"
+              + (f", reduced to {n_tracks} tracks to bound the run" if n_tracks else "") + ")")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "int64 / f64", "data": "synthetic",
+        "config": {"workload": "configs[1] central Pb-Pb (4000 tracks, 36 sectors, 5% noise)", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--batch-events", type=int, default=16)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -137,6 +137,9 @@ int tpc_launches_per_call(const tpc_tracker_t* t);
  * (tpc_set_stage_timing(t, 1) inserts CUDA events between the stages).  ms[0..4] = a1..a5.  Synchronises. */
 int tpc_set_stage_timing(tpc_tracker_t* t, int enable);
 int tpc_get_stage_ms(tpc_tracker_t* t, float ms[5]);
+/* Mean per-stage device times over the (up to 64) most recent calls made since stage timing was enabled;
+ * *n_calls (may be NULL) receives how many calls were averaged.  Synchronises on those calls' events. */
+int tpc_get_stage_ms_mean(tpc_tracker_t* t, float ms[5], int32_t* n_calls);
 
 /* ---- test-only exports: intermediate results of the most recent tpc_track call on this handle ----
  * All outputs are [device] buffers in id space (-1 = none), written asynchronously on `stream`. */

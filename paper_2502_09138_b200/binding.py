@@ -105,6 +105,7 @@ def load_library():
     lib.tpc_launches_per_call.argtypes = [C.c_void_p]
     lib.tpc_set_stage_timing.argtypes = [C.c_void_p, C.c_int]
     lib.tpc_get_stage_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+    lib.tpc_get_stage_ms_mean.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_int32)]
     lib.tpc_debug_copy_links.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.tpc_debug_copy_seeds.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.tpc_debug_copy_tracklets.argtypes = [C.c_void_p] + [C.c_void_p] * 6
@@ -260,6 +261,13 @@ class Tracker:
         ms = (C.c_float * 5)()
         self._check(self._lib.tpc_get_stage_ms(self._h, ms))
         return [float(v) for v in ms]
+
+    def stage_ms_mean(self):
+        """(mean ms per stage a1..a5, number of calls averaged) since set_stage_timing(True)."""
+        ms = (C.c_float * 5)()
+        n = C.c_int32()
+        self._check(self._lib.tpc_get_stage_ms_mean(self._h, ms, C.byref(n)))
+        return [float(v) for v in ms], int(n.value)
 
     # ---- test-only exports (tpc_debug_*) ----
     def debug_links(self, n: int, cleaned: bool):

@@ -244,7 +244,7 @@ int tpc_tracker_create(const tpc_geometry_t* geo, const tpc_field_t* field, tpc_
   g.row_dx = (const float*)((char*)t->geom_blob + o_dx);
   g.ny_row = (const int32_t*)((char*)t->geom_blob + o_ny);
   if (e == cudaSuccess) e = setup_a1_attributes(t);
-  for (int k = 0; k < 6 && e == cudaSuccess; ++k) e = cudaEventCreate(&t->ev[k]);
+  for (int k = 0; k < TIMING_SETS * 6 && e == cudaSuccess; ++k) e = cudaEventCreate(&t->ev[k]);
   if (e != cudaSuccess) {
     rc = e == cudaErrorMemoryAllocation ? TPC_ERR_NOMEM : TPC_ERR_CUDA;
     cudaGetLastError();
@@ -261,7 +261,7 @@ int tpc_tracker_destroy(tpc_tracker_t* t) {
   if (t->arena) cudaFree(t->arena);
   if (t->host_arena) cudaFree(t->host_arena);
   if (t->geom_blob) cudaFree(t->geom_blob);
-  for (int k = 0; k < 6; ++k)
+  for (int k = 0; k < TIMING_SETS * 6; ++k)
     if (t->ev[k]) cudaEventDestroy(t->ev[k]);
   delete t;
   return TPC_OK;
@@ -283,17 +283,21 @@ int tpc_track(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* strea
   t->last_y = cl->y;
   t->last_z = cl->z;
   TPC_CUDA(t, cudaMemsetAsync(t->s.ctl, 0, t->ctl_bytes, st));
-  if (t->timing) TPC_CUDA(t, cudaEventRecord(t->ev[0], st));
+  cudaEvent_t* ev = t->ev + (t->timed_calls % TIMING_SETS) * 6;   // ring of event sets, one per timed call
+  if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[0], st));
   TPC_CUDA(t, launch_a1_grid(t, cl->y, cl->z, cl->row_offsets, n, st));
-  if (t->timing) TPC_CUDA(t, cudaEventRecord(t->ev[1], st));
+  if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[1], st));
   TPC_CUDA(t, launch_a2_neighbours(t, cl->row_offsets, n, st));
-  if (t->timing) TPC_CUDA(t, cudaEventRecord(t->ev[2], st));
+  if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[2], st));
   TPC_CUDA(t, launch_a3_seeds(t, n, st));
-  if (t->timing) TPC_CUDA(t, cudaEventRecord(t->ev[3], st));
+  if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[3], st));
   TPC_CUDA(t, launch_a4_follow(t, cl->y, cl->z, cl->row_offsets, n, st));
-  if (t->timing) TPC_CUDA(t, cudaEventRecord(t->ev[4], st));
+  if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[4], st));
   TPC_CUDA(t, launch_a5_select(t, out, st));
-  if (t->timing) TPC_CUDA(t, cudaEventRecord(t->ev[5], st));
+  if (t->timing) {
+    TPC_CUDA(t, cudaEventRecord(ev[5], st));
+    ++t->timed_calls;
+  }
   return TPC_OK;
 }
 
@@ -358,13 +362,33 @@ int tpc_launches_per_call(const tpc_tracker_t* t) { return t ? 5 : 0; }
 int tpc_set_stage_timing(tpc_tracker_t* t, int enable) {
   if (!t) return TPC_ERR_ARG;
   t->timing = enable != 0;
+  t->timed_calls = 0;
   return TPC_OK;
 }
 
 int tpc_get_stage_ms(tpc_tracker_t* t, float ms[5]) {
-  if (!t || !ms) return TPC_ERR_ARG;
-  TPC_CUDA(t, cudaEventSynchronize(t->ev[5]));
-  for (int k = 0; k < 5; ++k) TPC_CUDA(t, cudaEventElapsedTime(&ms[k], t->ev[k], t->ev[k + 1]));
+  if (!t || !ms || t->timed_calls == 0) return TPC_ERR_ARG;
+  cudaEvent_t* ev = t->ev + ((t->timed_calls - 1) % TIMING_SETS) * 6;
+  TPC_CUDA(t, cudaEventSynchronize(ev[5]));
+  for (int k = 0; k < 5; ++k) TPC_CUDA(t, cudaEventElapsedTime(&ms[k], ev[k], ev[k + 1]));
+  return TPC_OK;
+}
+
+int tpc_get_stage_ms_mean(tpc_tracker_t* t, float ms[5], int32_t* n_calls) {
+  if (!t || !ms || t->timed_calls == 0) return TPC_ERR_ARG;
+  const int64_t m = t->timed_calls < TIMING_SETS ? t->timed_calls : TIMING_SETS;
+  double acc[5] = {0, 0, 0, 0, 0};
+  for (int64_t c = 0; c < m; ++c) {
+    cudaEvent_t* ev = t->ev + ((t->timed_calls - 1 - c) % TIMING_SETS) * 6;
+    TPC_CUDA(t, cudaEventSynchronize(ev[5]));
+    for (int k = 0; k < 5; ++k) {
+      float v;
+      TPC_CUDA(t, cudaEventElapsedTime(&v, ev[k], ev[k + 1]));
+      acc[k] += v;
+    }
+  }
+  for (int k = 0; k < 5; ++k) ms[k] = (float)(acc[k] / (double)m);
+  if (n_calls) *n_calls = (int32_t)m;
   return TPC_OK;
 }
 

@@ -58,6 +58,8 @@ struct Scratch {
   tpc_track_rec_t* st_tracks; int32_t* st_hits; int32_t* st_counts;
 };
 
+constexpr int TIMING_SETS = 64;   // ring of per-call stage-event sets (tpc_get_stage_ms_mean averages over them)
+
 struct tpc_tracker {
   int device;
   DevGeom g;                 // device pointers inside point at geom_blob
@@ -74,7 +76,7 @@ struct tpc_tracker {
   Scratch s;
   int64_t last_n; const uint32_t* last_ro; const int32_t* last_y; const int32_t* last_z;
   // stage timing
-  int timing; cudaEvent_t ev[6];
+  int timing; int64_t timed_calls; cudaEvent_t ev[TIMING_SETS * 6];
   cudaError_t last_err; char err_buf[256];
 };
 
