@@ -1,14 +1,22 @@
 // a4_follow.cu -- stage a4: Kalman-filter tracklet following with a helix model in constant Bz
-// (SURVEY 8(c) "Stage 4", P15-P24; Appendix C transport/Jacobian/update; north_star "one thread per seed ...
-// keeps the 5-parameter state and covariance in registers"), plus the a5 ownership vote
-// (atomicMax on packed (n_hits, rank) words, P26) fused at the end of each tracklet.
+// (SURVEY 8(c) "Stage 4", P15-P24; Appendix C transport/Jacobian/update; north_star "one thread per seed with
+// warp-level compaction of active seeds, that keeps the 5-parameter state and covariance in registers"), plus
+// the a5 ownership vote (atomicMax on packed (n_hits, rank) words, P26) cast when a tracklet ends.
 //
-// fp32 on the device.  To keep fp32 residuals exact for long drift offsets (configs[2]: |z| up to ~5400 cm) the
-// filter runs in coordinates relative to the seed's first cluster: hit - origin is an exact integer difference,
-// and the model is translation invariant in y and z.  The origin is added back in double at the end.
+// fp32 state on the device.  To keep fp32 residuals exact for long drift offsets (configs[2]: |z| up to ~5400 cm)
+// the filter runs in coordinates relative to the seed's first cluster: hit - origin is an exact integer
+// difference, and the model is translation invariant in y and z.  The origin is added back in double at the end.
 //
-// Thread per seed; seeds ascend by start id, so the lanes of a warp start in the same or adjacent rows of one
-// sector and step through the rows together.  Hit table layout [row][seed] makes those accesses coalesced.
+// Execution model (v2; v1 was a plain thread-per-seed kernel that ran 3.85 of 32 lanes,
+// profiles/r01_v1_a4_thread_per_seed.md):
+//  * Persistent warps, one lane per tracklet.  A lane whose tracklet ends takes the next seed rank from a device
+//    counter at the top of the loop, so the active lanes of a warp stay dense until the queue is empty.
+//  * One uniform per-row step for every phase of the method (init, A fit up the chain, B extend up, C refit down,
+//    D extend down, final transport): a phase only selects flags -- reset covariance?  transport by which dx?
+//    where does the hit come from (chain link / row search / recorded hit table / none)? -- and then all lanes run
+//    the same single transport and the same single update.  Lanes in different phases no longer serialise.
+//  * The per-tracklet row -> hit table lives in shared memory ([row][lane], one bank per lane); when a tracklet
+//    ends the whole warp writes it out coalesced and casts the ownership votes, 32 rows per instruction.
 #include "tpc_internal.cuh"
 
 namespace {
@@ -214,146 +222,196 @@ __device__ __forceinline__ Found search_row(const DevGeom& g, int sr, int row, c
   return f;
 }
 
-__global__ void __launch_bounds__(A4_BLOCK)
-a4_follow_kernel(const DevGeom g, int64_t s_cap, const DevCtl* __restrict__ ctl, const int32_t* __restrict__ y,
-                 const int32_t* __restrict__ z, const uint32_t* __restrict__ ro, const int32_t* __restrict__ ys,
-                 const int32_t* __restrict__ zs, const int32_t* __restrict__ ids, const int2* __restrict__ row_org,
-                 const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ up_c,
-                 const int32_t* __restrict__ seed_start, float* __restrict__ tl_par, float* __restrict__ tl_cov,
-                 float* __restrict__ tl_chi2, int32_t* __restrict__ tl_nhits, int32_t* __restrict__ tl_sr0,
-                 int32_t* __restrict__ tl_hits, uint32_t* __restrict__ owner) {
-  const int64_t i = (int64_t)blockIdx.x * A4_BLOCK + threadIdx.x;
-  if (i >= (int64_t)ctl->n_seeds) return;
-  const int nr = g.n_rows;
-  const int h0 = seed_start[i];
-  // (sector,row) of the seed: largest sr with ro[sr] <= h0
-  int lo = 0, hi = g.n_sectors * nr;
-  while (hi - lo > 1) {
-    const int mid = (lo + hi) >> 1;
-    if (ro[mid] <= (uint32_t)h0) lo = mid; else hi = mid;
-  }
-  const int sec_base = (lo / nr) * nr;
-  const int r0 = lo - sec_base;
-  int32_t* hits = tl_hits + i;   // hits[row * s_cap]
 
-  // P19 init from the first two chain hits
-  const int y0 = y[h0], z0 = z[h0];
-  int h = up_c[h0];
+enum : int { PH_IDLE = 0, PH_INIT, PH_A, PH_B, PH_CS, PH_CD, PH_FIN, PH_DONE };
+enum : int { M_NONE = 0, M_LINK, M_TABLE, M_SEARCH };
+
+constexpr int A4_WARPS = 1;   // warps per block; warps never synchronise with each other
+
+__global__ void __launch_bounds__(32 * A4_WARPS)
+a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restrict__ rec,
+                 const int32_t* __restrict__ ys, const int32_t* __restrict__ zs, const int32_t* __restrict__ ids,
+                 const int2* __restrict__ row_org, const uint32_t* __restrict__ bin_start,
+                 const int32_t* __restrict__ seed_start, const int32_t* __restrict__ seed_sr,
+                 float4* __restrict__ tl_rec, int32_t* __restrict__ tl_hits, uint32_t* __restrict__ owner) {
+  extern __shared__ int32_t tab_all[];
+  const unsigned FULL = 0xffffffffu;
+  const int lane = threadIdx.x & 31;
+  const int nr = g.n_rows;
+  int32_t* const wtab = tab_all + (threadIdx.x >> 5) * nr * 32;   // this warp's table, [row][lane]
+  int32_t* const tab = wtab + lane;
+  const uint32_t n_seeds = ctl->n_seeds;
+  if (n_seeds == 0) return;
+  // few seeds (one small event): spread them over all warps instead of filling the first warps' 32 lanes
+  const uint32_t n_warps = gridDim.x * A4_WARPS;
+  const int lanes_used = (int)min(32u, (n_seeds + n_warps - 1) / n_warps);
+
+  int phase = PH_IDLE;
+  bool exhausted = false;
+  int i = -1, h = -1, y0 = 0, z0 = 0, sec_base = 0, r0 = 0, row = 0, nh = 0, miss = 0, lowest = 0, rmin = 0, rmax = 0;
+  bool fail_dn = false;
+  float chi2 = 0.f;
   State p;
   Cov C;
-  {
-    const float dxr = g.row_dx[r0];
-    const float dy = (float)(y[h] - y0) * g.inv_units, dz = (float)(z[h] - z0) * g.inv_units;
-    const float ichord = rsqrtf(fmaf(dxr, dxr, dy * dy));
-    p.y = 0; p.z = 0; p.s = dy * ichord; p.t = dz * ichord; p.q = 0;
-  }
+  p.y = p.z = p.s = p.t = p.q = 0;
   cov_reset(g, C);
-  update(g, p, C, 0.f, 0.f);
-  hits[(int64_t)r0 * s_cap] = h0;
-  int row = r0, nh = 1;
-  bool fail_up = false;
 
-  // Phase A: fit up the chain, no gate
-  while (h >= 0) {
-    if (!transport<true>(g, g.row_dx[row], p, C)) { fail_up = true; break; }
-    ++row;
-    update(g, p, C, (float)(y[h] - y0) * g.inv_units, (float)(z[h] - z0) * g.inv_units);
-    hits[(int64_t)row * s_cap] = h;
-    ++nh;
-    h = up_c[h];
-  }
-  // Phase B: extend up with the gated nearest-hit search (P20)
-  if (!fail_up) {
-    int miss = 0;
-    while (row + 1 <= nr - 1 && miss < g.max_miss) {
-      if (!transport<true>(g, g.row_dx[row], p, C)) break;
-      ++row;
-      const Found f = search_row(g, sec_base + row, row, p, C, y0, z0, ys, zs, ids, row_org, bin_start);
-      hits[(int64_t)row * s_cap] = f.id;
-      if (f.id >= 0) {
-        update(g, p, C, f.y, f.z);
-        ++nh;
-        miss = 0;
-      } else {
-        ++miss;
+  while (true) {
+    // ---- refill free lanes from the seed queue ----
+    const bool want = phase == PH_IDLE && lane < lanes_used && !exhausted;
+    const unsigned idle = __ballot_sync(FULL, want);
+    if (idle) {
+      uint32_t base = 0;
+      if (lane == 0) base = atomicAdd(&ctl->next_seed, (uint32_t)__popc(idle));
+      base = __shfl_sync(FULL, base, 0);
+      if (base + (uint32_t)__popc(idle) >= n_seeds) exhausted = true;
+      const uint32_t k = base + (uint32_t)__popc(idle & ((1u << lane) - 1u));
+      if (want && k < n_seeds) {
+        // P19: state from the first two chain hits; the INIT step resets C and updates with the first hit
+        i = (int)k;
+        h = seed_start[k];
+        const int sr = seed_sr[k];
+        sec_base = (sr / nr) * nr;
+        r0 = sr - sec_base;
+        const int4 c0 = rec[h];
+        const int4 c1 = rec[c0.z];
+        y0 = c0.x;
+        z0 = c0.y;
+        const float dxr = g.row_dx[r0];
+        const float dy = (float)(c1.x - y0) * g.inv_units, dz = (float)(c1.y - z0) * g.inv_units;
+        const float ichord = rsqrtf(fmaf(dxr, dxr, dy * dy));
+        p.y = 0; p.z = 0; p.s = dy * ichord; p.t = dz * ichord; p.q = 0;
+        row = rmin = rmax = lowest = r0;
+        nh = 0; miss = 0; chi2 = 0.f; fail_dn = false;
+        phase = PH_INIT;
       }
     }
-  }
-  for (int r = row + 1; r < nr; ++r) hits[(int64_t)r * s_cap] = -1;
+    if (!__any_sync(FULL, phase != PH_IDLE)) break;
 
-  // Phase C: keep the state, reset the covariance (P22), refit down over the recorded hits;
-  // Phase D: below the seed's first row search as in B.
-  cov_reset(g, C);
-  float chi2 = 0.f;
-  {
-    const int hh = hits[(int64_t)row * s_cap];
-    if (hh >= 0) chi2 += update(g, p, C, (float)(y[hh] - y0) * g.inv_units, (float)(z[hh] - z0) * g.inv_units);
-  }
-  bool fail_dn = false;
-  int miss = 0, lowest = r0;
-  while (row > 0) {
-    if (row - 1 < r0 && miss >= g.max_miss) break;
-    if (!transport<true>(g, -g.row_dx[row - 1], p, C)) { fail_dn = true; break; }
-    --row;
-    if (row >= r0) {
-      const int hh = hits[(int64_t)row * s_cap];
-      if (hh >= 0) chi2 += update(g, p, C, (float)(y[hh] - y0) * g.inv_units, (float)(z[hh] - z0) * g.inv_units);
+    // ---- phase transitions that need no work ----
+    if (phase == PH_A && h < 0) phase = PH_B;                                                      // chain ended
+    if (phase == PH_B && !(row + 1 < nr && miss < g.max_miss)) phase = PH_CS;                      // P20
+    if (phase == PH_CD && (row == 0 || (row - 1 < r0 && miss >= g.max_miss))) phase = PH_FIN;      // P20
+    const int ph = phase;
+
+    // ---- what this step does ----
+    if (ph == PH_CS) { chi2 = 0.f; miss = 0; lowest = r0; }
+    if (ph == PH_INIT || ph == PH_CS) cov_reset(g, C);                                             // P19, P22
+    const int dir = (ph == PH_A || ph == PH_B) ? 1 : (ph == PH_CD ? -1 : 0);
+    int trow = row + dir;
+    bool tr = dir != 0;
+    float dx = 0.f;
+    if (dir > 0) dx = g.row_dx[row];
+    if (dir < 0) dx = -g.row_dx[row - 1];
+    int mode = M_NONE;
+    if (ph == PH_INIT || ph == PH_A) mode = M_LINK;
+    if (ph == PH_B || (ph == PH_CD && trow < r0)) mode = M_SEARCH;
+    if (ph == PH_CS || (ph == PH_CD && trow >= r0)) mode = M_TABLE;
+    if (ph == PH_FIN && !fail_dn && lowest != row) {   // P23: back to the lowest-row hit, no update
+      tr = true;
+      trow = lowest;
+      dx = (float)(g.row_x[lowest] - g.row_x[row]);
+    }
+    // hit known before the transport (chain link or recorded hit): start its gather now
+    int hid = -1;
+    if (mode == M_LINK) hid = h;
+    if (mode == M_TABLE) hid = tab[trow * 32];
+    int4 rc = make_int4(y0, z0, -1, -1);
+    if (hid >= 0) rc = rec[hid];
+
+    bool ok = ph != PH_IDLE && ph != PH_DONE;
+    if (ok && tr) ok = transport<true>(g, dx, p, C);
+    if (ok) {
+      row = trow;
+      float ym = (float)(rc.x - y0) * g.inv_units, zm = (float)(rc.y - z0) * g.inv_units;
+      if (mode == M_SEARCH) {
+        const Found f = search_row(g, sec_base + row, row, p, C, y0, z0, ys, zs, ids, row_org, bin_start);
+        hid = f.id;
+        ym = f.y;
+        zm = f.z;
+        tab[row * 32] = hid;
+        rmin = min(rmin, row);
+        rmax = max(rmax, row);
+        if (hid >= 0) {
+          ++nh;
+          miss = 0;
+          if (ph == PH_CD) lowest = row;
+        } else {
+          ++miss;
+        }
+      } else if (mode == M_LINK) {
+        tab[row * 32] = hid;
+        rmax = row;
+        ++nh;
+        h = rc.z;
+      }
+      if (mode != M_NONE && hid >= 0) chi2 += update(g, p, C, ym, zm);
+      if (ph == PH_INIT) phase = PH_A;
+      if (ph == PH_CS) phase = PH_CD;
+      if (ph == PH_FIN) phase = PH_DONE;
     } else {
-      const Found f = search_row(g, sec_base + row, row, p, C, y0, z0, ys, zs, ids, row_org, bin_start);
-      hits[(int64_t)row * s_cap] = f.id;
-      if (f.id >= 0) {
-        chi2 += update(g, p, C, f.y, f.z);
-        ++nh;
-        lowest = row;
-        miss = 0;
-      } else {
-        ++miss;
-      }
+      // transport failed (P18): the state stays where it is
+      if (ph == PH_A || ph == PH_B) phase = PH_CS;
+      if (ph == PH_CD) { fail_dn = true; phase = PH_FIN; }
+      if (ph == PH_FIN) phase = PH_DONE;
     }
-  }
-  // rows below the last visited one (rows < r0 only: rows >= r0 were all written in A/B)
-  for (int r = min(row, r0) - 1; r >= 0; --r) hits[(int64_t)r * s_cap] = -1;
 
-  // P23: transport (no update) back to the lowest-row hit
-  int xrow = row;
-  if (!fail_dn && lowest != row) {
-    const float dx = (float)(g.row_x[lowest] - g.row_x[row]);
-    if (transport<true>(g, dx, p, C)) xrow = lowest;
-  }
-  tl_par[0 * s_cap + i] = (float)g.row_x[xrow];
-  tl_par[1 * s_cap + i] = (float)((double)p.y + (double)y0 * g.inv_units_d);
-  tl_par[2 * s_cap + i] = (float)((double)p.z + (double)z0 * g.inv_units_d);
-  tl_par[3 * s_cap + i] = (float)p.s;
-  tl_par[4 * s_cap + i] = (float)p.t;
-  tl_par[5 * s_cap + i] = (float)p.q;
-  const float cv[15] = {(float)C.c00, (float)C.c10, (float)C.c11, (float)C.c20, (float)C.c21, (float)C.c22, (float)C.c30,
-                        (float)C.c31, (float)C.c32, (float)C.c33, (float)C.c40, (float)C.c41, (float)C.c42, (float)C.c43,
-                        (float)C.c44};
-#pragma unroll
-  for (int k = 0; k < 15; ++k) tl_cov[k * s_cap + i] = cv[k];
-  tl_chi2[i] = chi2;
-  tl_nhits[i] = nh;
-  tl_sr0[i] = sec_base + r0;
-
-  // a5 vote (P24, P26): owner(h) = surviving tracklet with the most hits, ties -> smallest rank
-  if (nh >= g.n_min_tracklet) {
-    const uint32_t word = ((uint32_t)nh << 24) | (0xFFFFFFu - (uint32_t)i);
-    for (int r = 0; r < nr; ++r) {
-      const int hh = hits[(int64_t)r * s_cap];
-      if (hh >= 0) atomicMax(&owner[hh], word);
+    // ---- tracklets that ended: record, hit table and ownership votes ----
+    const unsigned done = __ballot_sync(FULL, phase == PH_DONE);
+    if (done) {
+      if (phase == PH_DONE) {
+        float4* o = tl_rec + (size_t)i * TL_REC_V4;
+        o[0] = make_float4((float)g.row_x[row], (float)((double)p.y + (double)y0 * g.inv_units_d),
+                           (float)((double)p.z + (double)z0 * g.inv_units_d), (float)p.s);
+        o[1] = make_float4((float)p.t, (float)p.q, chi2, __int_as_float(nh));
+        o[2] = make_float4((float)C.c00, (float)C.c10, (float)C.c11, (float)C.c20);
+        o[3] = make_float4((float)C.c21, (float)C.c22, (float)C.c30, (float)C.c31);
+        o[4] = make_float4((float)C.c32, (float)C.c33, (float)C.c40, (float)C.c41);
+        o[5] = make_float4((float)C.c42, (float)C.c43, (float)C.c44, __int_as_float(sec_base + r0));
+      }
+      __syncwarp();
+      unsigned dm = done;
+      while (dm) {
+        const int src = __ffs(dm) - 1;
+        dm &= dm - 1;
+        const int si = __shfl_sync(FULL, i, src), snh = __shfl_sync(FULL, nh, src);
+        const int smin = __shfl_sync(FULL, rmin, src), smax = __shfl_sync(FULL, rmax, src);
+        // P24, P26: owner(h) = surviving tracklet with the most hits, ties -> smallest rank
+        const uint32_t word = snh >= g.n_min_tracklet ? (((uint32_t)snh << 24) | (0xFFFFFFu - (uint32_t)si)) : 0u;
+        int32_t* out = tl_hits + (size_t)si * nr;
+        for (int r = lane; r < nr; r += 32) {
+          const int v = (r >= smin && r <= smax) ? wtab[r * 32 + src] : -1;
+          out[r] = v;
+          if (word && v >= 0) atomicMax(&owner[v], word);
+        }
+      }
+      __syncwarp();
+      if (phase == PH_DONE) phase = PH_IDLE;
     }
   }
 }
 
 }  // namespace
 
-cudaError_t launch_a4_follow(const tpc_tracker* t, const int32_t* y, const int32_t* z, const uint32_t* ro, int64_t n,
-                             cudaStream_t st) {
+static size_t a4_smem_bytes(const DevGeom& g) { return (size_t)A4_WARPS * g.n_rows * 32 * sizeof(int32_t); }
+
+cudaError_t setup_a4_attributes(tpc_tracker* t) {
+  const size_t smem = a4_smem_bytes(t->g);
+  cudaError_t e = cudaFuncSetAttribute(a4_follow_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  int per_sm = 0, sms = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, a4_follow_kernel, 32 * A4_WARPS, smem);
+  if (e != cudaSuccess) return e;
+  e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, t->device);
+  if (e != cudaSuccess) return e;
+  t->a4_blocks = per_sm * sms;   // persistent grid: every resident warp slot of the device
+  return t->a4_blocks > 0 ? cudaSuccess : cudaErrorInvalidConfiguration;
+}
+
+cudaError_t launch_a4_follow(const tpc_tracker* t, int64_t n, cudaStream_t st) {
   if (n == 0 || t->s_cap == 0) return cudaSuccess;
-  const unsigned blocks = (unsigned)((t->s_cap + A4_BLOCK - 1) / A4_BLOCK);
-  a4_follow_kernel<<<blocks, A4_BLOCK, 0, st>>>(t->g, t->s_cap, t->s.ctl, y, z, ro, t->s.ys, t->s.zs, t->s.ids,
-                                               t->s.row_org, t->s.bin_start, t->s.up_c, t->s.seed_start, t->s.tl_par,
-                                               t->s.tl_cov, t->s.tl_chi2, t->s.tl_nhits, t->s.tl_sr0, t->s.tl_hits,
-                                               t->s.owner);
+  a4_follow_kernel<<<t->a4_blocks, 32 * A4_WARPS, a4_smem_bytes(t->g), st>>>(
+      t->g, t->s.ctl, t->s.rec, t->s.ys, t->s.zs, t->s.ids, t->s.row_org, t->s.bin_start, t->s.seed_start,
+      t->s.seed_sr, t->s.tl_rec, t->s.tl_hits, t->s.owner);
   return cudaGetLastError();
 }

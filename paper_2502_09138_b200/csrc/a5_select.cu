@@ -2,23 +2,31 @@
 // north_star "hit-ownership resolution with atomicMax on packed (quality, track-id) words").
 //
 // The votes (atomicMax of (n_hits << 24 | 0xFFFFFF - rank) per tracklet hit) were cast at the end of a4.
-// Here: thread per tracklet counts the hits it owns, keeps the tracklet iff owned >= n_min_owned (P27), and a
+// Here: the hits each tracklet owns are counted, a tracklet is kept iff owned >= n_min_owned (P27), and a
 // single-pass look-back scan over (kept, owned) gives each kept tracklet its output slot and hit offset in
 // ascending seed order (P29).  Track parameters are the a4 fit over all tracklet hits (P28).
 #include "tpc_internal.cuh"
 
 namespace {
 
+constexpr int A5_MASK_WORDS = 8;   // n_rows <= 255 (checked at create) -> at most 8 ballot words per tracklet
+
+// Block = A5_TILE threads = A5_TILE/32 warps, tile = A5_TILE tracklets.  Pass 1: each warp walks its 32 tracklets
+// one after the other, all lanes on one tracklet (32 rows per coalesced load of the [seed][row] hit table, one
+// owner gather per lane, ballot -> owned-hit mask kept in shared memory).  Then thread k of the block holds the
+// count of tracklet k, the block scan + look-back scan place it, and pass 2 writes the hit lists warp-wide.
 __global__ void __launch_bounds__(A5_TILE)
-a5_select_kernel(const DevGeom g, int64_t s_cap, DevCtl* __restrict__ ctl, const int32_t* __restrict__ seed_start,
-                 const float* __restrict__ tl_par, const float* __restrict__ tl_cov, const float* __restrict__ tl_chi2,
-                 const int32_t* __restrict__ tl_nhits, const int32_t* __restrict__ tl_sr0,
-                 const int32_t* __restrict__ tl_hits, const uint32_t* __restrict__ owner,
-                 uint64_t* __restrict__ status, tpc_track_rec_t* __restrict__ tracks, int32_t track_capacity,
-                 int32_t* __restrict__ hit_ids, int32_t hit_capacity, int32_t* __restrict__ counts) {
+a5_select_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int32_t* __restrict__ seed_start,
+                 const float4* __restrict__ tl_rec, const int32_t* __restrict__ tl_hits,
+                 const uint32_t* __restrict__ owner, uint64_t* __restrict__ status,
+                 tpc_track_rec_t* __restrict__ tracks, int32_t track_capacity, int32_t* __restrict__ hit_ids,
+                 int32_t hit_capacity, int32_t* __restrict__ counts) {
   __shared__ uint32_t wsum[33];
   __shared__ uint32_t sh_tile;
   __shared__ uint64_t sh_excl;
+  __shared__ uint32_t own_mask[A5_TILE][A5_MASK_WORDS];
+  __shared__ uint32_t sh_off[A5_TILE];   // output hit offset of a kept tracklet, 0xFFFFFFFF = no hit list to write
+  const unsigned FULL = 0xffffffffu;
   const uint32_t n_seeds = ctl->n_seeds;
   const uint32_t n_tiles = (n_seeds + A5_TILE - 1) / A5_TILE;
   if (n_seeds == 0) {
@@ -34,27 +42,41 @@ a5_select_kernel(const DevGeom g, int64_t s_cap, DevCtl* __restrict__ ctl, const
   if (threadIdx.x == 0) sh_tile = atomicAdd(&ctl->ticket_a5, 1u);
   __syncthreads();
   const uint32_t tile = sh_tile;
-  const int64_t i = (int64_t)tile * A5_TILE + threadIdx.x;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int nr = g.n_rows;
+  const int n_words = (nr + 31) >> 5;
+  const int64_t i = (int64_t)tile * A5_TILE + threadIdx.x;   // this thread's tracklet in the scans and the record
 
+  // pass 1
   uint32_t owned = 0;
   int first = -1, last = -1;
-  uint32_t word = 0;
-  if (i < n_seeds) {
-    const int nh = tl_nhits[i];
+  for (int t = 0; t < 32; ++t) {
+    const int64_t it = (int64_t)tile * A5_TILE + wid * 32 + t;
+    if (it >= n_seeds) break;   // warp-uniform
+    const int nh = __float_as_int(tl_rec[it * TL_REC_V4 + 1].w);
+    uint32_t cnt = 0;
+    int f = -1, l = -1;
     if (nh >= g.n_min_tracklet) {
-      word = ((uint32_t)nh << 24) | (0xFFFFFFu - (uint32_t)i);
-      for (int r = 0; r < nr; ++r) {
-        const int h = tl_hits[(int64_t)r * s_cap + i];
-        if (h >= 0 && owner[h] == word) {
-          ++owned;
-          if (first < 0) first = r;
-          last = r;
+      const uint32_t word = ((uint32_t)nh << 24) | (0xFFFFFFu - (uint32_t)it);
+      for (int k = 0; k < n_words; ++k) {
+        const int r = k * 32 + lane;
+        const int h = r < nr ? tl_hits[it * nr + r] : -1;
+        const unsigned m = __ballot_sync(FULL, h >= 0 && owner[h] == word);
+        if (lane == k) own_mask[wid * 32 + t][k] = m;
+        if (m) {
+          if (f < 0) f = k * 32 + __ffs(m) - 1;
+          l = k * 32 + 31 - __clz(m);
+          cnt += __popc(m);
         }
       }
     }
+    if (lane == t) {
+      owned = cnt;
+      first = f;
+      last = l;
+    }
   }
-  const bool keep = word != 0 && owned >= (uint32_t)g.n_min_owned;
+  const bool keep = owned >= (uint32_t)g.n_min_owned && owned > 0;   // P27
   if (!keep) owned = 0;
   uint32_t tot_k, tot_h;
   const uint32_t pos_k = block_excl_scan(keep ? 1u : 0u, wsum, &tot_k);
@@ -63,21 +85,22 @@ a5_select_kernel(const DevGeom g, int64_t s_cap, DevCtl* __restrict__ ctl, const
   const uint64_t ex = lookback_scan(status, tile, ((uint64_t)tot_k << 38) | tot_h, &sh_excl);
   const uint32_t excl[2] = {(uint32_t)(ex >> 38), (uint32_t)(ex & ((1ull << 38) - 1))};
 
+  uint32_t my_off = 0xFFFFFFFFu;
   if (keep) {
     const uint32_t slot = excl[0] + pos_k;
     const uint32_t off = excl[1] + pos_h;
     if (slot < (uint32_t)track_capacity) {
+      const float4* q = tl_rec + i * TL_REC_V4;
+      const float4 q0 = q[0], q1 = q[1], q2 = q[2], q3 = q[3], q4 = q[4], q5 = q[5];
       tpc_track_rec_t rec;
-      rec.x = tl_par[0 * s_cap + i];
-      rec.y = tl_par[1 * s_cap + i];
-      rec.z = tl_par[2 * s_cap + i];
-      rec.sinphi = tl_par[3 * s_cap + i];
-      rec.tanl = tl_par[4 * s_cap + i];
-      rec.qpt = tl_par[5 * s_cap + i];
-#pragma unroll
-      for (int k = 0; k < 15; ++k) rec.cov[k] = tl_cov[k * s_cap + i];
-      rec.chi2 = tl_chi2[i];
-      rec.sector = tl_sr0[i] / nr;
+      rec.x = q0.x; rec.y = q0.y; rec.z = q0.z; rec.sinphi = q0.w;
+      rec.tanl = q1.x; rec.qpt = q1.y;
+      rec.cov[0] = q2.x; rec.cov[1] = q2.y; rec.cov[2] = q2.z; rec.cov[3] = q2.w;
+      rec.cov[4] = q3.x; rec.cov[5] = q3.y; rec.cov[6] = q3.z; rec.cov[7] = q3.w;
+      rec.cov[8] = q4.x; rec.cov[9] = q4.y; rec.cov[10] = q4.z; rec.cov[11] = q4.w;
+      rec.cov[12] = q5.x; rec.cov[13] = q5.y; rec.cov[14] = q5.z;
+      rec.chi2 = q1.z;
+      rec.sector = __float_as_int(q5.w) / nr;
       rec.first_row = first;
       rec.last_row = last;
       rec.n_hits = (int32_t)owned;
@@ -85,12 +108,21 @@ a5_select_kernel(const DevGeom g, int64_t s_cap, DevCtl* __restrict__ ctl, const
       rec.seed_cluster = seed_start[i];
       tracks[slot] = rec;
     }
-    if ((uint64_t)off + owned <= (uint64_t)hit_capacity) {
-      uint32_t w = off;
-      for (int r = first; r <= last; ++r) {
-        const int h = tl_hits[(int64_t)r * s_cap + i];
-        if (h >= 0 && owner[h] == word) hit_ids[w++] = h;
-      }
+    if ((uint64_t)off + owned <= (uint64_t)hit_capacity) my_off = off;
+  }
+  sh_off[threadIdx.x] = my_off;
+  __syncwarp();   // sh_off and own_mask rows of this warp's tracklets are written and read by this warp only
+
+  // pass 2: hit lists, ascending row
+  for (int t = 0; t < 32; ++t) {
+    const int64_t it = (int64_t)tile * A5_TILE + wid * 32 + t;
+    if (it >= n_seeds) break;
+    uint32_t w = sh_off[wid * 32 + t];
+    if (w == 0xFFFFFFFFu) continue;
+    for (int k = 0; k < n_words; ++k) {
+      const unsigned m = own_mask[wid * 32 + t][k];
+      if ((m >> lane) & 1u) hit_ids[w + __popc(m & ((1u << lane) - 1u))] = tl_hits[it * nr + k * 32 + lane];
+      w += __popc(m);
     }
   }
   if (tile == n_tiles - 1 && threadIdx.x == 0) {
@@ -115,8 +147,7 @@ cudaError_t launch_a5_select(const tpc_tracker* t, const tpc_tracks_out_t* out, 
     return cudaGetLastError();
   }
   const unsigned blocks = (unsigned)((t->s_cap + A5_TILE - 1) / A5_TILE);
-  a5_select_kernel<<<blocks, A5_TILE, 0, st>>>(t->g, t->s_cap, t->s.ctl, t->s.seed_start, t->s.tl_par, t->s.tl_cov,
-                                              t->s.tl_chi2, t->s.tl_nhits, t->s.tl_sr0, t->s.tl_hits, t->s.owner,
+  a5_select_kernel<<<blocks, A5_TILE, 0, st>>>(t->g, t->s.ctl, t->s.seed_start, t->s.tl_rec, t->s.tl_hits, t->s.owner,
                                               t->s.scan_a5, out->tracks, out->track_capacity, out->hit_ids,
                                               out->hit_capacity, out->counts);
   return cudaGetLastError();

@@ -55,14 +55,11 @@ size_t layout(tpc_tracker* t, char* base, int64_t n, int64_t R) {
   s.bin_start = (uint32_t*)take((size_t)R * t->g.nb_stride * 4);
   s.link_up = (int32_t*)take((size_t)n * 4);
   s.link_dn = (int32_t*)take((size_t)n * 4);
-  s.up_c = (int32_t*)take((size_t)n * 4);
+  s.rec = (int4*)take((size_t)n * 16);
   s.owner = (uint32_t*)take((size_t)n * 4);
   s.seed_start = (int32_t*)take((size_t)s_cap * 4);
-  s.tl_par = (float*)take((size_t)s_cap * 6 * 4);
-  s.tl_cov = (float*)take((size_t)s_cap * 15 * 4);
-  s.tl_chi2 = (float*)take((size_t)s_cap * 4);
-  s.tl_nhits = (int32_t*)take((size_t)s_cap * 4);
-  s.tl_sr0 = (int32_t*)take((size_t)s_cap * 4);
+  s.seed_sr = (int32_t*)take((size_t)s_cap * 4);
+  s.tl_rec = (float4*)take((size_t)s_cap * TL_REC_V4 * 16);
   s.tl_hits = (int32_t*)take((size_t)s_cap * t->g.n_rows * 4);
   if (base) {
     t->s_cap = s_cap;
@@ -244,6 +241,7 @@ int tpc_tracker_create(const tpc_geometry_t* geo, const tpc_field_t* field, tpc_
   g.row_dx = (const float*)((char*)t->geom_blob + o_dx);
   g.ny_row = (const int32_t*)((char*)t->geom_blob + o_ny);
   if (e == cudaSuccess) e = setup_a1_attributes(t);
+  if (e == cudaSuccess) e = setup_a4_attributes(t);
   for (int k = 0; k < TIMING_SETS * 6 && e == cudaSuccess; ++k) e = cudaEventCreate(&t->ev[k]);
   if (e != cudaSuccess) {
     rc = e == cudaErrorMemoryAllocation ? TPC_ERR_NOMEM : TPC_ERR_CUDA;
@@ -289,9 +287,9 @@ int tpc_track(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* strea
   if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[1], st));
   TPC_CUDA(t, launch_a2_neighbours(t, cl->row_offsets, n, st));
   if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[2], st));
-  TPC_CUDA(t, launch_a3_seeds(t, n, st));
+  TPC_CUDA(t, launch_a3_seeds(t, cl->y, cl->z, cl->row_offsets, n, st));
   if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[3], st));
-  TPC_CUDA(t, launch_a4_follow(t, cl->y, cl->z, cl->row_offsets, n, st));
+  TPC_CUDA(t, launch_a4_follow(t, n, st));
   if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[4], st));
   TPC_CUDA(t, launch_a5_select(t, out, st));
   if (t->timing) {

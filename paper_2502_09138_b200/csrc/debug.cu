@@ -15,31 +15,31 @@ __global__ void dbg_clean_kernel(int64_t n, const int32_t* __restrict__ up, cons
 }
 
 __global__ void dbg_seed_len_kernel(const DevCtl* ctl, const int32_t* __restrict__ seed_start,
-                                    const int32_t* __restrict__ up_c, int32_t* __restrict__ start,
+                                    const int4* __restrict__ rec, int32_t* __restrict__ start,
                                     int32_t* __restrict__ len) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= (int64_t)ctl->n_seeds) return;
   const int h0 = seed_start[i];
   int l = 1;
-  for (int c = up_c[h0]; c >= 0; c = up_c[c]) ++l;
+  for (int c = rec[h0].z; c >= 0; c = rec[c].z) ++l;
   start[i] = h0;
   len[i] = l;
 }
 
-__global__ void dbg_tracklets_kernel(const DevCtl* ctl, int64_t s_cap, int n_rows, const float* __restrict__ tl_par,
-                                     const float* __restrict__ tl_cov, const float* __restrict__ tl_chi2,
-                                     const int32_t* __restrict__ tl_nhits, const int32_t* __restrict__ tl_hits,
-                                     float* par, float* cov, float* chi2, int32_t* n_hits, int32_t* hits) {
+__global__ void dbg_tracklets_kernel(const DevCtl* ctl, int n_rows, const float4* __restrict__ tl_rec,
+                                     const int32_t* __restrict__ tl_hits, float* par, float* cov, float* chi2,
+                                     int32_t* n_hits, int32_t* hits) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= (int64_t)ctl->n_seeds) return;
+  const float* q = (const float*)(tl_rec + i * TL_REC_V4);
   if (par)
-    for (int k = 0; k < 6; ++k) par[i * 6 + k] = tl_par[k * s_cap + i];
+    for (int k = 0; k < 6; ++k) par[i * 6 + k] = q[k];
   if (cov)
-    for (int k = 0; k < 15; ++k) cov[i * 15 + k] = tl_cov[k * s_cap + i];
-  if (chi2) chi2[i] = tl_chi2[i];
-  if (n_hits) n_hits[i] = tl_nhits[i];
+    for (int k = 0; k < 15; ++k) cov[i * 15 + k] = q[8 + k];
+  if (chi2) chi2[i] = q[6];
+  if (n_hits) n_hits[i] = __float_as_int(q[7]);
   if (hits)
-    for (int r = 0; r < n_rows; ++r) hits[i * n_rows + r] = tl_hits[(int64_t)r * s_cap + i];
+    for (int r = 0; r < n_rows; ++r) hits[i * n_rows + r] = tl_hits[i * n_rows + r];
 }
 
 __global__ void dbg_owner_kernel(int64_t n, const uint32_t* __restrict__ owner, int32_t* __restrict__ out) {
@@ -58,15 +58,14 @@ cudaError_t launch_dbg_clean(const tpc_tracker* t, int64_t n, int32_t* up, int32
 }
 cudaError_t launch_dbg_seed_len(const tpc_tracker* t, int32_t* start, int32_t* len, cudaStream_t st) {
   if (t->s_cap == 0) return cudaSuccess;
-  dbg_seed_len_kernel<<<(unsigned)((t->s_cap + 255) / 256), 256, 0, st>>>(t->s.ctl, t->s.seed_start, t->s.up_c, start, len);
+  dbg_seed_len_kernel<<<(unsigned)((t->s_cap + 255) / 256), 256, 0, st>>>(t->s.ctl, t->s.seed_start, t->s.rec, start, len);
   return cudaGetLastError();
 }
 cudaError_t launch_dbg_tracklets(const tpc_tracker* t, float* par, float* cov, float* chi2, int32_t* n_hits,
                                  int32_t* hits, cudaStream_t st) {
   if (t->s_cap == 0) return cudaSuccess;
   dbg_tracklets_kernel<<<(unsigned)((t->s_cap + 127) / 128), 128, 0, st>>>(
-      t->s.ctl, t->s_cap, t->g.n_rows, t->s.tl_par, t->s.tl_cov, t->s.tl_chi2, t->s.tl_nhits, t->s.tl_hits, par, cov,
-      chi2, n_hits, hits);
+      t->s.ctl, t->g.n_rows, t->s.tl_rec, t->s.tl_hits, par, cov, chi2, n_hits, hits);
   return cudaGetLastError();
 }
 cudaError_t launch_dbg_owner(const tpc_tracker* t, int64_t n, int32_t* owner, cudaStream_t st) {

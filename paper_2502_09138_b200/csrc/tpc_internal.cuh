@@ -29,7 +29,8 @@ struct DevCtl {
   uint32_t n_seeds;      // written by a3
   uint32_t ticket_a3;    // dynamic tile ids for the a3 look-back scan
   uint32_t ticket_a5;
-  uint32_t pad[13];
+  uint32_t next_seed;    // a4 work queue: next seed rank to hand to a free lane
+  uint32_t pad[12];
 };
 
 struct Scratch {
@@ -38,17 +39,16 @@ struct Scratch {
   int2* row_org;            // per (sector,row) grid origin
   uint32_t* bin_start;      // [R * nb_stride] global sorted index of the first cluster of each bin (+ sentinel)
   // a2 / a3 (id space)
-  int32_t *link_up, *link_dn, *up_c;
+  int32_t *link_up, *link_dn;
+  int4* rec;                // a3: per cluster id (y, z, cleaned up link, cleaned down link) -- one 16-B gather per a4 step
   uint32_t* owner;          // packed (n_hits << 24 | 0xFFFFFF - rank), 0 = none
   // a3 -> a4
   int32_t* seed_start;      // [s_cap] start cluster id, ascending
-  // a4 tracklets, SoA over seeds
-  float* tl_par;            // [6][s_cap]  x_ref, y, z, sinphi, tanl, qpt
-  float* tl_cov;            // [15][s_cap]
-  float* tl_chi2;           // [s_cap]
-  int32_t* tl_nhits;        // [s_cap]
-  int32_t* tl_sr0;          // [s_cap] sector * n_rows + first row of the seed
-  int32_t* tl_hits;         // [n_rows][s_cap] cluster id or -1
+  int32_t* seed_sr;         // [s_cap] sector * n_rows + row of the start cluster
+  // a4 tracklets, one 96-B record + one row table per seed
+  float4* tl_rec;           // [s_cap][6]: (x_ref,y,z,sinphi) (tanl,qpt,chi2,n_hits as int bits) cov[0..3] cov[4..7]
+                            //             cov[8..11] (cov[12],cov[13],cov[14],sector*n_rows+first seed row as int bits)
+  int32_t* tl_hits;         // [s_cap][n_rows] cluster id or -1
   // control
   DevCtl* ctl;
   uint64_t* scan_a3;        // look-back status words
@@ -72,6 +72,7 @@ struct tpc_tracker {
   int64_t cap_n, cap_rows;   // sizes the arena was laid out for
   int64_t s_cap;             // seed capacity of the current layout
   int64_t tiles_a3, tiles_a5;
+  int a4_blocks;             // persistent a4 grid: resident warps of the device (set at create)
   size_t ctl_bytes;          // bytes zeroed per call
   Scratch s;
   int64_t last_n; const uint32_t* last_ro; const int32_t* last_y; const int32_t* last_z;
@@ -82,13 +83,14 @@ struct tpc_tracker {
 
 constexpr int A3_TILE = 1024;   // ids per a3 block (256 threads x 4)
 constexpr int A5_TILE = 128;    // tracklets per a5 block
-constexpr int A4_BLOCK = 64;
+constexpr int TL_REC_V4 = 6;    // float4 words per tracklet record
 
 // launchers (each in its own .cu)
 cudaError_t launch_a1_grid(const tpc_tracker* t, const int32_t* y, const int32_t* z, const uint32_t* ro, int64_t n, cudaStream_t st);
 cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64_t n, cudaStream_t st);
-cudaError_t launch_a3_seeds(const tpc_tracker* t, int64_t n, cudaStream_t st);
-cudaError_t launch_a4_follow(const tpc_tracker* t, const int32_t* y, const int32_t* z, const uint32_t* ro, int64_t n, cudaStream_t st);
+cudaError_t launch_a3_seeds(const tpc_tracker* t, const int32_t* y, const int32_t* z, const uint32_t* ro, int64_t n, cudaStream_t st);
+cudaError_t launch_a4_follow(const tpc_tracker* t, int64_t n, cudaStream_t st);
+cudaError_t setup_a4_attributes(tpc_tracker* t);
 cudaError_t launch_a5_select(const tpc_tracker* t, const tpc_tracks_out_t* out, cudaStream_t st);
 cudaError_t setup_a1_attributes(const tpc_tracker* t);
 size_t a1_smem_bytes(const DevGeom& g);
