@@ -5,7 +5,7 @@
 //
 // One CTA per (sector,row):  pass 0 block-min of y and z -> grid origin;  pass 1 shared-memory histogram over
 // bins (y fastest);  block exclusive scan;  bin starts written as global sorted indices;  pass 2 scatter of
-// (y, z, id) into bin order.  Clusters beyond the geometry's nominal extent land in the edge bins (clamp),
+// (y, z, id) as one 16-byte record into bin order.  Clusters beyond the geometry's nominal extent land in the edge bins (clamp),
 // which keeps both searches exact (clamping is monotone, so bin distances never grow).
 #include "tpc_internal.cuh"
 
@@ -17,8 +17,8 @@ __device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? l
 
 __global__ void __launch_bounds__(A1_THREADS)
 a1_grid_kernel(const DevGeom g, const int32_t* __restrict__ y, const int32_t* __restrict__ z,
-               const uint32_t* __restrict__ ro, int32_t* __restrict__ ys, int32_t* __restrict__ zs,
-               int32_t* __restrict__ ids, int2* __restrict__ row_org, uint32_t* __restrict__ bin_start) {
+               const uint32_t* __restrict__ ro, int4* __restrict__ srt, int2* __restrict__ row_org,
+               uint32_t* __restrict__ bin_start) {
   extern __shared__ uint32_t hist[];
   __shared__ int red_y[A1_THREADS / 32], red_z[A1_THREADS / 32];
   __shared__ uint32_t wsum[33];
@@ -85,9 +85,7 @@ a1_grid_kernel(const DevGeom g, const int32_t* __restrict__ y, const int32_t* __
     int iy = clampi((yi - ymin) >> g.shift_y, 0, ny - 1);
     int iz = clampi((zi - zmin) >> g.shift_z, 0, nz - 1);
     uint32_t pos = a + atomicAdd(&hist[iz * ny + iy], 1u);
-    ys[pos] = yi;
-    zs[pos] = zi;
-    ids[pos] = (int32_t)i;
+    srt[pos] = make_int4(yi, zi, (int32_t)i, 0);
   }
 }
 
@@ -103,7 +101,7 @@ cudaError_t launch_a1_grid(const tpc_tracker* t, const int32_t* y, const int32_t
                            cudaStream_t st) {
   const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
   if (R == 0) return cudaSuccess;
-  a1_grid_kernel<<<(unsigned)R, A1_THREADS, a1_smem_bytes(t->g), st>>>(t->g, y, z, ro, t->s.ys, t->s.zs, t->s.ids,
-                                                                        t->s.row_org, t->s.bin_start);
+  a1_grid_kernel<<<(unsigned)R, A1_THREADS, a1_smem_bytes(t->g), st>>>(t->g, y, z, ro, t->s.srt, t->s.row_org,
+                                                                        t->s.bin_start);
   return cudaGetLastError();
 }

@@ -37,8 +37,7 @@ __device__ __forceinline__ Ranges window_ranges(const DevGeom& g, int yh, int zh
 }
 
 __global__ void __launch_bounds__(A2_THREADS)
-a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int32_t* __restrict__ ys,
-                     const int32_t* __restrict__ zs, const int32_t* __restrict__ ids,
+a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int4* __restrict__ srt,
                      const int2* __restrict__ row_org, const uint32_t* __restrict__ bin_start,
                      int32_t* __restrict__ link_up, int32_t* __restrict__ link_dn, uint32_t* __restrict__ owner) {
   const int sr = blockIdx.x;
@@ -57,7 +56,8 @@ a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int
     bs_d = bin_start + (size_t)(sr - 1) * g.nb_stride;
   }
   for (uint32_t j = a + threadIdx.x; j < b; j += A2_THREADS) {
-    const int yh = ys[j], zh = zs[j], hid = ids[j];
+    const int4 ch = srt[j];
+    const int yh = ch.x, zh = ch.y, hid = ch.z;
     int best_u = -1, best_d = -1;
     if (inner) {
       const Ranges qu = window_ranges(g, yh, zh, org_u, ny_u, bs_u);
@@ -67,19 +67,21 @@ a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int
       for (int pu = 0; pu < 2; ++pu) {
         const uint32_t ua = pu ? qu.a1 : qu.a0, ub = pu ? qu.b1 : qu.b0;
         for (uint32_t u = ua; u < ub; ++u) {
-          const int dyu = ys[u] - yh, dzu = zs[u] - zh;
+          const int4 cu = srt[u];
+          const int dyu = cu.x - yh, dzu = cu.y - zh;
           if (abs(dyu) > g.w_y || abs(dzu) > g.w_z) continue;
-          const int idu = ids[u];
+          const int idu = cu.z;
 #pragma unroll 1
           for (int pd = 0; pd < 2; ++pd) {
             const uint32_t da = pd ? qd.a1 : qd.a0, db = pd ? qd.b1 : qd.b0;
             for (uint32_t d = da; d < db; ++d) {
-              const int dyd = ys[d] - yh, dzd = zs[d] - zh;
+              const int4 cd = srt[d];
+              const int dyd = cd.x - yh, dzd = cd.y - zh;
               if (abs(dyd) > g.w_y || abs(dzd) > g.w_z) continue;
               const int ddy = dyu + dyd, ddz = dzu + dzd;
               const int cost = g.cost_wy * ddy * ddy + g.cost_wz * ddz * ddz;
               if (cost > best_cost) continue;
-              const int idd = ids[d];
+              const int idd = cd.z;
               if (cost < best_cost || idu < best_u || (idu == best_u && idd < best_d)) {   // P9
                 best_cost = cost;
                 best_u = idu;
@@ -102,7 +104,7 @@ a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int
 cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64_t n, cudaStream_t st) {
   const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
   if (R == 0) return cudaSuccess;
-  a2_neighbours_kernel<<<(unsigned)R, A2_THREADS, 0, st>>>(t->g, ro, t->s.ys, t->s.zs, t->s.ids, t->s.row_org,
+  a2_neighbours_kernel<<<(unsigned)R, A2_THREADS, 0, st>>>(t->g, ro, t->s.srt, t->s.row_org,
                                                           t->s.bin_start, t->s.link_up, t->s.link_dn, t->s.owner);
   return cudaGetLastError();
 }

@@ -176,43 +176,54 @@ struct Found {
   float y, z;   // relative coordinates of the accepted hit
 };
 
+// Geometry tables every step needs, copied to shared memory once per block (a lane reads them at its own row).
+struct RowTabs {
+  const double* row_x;
+  const float* row_dx;
+  const int32_t* ny_row;
+};
+
 // P17/P21: among the clusters of sector-row `sr` with |dy| <= gate_y and |dz| <= gate_z (cm) minimise (d, id),
-// d = dy^2/(Cyy + sy2) + dz^2/(Czz + sz2); accept iff d < gate_d.  The a1 grid only prunes.
-__device__ __forceinline__ Found search_row(const DevGeom& g, int sr, int row, const State& p, const Cov& C, int y0,
-                                            int z0, const int32_t* __restrict__ ys, const int32_t* __restrict__ zs,
-                                            const int32_t* __restrict__ ids, const int2* __restrict__ row_org,
+// d = dy^2/(Cyy + sy2) + dz^2/(Czz + sz2); accept iff d < gate_d.  The a1 grid only prunes: a cluster can only be
+// accepted if dy^2/(Cyy+sy2) < gate_d, so the bins that are read cover |dy| <= min(gate_y, sqrt(gate_d (Cyy+sy2)))
+// (widened by 0.2 % + 2 units against rounding), likewise in z; every accept/compare below is the definition's.
+__device__ __forceinline__ Found search_row(const DevGeom& g, int sr, int ny, const State& p, const Cov& C, int y0,
+                                            int z0, const int4* __restrict__ srt, const int2* __restrict__ row_org,
                                             const uint32_t* __restrict__ bin_start) {
   Found f;
   f.id = -1;
   f.y = f.z = 0.f;
   const int2 org = row_org[sr];
-  const int ny = g.ny_row[row];
   const uint32_t* bs = bin_start + (size_t)sr * g.nb_stride;
-  // integer superset of the float window (+-1 unit of slack on each side), clamped against overflow
+  const float vy = (float)C.c00 + g.sy2, vz = (float)C.c11 + g.sz2;
+  const float hy = fminf(g.gate_y, sqrtf(g.gate_d * vy) * 1.002f), hz = fminf(g.gate_z, sqrtf(g.gate_d * vz) * 1.002f);
+  // integer superset of the float window (+-2 units of slack on each side), clamped against overflow
   const float lim = 1.0e9f;
   const float py = (float)p.y, pz = (float)p.z;
-  const int ylo = y0 + (int)fminf(fmaxf(floorf((py - g.gate_y) * g.units) - 1.f, -lim), lim);
-  const int yhi = y0 + (int)fminf(fmaxf(ceilf((py + g.gate_y) * g.units) + 1.f, -lim), lim);
-  const int zlo = z0 + (int)fminf(fmaxf(floorf((pz - g.gate_z) * g.units) - 1.f, -lim), lim);
-  const int zhi = z0 + (int)fminf(fmaxf(ceilf((pz + g.gate_z) * g.units) + 1.f, -lim), lim);
+  const int ylo = y0 + (int)fminf(fmaxf(floorf((py - hy) * g.units) - 2.f, -lim), lim);
+  const int yhi = y0 + (int)fminf(fmaxf(ceilf((py + hy) * g.units) + 2.f, -lim), lim);
+  const int zlo = z0 + (int)fminf(fmaxf(floorf((pz - hz) * g.units) - 2.f, -lim), lim);
+  const int zhi = z0 + (int)fminf(fmaxf(ceilf((pz + hz) * g.units) + 2.f, -lim), lim);
   const int iy_lo = clampi((ylo - org.x) >> g.shift_y, 0, ny - 1);
   const int iy_hi = clampi((yhi - org.x) >> g.shift_y, 0, ny - 1);
   const int iz_lo = clampi((zlo - org.y) >> g.shift_z, 0, g.nz - 1);
   const int iz_hi = clampi((zhi - org.y) >> g.shift_z, 0, g.nz - 1);
-  const float wy = 1.f / ((float)C.c00 + g.sy2), wz = 1.f / ((float)C.c11 + g.sz2);
+  const float wy = 1.f / vy, wz = 1.f / vz;
   float bestd = __int_as_float(0x7f800000);
   for (int iz = iz_lo; iz <= iz_hi; ++iz) {
     const uint32_t a = bs[iz * ny + iy_lo], b = bs[iz * ny + iy_hi + 1];
+    if (a >= b) continue;
+    int4 nx = srt[a];
     for (uint32_t j = a; j < b; ++j) {
-      const float cy = (float)(ys[j] - y0) * g.inv_units, cz = (float)(zs[j] - z0) * g.inv_units;
+      const int4 c = nx;
+      if (j + 1 < b) nx = srt[j + 1];   // next candidate in flight while this one is tested
+      const float cy = (float)(c.x - y0) * g.inv_units, cz = (float)(c.y - z0) * g.inv_units;
       const float dy = cy - py, dz = cz - pz;
       if (fabsf(dy) > g.gate_y || fabsf(dz) > g.gate_z) continue;
       const float d = dy * dy * wy + dz * dz * wz;
-      if (d > bestd) continue;
-      const int id = ids[j];
-      if (d < bestd || id < f.id) {
+      if (d < bestd || (d == bestd && c.z < f.id)) {
         bestd = d;
-        f.id = id;
+        f.id = c.z;
         f.y = cy;
         f.z = cz;
       }
@@ -222,28 +233,37 @@ __device__ __forceinline__ Found search_row(const DevGeom& g, int sr, int row, c
   return f;
 }
 
-
 enum : int { PH_IDLE = 0, PH_INIT, PH_A, PH_B, PH_CS, PH_CD, PH_FIN, PH_DONE };
 enum : int { M_NONE = 0, M_LINK, M_TABLE, M_SEARCH };
 
-constexpr int A4_WARPS = 1;   // warps per block; warps never synchronise with each other
+constexpr int A4_MAX_WARPS = 16;   // warps per block (chosen at create to fill one SM's shared memory); warps
+                                   // never synchronise with each other after the geometry tables are loaded
 
-__global__ void __launch_bounds__(32 * A4_WARPS)
+__global__ void __launch_bounds__(32 * A4_MAX_WARPS)
 a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restrict__ rec,
-                 const int32_t* __restrict__ ys, const int32_t* __restrict__ zs, const int32_t* __restrict__ ids,
-                 const int2* __restrict__ row_org, const uint32_t* __restrict__ bin_start,
+                 const int4* __restrict__ srt, const int2* __restrict__ row_org, const uint32_t* __restrict__ bin_start,
                  const int32_t* __restrict__ seed_start, const int32_t* __restrict__ seed_sr,
                  float4* __restrict__ tl_rec, int32_t* __restrict__ tl_hits, uint32_t* __restrict__ owner) {
-  extern __shared__ int32_t tab_all[];
+  extern __shared__ double smem_a4[];
   const unsigned FULL = 0xffffffffu;
   const int lane = threadIdx.x & 31;
   const int nr = g.n_rows;
-  int32_t* const wtab = tab_all + (threadIdx.x >> 5) * nr * 32;   // this warp's table, [row][lane]
-  int32_t* const tab = wtab + lane;
   const uint32_t n_seeds = ctl->n_seeds;
   if (n_seeds == 0) return;
+  // shared memory: row_x[nr] (double) | row_dx[nr] | ny_row[nr] | per warp: hit table [nr][32]
+  double* const s_row_x = smem_a4;
+  float* const s_row_dx = (float*)(s_row_x + nr);
+  int32_t* const s_ny = (int32_t*)(s_row_dx + nr);
+  for (int r = threadIdx.x; r < nr; r += blockDim.x) {
+    s_row_x[r] = g.row_x[r];
+    s_row_dx[r] = g.row_dx[r];
+    s_ny[r] = g.ny_row[r];
+  }
+  __syncthreads();
+  int32_t* const wtab = s_ny + nr + (threadIdx.x >> 5) * nr * 32;   // this warp's table, [row][lane]
+  int32_t* const tab = wtab + lane;
   // few seeds (one small event): spread them over all warps instead of filling the first warps' 32 lanes
-  const uint32_t n_warps = gridDim.x * A4_WARPS;
+  const uint32_t n_warps = gridDim.x * (blockDim.x >> 5);
   const int lanes_used = (int)min(32u, (n_seeds + n_warps - 1) / n_warps);
 
   int phase = PH_IDLE;
@@ -277,7 +297,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
         const int4 c1 = rec[c0.z];
         y0 = c0.x;
         z0 = c0.y;
-        const float dxr = g.row_dx[r0];
+        const float dxr = s_row_dx[r0];
         const float dy = (float)(c1.x - y0) * g.inv_units, dz = (float)(c1.y - z0) * g.inv_units;
         const float ichord = rsqrtf(fmaf(dxr, dxr, dy * dy));
         p.y = 0; p.z = 0; p.s = dy * ichord; p.t = dz * ichord; p.q = 0;
@@ -301,8 +321,8 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
     int trow = row + dir;
     bool tr = dir != 0;
     float dx = 0.f;
-    if (dir > 0) dx = g.row_dx[row];
-    if (dir < 0) dx = -g.row_dx[row - 1];
+    if (dir > 0) dx = s_row_dx[row];
+    if (dir < 0) dx = -s_row_dx[row - 1];
     int mode = M_NONE;
     if (ph == PH_INIT || ph == PH_A) mode = M_LINK;
     if (ph == PH_B || (ph == PH_CD && trow < r0)) mode = M_SEARCH;
@@ -310,7 +330,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
     if (ph == PH_FIN && !fail_dn && lowest != row) {   // P23: back to the lowest-row hit, no update
       tr = true;
       trow = lowest;
-      dx = (float)(g.row_x[lowest] - g.row_x[row]);
+      dx = (float)(s_row_x[lowest] - s_row_x[row]);
     }
     // hit known before the transport (chain link or recorded hit): start its gather now
     int hid = -1;
@@ -325,7 +345,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
       row = trow;
       float ym = (float)(rc.x - y0) * g.inv_units, zm = (float)(rc.y - z0) * g.inv_units;
       if (mode == M_SEARCH) {
-        const Found f = search_row(g, sec_base + row, row, p, C, y0, z0, ys, zs, ids, row_org, bin_start);
+        const Found f = search_row(g, sec_base + row, s_ny[row], p, C, y0, z0, srt, row_org, bin_start);
         hid = f.id;
         ym = f.y;
         zm = f.z;
@@ -361,7 +381,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
     if (done) {
       if (phase == PH_DONE) {
         float4* o = tl_rec + (size_t)i * TL_REC_V4;
-        o[0] = make_float4((float)g.row_x[row], (float)((double)p.y + (double)y0 * g.inv_units_d),
+        o[0] = make_float4((float)s_row_x[row], (float)((double)p.y + (double)y0 * g.inv_units_d),
                            (float)((double)p.z + (double)z0 * g.inv_units_d), (float)p.s);
         o[1] = make_float4((float)p.t, (float)p.q, chi2, __int_as_float(nh));
         o[2] = make_float4((float)C.c00, (float)C.c10, (float)C.c11, (float)C.c20);
@@ -393,25 +413,34 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
 
 }  // namespace
 
-static size_t a4_smem_bytes(const DevGeom& g) { return (size_t)A4_WARPS * g.n_rows * 32 * sizeof(int32_t); }
+static size_t a4_smem_bytes(const DevGeom& g, int warps) {
+  return (size_t)g.n_rows * (8 + 4 + 4) + (size_t)warps * g.n_rows * 32 * sizeof(int32_t);
+}
 
 cudaError_t setup_a4_attributes(tpc_tracker* t) {
-  const size_t smem = a4_smem_bytes(t->g);
-  cudaError_t e = cudaFuncSetAttribute(a4_follow_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  int sms = 0, smem_max = 0;
+  cudaError_t e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, t->device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, t->device);
   if (e != cudaSuccess) return e;
-  int per_sm = 0, sms = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, a4_follow_kernel, 32 * A4_WARPS, smem);
+  // one block per SM with as many warps as hit tables fit next to the geometry tables
+  int warps = (int)(((size_t)smem_max - a4_smem_bytes(t->g, 0)) / ((size_t)t->g.n_rows * 128));
+  if (warps > A4_MAX_WARPS) warps = A4_MAX_WARPS;
+  if (warps < 1) return cudaErrorInvalidConfiguration;
+  const size_t smem = a4_smem_bytes(t->g, warps);
+  e = cudaFuncSetAttribute(a4_follow_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, t->device);
+  int per_sm = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, a4_follow_kernel, 32 * warps, smem);
   if (e != cudaSuccess) return e;
+  t->a4_warps = warps;
   t->a4_blocks = per_sm * sms;   // persistent grid: every resident warp slot of the device
   return t->a4_blocks > 0 ? cudaSuccess : cudaErrorInvalidConfiguration;
 }
 
 cudaError_t launch_a4_follow(const tpc_tracker* t, int64_t n, cudaStream_t st) {
   if (n == 0 || t->s_cap == 0) return cudaSuccess;
-  a4_follow_kernel<<<t->a4_blocks, 32 * A4_WARPS, a4_smem_bytes(t->g), st>>>(
-      t->g, t->s.ctl, t->s.rec, t->s.ys, t->s.zs, t->s.ids, t->s.row_org, t->s.bin_start, t->s.seed_start,
-      t->s.seed_sr, t->s.tl_rec, t->s.tl_hits, t->s.owner);
+  a4_follow_kernel<<<t->a4_blocks, 32 * t->a4_warps, a4_smem_bytes(t->g, t->a4_warps), st>>>(
+      t->g, t->s.ctl, t->s.rec, t->s.srt, t->s.row_org, t->s.bin_start, t->s.seed_start, t->s.seed_sr, t->s.tl_rec,
+      t->s.tl_hits, t->s.owner);
   return cudaGetLastError();
 }

@@ -48,9 +48,7 @@ size_t layout(tpc_tracker* t, char* base, int64_t n, int64_t R) {
   s.scan_a3 = (uint64_t*)take((size_t)tiles_a3 * 8);
   s.scan_a5 = (uint64_t*)take((size_t)tiles_a5 * 8);
   const size_t ctl_bytes = off;
-  s.ys = (int32_t*)take((size_t)n * 4 + 64);
-  s.zs = (int32_t*)take((size_t)n * 4 + 64);
-  s.ids = (int32_t*)take((size_t)n * 4 + 64);
+  s.srt = (int4*)take((size_t)n * 16 + 64);
   s.row_org = (int2*)take((size_t)R * sizeof(int2));
   s.bin_start = (uint32_t*)take((size_t)R * t->g.nb_stride * 4);
   s.link_up = (int32_t*)take((size_t)n * 4);
@@ -440,7 +438,8 @@ int tpc_debug_copy_grid(tpc_tracker_t* t, int32_t* ids_sorted, uint32_t* bin_sta
   cudaStream_t st = (cudaStream_t)stream;
   const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
   if (ids_sorted && t->last_n > 0)
-    TPC_CUDA(t, cudaMemcpyAsync(ids_sorted, t->s.ids, (size_t)t->last_n * 4, cudaMemcpyDeviceToDevice, st));
+    TPC_CUDA(t, cudaMemcpy2DAsync(ids_sorted, 4, &t->s.srt->z, sizeof(int4), 4, (size_t)t->last_n,
+                                  cudaMemcpyDeviceToDevice, st));
   if (bin_start && R > 0)
     TPC_CUDA(t, cudaMemcpyAsync(bin_start, t->s.bin_start, (size_t)R * t->g.nb_stride * 4, cudaMemcpyDeviceToDevice, st));
   return TPC_OK;

@@ -35,7 +35,7 @@ struct DevCtl {
 
 struct Scratch {
   // a1
-  int32_t *ys, *zs, *ids;   // sorted (bin order inside each row) coordinates and cluster ids
+  int4* srt;                // clusters in bin order inside each row: (y, z, cluster id, 0) -- one 16-B load per candidate
   int2* row_org;            // per (sector,row) grid origin
   uint32_t* bin_start;      // [R * nb_stride] global sorted index of the first cluster of each bin (+ sentinel)
   // a2 / a3 (id space)
@@ -72,7 +72,7 @@ struct tpc_tracker {
   int64_t cap_n, cap_rows;   // sizes the arena was laid out for
   int64_t s_cap;             // seed capacity of the current layout
   int64_t tiles_a3, tiles_a5;
-  int a4_blocks;             // persistent a4 grid: resident warps of the device (set at create)
+  int a4_blocks, a4_warps;   // persistent a4 grid: blocks x warps per block = resident warps of the device (set at create)
   size_t ctl_bytes;          // bytes zeroed per call
   Scratch s;
   int64_t last_n; const uint32_t* last_ro; const int32_t* last_y; const int32_t* last_z;
