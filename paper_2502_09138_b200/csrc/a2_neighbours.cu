@@ -18,12 +18,13 @@ struct Ranges {
 
 __device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
 
-__device__ __forceinline__ Ranges window_ranges(const DevGeom& g, int yh, int zh, int2 org, int ny,
+__device__ __forceinline__ Ranges window_ranges(const DevGeom& g, int yh, int zh, int org_z,
                                                 const uint32_t* __restrict__ bs) {
-  const int iy_lo = clampi((yh - g.w_y - org.x) >> g.shift_y, 0, ny - 1);
-  const int iy_hi = clampi((yh + g.w_y - org.x) >> g.shift_y, 0, ny - 1);
-  const int iz_lo = clampi((zh - g.w_z - org.y) >> g.shift_z, 0, g.nz - 1);
-  const int iz_hi = clampi((zh + g.w_z - org.y) >> g.shift_z, 0, g.nz - 1);
+  const int ny = g.ny;
+  const int iy_lo = clampi((yh - g.w_y - g.org_y) >> g.shift_y, 0, ny - 1);
+  const int iy_hi = clampi((yh + g.w_y - g.org_y) >> g.shift_y, 0, ny - 1);
+  const int iz_lo = clampi((zh - g.w_z - org_z) >> g.shift_z, 0, g.nz - 1);
+  const int iz_hi = clampi((zh + g.w_z - org_z) >> g.shift_z, 0, g.nz - 1);
   Ranges q;
   q.a0 = bs[iz_lo * ny + iy_lo];
   q.b0 = bs[iz_lo * ny + iy_hi + 1];
@@ -38,20 +39,15 @@ __device__ __forceinline__ Ranges window_ranges(const DevGeom& g, int yh, int zh
 
 __global__ void __launch_bounds__(A2_THREADS)
 a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int4* __restrict__ srt,
-                     const int2* __restrict__ row_org, const uint32_t* __restrict__ bin_start,
+                     const uint32_t* __restrict__ sec_key, const uint32_t* __restrict__ bin_start,
                      int32_t* __restrict__ link_up, int32_t* __restrict__ link_dn, uint32_t* __restrict__ owner) {
   const int sr = blockIdx.x;
   const int r = sr % g.n_rows;
   const uint32_t a = ro[sr], b = ro[sr + 1];
   const bool inner = r >= 1 && r <= g.n_rows - 2;   // P5
-  int2 org_u, org_d;
-  int ny_u = 1, ny_d = 1;
+  const int org_z = zmin_from_key(sec_key[sr / g.n_rows]);
   const uint32_t *bs_u = nullptr, *bs_d = nullptr;
   if (inner) {
-    org_u = row_org[sr + 1];
-    org_d = row_org[sr - 1];
-    ny_u = g.ny_row[r + 1];
-    ny_d = g.ny_row[r - 1];
     bs_u = bin_start + (size_t)(sr + 1) * g.nb_stride;
     bs_d = bin_start + (size_t)(sr - 1) * g.nb_stride;
   }
@@ -60,8 +56,8 @@ a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int
     const int yh = ch.x, zh = ch.y, hid = ch.z;
     int best_u = -1, best_d = -1;
     if (inner) {
-      const Ranges qu = window_ranges(g, yh, zh, org_u, ny_u, bs_u);
-      const Ranges qd = window_ranges(g, yh, zh, org_d, ny_d, bs_d);
+      const Ranges qu = window_ranges(g, yh, zh, org_z, bs_u);
+      const Ranges qd = window_ranges(g, yh, zh, org_z, bs_d);
       int best_cost = INT32_MAX;
 #pragma unroll 1
       for (int pu = 0; pu < 2; ++pu) {
@@ -104,7 +100,7 @@ a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int
 cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64_t n, cudaStream_t st) {
   const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
   if (R == 0) return cudaSuccess;
-  a2_neighbours_kernel<<<(unsigned)R, A2_THREADS, 0, st>>>(t->g, ro, t->s.srt, t->s.row_org,
+  a2_neighbours_kernel<<<(unsigned)R, A2_THREADS, 0, st>>>(t->g, ro, t->s.srt, t->s.sec_key,
                                                           t->s.bin_start, t->s.link_up, t->s.link_dn, t->s.owner);
   return cudaGetLastError();
 }

@@ -7,7 +7,7 @@
 // the filter runs in coordinates relative to the seed's first cluster: hit - origin is an exact integer
 // difference, and the model is translation invariant in y and z.  The origin is added back in double at the end.
 //
-// Execution model (v2; v1 was a plain thread-per-seed kernel that ran 3.85 of 32 lanes,
+// Execution model (v1 was a plain thread-per-seed kernel that ran 3.85 of 32 lanes,
 // profiles/r01_v1_a4_thread_per_seed.md):
 //  * Persistent warps, one lane per tracklet.  A lane whose tracklet ends takes the next seed rank from a device
 //    counter at the top of the loop, so the active lanes of a warp stay dense until the queue is empty.
@@ -15,8 +15,14 @@
 //    D extend down, final transport): a phase only selects flags -- reset covariance?  transport by which dx?
 //    where does the hit come from (chain link / row search / recorded hit table / none)? -- and then all lanes run
 //    the same single transport and the same single update.  Lanes in different phases no longer serialise.
-//  * The per-tracklet row -> hit table lives in shared memory ([row][lane], one bank per lane); when a tracklet
-//    ends the whole warp writes it out coalesced and casts the ownership votes, 32 rows per instruction.
+//  * The step is latency-bound on its gathers, so every gather whose address is known early is issued one step
+//    ahead and carried in registers: the next chain hit's record (its id is in the current record), the next two
+//    entries of the row -> hit table on the way down, and the bin starts of the next row's search window at the
+//    extrapolated position (validated against the exact window after the transport; a wrong guess only costs the
+//    direct loads).  The candidates of the current search are prefetched into L1 while the transport computes.
+//  * The row -> hit table is the tracklet's final [row] array in global memory (L2-resident while in use); when a
+//    tracklet ends the whole warp pads it with -1 and casts the ownership votes, 32 rows per instruction.  No
+//    shared memory beyond two small geometry tables, so L1 keeps its full size for the gathers.
 #include "tpc_internal.cuh"
 
 namespace {
@@ -176,47 +182,67 @@ struct Found {
   float y, z;   // relative coordinates of the accepted hit
 };
 
-// Geometry tables every step needs, copied to shared memory once per block (a lane reads them at its own row).
-struct RowTabs {
-  const double* row_x;
-  const float* row_dx;
-  const int32_t* ny_row;
+// The search window of P17/P21 in grid bins.  A cluster can only be accepted if dy^2/(Cyy+sy2) < gate_d, so the
+// bins that are read cover |dy| <= min(gate_y, sqrt(gate_d (Cyy+sy2))) (widened by 0.2 % + 2 units against
+// rounding), likewise in z: the grid only prunes, every accept/compare in search_row is the definition's.
+struct Window {
+  int iy_lo, iy_hi, iz_lo, iz_hi;
+  __device__ __forceinline__ uint32_t key_y() const { return ((uint32_t)iy_lo << 16) | (uint32_t)iy_hi; }
+  __device__ __forceinline__ uint32_t key_z(int row) const {
+    return ((uint32_t)row << 24) | ((uint32_t)iz_lo << 1) | (iz_hi != iz_lo ? 1u : 0u);
+  }
 };
 
-// P17/P21: among the clusters of sector-row `sr` with |dy| <= gate_y and |dz| <= gate_z (cm) minimise (d, id),
-// d = dy^2/(Cyy + sy2) + dz^2/(Czz + sz2); accept iff d < gate_d.  The a1 grid only prunes: a cluster can only be
-// accepted if dy^2/(Cyy+sy2) < gate_d, so the bins that are read cover |dy| <= min(gate_y, sqrt(gate_d (Cyy+sy2)))
-// (widened by 0.2 % + 2 units against rounding), likewise in z; every accept/compare below is the definition's.
-__device__ __forceinline__ Found search_row(const DevGeom& g, int sr, int ny, const State& p, const Cov& C, int y0,
-                                            int z0, const int4* __restrict__ srt, const int2* __restrict__ row_org,
-                                            const uint32_t* __restrict__ bin_start) {
-  Found f;
-  f.id = -1;
-  f.y = f.z = 0.f;
-  const int2 org = row_org[sr];
-  const uint32_t* bs = bin_start + (size_t)sr * g.nb_stride;
-  const float vy = (float)C.c00 + g.sy2, vz = (float)C.c11 + g.sz2;
+__device__ __forceinline__ Window search_window(const DevGeom& g, float py, float pz, float vy, float vz, int y0, int z0,
+                                                int org_z) {
   const float hy = fminf(g.gate_y, sqrtf(g.gate_d * vy) * 1.002f), hz = fminf(g.gate_z, sqrtf(g.gate_d * vz) * 1.002f);
-  // integer superset of the float window (+-2 units of slack on each side), clamped against overflow
-  const float lim = 1.0e9f;
-  const float py = (float)p.y, pz = (float)p.z;
+  const float lim = 1.0e9f;   // clamp against int overflow
   const int ylo = y0 + (int)fminf(fmaxf(floorf((py - hy) * g.units) - 2.f, -lim), lim);
   const int yhi = y0 + (int)fminf(fmaxf(ceilf((py + hy) * g.units) + 2.f, -lim), lim);
   const int zlo = z0 + (int)fminf(fmaxf(floorf((pz - hz) * g.units) - 2.f, -lim), lim);
   const int zhi = z0 + (int)fminf(fmaxf(ceilf((pz + hz) * g.units) + 2.f, -lim), lim);
-  const int iy_lo = clampi((ylo - org.x) >> g.shift_y, 0, ny - 1);
-  const int iy_hi = clampi((yhi - org.x) >> g.shift_y, 0, ny - 1);
-  const int iz_lo = clampi((zlo - org.y) >> g.shift_z, 0, g.nz - 1);
-  const int iz_hi = clampi((zhi - org.y) >> g.shift_z, 0, g.nz - 1);
+  Window w;
+  w.iy_lo = clampi((ylo - g.org_y) >> g.shift_y, 0, g.ny - 1);
+  w.iy_hi = clampi((yhi - g.org_y) >> g.shift_y, 0, g.ny - 1);
+  w.iz_lo = clampi((zlo - org_z) >> g.shift_z, 0, g.nz - 1);
+  w.iz_hi = clampi((zhi - org_z) >> g.shift_z, 0, g.nz - 1);   // bins are >= 2 gate_z wide: iz_hi <= iz_lo + 1
+  return w;
+}
+
+// Bin starts of a window: (a0,b0) = sorted range of the low z-bin, (a1,b1) of the high one (empty if the same).
+struct BinRanges {
+  uint32_t a0, b0, a1, b1;
+};
+
+__device__ __forceinline__ BinRanges load_ranges(const DevGeom& g, const uint32_t* __restrict__ bs, const Window& w) {
+  BinRanges q;
+  q.a0 = bs[w.iz_lo * g.ny + w.iy_lo];
+  q.b0 = bs[w.iz_lo * g.ny + w.iy_hi + 1];
+  q.a1 = q.b1 = 0;
+  if (w.iz_hi != w.iz_lo) {
+    q.a1 = bs[w.iz_hi * g.ny + w.iy_lo];
+    q.b1 = bs[w.iz_hi * g.ny + w.iy_hi + 1];
+  }
+  return q;
+}
+
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
+// P17/P21: among the candidates minimise (d, id), d = dy^2/(Cyy + sy2) + dz^2/(Czz + sz2), restricted to
+// |dy| <= gate_y and |dz| <= gate_z (cm); accept iff d < gate_d.
+__device__ __forceinline__ Found search_row(const DevGeom& g, const BinRanges& q, float py, float pz, float vy, float vz,
+                                            int y0, int z0, const int4* __restrict__ srt) {
+  Found f;
+  f.id = -1;
+  f.y = f.z = 0.f;
   const float wy = 1.f / vy, wz = 1.f / vz;
   float bestd = __int_as_float(0x7f800000);
-  for (int iz = iz_lo; iz <= iz_hi; ++iz) {
-    const uint32_t a = bs[iz * ny + iy_lo], b = bs[iz * ny + iy_hi + 1];
-    if (a >= b) continue;
-    int4 nx = srt[a];
-    for (uint32_t j = a; j < b; ++j) {
+  const uint32_t n0 = q.b0 - q.a0, total = n0 + (q.b1 - q.a1);
+  if (total) {
+    int4 nx = srt[n0 ? q.a0 : q.a1];
+    for (uint32_t t = 0; t < total; ++t) {   // one flat loop over both z-bins
       const int4 c = nx;
-      if (j + 1 < b) nx = srt[j + 1];   // next candidate in flight while this one is tested
+      if (t + 1 < total) nx = srt[t + 1 < n0 ? q.a0 + t + 1 : q.a1 + (t + 1 - n0)];   // next one in flight
       const float cy = (float)(c.x - y0) * g.inv_units, cz = (float)(c.y - z0) * g.inv_units;
       const float dy = cy - py, dz = cz - pz;
       if (fabsf(dy) > g.gate_y || fabsf(dz) > g.gate_z) continue;
@@ -236,32 +262,29 @@ __device__ __forceinline__ Found search_row(const DevGeom& g, int sr, int ny, co
 enum : int { PH_IDLE = 0, PH_INIT, PH_A, PH_B, PH_CS, PH_CD, PH_FIN, PH_DONE };
 enum : int { M_NONE = 0, M_LINK, M_TABLE, M_SEARCH };
 
-constexpr int A4_MAX_WARPS = 16;   // warps per block (chosen at create to fill one SM's shared memory); warps
-                                   // never synchronise with each other after the geometry tables are loaded
+constexpr int A4_THREADS = 128;   // warps never synchronise with each other after the geometry tables are loaded
+constexpr int A4_MIN_BLOCKS = 4;  // 16 warps per SM: registers capped at 128 per thread
 
-__global__ void __launch_bounds__(32 * A4_MAX_WARPS)
+__global__ void __launch_bounds__(A4_THREADS, A4_MIN_BLOCKS)
 a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restrict__ rec,
-                 const int4* __restrict__ srt, const int2* __restrict__ row_org, const uint32_t* __restrict__ bin_start,
-                 const int32_t* __restrict__ seed_start, const int32_t* __restrict__ seed_sr,
-                 float4* __restrict__ tl_rec, int32_t* __restrict__ tl_hits, uint32_t* __restrict__ owner) {
+                 const int4* __restrict__ srt, const uint32_t* __restrict__ sec_key,
+                 const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ seed_start,
+                 const int32_t* __restrict__ seed_sr, float4* __restrict__ tl_rec, int32_t* __restrict__ tl_hits,
+                 uint32_t* __restrict__ owner) {
   extern __shared__ double smem_a4[];
   const unsigned FULL = 0xffffffffu;
   const int lane = threadIdx.x & 31;
   const int nr = g.n_rows;
   const uint32_t n_seeds = ctl->n_seeds;
   if (n_seeds == 0) return;
-  // shared memory: row_x[nr] (double) | row_dx[nr] | ny_row[nr] | per warp: hit table [nr][32]
+  // shared memory: row_x[nr] (double) | row_dx[nr]
   double* const s_row_x = smem_a4;
   float* const s_row_dx = (float*)(s_row_x + nr);
-  int32_t* const s_ny = (int32_t*)(s_row_dx + nr);
   for (int r = threadIdx.x; r < nr; r += blockDim.x) {
     s_row_x[r] = g.row_x[r];
     s_row_dx[r] = g.row_dx[r];
-    s_ny[r] = g.ny_row[r];
   }
   __syncthreads();
-  int32_t* const wtab = s_ny + nr + (threadIdx.x >> 5) * nr * 32;   // this warp's table, [row][lane]
-  int32_t* const tab = wtab + lane;
   // few seeds (one small event): spread them over all warps instead of filling the first warps' 32 lanes
   const uint32_t n_warps = gridDim.x * (blockDim.x >> 5);
   const int lanes_used = (int)min(32u, (n_seeds + n_warps - 1) / n_warps);
@@ -269,12 +292,21 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
   int phase = PH_IDLE;
   bool exhausted = false;
   int i = -1, h = -1, y0 = 0, z0 = 0, sec_base = 0, r0 = 0, row = 0, nh = 0, miss = 0, lowest = 0, rmin = 0, rmax = 0;
+  int org_z = 0;
   bool fail_dn = false;
   float chi2 = 0.f;
+  int32_t* tab = tl_hits;   // this tracklet's row -> hit table
   State p;
   Cov C;
   p.y = p.z = p.s = p.t = p.q = 0;
   cov_reset(g, C);
+  // gathers issued one step ahead (a mismatch of the tag only costs the direct load)
+  int rcn_id = -1;                 // record of cluster rcn_id
+  int4 rcn = make_int4(0, 0, -1, -1);
+  int t1_row = -1, t1_val = -1;    // table entries of the next two rows on the way down
+  int t2_row = -1, t2_val = -1;
+  uint32_t pk_y = 0xFFFFFFFFu, pk_z = 0xFFFFFFFFu;   // bin ranges of the window keyed (pk_y, pk_z)
+  BinRanges pq = {0, 0, 0, 0};
 
   while (true) {
     // ---- refill free lanes from the seed queue ----
@@ -291,10 +323,15 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
         i = (int)k;
         h = seed_start[k];
         const int sr = seed_sr[k];
-        sec_base = (sr / nr) * nr;
+        const int sec = sr / nr;
+        sec_base = sec * nr;
         r0 = sr - sec_base;
+        org_z = zmin_from_key(sec_key[sec]);
+        tab = tl_hits + (size_t)k * nr;
         const int4 c0 = rec[h];
         const int4 c1 = rec[c0.z];
+        rcn_id = h;
+        rcn = c0;
         y0 = c0.x;
         z0 = c0.y;
         const float dxr = s_row_dx[r0];
@@ -303,6 +340,8 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
         p.y = 0; p.z = 0; p.s = dy * ichord; p.t = dz * ichord; p.q = 0;
         row = rmin = rmax = lowest = r0;
         nh = 0; miss = 0; chi2 = 0.f; fail_dn = false;
+        t1_row = t2_row = -1;
+        pk_y = pk_z = 0xFFFFFFFFu;
         phase = PH_INIT;
       }
     }
@@ -332,12 +371,49 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
       trow = lowest;
       dx = (float)(s_row_x[lowest] - s_row_x[row]);
     }
-    // hit known before the transport (chain link or recorded hit): start its gather now
+
+    // ---- hit known before the transport (chain link or recorded hit) ----
     int hid = -1;
+    bool t1_old = false;   // t1_val was loaded in an earlier step (safe to consume without waiting)
     if (mode == M_LINK) hid = h;
-    if (mode == M_TABLE) hid = tab[trow * 32];
+    if (mode == M_TABLE) {
+      if (t1_row == trow) hid = t1_val;
+      else if (t2_row == trow) hid = t2_val;
+      else hid = __ldcg(tab + trow);
+      // keep the entries of the next two rows down in flight
+      const int n1 = trow - 1, n2 = trow - 2;
+      int v1 = -1, v2 = -1;
+      bool v1_old = false;
+      if (n1 >= r0) {
+        if (t1_row == n1) { v1 = t1_val; v1_old = true; }
+        else if (t2_row == n1) { v1 = t2_val; v1_old = true; }
+        else v1 = __ldcg(tab + n1);
+      }
+      if (n2 >= r0) v2 = (t2_row == n2) ? t2_val : __ldcg(tab + n2);
+      t1_row = n1 >= r0 ? n1 : -1;
+      t1_val = v1;
+      t2_row = n2 >= r0 ? n2 : -1;
+      t2_val = v2;
+      t1_old = v1_old;
+    }
     int4 rc = make_int4(y0, z0, -1, -1);
-    if (hid >= 0) rc = rec[hid];
+    if (hid >= 0) rc = (hid == rcn_id) ? rcn : rec[hid];
+    // next step's record: the chain's next hit, or the recorded hit of the next row down
+    {
+      int nid = -1;
+      if (mode == M_LINK) nid = rc.z;
+      if (mode == M_TABLE && t1_old) nid = t1_val;
+      if (nid >= 0 && nid != rcn_id) {
+        rcn_id = nid;
+        rcn = rec[nid];
+      }
+    }
+    // candidates of this step's search: bin ranges were loaded last step; touch the candidates now
+    const uint32_t* bs = bin_start + (size_t)(sec_base + trow) * g.nb_stride;
+    if (mode == M_SEARCH && (pk_z >> 24) == (uint32_t)trow) {
+      if (pq.b0 > pq.a0) prefetch_l1(srt + pq.a0);
+      if (pq.b1 > pq.a1) prefetch_l1(srt + pq.a1);
+    }
 
     bool ok = ph != PH_IDLE && ph != PH_DONE;
     if (ok && tr) ok = transport<true>(g, dx, p, C);
@@ -345,11 +421,16 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
       row = trow;
       float ym = (float)(rc.x - y0) * g.inv_units, zm = (float)(rc.y - z0) * g.inv_units;
       if (mode == M_SEARCH) {
-        const Found f = search_row(g, sec_base + row, s_ny[row], p, C, y0, z0, srt, row_org, bin_start);
+        const float py = (float)p.y, pz = (float)p.z;
+        const float vy = (float)C.c00 + g.sy2, vz = (float)C.c11 + g.sz2;
+        const Window w = search_window(g, py, pz, vy, vz, y0, z0, org_z);
+        BinRanges q = pq;
+        if (w.key_y() != pk_y || w.key_z(row) != pk_z) q = load_ranges(g, bs, w);
+        const Found f = search_row(g, q, py, pz, vy, vz, y0, z0, srt);
         hid = f.id;
         ym = f.y;
         zm = f.z;
-        tab[row * 32] = hid;
+        tab[row] = hid;
         rmin = min(rmin, row);
         rmax = max(rmax, row);
         if (hid >= 0) {
@@ -360,7 +441,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
           ++miss;
         }
       } else if (mode == M_LINK) {
-        tab[row * 32] = hid;
+        tab[row] = hid;
         rmax = row;
         ++nh;
         h = rc.z;
@@ -376,7 +457,24 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
       if (ph == PH_FIN) phase = PH_DONE;
     }
 
-    // ---- tracklets that ended: record, hit table and ownership votes ----
+    // ---- bin ranges of the next step's search window, at the extrapolated position ----
+    {
+      int nrow = -1;
+      float ndx = 0.f;
+      if (((phase == PH_A && h < 0) || phase == PH_B) && row + 1 < nr) { nrow = row + 1; ndx = s_row_dx[row]; }
+      if (phase == PH_CD && row - 1 < r0 && row >= 1) { nrow = row - 1; ndx = -s_row_dx[row - 1]; }
+      if (nrow >= 0) {
+        const float ps = (float)p.s;
+        const float ic = rsqrtf(fmaxf(1.f - ps * ps, 0.05f));
+        const float py = (float)p.y + ndx * ps * ic, pz = (float)p.z + ndx * (float)p.t * ic;
+        const Window w = search_window(g, py, pz, (float)C.c00 + g.sy2, (float)C.c11 + g.sz2, y0, z0, org_z);
+        pk_y = w.key_y();
+        pk_z = w.key_z(nrow);
+        pq = load_ranges(g, bin_start + (size_t)(sec_base + nrow) * g.nb_stride, w);
+      }
+    }
+
+    // ---- tracklets that ended: record, padding of the hit table and ownership votes ----
     const unsigned done = __ballot_sync(FULL, phase == PH_DONE);
     if (done) {
       if (phase == PH_DONE) {
@@ -389,7 +487,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
         o[4] = make_float4((float)C.c32, (float)C.c33, (float)C.c40, (float)C.c41);
         o[5] = make_float4((float)C.c42, (float)C.c43, (float)C.c44, __int_as_float(sec_base + r0));
       }
-      __syncwarp();
+      __syncwarp();   // the table entries of the ending lanes are visible to the whole warp
       unsigned dm = done;
       while (dm) {
         const int src = __ffs(dm) - 1;
@@ -400,12 +498,14 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
         const uint32_t word = snh >= g.n_min_tracklet ? (((uint32_t)snh << 24) | (0xFFFFFFu - (uint32_t)si)) : 0u;
         int32_t* out = tl_hits + (size_t)si * nr;
         for (int r = lane; r < nr; r += 32) {
-          const int v = (r >= smin && r <= smax) ? wtab[r * 32 + src] : -1;
-          out[r] = v;
-          if (word && v >= 0) atomicMax(&owner[v], word);
+          if (r >= smin && r <= smax) {
+            const int v = __ldcg(out + r);
+            if (word && v >= 0) atomicMax(&owner[v], word);
+          } else {
+            out[r] = -1;
+          }
         }
       }
-      __syncwarp();
       if (phase == PH_DONE) phase = PH_IDLE;
     }
   }
@@ -413,34 +513,23 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
 
 }  // namespace
 
-static size_t a4_smem_bytes(const DevGeom& g, int warps) {
-  return (size_t)g.n_rows * (8 + 4 + 4) + (size_t)warps * g.n_rows * 32 * sizeof(int32_t);
-}
+static size_t a4_smem_bytes(const DevGeom& g) { return (size_t)g.n_rows * (8 + 4); }
 
 cudaError_t setup_a4_attributes(tpc_tracker* t) {
-  int sms = 0, smem_max = 0;
+  int sms = 0;
   cudaError_t e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, t->device);
-  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, t->device);
-  if (e != cudaSuccess) return e;
-  // one block per SM with as many warps as hit tables fit next to the geometry tables
-  int warps = (int)(((size_t)smem_max - a4_smem_bytes(t->g, 0)) / ((size_t)t->g.n_rows * 128));
-  if (warps > A4_MAX_WARPS) warps = A4_MAX_WARPS;
-  if (warps < 1) return cudaErrorInvalidConfiguration;
-  const size_t smem = a4_smem_bytes(t->g, warps);
-  e = cudaFuncSetAttribute(a4_follow_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   int per_sm = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, a4_follow_kernel, 32 * warps, smem);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, a4_follow_kernel, A4_THREADS, a4_smem_bytes(t->g));
   if (e != cudaSuccess) return e;
-  t->a4_warps = warps;
   t->a4_blocks = per_sm * sms;   // persistent grid: every resident warp slot of the device
   return t->a4_blocks > 0 ? cudaSuccess : cudaErrorInvalidConfiguration;
 }
 
 cudaError_t launch_a4_follow(const tpc_tracker* t, int64_t n, cudaStream_t st) {
   if (n == 0 || t->s_cap == 0) return cudaSuccess;
-  a4_follow_kernel<<<t->a4_blocks, 32 * t->a4_warps, a4_smem_bytes(t->g, t->a4_warps), st>>>(
-      t->g, t->s.ctl, t->s.rec, t->s.srt, t->s.row_org, t->s.bin_start, t->s.seed_start, t->s.seed_sr, t->s.tl_rec,
+  a4_follow_kernel<<<t->a4_blocks, A4_THREADS, a4_smem_bytes(t->g), st>>>(
+      t->g, t->s.ctl, t->s.rec, t->s.srt, t->s.sec_key, t->s.bin_start, t->s.seed_start, t->s.seed_sr, t->s.tl_rec,
       t->s.tl_hits, t->s.owner);
   return cudaGetLastError();
 }

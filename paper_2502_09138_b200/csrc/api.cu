@@ -47,9 +47,9 @@ size_t layout(tpc_tracker* t, char* base, int64_t n, int64_t R) {
   s.ctl = (DevCtl*)take(sizeof(DevCtl));
   s.scan_a3 = (uint64_t*)take((size_t)tiles_a3 * 8);
   s.scan_a5 = (uint64_t*)take((size_t)tiles_a5 * 8);
+  s.sec_key = (uint32_t*)take((size_t)(t->g.n_sectors > 0 ? t->g.n_sectors : 1) * 4);
   const size_t ctl_bytes = off;
   s.srt = (int4*)take((size_t)n * 16 + 64);
-  s.row_org = (int2*)take((size_t)R * sizeof(int2));
   s.bin_start = (uint32_t*)take((size_t)R * t->g.nb_stride * 4);
   s.link_up = (int32_t*)take((size_t)n * 4);
   s.link_dn = (int32_t*)take((size_t)n * 4);
@@ -187,27 +187,25 @@ int tpc_tracker_create(const tpc_geometry_t* geo, const tpc_field_t* field, tpc_
   g.shift_y = ceil_log2(2 * (prm.w_y > gy ? prm.w_y : gy) + 1);
   g.shift_z = ceil_log2(2 * (prm.w_z > gz ? prm.w_z : gz) + 1);
   const int64_t z_units = (int64_t)ceil(geo->z_extent_cm * geo->units_per_cm);
-  int* ny_host = new (std::nothrow) int[nr];
   float* dx_host = new (std::nothrow) float[nr];
-  if (!ny_host || !dx_host) {
-    delete[] ny_host;
-    delete[] dx_host;
+  if (!dx_host) {
     delete t;
     return TPC_ERR_NOMEM;
   }
+  double yh_max = 0;
+  for (int r = 0; r < nr; ++r) {
+    const double yh = geo->y_half_cm > 0 ? geo->y_half_cm : geo->row_x[r] * geo->y_half_tan;
+    if (yh > yh_max) yh_max = yh;
+  }
+  const int64_t y_units = (int64_t)ceil(2.0 * yh_max * geo->units_per_cm);
+  g.org_y = -(int32_t)(y_units / 2);
   int64_t nb;
   for (;;) {   // shrink the bin count until one row's histogram fits the shared memory of a CTA
-    int ny_max = 1;
-    for (int r = 0; r < nr; ++r) {
-      const double yh = geo->y_half_cm > 0 ? geo->y_half_cm : geo->row_x[r] * geo->y_half_tan;
-      const int64_t span = (int64_t)ceil(2.0 * yh * geo->units_per_cm);
-      ny_host[r] = (int)((span >> g.shift_y) + 2);
-      if (ny_host[r] > ny_max) ny_max = ny_host[r];
-    }
+    g.ny = (int)((y_units >> g.shift_y) + 1);
     g.nz = (int)((z_units >> g.shift_z) + 2);
-    nb = (int64_t)ny_max * g.nz;
+    nb = (int64_t)g.ny * g.nz;
     if (nb + 1 <= 48 * 1024) break;
-    if (g.nz > ny_max) ++g.shift_z; else ++g.shift_y;
+    if (g.nz > g.ny) ++g.shift_z; else ++g.shift_y;
   }
   g.nb_stride = (int)align_up((size_t)nb + 1, 4);
   for (int r = 0; r < nr; ++r) dx_host[r] = (float)(geo->row_x[r + 1 < nr ? r + 1 : r] - geo->row_x[r + 1 < nr ? r : r - 1]);
@@ -225,19 +223,16 @@ int tpc_tracker_create(const tpc_geometry_t* geo, const tpc_field_t* field, tpc_
   g.cq = (float)(prm.cq_per_tesla * field->bz_tesla);
   for (int k = 0; k < 5; ++k) g.c_reset[k] = (float)prm.c_reset[k];
 
-  // geometry tables in one small device blob: row_x (double) | row_dx (float) | ny_row (int)
-  const size_t o_dx = align_up((size_t)nr * 8, 256), o_ny = o_dx + align_up((size_t)nr * 4, 256);
-  const size_t blob = o_ny + align_up((size_t)nr * 4, 256);
+  // geometry tables in one small device blob: row_x (double) | row_dx (float)
+  const size_t o_dx = align_up((size_t)nr * 8, 256);
+  const size_t blob = o_dx + align_up((size_t)nr * 4, 256);
   int rc = TPC_OK;
   e = cudaMalloc(&t->geom_blob, blob);
   if (e == cudaSuccess) e = cudaMemcpy(t->geom_blob, geo->row_x, (size_t)nr * 8, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy((char*)t->geom_blob + o_dx, dx_host, (size_t)nr * 4, cudaMemcpyHostToDevice);
-  if (e == cudaSuccess) e = cudaMemcpy((char*)t->geom_blob + o_ny, ny_host, (size_t)nr * 4, cudaMemcpyHostToDevice);
-  delete[] ny_host;
   delete[] dx_host;
   g.row_x = (const double*)t->geom_blob;
   g.row_dx = (const float*)((char*)t->geom_blob + o_dx);
-  g.ny_row = (const int32_t*)((char*)t->geom_blob + o_ny);
   if (e == cudaSuccess) e = setup_a1_attributes(t);
   if (e == cudaSuccess) e = setup_a4_attributes(t);
   for (int k = 0; k < TIMING_SETS * 6 && e == cudaSuccess; ++k) e = cudaEventCreate(&t->ev[k]);
@@ -281,6 +276,7 @@ int tpc_track(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* strea
   TPC_CUDA(t, cudaMemsetAsync(t->s.ctl, 0, t->ctl_bytes, st));
   cudaEvent_t* ev = t->ev + (t->timed_calls % TIMING_SETS) * 6;   // ring of event sets, one per timed call
   if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[0], st));
+  TPC_CUDA(t, launch_a0_origin(t, cl->z, cl->row_offsets, n, st));
   TPC_CUDA(t, launch_a1_grid(t, cl->y, cl->z, cl->row_offsets, n, st));
   if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[1], st));
   TPC_CUDA(t, launch_a2_neighbours(t, cl->row_offsets, n, st));
@@ -353,7 +349,7 @@ int tpc_track_host(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* 
 
 int64_t tpc_scratch_bytes(const tpc_tracker_t* t) { return t ? (int64_t)(t->arena_bytes + t->host_arena_bytes) : 0; }
 
-int tpc_launches_per_call(const tpc_tracker_t* t) { return t ? 5 : 0; }
+int tpc_launches_per_call(const tpc_tracker_t* t) { return t ? 6 : 0; }
 
 int tpc_set_stage_timing(tpc_tracker_t* t, int enable) {
   if (!t) return TPC_ERR_ARG;

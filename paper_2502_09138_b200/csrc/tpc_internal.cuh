@@ -9,10 +9,10 @@
 // Device view of geometry + parameters, passed by value to every kernel.
 struct DevGeom {
   int32_t n_sectors, n_rows;
-  // a1 grid shape: bin = iz * ny_row[r] + iy, iy = (y - org.y) >> shift_y clamped to
-  // [0, ny-1], iz likewise with nz; org = per-row (min y, min z) of the data.
-  int32_t shift_y, shift_z, nz, nb_stride;
-  const int32_t* ny_row;   // [n_rows]
+  // a1 grid shape: bin = iz * ny + iy, iy = (y - org_y) >> shift_y clamped to [0, ny-1],
+  // iz = (z - org_z[sector]) >> shift_z clamped to [0, nz-1].  org_y comes from the geometry (minus the widest row's
+  // half width), org_z is the smallest z of the sector's clusters (a0), so drift offsets cost no bins.
+  int32_t shift_y, shift_z, ny, nz, nb_stride, org_y;
   const double* row_x;     // [n_rows] cm
   const float* row_dx;     // [n_rows] row_x[r+1] - row_x[r], rounded once from double (last entry repeats)
   // a2 / a3
@@ -36,7 +36,7 @@ struct DevCtl {
 struct Scratch {
   // a1
   int4* srt;                // clusters in bin order inside each row: (y, z, cluster id, 0) -- one 16-B load per candidate
-  int2* row_org;            // per (sector,row) grid origin
+  uint32_t* sec_key;        // [n_sectors] a0: order-preserving key of the sector's smallest z (zeroed per call)
   uint32_t* bin_start;      // [R * nb_stride] global sorted index of the first cluster of each bin (+ sentinel)
   // a2 / a3 (id space)
   int32_t *link_up, *link_dn;
@@ -83,9 +83,15 @@ struct tpc_tracker {
 
 constexpr int A3_TILE = 1024;   // ids per a3 block (256 threads x 4)
 constexpr int A5_TILE = 128;    // tracklets per a5 block
+// a0 keeps the smallest z of a sector as max over key(z) = ~(z ^ 0x80000000): zero-initialised memory then means
+// "no cluster yet" and atomicMax does the reduction.
+__host__ __device__ __forceinline__ uint32_t zmin_key(int32_t z) { return ~((uint32_t)z ^ 0x80000000u); }
+__host__ __device__ __forceinline__ int32_t zmin_from_key(uint32_t k) { return k ? (int32_t)(~k ^ 0x80000000u) : 0; }
+
 constexpr int TL_REC_V4 = 6;    // float4 words per tracklet record
 
 // launchers (each in its own .cu)
+cudaError_t launch_a0_origin(const tpc_tracker* t, const int32_t* z, const uint32_t* ro, int64_t n, cudaStream_t st);
 cudaError_t launch_a1_grid(const tpc_tracker* t, const int32_t* y, const int32_t* z, const uint32_t* ro, int64_t n, cudaStream_t st);
 cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64_t n, cudaStream_t st);
 cudaError_t launch_a3_seeds(const tpc_tracker* t, const int32_t* y, const int32_t* z, const uint32_t* ro, int64_t n, cudaStream_t st);
