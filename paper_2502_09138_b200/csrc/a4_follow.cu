@@ -228,6 +228,32 @@ __device__ __forceinline__ BinRanges load_ranges(const DevGeom& g, const uint32_
 
 __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
+// Predicated loads that write straight into their destination registers (the old value stays when `pred` is
+// false).  Written as PTX because `if (c) v = *p;` compiles to load-into-temporary + select, and the select waits
+// for the load right there -- which would turn every gather that is issued one step ahead into a blocking one.
+__device__ __forceinline__ void ld_v4_if(int4& v, const int4* p, bool pred) {
+  asm volatile("{ .reg .pred q; setp.ne.s32 q, %4, 0; @q ld.global.nc.v4.s32 {%0,%1,%2,%3}, [%5]; }"
+               : "+r"(v.x), "+r"(v.y), "+r"(v.z), "+r"(v.w) : "r"((int)pred), "l"(p));
+}
+__device__ __forceinline__ void ld_u32_if(uint32_t& v, const uint32_t* p, bool pred) {
+  asm volatile("{ .reg .pred q; setp.ne.s32 q, %1, 0; @q ld.global.nc.u32 %0, [%2]; }" : "+r"(v) : "r"((int)pred), "l"(p));
+}
+// .cg: the hit table is written by this kernel, so it is read from L2, never from a stale L1 line
+__device__ __forceinline__ void ld_cg_s32_if(int& v, const int32_t* p, bool pred) {
+  asm volatile("{ .reg .pred q; setp.ne.s32 q, %1, 0; @q ld.global.cg.s32 %0, [%2]; }" : "+r"(v) : "r"((int)pred), "l"(p) : "memory");
+}
+
+// Bin starts of window w of the row whose bin_start segment is bs, loaded into q iff pred.
+__device__ __forceinline__ void load_ranges_if(const DevGeom& g, const uint32_t* __restrict__ bs, const Window& w,
+                                               BinRanges& q, bool pred) {
+  const bool two = pred && w.iz_hi != w.iz_lo;
+  if (pred && !two) q.a1 = q.b1 = 0;
+  ld_u32_if(q.a0, bs + w.iz_lo * g.ny + w.iy_lo, pred);
+  ld_u32_if(q.b0, bs + w.iz_lo * g.ny + w.iy_hi + 1, pred);
+  ld_u32_if(q.a1, bs + w.iz_hi * g.ny + w.iy_lo, two);
+  ld_u32_if(q.b1, bs + w.iz_hi * g.ny + w.iy_hi + 1, two);
+}
+
 // P17/P21: among the candidates minimise (d, id), d = dy^2/(Cyy + sy2) + dz^2/(Czz + sz2), restricted to
 // |dy| <= gate_y and |dz| <= gate_z (cm); accept iff d < gate_d.
 __device__ __forceinline__ Found search_row(const DevGeom& g, const BinRanges& q, float py, float pz, float vy, float vz,
@@ -242,7 +268,8 @@ __device__ __forceinline__ Found search_row(const DevGeom& g, const BinRanges& q
     int4 nx = srt[n0 ? q.a0 : q.a1];
     for (uint32_t t = 0; t < total; ++t) {   // one flat loop over both z-bins
       const int4 c = nx;
-      if (t + 1 < total) nx = srt[t + 1 < n0 ? q.a0 + t + 1 : q.a1 + (t + 1 - n0)];   // next one in flight
+      const uint32_t tn = min(t + 1, total - 1);   // next one in flight (the last iteration re-reads itself)
+      nx = srt[tn < n0 ? q.a0 + tn : q.a1 + (tn - n0)];
       const float cy = (float)(c.x - y0) * g.inv_units, cz = (float)(c.y - z0) * g.inv_units;
       const float dy = cy - py, dz = cz - pz;
       if (fabsf(dy) > g.gate_y || fabsf(dz) > g.gate_z) continue;
@@ -374,39 +401,34 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
 
     // ---- hit known before the transport (chain link or recorded hit) ----
     int hid = -1;
-    bool t1_old = false;   // t1_val was loaded in an earlier step (safe to consume without waiting)
     if (mode == M_LINK) hid = h;
+    int nid = -1;   // hit whose record the next step will want
     if (mode == M_TABLE) {
-      if (t1_row == trow) hid = t1_val;
-      else if (t2_row == trow) hid = t2_val;
-      else hid = __ldcg(tab + trow);
-      // keep the entries of the next two rows down in flight
+      // rolling two-deep pipeline over the table on the way down: t1 = entry of this row, t2 = of the next
+      if (t1_row != trow) {
+        t1_val = -1;
+        ld_cg_s32_if(t1_val, tab + trow, true);
+      }
+      hid = t1_val;
       const int n1 = trow - 1, n2 = trow - 2;
-      int v1 = -1, v2 = -1;
-      bool v1_old = false;
-      if (n1 >= r0) {
-        if (t1_row == n1) { v1 = t1_val; v1_old = true; }
-        else if (t2_row == n1) { v1 = t2_val; v1_old = true; }
-        else v1 = __ldcg(tab + n1);
-      }
-      if (n2 >= r0) v2 = (t2_row == n2) ? t2_val : __ldcg(tab + n2);
-      t1_row = n1 >= r0 ? n1 : -1;
-      t1_val = v1;
+      const bool have1 = t2_row == n1;
+      t1_val = t2_val;
+      t1_row = n1;
+      if (have1) nid = t1_val;   // loaded in an earlier step: safe to consume without waiting
+      ld_cg_s32_if(t1_val, tab + n1, !have1 && n1 >= r0);
+      if (n1 < r0) t1_row = -1;
       t2_row = n2 >= r0 ? n2 : -1;
-      t2_val = v2;
-      t1_old = v1_old;
+      ld_cg_s32_if(t2_val, tab + n2, n2 >= r0);
     }
-    int4 rc = make_int4(y0, z0, -1, -1);
-    if (hid >= 0) rc = (hid == rcn_id) ? rcn : rec[hid];
+    int4 rc = rcn;
+    if (hid < 0) rc = make_int4(y0, z0, -1, -1);
+    ld_v4_if(rc, rec + hid, hid >= 0 && hid != rcn_id);
     // next step's record: the chain's next hit, or the recorded hit of the next row down
+    if (mode == M_LINK) nid = rc.z;
     {
-      int nid = -1;
-      if (mode == M_LINK) nid = rc.z;
-      if (mode == M_TABLE && t1_old) nid = t1_val;
-      if (nid >= 0 && nid != rcn_id) {
-        rcn_id = nid;
-        rcn = rec[nid];
-      }
+      const bool fetch = nid >= 0 && nid != rcn_id;
+      if (fetch) rcn_id = nid;
+      ld_v4_if(rcn, rec + nid, fetch);
     }
     // candidates of this step's search: bin ranges were loaded last step; touch the candidates now
     const uint32_t* bs = bin_start + (size_t)(sec_base + trow) * g.nb_stride;
@@ -425,7 +447,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
         const float vy = (float)C.c00 + g.sy2, vz = (float)C.c11 + g.sz2;
         const Window w = search_window(g, py, pz, vy, vz, y0, z0, org_z);
         BinRanges q = pq;
-        if (w.key_y() != pk_y || w.key_z(row) != pk_z) q = load_ranges(g, bs, w);
+        load_ranges_if(g, bs, w, q, w.key_y() != pk_y || w.key_z(row) != pk_z);
         const Found f = search_row(g, q, py, pz, vy, vz, y0, z0, srt);
         hid = f.id;
         ym = f.y;
@@ -460,18 +482,20 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
     // ---- bin ranges of the next step's search window, at the extrapolated position ----
     {
       int nrow = -1;
-      float ndx = 0.f;
-      if (((phase == PH_A && h < 0) || phase == PH_B) && row + 1 < nr) { nrow = row + 1; ndx = s_row_dx[row]; }
-      if (phase == PH_CD && row - 1 < r0 && row >= 1) { nrow = row - 1; ndx = -s_row_dx[row - 1]; }
-      if (nrow >= 0) {
-        const float ps = (float)p.s;
-        const float ic = rsqrtf(fmaxf(1.f - ps * ps, 0.05f));
-        const float py = (float)p.y + ndx * ps * ic, pz = (float)p.z + ndx * (float)p.t * ic;
-        const Window w = search_window(g, py, pz, (float)C.c00 + g.sy2, (float)C.c11 + g.sz2, y0, z0, org_z);
+      if (((phase == PH_A && h < 0) || phase == PH_B) && row + 1 < nr) nrow = row + 1;
+      if (phase == PH_CD && row - 1 < r0 && row >= 1) nrow = row - 1;
+      const bool pred = nrow >= 0;
+      const int srow = pred ? nrow : row;
+      const float ndx = srow > row ? s_row_dx[row] : (srow < row ? -s_row_dx[srow] : 0.f);
+      const float ps = (float)p.s;
+      const float ic = rsqrtf(fmaxf(1.f - ps * ps, 0.05f));
+      const float py = (float)p.y + ndx * ps * ic, pz = (float)p.z + ndx * (float)p.t * ic;
+      const Window w = search_window(g, py, pz, (float)C.c00 + g.sy2, (float)C.c11 + g.sz2, y0, z0, org_z);
+      if (pred) {
         pk_y = w.key_y();
         pk_z = w.key_z(nrow);
-        pq = load_ranges(g, bin_start + (size_t)(sec_base + nrow) * g.nb_stride, w);
       }
+      load_ranges_if(g, bin_start + (size_t)(sec_base + srow) * g.nb_stride, w, pq, pred);
     }
 
     // ---- tracklets that ended: record, padding of the hit table and ownership votes ----
