@@ -231,9 +231,15 @@ __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefe
 // Predicated loads that write straight into their destination registers (the old value stays when `pred` is
 // false).  Written as PTX because `if (c) v = *p;` compiles to load-into-temporary + select, and the select waits
 // for the load right there -- which would turn every gather that is issued one step ahead into a blocking one.
-__device__ __forceinline__ void ld_v4_if(int4& v, const int4* p, bool pred) {
-  asm volatile("{ .reg .pred q; setp.ne.s32 q, %4, 0; @q ld.global.nc.v4.s32 {%0,%1,%2,%3}, [%5]; }"
-               : "+r"(v.x), "+r"(v.y), "+r"(v.z), "+r"(v.w) : "r"((int)pred), "l"(p));
+// (y, z, up link) of a cluster record as three scalar loads: a predicated 128-bit load needs an aligned register
+// quad, which ptxas then copies out of right behind the load (and so waits for it); scalars land in place.
+struct Rec3 {
+  int y, z, up;
+};
+__device__ __forceinline__ void ld_rec_if(Rec3& v, const int4* p, bool pred) {
+  asm volatile("{ .reg .pred q; setp.ne.s32 q, %3, 0; @q ld.global.nc.s32 %0, [%4]; @q ld.global.nc.s32 %1, [%4+4];"
+               " @q ld.global.nc.s32 %2, [%4+8]; }"
+               : "+r"(v.y), "+r"(v.z), "+r"(v.up) : "r"((int)pred), "l"(p));
 }
 __device__ __forceinline__ void ld_u32_if(uint32_t& v, const uint32_t* p, bool pred) {
   asm volatile("{ .reg .pred q; setp.ne.s32 q, %1, 0; @q ld.global.nc.u32 %0, [%2]; }" : "+r"(v) : "r"((int)pred), "l"(p));
@@ -329,7 +335,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
   cov_reset(g, C);
   // gathers issued one step ahead (a mismatch of the tag only costs the direct load)
   int rcn_id = -1;                 // record of cluster rcn_id
-  int4 rcn = make_int4(0, 0, -1, -1);
+  Rec3 rcn = {0, 0, -1};
   int t1_row = -1, t1_val = -1;    // table entries of the next two rows on the way down
   int t2_row = -1, t2_val = -1;
   uint32_t pk_y = 0xFFFFFFFFu, pk_z = 0xFFFFFFFFu;   // bin ranges of the window keyed (pk_y, pk_z)
@@ -358,7 +364,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
         const int4 c0 = rec[h];
         const int4 c1 = rec[c0.z];
         rcn_id = h;
-        rcn = c0;
+        rcn.y = c0.x; rcn.z = c0.y; rcn.up = c0.z;
         y0 = c0.x;
         z0 = c0.y;
         const float dxr = s_row_dx[r0];
@@ -420,15 +426,15 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
       t2_row = n2 >= r0 ? n2 : -1;
       ld_cg_s32_if(t2_val, tab + n2, n2 >= r0);
     }
-    int4 rc = rcn;
-    if (hid < 0) rc = make_int4(y0, z0, -1, -1);
-    ld_v4_if(rc, rec + hid, hid >= 0 && hid != rcn_id);
+    Rec3 rc = rcn;
+    if (hid < 0) { rc.y = y0; rc.z = z0; rc.up = -1; }
+    ld_rec_if(rc, rec + hid, hid >= 0 && hid != rcn_id);
     // next step's record: the chain's next hit, or the recorded hit of the next row down
-    if (mode == M_LINK) nid = rc.z;
+    if (mode == M_LINK) nid = rc.up;
     {
       const bool fetch = nid >= 0 && nid != rcn_id;
       if (fetch) rcn_id = nid;
-      ld_v4_if(rcn, rec + nid, fetch);
+      ld_rec_if(rcn, rec + nid, fetch);
     }
     // candidates of this step's search: bin ranges were loaded last step; touch the candidates now
     const uint32_t* bs = bin_start + (size_t)(sec_base + trow) * g.nb_stride;
@@ -441,7 +447,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
     if (ok && tr) ok = transport<true>(g, dx, p, C);
     if (ok) {
       row = trow;
-      float ym = (float)(rc.x - y0) * g.inv_units, zm = (float)(rc.y - z0) * g.inv_units;
+      float ym = (float)(rc.y - y0) * g.inv_units, zm = (float)(rc.z - z0) * g.inv_units;
       if (mode == M_SEARCH) {
         const float py = (float)p.y, pz = (float)p.z;
         const float vy = (float)C.c00 + g.sy2, vz = (float)C.c11 + g.sz2;
@@ -466,7 +472,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
         tab[row] = hid;
         rmax = row;
         ++nh;
-        h = rc.z;
+        h = rc.up;
       }
       if (mode != M_NONE && hid >= 0) chi2 += update(g, p, C, ym, zm);
       if (ph == PH_INIT) phase = PH_A;
@@ -521,13 +527,18 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
         // P24, P26: owner(h) = surviving tracklet with the most hits, ties -> smallest rank
         const uint32_t word = snh >= g.n_min_tracklet ? (((uint32_t)snh << 24) | (0xFFFFFFu - (uint32_t)si)) : 0u;
         int32_t* out = tl_hits + (size_t)si * nr;
-        for (int r = lane; r < nr; r += 32) {
-          if (r >= smin && r <= smax) {
-            const int v = __ldcg(out + r);
-            if (word && v >= 0) atomicMax(&owner[v], word);
-          } else {
-            out[r] = -1;
-          }
+        int v[8];   // n_rows <= 255: all loads of the table first, then the votes
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const int r = k * 32 + lane;
+          v[k] = -1;
+          ld_cg_s32_if(v[k], out + r, r >= smin && r <= smax);
+        }
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const int r = k * 32 + lane;
+          if (r < nr && (r < smin || r > smax)) out[r] = -1;
+          if (word && v[k] >= 0) atomicMax(&owner[v[k]], word);
         }
       }
       if (phase == PH_DONE) phase = PH_IDLE;
