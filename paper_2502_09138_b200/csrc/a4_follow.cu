@@ -342,6 +342,8 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
   BinRanges pq = {0, 0, 0, 0};
 
   while (true) {
+    uint32_t nk_y, nk_z;   // next step's window key and bin ranges (loaded during this step)
+    BinRanges npq;
     // ---- refill free lanes from the seed queue ----
     const bool want = phase == PH_IDLE && lane < lanes_used && !exhausted;
     const unsigned idle = __ballot_sync(FULL, want);
@@ -436,11 +438,31 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
       if (fetch) rcn_id = nid;
       ld_rec_if(rcn, rec + nid, fetch);
     }
-    // candidates of this step's search: bin ranges were loaded last step; touch the candidates now
+    // candidates of this step's search: their bin ranges were loaded during the last step; touch them now
     const uint32_t* bs = bin_start + (size_t)(sec_base + trow) * g.nb_stride;
     if (mode == M_SEARCH && (pk_z >> 24) == (uint32_t)trow) {
       if (pq.b0 > pq.a0) prefetch_l1(srt + pq.a0);
       if (pq.b1 > pq.a1) prefetch_l1(srt + pq.a1);
+    }
+    // bin ranges of the NEXT step's search window, at the position extrapolated from the state before this step
+    // (issued here so that this step's transport and update hide the latency; ptxas waits for loads that are in
+    // flight at the loop's back edge, so nothing may be issued at the end of the body)
+    {
+      int nrow = -1;
+      if (((ph == PH_A && rc.up < 0) || ph == PH_B) && trow + 1 < nr) nrow = trow + 1;
+      if ((ph == PH_CS || ph == PH_CD) && trow - 1 < r0 && trow >= 1) nrow = trow - 1;
+      const bool pred = nrow >= 0;
+      const int srow = pred ? nrow : row;
+      const float ndx = (float)(s_row_x[srow] - s_row_x[row]);
+      const float ps = (float)p.s;
+      const float ic = rsqrtf(fmaxf(1.f - ps * ps, 0.05f));
+      const float py = (float)p.y + ndx * ps * ic, pz = (float)p.z + ndx * (float)p.t * ic;
+      const Window w = search_window(g, py, pz, (float)C.c00 + g.sy2, (float)C.c11 + g.sz2, y0, z0, org_z);
+      BinRanges nq = pq;
+      load_ranges_if(g, bin_start + (size_t)(sec_base + srow) * g.nb_stride, w, nq, pred);
+      nk_y = pred ? w.key_y() : pk_y;
+      nk_z = pred ? w.key_z(nrow) : pk_z;
+      npq = nq;
     }
 
     bool ok = ph != PH_IDLE && ph != PH_DONE;
@@ -485,24 +507,9 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
       if (ph == PH_FIN) phase = PH_DONE;
     }
 
-    // ---- bin ranges of the next step's search window, at the extrapolated position ----
-    {
-      int nrow = -1;
-      if (((phase == PH_A && h < 0) || phase == PH_B) && row + 1 < nr) nrow = row + 1;
-      if (phase == PH_CD && row - 1 < r0 && row >= 1) nrow = row - 1;
-      const bool pred = nrow >= 0;
-      const int srow = pred ? nrow : row;
-      const float ndx = srow > row ? s_row_dx[row] : (srow < row ? -s_row_dx[srow] : 0.f);
-      const float ps = (float)p.s;
-      const float ic = rsqrtf(fmaxf(1.f - ps * ps, 0.05f));
-      const float py = (float)p.y + ndx * ps * ic, pz = (float)p.z + ndx * (float)p.t * ic;
-      const Window w = search_window(g, py, pz, (float)C.c00 + g.sy2, (float)C.c11 + g.sz2, y0, z0, org_z);
-      if (pred) {
-        pk_y = w.key_y();
-        pk_z = w.key_z(nrow);
-      }
-      load_ranges_if(g, bin_start + (size_t)(sec_base + srow) * g.nb_stride, w, pq, pred);
-    }
+    pk_y = nk_y;
+    pk_z = nk_z;
+    pq = npq;
 
     // ---- tracklets that ended: record, padding of the hit table and ownership votes ----
     const unsigned done = __ballot_sync(FULL, phase == PH_DONE);
