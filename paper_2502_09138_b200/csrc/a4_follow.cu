@@ -195,17 +195,19 @@ struct Window {
 
 __device__ __forceinline__ Window search_window(const DevGeom& g, float py, float pz, float vy, float vz, int y0, int z0,
                                                 int org_z) {
-  const float hy = fminf(g.gate_y, sqrtf(g.gate_d * vy) * 1.002f), hz = fminf(g.gate_z, sqrtf(g.gate_d * vz) * 1.002f);
-  const float lim = 1.0e9f;   // clamp against int overflow
-  const int ylo = y0 + (int)fminf(fmaxf(floorf((py - hy) * g.units) - 2.f, -lim), lim);
-  const int yhi = y0 + (int)fminf(fmaxf(ceilf((py + hy) * g.units) + 2.f, -lim), lim);
-  const int zlo = z0 + (int)fminf(fmaxf(floorf((pz - hz) * g.units) - 2.f, -lim), lim);
-  const int zhi = z0 + (int)fminf(fmaxf(ceilf((pz + hz) * g.units) + 2.f, -lim), lim);
+  // half widths in units: gate_d*v*rsqrt(gate_d*v) = sqrt(gate_d*v) to 2 ulp, inside the 0.2 % margin.
+  // float -> int conversions saturate; a state so far off that y0 + (...) wraps has no cluster within the gate
+  // (coordinates stay within +-2^24 units of the extents), and the clamps keep every index in range regardless.
+  const float ay = g.gate_d * vy, az = g.gate_d * vz;
+  const float hy = fminf(g.gate_y, ay * rsqrtf(ay) * 1.002f) * g.units + 2.f;
+  const float hz = fminf(g.gate_z, az * rsqrtf(az) * 1.002f) * g.units + 2.f;
+  const float cy = py * g.units, cz = pz * g.units;
+  const int oy = y0 - g.org_y, oz = z0 - org_z;
   Window w;
-  w.iy_lo = clampi((ylo - g.org_y) >> g.shift_y, 0, g.ny - 1);
-  w.iy_hi = clampi((yhi - g.org_y) >> g.shift_y, 0, g.ny - 1);
-  w.iz_lo = clampi((zlo - org_z) >> g.shift_z, 0, g.nz - 1);
-  w.iz_hi = clampi((zhi - org_z) >> g.shift_z, 0, g.nz - 1);   // bins are >= 2 gate_z wide: iz_hi <= iz_lo + 1
+  w.iy_lo = min(max((__float2int_rd(cy - hy) + oy) >> g.shift_y, 0), g.ny - 1);
+  w.iy_hi = min(max((__float2int_ru(cy + hy) + oy) >> g.shift_y, 0), g.ny - 1);
+  w.iz_lo = min(max((__float2int_rd(cz - hz) + oz) >> g.shift_z, 0), g.nz - 1);
+  w.iz_hi = min(max((__float2int_ru(cz + hz) + oz) >> g.shift_z, 0), g.nz - 1);   // bins >= 2 gate_z: iz_hi <= iz_lo + 1
   return w;
 }
 
