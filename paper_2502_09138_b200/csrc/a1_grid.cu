@@ -19,93 +19,170 @@ constexpr int A1_THREADS = 128;
 __device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
 
 constexpr int A0_THREADS = 256;
+constexpr int A0_PER_THREAD = 8;
 
+// grid = (chunks, n_sectors): block (c, s) reduces its slice of sector s's contiguous cluster range.
 __global__ void __launch_bounds__(A0_THREADS)
-a0_origin_kernel(const DevGeom g, int64_t R, const int32_t* __restrict__ z, const uint32_t* __restrict__ ro,
+a0_origin_kernel(const DevGeom g, const int32_t* __restrict__ z, const uint32_t* __restrict__ ro,
                  uint32_t* __restrict__ sec_key) {
-  const int64_t sr = (int64_t)blockIdx.x * (A0_THREADS / 32) + (threadIdx.x >> 5);
-  if (sr >= R) return;
-  const unsigned lane = threadIdx.x & 31;
-  const uint32_t a = ro[sr], b = ro[sr + 1];
-  if (a == b) return;
+  __shared__ int red[A0_THREADS / 32];
+  for (int sec = blockIdx.y; sec < g.n_sectors; sec += gridDim.y) {   // block-uniform loop (gridDim.y caps at 65535)
+  const uint32_t a = ro[(size_t)sec * g.n_rows], b = ro[(size_t)(sec + 1) * g.n_rows];
   int zmin = INT32_MAX;
-  for (uint32_t i = a + lane; i < b; i += 32) zmin = min(zmin, z[i]);
+  for (uint32_t base = a + blockIdx.x * (A0_THREADS * A0_PER_THREAD); base < b;
+       base += gridDim.x * (A0_THREADS * A0_PER_THREAD)) {
+    int v[A0_PER_THREAD];
+#pragma unroll
+    for (int k = 0; k < A0_PER_THREAD; ++k) {
+      const uint32_t i = base + k * A0_THREADS + threadIdx.x;
+      v[k] = i < b ? z[i] : INT32_MAX;
+    }
+#pragma unroll
+    for (int k = 0; k < A0_PER_THREAD; ++k) zmin = min(zmin, v[k]);
+  }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) zmin = min(zmin, __shfl_xor_sync(0xffffffffu, zmin, o));
-  if (lane == 0) atomicMax(&sec_key[sr / g.n_rows], zmin_key(zmin));
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = zmin;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int w = 0; w < A0_THREADS / 32; ++w) zmin = min(zmin, red[w]);
+    if (zmin != INT32_MAX) atomicMax(&sec_key[sec], zmin_key(zmin));
+  }
+  __syncthreads();   // red[] is reused by the next sector
+  }
 }
 
+// G threads per (sector,row): 32 (a warp per row, 4 rows per block, warp-level sync only) for sparse rows, the whole
+// block for long rows.  Bins far outnumber clusters in sparse events, so the per-bin work (zero, scan, write) is
+// what a row costs; a warp does it with shuffles and no block barrier.
+template <int G>
+__device__ __forceinline__ void group_sync() {
+  if (G == 32) __syncwarp(); else __syncthreads();
+}
+
+template <int G>
 __global__ void __launch_bounds__(A1_THREADS)
-a1_grid_kernel(const DevGeom g, const int32_t* __restrict__ y, const int32_t* __restrict__ z,
+a1_grid_kernel(const DevGeom g, int64_t R, const int32_t* __restrict__ y, const int32_t* __restrict__ z,
                const uint32_t* __restrict__ ro, const uint32_t* __restrict__ sec_key, int4* __restrict__ srt,
                uint32_t* __restrict__ bin_start) {
-  extern __shared__ uint32_t hist[];
+  extern __shared__ uint32_t hist_all[];
   __shared__ uint32_t wsum[33];
-  const int sr = blockIdx.x;
+  const int grp = threadIdx.x / G, gt = threadIdx.x % G;
+  const int64_t sr = (int64_t)blockIdx.x * (A1_THREADS / G) + grp;
+  if (sr >= R) return;   // G == 32 only (whole warps); with G == A1_THREADS the grid is exactly R
+  uint32_t* const hist = hist_all + (size_t)grp * g.nb_stride;
   const uint32_t a = ro[sr], b = ro[sr + 1];
   const int ny = g.ny, nz = g.nz;
   const int nb = ny * nz;
-  const int tid = threadIdx.x;
   const int ymin = g.org_y, zmin = zmin_from_key(sec_key[sr / g.n_rows]);
-  for (int k = tid; k < nb; k += A1_THREADS) hist[k] = 0;
-  __syncthreads();
+  for (int k = gt; k < nb; k += G) hist[k] = 0;
+  group_sync<G>();
 
-  // pass 1: histogram
-  for (uint32_t i = a + tid; i < b; i += A1_THREADS) {
-    int iy = clampi((y[i] - ymin) >> g.shift_y, 0, ny - 1);
-    int iz = clampi((z[i] - zmin) >> g.shift_z, 0, nz - 1);
+  // pass 1: histogram (the bin index of up to 4 clusters per thread is kept for pass 2)
+  constexpr int KEEP = 4;
+  int bin[KEEP];
+#pragma unroll
+  for (int k = 0; k < KEEP; ++k) {
+    const uint32_t i = a + k * G + gt;
+    bin[k] = -1;
+    if (i < b) {
+      const int iy = clampi((y[i] - ymin) >> g.shift_y, 0, ny - 1);
+      const int iz = clampi((z[i] - zmin) >> g.shift_z, 0, nz - 1);
+      bin[k] = iz * ny + iy;
+      atomicAdd(&hist[bin[k]], 1u);
+    }
+  }
+  for (uint32_t i = a + KEEP * G + gt; i < b; i += G) {
+    const int iy = clampi((y[i] - ymin) >> g.shift_y, 0, ny - 1);
+    const int iz = clampi((z[i] - zmin) >> g.shift_z, 0, nz - 1);
     atomicAdd(&hist[iz * ny + iy], 1u);
   }
-  __syncthreads();
+  group_sync<G>();
 
   // exclusive scan over bins: each thread owns a contiguous chunk
-  const int chunk = (nb + A1_THREADS - 1) / A1_THREADS;
-  const int k0 = min(tid * chunk, nb), k1 = min(k0 + chunk, nb);
-  uint32_t s = 0;
-  for (int k = k0; k < k1; ++k) s += hist[k];
-  uint32_t total;
-  uint32_t run = block_excl_scan(s, wsum, &total);
-  uint32_t* bs = bin_start + (size_t)sr * g.nb_stride;
+  const int chunk = (nb + G - 1) / G;
+  const int k0 = min(gt * chunk, nb), k1 = min(k0 + chunk, nb);
+  uint32_t sum = 0;
+  for (int k = k0; k < k1; ++k) sum += hist[k];
+  uint32_t run;
+  if (G == 32) {
+    uint32_t inc = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+      if (gt >= o) inc += t;
+    }
+    run = inc - sum;
+  } else {
+    uint32_t total;
+    run = block_excl_scan(sum, wsum, &total);
+  }
   for (int k = k0; k < k1; ++k) {
-    uint32_t c = hist[k];
+    const uint32_t c = hist[k];
     hist[k] = run;
-    bs[k] = a + run;
     run += c;
   }
-  if (tid == 0) bs[nb] = b;
-  __syncthreads();
+  group_sync<G>();
+  uint32_t* bs = bin_start + (size_t)sr * g.nb_stride;
+  for (int k = gt; k < nb; k += G) bs[k] = a + hist[k];   // coalesced
+  if (gt == 0) bs[nb] = b;
+  group_sync<G>();
 
   // pass 2: scatter into bin order (order inside a bin is arbitrary; every consumer breaks ties by id)
-  for (uint32_t i = a + tid; i < b; i += A1_THREADS) {
-    int yi = y[i], zi = z[i];
-    int iy = clampi((yi - ymin) >> g.shift_y, 0, ny - 1);
-    int iz = clampi((zi - zmin) >> g.shift_z, 0, nz - 1);
-    uint32_t pos = a + atomicAdd(&hist[iz * ny + iy], 1u);
-    srt[pos] = make_int4(yi, zi, (int32_t)i, 0);
+#pragma unroll
+  for (int k = 0; k < KEEP; ++k) {
+    const uint32_t i = a + k * G + gt;
+    if (bin[k] >= 0) srt[a + atomicAdd(&hist[bin[k]], 1u)] = make_int4(y[i], z[i], (int32_t)i, 0);
+  }
+  for (uint32_t i = a + KEEP * G + gt; i < b; i += G) {
+    const int yi = y[i], zi = z[i];
+    const int iy = clampi((yi - ymin) >> g.shift_y, 0, ny - 1);
+    const int iz = clampi((zi - zmin) >> g.shift_z, 0, nz - 1);
+    srt[a + atomicAdd(&hist[iz * ny + iy], 1u)] = make_int4(yi, zi, (int32_t)i, 0);
   }
 }
 
 }  // namespace
 
+// rows per block and shared memory of the variant chosen for this call
+static bool a1_warp_rows(const tpc_tracker* t, int64_t n) {
+  const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
+  return t->g.nb_stride <= 4096 && n <= R * 256;   // sparse rows: a warp per row
+}
+
 size_t a1_smem_bytes(const DevGeom& g) { return (size_t)(g.nb_stride) * sizeof(uint32_t); }
 
 cudaError_t setup_a1_attributes(const tpc_tracker* t) {
-  return cudaFuncSetAttribute(a1_grid_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)a1_smem_bytes(t->g));
+  cudaError_t e = cudaFuncSetAttribute(a1_grid_kernel<A1_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)a1_smem_bytes(t->g));
+  if (e != cudaSuccess || t->g.nb_stride > 4096) return e;
+  return cudaFuncSetAttribute(a1_grid_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)(a1_smem_bytes(t->g) * (A1_THREADS / 32)));
 }
 
 cudaError_t launch_a1_grid(const tpc_tracker* t, const int32_t* y, const int32_t* z, const uint32_t* ro, int64_t n,
                            cudaStream_t st) {
   const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
   if (R == 0) return cudaSuccess;
-  a1_grid_kernel<<<(unsigned)R, A1_THREADS, a1_smem_bytes(t->g), st>>>(t->g, y, z, ro, t->s.sec_key, t->s.srt,
-                                                                        t->s.bin_start);
+  if (a1_warp_rows(t, n)) {
+    const int per = A1_THREADS / 32;
+    a1_grid_kernel<32><<<(unsigned)((R + per - 1) / per), A1_THREADS, a1_smem_bytes(t->g) * per, st>>>(
+        t->g, R, y, z, ro, t->s.sec_key, t->s.srt, t->s.bin_start);
+  } else {
+    a1_grid_kernel<A1_THREADS><<<(unsigned)R, A1_THREADS, a1_smem_bytes(t->g), st>>>(
+        t->g, R, y, z, ro, t->s.sec_key, t->s.srt, t->s.bin_start);
+  }
   return cudaGetLastError();
 }
 
 cudaError_t launch_a0_origin(const tpc_tracker* t, const int32_t* z, const uint32_t* ro, int64_t n, cudaStream_t st) {
-  const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
-  if (R == 0 || n == 0) return cudaSuccess;
-  const int per = A0_THREADS / 32;
-  a0_origin_kernel<<<(unsigned)((R + per - 1) / per), A0_THREADS, 0, st>>>(t->g, R, z, ro, t->s.sec_key);
+  if (t->g.n_sectors == 0 || n == 0) return cudaSuccess;
+  // chunks per sector from the average sector size (a sector larger than that just loops)
+  const int64_t per_block = A0_THREADS * A0_PER_THREAD;
+  int64_t chunks = (n / t->g.n_sectors + per_block - 1) / per_block;
+  if (chunks < 1) chunks = 1;
+  if (chunks > 1024) chunks = 1024;
+  a0_origin_kernel<<<dim3((unsigned)chunks, (unsigned)(t->g.n_sectors < 65535 ? t->g.n_sectors : 65535)), A0_THREADS, 0, st>>>(t->g, z, ro, t->s.sec_key);
   return cudaGetLastError();
 }

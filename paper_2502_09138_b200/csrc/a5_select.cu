@@ -10,12 +10,14 @@
 namespace {
 
 constexpr int A5_MASK_WORDS = 8;   // n_rows <= 255 (checked at create) -> at most 8 ballot words per tracklet
+constexpr int A5_UNROLL = 8;       // tracklets whose loads one warp keeps in flight
 
-// Block = A5_TILE threads = A5_TILE/32 warps, tile = A5_TILE tracklets.  Pass 1: each warp walks its 32 tracklets
-// one after the other, all lanes on one tracklet (32 rows per coalesced load of the [seed][row] hit table, one
-// owner gather per lane, ballot -> owned-hit mask kept in shared memory).  Then thread k of the block holds the
-// count of tracklet k, the block scan + look-back scan place it, and pass 2 writes the hit lists warp-wide.
-__global__ void __launch_bounds__(A5_TILE)
+// Block = max(A5_TILE, 32 * ceil(n_rows / 32)) threads, tile = A5_TILE tracklets.
+// Pass 1: warp w owns rows 32w .. 32w+31 and walks the tile's tracklets, A5_UNROLL at a time: one coalesced load of
+// the [seed][row] hit table and one owner gather per lane, ballot -> the tracklet's owned-hit mask word w in shared
+// memory.  Then thread k of the block holds the count of tracklet k, the block scan + look-back scan place it, and
+// pass 2 writes the hit lists, one warp per tracklet.
+__global__ void __launch_bounds__(256)
 a5_select_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int32_t* __restrict__ seed_start,
                  const float4* __restrict__ tl_rec, const int32_t* __restrict__ tl_hits,
                  const uint32_t* __restrict__ owner, uint64_t* __restrict__ status,
@@ -25,6 +27,7 @@ a5_select_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int32_t* __res
   __shared__ uint32_t sh_tile;
   __shared__ uint64_t sh_excl;
   __shared__ uint32_t own_mask[A5_TILE][A5_MASK_WORDS];
+  __shared__ uint32_t s_word[A5_TILE];   // packed vote word of a surviving tracklet, 0 = discarded (P24)
   __shared__ uint32_t sh_off[A5_TILE];   // output hit offset of a kept tracklet, 0xFFFFFFFF = no hit list to write
   const unsigned FULL = 0xffffffffu;
   const uint32_t n_seeds = ctl->n_seeds;
@@ -42,38 +45,56 @@ a5_select_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int32_t* __res
   if (threadIdx.x == 0) sh_tile = atomicAdd(&ctl->ticket_a5, 1u);
   __syncthreads();
   const uint32_t tile = sh_tile;
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, n_warps = blockDim.x >> 5;
   const int nr = g.n_rows;
   const int n_words = (nr + 31) >> 5;
-  const int64_t i = (int64_t)tile * A5_TILE + threadIdx.x;   // this thread's tracklet in the scans and the record
+  const int64_t t0 = (int64_t)tile * A5_TILE;
+  const int n_here = (int)min((int64_t)A5_TILE, (int64_t)n_seeds - t0);
+  const int64_t i = t0 + threadIdx.x;   // this thread's tracklet in the scans and the record
+
+  if (threadIdx.x < A5_TILE) {
+    uint32_t w = 0;
+    if (threadIdx.x < n_here) {
+      const int nh = __float_as_int(tl_rec[i * TL_REC_V4 + 1].w);
+      if (nh >= g.n_min_tracklet) w = ((uint32_t)nh << 24) | (0xFFFFFFu - (uint32_t)i);
+    }
+    s_word[threadIdx.x] = w;
+  }
+  __syncthreads();
 
   // pass 1
-  uint32_t owned = 0;
-  int first = -1, last = -1;
-  for (int t = 0; t < 32; ++t) {
-    const int64_t it = (int64_t)tile * A5_TILE + wid * 32 + t;
-    if (it >= n_seeds) break;   // warp-uniform
-    const int nh = __float_as_int(tl_rec[it * TL_REC_V4 + 1].w);
-    uint32_t cnt = 0;
-    int f = -1, l = -1;
-    if (nh >= g.n_min_tracklet) {
-      const uint32_t word = ((uint32_t)nh << 24) | (0xFFFFFFu - (uint32_t)it);
-      for (int k = 0; k < n_words; ++k) {
-        const int r = k * 32 + lane;
-        const int h = r < nr ? tl_hits[it * nr + r] : -1;
-        const unsigned m = __ballot_sync(FULL, h >= 0 && owner[h] == word);
-        if (lane == k) own_mask[wid * 32 + t][k] = m;
-        if (m) {
-          if (f < 0) f = k * 32 + __ffs(m) - 1;
-          l = k * 32 + 31 - __clz(m);
-          cnt += __popc(m);
+  if (wid < n_words) {
+    const int r = wid * 32 + lane;
+    const bool in_row = r < nr;
+    const int32_t* col = tl_hits + t0 * nr + r;
+    for (int tb = 0; tb < n_here; tb += A5_UNROLL) {
+      int h[A5_UNROLL];
+      uint32_t ow[A5_UNROLL];
+#pragma unroll
+      for (int u = 0; u < A5_UNROLL; ++u) h[u] = (in_row && tb + u < n_here) ? col[(int64_t)(tb + u) * nr] : -1;
+#pragma unroll
+      for (int u = 0; u < A5_UNROLL; ++u) ow[u] = h[u] >= 0 ? owner[h[u]] : 0u;
+#pragma unroll
+      for (int u = 0; u < A5_UNROLL; ++u) {
+        if (tb + u < n_here) {   // warp-uniform
+          const uint32_t w = s_word[tb + u];
+          const unsigned m = __ballot_sync(FULL, w != 0u && ow[u] == w);
+          if (lane == 0) own_mask[tb + u][wid] = m;
         }
       }
     }
-    if (lane == t) {
-      owned = cnt;
-      first = f;
-      last = l;
+  }
+  __syncthreads();
+  uint32_t owned = 0;
+  int first = -1, last = -1;
+  if (threadIdx.x < n_here) {
+    for (int k = 0; k < n_words; ++k) {
+      const unsigned m = own_mask[threadIdx.x][k];
+      if (m) {
+        if (first < 0) first = k * 32 + __ffs(m) - 1;
+        last = k * 32 + 31 - __clz(m);
+        owned += __popc(m);
+      }
     }
   }
   const bool keep = owned >= (uint32_t)g.n_min_owned && owned > 0;   // P27
@@ -110,18 +131,17 @@ a5_select_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int32_t* __res
     }
     if ((uint64_t)off + owned <= (uint64_t)hit_capacity) my_off = off;
   }
-  sh_off[threadIdx.x] = my_off;
-  __syncwarp();   // sh_off and own_mask rows of this warp's tracklets are written and read by this warp only
+  if (threadIdx.x < A5_TILE) sh_off[threadIdx.x] = my_off;
+  __syncthreads();
 
-  // pass 2: hit lists, ascending row
-  for (int t = 0; t < 32; ++t) {
-    const int64_t it = (int64_t)tile * A5_TILE + wid * 32 + t;
-    if (it >= n_seeds) break;
-    uint32_t w = sh_off[wid * 32 + t];
+  // pass 2: hit lists, ascending row, one warp per tracklet
+  for (int t = wid; t < n_here; t += n_warps) {
+    uint32_t w = sh_off[t];
     if (w == 0xFFFFFFFFu) continue;
+    const int32_t* src = tl_hits + (t0 + t) * nr;
     for (int k = 0; k < n_words; ++k) {
-      const unsigned m = own_mask[wid * 32 + t][k];
-      if ((m >> lane) & 1u) hit_ids[w + __popc(m & ((1u << lane) - 1u))] = tl_hits[it * nr + k * 32 + lane];
+      const unsigned m = own_mask[t][k];
+      if ((m >> lane) & 1u) hit_ids[w + __popc(m & ((1u << lane) - 1u))] = src[k * 32 + lane];
       w += __popc(m);
     }
   }
@@ -147,7 +167,8 @@ cudaError_t launch_a5_select(const tpc_tracker* t, const tpc_tracks_out_t* out, 
     return cudaGetLastError();
   }
   const unsigned blocks = (unsigned)((t->s_cap + A5_TILE - 1) / A5_TILE);
-  a5_select_kernel<<<blocks, A5_TILE, 0, st>>>(t->g, t->s.ctl, t->s.seed_start, t->s.tl_rec, t->s.tl_hits, t->s.owner,
+  const int row_threads = 32 * ((t->g.n_rows + 31) / 32);
+  a5_select_kernel<<<blocks, row_threads > A5_TILE ? row_threads : A5_TILE, 0, st>>>(t->g, t->s.ctl, t->s.seed_start, t->s.tl_rec, t->s.tl_hits, t->s.owner,
                                               t->s.scan_a5, out->tracks, out->track_capacity, out->hit_ids,
                                               out->hit_capacity, out->counts);
   return cudaGetLastError();
