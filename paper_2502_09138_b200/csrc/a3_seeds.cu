@@ -28,45 +28,82 @@ a3_seeds_kernel(const DevGeom g, int64_t n, const int32_t* __restrict__ y, const
   const uint32_t tile = sh_tile;
   const int64_t base = (int64_t)tile * A3_TILE;
 
-  bool seed[A3_ITEMS];
-  uint32_t pos[A3_ITEMS];
-  uint32_t running = 0;
+  // Each thread owns A3_ITEMS consecutive ids: every load level is issued for all items before any is used, so
+  // the gathers of one level are in flight together (the kernel is bound by their latency, not by bandwidth).
+  const int64_t h0 = base + (int64_t)threadIdx.x * A3_ITEMS;
+  int u[A3_ITEMS], d[A3_ITEMS], yy[A3_ITEMS], zz[A3_ITEMS];
+  static_assert(A3_ITEMS == 4, "one 16-byte load per array and thread");
+  const bool vec = h0 + A3_ITEMS <= n && ((((uintptr_t)y | (uintptr_t)z) & 15) == 0);   // up, dn: arena, 256-B aligned
+  if (vec) {
+    const int4 vu = *(const int4*)(up + h0), vd = *(const int4*)(dn + h0);
+    const int4 vy = *(const int4*)(y + h0), vz = *(const int4*)(z + h0);
+    u[0] = vu.x; u[1] = vu.y; u[2] = vu.z; u[3] = vu.w;
+    d[0] = vd.x; d[1] = vd.y; d[2] = vd.z; d[3] = vd.w;
+    yy[0] = vy.x; yy[1] = vy.y; yy[2] = vy.z; yy[3] = vy.w;
+    zz[0] = vz.x; zz[1] = vz.y; zz[2] = vz.z; zz[3] = vz.w;
+  } else {
+#pragma unroll
+    for (int k = 0; k < A3_ITEMS; ++k) {
+      const bool in = h0 + k < n;
+      u[k] = in ? up[h0 + k] : -1;
+      d[k] = in ? dn[h0 + k] : -1;
+      yy[k] = in ? y[h0 + k] : 0;
+      zz[k] = in ? z[h0 + k] : 0;
+    }
+  }
+  int du[A3_ITEMS], ud[A3_ITEMS];
 #pragma unroll
   for (int k = 0; k < A3_ITEMS; ++k) {
-    const int64_t h = base + k * A3_THREADS + threadIdx.x;
-    seed[k] = false;
-    if (h < n) {
-      const int u = up[h], d = dn[h];
-      const int uc = (u >= 0 && dn[u] == (int)h) ? u : -1;   // P11
-      const int dc = (d >= 0 && up[d] == (int)h) ? d : -1;
-      rec[h] = make_int4(y[h], z[h], uc, dc);
-      if (dc < 0 && uc >= 0) {   // P12 chain start; the walk uses raw links + the mutual test (= cleaned links)
-        int len = 2, c = uc;
-        while (len < g.l_min) {
-          const int nx = up[c];
-          if (nx < 0 || dn[nx] != c) break;
-          c = nx;
-          ++len;
-        }
-        seed[k] = len >= g.l_min;   // P13
-      }
-    }
-    uint32_t tot;
-    pos[k] = running + block_excl_scan(seed[k] ? 1u : 0u, wsum, &tot);
-    running += tot;
+    du[k] = u[k] >= 0 ? dn[u[k]] : -1;
+    ud[k] = d[k] >= 0 ? up[d[k]] : -1;
   }
+  int c[A3_ITEMS], len[A3_ITEMS];
+  bool walk[A3_ITEMS];
+#pragma unroll
+  for (int k = 0; k < A3_ITEMS; ++k) {
+    const int h = (int)(h0 + k);
+    const int uc = (u[k] >= 0 && du[k] == h) ? u[k] : -1;   // P11
+    const int dc = (d[k] >= 0 && ud[k] == h) ? d[k] : -1;
+    if (h0 + k < n) rec[h0 + k] = make_int4(yy[k], zz[k], uc, dc);
+    walk[k] = dc < 0 && uc >= 0;   // P12 chain start; the walk uses raw links + the mutual test (= cleaned links)
+    c[k] = uc;
+    len[k] = 2;
+  }
+  for (int step = 2; step < g.l_min; ++step) {   // all walks of the thread advance together
+    int nx[A3_ITEMS], back[A3_ITEMS];
+#pragma unroll
+    for (int k = 0; k < A3_ITEMS; ++k) nx[k] = (walk[k] && len[k] == step) ? up[c[k]] : -1;
+#pragma unroll
+    for (int k = 0; k < A3_ITEMS; ++k) back[k] = nx[k] >= 0 ? dn[nx[k]] : -1;
+#pragma unroll
+    for (int k = 0; k < A3_ITEMS; ++k)
+      if (nx[k] >= 0 && back[k] == c[k]) {
+        c[k] = nx[k];
+        ++len[k];
+      }
+  }
+  bool seed[A3_ITEMS];
+  uint32_t mine = 0;
+#pragma unroll
+  for (int k = 0; k < A3_ITEMS; ++k) {
+    seed[k] = walk[k] && len[k] >= g.l_min;   // P13
+    mine += seed[k] ? 1u : 0u;
+  }
+  uint32_t running;
+  uint32_t pos = block_excl_scan(mine, wsum, &running);   // ids ascend with (thread, item): ranks follow (P14)
   const uint32_t excl = (uint32_t)lookback_scan(status, tile, running, &sh_excl);
 #pragma unroll
   for (int k = 0; k < A3_ITEMS; ++k)
     if (seed[k]) {
-      const uint32_t h = (uint32_t)(base + k * A3_THREADS + threadIdx.x);
+      const uint32_t h = (uint32_t)(h0 + k);
       int lo = 0, hi = g.n_sectors * g.n_rows;   // (sector,row) of the start: largest sr with ro[sr] <= h
       while (hi - lo > 1) {
         const int mid = (lo + hi) >> 1;
         if (ro[mid] <= h) lo = mid; else hi = mid;
       }
-      seed_start[excl + pos[k]] = (int32_t)h;
-      seed_sr[excl + pos[k]] = lo;
+      seed_start[excl + pos] = (int32_t)h;
+      seed_sr[excl + pos] = lo;
+      ++pos;
     }
   if (tile == n_tiles - 1 && threadIdx.x == 0) ctl->n_seeds = excl + running;
 }
