@@ -18,21 +18,33 @@ struct Ranges {
 
 __device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
 
-__device__ __forceinline__ Ranges window_ranges(const DevGeom& g, int yh, int zh, int org_z,
-                                                const uint32_t* __restrict__ bs) {
+struct Window {
+  int lo0, hi0, lo1, hi1;   // bin indices of the range ends in the low and the high z-bin (equal if one z-bin)
+};
+
+// Rows of one sector share the grid shape and origin, so one window serves both neighbour rows.
+__device__ __forceinline__ Window window_bins(const DevGeom& g, int yh, int zh, int org_z) {
   const int ny = g.ny;
   const int iy_lo = clampi((yh - g.w_y - g.org_y) >> g.shift_y, 0, ny - 1);
   const int iy_hi = clampi((yh + g.w_y - g.org_y) >> g.shift_y, 0, ny - 1);
   const int iz_lo = clampi((zh - g.w_z - org_z) >> g.shift_z, 0, g.nz - 1);
-  const int iz_hi = clampi((zh + g.w_z - org_z) >> g.shift_z, 0, g.nz - 1);
+  const int iz_hi = clampi((zh + g.w_z - org_z) >> g.shift_z, 0, g.nz - 1);   // bins >= 2*w_z wide: <= iz_lo + 1
+  Window w;
+  w.lo0 = iz_lo * ny + iy_lo;
+  w.hi0 = iz_lo * ny + iy_hi + 1;
+  w.lo1 = iz_hi * ny + iy_lo;
+  w.hi1 = iz_hi * ny + iy_hi + 1;
+  return w;
+}
+
+__device__ __forceinline__ Ranges load_ranges(const Window& w, const uint32_t* __restrict__ bs) {
   Ranges q;
-  q.a0 = bs[iz_lo * ny + iy_lo];
-  q.b0 = bs[iz_lo * ny + iy_hi + 1];
-  if (iz_hi != iz_lo) {   // bins are >= 2*w_z wide, so iz_hi <= iz_lo + 1
-    q.a1 = bs[iz_hi * ny + iy_lo];
-    q.b1 = bs[iz_hi * ny + iy_hi + 1];
-  } else {
-    q.a1 = q.b1 = 0;
+  q.a0 = bs[w.lo0];
+  q.b0 = bs[w.hi0];
+  q.a1 = q.b1 = 0;
+  if (w.lo1 != w.lo0) {
+    q.a1 = bs[w.lo1];
+    q.b1 = bs[w.hi1];
   }
   return q;
 }
@@ -56,8 +68,9 @@ a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int
     const int yh = ch.x, zh = ch.y, hid = ch.z;
     int best_u = -1, best_d = -1;
     if (inner) {
-      const Ranges qu = window_ranges(g, yh, zh, org_z, bs_u);
-      const Ranges qd = window_ranges(g, yh, zh, org_z, bs_d);
+      const Window w = window_bins(g, yh, zh, org_z);
+      const Ranges qu = load_ranges(w, bs_u);
+      const Ranges qd = load_ranges(w, bs_d);
       int best_cost = INT32_MAX;
 #pragma unroll 1
       for (int pu = 0; pu < 2; ++pu) {
