@@ -49,6 +49,40 @@ __device__ __forceinline__ Ranges load_ranges(const Window& w, const uint32_t* _
   return q;
 }
 
+// The definition's nested scan over the up and down ranges.
+__device__ __forceinline__ void pair_search_nested(const DevGeom& g, const int4* __restrict__ srt, const Ranges& qu,
+                                                   const Ranges& qd, int yh, int zh, int& best_cost, int& best_u,
+                                                   int& best_d) {
+#pragma unroll 1
+  for (int pu = 0; pu < 2; ++pu) {
+    const uint32_t ua = pu ? qu.a1 : qu.a0, ub = pu ? qu.b1 : qu.b0;
+    for (uint32_t u = ua; u < ub; ++u) {
+      const int4 cu = srt[u];
+      const int dyu = cu.x - yh, dzu = cu.y - zh;
+      if (abs(dyu) > g.w_y || abs(dzu) > g.w_z) continue;
+      const int idu = cu.z;
+#pragma unroll 1
+      for (int pd = 0; pd < 2; ++pd) {
+        const uint32_t da = pd ? qd.a1 : qd.a0, db = pd ? qd.b1 : qd.b0;
+        for (uint32_t d = da; d < db; ++d) {
+          const int4 cd = srt[d];
+          const int dyd = cd.x - yh, dzd = cd.y - zh;
+          if (abs(dyd) > g.w_y || abs(dzd) > g.w_z) continue;
+          const int ddy = dyu + dyd, ddz = dzu + dzd;
+          const int cost = g.cost_wy * ddy * ddy + g.cost_wz * ddz * ddz;
+          if (cost > best_cost) continue;
+          const int idd = cd.z;
+          if (cost < best_cost || idu < best_u || (idu == best_u && idd < best_d)) {   // P9
+            best_cost = cost;
+            best_u = idu;
+            best_d = idd;
+          }
+        }
+      }
+    }
+  }
+}
+
 __global__ void __launch_bounds__(A2_THREADS)
 a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int4* __restrict__ srt,
                      const uint32_t* __restrict__ sec_key, const uint32_t* __restrict__ bin_start,
@@ -72,32 +106,94 @@ a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int
       const Ranges qu = load_ranges(w, bs_u);
       const Ranges qd = load_ranges(w, bs_d);
       int best_cost = INT32_MAX;
-#pragma unroll 1
-      for (int pu = 0; pu < 2; ++pu) {
-        const uint32_t ua = pu ? qu.a1 : qu.a0, ub = pu ? qu.b1 : qu.b0;
-        for (uint32_t u = ua; u < ub; ++u) {
-          const int4 cu = srt[u];
-          const int dyu = cu.x - yh, dzu = cu.y - zh;
-          if (abs(dyu) > g.w_y || abs(dzu) > g.w_z) continue;
-          const int idu = cu.z;
-#pragma unroll 1
-          for (int pd = 0; pd < 2; ++pd) {
-            const uint32_t da = pd ? qd.a1 : qd.a0, db = pd ? qd.b1 : qd.b0;
-            for (uint32_t d = da; d < db; ++d) {
-              const int4 cd = srt[d];
-              const int dyd = cd.x - yh, dzd = cd.y - zh;
-              if (abs(dyd) > g.w_y || abs(dzd) > g.w_z) continue;
-              const int ddy = dyu + dyd, ddz = dzu + dzd;
-              const int cost = g.cost_wy * ddy * ddy + g.cost_wz * ddz * ddz;
-              if (cost > best_cost) continue;
-              const int idd = cd.z;
-              if (cost < best_cost || idu < best_u || (idu == best_u && idd < best_d)) {   // P9
-                best_cost = cost;
-                best_u = idu;
-                best_d = idd;
-              }
-            }
+      pair_search_nested(g, srt, qu, qd, yh, zh, best_cost, best_u, best_d);
+      if (best_u < 0 || best_cost > g.c_max) best_u = best_d = -1;   // P10
+    }
+    link_up[hid] = best_u;
+    link_dn[hid] = best_d;
+    owner[hid] = 0u;   // a5 ownership words start empty
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Dense rows (several clusters per grid bin: pile-up at high density).  The nested scan above tests every cluster
+// of the down ranges once per up candidate; here each side's ranges are filtered once into a short list in shared
+// memory and the pair loop runs over |U| x |D| window candidates only (a few, against hundreds of range pairs).
+// A cluster with more than A2_KEEP candidates on a side falls back to the nested scan.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int A2_KEEP = 12;
+
+__device__ __forceinline__ int filter_side(const DevGeom& g, const int4* __restrict__ srt, const Ranges& q, int yh,
+                                           int zh, int* __restrict__ col /* [A2_KEEP][3][A2_THREADS] column */) {
+  const uint32_t n0 = q.b0 - q.a0, total = n0 + (q.b1 - q.a1);
+  int cnt = 0;
+  if (total) {
+    int4 nx = srt[n0 ? q.a0 : q.a1];
+    for (uint32_t t = 0; t < total; ++t) {
+      const int4 c = nx;
+      const uint32_t tn = min(t + 1, total - 1);   // next one in flight (the last iteration re-reads itself)
+      nx = srt[tn < n0 ? q.a0 + tn : q.a1 + (tn - n0)];
+      const int dy = c.x - yh, dz = c.y - zh;
+      if (abs(dy) <= g.w_y && abs(dz) <= g.w_z) {   // P7, inclusive
+        if (cnt < A2_KEEP) {
+          int* e = col + cnt * 3 * A2_THREADS;
+          e[0] = dy;
+          e[A2_THREADS] = dz;
+          e[2 * A2_THREADS] = c.z;
+        }
+        ++cnt;
+      }
+    }
+  }
+  return cnt;
+}
+
+__global__ void __launch_bounds__(A2_THREADS)
+a2_neighbours_dense_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int4* __restrict__ srt,
+                           const uint32_t* __restrict__ sec_key, const uint32_t* __restrict__ bin_start,
+                           int32_t* __restrict__ link_up, int32_t* __restrict__ link_dn,
+                           uint32_t* __restrict__ owner) {
+  __shared__ int cand[2][A2_KEEP][3][A2_THREADS];   // [side][slot][dy, dz, id][thread]: a thread reads only its column
+  const int sr = blockIdx.x;
+  const int r = sr % g.n_rows;
+  const uint32_t a = ro[sr], b = ro[sr + 1];
+  const bool inner = r >= 1 && r <= g.n_rows - 2;   // P5
+  const int org_z = zmin_from_key(sec_key[sr / g.n_rows]);
+  const uint32_t *bs_u = nullptr, *bs_d = nullptr;
+  if (inner) {
+    bs_u = bin_start + (size_t)(sr + 1) * g.nb_stride;
+    bs_d = bin_start + (size_t)(sr - 1) * g.nb_stride;
+  }
+  int* const col_u = &cand[0][0][0][threadIdx.x];
+  int* const col_d = &cand[1][0][0][threadIdx.x];
+  for (uint32_t j = a + threadIdx.x; j < b; j += A2_THREADS) {
+    const int4 ch = srt[j];
+    const int yh = ch.x, zh = ch.y, hid = ch.z;
+    int best_u = -1, best_d = -1;
+    if (inner) {
+      const Window w = window_bins(g, yh, zh, org_z);
+      const Ranges qu = load_ranges(w, bs_u);
+      const Ranges qd = load_ranges(w, bs_d);
+      int best_cost = INT32_MAX;
+      const int nu = filter_side(g, srt, qu, yh, zh, col_u);
+      const int nd = nu > 0 ? filter_side(g, srt, qd, yh, zh, col_d) : 0;
+      if (nu > A2_KEEP || nd > A2_KEEP) {
+        pair_search_nested(g, srt, qu, qd, yh, zh, best_cost, best_u, best_d);
+      } else {
+        const int np = nu * nd;   // one flat loop over the pairs
+        int iu = 0, id = 0;
+        for (int t = 0; t < np; ++t) {
+          const int* eu = col_u + iu * 3 * A2_THREADS;
+          const int* ed = col_d + id * 3 * A2_THREADS;
+          const int ddy = eu[0] + ed[0], ddz = eu[A2_THREADS] + ed[A2_THREADS];
+          const int cost = g.cost_wy * ddy * ddy + g.cost_wz * ddz * ddz;   // P8
+          const int idu = eu[2 * A2_THREADS], idd = ed[2 * A2_THREADS];
+          if (cost < best_cost || (cost == best_cost && (idu < best_u || (idu == best_u && idd < best_d)))) {   // P9
+            best_cost = cost;
+            best_u = idu;
+            best_d = idd;
           }
+          if (++id == nd) { id = 0; ++iu; }
         }
       }
       if (best_u < 0 || best_cost > g.c_max) best_u = best_d = -1;   // P10
@@ -113,6 +209,13 @@ a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int
 cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64_t n, cudaStream_t st) {
   const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
   if (R == 0) return cudaSuccess;
+  // clusters per grid bin decide the variant (both compute the same links)
+  const bool dense = (double)n > 0.75 * (double)R * (double)(t->g.ny * t->g.nz);
+  if (dense) {
+    a2_neighbours_dense_kernel<<<(unsigned)R, A2_THREADS, 0, st>>>(t->g, ro, t->s.srt, t->s.sec_key, t->s.bin_start,
+                                                                  t->s.link_up, t->s.link_dn, t->s.owner);
+    return cudaGetLastError();
+  }
   a2_neighbours_kernel<<<(unsigned)R, A2_THREADS, 0, st>>>(t->g, ro, t->s.srt, t->s.sec_key,
                                                           t->s.bin_start, t->s.link_up, t->s.link_dn, t->s.owner);
   return cudaGetLastError();

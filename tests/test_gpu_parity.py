@@ -111,6 +111,32 @@ def test_config2_slice_small(orc):
     compare(ev, orc, _run_gpu(ev), orc.track(ev), label="cfg2/6coll")
 
 
+def test_config2_full_slice(orc):
+    """configs[2] at full size: 100 collisions, ~18 M clusters, rows of ~3400 clusters over a 5400 cm z-extent
+    (a1's block-per-row variant, 11.8 k bins per row)."""
+    ev = make_event(2)
+    assert ev.n > 15_000_000
+    compare(ev, orc, _run_gpu(ev), orc.track(ev), label="cfg2 full")
+
+
+def test_config3_literal_dense(orc):
+    """configs[3] as written (5000 collisions x 30 tracks, ~22 M clusters, ~7 clusters per grid bin): a2's dense
+    variant, hit-ownership contention."""
+    ev = make_event(3)
+    assert ev.n > 18_000_000
+    compare(ev, orc, _run_gpu(ev), orc.track(ev), label="cfg3 literal")
+
+
+def test_bench_configuration_full_size(orc):
+    """The launch configuration bench.py times: 16 distinct full configs[1] events in one call (576 sectors,
+    ~9.6 M clusters), every output compared."""
+    from bench import shard_seeds
+    evs = [make_event(1, s) for s in shard_seeds(0, 1, 16)]
+    ev = concat_events(evs)
+    assert ev.n_sectors == 576 and ev.n > 9_000_000
+    compare(ev, orc, _run_gpu(ev), orc.track(ev), label="bench batch")
+
+
 def test_batch_as_extra_sectors(orc):
     """bench.py's launch configuration: B events concatenated as B*36 sectors in one call."""
     evs = [make_event(1, 1000 + k, n_tracks=600) for k in range(3)]
