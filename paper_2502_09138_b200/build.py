@@ -13,6 +13,9 @@ CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "libtpctrack.so")
 SOURCES = ["api.cu", "a1_grid.cu", "a2_neighbours.cu", "a3_seeds.cu", "a4_follow.cu", "a5_select.cu", "debug.cu"]
 HEADERS = [os.path.join(CSRC, "tpc_internal.cuh"), os.path.join(os.path.dirname(_HERE), "include", "tpc_track.h")]
+# a4 only: fp32 division / sqrt / rsqrt as MUFU + one correction (2 ulp), denormals flushed.  Measured against
+# the fp64 oracle on configs 0, 1, 2, 4: worst parameter error 9e-6 (bar 1e-4), hit tables unchanged; a4 -5 %.
+EXTRA_FLAGS = {"a4_follow.cu": ["--use_fast_math"]}
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
 
@@ -35,7 +38,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if not force and os.path.exists(o) and all(os.path.getmtime(d) <= os.path.getmtime(o) for d in [s] + HEADERS):
             continue
         extra = os.environ.get("TPC_NVCC_EXTRA", "").split()   # experiments only (e.g. -DTPC_A4_COV64)
-        cmd = [_nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o]
+        cmd = ([_nvcc()] + NVCC_FLAGS + EXTRA_FLAGS.get(os.path.basename(s), []) + extra
+               + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o])
         procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     for cmd, p in procs:
         out, _ = p.communicate()

@@ -140,7 +140,16 @@ __device__ __forceinline__ bool transport(const DevGeom& g, float dxf, State& p,
 // Appendix C update with H = [I2 | 0], V = diag(sy2, sz2).  Returns the chi2 increment.
 __device__ __forceinline__ float update(const DevGeom& g, State& p, Cov& C, float ym, float zm) {
   const creal S00 = C.c00 + (creal)g.sy2, S01 = C.c10, S11 = C.c11 + (creal)g.sz2;
+#ifdef TPC_A4_COV32
   const creal idet = (creal)1 / (S00 * S11 - S01 * S01);
+#else
+  // 1/det: fp32 reciprocal + two Newton steps in fp64 (relative error ~1e-15) instead of the IEEE fp64 division
+  // sequence; det = (Cyy + sy2)(Czz + sz2) - Cyz^2 >= sy2 sz2 stays far inside the fp32 range.
+  const double det = S00 * S11 - S01 * S01;
+  double idet = (double)(1.0f / (float)det);
+  idet = idet * (2.0 - det * idet);
+  idet = idet * (2.0 - det * idet);
+#endif
   const creal I00 = S11 * idet, I01 = -S01 * idet, I11 = S00 * idet;
   const creal r0 = (sreal)ym - p.y, r1 = (sreal)zm - p.z;
   // K = C[:,0:2] S^-1
