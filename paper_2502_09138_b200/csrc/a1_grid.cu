@@ -154,11 +154,13 @@ static bool a1_warp_rows(const tpc_tracker* t, int64_t n) {
 size_t a1_smem_bytes(const DevGeom& g) { return (size_t)(g.nb_stride) * sizeof(uint32_t); }
 
 cudaError_t setup_a1_attributes(const tpc_tracker* t) {
+  // the grid shape may change from call to call (api.cu: choose_grid): allow the largest histogram up front
+  (void)t;
   cudaError_t e = cudaFuncSetAttribute(a1_grid_kernel<A1_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)a1_smem_bytes(t->g));
-  if (e != cudaSuccess || t->g.nb_stride > 4096) return e;
+                                       (GRID_MAX_BINS + 4) * (int)sizeof(uint32_t));
+  if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(a1_grid_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              (int)(a1_smem_bytes(t->g) * (A1_THREADS / 32)));
+                              4096 * (int)sizeof(uint32_t) * (A1_THREADS / 32));
 }
 
 cudaError_t launch_a1_grid(const tpc_tracker* t, const int32_t* y, const int32_t* z, const uint32_t* ro, int64_t n,

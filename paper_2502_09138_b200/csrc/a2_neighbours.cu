@@ -19,70 +19,102 @@ struct Ranges {
 __device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
 
 struct Window {
-  int lo0, hi0, lo1, hi1;   // bin indices of the range ends in the low and the high z-bin (equal if one z-bin)
+  int iy_lo, iy_hi, iz_lo, iz_hi;   // inclusive bin ranges
 };
 
 // Rows of one sector share the grid shape and origin, so one window serves both neighbour rows.
 __device__ __forceinline__ Window window_bins(const DevGeom& g, int yh, int zh, int org_z) {
-  const int ny = g.ny;
-  const int iy_lo = clampi((yh - g.w_y - g.org_y) >> g.shift_y, 0, ny - 1);
-  const int iy_hi = clampi((yh + g.w_y - g.org_y) >> g.shift_y, 0, ny - 1);
-  const int iz_lo = clampi((zh - g.w_z - org_z) >> g.shift_z, 0, g.nz - 1);
-  const int iz_hi = clampi((zh + g.w_z - org_z) >> g.shift_z, 0, g.nz - 1);   // bins >= 2*w_z wide: <= iz_lo + 1
   Window w;
-  w.lo0 = iz_lo * ny + iy_lo;
-  w.hi0 = iz_lo * ny + iy_hi + 1;
-  w.lo1 = iz_hi * ny + iy_lo;
-  w.hi1 = iz_hi * ny + iy_hi + 1;
+  w.iy_lo = clampi((yh - g.w_y - g.org_y) >> g.shift_y, 0, g.ny - 1);
+  w.iy_hi = clampi((yh + g.w_y - g.org_y) >> g.shift_y, 0, g.ny - 1);
+  w.iz_lo = clampi((zh - g.w_z - org_z) >> g.shift_z, 0, g.nz - 1);
+  w.iz_hi = clampi((zh + g.w_z - org_z) >> g.shift_z, 0, g.nz - 1);
   return w;
 }
 
-__device__ __forceinline__ Ranges load_ranges(const Window& w, const uint32_t* __restrict__ bs) {
+// Coarse grid (bins >= 2*w_z wide): the window touches at most two z-bins, both ranges are loaded up front.
+__device__ __forceinline__ Ranges load_ranges(const DevGeom& g, const Window& w, const uint32_t* __restrict__ bs) {
   Ranges q;
-  q.a0 = bs[w.lo0];
-  q.b0 = bs[w.hi0];
+  q.a0 = bs[w.iz_lo * g.ny + w.iy_lo];
+  q.b0 = bs[w.iz_lo * g.ny + w.iy_hi + 1];
   q.a1 = q.b1 = 0;
-  if (w.lo1 != w.lo0) {
-    q.a1 = bs[w.lo1];
-    q.b1 = bs[w.hi1];
+  if (w.iz_hi != w.iz_lo) {
+    q.a1 = bs[w.iz_hi * g.ny + w.iy_lo];
+    q.b1 = bs[w.iz_hi * g.ny + w.iy_hi + 1];
   }
   return q;
 }
 
-// The definition's nested scan over the up and down ranges.
-__device__ __forceinline__ void pair_search_nested(const DevGeom& g, const int4* __restrict__ srt, const Ranges& qu,
-                                                   const Ranges& qd, int yh, int zh, int& best_cost, int& best_u,
-                                                   int& best_d) {
+// One candidate pair against the running best (P8, P9).
+__device__ __forceinline__ void try_pair(const DevGeom& g, int dyu, int dzu, int idu, const int4& cd, int yh, int zh,
+                                         int& best_cost, int& best_u, int& best_d) {
+  const int dyd = cd.x - yh, dzd = cd.y - zh;
+  if (abs(dyd) > g.w_y || abs(dzd) > g.w_z) return;
+  const int ddy = dyu + dyd, ddz = dzu + dzd;
+  const int cost = g.cost_wy * ddy * ddy + g.cost_wz * ddz * ddz;
+  if (cost > best_cost) return;
+  const int idd = cd.z;
+  if (cost < best_cost || idu < best_u || (idu == best_u && idd < best_d)) {
+    best_cost = cost;
+    best_u = idu;
+    best_d = idd;
+  }
+}
+
+// The definition's nested scan over the up and down candidates of the window.  FINE: the call refined the grid
+// (api.cu: choose_grid), a window may span any number of z-bins and the ranges are read bin row by bin row.
+template <bool FINE>
+__device__ __forceinline__ void pair_search_nested(const DevGeom& g, const int4* __restrict__ srt, const Window& w,
+                                                   const uint32_t* __restrict__ bs_u,
+                                                   const uint32_t* __restrict__ bs_d, int yh, int zh, int& best_cost,
+                                                   int& best_u, int& best_d) {
+  if (!FINE) {
+    const Ranges qu = load_ranges(g, w, bs_u), qd = load_ranges(g, w, bs_d);
 #pragma unroll 1
-  for (int pu = 0; pu < 2; ++pu) {
-    const uint32_t ua = pu ? qu.a1 : qu.a0, ub = pu ? qu.b1 : qu.b0;
-    for (uint32_t u = ua; u < ub; ++u) {
-      const int4 cu = srt[u];
-      const int dyu = cu.x - yh, dzu = cu.y - zh;
-      if (abs(dyu) > g.w_y || abs(dzu) > g.w_z) continue;
-      const int idu = cu.z;
+    for (int pu = 0; pu < 2; ++pu) {
+      const uint32_t ua = pu ? qu.a1 : qu.a0, ub = pu ? qu.b1 : qu.b0;
+      for (uint32_t u = ua; u < ub; ++u) {
+        const int4 cu = srt[u];
+        const int dyu = cu.x - yh, dzu = cu.y - zh;
+        if (abs(dyu) > g.w_y || abs(dzu) > g.w_z) continue;
 #pragma unroll 1
-      for (int pd = 0; pd < 2; ++pd) {
-        const uint32_t da = pd ? qd.a1 : qd.a0, db = pd ? qd.b1 : qd.b0;
-        for (uint32_t d = da; d < db; ++d) {
-          const int4 cd = srt[d];
-          const int dyd = cd.x - yh, dzd = cd.y - zh;
-          if (abs(dyd) > g.w_y || abs(dzd) > g.w_z) continue;
-          const int ddy = dyu + dyd, ddz = dzu + dzd;
-          const int cost = g.cost_wy * ddy * ddy + g.cost_wz * ddz * ddz;
-          if (cost > best_cost) continue;
-          const int idd = cd.z;
-          if (cost < best_cost || idu < best_u || (idu == best_u && idd < best_d)) {   // P9
-            best_cost = cost;
-            best_u = idu;
-            best_d = idd;
+        const int idu = cu.z;
+        for (int pd = 0; pd < 2; ++pd) {
+          const uint32_t da = pd ? qd.a1 : qd.a0, db = pd ? qd.b1 : qd.b0;
+          for (uint32_t d = da; d < db; ++d) {
+            const int4 cd = srt[d];
+            const int dyd = cd.x - yh, dzd = cd.y - zh;
+            if (abs(dyd) > g.w_y || abs(dzd) > g.w_z) continue;
+            const int ddy = dyu + dyd, ddz = dzu + dzd;
+            const int cost = g.cost_wy * ddy * ddy + g.cost_wz * ddz * ddz;
+            if (cost > best_cost) continue;
+            const int idd = cd.z;
+            if (cost < best_cost || idu < best_u || (idu == best_u && idd < best_d)) {   // P9
+              best_cost = cost;
+              best_u = idu;
+              best_d = idd;
+            }
           }
+        }
+      }
+    }
+  } else {
+    for (int izu = w.iz_lo; izu <= w.iz_hi; ++izu) {
+      const uint32_t ua = bs_u[izu * g.ny + w.iy_lo], ub = bs_u[izu * g.ny + w.iy_hi + 1];
+      for (uint32_t u = ua; u < ub; ++u) {
+        const int4 cu = srt[u];
+        const int dyu = cu.x - yh, dzu = cu.y - zh;
+        if (abs(dyu) > g.w_y || abs(dzu) > g.w_z) continue;
+        for (int izd = w.iz_lo; izd <= w.iz_hi; ++izd) {
+          const uint32_t da = bs_d[izd * g.ny + w.iy_lo], db = bs_d[izd * g.ny + w.iy_hi + 1];
+          for (uint32_t d = da; d < db; ++d) try_pair(g, dyu, dzu, cu.z, srt[d], yh, zh, best_cost, best_u, best_d);
         }
       }
     }
   }
 }
 
+template <bool FINE>
 __global__ void __launch_bounds__(A2_THREADS)
 a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int4* __restrict__ srt,
                      const uint32_t* __restrict__ sec_key, const uint32_t* __restrict__ bin_start,
@@ -103,10 +135,8 @@ a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int
     int best_u = -1, best_d = -1;
     if (inner) {
       const Window w = window_bins(g, yh, zh, org_z);
-      const Ranges qu = load_ranges(w, bs_u);
-      const Ranges qd = load_ranges(w, bs_d);
       int best_cost = INT32_MAX;
-      pair_search_nested(g, srt, qu, qd, yh, zh, best_cost, best_u, best_d);
+      pair_search_nested<FINE>(g, srt, w, bs_u, bs_d, yh, zh, best_cost, best_u, best_d);
       if (best_u < 0 || best_cost > g.c_max) best_u = best_d = -1;   // P10
     }
     link_up[hid] = best_u;
@@ -123,16 +153,17 @@ a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int A2_KEEP = 12;
 
-__device__ __forceinline__ int filter_side(const DevGeom& g, const int4* __restrict__ srt, const Ranges& q, int yh,
-                                           int zh, int* __restrict__ col /* [A2_KEEP][3][A2_THREADS] column */) {
-  const uint32_t n0 = q.b0 - q.a0, total = n0 + (q.b1 - q.a1);
+__device__ __forceinline__ int filter_side(const DevGeom& g, const int4* __restrict__ srt, const Window& w,
+                                           const uint32_t* __restrict__ bs, int yh, int zh,
+                                           int* __restrict__ col /* [A2_KEEP][3][A2_THREADS] column */) {
   int cnt = 0;
-  if (total) {
-    int4 nx = srt[n0 ? q.a0 : q.a1];
-    for (uint32_t t = 0; t < total; ++t) {
+  for (int iz = w.iz_lo; iz <= w.iz_hi; ++iz) {   // one contiguous sorted range per z-bin row of the window
+    const uint32_t ra = bs[iz * g.ny + w.iy_lo], rb = bs[iz * g.ny + w.iy_hi + 1];
+    if (ra >= rb) continue;
+    int4 nx = srt[ra];
+    for (uint32_t t = ra; t < rb; ++t) {
       const int4 c = nx;
-      const uint32_t tn = min(t + 1, total - 1);   // next one in flight (the last iteration re-reads itself)
-      nx = srt[tn < n0 ? q.a0 + tn : q.a1 + (tn - n0)];
+      nx = srt[min(t + 1, rb - 1)];   // next one in flight (the last iteration re-reads itself)
       const int dy = c.x - yh, dz = c.y - zh;
       if (abs(dy) <= g.w_y && abs(dz) <= g.w_z) {   // P7, inclusive
         if (cnt < A2_KEEP) {
@@ -148,6 +179,7 @@ __device__ __forceinline__ int filter_side(const DevGeom& g, const int4* __restr
   return cnt;
 }
 
+template <bool FINE>
 __global__ void __launch_bounds__(A2_THREADS)
 a2_neighbours_dense_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int4* __restrict__ srt,
                            const uint32_t* __restrict__ sec_key, const uint32_t* __restrict__ bin_start,
@@ -172,13 +204,11 @@ a2_neighbours_dense_kernel(const DevGeom g, const uint32_t* __restrict__ ro, con
     int best_u = -1, best_d = -1;
     if (inner) {
       const Window w = window_bins(g, yh, zh, org_z);
-      const Ranges qu = load_ranges(w, bs_u);
-      const Ranges qd = load_ranges(w, bs_d);
       int best_cost = INT32_MAX;
-      const int nu = filter_side(g, srt, qu, yh, zh, col_u);
-      const int nd = nu > 0 ? filter_side(g, srt, qd, yh, zh, col_d) : 0;
+      const int nu = filter_side(g, srt, w, bs_u, yh, zh, col_u);
+      const int nd = nu > 0 ? filter_side(g, srt, w, bs_d, yh, zh, col_d) : 0;
       if (nu > A2_KEEP || nd > A2_KEEP) {
-        pair_search_nested(g, srt, qu, qd, yh, zh, best_cost, best_u, best_d);
+        pair_search_nested<FINE>(g, srt, w, bs_u, bs_d, yh, zh, best_cost, best_u, best_d);
       } else {
         const int np = nu * nd;   // one flat loop over the pairs
         int iu = 0, id = 0;
@@ -209,14 +239,15 @@ a2_neighbours_dense_kernel(const DevGeom g, const uint32_t* __restrict__ ro, con
 cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64_t n, cudaStream_t st) {
   const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
   if (R == 0) return cudaSuccess;
-  // clusters per grid bin decide the variant (both compute the same links)
+  // clusters per grid bin decide the variant (both compute the same links); a refined grid (choose_grid) may have
+  // z-bins narrower than the window
   const bool dense = (double)n > 0.75 * (double)R * (double)(t->g.ny * t->g.nz);
-  if (dense) {
-    a2_neighbours_dense_kernel<<<(unsigned)R, A2_THREADS, 0, st>>>(t->g, ro, t->s.srt, t->s.sec_key, t->s.bin_start,
-                                                                  t->s.link_up, t->s.link_dn, t->s.owner);
-    return cudaGetLastError();
-  }
-  a2_neighbours_kernel<<<(unsigned)R, A2_THREADS, 0, st>>>(t->g, ro, t->s.srt, t->s.sec_key,
-                                                          t->s.bin_start, t->s.link_up, t->s.link_dn, t->s.owner);
+  const bool fine = t->g.shift_z < t->base_shift_z;
+#define A2_ARGS t->g, ro, t->s.srt, t->s.sec_key, t->s.bin_start, t->s.link_up, t->s.link_dn, t->s.owner
+  if (dense && fine) a2_neighbours_dense_kernel<true><<<(unsigned)R, A2_THREADS, 0, st>>>(A2_ARGS);
+  else if (dense) a2_neighbours_dense_kernel<false><<<(unsigned)R, A2_THREADS, 0, st>>>(A2_ARGS);
+  else if (fine) a2_neighbours_kernel<true><<<(unsigned)R, A2_THREADS, 0, st>>>(A2_ARGS);
+  else a2_neighbours_kernel<false><<<(unsigned)R, A2_THREADS, 0, st>>>(A2_ARGS);
+#undef A2_ARGS
   return cudaGetLastError();
 }

@@ -198,7 +198,7 @@ struct Window {
   int iy_lo, iy_hi, iz_lo, iz_hi;
   __device__ __forceinline__ uint32_t key_y() const { return ((uint32_t)iy_lo << 16) | (uint32_t)iy_hi; }
   __device__ __forceinline__ uint32_t key_z(int row) const {
-    return ((uint32_t)row << 24) | ((uint32_t)iz_lo << 1) | (iz_hi != iz_lo ? 1u : 0u);
+    return ((uint32_t)row << 24) | ((uint32_t)iz_lo << 8) | (uint32_t)min(iz_hi - iz_lo, 255);   // nz < 2^16
   }
 };
 
@@ -272,14 +272,10 @@ __device__ __forceinline__ void load_ranges_if(const DevGeom& g, const uint32_t*
 }
 
 // P17/P21: among the candidates minimise (d, id), d = dy^2/(Cyy + sy2) + dz^2/(Czz + sz2), restricted to
-// |dy| <= gate_y and |dz| <= gate_z (cm); accept iff d < gate_d.
-__device__ __forceinline__ Found search_row(const DevGeom& g, const BinRanges& q, float py, float pz, float vy, float vz,
-                                            int y0, int z0, const int4* __restrict__ srt) {
-  Found f;
-  f.id = -1;
-  f.y = f.z = 0.f;
-  const float wy = 1.f / vy, wz = 1.f / vz;
-  float bestd = __int_as_float(0x7f800000);
+// |dy| <= gate_y and |dz| <= gate_z (cm).  Accumulates into (f, bestd); the caller applies the gate d < gate_d.
+__device__ __forceinline__ void search_ranges(const DevGeom& g, const BinRanges& q, float py, float pz, float wy,
+                                              float wz, int y0, int z0, const int4* __restrict__ srt, Found& f,
+                                              float& bestd) {
   const uint32_t n0 = q.b0 - q.a0, total = n0 + (q.b1 - q.a1);
   if (total) {
     int4 nx = srt[n0 ? q.a0 : q.a1];
@@ -299,8 +295,6 @@ __device__ __forceinline__ Found search_row(const DevGeom& g, const BinRanges& q
       }
     }
   }
-  if (!(bestd < g.gate_d)) f.id = -1;
-  return f;
 }
 
 enum : int { PH_IDLE = 0, PH_INIT, PH_A, PH_B, PH_CS, PH_CD, PH_FIN, PH_DONE };
@@ -485,9 +479,26 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
         const float py = (float)p.y, pz = (float)p.z;
         const float vy = (float)C.c00 + g.sy2, vz = (float)C.c11 + g.sz2;
         const Window w = search_window(g, py, pz, vy, vz, y0, z0, org_z);
-        BinRanges q = pq;
-        load_ranges_if(g, bs, w, q, w.key_y() != pk_y || w.key_z(row) != pk_z);
-        const Found f = search_row(g, q, py, pz, vy, vz, y0, z0, srt);
+        Found f;
+        f.id = -1;
+        f.y = f.z = 0.f;
+        float bestd = __int_as_float(0x7f800000);
+        const float wy = 1.f / vy, wz = 1.f / vz;
+        if (w.iz_hi <= w.iz_lo + 1) {   // always so on the coarse grid (bins >= 2 gate_z wide)
+          BinRanges q = pq;
+          load_ranges_if(g, bs, w, q, w.key_y() != pk_y || w.key_z(row) != pk_z);
+          search_ranges(g, q, py, pz, wy, wz, y0, z0, srt, f, bestd);
+        } else {   // refined grid (dense call) and a wide gate: two z-bin rows at a time
+          for (int iz = w.iz_lo; iz <= w.iz_hi; iz += 2) {
+            Window w2 = w;
+            w2.iz_lo = iz;
+            w2.iz_hi = min(iz + 1, w.iz_hi);
+            BinRanges q2 = {0, 0, 0, 0};
+            load_ranges_if(g, bs, w2, q2, true);
+            search_ranges(g, q2, py, pz, wy, wz, y0, z0, srt, f, bestd);
+          }
+        }
+        if (!(bestd < g.gate_d)) f.id = -1;   // P21
         hid = f.id;
         ym = f.y;
         zm = f.z;

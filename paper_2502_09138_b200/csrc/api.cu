@@ -68,8 +68,38 @@ size_t layout(tpc_tracker* t, char* base, int64_t n, int64_t R) {
   return off;
 }
 
+void set_grid_shape(tpc_tracker* t, int64_t y_units, int64_t z_units) {
+  DevGeom& g = t->g;
+  g.ny = (int)((y_units >> g.shift_y) + 1);
+  g.nz = (int)((z_units >> g.shift_z) + 2);
+  g.nb_stride = (int)align_up((size_t)g.ny * g.nz + 1, 4);
+}
+
+// Grid resolution of this call.  The coarsest grid (bins >= 2 x the widest search window, so a window touches at
+// most 2 x 2 bins) is right while bins outnumber clusters; a dense call (pile-up: several clusters per bin) halves
+// the bin sizes until bins outnumber clusters again (configs[3] literal: 36.8 -> 24.9 ms per call).  The grid only prunes, so the results do not depend on it.
+void choose_grid(tpc_tracker* t, int64_t n, int64_t R) {
+  DevGeom& g = t->g;
+  g.shift_y = t->base_shift_y;
+  g.shift_z = t->base_shift_z;
+  set_grid_shape(t, t->y_units, t->z_units);
+  while (R > 0 && (double)n > 1.0 * (double)R * g.ny * g.nz) {
+    const int sy = g.shift_y, sz = g.shift_z;
+    if (g.shift_z >= g.shift_y && g.shift_z > GRID_MIN_SHIFT) --g.shift_z;
+    else if (g.shift_y > GRID_MIN_SHIFT) --g.shift_y;
+    else break;
+    set_grid_shape(t, t->y_units, t->z_units);
+    if ((int64_t)g.ny * g.nz + 1 > GRID_MAX_BINS) {   // too many bins for a1's histogram: keep the previous shape
+      g.shift_y = sy;
+      g.shift_z = sz;
+      set_grid_shape(t, t->y_units, t->z_units);
+      break;
+    }
+  }
+}
+
 int ensure_arena(tpc_tracker* t, int64_t n, int64_t R) {
-  if (t->arena && n <= t->cap_n && R <= t->cap_rows) {
+  if (t->arena && layout(t, nullptr, n, R) <= t->arena_bytes) {
     // same allocation, but s_cap / tile counts follow the actual n so that grids stay tight
     layout(t, (char*)t->arena, n, R);
     return TPC_OK;
@@ -199,15 +229,15 @@ int tpc_tracker_create(const tpc_geometry_t* geo, const tpc_field_t* field, tpc_
   }
   const int64_t y_units = (int64_t)ceil(2.0 * yh_max * geo->units_per_cm);
   g.org_y = -(int32_t)(y_units / 2);
-  int64_t nb;
-  for (;;) {   // shrink the bin count until one row's histogram fits the shared memory of a CTA
-    g.ny = (int)((y_units >> g.shift_y) + 1);
-    g.nz = (int)((z_units >> g.shift_z) + 2);
-    nb = (int64_t)g.ny * g.nz;
-    if (nb + 1 <= 48 * 1024) break;
+  for (;;) {   // coarsen until one row's histogram fits the shared memory of a CTA
+    set_grid_shape(t, y_units, z_units);
+    if ((int64_t)g.ny * g.nz + 1 <= GRID_MAX_BINS) break;
     if (g.nz > g.ny) ++g.shift_z; else ++g.shift_y;
   }
-  g.nb_stride = (int)align_up((size_t)nb + 1, 4);
+  t->base_shift_y = g.shift_y;
+  t->base_shift_z = g.shift_z;
+  t->y_units = y_units;
+  t->z_units = z_units;
   for (int r = 0; r < nr; ++r) dx_host[r] = (float)(geo->row_x[r + 1 < nr ? r + 1 : r] - geo->row_x[r + 1 < nr ? r : r - 1]);
   g.w_y = prm.w_y; g.w_z = prm.w_z; g.cost_wy = prm.cost_wy; g.cost_wz = prm.cost_wz; g.c_max = prm.c_max;
   g.l_min = prm.l_min; g.max_miss = prm.max_miss; g.n_min_tracklet = prm.n_min_tracklet; g.n_min_owned = prm.n_min_owned;
@@ -267,6 +297,7 @@ int tpc_track(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* strea
   if (n >= ((int64_t)1 << 31) || n / t->params.l_min + 1 >= 0xFFFFFF) return TPC_ERR_CAPACITY;
   cudaStream_t st = (cudaStream_t)stream;
   const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
+  choose_grid(t, n, R);
   int rc = ensure_arena(t, n, R);
   if (rc != TPC_OK) return rc;
   t->last_n = n;

@@ -70,6 +70,8 @@ struct tpc_tracker {
   void* arena; size_t arena_bytes;
   void* host_arena; size_t host_arena_bytes;   // staging for tpc_track_host
   int64_t cap_n, cap_rows;   // sizes the arena was laid out for
+  int base_shift_y, base_shift_z;   // coarsest grid (bins >= 2 x the widest window); dense calls refine it
+  int64_t y_units, z_units;         // grid extents in fixed-point units
   int64_t s_cap;             // seed capacity of the current layout
   int64_t tiles_a3, tiles_a5;
   int a4_blocks, a4_warps;   // persistent a4 grid: blocks x warps per block = resident warps of the device (set at create)
@@ -81,6 +83,8 @@ struct tpc_tracker {
   cudaError_t last_err; char err_buf[256];
 };
 
+constexpr int GRID_MAX_BINS = 48 * 1024;   // bins per row: one row's histogram fits a CTA's shared memory
+constexpr int GRID_MIN_SHIFT = 9;          // finest bins: 512 units = 0.8 cm
 constexpr int A3_TILE = 1024;   // ids per a3 block (256 threads x 4)
 constexpr int A5_TILE = 128;    // tracklets per a5 block
 // a0 keeps the smallest z of a sector as max over key(z) = ~(z ^ 0x80000000): zero-initialised memory then means
