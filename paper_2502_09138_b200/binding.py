@@ -305,6 +305,13 @@ class Tracker:
         self._check(self._lib.tpc_debug_copy_owner(self._h, _ptr(o), self._stream_ptr(None)))
         return o.cpu().numpy()
 
+    def grid_shape(self):
+        """Grid of the most recent call (api.cu: choose_grid): bins-per-row stride, nz, shift_y, shift_z."""
+        vals = [C.c_int32() for _ in range(4)]
+        self._check(self._lib.tpc_debug_grid_info(self._h, *[C.byref(v) for v in vals]))
+        stride, nz, sy, sz = [int(v.value) for v in vals]
+        return dict(stride=stride, nz=nz, shift_y=sy, shift_z=sz)
+
     def debug_grid(self, n: int):
         import torch
         vals = [C.c_int32() for _ in range(4)]

@@ -27,6 +27,7 @@ def _run_gpu(ev, params=None):
     res["seed_start"], res["seed_len"] = trk.debug_seeds(ev.n, ns)
     res["par"], res["cov"], res["chi2"], res["n_hits"], res["hits"] = trk.debug_tracklets(ns)
     res["owner"] = trk.debug_owner(ev.n)
+    res["grid"] = trk.grid_shape()
     torch.cuda.synchronize()
     trk.close()
     return res
@@ -124,7 +125,9 @@ def test_config3_literal_dense(orc):
     variant, hit-ownership contention."""
     ev = make_event(3)
     assert ev.n > 18_000_000
-    compare(ev, orc, _run_gpu(ev), orc.track(ev), label="cfg3 literal")
+    g = _run_gpu(ev)
+    assert g["grid"]["shift_z"] < 12 and g["grid"]["shift_y"] < 12, g["grid"]   # the call refined the grid
+    compare(ev, orc, g, orc.track(ev), label="cfg3 literal")
 
 
 def test_bench_configuration_full_size(orc):
@@ -135,6 +138,43 @@ def test_bench_configuration_full_size(orc):
     ev = concat_events(evs)
     assert ev.n_sectors == 576 and ev.n > 9_000_000
     compare(ev, orc, _run_gpu(ev), orc.track(ev), label="bench batch")
+
+
+def test_config3_medium_density_refined_sparse_grid(orc):
+    """configs[3] recipe with 1800 collisions (~1.3 clusters per coarse grid bin): the call refines the grid once
+    and lands in the sparse regime -> a2's FINE nested variant, a4 windows spanning more than two z-bin rows."""
+    ev = make_event(3, collisions=1800)
+    g = _run_gpu(ev)
+    bins = (g["grid"]["stride"] - 1) * ev.n_sectors * ev.n_rows
+    assert g["grid"]["shift_z"] == 11 and 0.4 * bins < ev.n < 0.75 * bins, (g["grid"], ev.n, bins)   # refined, sparse
+    compare(ev, orc, g, orc.track(ev), label="cfg3/1800")
+
+
+def test_small_geometry_40_rows(orc):
+    """A geometry whose row count is neither 152 nor a multiple of 32 (a4's row tables, a5's row columns)."""
+    from gen.events import Config
+    cfg = Config("one_sector_40_rows", n_sectors=1, open_sector=True, tracks_per_collision=150, pt_min=0.3,
+                 noise=0.05, n_rows=40)
+    ev = make_event(cfg, seed=7)
+    assert ev.n_rows == 40
+    g, o = _run_gpu(ev), orc.track(ev)
+    assert len(o["seed_start"]) > 20
+    compare(ev, orc, g, o, label="40 rows", min_assign=0.99)
+
+
+def test_non_default_parameters(orc):
+    """tpc_params_t reaches every stage: narrower windows, shorter seeds, fewer allowed misses, tighter gate."""
+    from paper_2502_09138_b200.binding import default_params
+    ev = make_event(1, 55, n_tracks=800)
+    gp, op = default_params(), orc.default_params()
+    for p in (gp, op):
+        p.w_y, p.w_z, p.c_max, p.l_min = 1000, 1300, 2500000, 4
+        p.max_miss, p.n_min_tracklet, p.n_min_owned = 3, 8, 6
+        p.gate_d, p.gate_y_cm, p.gate_z_cm, p.sinphi_max = 9.0, 1.5, 2.0, 0.9
+        p.c_reset[4] = 16.0
+    g, o = _run_gpu(ev, gp), orc.track(ev, op)
+    assert len(o["trk_seed"]) > 100
+    compare(ev, orc, g, o, label="params", min_assign=0.998)
 
 
 def test_batch_as_extra_sectors(orc):
