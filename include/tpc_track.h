@@ -154,7 +154,8 @@ int tpc_debug_copy_tracklets(tpc_tracker_t* t, float* par, float* cov, float* ch
                              void* stream);
 /* owner[h] = rank of the owning seed or -1; n int32. */
 int tpc_debug_copy_owner(tpc_tracker_t* t, int32_t* owner, void* stream);
-/* Sorted-grid view of a1: ids_sorted[n] (cluster id at each sorted position), bin_start [n_sectors*n_rows *
+/* Sorted-grid view of a1 for the most recent call (the grid resolution is chosen per call from the cluster
+ * density): ids_sorted[n] (cluster id at each sorted position), bin_start [n_sectors*n_rows *
  * bins_per_row_stride] ; returns the stride and per-row bin shape through the scalars (host). */
 int tpc_debug_grid_info(const tpc_tracker_t* t, int32_t* bins_stride, int32_t* nz, int32_t* shift_y, int32_t* shift_z);
 int tpc_debug_copy_grid(tpc_tracker_t* t, int32_t* ids_sorted, uint32_t* bin_start, void* stream);
