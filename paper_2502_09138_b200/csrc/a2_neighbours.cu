@@ -129,8 +129,7 @@ a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int
     bs_u = bin_start + (size_t)(sr + 1) * g.nb_stride;
     bs_d = bin_start + (size_t)(sr - 1) * g.nb_stride;
   }
-  // gridDim.y CTAs share a long row (pile-up slices: thousands of clusters per row)
-  for (uint32_t j = a + blockIdx.y * A2_THREADS + threadIdx.x; j < b; j += gridDim.y * A2_THREADS) {
+  for (uint32_t j = a + threadIdx.x; j < b; j += A2_THREADS) {
     const int4 ch = srt[j];
     const int yh = ch.x, zh = ch.y, hid = ch.z;
     int best_u = -1, best_d = -1;
@@ -199,7 +198,7 @@ a2_neighbours_dense_kernel(const DevGeom g, const uint32_t* __restrict__ ro, con
   }
   int* const col_u = &cand[0][0][0][threadIdx.x];
   int* const col_d = &cand[1][0][0][threadIdx.x];
-  // gridDim.y CTAs share a long row (pile-up slices: thousands of clusters per row)
+  // gridDim.y CTAs share a row (dense rows hold thousands of clusters)
   for (uint32_t j = a + blockIdx.y * A2_THREADS + threadIdx.x; j < b; j += gridDim.y * A2_THREADS) {
     const int4 ch = srt[j];
     const int yh = ch.x, zh = ch.y, hid = ch.z;
@@ -245,16 +244,15 @@ cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64
   // z-bins narrower than the window
   const bool dense = (double)n > 0.75 * (double)R * (double)(t->g.ny * t->g.nz);
   const bool fine = t->g.shift_z < t->base_shift_z;
-  // CTAs per row from the average row length (a longer row just loops)
-  int64_t per_row = (n / R + A2_THREADS - 1) / A2_THREADS;
-  if (per_row < 1) per_row = 1;
-  if (per_row > 64) per_row = 64;
-  const dim3 grid((unsigned)R, (unsigned)per_row);
 #define A2_ARGS t->g, ro, t->s.srt, t->s.sec_key, t->s.bin_start, t->s.link_up, t->s.link_dn, t->s.owner
-  if (dense && fine) a2_neighbours_dense_kernel<true><<<grid, A2_THREADS, 0, st>>>(A2_ARGS);
-  else if (dense) a2_neighbours_dense_kernel<false><<<grid, A2_THREADS, 0, st>>>(A2_ARGS);
-  else if (fine) a2_neighbours_kernel<true><<<grid, A2_THREADS, 0, st>>>(A2_ARGS);
-  else a2_neighbours_kernel<false><<<grid, A2_THREADS, 0, st>>>(A2_ARGS);
+  // dense rows: CTAs per row from the average row length (a longer row just loops)
+  int64_t per_row = (n / R + A2_THREADS - 1) / A2_THREADS;
+  per_row = per_row < 1 ? 1 : (per_row > 64 ? 64 : per_row);
+  const dim3 grid2((unsigned)R, (unsigned)per_row);
+  if (dense && fine) a2_neighbours_dense_kernel<true><<<grid2, A2_THREADS, 0, st>>>(A2_ARGS);
+  else if (dense) a2_neighbours_dense_kernel<false><<<grid2, A2_THREADS, 0, st>>>(A2_ARGS);
+  else if (fine) a2_neighbours_kernel<true><<<(unsigned)R, A2_THREADS, 0, st>>>(A2_ARGS);
+  else a2_neighbours_kernel<false><<<(unsigned)R, A2_THREADS, 0, st>>>(A2_ARGS);
 #undef A2_ARGS
   return cudaGetLastError();
 }
