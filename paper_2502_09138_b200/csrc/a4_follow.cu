@@ -29,7 +29,7 @@ namespace {
 
 // Precision: state in fp32, covariance and gain in fp64.  With an fp32 covariance
 // 0.6 % (config 1) to 1.3 % (config 4) of the tracklets miss the 1e-4 bar on q/pT (cancellation in C - K H C
-// after the P22 reset); with the covariance in fp64 none does (measured: profiles/r01_a4_precision.md).
+// after the P22 reset); with the covariance in fp64 none does.
 #ifdef TPC_A4_COV32
 typedef float creal;
 #else
