@@ -301,7 +301,10 @@ enum : int { PH_IDLE = 0, PH_INIT, PH_A, PH_B, PH_CS, PH_CD, PH_FIN, PH_DONE };
 enum : int { M_NONE = 0, M_LINK, M_TABLE, M_SEARCH };
 
 constexpr int A4_THREADS = 128;   // warps never synchronise with each other after the geometry tables are loaded
-constexpr int A4_MIN_BLOCKS = 4;  // 16 warps per SM: registers capped at 128 per thread
+#ifndef TPC_A4_MIN_BLOCKS
+#define TPC_A4_MIN_BLOCKS 4   // 16 warps per SM: registers capped at 128 per thread (5 and 6 measured slower)
+#endif
+constexpr int A4_MIN_BLOCKS = TPC_A4_MIN_BLOCKS;
 
 __global__ void __launch_bounds__(A4_THREADS, A4_MIN_BLOCKS)
 a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restrict__ rec,
