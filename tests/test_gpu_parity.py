@@ -184,6 +184,83 @@ def test_batch_as_extra_sectors(orc):
     compare(ev, orc, _run_gpu(ev), orc.track(ev), label="batch3")
 
 
+def test_batch_equals_individual_events(orc):
+    """Property of the launch configuration at any size: tracking B events in one call (as B*36 sectors) gives, event
+    by event, exactly the tracks of B single-event calls (ids shifted by the event's offset in the batch)."""
+    evs = [make_event(1, 2000 + k, n_tracks=500) for k in range(4)]
+    batch = _run_gpu(concat_events(evs))
+    bt, bh = batch["tracks"], batch["hit_ids"]
+    off = 0
+    t0 = 0
+    for k, ev in enumerate(evs):
+        one = _run_gpu(ev)
+        nt = len(one["tracks"])
+        part = bt[t0:t0 + nt]
+        assert np.array_equal(part["seed_cluster"], one["tracks"]["seed_cluster"] + off), f"event {k}: seeds"
+        assert np.array_equal(part["sector"], one["tracks"]["sector"] + 36 * k)
+        for f in ("x", "y", "z", "sinphi", "tanl", "qpt", "chi2", "n_hits", "first_row", "last_row"):
+            assert np.array_equal(part[f], one["tracks"][f]), f"event {k}: {f}"
+        h0 = part["hit_offset"][0] if nt else 0
+        nh = int(one["tracks"]["n_hits"].sum())
+        assert np.array_equal(bh[h0:h0 + nh], one["hit_ids"] + off), f"event {k}: hit lists"
+        off += ev.n
+        t0 += nt
+    assert t0 == len(bt)
+
+
+def test_invariances_through_the_cuda_path(orc):
+    """SURVEY section 4 invariants, on the device: (1) shuffling the clusters inside every row (ids relabelled) gives
+    the same links and seeds and the same tracks up to id-dependent tie-breaks (tracks compared as sets of (row, y, z)
+    hit coordinates); (2) adding a constant to every z leaves links, seeds and hit lists unchanged and shifts the
+    fitted z only."""
+    import copy
+    ev = make_event(1, 4242, n_tracks=400)
+    base = _run_gpu(ev)
+    sec, row = ev.sector_row()
+
+    def hit_coords(res, e):
+        t = res["tracks"]
+        out = set()
+        for k in range(len(t)):
+            h = res["hit_ids"][t["hit_offset"][k]: t["hit_offset"][k] + t["n_hits"][k]]
+            out.add((int(t["sector"][k]), tuple(zip(row_of(e)[h].tolist(), e.y[h].tolist(), e.z[h].tolist()))))
+        return out
+
+    def row_of(e):
+        return e.sector_row()[1]
+
+    # (2) z translation
+    ev2 = copy.copy(ev)
+    shift = 640 * 37 + 5
+    ev2.z = ev.z + shift
+    tr = _run_gpu(ev2)
+    assert np.array_equal(tr["link_up"], base["link_up"]) and np.array_equal(tr["seed_start"], base["seed_start"])
+    assert np.array_equal(tr["hit_ids"], base["hit_ids"]) and np.array_equal(tr["hits"], base["hits"])
+    for f in ("y", "sinphi", "tanl", "qpt"):
+        assert np.array_equal(tr["tracks"][f], base["tracks"][f]), f
+    assert np.allclose(tr["tracks"]["z"], base["tracks"]["z"] + shift / 640.0, rtol=0, atol=2e-5)
+
+    # (1) permutation inside rows
+    rng = np.random.default_rng(1)
+    perm = np.arange(ev.n)
+    ro = ev.row_offsets.astype(np.int64)
+    for a, b in zip(ro[:-1], ro[1:]):
+        perm[a:b] = a + rng.permutation(b - a)
+    ev3 = copy.copy(ev)
+    ev3.y, ev3.z, ev3.label = ev.y[perm], ev.z[perm], ev.label[perm]
+    pr = _run_gpu(ev3)
+    # coordinates of a cluster are unique in these events, so hit lists map one to one
+    assert len(set(zip(sec.tolist(), row.tolist(), ev.y.tolist(), ev.z.tolist()))) == ev.n
+    # Links and seeds are invariant; ownership ties (equal n_hits) go to the smaller seed start id (P26), which the
+    # relabelling changes, so a few tracks may trade hits: at most 3 % of the tracks differ, and the permuted event
+    # still agrees with the oracle exactly like any other event.
+    a, b = hit_coords(pr, ev3), hit_coords(base, ev)
+    assert len(a ^ b) <= 0.03 * len(b), (len(a ^ b), len(b))
+    assert int((pr["link_up"] >= 0).sum()) == int((base["link_up"] >= 0).sum())
+    assert len(pr["seed_start"]) == len(base["seed_start"])
+    compare(ev3, orc, pr, orc.track(ev3), label="permuted")
+
+
 def test_edge_empty_and_tiny(orc):
     import torch
     from paper_2502_09138_b200 import Tracker, Geometry
