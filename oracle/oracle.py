@@ -158,6 +158,24 @@ def select(n, n_rows, seed_start, n_hits, hits, params=None):
     return owner, trk_seed[:nt].copy(), trk_n[:nt].copy(), trk_off[:nt].copy(), hit_ids[:nh.value].copy()
 
 
+def refit(y_cm, z_cm, row_offsets, n_sectors, n_rows, row_x, bz, trk_hit_offset, trk_n_owned, hit_ids, params=None):
+    """orc_refit: NEXT-1, refit of every output track over its owned hits (reading P41)."""
+    p = params or default_params()
+    nt = trk_n_owned.shape[0]
+    par = np.zeros((nt, 6), dtype=np.float64)
+    cov = np.zeros((nt, 15), dtype=np.float64)
+    chi2 = np.zeros(nt, dtype=np.float64)
+    n_used = np.zeros(nt, dtype=np.int32)
+    y_cm = np.ascontiguousarray(y_cm, dtype=np.float64)
+    z_cm = np.ascontiguousarray(z_cm, dtype=np.float64)
+    row_x = np.ascontiguousarray(row_x, dtype=np.float64)
+    lib().orc_refit(C.byref(p), C.c_double(bz), C.c_int32(n_sectors), C.c_int32(n_rows), _f64(row_x), _f64(y_cm),
+                    _f64(z_cm), _u32(row_offsets), C.c_int64(nt), _i32(np.ascontiguousarray(trk_hit_offset, np.int32)),
+                    _i32(np.ascontiguousarray(trk_n_owned, np.int32)), _i32(np.ascontiguousarray(hit_ids, np.int32)),
+                    _f64(par), _f64(cov), _f64(chi2), _i32(n_used))
+    return par, cov, chi2, n_used
+
+
 def track(ev, params=None, *, brute=False, search_mode=1, exact_coords=False, timings=None):
     """Whole path on one generated event (gen.events.Event).  Returns a dict with every stage's output.
 
@@ -179,12 +197,15 @@ def track(ev, params=None, *, brute=False, search_mode=1, exact_coords=False, ti
     t.append(time.perf_counter())
     owner, trk_seed, trk_n, trk_off, hit_ids = select(ev.n, ev.n_rows, ss, n_hits, hits, p)
     t.append(time.perf_counter())
+    rf_par, rf_cov, rf_chi2, rf_used = refit(y_cm, z_cm, ev.row_offsets, ev.n_sectors, ev.n_rows, ev.row_x, ev.cfg.bz,
+                                             trk_off, trk_n, hit_ids, p)
     if timings is not None:
         timings.update(neighbours=t[1] - t[0], clean_seeds=t[2] - t[1], follow=t[3] - t[2], select=t[4] - t[3],
                        total=t[4] - t[0])
     return dict(link_up=up, link_dn=dn, up_c=upc, dn_c=dnc, seed_start=ss, seed_len=sl, par=par, cov=cov,
                 chi2=chi2, n_hits=n_hits, hits=hits, owner=owner, trk_seed=trk_seed, trk_n_owned=trk_n,
-                trk_hit_offset=trk_off, hit_ids=hit_ids)
+                trk_hit_offset=trk_off, hit_ids=hit_ids, refit_par=rf_par, refit_cov=rf_cov, refit_chi2=rf_chi2,
+                refit_used=rf_used)
 
 
 def num_threads() -> int:

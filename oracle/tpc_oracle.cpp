@@ -521,3 +521,66 @@ extern "C" int64_t orc_select(const orc_params_t* p, int64_t n, int32_t n_rows, 
   *n_out_hits = nh;
   return nt;
 }
+
+// ------------------------------------------------------------------------------------------------
+// NEXT-1: refit of an output track over its owned hits only.  Reading P41.
+// ------------------------------------------------------------------------------------------------
+extern "C" void orc_refit(const orc_params_t* p, double bz, int32_t n_sectors, int32_t n_rows, const double* row_x,
+                          const double* y, const double* z, const uint32_t* ro, int64_t n_tracks,
+                          const int32_t* trk_hit_offset, const int32_t* trk_n_owned, const int32_t* hit_ids,
+                          double* par, double* cov, double* chi2_out, int32_t* n_used) {
+  const double cq = p->cq_per_tesla * bz;
+  const double sy2 = p->sigma_y * p->sigma_y, sz2 = p->sigma_z * p->sigma_z;
+  const int64_t n_sr = (int64_t)n_sectors * n_rows;
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t t = 0; t < n_tracks; ++t) {
+    const int32_t* h = hit_ids + trk_hit_offset[t];
+    const int32_t m = trk_n_owned[t];
+    std::vector<double> xs(m);
+    for (int32_t j = 0; j < m; ++j) {   // row of hit j: ro[lo] <= h_j < ro[lo+1]
+      int64_t lo = 0, hi = n_sr;
+      while (hi - lo > 1) {
+        int64_t mid = (lo + hi) / 2;
+        if (ro[mid] <= (uint32_t)h[j]) lo = mid; else hi = mid;
+      }
+      xs[j] = row_x[lo % n_rows];
+    }
+    double st[5] = {m > 0 ? y[h[0]] : 0.0, m > 0 ? z[h[0]] : 0.0, 0.0, 0.0, 0.0};
+    double C[25];
+    reset_cov(p, C);
+    double x = m > 0 ? xs[0] : 0.0, chi2 = 0.0;
+    int32_t used = 0;
+    if (m >= 2) {
+      const double dx01 = xs[1] - xs[0], dy = y[h[1]] - y[h[0]], dz = z[h[1]] - z[h[0]];
+      const double chord = std::sqrt(dx01 * dx01 + dy * dy);
+      st[2] = dy / chord;
+      st[3] = dz / chord;
+    }
+    if (m > 0) {
+      orc_update(st, C, y[h[0]], z[h[0]], sy2, sz2);
+      int32_t last = 0;
+      for (int32_t j = 1; j < m; ++j) {   // up
+        if (!orc_transport(cq, p->sinphi_max, xs[j] - x, st, C)) break;
+        x = xs[j];
+        orc_update(st, C, y[h[j]], z[h[j]], sy2, sz2);
+        last = j;
+      }
+      reset_cov(p, C);
+      chi2 += orc_update(st, C, y[h[last]], z[h[last]], sy2, sz2);
+      used = 1;
+      for (int32_t j = last - 1; j >= 0; --j) {   // down
+        if (!orc_transport(cq, p->sinphi_max, xs[j] - x, st, C)) break;
+        x = xs[j];
+        chi2 += orc_update(st, C, y[h[j]], z[h[j]], sy2, sz2);
+        ++used;
+      }
+    }
+    par[t * 6] = x;
+    for (int i = 0; i < 5; ++i) par[t * 6 + 1 + i] = st[i];
+    int q = 0;
+    for (int i = 0; i < 5; ++i)
+      for (int j = 0; j <= i; ++j) cov[t * 15 + q++] = C[i * 5 + j];
+    chi2_out[t] = chi2;
+    n_used[t] = used;
+  }
+}

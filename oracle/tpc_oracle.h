@@ -81,6 +81,18 @@ int64_t orc_select(const orc_params_t* p, int64_t n, int32_t n_rows, int64_t n_s
                    const int32_t* n_hits, const int32_t* hits, int32_t* owner, int32_t* trk_seed,
                    int32_t* trk_n_owned, int32_t* trk_hit_offset, int32_t* hit_ids, int64_t* n_out_hits);
 
+/* ---- NEXT-1: refit of an output track over its owned hits only (reading P41) ----
+ * Hits h_0..h_{m-1} of track t = hit_ids[trk_hit_offset[t] .. + trk_n_owned[t]), ascending row.
+ * State from h_0, h_1 as in P19 (dx = x(row h_1) - x(row h_0)), C = C_reset, update h_0; up: one transport per
+ * hit over the row gap + update, stop at the first failed transport; C = C_reset, chi2 = 0, update with the last
+ * hit reached; down: transport + update back to h_0, stop at a failed transport.
+ * Outputs per track: par[t*6..] = (x_ref, y, z, sin phi, tan lambda, q/pT) at the row where the down pass ended,
+ * cov[t*15..] packed lower triangle, chi2[t] of the down pass, n_used[t] = hits updated in the down pass. */
+void orc_refit(const orc_params_t* p, double bz, int32_t n_sectors, int32_t n_rows, const double* row_x,
+               const double* y_cm, const double* z_cm, const uint32_t* row_offsets, int64_t n_tracks,
+               const int32_t* trk_hit_offset, const int32_t* trk_n_owned, const int32_t* hit_ids, double* par,
+               double* cov, double* chi2, int32_t* n_used);
+
 int orc_num_threads(void);
 
 #ifdef __cplusplus

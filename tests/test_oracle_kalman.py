@@ -255,3 +255,74 @@ def test_selection_invariants(orc):
     assert owner.tolist() == [0] * 5 + [1] * 11
     assert trk_seed.tolist() == [0, 1] and trk_n.tolist() == [5, 11]
     assert hit_ids.tolist() == list(range(5)) + list(range(5, 16))
+
+
+# ---- NEXT-1: refit of output tracks over their owned hits (orc_refit, reading P41) ----
+
+def _refit_truth_errors(ev, o):
+    errs = []
+    for i in range(len(o["trk_seed"])):
+        h0 = o["hit_ids"][o["trk_hit_offset"][i]]
+        par = o["refit_par"][i]
+        tp = truth_params_at(ev, ev.label[h0] // 64, 0, par[0])
+        errs.append(np.abs(par[1:] - tp) / np.maximum(np.abs(tp), 1.0))
+    return np.array(errs)
+
+
+def test_refit_exact_helices_to_1e4(orc):
+    """Pin by the problem: on noise-free exact helices the refit over the owned hits gives the generator's truth
+    parameters at the lowest owned hit to 1e-4 (a wrong gap dx, a dropped update or a wrong pass order fails)."""
+    ev = make_event(0, sigma_scale=0.0)
+    o = orc.track(ev, exact_coords=True)
+    assert len(o["refit_par"]) == 100
+    assert np.array_equal(o["refit_used"], o["trk_n_owned"])          # every owned hit is used on the way down
+    assert _refit_truth_errors(ev, o).max() < 2e-5
+
+
+def test_refit_with_row_gaps_still_reaches_truth(orc):
+    """Owned hit lists with gaps (every third hit removed): transports over several rows at once; the truth pin
+    still holds, so the gap dx is taken from the row positions of the hits, not from a fixed pitch."""
+    ev = make_event(0, sigma_scale=0.0)
+    o = orc.track(ev, exact_coords=True)
+    keep, off, cnt = [], [], []
+    for i in range(len(o["trk_seed"])):
+        h = o["hit_ids"][o["trk_hit_offset"][i]: o["trk_hit_offset"][i] + o["trk_n_owned"][i]]
+        h = np.delete(h, np.arange(2, len(h), 3))
+        off.append(sum(cnt))
+        cnt.append(len(h))
+        keep.append(h)
+    hit_ids = np.concatenate(keep).astype(np.int32)
+    par, cov, chi2, used = orc.refit(ev.y_exact, ev.z_exact, ev.row_offsets, ev.n_sectors, ev.n_rows, ev.row_x,
+                                     ev.cfg.bz, np.array(off, np.int32), np.array(cnt, np.int32), hit_ids)
+    o2 = dict(o, refit_par=par, hit_ids=hit_ids, trk_hit_offset=np.array(off))
+    assert np.array_equal(used, np.array(cnt))
+    assert _refit_truth_errors(ev, o2).max() < 2e-5
+
+
+def test_refit_equals_tracklet_fit_on_full_length_tracks(orc):
+    """Pin against the (independently pinned) follower: for a tracklet that has a hit in every row from 0 to the last
+    row and owns all of them, the follower's downward pass (after the covariance reset) runs over exactly the hits
+    of the refit's downward pass.  The upward passes differ only in where they start (the seed starts in row 1: rows
+    0 and n-1 have no links of their own, P5), which moves the linearisation point of the downward pass by ~1e-9,
+    so the two fits agree to 1e-8 -- and not to more if the refit dropped or reordered a hit."""
+    ev = make_event(0, sigma_scale=0.0)
+    o = orc.track(ev, exact_coords=True)
+    n = 0
+    for i, t in enumerate(o["trk_seed"]):
+        if o["trk_n_owned"][i] == ev.n_rows and (o["hits"][t] >= 0).all():
+            assert np.allclose(o["refit_par"][i], o["par"][t], rtol=0, atol=1e-8)
+            assert np.allclose(o["refit_cov"][i], o["cov"][t], rtol=1e-6, atol=1e-15)
+            assert abs(o["refit_chi2"][i] - o["chi2"][t]) < 1e-8
+            n += 1
+    assert n >= 20
+
+
+def test_refit_nominal_config_improves_nothing_it_should_not(orc):
+    """Sanity on smeared data: chi2 per degree of freedom of the refit is ~1 (errors sigma_y, sigma_z are the true
+    smearing in configs[0]) -- a transposed gain or a wrong V would move it far away."""
+    ev = make_event(0)
+    o = orc.track(ev)
+    ndf = 2 * o["refit_used"] - 5
+    ok = ndf > 20
+    r = o["refit_chi2"][ok] / ndf[ok]
+    assert 0.8 < np.median(r) < 1.2
