@@ -122,6 +122,16 @@ int tpc_track(tpc_tracker_t* t, const tpc_clusters_t* clusters, int64_t n, void*
 int tpc_track_host(tpc_tracker_t* t, const tpc_clusters_t* clusters_host, int64_t n, void* stream,
                    tpc_tracks_out_t* out_host);
 
+/* NEXT-1 (reading P41 in DESIGN.md): refit of the tracks the most recent tpc_track call on this handle
+ * wrote, over their owned hits only (the parameters tpc_track reports are the fit over all hits of the tracklet,
+ * P28).  `clusters` and `n` must be those of that call, `tracks` its output (all [device]); refit_out: [device]
+ * track_capacity records, written for the first min(counts[0], track_capacity) tracks: x .. chi2 hold the refit at
+ * the row where its downward pass ended, n_hits the hits used on the way down, the other fields are copied.
+ * Asynchronous on `stream` (the same stream, or one ordered after the tpc_track call).  Not part of tpc_track.
+ * Errors: TPC_ERR_ARG (also when `clusters` is not the input of the handle's last call), TPC_ERR_CUDA. */
+int tpc_refit(tpc_tracker_t* t, const tpc_clusters_t* clusters, int64_t n, void* stream, const tpc_tracks_out_t* tracks,
+              tpc_track_rec_t* refit_out);
+
 int tpc_tracker_destroy(tpc_tracker_t* t);
 
 const char* tpc_status_string(int status);

@@ -95,6 +95,8 @@ def load_library():
     lib.tpc_tracker_create.argtypes = [C.POINTER(_Geometry), C.POINTER(_Field), C.POINTER(C.c_void_p)]
     lib.tpc_track.argtypes = [C.c_void_p, C.POINTER(_Clusters), C.c_int64, C.c_void_p, C.POINTER(_TracksOut)]
     lib.tpc_track_host.argtypes = lib.tpc_track.argtypes
+    lib.tpc_refit.argtypes = [C.c_void_p, C.POINTER(_Clusters), C.c_int64, C.c_void_p, C.POINTER(_TracksOut),
+                              C.c_void_p]
     lib.tpc_tracker_destroy.argtypes = [C.c_void_p]
     lib.tpc_status_string.argtypes = [C.c_int]
     lib.tpc_status_string.restype = C.c_char_p
@@ -236,6 +238,19 @@ class Tracker:
                        _ptr(out.hit_ids), _ptr(out.counts))
         self._check(self._lib.tpc_track(self._h, C.byref(cl), C.c_int64(n), self._stream_ptr(stream), C.byref(o)))
         return out
+
+    def refit(self, y, z, row_offsets, out: "TracksOut", stream=None):
+        """tpc_refit on the output of the last track() call with the same inputs; returns a device uint8 tensor of
+        track records (same layout as out.tracks)."""
+        import torch
+        n = int(y.shape[0])
+        cl = _Clusters(_ptr(y), _ptr(z), _ptr(row_offsets))
+        o = _TracksOut(_ptr(out.tracks), int(out.tracks.shape[0] // 112), int(out.hit_ids.shape[0]), _ptr(out.hit_ids),
+                       _ptr(out.counts))
+        ref = torch.zeros_like(out.tracks)
+        self._check(self._lib.tpc_refit(self._h, C.byref(cl), C.c_int64(n), self._stream_ptr(stream), C.byref(o),
+                                        _ptr(ref)))
+        return ref
 
     def track_host(self, y, z, row_offsets, tracks, hit_ids, counts, stream=None):
         """tpc_track_host: all arguments are HOST tensors (pinned for asynchronous copies): y, z int32 [n],

@@ -1,0 +1,147 @@
+// a6_refit.cu -- NEXT-1: refit of the output tracks over their owned hits only (reading P41,
+// DESIGN.md; the a4 fit of a track runs over all hits of its tracklet, P28, including hits another track won).
+//
+// Per track with owned hits h_0 .. h_{m-1} (ascending row): state from h_0, h_1 as in P19 (dx = the row gap),
+// C = C_reset, update h_0; up: one transport over the row gap + update per hit, stop at a failed transport;
+// C = C_reset, chi2 = 0, update with the last hit reached; down: transport + update back to h_0.  Result: state,
+// covariance and x at the row where the down pass ended, chi2 and the number of hits of the down pass.
+//
+// Same execution model as a4: persistent warps, one lane per track, lanes refill from a device counter, one
+// uniform step (optional covariance reset, optional transport, update) for both passes; fp32 state relative to
+// the first hit, fp64 covariance.  The hit's (y, z) comes from the a3 records of the same call (rec[id]).
+#include "tpc_internal.cuh"
+#include "kalman.cuh"
+
+namespace {
+
+constexpr int A6_THREADS = 128;
+
+enum : int { R_IDLE = 0, R_FIRST, R_UP, R_TOP, R_DOWN };
+
+__global__ void __launch_bounds__(A6_THREADS, 4)
+a6_refit_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const uint32_t* __restrict__ ro,
+                const int4* __restrict__ rec, const tpc_track_rec_t* __restrict__ tracks, int32_t track_capacity,
+                const int32_t* __restrict__ hit_ids, int32_t hit_capacity, const int32_t* __restrict__ counts,
+                tpc_track_rec_t* __restrict__ out) {
+  extern __shared__ double s_row_x[];
+  const unsigned FULL = 0xffffffffu;
+  const int lane = threadIdx.x & 31;
+  const int nr = g.n_rows;
+  for (int r = threadIdx.x; r < nr; r += blockDim.x) s_row_x[r] = g.row_x[r];
+  __syncthreads();
+  // tracks whose record or hit list was not written (capacity overflow) are not refitted
+  const uint32_t n_tracks = (uint32_t)min(counts[0], track_capacity);
+  const bool hits_ok = counts[1] <= hit_capacity;
+  if (n_tracks == 0 || !hits_ok) return;
+
+  int phase = R_IDLE;
+  bool exhausted = false;
+  int k = -1, m = 0, j = 0, last = 0, used = 0, sb = 0, row = 0, y0 = 0, z0 = 0;
+  const int32_t* hl = hit_ids;
+  float chi2 = 0.f;
+  State p;
+  Cov C;
+  p.y = p.z = p.s = p.t = p.q = 0;
+  cov_reset(g, C);
+
+  while (true) {
+    const bool want = phase == R_IDLE && !exhausted;
+    const unsigned idle = __ballot_sync(FULL, want);
+    if (idle) {
+      uint32_t base = 0;
+      if (lane == 0) base = atomicAdd(&ctl->next_track, (uint32_t)__popc(idle));
+      base = __shfl_sync(FULL, base, 0);
+      if (base + (uint32_t)__popc(idle) >= n_tracks) exhausted = true;
+      const uint32_t kk = base + (uint32_t)__popc(idle & ((1u << lane) - 1u));
+      if (want && kk < n_tracks) {
+        k = (int)kk;
+        const tpc_track_rec_t* t = tracks + k;
+        m = t->n_hits;
+        hl = hit_ids + t->hit_offset;
+        sb = t->sector * nr;
+        row = t->first_row;
+        const int4 c0 = rec[hl[0]];
+        y0 = c0.x;
+        z0 = c0.y;
+        p.y = 0; p.z = 0; p.s = 0; p.t = 0; p.q = 0;
+        if (m >= 2) {   // P19 with the gap to the second owned hit
+          const int h1 = hl[1];
+          int r1 = row;
+          while (ro[sb + r1 + 1] <= (uint32_t)h1) ++r1;
+          const int4 c1 = rec[h1];
+          const float dxr = (float)(s_row_x[r1] - s_row_x[row]);
+          const float dy = (float)(c1.x - y0) * g.inv_units, dz = (float)(c1.y - z0) * g.inv_units;
+          const float ichord = rsqrtf(fmaf(dxr, dxr, dy * dy));
+          p.s = dy * ichord;
+          p.t = dz * ichord;
+        }
+        j = 0; last = 0; used = 0; chi2 = 0.f;
+        phase = R_FIRST;
+      }
+    }
+    if (!__any_sync(FULL, phase != R_IDLE)) break;
+
+    // ---- one step: which hit, reset?, transport? ----
+    if (phase == R_UP && j >= m) phase = R_TOP;
+    if (phase == R_TOP) j = last;
+    const int ph = phase;
+    const bool active = ph != R_IDLE;
+    const bool reset = ph == R_FIRST || ph == R_TOP;
+    const bool tr = ph == R_UP || ph == R_DOWN;
+    int hid = 0, trow = row;
+    int4 c = make_int4(y0, z0, 0, 0);
+    if (active) {
+      hid = hl[j];
+      c = rec[hid];
+      if (ph == R_UP) while (ro[sb + trow + 1] <= (uint32_t)hid) ++trow;
+      if (ph == R_DOWN) while (ro[sb + trow] > (uint32_t)hid) --trow;
+    }
+    if (active && reset) cov_reset(g, C);
+    if (ph == R_TOP) { chi2 = 0.f; used = 0; }
+    bool ok = active;
+    if (tr) ok = transport<true>(g, (float)(s_row_x[trow] - s_row_x[row]), p, C);
+    if (ok) {
+      row = trow;
+      chi2 += update(g, p, C, (float)(c.x - y0) * g.inv_units, (float)(c.y - z0) * g.inv_units);
+      ++used;
+      if (ph == R_FIRST) { phase = R_UP; j = 1; }
+      else if (ph == R_UP) { last = j; ++j; }
+      else if (ph == R_TOP) { phase = R_DOWN; j = last - 1; }
+      else --j;
+    } else if (ph == R_UP) {
+      phase = R_TOP;   // P18: the up pass stops, the hits above are not used
+    }
+    // the down pass is over: transport failed, or h_0 is done
+    if (active && ((ph == R_DOWN && !ok) || (phase == R_DOWN && j < 0))) {
+      tpc_track_rec_t r = tracks[k];
+      r.x = (float)s_row_x[row];
+      r.y = (float)((double)p.y + (double)y0 * g.inv_units_d);
+      r.z = (float)((double)p.z + (double)z0 * g.inv_units_d);
+      r.sinphi = (float)p.s;
+      r.tanl = (float)p.t;
+      r.qpt = (float)p.q;
+      const float cv[15] = {(float)C.c00, (float)C.c10, (float)C.c11, (float)C.c20, (float)C.c21,
+                            (float)C.c22, (float)C.c30, (float)C.c31, (float)C.c32, (float)C.c33,
+                            (float)C.c40, (float)C.c41, (float)C.c42, (float)C.c43, (float)C.c44};
+#pragma unroll
+      for (int q = 0; q < 15; ++q) r.cov[q] = cv[q];
+      r.chi2 = chi2;
+      r.n_hits = used;
+      out[k] = r;
+      phase = R_IDLE;
+    }
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_a6_refit(const tpc_tracker* t, const uint32_t* ro, const tpc_tracks_out_t* tracks,
+                            tpc_track_rec_t* refit_out, cudaStream_t st) {
+  if (t->last_n == 0 || t->a4_blocks == 0 || tracks->track_capacity == 0) return cudaSuccess;
+  cudaError_t e = cudaMemsetAsync(&t->s.ctl->next_track, 0, sizeof(uint32_t), st);
+  if (e != cudaSuccess) return e;
+  a6_refit_kernel<<<t->a4_blocks, A6_THREADS, (size_t)t->g.n_rows * sizeof(double), st>>>(
+      t->g, t->s.ctl, ro, t->s.rec, tracks->tracks, tracks->track_capacity, tracks->hit_ids, tracks->hit_capacity,
+      tracks->counts, refit_out);
+  return cudaGetLastError();
+}

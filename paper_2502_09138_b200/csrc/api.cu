@@ -324,6 +324,19 @@ int tpc_track(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* strea
   return TPC_OK;
 }
 
+int tpc_refit(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* stream, const tpc_tracks_out_t* tracks,
+              tpc_track_rec_t* refit_out) {
+  if (!t || !cl || !tracks || n < 0) return TPC_ERR_ARG;
+  if (!tracks->counts || tracks->track_capacity < 0 || tracks->hit_capacity < 0) return TPC_ERR_ARG;
+  if (tracks->track_capacity > 0 && (!tracks->tracks || !refit_out)) return TPC_ERR_ARG;
+  if (tracks->hit_capacity > 0 && !tracks->hit_ids) return TPC_ERR_ARG;
+  // the records of the clusters (a3) must be those of the call that produced `tracks`
+  if (!t->arena || n != t->last_n || cl->row_offsets != t->last_ro || cl->y != t->last_y || cl->z != t->last_z)
+    return TPC_ERR_ARG;
+  TPC_CUDA(t, launch_a6_refit(t, cl->row_offsets, tracks, refit_out, (cudaStream_t)stream));
+  return TPC_OK;
+}
+
 int tpc_track_host(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* stream, tpc_tracks_out_t* out) {
   if (!t || !cl || !out || n < 0) return TPC_ERR_ARG;
   if (!out->counts || out->track_capacity < 0 || out->hit_capacity < 0) return TPC_ERR_ARG;

@@ -30,7 +30,8 @@ struct DevCtl {
   uint32_t ticket_a3;    // dynamic tile ids for the a3 look-back scan
   uint32_t ticket_a5;
   uint32_t next_seed;    // a4 work queue: next seed rank to hand to a free lane
-  uint32_t pad[12];
+  uint32_t next_track;   // a6 work queue
+  uint32_t pad[11];
 };
 
 struct Scratch {
@@ -102,6 +103,8 @@ cudaError_t launch_a3_seeds(const tpc_tracker* t, const int32_t* y, const int32_
 cudaError_t launch_a4_follow(const tpc_tracker* t, int64_t n, cudaStream_t st);
 cudaError_t setup_a4_attributes(tpc_tracker* t);
 cudaError_t launch_a5_select(const tpc_tracker* t, const tpc_tracks_out_t* out, cudaStream_t st);
+cudaError_t launch_a6_refit(const tpc_tracker* t, const uint32_t* ro, const tpc_tracks_out_t* tracks,
+                            tpc_track_rec_t* refit_out, cudaStream_t st);
 cudaError_t setup_a1_attributes(const tpc_tracker* t);
 size_t a1_smem_bytes(const DevGeom& g);
 

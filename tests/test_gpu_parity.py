@@ -261,6 +261,72 @@ def test_invariances_through_the_cuda_path(orc):
     compare(ev3, orc, pr, orc.track(ev3), label="permuted")
 
 
+def _refit_parity(ev, orc, label, params=None):
+    """tpc_refit against orc_refit on the tracks both sides output with identical hit lists."""
+    import torch
+    from paper_2502_09138_b200 import Tracker, TRACK_DTYPE
+    from paper_2502_09138_b200.events import geometry_from_event, upload
+    trk = Tracker(geometry_from_event(ev, params))
+    y, z, ro = upload(ev)
+    out = trk.track(y, z, ro)
+    ref = trk.refit(y, z, ro, out)
+    tracks, hit_ids, _ = out.to_host()
+    rf = ref[: len(tracks) * 112].cpu().numpy().view(TRACK_DTYPE)
+    trk.close()
+    o = orc.track(ev)
+    okey = {int(s): i for i, s in enumerate(o["seed_start"][o["trk_seed"]])}
+    n_same = n_bad = 0
+    worst = np.zeros(5)
+    for k in range(len(tracks)):
+        i = okey.get(int(tracks["seed_cluster"][k]))
+        if i is None:
+            continue
+        gh = hit_ids[tracks["hit_offset"][k]: tracks["hit_offset"][k] + tracks["n_hits"][k]]
+        oh = o["hit_ids"][o["trk_hit_offset"][i]: o["trk_hit_offset"][i] + o["trk_n_owned"][i]]
+        if len(gh) != len(oh) or not np.array_equal(gh, oh):
+            continue
+        n_same += 1
+        rp = o["refit_par"][i]
+        assert rf["x"][k] == np.float32(rp[0]), f"{label}: x_ref of track {k}"
+        assert rf["n_hits"][k] == o["refit_used"][i], f"{label}: hits used by the refit of track {k}"
+        g = np.array([rf["y"][k], rf["z"][k], rf["sinphi"][k], rf["tanl"][k], rf["qpt"][k]], dtype=np.float64)
+        err = np.abs(g - rp[1:]) / np.maximum(np.abs(rp[1:]), 1.0)
+        worst = np.maximum(worst, err)
+        n_bad += int((err > TOL).any())
+        assert abs(rf["chi2"][k] - o["refit_chi2"][i]) <= 1e-3 * max(1.0, o["refit_chi2"][i])
+        for f in ("sector", "first_row", "last_row", "hit_offset", "seed_cluster"):
+            assert rf[f][k] == tracks[f][k]
+    assert n_same >= 0.999 * len(o["trk_seed"]), (label, n_same, len(o["trk_seed"]))
+    assert n_bad <= 1e-3 * n_same, f"{label}: {n_bad} refits beyond 1e-4, worst {worst}"
+    return n_same, worst
+
+
+def test_refit_config0_and_exact(orc):
+    """NEXT-1: refit over owned hits, CUDA against the oracle; on exact helices every refit uses all its hits."""
+    for ev in (make_event(0), make_event(0, 1), make_event(0, sigma_scale=0.0)):
+        n, worst = _refit_parity(ev, orc, "refit cfg0")
+        assert n >= 100 and worst.max() < TOL
+
+
+def test_refit_config1_and_stress(orc):
+    _refit_parity(make_event(1, 1000), orc, "refit cfg1")
+    _refit_parity(make_event(4), orc, "refit cfg4")       # loopers: failed transports, short down passes
+
+
+def test_refit_rejects_foreign_input(orc):
+    import torch
+    from paper_2502_09138_b200 import Tracker
+    from paper_2502_09138_b200.binding import TpcError
+    from paper_2502_09138_b200.events import geometry_from_event, upload
+    ev = make_event(0)
+    trk = Tracker(geometry_from_event(ev))
+    y, z, ro = upload(ev)
+    out = trk.track(y, z, ro)
+    with pytest.raises(TpcError):
+        trk.refit(y.clone(), z, ro, out)      # not the arrays of the last call
+    trk.close()
+
+
 def test_edge_empty_and_tiny(orc):
     import torch
     from paper_2502_09138_b200 import Tracker, Geometry
