@@ -187,6 +187,18 @@ def run_ours(args):
     grid = trk.debug_grid(n)
     n_bins = float(grid["stride"]) * trk.n_sectors * trk.n_rows
 
+    # ---- NEXT-1: tpc_refit on the tracks of the last call (not part of the step; reported beside it) --------
+    for _ in range(2):
+        trk.refit(y, z, ro, out, stream)
+    torch.cuda.synchronize()
+    r0e, r1e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    r0e.record(stream)
+    for _ in range(5):
+        trk.refit(y, z, ro, out, stream)
+    r1e.record(stream)
+    torch.cuda.synchronize()
+    refit_ms = r0e.elapsed_time(r1e) / 5
+
     # ---- single-event latency (B = 1), for context -------------------------------------------------------
     ev1 = evs[0]
     trk1 = Tracker(geometry_from_event(ev1))
@@ -313,6 +325,8 @@ def run_ours(args):
                              f"> 126 MB L2; no explicit flush"},
             "tracks_per_s": len(tracks) * world * args.steps / (ms_max * 1e-3),
             "single_event_latency_ms": latency_ms,
+            "next": {"a6_refit_ms": refit_ms, "tracks_refitted": len(tracks),
+                     "note": "tpc_refit over the step's output tracks; outside the timed step"},
             "e2e": {"value": e2e_units / (e2e_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "steps": e2e_steps, "ms_per_step": e2e_max / e2e_steps,
                     "host_threads": T},
