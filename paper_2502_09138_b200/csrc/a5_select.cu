@@ -21,7 +21,8 @@ __global__ void __launch_bounds__(256)
 a5_select_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int32_t* __restrict__ seed_start,
                  const float4* __restrict__ tl_rec, const int32_t* __restrict__ tl_hits,
                  const uint32_t* __restrict__ owner, uint64_t* __restrict__ status,
-                 tpc_track_rec_t* __restrict__ tracks, int32_t track_capacity, int32_t* __restrict__ hit_ids,
+                 uint8_t* __restrict__ hit_row, tpc_track_rec_t* __restrict__ tracks, int32_t track_capacity,
+                 int32_t* __restrict__ hit_ids,
                  int32_t hit_capacity, int32_t* __restrict__ counts) {
   __shared__ uint32_t wsum[33];
   __shared__ uint32_t sh_tile;
@@ -141,7 +142,11 @@ a5_select_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int32_t* __res
     const int32_t* src = tl_hits + (t0 + t) * nr;
     for (int k = 0; k < n_words; ++k) {
       const unsigned m = own_mask[t][k];
-      if ((m >> lane) & 1u) hit_ids[w + __popc(m & ((1u << lane) - 1u))] = src[k * 32 + lane];
+      if ((m >> lane) & 1u) {
+        const uint32_t at = w + __popc(m & ((1u << lane) - 1u));
+        hit_ids[at] = src[k * 32 + lane];
+        hit_row[at] = (uint8_t)(k * 32 + lane);   // for a6 (tpc_refit): the row of every output hit
+      }
       w += __popc(m);
     }
   }
@@ -169,7 +174,7 @@ cudaError_t launch_a5_select(const tpc_tracker* t, const tpc_tracks_out_t* out, 
   const unsigned blocks = (unsigned)((t->s_cap + A5_TILE - 1) / A5_TILE);
   const int row_threads = 32 * ((t->g.n_rows + 31) / 32);
   a5_select_kernel<<<blocks, row_threads > A5_TILE ? row_threads : A5_TILE, 0, st>>>(t->g, t->s.ctl, t->s.seed_start, t->s.tl_rec, t->s.tl_hits, t->s.owner,
-                                              t->s.scan_a5, out->tracks, out->track_capacity, out->hit_ids,
+                                              t->s.scan_a5, t->s.hit_row, out->tracks, out->track_capacity, out->hit_ids,
                                               out->hit_capacity, out->counts);
   return cudaGetLastError();
 }

@@ -8,7 +8,8 @@
 //
 // Same execution model as a4: persistent warps, one lane per track, lanes refill from a device counter, one
 // uniform step (optional covariance reset, optional transport, update) for both passes; fp32 state relative to
-// the first hit, fp64 covariance.  The hit's (y, z) comes from the a3 records of the same call (rec[id]).
+// the first hit, fp64 covariance.  The hit's (y, z) comes from the a3 records of the same call (rec[id]), requested
+// one step ahead; its row from the row list a5 wrote next to the hit list.
 #include "tpc_internal.cuh"
 #include "kalman.cuh"
 
@@ -18,11 +19,17 @@ constexpr int A6_THREADS = 128;
 
 enum : int { R_IDLE = 0, R_FIRST, R_UP, R_TOP, R_DOWN };
 
+// Predicated loads straight into their destination registers (see a4_follow.cu for why they are PTX).
+__device__ __forceinline__ void ld_yz_if(int& y, int& z, const int4* p, bool pred) {
+  asm volatile("{ .reg .pred q; setp.ne.s32 q, %2, 0; @q ld.global.nc.s32 %0, [%3]; @q ld.global.nc.s32 %1, [%3+4]; }"
+               : "+r"(y), "+r"(z) : "r"((int)pred), "l"(p));
+}
+
 __global__ void __launch_bounds__(A6_THREADS, 4)
-a6_refit_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const uint32_t* __restrict__ ro,
-                const int4* __restrict__ rec, const tpc_track_rec_t* __restrict__ tracks, int32_t track_capacity,
-                const int32_t* __restrict__ hit_ids, int32_t hit_capacity, const int32_t* __restrict__ counts,
-                tpc_track_rec_t* __restrict__ out) {
+a6_refit_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restrict__ rec,
+                const uint8_t* __restrict__ hit_row, const tpc_track_rec_t* __restrict__ tracks,
+                int32_t track_capacity, const int32_t* __restrict__ hit_ids, int32_t hit_capacity,
+                const int32_t* __restrict__ counts, tpc_track_rec_t* __restrict__ out) {
   extern __shared__ double s_row_x[];
   const unsigned FULL = 0xffffffffu;
   const int lane = threadIdx.x & 31;
@@ -36,8 +43,10 @@ a6_refit_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const uint32_t* __res
 
   int phase = R_IDLE;
   bool exhausted = false;
-  int k = -1, m = 0, j = 0, last = 0, used = 0, sb = 0, row = 0, y0 = 0, z0 = 0;
-  const int32_t* hl = hit_ids;
+  int k = -1, m = 0, j = 0, last = 0, used = 0, row = 0, y0 = 0, z0 = 0;
+  const int32_t* hl = hit_ids;     // this track's hit ids ...
+  const uint8_t* hr = hit_row;     // ... and their rows (a5)
+  int pf_j = -1, pf_y = 0, pf_z = 0;   // (y, z) of hit pf_j, requested one step ahead
   float chi2 = 0.f;
   State p;
   Cov C;
@@ -58,18 +67,16 @@ a6_refit_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const uint32_t* __res
         const tpc_track_rec_t* t = tracks + k;
         m = t->n_hits;
         hl = hit_ids + t->hit_offset;
-        sb = t->sector * nr;
-        row = t->first_row;
+        hr = hit_row + t->hit_offset;
+        row = hr[0];
         const int4 c0 = rec[hl[0]];
         y0 = c0.x;
         z0 = c0.y;
+        pf_j = 0; pf_y = y0; pf_z = z0;
         p.y = 0; p.z = 0; p.s = 0; p.t = 0; p.q = 0;
         if (m >= 2) {   // P19 with the gap to the second owned hit
-          const int h1 = hl[1];
-          int r1 = row;
-          while (ro[sb + r1 + 1] <= (uint32_t)h1) ++r1;
-          const int4 c1 = rec[h1];
-          const float dxr = (float)(s_row_x[r1] - s_row_x[row]);
+          const int4 c1 = rec[hl[1]];
+          const float dxr = (float)(s_row_x[hr[1]] - s_row_x[row]);
           const float dy = (float)(c1.x - y0) * g.inv_units, dz = (float)(c1.y - z0) * g.inv_units;
           const float ichord = rsqrtf(fmaf(dxr, dxr, dy * dy));
           p.s = dy * ichord;
@@ -88,13 +95,22 @@ a6_refit_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const uint32_t* __res
     const bool active = ph != R_IDLE;
     const bool reset = ph == R_FIRST || ph == R_TOP;
     const bool tr = ph == R_UP || ph == R_DOWN;
-    int hid = 0, trow = row;
-    int4 c = make_int4(y0, z0, 0, 0);
+    int trow = row, cy = pf_y, cz = pf_z;
     if (active) {
-      hid = hl[j];
-      c = rec[hid];
-      if (ph == R_UP) while (ro[sb + trow + 1] <= (uint32_t)hid) ++trow;
-      if (ph == R_DOWN) while (ro[sb + trow] > (uint32_t)hid) --trow;
+      trow = hr[j];
+      ld_yz_if(cy, cz, rec + hl[j], pf_j != j);   // not requested ahead (after a pass ended early): load now
+    }
+    // the hit of the next step: its record is requested now and used then
+    {
+      int jn = -1;
+      if (ph == R_FIRST) jn = 1;
+      if (ph == R_UP) jn = j + 1;
+      if (ph == R_TOP || ph == R_DOWN) jn = j - 1;
+      const bool fetch = active && jn >= 0 && jn < m;
+      int hn = 0;
+      if (fetch) hn = hl[jn];
+      if (fetch) pf_j = jn;
+      ld_yz_if(pf_y, pf_z, rec + hn, fetch);
     }
     if (active && reset) cov_reset(g, C);
     if (ph == R_TOP) { chi2 = 0.f; used = 0; }
@@ -102,7 +118,7 @@ a6_refit_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const uint32_t* __res
     if (tr) ok = transport<true>(g, (float)(s_row_x[trow] - s_row_x[row]), p, C);
     if (ok) {
       row = trow;
-      chi2 += update(g, p, C, (float)(c.x - y0) * g.inv_units, (float)(c.y - z0) * g.inv_units);
+      chi2 += update(g, p, C, (float)(cy - y0) * g.inv_units, (float)(cz - z0) * g.inv_units);
       ++used;
       if (ph == R_FIRST) { phase = R_UP; j = 1; }
       else if (ph == R_UP) { last = j; ++j; }
@@ -141,7 +157,7 @@ cudaError_t launch_a6_refit(const tpc_tracker* t, const uint32_t* ro, const tpc_
   cudaError_t e = cudaMemsetAsync(&t->s.ctl->next_track, 0, sizeof(uint32_t), st);
   if (e != cudaSuccess) return e;
   a6_refit_kernel<<<t->a4_blocks, A6_THREADS, (size_t)t->g.n_rows * sizeof(double), st>>>(
-      t->g, t->s.ctl, ro, t->s.rec, tracks->tracks, tracks->track_capacity, tracks->hit_ids, tracks->hit_capacity,
-      tracks->counts, refit_out);
+      t->g, t->s.ctl, t->s.rec, t->s.hit_row, tracks->tracks, tracks->track_capacity, tracks->hit_ids,
+      tracks->hit_capacity, tracks->counts, refit_out);
   return cudaGetLastError();
 }

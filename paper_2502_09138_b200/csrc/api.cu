@@ -55,6 +55,7 @@ size_t layout(tpc_tracker* t, char* base, int64_t n, int64_t R) {
   s.link_dn = (int32_t*)take((size_t)n * 4);
   s.rec = (int4*)take((size_t)n * 16);
   s.owner = (uint32_t*)take((size_t)n * 4);
+  s.hit_row = (uint8_t*)take((size_t)n + 64);
   s.seed_start = (int32_t*)take((size_t)s_cap * 4);
   s.seed_sr = (int32_t*)take((size_t)s_cap * 4);
   s.tl_rec = (float4*)take((size_t)s_cap * TL_REC_V4 * 16);

@@ -43,6 +43,7 @@ struct Scratch {
   int32_t *link_up, *link_dn;
   int4* rec;                // a3: per cluster id (y, z, cleaned up link, cleaned down link) -- one 16-B gather per a4 step
   uint32_t* owner;          // packed (n_hits << 24 | 0xFFFFFF - rank), 0 = none
+  uint8_t* hit_row;         // [n] a5: row of the hit at each position of the output hit list (for a6)
   // a3 -> a4
   int32_t* seed_start;      // [s_cap] start cluster id, ascending
   int32_t* seed_sr;         // [s_cap] sector * n_rows + row of the start cluster
