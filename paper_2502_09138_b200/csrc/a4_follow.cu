@@ -24,122 +24,9 @@
 //    tracklet ends the whole warp pads it with -1 and casts the ownership votes, 32 rows per instruction.  No
 //    shared memory beyond two small geometry tables, so L1 keeps its full size for the gathers.
 #include "tpc_internal.cuh"
-#include "kalman.cuh"
+#include "a4_search.cuh"
 
 namespace {
-
-__device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
-
-struct Found {
-  int id;
-  float y, z;   // relative coordinates of the accepted hit
-};
-
-// The search window of P17/P21 in grid bins.  A cluster can only be accepted if dy^2/(Cyy+sy2) < gate_d, so the
-// bins that are read cover |dy| <= min(gate_y, sqrt(gate_d (Cyy+sy2))) (widened by 0.2 % + 2 units against
-// rounding), likewise in z: the grid only prunes, every accept/compare in search_row is the definition's.
-struct Window {
-  int iy_lo, iy_hi, iz_lo, iz_hi;
-  __device__ __forceinline__ uint32_t key_y() const { return ((uint32_t)iy_lo << 16) | (uint32_t)iy_hi; }
-  __device__ __forceinline__ uint32_t key_z(int row) const {
-    return ((uint32_t)row << 24) | ((uint32_t)iz_lo << 8) | (uint32_t)min(iz_hi - iz_lo, 255);   // nz < 2^16
-  }
-};
-
-__device__ __forceinline__ Window search_window(const DevGeom& g, float py, float pz, float vy, float vz, int y0, int z0,
-                                                int org_z) {
-  // half widths in units: gate_d*v*rsqrt(gate_d*v) = sqrt(gate_d*v) to 2 ulp, inside the 0.2 % margin.
-  // float -> int conversions saturate; a state so far off that y0 + (...) wraps has no cluster within the gate
-  // (coordinates stay within +-2^24 units of the extents), and the clamps keep every index in range regardless.
-  const float ay = g.gate_d * vy, az = g.gate_d * vz;
-  const float hy = fminf(g.gate_y, ay * rsqrtf(ay) * 1.002f) * g.units + 2.f;
-  const float hz = fminf(g.gate_z, az * rsqrtf(az) * 1.002f) * g.units + 2.f;
-  const float cy = py * g.units, cz = pz * g.units;
-  const int oy = y0 - g.org_y, oz = z0 - org_z;
-  Window w;
-  w.iy_lo = min(max((__float2int_rd(cy - hy) + oy) >> g.shift_y, 0), g.ny - 1);
-  w.iy_hi = min(max((__float2int_ru(cy + hy) + oy) >> g.shift_y, 0), g.ny - 1);
-  w.iz_lo = min(max((__float2int_rd(cz - hz) + oz) >> g.shift_z, 0), g.nz - 1);
-  w.iz_hi = min(max((__float2int_ru(cz + hz) + oz) >> g.shift_z, 0), g.nz - 1);   // bins >= 2 gate_z: iz_hi <= iz_lo + 1
-  return w;
-}
-
-// Bin starts of a window: (a0,b0) = sorted range of the low z-bin, (a1,b1) of the high one (empty if the same).
-struct BinRanges {
-  uint32_t a0, b0, a1, b1;
-};
-
-__device__ __forceinline__ BinRanges load_ranges(const DevGeom& g, const uint32_t* __restrict__ bs, const Window& w) {
-  BinRanges q;
-  q.a0 = bs[w.iz_lo * g.ny + w.iy_lo];
-  q.b0 = bs[w.iz_lo * g.ny + w.iy_hi + 1];
-  q.a1 = q.b1 = 0;
-  if (w.iz_hi != w.iz_lo) {
-    q.a1 = bs[w.iz_hi * g.ny + w.iy_lo];
-    q.b1 = bs[w.iz_hi * g.ny + w.iy_hi + 1];
-  }
-  return q;
-}
-
-__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
-
-// Predicated loads that write straight into their destination registers (the old value stays when `pred` is
-// false).  Written as PTX because `if (c) v = *p;` compiles to load-into-temporary + select, and the select waits
-// for the load right there -- which would turn every gather that is issued one step ahead into a blocking one.
-// (y, z, up link) of a cluster record as three scalar loads: a predicated 128-bit load needs an aligned register
-// quad, which ptxas then copies out of right behind the load (and so waits for it); scalars land in place.
-struct Rec3 {
-  int y, z, up;
-};
-__device__ __forceinline__ void ld_rec_if(Rec3& v, const int4* p, bool pred) {
-  asm volatile("{ .reg .pred q; setp.ne.s32 q, %3, 0; @q ld.global.nc.s32 %0, [%4]; @q ld.global.nc.s32 %1, [%4+4];"
-               " @q ld.global.nc.s32 %2, [%4+8]; }"
-               : "+r"(v.y), "+r"(v.z), "+r"(v.up) : "r"((int)pred), "l"(p));
-}
-__device__ __forceinline__ void ld_u32_if(uint32_t& v, const uint32_t* p, bool pred) {
-  asm volatile("{ .reg .pred q; setp.ne.s32 q, %1, 0; @q ld.global.nc.u32 %0, [%2]; }" : "+r"(v) : "r"((int)pred), "l"(p));
-}
-// .cg: the hit table is written by this kernel, so it is read from L2, never from a stale L1 line
-__device__ __forceinline__ void ld_cg_s32_if(int& v, const int32_t* p, bool pred) {
-  asm volatile("{ .reg .pred q; setp.ne.s32 q, %1, 0; @q ld.global.cg.s32 %0, [%2]; }" : "+r"(v) : "r"((int)pred), "l"(p) : "memory");
-}
-
-// Bin starts of window w of the row whose bin_start segment is bs, loaded into q iff pred.
-__device__ __forceinline__ void load_ranges_if(const DevGeom& g, const uint32_t* __restrict__ bs, const Window& w,
-                                               BinRanges& q, bool pred) {
-  const bool two = pred && w.iz_hi != w.iz_lo;
-  if (pred && !two) q.a1 = q.b1 = 0;
-  ld_u32_if(q.a0, bs + w.iz_lo * g.ny + w.iy_lo, pred);
-  ld_u32_if(q.b0, bs + w.iz_lo * g.ny + w.iy_hi + 1, pred);
-  ld_u32_if(q.a1, bs + w.iz_hi * g.ny + w.iy_lo, two);
-  ld_u32_if(q.b1, bs + w.iz_hi * g.ny + w.iy_hi + 1, two);
-}
-
-// P17/P21: among the candidates minimise (d, id), d = dy^2/(Cyy + sy2) + dz^2/(Czz + sz2), restricted to
-// |dy| <= gate_y and |dz| <= gate_z (cm).  Accumulates into (f, bestd); the caller applies the gate d < gate_d.
-__device__ __forceinline__ void search_ranges(const DevGeom& g, const BinRanges& q, float py, float pz, float wy,
-                                              float wz, int y0, int z0, const int4* __restrict__ srt, Found& f,
-                                              float& bestd) {
-  const uint32_t n0 = q.b0 - q.a0, total = n0 + (q.b1 - q.a1);
-  if (total) {
-    int4 nx = srt[n0 ? q.a0 : q.a1];
-    for (uint32_t t = 0; t < total; ++t) {   // one flat loop over both z-bins
-      const int4 c = nx;
-      const uint32_t tn = min(t + 1, total - 1);   // next one in flight (the last iteration re-reads itself)
-      nx = srt[tn < n0 ? q.a0 + tn : q.a1 + (tn - n0)];
-      const float cy = (float)(c.x - y0) * g.inv_units, cz = (float)(c.y - z0) * g.inv_units;
-      const float dy = cy - py, dz = cz - pz;
-      if (fabsf(dy) > g.gate_y || fabsf(dz) > g.gate_z) continue;
-      const float d = dy * dy * wy + dz * dz * wz;
-      if (d < bestd || (d == bestd && c.z < f.id)) {
-        bestd = d;
-        f.id = c.z;
-        f.y = cy;
-        f.z = cz;
-      }
-    }
-  }
-}
 
 enum : int { PH_IDLE = 0, PH_INIT, PH_A, PH_B, PH_CS, PH_CD, PH_FIN, PH_DONE };
 enum : int { M_NONE = 0, M_LINK, M_TABLE, M_SEARCH };

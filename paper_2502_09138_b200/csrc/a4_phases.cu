@@ -1,0 +1,563 @@
+// a4_phases.cu -- stage a4 as four phase-specialised persistent kernels (same arithmetic, same results as
+// a4_follow.cu).  In the single uniform kernel every warp pays for the row search in every
+// step although only ~7 of its 32 lanes search; here the tracklets of one phase run together:
+//   A  P19 state + fit up the seed chain          (no search: transport + update, next chain record a step ahead)
+//   B  extend up with the gated search            (every live lane searches)
+//   C  covariance reset + refit down to the seed's first row over the recorded hits (no search)
+//   D  extend down with the search, final transport, tracklet record, table padding and ownership votes
+// Between two phases a tracklet's filter state is parked in HBM (176 bytes) and its seed rank is pushed into the next
+// phase's queue; a kernel boundary separates producers and consumers, so the queues need no flags or fences.
+#include "tpc_internal.cuh"
+#include "a4_search.cuh"
+
+namespace {
+
+constexpr int AP_THREADS = 128;
+enum : int { Q_B = 0, Q_C = 1, Q_D = 2 };
+
+struct Env {   // everything a warp needs that does not change during a kernel
+  DevGeom g;
+  DevCtl* ctl;
+  const int4* rec;
+  const int4* srt;
+  const uint32_t* sec_key;
+  const uint32_t* bin_start;
+  const int32_t* seed_start;
+  const int32_t* seed_sr;
+  float4* tl_rec;
+  int32_t* tl_hits;
+  int4* tl_state;
+  uint32_t* q_items;
+  uint32_t* tl_span;
+  const double* s_row_x;   // shared-memory copies
+  const float* s_row_dx;
+  uint32_t n_seeds, s_cap;
+  int lane, lanes_used;
+};
+
+struct Trk {   // per-tracklet constants, recomputed from the seed rank when a lane picks the tracklet up
+  int i, h0, y0, z0, up0, sec_base, r0, org_z;
+  int32_t* tab;   // its row -> hit table = its final hit list
+};
+
+__device__ __forceinline__ Trk trk_of(const Env& e, int i) {
+  Trk t;
+  t.i = i;
+  t.h0 = e.seed_start[i];
+  const int sr = e.seed_sr[i];
+  const int sec = sr / e.g.n_rows;
+  t.sec_base = sec * e.g.n_rows;
+  t.r0 = sr - t.sec_base;
+  t.org_z = zmin_from_key(e.sec_key[sec]);
+  t.tab = e.tl_hits + (size_t)i * e.g.n_rows;
+  const int4 c0 = e.rec[t.h0];
+  t.y0 = c0.x;
+  t.z0 = c0.y;
+  t.up0 = c0.z;
+  return t;
+}
+
+struct Book {   // bookkeeping that travels with the filter state
+  int row, nh, miss, lowest, rmin, rmax;
+  bool fail_dn;
+  float chi2;
+};
+
+__device__ __forceinline__ void state_save(const Env& e, const Trk& t, const State& p, const Cov& C, const Book& b) {
+  const int i = t.i;
+  double2* d = (double2*)(e.tl_state + (size_t)i * A4_STATE_V4);
+  d[0] = make_double2(C.c00, C.c10); d[1] = make_double2(C.c11, C.c20); d[2] = make_double2(C.c21, C.c22);
+  d[3] = make_double2(C.c30, C.c31); d[4] = make_double2(C.c32, C.c33); d[5] = make_double2(C.c40, C.c41);
+  d[6] = make_double2(C.c42, C.c43); d[7] = make_double2(C.c44, 0.0);
+  float4* f = (float4*)(d + 8);
+  f[0] = make_float4((float)p.y, (float)p.z, (float)p.s, (float)p.t);
+  f[1] = make_float4((float)p.q, b.chi2, __int_as_float(b.row), __int_as_float(b.nh));
+  f[2] = make_float4(__int_as_float(b.miss), __int_as_float(b.lowest),
+                     __int_as_float(b.rmin | (b.rmax << 8) | (b.fail_dn ? 1 << 16 : 0)), 0.f);
+  ((int4*)f)[3] = make_int4(t.y0, t.z0, t.sec_base + t.r0, t.org_z);   // so that the next phase needs one gather level
+}
+
+__device__ __forceinline__ void state_load(const Env& e, int i, Trk& t, State& p, Cov& C, Book& b) {
+  const double2* d = (const double2*)(e.tl_state + (size_t)i * A4_STATE_V4);
+  const double2 d0 = d[0], d1 = d[1], d2 = d[2], d3 = d[3], d4 = d[4], d5 = d[5], d6 = d[6], d7 = d[7];
+  const float4* f = (const float4*)(d + 8);
+  const float4 f0 = f[0], f1 = f[1], f2 = f[2];
+  const int4 o = ((const int4*)f)[3];
+  t.i = i;
+  t.y0 = o.x;
+  t.z0 = o.y;
+  t.sec_base = (o.z / e.g.n_rows) * e.g.n_rows;
+  t.r0 = o.z - t.sec_base;
+  t.org_z = o.w;
+  t.tab = e.tl_hits + (size_t)i * e.g.n_rows;
+  t.h0 = t.up0 = -1;
+  C.c00 = d0.x; C.c10 = d0.y; C.c11 = d1.x; C.c20 = d1.y; C.c21 = d2.x; C.c22 = d2.y; C.c30 = d3.x; C.c31 = d3.y;
+  C.c32 = d4.x; C.c33 = d4.y; C.c40 = d5.x; C.c41 = d5.y; C.c42 = d6.x; C.c43 = d6.y; C.c44 = d7.x;
+  p.y = f0.x; p.z = f0.y; p.s = f0.z; p.t = f0.w; p.q = f1.x;
+  b.chi2 = f1.y;
+  b.row = __float_as_int(f1.z);
+  b.nh = __float_as_int(f1.w);
+  b.miss = __float_as_int(f2.x);
+  b.lowest = __float_as_int(f2.y);
+  const int pk = __float_as_int(f2.z);
+  b.rmin = pk & 0xff;
+  b.rmax = (pk >> 8) & 0xff;
+  b.fail_dn = (pk >> 16) & 1;
+}
+
+// Producer side (lanes with pred, after state_save): one atomic per warp.
+__device__ __forceinline__ void queue_push(const Env& e, int q, int i, bool pred) {
+  const unsigned m = __ballot_sync(0xffffffffu, pred);
+  if (!m) return;
+  const int leader = __ffs(m) - 1;
+  uint32_t base = 0;
+  if (e.lane == leader) base = atomicAdd(&e.ctl->q_alloc[q].v, (uint32_t)__popc(m));
+  base = __shfl_sync(0xffffffffu, base, leader);
+  if (pred) e.q_items[(size_t)q * e.s_cap + base + __popc(m & ((1u << e.lane) - 1u))] = (uint32_t)i;
+}
+
+// Consumer side: the queue is complete (its producers ran in earlier launches); a claim is one fetch-add.
+__device__ __forceinline__ int queue_pop(const Env& e, int q, uint32_t total, unsigned want, bool mine, bool* dry) {
+  uint32_t base = 0;
+  if (e.lane == 0) base = atomicAdd(&e.ctl->q_head[q].v, (uint32_t)__popc(want));
+  base = __shfl_sync(0xffffffffu, base, 0);
+  *dry = base + (uint32_t)__popc(want) >= total;
+  const uint32_t k = base + (uint32_t)__popc(want & ((1u << e.lane) - 1u));
+  return (mine && k < total) ? (int)e.q_items[(size_t)q * e.s_cap + k] : -1;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Phase A: P19 initial state + fit up the seed chain, no gate.  Items = seed ranks from ctl->next_seed.
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void phase_a(const Env& e) {
+  const unsigned FULL = 0xffffffffu;
+  const DevGeom& g = e.g;
+  bool live = false, first = false, exhausted = false;
+  Trk t = {};
+  Book b = {};
+  State p;
+  Cov C;
+  p.y = p.z = p.s = p.t = p.q = 0;
+  cov_reset(g, C);
+  int h = -1;
+  Rec3 rcn = {0, 0, -1};
+  while (true) {
+    const bool want = !live && e.lane < e.lanes_used && !exhausted;
+    const unsigned idle = __ballot_sync(FULL, want);
+    if (idle) {
+      uint32_t base = 0;
+      if (e.lane == 0) base = atomicAdd(&e.ctl->next_seed, (uint32_t)__popc(idle));
+      base = __shfl_sync(FULL, base, 0);
+      if (base + (uint32_t)__popc(idle) >= e.n_seeds) exhausted = true;
+      const uint32_t k = base + (uint32_t)__popc(idle & ((1u << e.lane) - 1u));
+      if (want && k < e.n_seeds) {
+        t = trk_of(e, (int)k);
+        h = t.h0;
+        const int4 c1 = e.rec[t.up0];
+        rcn.y = t.y0; rcn.z = t.z0; rcn.up = t.up0;
+        const float dxr = e.s_row_dx[t.r0];
+        const float dy = (float)(c1.x - t.y0) * g.inv_units, dz = (float)(c1.y - t.z0) * g.inv_units;
+        const float ichord = rsqrtf(fmaf(dxr, dxr, dy * dy));
+        p.y = 0; p.z = 0; p.s = dy * ichord; p.t = dz * ichord; p.q = 0;
+        b.row = b.rmin = b.rmax = b.lowest = t.r0;
+        b.nh = 0; b.miss = 0; b.chi2 = 0.f; b.fail_dn = false;
+        first = true;
+        live = true;
+      }
+    }
+    if (!__any_sync(FULL, live)) return;
+
+    if (live && first) cov_reset(g, C);   // P19
+    const bool tr = live && !first;
+    const int trow = b.row + (tr ? 1 : 0);
+    const float dx = e.s_row_dx[b.row];
+    const int hid = h;
+    const Rec3 rc = rcn;
+    ld_rec_if(rcn, e.rec + rc.up, live && rc.up >= 0);   // the next chain hit, one step ahead
+    bool ok = live;
+    if (tr) ok = transport<true>(g, dx, p, C);
+    if (ok) {
+      b.row = trow;
+      update(g, p, C, (float)(rc.y - t.y0) * g.inv_units, (float)(rc.z - t.z0) * g.inv_units);
+      t.tab[trow] = hid;
+      b.rmax = trow;
+      ++b.nh;
+      h = rc.up;
+      first = false;
+    }
+    // the chain ended, or the transport failed (P18; then phase B is skipped)
+    const bool leave = live && (!ok || h < 0);
+    if (leave) state_save(e, t, p, C, b);
+    const bool to_b = leave && ok && b.row + 1 < g.n_rows;
+    queue_push(e, Q_B, t.i, to_b);
+    queue_push(e, Q_C, t.i, leave && !to_b);
+    if (leave) live = false;
+  }
+}
+
+// Search step shared by phases B and D (P17, P21): exact window after the transport, bin ranges from the prediction
+// when it matches, candidates.
+__device__ __forceinline__ Found search_step(const Env& e, const Trk& t, const State& p, const Cov& C, int row,
+                                             uint32_t pk_y, uint32_t pk_z, const BinRanges& pq) {
+  const DevGeom& g = e.g;
+  const float py = (float)p.y, pz = (float)p.z;
+  const float vy = (float)C.c00 + g.sy2, vz = (float)C.c11 + g.sz2;
+  const Window w = search_window(g, py, pz, vy, vz, t.y0, t.z0, t.org_z);
+  const uint32_t* bs = e.bin_start + (size_t)(t.sec_base + row) * g.nb_stride;
+  Found f;
+  f.id = -1;
+  f.y = f.z = 0.f;
+  float bestd = __int_as_float(0x7f800000);
+  const float wy = 1.f / vy, wz = 1.f / vz;
+  if (w.iz_hi <= w.iz_lo + 1) {   // always so on the coarse grid
+    BinRanges q = pq;
+    load_ranges_if(g, bs, w, q, w.key_y() != pk_y || w.key_z(row) != pk_z);
+    search_ranges(g, q, py, pz, wy, wz, t.y0, t.z0, e.srt, f, bestd);
+  } else {   // refined grid and a wide gate: two z-bin rows at a time
+    for (int iz = w.iz_lo; iz <= w.iz_hi; iz += 2) {
+      Window w2 = w;
+      w2.iz_lo = iz;
+      w2.iz_hi = min(iz + 1, w.iz_hi);
+      BinRanges q2 = {0, 0, 0, 0};
+      load_ranges_if(g, bs, w2, q2, true);
+      search_ranges(g, q2, py, pz, wy, wz, t.y0, t.z0, e.srt, f, bestd);
+    }
+  }
+  if (!(bestd < g.gate_d)) f.id = -1;   // P21
+  return f;
+}
+
+// Bin ranges of the search window of row `nrow` at the position extrapolated from the state at row `row`
+// (requested before the current step's transport so that the step hides the latency).
+__device__ __forceinline__ void predict_ranges(const Env& e, const Trk& t, const State& p, const Cov& C, int row,
+                                               int nrow, bool pred, uint32_t& nk_y, uint32_t& nk_z, BinRanges& nq) {
+  const DevGeom& g = e.g;
+  const int srow = pred ? nrow : row;
+  const float ndx = (float)(e.s_row_x[srow] - e.s_row_x[row]);
+  const float ps = (float)p.s;
+  const float ic = rsqrtf(fmaxf(1.f - ps * ps, 0.05f));
+  const float py = (float)p.y + ndx * ps * ic, pz = (float)p.z + ndx * (float)p.t * ic;
+  const Window w = search_window(g, py, pz, (float)C.c00 + g.sy2, (float)C.c11 + g.sz2, t.y0, t.z0, t.org_z);
+  load_ranges_if(g, e.bin_start + (size_t)(t.sec_base + srow) * g.nb_stride, w, nq, pred);
+  if (pred) {
+    nk_y = w.key_y();
+    nk_z = w.key_z(nrow);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Phase B: extend up with the gated nearest-hit search (P17, P20, P21).  Every live lane searches in every step.
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void phase_b(const Env& e) {
+  const unsigned FULL = 0xffffffffu;
+  const DevGeom& g = e.g;
+  const uint32_t total = e.ctl->q_alloc[Q_B].v;
+  bool live = false, dry = false;
+  Trk t = {};
+  Book b = {};
+  State p;
+  Cov C;
+  p.y = p.z = p.s = p.t = p.q = 0;
+  cov_reset(g, C);
+  uint32_t pk_y = 0xFFFFFFFFu, pk_z = 0xFFFFFFFFu;
+  BinRanges pq = {0, 0, 0, 0};
+  while (true) {
+    const bool want = !live && e.lane < e.lanes_used && !dry;
+    const unsigned idle = __ballot_sync(FULL, want);
+    if (idle) {
+      const int i = queue_pop(e, Q_B, total, idle, want, &dry);
+      if (i >= 0) {
+        state_load(e, i, t, p, C, b);
+        pk_y = pk_z = 0xFFFFFFFFu;
+        live = true;
+      }
+    }
+    if (!__any_sync(FULL, live)) return;
+
+    const int trow = b.row + 1;   // a live lane always has a row above and fewer than max_miss misses
+    const float dx = e.s_row_dx[b.row];
+    if (live && (pk_z >> 24) == (uint32_t)trow) {   // this step's first candidates into L1 during the transport
+      if (pq.b0 > pq.a0) prefetch_l1(e.srt + pq.a0);
+      if (pq.b1 > pq.a1) prefetch_l1(e.srt + pq.a1);
+    }
+    uint32_t nk_y = pk_y, nk_z = pk_z;
+    BinRanges nq = pq;
+    predict_ranges(e, t, p, C, b.row, trow + 1, live && trow + 1 < g.n_rows, nk_y, nk_z, nq);
+    bool ok = live;
+    if (ok) ok = transport<true>(g, dx, p, C);
+    if (ok) {
+      b.row = trow;
+      const Found f = search_step(e, t, p, C, trow, pk_y, pk_z, pq);
+      t.tab[trow] = f.id;
+      b.rmax = trow;
+      if (f.id >= 0) {
+        update(g, p, C, f.y, f.z);
+        ++b.nh;
+        b.miss = 0;
+      } else {
+        ++b.miss;
+      }
+    }
+    pk_y = nk_y;
+    pk_z = nk_z;
+    pq = nq;
+    const bool leave = live && (!ok || !(b.row + 1 < g.n_rows && b.miss < g.max_miss));   // P18, P20
+    if (leave) state_save(e, t, p, C, b);
+    queue_push(e, Q_C, t.i, leave);
+    if (leave) live = false;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Phase C: covariance reset (P22), then refit down over the recorded hits to the seed's first row.  The first step
+// of a tracklet (reset + update with the top row's hit) has no transport.  Table entries of the next two rows and
+// the record of the next hit are requested one step ahead.
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void phase_c(const Env& e) {
+  const unsigned FULL = 0xffffffffu;
+  const DevGeom& g = e.g;
+  const uint32_t total = e.ctl->q_alloc[Q_C].v;
+  bool live = false, first = false, dry = false;
+  Trk t = {};
+  Book b = {};
+  State p;
+  Cov C;
+  p.y = p.z = p.s = p.t = p.q = 0;
+  cov_reset(g, C);
+  int t1_row = -1, t1_val = -1, t2_row = -1, t2_val = -1;   // table entries of this step's row and the one below
+  int rcn_id = -1;
+  Rec3 rcn = {0, 0, -1};
+  while (true) {
+    const bool want = !live && e.lane < e.lanes_used && !dry;
+    const unsigned idle = __ballot_sync(FULL, want);
+    if (idle) {
+      const int i = queue_pop(e, Q_C, total, idle, want, &dry);
+      if (i >= 0) {
+        state_load(e, i, t, p, C, b);
+        t1_row = t2_row = -1;
+        rcn_id = -1;
+        first = true;
+        live = true;
+      }
+    }
+    if (!__any_sync(FULL, live)) return;
+
+    if (live && first) {   // P22
+      cov_reset(g, C);
+      b.chi2 = 0.f;
+      b.miss = 0;
+      b.lowest = t.r0;
+    }
+    const bool tr = live && !first;
+    const int trow = b.row - (tr ? 1 : 0);
+    const float dx = -e.s_row_dx[max(b.row - 1, 0)];
+    int hid = -1, nid = -1;
+    if (live) {   // rolling two-deep pipeline over the table on the way down
+      if (t1_row != trow) {
+        t1_val = -1;
+        ld_cg_s32_if(t1_val, t.tab + trow, true);
+      }
+      hid = t1_val;
+      const int n1 = trow - 1, n2 = trow - 2;
+      const bool have1 = t2_row == n1;
+      t1_val = t2_val;
+      t1_row = n1;
+      if (have1) nid = t1_val;   // loaded in an earlier step: safe to consume without waiting
+      ld_cg_s32_if(t1_val, t.tab + n1, !have1 && n1 >= t.r0);
+      if (n1 < t.r0) t1_row = -1;
+      t2_row = n2 >= t.r0 ? n2 : -1;
+      ld_cg_s32_if(t2_val, t.tab + n2, n2 >= t.r0);
+    }
+    Rec3 rc = rcn;
+    if (hid < 0) { rc.y = t.y0; rc.z = t.z0; rc.up = -1; }
+    ld_rec_if(rc, e.rec + hid, hid >= 0 && hid != rcn_id);
+    {
+      const bool fetch = nid >= 0 && nid != rcn_id;
+      if (fetch) rcn_id = nid;
+      ld_rec_if(rcn, e.rec + nid, fetch);
+    }
+    bool ok = live;
+    if (tr) ok = transport<true>(g, dx, p, C);
+    if (ok) {
+      b.row = trow;
+      if (hid >= 0) b.chi2 += update(g, p, C, (float)(rc.y - t.y0) * g.inv_units, (float)(rc.z - t.z0) * g.inv_units);
+      first = false;
+    } else if (live) {
+      b.fail_dn = true;   // P18: the state stays at the row where it stopped
+    }
+    const bool leave = live && (!ok || b.row <= t.r0);   // below the seed's first row phase D searches
+    if (leave) state_save(e, t, p, C, b);
+    queue_push(e, Q_D, t.i, leave);
+    if (leave) live = false;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Phase D: extend down below the seed's first row with the search (P20), then the final transport to the
+// lowest-row hit (P23) and the tracklet record.  The padding of the hit tables and the ownership votes (P24, P26)
+// are a flat kernel of their own (a4_votes_kernel): a warp per tracklet, 32 rows per instruction.
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void phase_d(const Env& e) {
+  const unsigned FULL = 0xffffffffu;
+  const DevGeom& g = e.g;
+  const int nr = g.n_rows;
+  const uint32_t total = e.ctl->q_alloc[Q_D].v;
+  bool live = false, dry = false;
+  Trk t = {};
+  Book b = {};
+  State p;
+  Cov C;
+  p.y = p.z = p.s = p.t = p.q = 0;
+  cov_reset(g, C);
+  uint32_t pk_y = 0xFFFFFFFFu, pk_z = 0xFFFFFFFFu;
+  BinRanges pq = {0, 0, 0, 0};
+  while (true) {
+    const bool want = !live && e.lane < e.lanes_used && !dry;
+    const unsigned idle = __ballot_sync(FULL, want);
+    if (idle) {
+      const int i = queue_pop(e, Q_D, total, idle, want, &dry);
+      if (i >= 0) {
+        state_load(e, i, t, p, C, b);
+        pk_y = pk_z = 0xFFFFFFFFu;
+        live = true;
+      }
+    }
+    if (!__any_sync(FULL, live)) return;
+
+    // search step down, or the final transport once the extension is over
+    const bool srch = live && !b.fail_dn && b.row > 0 && b.miss < g.max_miss;
+    const bool fin = live && !srch;
+    bool tr = srch;
+    int trow = b.row - (srch ? 1 : 0);
+    float dx = -e.s_row_dx[max(b.row - 1, 0)];
+    if (fin && !b.fail_dn && b.lowest != b.row) {   // P23
+      tr = true;
+      trow = b.lowest;
+      dx = (float)(e.s_row_x[b.lowest] - e.s_row_x[b.row]);
+    }
+    if (srch && (pk_z >> 24) == (uint32_t)trow) {
+      if (pq.b0 > pq.a0) prefetch_l1(e.srt + pq.a0);
+      if (pq.b1 > pq.a1) prefetch_l1(e.srt + pq.a1);
+    }
+    uint32_t nk_y = pk_y, nk_z = pk_z;
+    BinRanges nq = pq;
+    predict_ranges(e, t, p, C, b.row, trow - 1, srch && trow >= 1, nk_y, nk_z, nq);
+    bool ok = live;
+    if (tr) ok = transport<true>(g, dx, p, C);
+    if (ok) b.row = trow;
+    if (srch) {
+      if (ok) {
+        const Found f = search_step(e, t, p, C, trow, pk_y, pk_z, pq);
+        t.tab[trow] = f.id;
+        b.rmin = min(b.rmin, trow);
+        if (f.id >= 0) {
+          b.chi2 += update(g, p, C, f.y, f.z);
+          ++b.nh;
+          b.miss = 0;
+          b.lowest = trow;
+        } else {
+          ++b.miss;
+        }
+      } else {
+        b.fail_dn = true;
+      }
+    }
+    pk_y = nk_y;
+    pk_z = nk_z;
+    pq = nq;
+
+    // ---- tracklets that ended: record, padding of the hit table and ownership votes ----
+    const unsigned done = __ballot_sync(FULL, fin);
+    if (done) {
+      if (fin) {
+        float4* o = e.tl_rec + (size_t)t.i * TL_REC_V4;
+        o[0] = make_float4((float)e.s_row_x[b.row], (float)((double)p.y + (double)t.y0 * g.inv_units_d),
+                           (float)((double)p.z + (double)t.z0 * g.inv_units_d), (float)p.s);
+        o[1] = make_float4((float)p.t, (float)p.q, b.chi2, __int_as_float(b.nh));
+        o[2] = make_float4((float)C.c00, (float)C.c10, (float)C.c11, (float)C.c20);
+        o[3] = make_float4((float)C.c21, (float)C.c22, (float)C.c30, (float)C.c31);
+        o[4] = make_float4((float)C.c32, (float)C.c33, (float)C.c40, (float)C.c41);
+        o[5] = make_float4((float)C.c42, (float)C.c43, (float)C.c44, __int_as_float(t.sec_base + t.r0));
+        e.tl_span[t.i] = (uint32_t)b.rmin | ((uint32_t)b.rmax << 8);
+      }
+      if (fin) live = false;
+    }
+  }
+}
+
+// P24, P26: owner(h) = surviving tracklet with the most hits, ties -> smallest rank; rows a tracklet never visited
+// get -1.  One warp per tracklet, grid-stride.
+__global__ void __launch_bounds__(256)
+a4_votes_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, const float4* __restrict__ tl_rec,
+                const uint32_t* __restrict__ tl_span, int32_t* __restrict__ tl_hits, uint32_t* __restrict__ owner) {
+  const int nr = g.n_rows, lane = threadIdx.x & 31;
+  const uint32_t n_seeds = ctl->n_seeds;
+  const uint32_t warps = gridDim.x * (blockDim.x >> 5);
+  for (uint32_t i = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); i < n_seeds; i += warps) {
+    const int nh = __float_as_int(tl_rec[(size_t)i * TL_REC_V4 + 1].w);
+    const uint32_t span = tl_span[i];
+    const int smin = span & 0xff, smax = (span >> 8) & 0xff;
+    const uint32_t word = nh >= g.n_min_tracklet ? (((uint32_t)nh << 24) | (0xFFFFFFu - i)) : 0u;
+    int32_t* out = tl_hits + (size_t)i * nr;
+    for (int r = lane; r < nr; r += 32) {
+      if (r >= smin && r <= smax) {
+        const int v = out[r];
+        if (word && v >= 0) atomicMax(&owner[v], word);
+      } else {
+        out[r] = -1;
+      }
+    }
+  }
+}
+
+template <int PH>
+__global__ void __launch_bounds__(AP_THREADS, 4)
+a4_phase_kernel(const DevGeom g, uint32_t s_cap, DevCtl* __restrict__ ctl, const int4* __restrict__ rec,
+                const int4* __restrict__ srt, const uint32_t* __restrict__ sec_key,
+                const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ seed_start,
+                const int32_t* __restrict__ seed_sr, float4* __restrict__ tl_rec, int32_t* __restrict__ tl_hits,
+                int4* __restrict__ tl_state, uint32_t* __restrict__ q_items, uint32_t* __restrict__ tl_span) {
+  extern __shared__ double smem_ap[];
+  const int nr = g.n_rows;
+  const uint32_t n_seeds = ctl->n_seeds;
+  if (n_seeds == 0) return;
+  double* const s_row_x = smem_ap;
+  float* const s_row_dx = (float*)(s_row_x + nr);
+  for (int r = threadIdx.x; r < nr; r += blockDim.x) {
+    s_row_x[r] = g.row_x[r];
+    s_row_dx[r] = g.row_dx[r];
+  }
+  __syncthreads();
+  Env e;
+  e.g = g;
+  e.ctl = ctl; e.rec = rec; e.srt = srt; e.sec_key = sec_key; e.bin_start = bin_start;
+  e.seed_start = seed_start; e.seed_sr = seed_sr; e.tl_rec = tl_rec; e.tl_hits = tl_hits; e.tl_state = tl_state;
+  e.q_items = q_items; e.tl_span = tl_span; e.s_row_x = s_row_x; e.s_row_dx = s_row_dx;
+  e.n_seeds = n_seeds; e.s_cap = s_cap;
+  e.lane = threadIdx.x & 31;
+  // few seeds (one small event): spread them over all warps instead of filling the first warps' 32 lanes
+  const uint32_t n_warps = gridDim.x * (blockDim.x >> 5);
+  e.lanes_used = (int)min(32u, (n_seeds + n_warps - 1) / n_warps);
+  if (PH == 0) phase_a(e);
+  if (PH == 1) phase_b(e);
+  if (PH == 2) phase_c(e);
+  if (PH == 3) phase_d(e);
+}
+
+}  // namespace
+
+cudaError_t launch_a4_phases(const tpc_tracker* t, int64_t n, cudaStream_t st) {
+  if (n == 0 || t->s_cap == 0) return cudaSuccess;
+  const size_t smem = (size_t)t->g.n_rows * (8 + 4);
+#define AP_LAUNCH(PH)                                                                                         \
+  a4_phase_kernel<PH><<<t->a4_blocks, AP_THREADS, smem, st>>>(                                                \
+      t->g, (uint32_t)t->s_cap, t->s.ctl, t->s.rec, t->s.srt, t->s.sec_key, t->s.bin_start, t->s.seed_start, \
+      t->s.seed_sr, t->s.tl_rec, t->s.tl_hits, t->s.tl_state, t->s.q_items, t->s.tl_span)
+  AP_LAUNCH(0);
+  AP_LAUNCH(1);
+  AP_LAUNCH(2);
+  AP_LAUNCH(3);
+#undef AP_LAUNCH
+  a4_votes_kernel<<<148 * 8, 256, 0, st>>>(t->g, t->s.ctl, t->s.tl_rec, t->s.tl_span, t->s.tl_hits, t->s.owner);
+  return cudaGetLastError();
+}

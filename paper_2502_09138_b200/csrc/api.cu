@@ -4,6 +4,7 @@
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
+#include <stdlib.h>
 
 #include <new>
 
@@ -56,6 +57,9 @@ size_t layout(tpc_tracker* t, char* base, int64_t n, int64_t R) {
   s.rec = (int4*)take((size_t)n * 16);
   s.owner = (uint32_t*)take((size_t)n * 4);
   s.hit_row = (uint8_t*)take((size_t)n + 64);
+  s.q_items = (uint32_t*)take((size_t)s_cap * 3 * 4);
+  s.tl_state = (int4*)take((size_t)s_cap * A4_STATE_V4 * 16);
+  s.tl_span = (uint32_t*)take((size_t)s_cap * 4);
   s.seed_start = (int32_t*)take((size_t)s_cap * 4);
   s.seed_sr = (int32_t*)take((size_t)s_cap * 4);
   s.tl_rec = (float4*)take((size_t)s_cap * TL_REC_V4 * 16);
@@ -315,7 +319,13 @@ int tpc_track(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* strea
   if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[2], st));
   TPC_CUDA(t, launch_a3_seeds(t, cl->y, cl->z, cl->row_offsets, n, st));
   if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[3], st));
-  TPC_CUDA(t, launch_a4_follow(t, n, st));
+  // a4 variant: large calls run the follower as four phase-specialised kernels + a vote kernel (20 % fewer
+  // instructions per tracklet, but five launches and a queue tail each: measured slower below ~10 events of
+  // configs[1]); small calls run the single uniform kernel.  TPC_A4_MODE=uniform|phased overrides (tests).
+  const char* mode = getenv("TPC_A4_MODE");
+  t->a4_phased = mode ? (strcmp(mode, "phased") == 0) : (n >= A4_PHASED_MIN_CLUSTERS);
+  if (t->a4_phased) TPC_CUDA(t, launch_a4_phases(t, n, st));
+  else TPC_CUDA(t, launch_a4_follow(t, n, st));
   if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[4], st));
   TPC_CUDA(t, launch_a5_select(t, out, st));
   if (t->timing) {
@@ -394,7 +404,7 @@ int tpc_track_host(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* 
 
 int64_t tpc_scratch_bytes(const tpc_tracker_t* t) { return t ? (int64_t)(t->arena_bytes + t->host_arena_bytes) : 0; }
 
-int tpc_launches_per_call(const tpc_tracker_t* t) { return t ? 6 : 0; }
+int tpc_launches_per_call(const tpc_tracker_t* t) { return t ? (t->a4_phased ? 10 : 6) : 0; }
 
 int tpc_set_stage_timing(tpc_tracker_t* t, int enable) {
   if (!t) return TPC_ERR_ARG;

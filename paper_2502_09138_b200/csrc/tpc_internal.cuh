@@ -25,13 +25,19 @@ struct DevGeom {
 };
 
 // Counters living in device memory, zeroed at the start of every call.
+struct CtlLine {         // one hot counter per 128-byte line
+  uint32_t v;
+  uint32_t pad[31];
+};
 struct DevCtl {
   uint32_t n_seeds;      // written by a3
   uint32_t ticket_a3;    // dynamic tile ids for the a3 look-back scan
   uint32_t ticket_a5;
   uint32_t next_seed;    // a4 work queue: next seed rank to hand to a free lane
   uint32_t next_track;   // a6 work queue
-  uint32_t pad[11];
+  uint32_t pad[27];
+  CtlLine q_alloc[3];    // a4 phase queues B, C, D: items pushed by the previous phase(s) ...
+  CtlLine q_head[3];     // ... and items claimed by the consuming phase
 };
 
 struct Scratch {
@@ -44,6 +50,9 @@ struct Scratch {
   int4* rec;                // a3: per cluster id (y, z, cleaned up link, cleaned down link) -- one 16-B gather per a4 step
   uint32_t* owner;          // packed (n_hits << 24 | 0xFFFFFF - rank), 0 = none
   uint8_t* hit_row;         // [n] a5: row of the hit at each position of the output hit list (for a6)
+  uint32_t* q_items;        // [3][s_cap] a4 phase queues: seed ranks
+  int4* tl_state;           // [s_cap][A4_STATE_V4] a4 filter state of a tracklet between two phases
+  uint32_t* tl_span;        // [s_cap] first | last << 8 row a tracklet visited (rows outside hold no hit)
   // a3 -> a4
   int32_t* seed_start;      // [s_cap] start cluster id, ascending
   int32_t* seed_sr;         // [s_cap] sector * n_rows + row of the start cluster
@@ -76,6 +85,7 @@ struct tpc_tracker {
   int64_t y_units, z_units;         // grid extents in fixed-point units
   int64_t s_cap;             // seed capacity of the current layout
   int64_t tiles_a3, tiles_a5;
+  int a4_phased;             // the most recent call ran a4 as phase kernels (api.cu)
   int a4_blocks, a4_warps;   // persistent a4 grid: blocks x warps per block = resident warps of the device (set at create)
   size_t ctl_bytes;          // bytes zeroed per call
   Scratch s;
@@ -85,6 +95,7 @@ struct tpc_tracker {
   cudaError_t last_err; char err_buf[256];
 };
 
+constexpr int64_t A4_PHASED_MIN_CLUSTERS = 6000000;   // calls at least this large run a4 as phase kernels
 constexpr int GRID_MAX_BINS = 48 * 1024;   // bins per row: one row's histogram fits a CTA's shared memory
 constexpr int GRID_MIN_SHIFT = 9;          // finest bins: 512 units = 0.8 cm
 constexpr int A3_TILE = 1024;   // ids per a3 block (256 threads x 4)
@@ -94,6 +105,7 @@ constexpr int A5_TILE = 128;    // tracklets per a5 block
 __host__ __device__ __forceinline__ uint32_t zmin_key(int32_t z) { return ~((uint32_t)z ^ 0x80000000u); }
 __host__ __device__ __forceinline__ int32_t zmin_from_key(uint32_t k) { return k ? (int32_t)(~k ^ 0x80000000u) : 0; }
 
+constexpr int A4_STATE_V4 = 12; // 16-byte words of a parked a4 state: 15 fp64 covariance, 5 state, bookkeeping, origin
 constexpr int TL_REC_V4 = 6;    // float4 words per tracklet record
 
 // launchers (each in its own .cu)
@@ -103,6 +115,7 @@ cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64
 cudaError_t launch_a3_seeds(const tpc_tracker* t, const int32_t* y, const int32_t* z, const uint32_t* ro, int64_t n, cudaStream_t st);
 cudaError_t launch_a4_follow(const tpc_tracker* t, int64_t n, cudaStream_t st);
 cudaError_t setup_a4_attributes(tpc_tracker* t);
+cudaError_t launch_a4_phases(const tpc_tracker* t, int64_t n, cudaStream_t st);
 cudaError_t launch_a5_select(const tpc_tracker* t, const tpc_tracks_out_t* out, cudaStream_t st);
 cudaError_t launch_a6_refit(const tpc_tracker* t, const uint32_t* ro, const tpc_tracks_out_t* tracks,
                             tpc_track_rec_t* refit_out, cudaStream_t st);

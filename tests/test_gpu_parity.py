@@ -327,6 +327,16 @@ def test_refit_rejects_foreign_input(orc):
     trk.close()
 
 
+@pytest.mark.parametrize("mode", ["uniform", "phased"])
+def test_both_a4_variants_on_small_and_stress_events(orc, mode, monkeypatch):
+    """The library picks the a4 variant by call size (phase kernels for large calls); both must give the oracle's
+    result on any input, so both are forced here on events of either size class."""
+    monkeypatch.setenv("TPC_A4_MODE", mode)
+    for ev, lab in ((make_event(0), "cfg0"), (make_event(1, 1001), "cfg1"), (make_event(4), "cfg4"),
+                    (make_event(2, collisions=6), "cfg2/6")):
+        compare(ev, orc, _run_gpu(ev), orc.track(ev), label=f"{lab} a4={mode}")
+
+
 def test_edge_empty_and_tiny(orc):
     import torch
     from paper_2502_09138_b200 import Tracker, Geometry
