@@ -390,7 +390,7 @@ def main():
     ap.add_argument("--batch-events", type=int, default=32)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--e2e-threads", type=int, default=2, help="host threads (handles, streams) of the e2e arm")
+    ap.add_argument("--e2e-threads", type=int, default=3, help="host threads (handles, streams) of the e2e arm")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
