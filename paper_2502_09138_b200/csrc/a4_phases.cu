@@ -105,25 +105,49 @@ __device__ __forceinline__ void state_load(const Env& e, int i, Trk& t, State& p
   b.fail_dn = (pk >> 16) & 1;
 }
 
-// Producer side (lanes with pred, after state_save): one atomic per warp.
-__device__ __forceinline__ void queue_push(const Env& e, int q, int i, bool pred) {
-  const unsigned m = __ballot_sync(0xffffffffu, pred);
-  if (!m) return;
-  const int leader = __ffs(m) - 1;
-  uint32_t base = 0;
-  if (e.lane == leader) base = atomicAdd(&e.ctl->q_alloc[q].v, (uint32_t)__popc(m));
-  base = __shfl_sync(0xffffffffu, base, leader);
-  if (pred) e.q_items[(size_t)q * e.s_cap + base + __popc(m & ((1u << e.lane) - 1u))] = (uint32_t)i;
+// Length bucket of a tracklet entering a phase: the rows it has left to cover.  Longest first (bucket 0), so that
+// the tail of each phase kernel consists of short tracklets.
+__device__ __forceinline__ int len_bucket(int rows_left) {
+  return rows_left >= 100 ? 0 : (rows_left >= 50 ? 1 : (rows_left >= 15 ? 2 : 3));
 }
 
-// Consumer side: the queue is complete (its producers ran in earlier launches); a claim is one fetch-add.
-__device__ __forceinline__ int queue_pop(const Env& e, int q, uint32_t total, unsigned want, bool mine, bool* dry) {
-  uint32_t base = 0;
-  if (e.lane == 0) base = atomicAdd(&e.ctl->q_head[q].v, (uint32_t)__popc(want));
-  base = __shfl_sync(0xffffffffu, base, 0);
-  *dry = base + (uint32_t)__popc(want) >= total;
-  const uint32_t k = base + (uint32_t)__popc(want & ((1u << e.lane) - 1u));
-  return (mine && k < total) ? (int)e.q_items[(size_t)q * e.s_cap + k] : -1;
+// Producer side (lanes with pred, after state_save): one atomic per warp and bucket.
+__device__ __forceinline__ void queue_push(const Env& e, int q, int bucket, int i, bool pred) {
+  if (!__any_sync(0xffffffffu, pred)) return;
+#pragma unroll
+  for (int bk = 0; bk < A4_Q_BUCKETS; ++bk) {
+    const bool mine = pred && bucket == bk;
+    const unsigned m = __ballot_sync(0xffffffffu, mine);
+    if (!m) continue;
+    const int qq = q * A4_Q_BUCKETS + bk;
+    const int leader = __ffs(m) - 1;
+    uint32_t base = 0;
+    if (e.lane == leader) base = atomicAdd(&e.ctl->q_alloc[qq].v, (uint32_t)__popc(m));
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (mine) e.q_items[(size_t)qq * e.s_cap + base + __popc(m & ((1u << e.lane) - 1u))] = (uint32_t)i;
+  }
+}
+
+// Consumer side: the queues are complete (their producers ran in earlier launches); a claim is one fetch-add.
+// `bk` is the bucket the warp currently drains (warp-uniform); `dry` is set once the last bucket ran out.
+__device__ __forceinline__ int queue_pop(const Env& e, int q, unsigned want, bool mine, int* bk, bool* dry) {
+  int i = -1;
+  unsigned w = want;
+  while (w && *bk < A4_Q_BUCKETS) {   // warp-uniform loop
+    const int qq = q * A4_Q_BUCKETS + *bk;
+    const uint32_t total = e.ctl->q_alloc[qq].v;
+    uint32_t base = 0;
+    if (e.lane == 0) base = atomicAdd(&e.ctl->q_head[qq].v, (uint32_t)__popc(w));
+    base = __shfl_sync(0xffffffffu, base, 0);
+    const uint32_t k = base + (uint32_t)__popc(w & ((1u << e.lane) - 1u));
+    const bool got = mine && i < 0 && ((w >> e.lane) & 1u) && k < total;
+    if (got) i = (int)e.q_items[(size_t)qq * e.s_cap + k];
+    const uint32_t claimed = (uint32_t)__popc(w);
+    w &= ~__ballot_sync(0xffffffffu, got);
+    if (base + claimed >= total) ++*bk;   // this bucket is empty now: move on to the next
+  }
+  *dry = *bk >= A4_Q_BUCKETS;
+  return i;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -189,8 +213,8 @@ __device__ __forceinline__ void phase_a(const Env& e) {
     const bool leave = live && (!ok || h < 0);
     if (leave) state_save(e, t, p, C, b);
     const bool to_b = leave && ok && b.row + 1 < g.n_rows;
-    queue_push(e, Q_B, t.i, to_b);
-    queue_push(e, Q_C, t.i, leave && !to_b);
+    queue_push(e, Q_B, len_bucket(g.n_rows - 1 - b.row), t.i, to_b);
+    queue_push(e, Q_C, len_bucket(b.row - t.r0), t.i, leave && !to_b);
     if (leave) live = false;
   }
 }
@@ -251,7 +275,7 @@ __device__ __forceinline__ void predict_ranges(const Env& e, const Trk& t, const
 __device__ __forceinline__ void phase_b(const Env& e) {
   const unsigned FULL = 0xffffffffu;
   const DevGeom& g = e.g;
-  const uint32_t total = e.ctl->q_alloc[Q_B].v;
+  int bk = 0;
   bool live = false, dry = false;
   Trk t = {};
   Book b = {};
@@ -265,7 +289,7 @@ __device__ __forceinline__ void phase_b(const Env& e) {
     const bool want = !live && e.lane < e.lanes_used && !dry;
     const unsigned idle = __ballot_sync(FULL, want);
     if (idle) {
-      const int i = queue_pop(e, Q_B, total, idle, want, &dry);
+      const int i = queue_pop(e, Q_B, idle, want, &bk, &dry);
       if (i >= 0) {
         state_load(e, i, t, p, C, b);
         pk_y = pk_z = 0xFFFFFFFFu;
@@ -303,7 +327,7 @@ __device__ __forceinline__ void phase_b(const Env& e) {
     pq = nq;
     const bool leave = live && (!ok || !(b.row + 1 < g.n_rows && b.miss < g.max_miss));   // P18, P20
     if (leave) state_save(e, t, p, C, b);
-    queue_push(e, Q_C, t.i, leave);
+    queue_push(e, Q_C, len_bucket(b.row - t.r0), t.i, leave);
     if (leave) live = false;
   }
 }
@@ -316,7 +340,7 @@ __device__ __forceinline__ void phase_b(const Env& e) {
 __device__ __forceinline__ void phase_c(const Env& e) {
   const unsigned FULL = 0xffffffffu;
   const DevGeom& g = e.g;
-  const uint32_t total = e.ctl->q_alloc[Q_C].v;
+  int bk = 0;
   bool live = false, first = false, dry = false;
   Trk t = {};
   Book b = {};
@@ -331,7 +355,7 @@ __device__ __forceinline__ void phase_c(const Env& e) {
     const bool want = !live && e.lane < e.lanes_used && !dry;
     const unsigned idle = __ballot_sync(FULL, want);
     if (idle) {
-      const int i = queue_pop(e, Q_C, total, idle, want, &dry);
+      const int i = queue_pop(e, Q_C, idle, want, &bk, &dry);
       if (i >= 0) {
         state_load(e, i, t, p, C, b);
         t1_row = t2_row = -1;
@@ -387,7 +411,7 @@ __device__ __forceinline__ void phase_c(const Env& e) {
     }
     const bool leave = live && (!ok || b.row <= t.r0);   // below the seed's first row phase D searches
     if (leave) state_save(e, t, p, C, b);
-    queue_push(e, Q_D, t.i, leave);
+    queue_push(e, Q_D, len_bucket(b.row), t.i, leave);
     if (leave) live = false;
   }
 }
@@ -401,7 +425,7 @@ __device__ __forceinline__ void phase_d(const Env& e) {
   const unsigned FULL = 0xffffffffu;
   const DevGeom& g = e.g;
   const int nr = g.n_rows;
-  const uint32_t total = e.ctl->q_alloc[Q_D].v;
+  int bk = 0;
   bool live = false, dry = false;
   Trk t = {};
   Book b = {};
@@ -415,7 +439,7 @@ __device__ __forceinline__ void phase_d(const Env& e) {
     const bool want = !live && e.lane < e.lanes_used && !dry;
     const unsigned idle = __ballot_sync(FULL, want);
     if (idle) {
-      const int i = queue_pop(e, Q_D, total, idle, want, &dry);
+      const int i = queue_pop(e, Q_D, idle, want, &bk, &dry);
       if (i >= 0) {
         state_load(e, i, t, p, C, b);
         pk_y = pk_z = 0xFFFFFFFFu;

@@ -57,7 +57,7 @@ size_t layout(tpc_tracker* t, char* base, int64_t n, int64_t R) {
   s.rec = (int4*)take((size_t)n * 16);
   s.owner = (uint32_t*)take((size_t)n * 4);
   s.hit_row = (uint8_t*)take((size_t)n + 64);
-  s.q_items = (uint32_t*)take((size_t)s_cap * 3 * 4);
+  s.q_items = (uint32_t*)take((size_t)s_cap * 3 * A4_Q_BUCKETS * 4);
   s.tl_state = (int4*)take((size_t)s_cap * A4_STATE_V4 * 16);
   s.tl_span = (uint32_t*)take((size_t)s_cap * 4);
   s.seed_start = (int32_t*)take((size_t)s_cap * 4);

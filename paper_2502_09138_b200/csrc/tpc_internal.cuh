@@ -25,6 +25,7 @@ struct DevGeom {
 };
 
 // Counters living in device memory, zeroed at the start of every call.
+constexpr int A4_Q_BUCKETS = 4;   // a4 phase queues are split by expected tracklet length, longest served first
 struct CtlLine {         // one hot counter per 128-byte line
   uint32_t v;
   uint32_t pad[31];
@@ -36,8 +37,8 @@ struct DevCtl {
   uint32_t next_seed;    // a4 work queue: next seed rank to hand to a free lane
   uint32_t next_track;   // a6 work queue
   uint32_t pad[27];
-  CtlLine q_alloc[3];    // a4 phase queues B, C, D: items pushed by the previous phase(s) ...
-  CtlLine q_head[3];     // ... and items claimed by the consuming phase
+  CtlLine q_alloc[3 * A4_Q_BUCKETS];   // a4 phase queues B, C, D x length bucket: items pushed by earlier phases ...
+  CtlLine q_head[3 * A4_Q_BUCKETS];    // ... and items claimed by the consuming phase
 };
 
 struct Scratch {
@@ -50,7 +51,7 @@ struct Scratch {
   int4* rec;                // a3: per cluster id (y, z, cleaned up link, cleaned down link) -- one 16-B gather per a4 step
   uint32_t* owner;          // packed (n_hits << 24 | 0xFFFFFF - rank), 0 = none
   uint8_t* hit_row;         // [n] a5: row of the hit at each position of the output hit list (for a6)
-  uint32_t* q_items;        // [3][s_cap] a4 phase queues: seed ranks
+  uint32_t* q_items;        // [3 * A4_Q_BUCKETS][s_cap] a4 phase queues: seed ranks
   int4* tl_state;           // [s_cap][A4_STATE_V4] a4 filter state of a tracklet between two phases
   uint32_t* tl_span;        // [s_cap] first | last << 8 row a tracklet visited (rows outside hold no hit)
   // a3 -> a4
