@@ -582,6 +582,6 @@ cudaError_t launch_a4_phases(const tpc_tracker* t, int64_t n, cudaStream_t st) {
   AP_LAUNCH(2);
   AP_LAUNCH(3);
 #undef AP_LAUNCH
-  a4_votes_kernel<<<148 * 8, 256, 0, st>>>(t->g, t->s.ctl, t->s.tl_rec, t->s.tl_span, t->s.tl_hits, t->s.owner);
+  a4_votes_kernel<<<148 * 64, 256, 0, st>>>(t->g, t->s.ctl, t->s.tl_rec, t->s.tl_span, t->s.tl_hits, t->s.owner);
   return cudaGetLastError();
 }
