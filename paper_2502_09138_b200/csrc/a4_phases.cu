@@ -107,8 +107,9 @@ __device__ __forceinline__ void state_load(const Env& e, int i, Trk& t, State& p
 
 // Length bucket of a tracklet entering a phase: the rows it has left to cover.  Longest first (bucket 0), so that
 // the tail of each phase kernel consists of short tracklets.
-__device__ __forceinline__ int len_bucket(int rows_left) {
-  return rows_left >= 100 ? 0 : (rows_left >= 50 ? 1 : (rows_left >= 15 ? 2 : 3));
+__device__ __forceinline__ int len_bucket(int rows_left, int n_rows) {
+  const int b = (A4_Q_BUCKETS - 1) - min(max(rows_left, 0), n_rows - 1) * A4_Q_BUCKETS / n_rows;
+  return b < 0 ? 0 : b;
 }
 
 // Producer side (lanes with pred, after state_save): one atomic per warp and bucket.
@@ -213,8 +214,8 @@ __device__ __forceinline__ void phase_a(const Env& e) {
     const bool leave = live && (!ok || h < 0);
     if (leave) state_save(e, t, p, C, b);
     const bool to_b = leave && ok && b.row + 1 < g.n_rows;
-    queue_push(e, Q_B, len_bucket(g.n_rows - 1 - b.row), t.i, to_b);
-    queue_push(e, Q_C, len_bucket(b.row - t.r0), t.i, leave && !to_b);
+    queue_push(e, Q_B, len_bucket(g.n_rows - 1 - b.row, g.n_rows), t.i, to_b);
+    queue_push(e, Q_C, len_bucket(b.row - t.r0, g.n_rows), t.i, leave && !to_b);
     if (leave) live = false;
   }
 }
@@ -327,7 +328,7 @@ __device__ __forceinline__ void phase_b(const Env& e) {
     pq = nq;
     const bool leave = live && (!ok || !(b.row + 1 < g.n_rows && b.miss < g.max_miss));   // P18, P20
     if (leave) state_save(e, t, p, C, b);
-    queue_push(e, Q_C, len_bucket(b.row - t.r0), t.i, leave);
+    queue_push(e, Q_C, len_bucket(b.row - t.r0, g.n_rows), t.i, leave);
     if (leave) live = false;
   }
 }
@@ -411,7 +412,7 @@ __device__ __forceinline__ void phase_c(const Env& e) {
     }
     const bool leave = live && (!ok || b.row <= t.r0);   // below the seed's first row phase D searches
     if (leave) state_save(e, t, p, C, b);
-    queue_push(e, Q_D, len_bucket(b.row), t.i, leave);
+    queue_push(e, Q_D, len_bucket(b.row, g.n_rows), t.i, leave);
     if (leave) live = false;
   }
 }

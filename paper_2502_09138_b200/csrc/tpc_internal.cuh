@@ -25,7 +25,7 @@ struct DevGeom {
 };
 
 // Counters living in device memory, zeroed at the start of every call.
-constexpr int A4_Q_BUCKETS = 4;   // a4 phase queues are split by expected tracklet length, longest served first
+constexpr int A4_Q_BUCKETS = 8;   // a4 phase queues are split by expected tracklet length, longest served first
 struct CtlLine {         // one hot counter per 128-byte line
   uint32_t v;
   uint32_t pad[31];
