@@ -114,18 +114,18 @@ __device__ __forceinline__ int len_bucket(int rows_left, int n_rows) {
 
 // Producer side (lanes with pred, after state_save): one atomic per warp and bucket.
 __device__ __forceinline__ void queue_push(const Env& e, int q, int bucket, int i, bool pred) {
-  if (!__any_sync(0xffffffffu, pred)) return;
-#pragma unroll
-  for (int bk = 0; bk < A4_Q_BUCKETS; ++bk) {
+  unsigned todo = __ballot_sync(0xffffffffu, pred);
+  while (todo) {   // one round per distinct bucket among the leaving lanes (usually one or two)
+    const int bk = __shfl_sync(0xffffffffu, bucket, __ffs(todo) - 1);
     const bool mine = pred && bucket == bk;
     const unsigned m = __ballot_sync(0xffffffffu, mine);
-    if (!m) continue;
     const int qq = q * A4_Q_BUCKETS + bk;
     const int leader = __ffs(m) - 1;
     uint32_t base = 0;
     if (e.lane == leader) base = atomicAdd(&e.ctl->q_alloc[qq].v, (uint32_t)__popc(m));
     base = __shfl_sync(0xffffffffu, base, leader);
     if (mine) e.q_items[(size_t)qq * e.s_cap + base + __popc(m & ((1u << e.lane) - 1u))] = (uint32_t)i;
+    todo &= ~m;
   }
 }
 
