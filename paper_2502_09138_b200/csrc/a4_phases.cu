@@ -13,6 +13,10 @@
 namespace {
 
 constexpr int AP_THREADS = 128;
+#ifndef TPC_A4_REFILL_MIN
+#define TPC_A4_REFILL_MIN 8
+#endif
+constexpr int A4_REFILL_MIN = TPC_A4_REFILL_MIN;
 enum : int { Q_B = 0, Q_C = 1, Q_D = 2 };
 
 struct Env {   // everything a warp needs that does not change during a kernel
@@ -169,7 +173,8 @@ __device__ __forceinline__ void phase_a(const Env& e) {
   while (true) {
     const bool want = !live && e.lane < e.lanes_used && !exhausted;
     const unsigned idle = __ballot_sync(FULL, want);
-    if (idle) {
+    // refill in batches: a refill stalls the warp for its gathers, so wait until several lanes are free
+    if (idle && (__popc(idle) >= A4_REFILL_MIN || !__any_sync(FULL, live))) {
       uint32_t base = 0;
       if (e.lane == 0) base = atomicAdd(&e.ctl->next_seed, (uint32_t)__popc(idle));
       base = __shfl_sync(FULL, base, 0);
@@ -289,7 +294,8 @@ __device__ __forceinline__ void phase_b(const Env& e) {
   while (true) {
     const bool want = !live && e.lane < e.lanes_used && !dry;
     const unsigned idle = __ballot_sync(FULL, want);
-    if (idle) {
+    // refill in batches: a refill stalls the warp for its gathers, so wait until several lanes are free
+    if (idle && (__popc(idle) >= A4_REFILL_MIN || !__any_sync(FULL, live))) {
       const int i = queue_pop(e, Q_B, idle, want, &bk, &dry);
       if (i >= 0) {
         state_load(e, i, t, p, C, b);
@@ -355,7 +361,8 @@ __device__ __forceinline__ void phase_c(const Env& e) {
   while (true) {
     const bool want = !live && e.lane < e.lanes_used && !dry;
     const unsigned idle = __ballot_sync(FULL, want);
-    if (idle) {
+    // refill in batches: a refill stalls the warp for its gathers, so wait until several lanes are free
+    if (idle && (__popc(idle) >= A4_REFILL_MIN || !__any_sync(FULL, live))) {
       const int i = queue_pop(e, Q_C, idle, want, &bk, &dry);
       if (i >= 0) {
         state_load(e, i, t, p, C, b);
@@ -439,7 +446,8 @@ __device__ __forceinline__ void phase_d(const Env& e) {
   while (true) {
     const bool want = !live && e.lane < e.lanes_used && !dry;
     const unsigned idle = __ballot_sync(FULL, want);
-    if (idle) {
+    // refill in batches: a refill stalls the warp for its gathers, so wait until several lanes are free
+    if (idle && (__popc(idle) >= A4_REFILL_MIN || !__any_sync(FULL, live))) {
       const int i = queue_pop(e, Q_D, idle, want, &bk, &dry);
       if (i >= 0) {
         state_load(e, i, t, p, C, b);
