@@ -96,7 +96,7 @@ struct tpc_tracker {
   cudaError_t last_err; char err_buf[256];
 };
 
-constexpr int64_t A4_PHASED_MIN_CLUSTERS = 6000000;   // calls at least this large run a4 as phase kernels
+constexpr int64_t A4_PHASED_MIN_CLUSTERS = 5000000;   // calls at least this large run a4 as phase kernels
 constexpr int GRID_MAX_BINS = 48 * 1024;   // bins per row: one row's histogram fits a CTA's shared memory
 constexpr int GRID_MIN_SHIFT = 9;          // finest bins: 512 units = 0.8 cm
 constexpr int A3_TILE = 1024;   // ids per a3 block (256 threads x 4)
