@@ -146,6 +146,85 @@ a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// Sparse and medium rows on the coarse grid (the common case).  In the nested scan a warp pays, per up candidate of
+// any lane, the longest down range of any lane, although a lane's own window holds one or two clusters per side.
+// Here each side's ranges are tested once, the clusters inside the window become bits of a 32-bit mask (bit t = the
+// t-th cluster of the concatenated ranges), and the pair loop visits set bits only.  More than 32 range clusters on
+// a side: the nested scan.
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t range_at(const Ranges& q, uint32_t n0, uint32_t t) {
+  return t < n0 ? q.a0 + t : q.a1 + (t - n0);
+}
+
+__device__ __forceinline__ uint32_t side_mask(const DevGeom& g, const int4* __restrict__ srt, const Ranges& q,
+                                              uint32_t n0, uint32_t n, int yh, int zh) {
+  uint32_t m = 0;
+  const uint32_t span_y = 2u * (uint32_t)g.w_y, span_z = 2u * (uint32_t)g.w_z;
+  for (uint32_t t = 0; t < n; ++t) {
+    const int2 c = *reinterpret_cast<const int2*>(srt + range_at(q, n0, t));
+    // P7, inclusive: |dy| <= w_y and |dz| <= w_z
+    if ((uint32_t)(c.x - yh + g.w_y) <= span_y && (uint32_t)(c.y - zh + g.w_z) <= span_z) m |= 1u << t;
+  }
+  return m;
+}
+
+__global__ void __launch_bounds__(A2_THREADS)
+a2_neighbours_mask_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int4* __restrict__ srt,
+                          const uint32_t* __restrict__ sec_key, const uint32_t* __restrict__ bin_start,
+                          int32_t* __restrict__ link_up, int32_t* __restrict__ link_dn,
+                          uint32_t* __restrict__ owner) {
+  const int sr = blockIdx.x;
+  const int r = sr % g.n_rows;
+  const uint32_t a = ro[sr], b = ro[sr + 1];
+  const bool inner = r >= 1 && r <= g.n_rows - 2;   // P5
+  const int org_z = zmin_from_key(sec_key[sr / g.n_rows]);
+  const uint32_t *bs_u = nullptr, *bs_d = nullptr;
+  if (inner) {
+    bs_u = bin_start + (size_t)(sr + 1) * g.nb_stride;
+    bs_d = bin_start + (size_t)(sr - 1) * g.nb_stride;
+  }
+  for (uint32_t j = a + threadIdx.x; j < b; j += A2_THREADS) {
+    const int4 ch = srt[j];
+    const int yh = ch.x, zh = ch.y, hid = ch.z;
+    int best_u = -1, best_d = -1;
+    if (inner) {
+      const Window w = window_bins(g, yh, zh, org_z);
+      int best_cost = INT32_MAX;
+      const Ranges qu = load_ranges(g, w, bs_u), qd = load_ranges(g, w, bs_d);
+      const uint32_t nu0 = qu.b0 - qu.a0, nu = nu0 + (qu.b1 - qu.a1);
+      const uint32_t nd0 = qd.b0 - qd.a0, nd = nd0 + (qd.b1 - qd.a1);
+      if (nu > 32u || nd > 32u) {
+        pair_search_nested<false>(g, srt, w, bs_u, bs_d, yh, zh, best_cost, best_u, best_d);
+      } else if (nu && nd) {
+        const uint32_t mu = side_mask(g, srt, qu, nu0, nu, yh, zh);
+        const uint32_t md = mu ? side_mask(g, srt, qd, nd0, nd, yh, zh) : 0u;
+        if (md) {
+          for (uint32_t bu = mu; bu; bu &= bu - 1u) {
+            const int4 cu = srt[range_at(qu, nu0, (uint32_t)__ffs((int)bu) - 1u)];
+            const int dyu = cu.x - yh, dzu = cu.y - zh, idu = cu.z;
+            for (uint32_t bd = md; bd; bd &= bd - 1u) {
+              const int4 cd = srt[range_at(qd, nd0, (uint32_t)__ffs((int)bd) - 1u)];
+              const int ddy = dyu + (cd.x - yh), ddz = dzu + (cd.y - zh);
+              const int cost = g.cost_wy * ddy * ddy + g.cost_wz * ddz * ddz;   // P8
+              const int idd = cd.z;
+              if (cost < best_cost || (cost == best_cost && (idu < best_u || (idu == best_u && idd < best_d)))) {   // P9
+                best_cost = cost;
+                best_u = idu;
+                best_d = idd;
+              }
+            }
+          }
+        }
+      }
+      if (best_u < 0 || best_cost > g.c_max) best_u = best_d = -1;   // P10
+    }
+    link_up[hid] = best_u;
+    link_dn[hid] = best_d;
+    owner[hid] = 0u;   // a5 ownership words start empty
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // Dense rows (several clusters per grid bin: pile-up at high density).  The nested scan above tests every cluster
 // of the down ranges once per up candidate; here each side's ranges are filtered once into a short list in shared
 // memory and the pair loop runs over |U| x |D| window candidates only (a few, against hundreds of range pairs).
@@ -252,7 +331,7 @@ cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64
   if (dense && fine) a2_neighbours_dense_kernel<true><<<grid2, A2_THREADS, 0, st>>>(A2_ARGS);
   else if (dense) a2_neighbours_dense_kernel<false><<<grid2, A2_THREADS, 0, st>>>(A2_ARGS);
   else if (fine) a2_neighbours_kernel<true><<<(unsigned)R, A2_THREADS, 0, st>>>(A2_ARGS);
-  else a2_neighbours_kernel<false><<<(unsigned)R, A2_THREADS, 0, st>>>(A2_ARGS);
+  else a2_neighbours_mask_kernel<<<(unsigned)R, A2_THREADS, 0, st>>>(A2_ARGS);
 #undef A2_ARGS
   return cudaGetLastError();
 }
