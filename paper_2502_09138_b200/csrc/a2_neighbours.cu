@@ -11,6 +11,9 @@
 namespace {
 
 constexpr int A2_THREADS = 128;
+#ifndef A2_MASK_UNROLL
+#define A2_MASK_UNROLL 2
+#endif
 
 struct Ranges {
   uint32_t a0, b0, a1, b1;   // up to two contiguous sorted ranges (second empty if the window is in one z-bin)
@@ -160,10 +163,19 @@ __device__ __forceinline__ uint32_t side_mask(const DevGeom& g, const int4* __re
                                               uint32_t n0, uint32_t n, int yh, int zh) {
   uint32_t m = 0;
   const uint32_t span_y = 2u * (uint32_t)g.w_y, span_z = 2u * (uint32_t)g.w_z;
-  for (uint32_t t = 0; t < n; ++t) {
-    const int2 c = *reinterpret_cast<const int2*>(srt + range_at(q, n0, t));
-    // P7, inclusive: |dy| <= w_y and |dz| <= w_z
-    if ((uint32_t)(c.x - yh + g.w_y) <= span_y && (uint32_t)(c.y - zh + g.w_z) <= span_z) m |= 1u << t;
+  // A2_MASK_UNROLL independent loads per trip (the tail re-reads the last cluster; its bits are masked off)
+  for (uint32_t t = 0; t < n; t += A2_MASK_UNROLL) {
+    int2 c[A2_MASK_UNROLL];
+#pragma unroll
+    for (int i = 0; i < A2_MASK_UNROLL; ++i)
+      c[i] = *reinterpret_cast<const int2*>(srt + range_at(q, n0, min(t + (uint32_t)i, n - 1u)));
+#pragma unroll
+    for (int i = 0; i < A2_MASK_UNROLL; ++i) {
+      // P7, inclusive: |dy| <= w_y and |dz| <= w_z
+      const bool in = (uint32_t)(c[i].x - yh + g.w_y) <= span_y && (uint32_t)(c[i].y - zh + g.w_z) <= span_z &&
+                      t + (uint32_t)i < n;
+      m |= (uint32_t)in << ((t + (uint32_t)i) & 31u);
+    }
   }
   return m;
 }
