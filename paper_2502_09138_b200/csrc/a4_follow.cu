@@ -320,6 +320,7 @@ cudaError_t setup_a4_attributes(tpc_tracker* t) {
   int per_sm = 0;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, a4_follow_kernel, A4_THREADS, a4_smem_bytes(t->g));
   if (e != cudaSuccess) return e;
+  t->a4_sms = sms;
   t->a4_blocks = per_sm * sms;   // persistent grid: every resident warp slot of the device
   return t->a4_blocks > 0 ? cudaSuccess : cudaErrorInvalidConfiguration;
 }

@@ -543,8 +543,12 @@ a4_votes_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, const float4* _
   }
 }
 
+// Resident CTAs per SM: the refit phase fits 96 registers without spilling, so it runs at 20 warps per SM; the
+// other three need the full 128 (16 warps).
+constexpr int ap_min_blocks(int ph) { return ph == 2 ? 5 : 4; }
+
 template <int PH>
-__global__ void __launch_bounds__(AP_THREADS, 4)
+__global__ void __launch_bounds__(AP_THREADS, ap_min_blocks(PH))
 a4_phase_kernel(const DevGeom g, uint32_t s_cap, DevCtl* __restrict__ ctl, const int4* __restrict__ rec,
                 const int4* __restrict__ srt, const uint32_t* __restrict__ sec_key,
                 const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ seed_start,
@@ -583,7 +587,7 @@ cudaError_t launch_a4_phases(const tpc_tracker* t, int64_t n, cudaStream_t st) {
   if (n == 0 || t->s_cap == 0) return cudaSuccess;
   const size_t smem = (size_t)t->g.n_rows * (8 + 4);
 #define AP_LAUNCH(PH)                                                                                         \
-  a4_phase_kernel<PH><<<t->a4_blocks, AP_THREADS, smem, st>>>(                                                \
+  a4_phase_kernel<PH><<<t->a4_sms * ap_min_blocks(PH), AP_THREADS, smem, st>>>(                                                \
       t->g, (uint32_t)t->s_cap, t->s.ctl, t->s.rec, t->s.srt, t->s.sec_key, t->s.bin_start, t->s.seed_start, \
       t->s.seed_sr, t->s.tl_rec, t->s.tl_hits, t->s.tl_state, t->s.q_items, t->s.tl_span)
   AP_LAUNCH(0);

@@ -87,6 +87,7 @@ struct tpc_tracker {
   int64_t s_cap;             // seed capacity of the current layout
   int64_t tiles_a3, tiles_a5;
   int a4_phased;             // the most recent call ran a4 as phase kernels (api.cu)
+  int a4_sms;              // SMs of the device (phase kernels size their own persistent grids)
   int a4_blocks, a4_warps;   // persistent a4 grid: blocks x warps per block = resident warps of the device (set at create)
   size_t ctl_bytes;          // bytes zeroed per call
   Scratch s;
