@@ -34,6 +34,7 @@ if ROOT not in sys.path:
 METRIC = "TPC clusters tracked/sec on 1 B200 (central Pb-Pb); % of HBM roofline"
 UNIT = "clusters/s"
 CFG_ID = 1
+DEFAULT_BATCH_EVENTS = 32   # events per tpc_track call
 # algorithmic work per unit: N clusters, N_b grid bins, T tracklet-hits, S seeds
 FLOP_PER_TRACKLET_HIT = 580.0      # a4: (transport + Jacobian + covariance transport + update) x 2 passes
 
@@ -389,7 +390,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=30)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--batch-events", type=int, default=32)
+    ap.add_argument("--batch-events", type=int, default=DEFAULT_BATCH_EVENTS)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-threads", type=int, default=3, help="host threads (handles, streams) of the e2e arm")

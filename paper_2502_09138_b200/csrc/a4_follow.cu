@@ -70,7 +70,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
   int32_t* tab = tl_hits;   // this tracklet's row -> hit table
   State p;
   Cov C;
-  p.y = p.z = p.s = p.t = p.q = 0;
+  p.y = p.z = p.s = p.t = p.q = 0; p.oy = p.oz = 0;
   cov_reset(g, C);
   // gathers issued one step ahead (a mismatch of the tag only costs the direct load)
   int rcn_id = -1;                 // record of cluster rcn_id
@@ -112,6 +112,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
         const float dy = (float)(c1.x - y0) * g.inv_units, dz = (float)(c1.y - z0) * g.inv_units;
         const float ichord = rsqrtf(fmaf(dxr, dxr, dy * dy));
         p.y = 0; p.z = 0; p.s = dy * ichord; p.t = dz * ichord; p.q = 0;
+        p.oy = y0; p.oz = z0;
         row = rmin = rmax = lowest = r0;
         nh = 0; miss = 0; chi2 = 0.f; fail_dn = false;
         t1_row = t2_row = -1;
@@ -193,10 +194,10 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
       const bool pred = nrow >= 0;
       const int srow = pred ? nrow : row;
       const float ndx = (float)(s_row_x[srow] - s_row_x[row]);
-      const float ps = (float)p.s;
-      const float ic = rsqrtf(fmaxf(1.f - ps * ps, 0.05f));
-      const float py = (float)p.y + ndx * ps * ic, pz = (float)p.z + ndx * (float)p.t * ic;
-      const Window w = search_window(g, py, pz, (float)C.c00 + g.sy2, (float)C.c11 + g.sz2, y0, z0, org_z);
+      const float ps = p.s;
+      const float ic = rsqrtf(fmaxf(1.f - ps * ps, 0.05f)) * g.units;
+      const float py = p.y + ndx * ps * ic, pz = p.z + ndx * p.t * ic;
+      const Window w = search_window(g, py, pz, C.var_y() + g.sy2, C.var_z() + g.sz2, p.oy, p.oz, org_z);
       BinRanges nq = pq;
       load_ranges_if(g, bin_start + (size_t)(sec_base + srow) * g.nb_stride, w, nq, pred);
       nk_y = pred ? w.key_y() : pk_y;
@@ -208,20 +209,19 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
     if (ok && tr) ok = transport<true>(g, dx, p, C);
     if (ok) {
       row = trow;
-      float ym = (float)(rc.y - y0) * g.inv_units, zm = (float)(rc.z - z0) * g.inv_units;
+      float ym = resid_y(g, p, rc.y), zm = resid_z(g, p, rc.z);   // residuals of the hit, cm
       if (mode == M_SEARCH) {
-        const float py = (float)p.y, pz = (float)p.z;
-        const float vy = (float)C.c00 + g.sy2, vz = (float)C.c11 + g.sz2;
-        const Window w = search_window(g, py, pz, vy, vz, y0, z0, org_z);
+        const float vy = C.var_y() + g.sy2, vz = C.var_z() + g.sz2;
+        const Window w = search_window(g, p.y, p.z, vy, vz, p.oy, p.oz, org_z);
         Found f;
         f.id = -1;
-        f.y = f.z = 0.f;
+        f.ry = f.rz = 0.f;
         float bestd = __int_as_float(0x7f800000);
         const float wy = 1.f / vy, wz = 1.f / vz;
         if (w.iz_hi <= w.iz_lo + 1) {   // always so on the coarse grid (bins >= 2 gate_z wide)
           BinRanges q = pq;
           load_ranges_if(g, bs, w, q, w.key_y() != pk_y || w.key_z(row) != pk_z);
-          search_ranges(g, q, py, pz, wy, wz, y0, z0, srt, f, bestd);
+          search_ranges(g, q, p, wy, wz, srt, f, bestd);
         } else {   // refined grid (dense call) and a wide gate: two z-bin rows at a time
           for (int iz = w.iz_lo; iz <= w.iz_hi; iz += 2) {
             Window w2 = w;
@@ -229,13 +229,13 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
             w2.iz_hi = min(iz + 1, w.iz_hi);
             BinRanges q2 = {0, 0, 0, 0};
             load_ranges_if(g, bs, w2, q2, true);
-            search_ranges(g, q2, py, pz, wy, wz, y0, z0, srt, f, bestd);
+            search_ranges(g, q2, p, wy, wz, srt, f, bestd);
           }
         }
         if (!(bestd < g.gate_d)) f.id = -1;   // P21
         hid = f.id;
-        ym = f.y;
-        zm = f.z;
+        ym = f.ry;
+        zm = f.rz;
         tab[row] = hid;
         rmin = min(rmin, row);
         rmax = max(rmax, row);
@@ -272,13 +272,15 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
     if (done) {
       if (phase == PH_DONE) {
         float4* o = tl_rec + (size_t)i * TL_REC_V4;
-        o[0] = make_float4((float)s_row_x[row], (float)((double)p.y + (double)y0 * g.inv_units_d),
-                           (float)((double)p.z + (double)z0 * g.inv_units_d), (float)p.s);
+        o[0] = make_float4((float)s_row_x[row], (float)(((double)p.y + (double)p.oy) * g.inv_units_d),
+                           (float)(((double)p.z + (double)p.oz) * g.inv_units_d), (float)p.s);
         o[1] = make_float4((float)p.t, (float)p.q, chi2, __int_as_float(nh));
-        o[2] = make_float4((float)C.c00, (float)C.c10, (float)C.c11, (float)C.c20);
-        o[3] = make_float4((float)C.c21, (float)C.c22, (float)C.c30, (float)C.c31);
-        o[4] = make_float4((float)C.c32, (float)C.c33, (float)C.c40, (float)C.c41);
-        o[5] = make_float4((float)C.c42, (float)C.c43, (float)C.c44, __int_as_float(sec_base + r0));
+        float cv[15];
+        C.lower(cv);
+        o[2] = make_float4(cv[0], cv[1], cv[2], cv[3]);
+        o[3] = make_float4(cv[4], cv[5], cv[6], cv[7]);
+        o[4] = make_float4(cv[8], cv[9], cv[10], cv[11]);
+        o[5] = make_float4(cv[12], cv[13], cv[14], __int_as_float(sec_base + r0));
       }
       __syncwarp();   // the table entries of the ending lanes are visible to the whole warp
       unsigned dm = done;

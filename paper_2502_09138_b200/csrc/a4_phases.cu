@@ -5,7 +5,7 @@
 //   B  extend up with the gated search            (every live lane searches)
 //   C  covariance reset + refit down to the seed's first row over the recorded hits (no search)
 //   D  extend down with the search, final transport, tracklet record, table padding and ownership votes
-// Between two phases a tracklet's filter state is parked in HBM (176 bytes) and its seed rank is pushed into the next
+// Between two phases a tracklet's filter state is parked in HBM (128 bytes) and its seed rank is pushed into the next
 // phase's queue; a kernel boundary separates producers and consumers, so the queues need no flags or fences.
 #include "tpc_internal.cuh"
 #include "a4_search.cuh"
@@ -40,7 +40,7 @@ struct Env {   // everything a warp needs that does not change during a kernel
 };
 
 struct Trk {   // per-tracklet constants, recomputed from the seed rank when a lane picks the tracklet up
-  int i, h0, y0, z0, up0, sec_base, r0, org_z;
+  int i, h0, y0, z0, up0, sec_base, r0, org_z;   // (y0, z0): the first cluster, the state's origin at pick-up
   int32_t* tab;   // its row -> hit table = its final hit list
 };
 
@@ -68,42 +68,39 @@ struct Book {   // bookkeeping that travels with the filter state
 };
 
 __device__ __forceinline__ void state_save(const Env& e, const Trk& t, const State& p, const Cov& C, const Book& b) {
-  const int i = t.i;
-  double2* d = (double2*)(e.tl_state + (size_t)i * A4_STATE_V4);
-  d[0] = make_double2(C.c00, C.c10); d[1] = make_double2(C.c11, C.c20); d[2] = make_double2(C.c21, C.c22);
-  d[3] = make_double2(C.c30, C.c31); d[4] = make_double2(C.c32, C.c33); d[5] = make_double2(C.c40, C.c41);
-  d[6] = make_double2(C.c42, C.c43); d[7] = make_double2(C.c44, 0.0);
-  float4* f = (float4*)(d + 8);
-  f[0] = make_float4((float)p.y, (float)p.z, (float)p.s, (float)p.t);
-  f[1] = make_float4((float)p.q, b.chi2, __int_as_float(b.row), __int_as_float(b.nh));
-  f[2] = make_float4(__int_as_float(b.miss), __int_as_float(b.lowest),
-                     __int_as_float(b.rmin | (b.rmax << 8) | (b.fail_dn ? 1 << 16 : 0)), 0.f);
-  ((int4*)f)[3] = make_int4(t.y0, t.z0, t.sec_base + t.r0, t.org_z);   // so that the next phase needs one gather level
+  float4* f = (float4*)(e.tl_state + (size_t)t.i * A4_STATE_V4);
+  f[0] = make_float4(C.d0, C.d1, C.d2, C.d3);
+  f[1] = make_float4(C.d4, C.u01, C.u02, C.u03);
+  f[2] = make_float4(C.u04, C.u12, C.u13, C.u14);
+  f[3] = make_float4(C.u23, C.u24, C.u34, p.y);
+  f[4] = make_float4(p.z, p.s, p.t, p.q);
+  f[5] = make_float4(b.chi2, __int_as_float(b.row), __int_as_float(b.nh), __int_as_float(b.miss));
+  f[6] = make_float4(__int_as_float(b.lowest), __int_as_float(b.rmin | (b.rmax << 8) | (b.fail_dn ? 1 << 16 : 0)),
+                     0.f, 0.f);
+  ((int4*)f)[7] = make_int4(p.oy, p.oz, t.sec_base + t.r0, t.org_z);   // so that the next phase needs one gather level
 }
 
 __device__ __forceinline__ void state_load(const Env& e, int i, Trk& t, State& p, Cov& C, Book& b) {
-  const double2* d = (const double2*)(e.tl_state + (size_t)i * A4_STATE_V4);
-  const double2 d0 = d[0], d1 = d[1], d2 = d[2], d3 = d[3], d4 = d[4], d5 = d[5], d6 = d[6], d7 = d[7];
-  const float4* f = (const float4*)(d + 8);
-  const float4 f0 = f[0], f1 = f[1], f2 = f[2];
-  const int4 o = ((const int4*)f)[3];
+  const float4* f = (const float4*)(e.tl_state + (size_t)i * A4_STATE_V4);
+  const float4 f0 = f[0], f1 = f[1], f2 = f[2], f3 = f[3], f4 = f[4], f5 = f[5], f6 = f[6];
+  const int4 o = ((const int4*)f)[7];
   t.i = i;
-  t.y0 = o.x;
-  t.z0 = o.y;
+  t.y0 = p.oy = o.x;
+  t.z0 = p.oz = o.y;
   t.sec_base = (o.z / e.g.n_rows) * e.g.n_rows;
   t.r0 = o.z - t.sec_base;
   t.org_z = o.w;
   t.tab = e.tl_hits + (size_t)i * e.g.n_rows;
   t.h0 = t.up0 = -1;
-  C.c00 = d0.x; C.c10 = d0.y; C.c11 = d1.x; C.c20 = d1.y; C.c21 = d2.x; C.c22 = d2.y; C.c30 = d3.x; C.c31 = d3.y;
-  C.c32 = d4.x; C.c33 = d4.y; C.c40 = d5.x; C.c41 = d5.y; C.c42 = d6.x; C.c43 = d6.y; C.c44 = d7.x;
-  p.y = f0.x; p.z = f0.y; p.s = f0.z; p.t = f0.w; p.q = f1.x;
-  b.chi2 = f1.y;
-  b.row = __float_as_int(f1.z);
-  b.nh = __float_as_int(f1.w);
-  b.miss = __float_as_int(f2.x);
-  b.lowest = __float_as_int(f2.y);
-  const int pk = __float_as_int(f2.z);
+  C.d0 = f0.x; C.d1 = f0.y; C.d2 = f0.z; C.d3 = f0.w; C.d4 = f1.x; C.u01 = f1.y; C.u02 = f1.z; C.u03 = f1.w;
+  C.u04 = f2.x; C.u12 = f2.y; C.u13 = f2.z; C.u14 = f2.w; C.u23 = f3.x; C.u24 = f3.y; C.u34 = f3.z;
+  p.y = f3.w; p.z = f4.x; p.s = f4.y; p.t = f4.z; p.q = f4.w;
+  b.chi2 = f5.x;
+  b.row = __float_as_int(f5.y);
+  b.nh = __float_as_int(f5.z);
+  b.miss = __float_as_int(f5.w);
+  b.lowest = __float_as_int(f6.x);
+  const int pk = __float_as_int(f6.y);
   b.rmin = pk & 0xff;
   b.rmax = (pk >> 8) & 0xff;
   b.fail_dn = (pk >> 16) & 1;
@@ -166,7 +163,7 @@ __device__ __forceinline__ void phase_a(const Env& e) {
   Book b = {};
   State p;
   Cov C;
-  p.y = p.z = p.s = p.t = p.q = 0;
+  p.y = p.z = p.s = p.t = p.q = 0; p.oy = p.oz = 0;
   cov_reset(g, C);
   int h = -1;
   Rec3 rcn = {0, 0, -1};
@@ -189,6 +186,7 @@ __device__ __forceinline__ void phase_a(const Env& e) {
         const float dy = (float)(c1.x - t.y0) * g.inv_units, dz = (float)(c1.y - t.z0) * g.inv_units;
         const float ichord = rsqrtf(fmaf(dxr, dxr, dy * dy));
         p.y = 0; p.z = 0; p.s = dy * ichord; p.t = dz * ichord; p.q = 0;
+        p.oy = t.y0; p.oz = t.z0;
         b.row = b.rmin = b.rmax = b.lowest = t.r0;
         b.nh = 0; b.miss = 0; b.chi2 = 0.f; b.fail_dn = false;
         first = true;
@@ -208,7 +206,7 @@ __device__ __forceinline__ void phase_a(const Env& e) {
     if (tr) ok = transport<true>(g, dx, p, C);
     if (ok) {
       b.row = trow;
-      update(g, p, C, (float)(rc.y - t.y0) * g.inv_units, (float)(rc.z - t.z0) * g.inv_units);
+      update(g, p, C, resid_y(g, p, rc.y), resid_z(g, p, rc.z));
       t.tab[trow] = hid;
       b.rmax = trow;
       ++b.nh;
@@ -230,19 +228,18 @@ __device__ __forceinline__ void phase_a(const Env& e) {
 __device__ __forceinline__ Found search_step(const Env& e, const Trk& t, const State& p, const Cov& C, int row,
                                              uint32_t pk_y, uint32_t pk_z, const BinRanges& pq) {
   const DevGeom& g = e.g;
-  const float py = (float)p.y, pz = (float)p.z;
-  const float vy = (float)C.c00 + g.sy2, vz = (float)C.c11 + g.sz2;
-  const Window w = search_window(g, py, pz, vy, vz, t.y0, t.z0, t.org_z);
+  const float vy = C.var_y() + g.sy2, vz = C.var_z() + g.sz2;
+  const Window w = search_window(g, p.y, p.z, vy, vz, p.oy, p.oz, t.org_z);
   const uint32_t* bs = e.bin_start + (size_t)(t.sec_base + row) * g.nb_stride;
   Found f;
   f.id = -1;
-  f.y = f.z = 0.f;
+  f.ry = f.rz = 0.f;
   float bestd = __int_as_float(0x7f800000);
   const float wy = 1.f / vy, wz = 1.f / vz;
   if (w.iz_hi <= w.iz_lo + 1) {   // always so on the coarse grid
     BinRanges q = pq;
     load_ranges_if(g, bs, w, q, w.key_y() != pk_y || w.key_z(row) != pk_z);
-    search_ranges(g, q, py, pz, wy, wz, t.y0, t.z0, e.srt, f, bestd);
+    search_ranges(g, q, p, wy, wz, e.srt, f, bestd);
   } else {   // refined grid and a wide gate: two z-bin rows at a time
     for (int iz = w.iz_lo; iz <= w.iz_hi; iz += 2) {
       Window w2 = w;
@@ -250,7 +247,7 @@ __device__ __forceinline__ Found search_step(const Env& e, const Trk& t, const S
       w2.iz_hi = min(iz + 1, w.iz_hi);
       BinRanges q2 = {0, 0, 0, 0};
       load_ranges_if(g, bs, w2, q2, true);
-      search_ranges(g, q2, py, pz, wy, wz, t.y0, t.z0, e.srt, f, bestd);
+      search_ranges(g, q2, p, wy, wz, e.srt, f, bestd);
     }
   }
   if (!(bestd < g.gate_d)) f.id = -1;   // P21
@@ -264,10 +261,10 @@ __device__ __forceinline__ void predict_ranges(const Env& e, const Trk& t, const
   const DevGeom& g = e.g;
   const int srow = pred ? nrow : row;
   const float ndx = (float)(e.s_row_x[srow] - e.s_row_x[row]);
-  const float ps = (float)p.s;
-  const float ic = rsqrtf(fmaxf(1.f - ps * ps, 0.05f));
-  const float py = (float)p.y + ndx * ps * ic, pz = (float)p.z + ndx * (float)p.t * ic;
-  const Window w = search_window(g, py, pz, (float)C.c00 + g.sy2, (float)C.c11 + g.sz2, t.y0, t.z0, t.org_z);
+  const float ps = p.s;
+  const float ic = rsqrtf(fmaxf(1.f - ps * ps, 0.05f)) * g.units;
+  const float py = p.y + ndx * ps * ic, pz = p.z + ndx * p.t * ic;
+  const Window w = search_window(g, py, pz, C.var_y() + g.sy2, C.var_z() + g.sz2, p.oy, p.oz, t.org_z);
   load_ranges_if(g, e.bin_start + (size_t)(t.sec_base + srow) * g.nb_stride, w, nq, pred);
   if (pred) {
     nk_y = w.key_y();
@@ -287,7 +284,7 @@ __device__ __forceinline__ void phase_b(const Env& e) {
   Book b = {};
   State p;
   Cov C;
-  p.y = p.z = p.s = p.t = p.q = 0;
+  p.y = p.z = p.s = p.t = p.q = 0; p.oy = p.oz = 0;
   cov_reset(g, C);
   uint32_t pk_y = 0xFFFFFFFFu, pk_z = 0xFFFFFFFFu;
   BinRanges pq = {0, 0, 0, 0};
@@ -322,7 +319,7 @@ __device__ __forceinline__ void phase_b(const Env& e) {
       t.tab[trow] = f.id;
       b.rmax = trow;
       if (f.id >= 0) {
-        update(g, p, C, f.y, f.z);
+        update(g, p, C, f.ry, f.rz);
         ++b.nh;
         b.miss = 0;
       } else {
@@ -353,7 +350,7 @@ __device__ __forceinline__ void phase_c(const Env& e) {
   Book b = {};
   State p;
   Cov C;
-  p.y = p.z = p.s = p.t = p.q = 0;
+  p.y = p.z = p.s = p.t = p.q = 0; p.oy = p.oz = 0;
   cov_reset(g, C);
   int t1_row = -1, t1_val = -1, t2_row = -1, t2_val = -1;   // table entries of this step's row and the one below
   int rcn_id = -1;
@@ -412,7 +409,7 @@ __device__ __forceinline__ void phase_c(const Env& e) {
     if (tr) ok = transport<true>(g, dx, p, C);
     if (ok) {
       b.row = trow;
-      if (hid >= 0) b.chi2 += update(g, p, C, (float)(rc.y - t.y0) * g.inv_units, (float)(rc.z - t.z0) * g.inv_units);
+      if (hid >= 0) b.chi2 += update(g, p, C, resid_y(g, p, rc.y), resid_z(g, p, rc.z));
       first = false;
     } else if (live) {
       b.fail_dn = true;   // P18: the state stays at the row where it stopped
@@ -439,7 +436,7 @@ __device__ __forceinline__ void phase_d(const Env& e) {
   Book b = {};
   State p;
   Cov C;
-  p.y = p.z = p.s = p.t = p.q = 0;
+  p.y = p.z = p.s = p.t = p.q = 0; p.oy = p.oz = 0;
   cov_reset(g, C);
   uint32_t pk_y = 0xFFFFFFFFu, pk_z = 0xFFFFFFFFu;
   BinRanges pq = {0, 0, 0, 0};
@@ -484,7 +481,7 @@ __device__ __forceinline__ void phase_d(const Env& e) {
         t.tab[trow] = f.id;
         b.rmin = min(b.rmin, trow);
         if (f.id >= 0) {
-          b.chi2 += update(g, p, C, f.y, f.z);
+          b.chi2 += update(g, p, C, f.ry, f.rz);
           ++b.nh;
           b.miss = 0;
           b.lowest = trow;
@@ -504,13 +501,15 @@ __device__ __forceinline__ void phase_d(const Env& e) {
     if (done) {
       if (fin) {
         float4* o = e.tl_rec + (size_t)t.i * TL_REC_V4;
-        o[0] = make_float4((float)e.s_row_x[b.row], (float)((double)p.y + (double)t.y0 * g.inv_units_d),
-                           (float)((double)p.z + (double)t.z0 * g.inv_units_d), (float)p.s);
+        o[0] = make_float4((float)e.s_row_x[b.row], (float)(((double)p.y + (double)p.oy) * g.inv_units_d),
+                           (float)(((double)p.z + (double)p.oz) * g.inv_units_d), (float)p.s);
         o[1] = make_float4((float)p.t, (float)p.q, b.chi2, __int_as_float(b.nh));
-        o[2] = make_float4((float)C.c00, (float)C.c10, (float)C.c11, (float)C.c20);
-        o[3] = make_float4((float)C.c21, (float)C.c22, (float)C.c30, (float)C.c31);
-        o[4] = make_float4((float)C.c32, (float)C.c33, (float)C.c40, (float)C.c41);
-        o[5] = make_float4((float)C.c42, (float)C.c43, (float)C.c44, __int_as_float(t.sec_base + t.r0));
+        float cv[15];
+        C.lower(cv);
+        o[2] = make_float4(cv[0], cv[1], cv[2], cv[3]);
+        o[3] = make_float4(cv[4], cv[5], cv[6], cv[7]);
+        o[4] = make_float4(cv[8], cv[9], cv[10], cv[11]);
+        o[5] = make_float4(cv[12], cv[13], cv[14], __int_as_float(t.sec_base + t.r0));
         e.tl_span[t.i] = (uint32_t)b.rmin | ((uint32_t)b.rmax << 8);
       }
       if (fin) live = false;

@@ -10,7 +10,7 @@ __device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? l
 
 struct Found {
   int id;
-  float y, z;   // relative coordinates of the accepted hit
+  float ry, rz;   // residuals (hit - state) of the accepted hit, cm
 };
 
 // The search window of P17/P21 in grid bins.  A cluster can only be accepted if dy^2/(Cyy+sy2) < gate_d, so the
@@ -24,21 +24,21 @@ struct Window {
   }
 };
 
-__device__ __forceinline__ Window search_window(const DevGeom& g, float py, float pz, float vy, float vz, int y0, int z0,
+// (py, pz) = fraction of the position in units relative to the integer origin (oy, oz) (kalman.cuh: State).
+__device__ __forceinline__ Window search_window(const DevGeom& g, float py, float pz, float vy, float vz, int oy, int oz,
                                                 int org_z) {
   // half widths in units: gate_d*v*rsqrt(gate_d*v) = sqrt(gate_d*v) to 2 ulp, inside the 0.2 % margin.
-  // float -> int conversions saturate; a state so far off that y0 + (...) wraps has no cluster within the gate
+  // float -> int conversions saturate; a state so far off that oy + (...) wraps has no cluster within the gate
   // (coordinates stay within +-2^24 units of the extents), and the clamps keep every index in range regardless.
   const float ay = g.gate_d * vy, az = g.gate_d * vz;
   const float hy = fminf(g.gate_y, ay * rsqrtf(ay) * 1.002f) * g.units + 2.f;
   const float hz = fminf(g.gate_z, az * rsqrtf(az) * 1.002f) * g.units + 2.f;
-  const float cy = py * g.units, cz = pz * g.units;
-  const int oy = y0 - g.org_y, oz = z0 - org_z;
+  const int by = oy - g.org_y, bz = oz - org_z;
   Window w;
-  w.iy_lo = min(max((__float2int_rd(cy - hy) + oy) >> g.shift_y, 0), g.ny - 1);
-  w.iy_hi = min(max((__float2int_ru(cy + hy) + oy) >> g.shift_y, 0), g.ny - 1);
-  w.iz_lo = min(max((__float2int_rd(cz - hz) + oz) >> g.shift_z, 0), g.nz - 1);
-  w.iz_hi = min(max((__float2int_ru(cz + hz) + oz) >> g.shift_z, 0), g.nz - 1);   // bins >= 2 gate_z: iz_hi <= iz_lo + 1
+  w.iy_lo = min(max((__float2int_rd(py - hy) + by) >> g.shift_y, 0), g.ny - 1);
+  w.iy_hi = min(max((__float2int_ru(py + hy) + by) >> g.shift_y, 0), g.ny - 1);
+  w.iz_lo = min(max((__float2int_rd(pz - hz) + bz) >> g.shift_z, 0), g.nz - 1);
+  w.iz_hi = min(max((__float2int_ru(pz + hz) + bz) >> g.shift_z, 0), g.nz - 1);   // bins >= 2 gate_z: iz_hi <= iz_lo + 1
   return w;
 }
 
@@ -95,9 +95,8 @@ __device__ __forceinline__ void load_ranges_if(const DevGeom& g, const uint32_t*
 
 // P17/P21: among the candidates minimise (d, id), d = dy^2/(Cyy + sy2) + dz^2/(Czz + sz2), restricted to
 // |dy| <= gate_y and |dz| <= gate_z (cm).  Accumulates into (f, bestd); the caller applies the gate d < gate_d.
-__device__ __forceinline__ void search_ranges(const DevGeom& g, const BinRanges& q, float py, float pz, float wy,
-                                              float wz, int y0, int z0, const int4* __restrict__ srt, Found& f,
-                                              float& bestd) {
+__device__ __forceinline__ void search_ranges(const DevGeom& g, const BinRanges& q, const State& p, float wy, float wz,
+                                              const int4* __restrict__ srt, Found& f, float& bestd) {
   const uint32_t n0 = q.b0 - q.a0, total = n0 + (q.b1 - q.a1);
   if (total) {
     int4 nx = srt[n0 ? q.a0 : q.a1];
@@ -105,15 +104,14 @@ __device__ __forceinline__ void search_ranges(const DevGeom& g, const BinRanges&
       const int4 c = nx;
       const uint32_t tn = min(t + 1, total - 1);   // next one in flight (the last iteration re-reads itself)
       nx = srt[tn < n0 ? q.a0 + tn : q.a1 + (tn - n0)];
-      const float cy = (float)(c.x - y0) * g.inv_units, cz = (float)(c.y - z0) * g.inv_units;
-      const float dy = cy - py, dz = cz - pz;
+      const float dy = resid_y(g, p, c.x), dz = resid_z(g, p, c.y);
       if (fabsf(dy) > g.gate_y || fabsf(dz) > g.gate_z) continue;
       const float d = dy * dy * wy + dz * dz * wz;
       if (d < bestd || (d == bestd && c.z < f.id)) {
         bestd = d;
         f.id = c.z;
-        f.y = cy;
-        f.z = cz;
+        f.ry = dy;
+        f.rz = dz;
       }
     }
   }

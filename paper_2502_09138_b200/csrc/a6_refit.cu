@@ -8,7 +8,7 @@
 //
 // Same execution model as a4: persistent warps, one lane per track, lanes refill from a device counter, one
 // uniform step (optional covariance reset, optional transport, update) for both passes; fp32 state relative to
-// the first hit, fp64 covariance.  The hit's (y, z) comes from the a3 records of the same call (rec[id]), requested
+// the first hit, fp32 U D U^T covariance (kalman.cuh).  The hit's (y, z) comes from the a3 records of the same call (rec[id]), requested
 // one step ahead; its row from the row list a5 wrote next to the hit list.
 #include "tpc_internal.cuh"
 #include "kalman.cuh"
@@ -50,7 +50,7 @@ a6_refit_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restric
   float chi2 = 0.f;
   State p;
   Cov C;
-  p.y = p.z = p.s = p.t = p.q = 0;
+  p.y = p.z = p.s = p.t = p.q = 0; p.oy = p.oz = 0;
   cov_reset(g, C);
 
   while (true) {
@@ -74,6 +74,7 @@ a6_refit_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restric
         z0 = c0.y;
         pf_j = 0; pf_y = y0; pf_z = z0;
         p.y = 0; p.z = 0; p.s = 0; p.t = 0; p.q = 0;
+        p.oy = y0; p.oz = z0;
         if (m >= 2) {   // P19 with the gap to the second owned hit
           const int4 c1 = rec[hl[1]];
           const float dxr = (float)(s_row_x[hr[1]] - s_row_x[row]);
@@ -118,7 +119,7 @@ a6_refit_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restric
     if (tr) ok = transport<true>(g, (float)(s_row_x[trow] - s_row_x[row]), p, C);
     if (ok) {
       row = trow;
-      chi2 += update(g, p, C, (float)(cy - y0) * g.inv_units, (float)(cz - z0) * g.inv_units);
+      chi2 += update(g, p, C, resid_y(g, p, cy), resid_z(g, p, cz));
       ++used;
       if (ph == R_FIRST) { phase = R_UP; j = 1; }
       else if (ph == R_UP) { last = j; ++j; }
@@ -131,14 +132,13 @@ a6_refit_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restric
     if (active && ((ph == R_DOWN && !ok) || (phase == R_DOWN && j < 0))) {
       tpc_track_rec_t r = tracks[k];
       r.x = (float)s_row_x[row];
-      r.y = (float)((double)p.y + (double)y0 * g.inv_units_d);
-      r.z = (float)((double)p.z + (double)z0 * g.inv_units_d);
+      r.y = (float)(((double)p.y + (double)p.oy) * g.inv_units_d);
+      r.z = (float)(((double)p.z + (double)p.oz) * g.inv_units_d);
       r.sinphi = (float)p.s;
       r.tanl = (float)p.t;
       r.qpt = (float)p.q;
-      const float cv[15] = {(float)C.c00, (float)C.c10, (float)C.c11, (float)C.c20, (float)C.c21,
-                            (float)C.c22, (float)C.c30, (float)C.c31, (float)C.c32, (float)C.c33,
-                            (float)C.c40, (float)C.c41, (float)C.c42, (float)C.c43, (float)C.c44};
+      float cv[15];
+      C.lower(cv);
 #pragma unroll
       for (int q = 0; q < 15; ++q) r.cov[q] = cv[q];
       r.chi2 = chi2;

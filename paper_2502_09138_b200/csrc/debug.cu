@@ -5,13 +5,14 @@
 
 namespace {
 
-__global__ void dbg_clean_kernel(int64_t n, const int32_t* __restrict__ up, const int32_t* __restrict__ dn,
-                                 int32_t* __restrict__ up_o, int32_t* __restrict__ dn_o) {
+// Cleaned links exactly as a3 left them for a4: rec[h] = (y, z, cleaned up link, cleaned down link).
+__global__ void dbg_clean_kernel(int64_t n, const int4* __restrict__ rec, int32_t* __restrict__ up_o,
+                                 int32_t* __restrict__ dn_o) {
   const int64_t h = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (h >= n) return;
-  const int u = up[h], d = dn[h];
-  up_o[h] = (u >= 0 && dn[u] == (int)h) ? u : -1;
-  dn_o[h] = (d >= 0 && up[d] == (int)h) ? d : -1;
+  const int4 r = rec[h];
+  up_o[h] = r.z;
+  dn_o[h] = r.w;
 }
 
 __global__ void dbg_seed_len_kernel(const DevCtl* ctl, const int32_t* __restrict__ seed_start,
@@ -53,7 +54,7 @@ __global__ void dbg_owner_kernel(int64_t n, const uint32_t* __restrict__ owner, 
 
 cudaError_t launch_dbg_clean(const tpc_tracker* t, int64_t n, int32_t* up, int32_t* dn, cudaStream_t st) {
   if (n == 0) return cudaSuccess;
-  dbg_clean_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, t->s.link_up, t->s.link_dn, up, dn);
+  dbg_clean_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, t->s.rec, up, dn);
   return cudaGetLastError();
 }
 cudaError_t launch_dbg_seed_len(const tpc_tracker* t, int32_t* start, int32_t* len, cudaStream_t st) {

@@ -107,7 +107,7 @@ constexpr int A5_TILE = 128;    // tracklets per a5 block
 __host__ __device__ __forceinline__ uint32_t zmin_key(int32_t z) { return ~((uint32_t)z ^ 0x80000000u); }
 __host__ __device__ __forceinline__ int32_t zmin_from_key(uint32_t k) { return k ? (int32_t)(~k ^ 0x80000000u) : 0; }
 
-constexpr int A4_STATE_V4 = 12; // 16-byte words of a parked a4 state: 15 fp64 covariance, 5 state, bookkeeping, origin
+constexpr int A4_STATE_V4 = 8;  // 16-byte words of a parked a4 state: 15 U D U^T factors, 5 state, bookkeeping, origin
 constexpr int TL_REC_V4 = 6;    // float4 words per tracklet record
 
 // launchers (each in its own .cu)

@@ -33,16 +33,31 @@ def _run_gpu(ev, params=None):
     return res
 
 
+COV_TOL = 1e-3    # |dC_ij| <= COV_TOL * sqrt(C_ii C_jj) (oracle's C): DESIGN.md "Tolerance derivation"
+CHI2_TOL = 1e-3   # |dchi2| <= CHI2_TOL * max(chi2, 1)
+_COV_DIAG = np.array([0, 2, 5, 9, 14])
+_COV_IJ = [(i, j) for i in range(5) for j in range(i + 1)]
+
+
+def cov_scaled_error(c, ref):
+    """|c - ref| / sqrt(ref_ii ref_jj) per packed lower-triangle element (correlation-scale error)."""
+    sd = np.sqrt(np.abs(ref[:, _COV_DIAG]))
+    scale = np.stack([sd[:, i] * sd[:, j] for (i, j) in _COV_IJ], axis=1)
+    return np.abs(c.astype(np.float64) - ref) / np.maximum(scale, 1e-300)
+
+
 def compare(ev, orc, g, o, *, min_assign=0.999, label=""):
     # ---- integer stages: bit-exact ----
     assert np.array_equal(g["link_up"], o["link_up"]), label + " raw up links"
     assert np.array_equal(g["link_dn"], o["link_dn"]), label + " raw dn links"
-    assert np.array_equal(g["up_c"], o["up_c"]) and np.array_equal(g["dn_c"], o["dn_c"]), label + " cleaned links"
+    # cleaned links: what a3 itself wrote for a4 (not a recomputation from the raw tables)
+    assert np.array_equal(g["up_c"], o["up_c"]), label + " cleaned up links"
+    assert np.array_equal(g["dn_c"], o["dn_c"]), label + " cleaned down links"
     assert np.array_equal(g["seed_start"], o["seed_start"]), label + " seed starts"
     assert np.array_equal(g["seed_len"], o["seed_len"]), label + " seed lengths"
     ns = len(o["seed_start"])
     assert g["n_seeds"] == ns
-    # ---- tracklets: hit lists, then parameters on identical hit lists (P25) ----
+    # ---- tracklets: hit lists, then parameters / covariance / chi2 on identical hit lists (P25) ----
     same = np.all(g["hits"] == o["hits"], axis=1) if ns else np.zeros(0, bool)
     frac_same = same.mean() if ns else 1.0
     assert frac_same >= min_assign, f"{label} tracklet hit lists identical for {frac_same:.5f}"
@@ -50,16 +65,42 @@ def compare(ev, orc, g, o, *, min_assign=0.999, label=""):
     err = np.abs(g["par"][same].astype(np.float64) - ref) / np.maximum(np.abs(ref), 1.0)
     worst = err.max(axis=0) if err.size else np.zeros(6)
     n_bad = int((err[:, 1:] > TOL).any(axis=1).sum()) if err.size else 0
-    # P25: parameters within 1e-4; the few that are not count against the 0.1 % budget together with differing lists
-    assert (n_bad + (~same).sum()) <= (1 - min_assign) * max(ns, 1) + 1e-9, \
-        f"{label} {n_bad} tracklets beyond 1e-4 (worst {worst}), {(~same).sum()} differing hit lists of {ns}"
+    # north_star: parameters within 1e-4 -- a bar of its own, not part of the 0.1 % hit-list budget.  Allowed: 2 per
+    # 100 000 tracklets (0 below 50 000), for the ill-conditioned trajectories DESIGN.md "a4 precision" describes: right
+    # after the P22 reset a low-pT tracklet's q/pT estimate can swing to |q/pT| ~ 40 for a few rows, and that stretch
+    # amplifies any rounding difference (fp32 against fp64) by ~1e3.  Measured: 2 of 380 787 (bench batch), 1 of ~1 M.
+    n_allowed = int(2e-5 * same.sum())
+    assert n_bad <= n_allowed, \
+        f"{label} {n_bad} tracklets beyond 1e-4 (worst {worst}) of {int(same.sum())} with identical hit lists"
     assert np.array_equal(g["par"][same][:, 0].astype(np.float64), ref[:, 0].astype(np.float32).astype(np.float64))
+    assert np.array_equal(g["n_hits"][same], o["n_hits"][same]), label + " tracklet n_hits"
+    cerr = cov_scaled_error(g["cov"][same], o["cov"][same]) if err.size else np.zeros((0, 15))
+    worst_cov = float(cerr.max()) if cerr.size else 0.0
+    assert worst_cov <= COV_TOL, f"{label} covariance off by {worst_cov:.3e} (scaled), element {np.unravel_index(cerr.argmax(), cerr.shape)}"
+    xref = o["chi2"][same]
+    xerr = np.abs(g["chi2"][same].astype(np.float64) - xref) / np.maximum(xref, 1.0) if err.size else np.zeros(0)
+    worst_chi2 = float(xerr.max()) if xerr.size else 0.0
+    assert worst_chi2 <= CHI2_TOL, f"{label} chi2 off by {worst_chi2:.3e}"
     # ---- output tracks ----
     gt = g["tracks"]
     frac, pairs = assignment_match(gt["seed_cluster"], gt["hit_offset"], gt["n_hits"], g["hit_ids"],
                                    o["seed_start"][o["trk_seed"]], o["trk_hit_offset"], o["trk_n_owned"], o["hit_ids"])
     assert frac >= min_assign, f"{label} assignments match {frac:.5f}"
     assert np.all(np.diff(gt["seed_cluster"]) > 0), "output order = ascending seed start id (P29)"
+    # the output record of a track carries the fit of its tracklet (P28): bit for bit the tracklet export, and hence
+    # within the bars above of the oracle's par / cov / chi2 of that seed
+    if len(gt):
+        k = np.searchsorted(g["seed_start"], gt["seed_cluster"])
+        assert np.array_equal(g["seed_start"][k], gt["seed_cluster"])
+        rec_par = np.stack([gt[f] for f in ("x", "y", "z", "sinphi", "tanl", "qpt")], axis=1)
+        assert np.array_equal(rec_par, g["par"][k]), label + " track record parameters != tracklet fit"
+        assert np.array_equal(gt["cov"], g["cov"][k]), label + " track record covariance != tracklet fit"
+        assert np.array_equal(gt["chi2"], g["chi2"][k]), label + " track record chi2 != tracklet fit"
+        ks = same[k]
+        rerr = np.abs(rec_par[ks].astype(np.float64) - o["par"][k][ks]) / np.maximum(np.abs(o["par"][k][ks]), 1.0)
+        assert rerr.size == 0 or int((rerr[:, 1:] > TOL).any(axis=1).sum()) <= n_allowed, \
+            label + " track record parameters vs oracle"
+        assert rerr.size == 0 or cov_scaled_error(gt["cov"][ks], o["cov"][k][ks]).max() <= COV_TOL
     sec, row = ev.sector_row()
     for t in range(0, len(gt), max(1, len(gt) // 200)):
         h = g["hit_ids"][gt["hit_offset"][t]: gt["hit_offset"][t] + gt["n_hits"][t]]
@@ -72,7 +113,11 @@ def compare(ev, orc, g, o, *, min_assign=0.999, label=""):
     osec = sec[o["seed_start"][o["trk_seed"]]] if len(o["trk_seed"]) else np.zeros(0, int)
     mo = match_tracks(ev, osec, o["trk_hit_offset"], o["trk_n_owned"], o["hit_ids"])
     assert abs(mg["efficiency"] - mo["efficiency"]) <= 1e-3 and abs(mg["fake_rate"] - mo["fake_rate"]) <= 1e-3, (mg, mo)
-    return dict(frac_same=frac_same, worst=worst, n_bad=n_bad, assign=frac, gpu=mg, orc=mo)
+    res = dict(frac_same=frac_same, worst=worst, n_bad=n_bad, worst_cov=worst_cov, worst_chi2=worst_chi2, assign=frac,
+               gpu=mg, orc=mo)
+    print(f"[parity] {label}: n={ev.n} seeds={ns} same={frac_same:.6f} n_bad={n_bad} worst_par={worst[1:].max():.2e} "
+          f"worst_cov={worst_cov:.2e} worst_chi2={worst_chi2:.2e} assign={frac:.6f}")
+    return res
 
 
 @pytest.mark.parametrize("seed", [0, 1, 2])
@@ -131,12 +176,12 @@ def test_config3_literal_dense(orc):
 
 
 def test_bench_configuration_full_size(orc):
-    """The launch configuration bench.py times: 16 distinct full configs[1] events in one call (576 sectors,
-    ~9.6 M clusters), every output compared."""
-    from bench import shard_seeds
-    evs = [make_event(1, s) for s in shard_seeds(0, 1, 16)]
+    """The launch configuration bench.py times: its default batch of distinct full configs[1] events in one call
+    (32 events = 1152 sectors, ~19.2 M clusters), every output compared."""
+    from bench import shard_seeds, DEFAULT_BATCH_EVENTS
+    evs = [make_event(1, s) for s in shard_seeds(0, 1, DEFAULT_BATCH_EVENTS)]
     ev = concat_events(evs)
-    assert ev.n_sectors == 576 and ev.n > 9_000_000
+    assert ev.n_sectors == 36 * DEFAULT_BATCH_EVENTS and ev.n > 18_000_000
     compare(ev, orc, _run_gpu(ev), orc.track(ev), label="bench batch")
 
 
@@ -153,19 +198,19 @@ def test_config3_medium_density_refined_sparse_grid(orc):
 def test_small_geometry_40_rows(orc):
     """A geometry whose row count is neither 152 nor a multiple of 32 (a4's row tables, a5's row columns)."""
     from gen.events import Config
-    cfg = Config("one_sector_40_rows", n_sectors=1, open_sector=True, tracks_per_collision=150, pt_min=0.3,
+    cfg = Config("one_sector_40_rows", n_sectors=1, open_sector=True, tracks_per_collision=1500, pt_min=0.3,
                  noise=0.05, n_rows=40)
     ev = make_event(cfg, seed=7)
     assert ev.n_rows == 40
     g, o = _run_gpu(ev), orc.track(ev)
-    assert len(o["seed_start"]) > 20
-    compare(ev, orc, g, o, label="40 rows", min_assign=0.99)
+    assert len(o["seed_start"]) > 1000
+    compare(ev, orc, g, o, label="40 rows")
 
 
 def test_non_default_parameters(orc):
     """tpc_params_t reaches every stage: narrower windows, shorter seeds, fewer allowed misses, tighter gate."""
     from paper_2502_09138_b200.binding import default_params
-    ev = make_event(1, 55, n_tracks=800)
+    ev = make_event(1, 55, n_tracks=2500)
     gp, op = default_params(), orc.default_params()
     for p in (gp, op):
         p.w_y, p.w_z, p.c_max, p.l_min = 1000, 1300, 2500000, 4
@@ -173,8 +218,8 @@ def test_non_default_parameters(orc):
         p.gate_d, p.gate_y_cm, p.gate_z_cm, p.sinphi_max = 9.0, 1.5, 2.0, 0.9
         p.c_reset[4] = 16.0
     g, o = _run_gpu(ev, gp), orc.track(ev, op)
-    assert len(o["trk_seed"]) > 100
-    compare(ev, orc, g, o, label="params", min_assign=0.998)
+    assert len(o["trk_seed"]) > 1000
+    compare(ev, orc, g, o, label="params")
 
 
 def test_batch_as_extra_sectors(orc):
@@ -358,13 +403,13 @@ def test_edge_empty_and_tiny(orc):
 
 def test_ragged_rows_and_clusters_outside_nominal_extent(orc):
     """Rows with 0 / 1 / many clusters, and clusters far outside the geometry's nominal y/z extent (edge bins)."""
-    ev = make_event(1, 77, n_tracks=300)
+    ev = make_event(1, 77, n_tracks=1500)
     y = ev.y.copy()
     z = ev.z.copy()
     z[::7] += 640 * 300      # well beyond z_extent
     y[::11] -= 640 * 200     # well beyond the sector edge
     ev.y, ev.z = y, z
-    compare(ev, orc, _run_gpu(ev), orc.track(ev), label="outside-extent", min_assign=0.995)
+    compare(ev, orc, _run_gpu(ev), orc.track(ev), label="outside-extent")
 
 
 def test_capacity_overflow_flags(orc):
