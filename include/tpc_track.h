@@ -40,6 +40,11 @@ extern "C" {
 /* device-side flags OR-ed into counts[2] */
 #define TPC_FLAG_TRACK_OVERFLOW 1u /* more output tracks than track_capacity: tracks beyond it not written */
 #define TPC_FLAG_HIT_OVERFLOW 2u   /* more output hits than hit_capacity: those tracks' hit lists not written */
+#define TPC_FLAG_SEED_OVERFLOW 4u  /* more seeds than the handle's seed capacity (n/16 + 4096 unless reserved): the
+                                      seeds beyond it (in bin order of their start cluster) were not followed, so
+                                      tracks are missing; counts[3] holds the number of seeds the call needs --
+                                      pass it to tpc_reserve_seeds and repeat the call */
+#define TPC_FLAG_BAD_OFFSETS 8u    /* row_offsets not ascending or row_offsets[last] != n: nothing was tracked */
 
 /* Free constants of the method.  tpc_default_params fills the defaults. */
 typedef struct {
@@ -100,7 +105,8 @@ typedef struct {
   int32_t* hit_ids;        /* [device] hit_capacity cluster ids; per track ascending row */
   int32_t* counts;         /* [device] 4 x int32: [0] tracks found, [1] hits found (both may exceed the
                               capacities: then the matching TPC_FLAG_* is set and the excess is not written),
-                              [2] flags, [3] number of seeds (tracklets followed) */
+                              [2] flags, [3] number of seeds the call holds (= tracklets followed, unless
+                              TPC_FLAG_SEED_OVERFLOW is set) */
 } tpc_tracks_out_t;
 
 typedef struct tpc_tracker tpc_tracker_t;
@@ -116,9 +122,17 @@ int tpc_tracker_create(const tpc_geometry_t* geometry, const tpc_field_t* field,
  * Errors: TPC_ERR_ARG, TPC_ERR_CAPACITY, TPC_ERR_NOMEM, TPC_ERR_CUDA. */
 int tpc_track(tpc_tracker_t* t, const tpc_clusters_t* clusters, int64_t n, void* stream, tpc_tracks_out_t* out);
 
+/* Seed capacity of the handle.  Scratch per seed is ~2.2 KB (hit table, measurement stream, filter state), so the
+ * default bound is n/16 + 4096 seeds per call instead of the worst case n/l_min; events with more seeds set
+ * TPC_FLAG_SEED_OVERFLOW.  tpc_reserve_seeds raises the bound for all later calls (never lowers it).  The
+ * synthetic configs of BASELINE.json need n/50 (central Pb-Pb) to n/20 (stress).  Errors: TPC_ERR_ARG. */
+int tpc_reserve_seeds(tpc_tracker_t* t, int64_t n_seeds);
+
 /* Same computation with HOST buffers: copies y, z, row_offsets to device staging owned by the handle, runs
  * tpc_track, copies counts, tracks and hit_ids back into the [host] buffers of `out_host`, and synchronises
- * `stream` before returning.  Pinned host memory makes the copies asynchronous but is not required. */
+ * `stream` before returning.  Pinned host memory makes the copies asynchronous but is not required.
+ * On TPC_FLAG_SEED_OVERFLOW it reserves the seeds the call asked for and runs it once more before returning.
+ * Hit ids are copied for min(counts[1], hit_capacity) entries (the lists of the tracks that fitted). */
 int tpc_track_host(tpc_tracker_t* t, const tpc_clusters_t* clusters_host, int64_t n, void* stream,
                    tpc_tracks_out_t* out_host);
 
@@ -151,11 +165,17 @@ int tpc_get_stage_ms(tpc_tracker_t* t, float ms[5]);
  * *n_calls (may be NULL) receives how many calls were averaged.  Synchronises on those calls' events. */
 int tpc_get_stage_ms_mean(tpc_tracker_t* t, float ms[5], int32_t* n_calls);
 
+/* ---- test-only: a4 has two variants that compute the same thing (phase kernels for large calls, one uniform
+ * kernel for small ones).  0 = choose by call size (default), 1 = uniform, 2 = phased. */
+int tpc_debug_set_a4_variant(tpc_tracker_t* t, int variant);
+
 /* ---- test-only exports: intermediate results of the most recent tpc_track call on this handle ----
  * All outputs are [device] buffers in id space (-1 = none), written asynchronously on `stream`. */
-/* which = 0: raw a2 link tables; 1: cleaned (a3).  up, dn: n int32 each. */
+/* which = 0: raw a2 link tables; 1: cleaned links as a3 stored them (the up link per cluster; the down links are
+ * the inverse of those, a3 keeps no down table).  Internally links are sorted positions; the export translates
+ * them to cluster ids.  up, dn: n int32 each. */
 int tpc_debug_copy_links(tpc_tracker_t* t, int which, int32_t* up, int32_t* dn, void* stream);
-/* start, len: capacity n/l_min + 1 each (seeds ascend by start id, P14). */
+/* start, len: counts[3] entries each (seeds ascend by start id, P14). */
 int tpc_debug_copy_seeds(tpc_tracker_t* t, int32_t* start, int32_t* len, void* stream);
 /* Tracklets of all seeds, seed-major: par[s*6 + 0..5] = (x_ref, y, z, sin phi, tan lambda, q/pT),
  * cov[s*15 + ..], chi2[s], n_hits[s], hits[s*n_rows + r] = cluster id in row r or -1.

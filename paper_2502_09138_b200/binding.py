@@ -105,6 +105,8 @@ def load_library():
     lib.tpc_scratch_bytes.argtypes = [C.c_void_p]
     lib.tpc_scratch_bytes.restype = C.c_int64
     lib.tpc_launches_per_call.argtypes = [C.c_void_p]
+    lib.tpc_reserve_seeds.argtypes = [C.c_void_p, C.c_int64]
+    lib.tpc_debug_set_a4_variant.argtypes = [C.c_void_p, C.c_int]
     lib.tpc_set_stage_timing.argtypes = [C.c_void_p, C.c_int]
     lib.tpc_get_stage_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
     lib.tpc_get_stage_ms_mean.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_int32)]
@@ -292,9 +294,17 @@ class Tracker:
         self._check(self._lib.tpc_debug_copy_links(self._h, 1 if cleaned else 0, _ptr(up), _ptr(dn), self._stream_ptr(None)))
         return up.cpu().numpy(), dn.cpu().numpy()
 
+    def reserve_seeds(self, n_seeds: int):
+        """tpc_reserve_seeds: raise the handle's seed capacity (after TPC_FLAG_SEED_OVERFLOW)."""
+        self._check(self._lib.tpc_reserve_seeds(self._h, C.c_int64(int(n_seeds))))
+
+    def set_a4_variant(self, variant: int):
+        """tpc_debug_set_a4_variant: 0 = by call size, 1 = uniform kernel, 2 = phase kernels (tests)."""
+        self._check(self._lib.tpc_debug_set_a4_variant(self._h, C.c_int(int(variant))))
+
     def debug_seeds(self, n: int, n_seeds: int):
         import torch
-        cap = n // self.l_min + 1
+        cap = max(int(n_seeds), 1)
         st = torch.empty(cap, dtype=torch.int32, device="cuda")
         ln = torch.empty(cap, dtype=torch.int32, device="cuda")
         self._check(self._lib.tpc_debug_copy_seeds(self._h, _ptr(st), _ptr(ln), self._stream_ptr(None)))

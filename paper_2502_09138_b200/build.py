@@ -38,8 +38,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         objs.append(o)
         if not force and os.path.exists(o) and all(os.path.getmtime(d) <= os.path.getmtime(o) for d in [s] + HEADERS):
             continue
-        extra = os.environ.get("TPC_NVCC_EXTRA", "").split()   # experiments only (e.g. -DTPC_A4_COV32)
-        cmd = ([_nvcc()] + NVCC_FLAGS + EXTRA_FLAGS.get(os.path.basename(s), []) + extra
+        cmd = ([_nvcc()] + NVCC_FLAGS + EXTRA_FLAGS.get(os.path.basename(s), [])
                + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o])
         procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     for cmd, p in procs:

@@ -21,11 +21,24 @@ __device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? l
 constexpr int A0_THREADS = 256;
 constexpr int A0_PER_THREAD = 8;
 
+// Input contract check (tpc_track.h): row_offsets must be an ascending CSR over exactly n clusters, starting at 0.
+// A violation raises ctl->bad_offsets; a0..a3 then return at once (malformed offsets would become out-of-range
+// scatter addresses in a1), no seed exists, and a5 reports TPC_FLAG_BAD_OFFSETS with zero tracks.
+__global__ void __launch_bounds__(256)
+a0_check_kernel(int64_t R, int64_t n, const uint32_t* __restrict__ ro, DevCtl* __restrict__ ctl) {
+  bool bad = false;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < R; i += (int64_t)gridDim.x * blockDim.x)
+    bad |= ro[i] > ro[i + 1];
+  if (blockIdx.x == 0 && threadIdx.x == 0) bad |= ro[0] != 0u || (int64_t)ro[R] != n;
+  if (bad) ctl->bad_offsets = 1u;
+}
+
 // grid = (chunks, n_sectors): block (c, s) reduces its slice of sector s's contiguous cluster range.
 __global__ void __launch_bounds__(A0_THREADS)
-a0_origin_kernel(const DevGeom g, const int32_t* __restrict__ z, const uint32_t* __restrict__ ro,
-                 uint32_t* __restrict__ sec_key) {
+a0_origin_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, const int32_t* __restrict__ z,
+                 const uint32_t* __restrict__ ro, uint32_t* __restrict__ sec_key) {
   __shared__ int red[A0_THREADS / 32];
+  if (ctl->bad_offsets) return;
   for (int sec = blockIdx.y; sec < g.n_sectors; sec += gridDim.y) {   // block-uniform loop (gridDim.y caps at 65535)
   const uint32_t a = ro[(size_t)sec * g.n_rows], b = ro[(size_t)(sec + 1) * g.n_rows];
   int zmin = INT32_MAX;
@@ -63,11 +76,12 @@ __device__ __forceinline__ void group_sync() {
 
 template <int G>
 __global__ void __launch_bounds__(A1_THREADS)
-a1_grid_kernel(const DevGeom g, int64_t R, const int32_t* __restrict__ y, const int32_t* __restrict__ z,
-               const uint32_t* __restrict__ ro, const uint32_t* __restrict__ sec_key, int4* __restrict__ srt,
-               uint32_t* __restrict__ bin_start) {
+a1_grid_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, int64_t R, const int32_t* __restrict__ y,
+               const int32_t* __restrict__ z, const uint32_t* __restrict__ ro, const uint32_t* __restrict__ sec_key,
+               int4* __restrict__ srt, uint32_t* __restrict__ bin_start) {
   extern __shared__ uint32_t hist_all[];
   __shared__ uint32_t wsum[33];
+  if (ctl->bad_offsets) return;
   const int grp = threadIdx.x / G, gt = threadIdx.x % G;
   const int64_t sr = (int64_t)blockIdx.x * (A1_THREADS / G) + grp;
   if (sr >= R) return;   // G == 32 only (whole warps); with G == A1_THREADS the grid is exactly R
@@ -170,11 +184,19 @@ cudaError_t launch_a1_grid(const tpc_tracker* t, const int32_t* y, const int32_t
   if (a1_warp_rows(t, n)) {
     const int per = A1_THREADS / 32;
     a1_grid_kernel<32><<<(unsigned)((R + per - 1) / per), A1_THREADS, a1_smem_bytes(t->g) * per, st>>>(
-        t->g, R, y, z, ro, t->s.sec_key, t->s.srt, t->s.bin_start);
+        t->g, t->s.ctl, R, y, z, ro, t->s.sec_key, t->s.srt, t->s.bin_start);
   } else {
     a1_grid_kernel<A1_THREADS><<<(unsigned)R, A1_THREADS, a1_smem_bytes(t->g), st>>>(
-        t->g, R, y, z, ro, t->s.sec_key, t->s.srt, t->s.bin_start);
+        t->g, t->s.ctl, R, y, z, ro, t->s.sec_key, t->s.srt, t->s.bin_start);
   }
+  return cudaGetLastError();
+}
+
+cudaError_t launch_a0_check(const tpc_tracker* t, const uint32_t* ro, int64_t n, cudaStream_t st) {
+  const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
+  int64_t blocks = (R + 255) / 256;
+  blocks = blocks < 1 ? 1 : (blocks > 1024 ? 1024 : blocks);
+  a0_check_kernel<<<(unsigned)blocks, 256, 0, st>>>(R, n, ro, t->s.ctl);
   return cudaGetLastError();
 }
 
@@ -185,6 +207,6 @@ cudaError_t launch_a0_origin(const tpc_tracker* t, const int32_t* z, const uint3
   int64_t chunks = (n / t->g.n_sectors + per_block - 1) / per_block;
   if (chunks < 1) chunks = 1;
   if (chunks > 1024) chunks = 1024;
-  a0_origin_kernel<<<dim3((unsigned)chunks, (unsigned)(t->g.n_sectors < 65535 ? t->g.n_sectors : 65535)), A0_THREADS, 0, st>>>(t->g, z, ro, t->s.sec_key);
+  a0_origin_kernel<<<dim3((unsigned)chunks, (unsigned)(t->g.n_sectors < 65535 ? t->g.n_sectors : 65535)), A0_THREADS, 0, st>>>(t->g, t->s.ctl, z, ro, t->s.sec_key);
   return cudaGetLastError();
 }

@@ -3,7 +3,9 @@
 //
 // For cluster h in row r (1 <= r <= n_rows-2): U = clusters of row r+1 with |dy| <= w_y and |dz| <= w_z,
 // D likewise in row r-1; pick the pair minimising (cost, id_u, id_d), cost = cost_wy*(yu+yd-2yh)^2 +
-// cost_wz*(zu+zd-2zh)^2; accept iff cost <= c_max.  Links are written in id space.
+// cost_wz*(zu+zd-2zh)^2; accept iff cost <= c_max.  Ties are broken by cluster id (P9); the links are written in
+// SORTED space (the position of the linked cluster in srt), at the sorted position of h: coalesced stores, and a3 / a4
+// follow them through the same bin-ordered array the searches read.
 // The a1 grid prunes the candidates: bins are at least 2*w wide, so a window touches at most 2 x 2 bins, and
 // with y-fastest bin order each z-bin contributes one contiguous range of sorted clusters.
 #include "tpc_internal.cuh"
@@ -11,9 +13,7 @@
 namespace {
 
 constexpr int A2_THREADS = 128;
-#ifndef A2_MASK_UNROLL
-#define A2_MASK_UNROLL 2
-#endif
+constexpr int A2_MASK_UNROLL = 2;   // independent loads per trip of the window test
 
 struct Ranges {
   uint32_t a0, b0, a1, b1;   // up to two contiguous sorted ranges (second empty if the window is in one z-bin)
@@ -48,19 +48,28 @@ __device__ __forceinline__ Ranges load_ranges(const DevGeom& g, const Window& w,
   return q;
 }
 
+struct Best {   // running best pair: cost and sorted positions (what is stored).  The ids that break cost ties
+  int cost, pu, pd;   // (P9) are read back from srt only when a tie happens: one pair in ~1e4
+};
+
+// P9 on a cost tie: does the pair (idu, idd) come before the running best in (id_u, id_d) order?
+__device__ __forceinline__ bool tie_wins(const int4* __restrict__ srt, const Best& b, int idu, int idd) {
+  const int bu = srt[b.pu].z;
+  return idu < bu || (idu == bu && idd < srt[b.pd].z);
+}
+
 // One candidate pair against the running best (P8, P9).
-__device__ __forceinline__ void try_pair(const DevGeom& g, int dyu, int dzu, int idu, const int4& cd, int yh, int zh,
-                                         int& best_cost, int& best_u, int& best_d) {
+__device__ __forceinline__ void try_pair(const DevGeom& g, const int4* __restrict__ srt, int dyu, int dzu, int idu,
+                                         uint32_t pu, const int4& cd, uint32_t pd, int yh, int zh, Best& b) {
   const int dyd = cd.x - yh, dzd = cd.y - zh;
   if (abs(dyd) > g.w_y || abs(dzd) > g.w_z) return;
   const int ddy = dyu + dyd, ddz = dzu + dzd;
   const int cost = g.cost_wy * ddy * ddy + g.cost_wz * ddz * ddz;
-  if (cost > best_cost) return;
-  const int idd = cd.z;
-  if (cost < best_cost || idu < best_u || (idu == best_u && idd < best_d)) {
-    best_cost = cost;
-    best_u = idu;
-    best_d = idd;
+  if (cost > b.cost) return;
+  if (cost < b.cost || tie_wins(srt, b, idu, cd.z)) {
+    b.cost = cost;
+    b.pu = (int)pu;
+    b.pd = (int)pd;
   }
 }
 
@@ -69,8 +78,7 @@ __device__ __forceinline__ void try_pair(const DevGeom& g, int dyu, int dzu, int
 template <bool FINE>
 __device__ __forceinline__ void pair_search_nested(const DevGeom& g, const int4* __restrict__ srt, const Window& w,
                                                    const uint32_t* __restrict__ bs_u,
-                                                   const uint32_t* __restrict__ bs_d, int yh, int zh, int& best_cost,
-                                                   int& best_u, int& best_d) {
+                                                   const uint32_t* __restrict__ bs_d, int yh, int zh, Best& b) {
   if (!FINE) {
     const Ranges qu = load_ranges(g, w, bs_u), qd = load_ranges(g, w, bs_d);
 #pragma unroll 1
@@ -81,23 +89,9 @@ __device__ __forceinline__ void pair_search_nested(const DevGeom& g, const int4*
         const int dyu = cu.x - yh, dzu = cu.y - zh;
         if (abs(dyu) > g.w_y || abs(dzu) > g.w_z) continue;
 #pragma unroll 1
-        const int idu = cu.z;
         for (int pd = 0; pd < 2; ++pd) {
           const uint32_t da = pd ? qd.a1 : qd.a0, db = pd ? qd.b1 : qd.b0;
-          for (uint32_t d = da; d < db; ++d) {
-            const int4 cd = srt[d];
-            const int dyd = cd.x - yh, dzd = cd.y - zh;
-            if (abs(dyd) > g.w_y || abs(dzd) > g.w_z) continue;
-            const int ddy = dyu + dyd, ddz = dzu + dzd;
-            const int cost = g.cost_wy * ddy * ddy + g.cost_wz * ddz * ddz;
-            if (cost > best_cost) continue;
-            const int idd = cd.z;
-            if (cost < best_cost || idu < best_u || (idu == best_u && idd < best_d)) {   // P9
-              best_cost = cost;
-              best_u = idu;
-              best_d = idd;
-            }
-          }
+          for (uint32_t d = da; d < db; ++d) try_pair(g, srt, dyu, dzu, cu.z, u, srt[d], d, yh, zh, b);
         }
       }
     }
@@ -110,7 +104,7 @@ __device__ __forceinline__ void pair_search_nested(const DevGeom& g, const int4*
         if (abs(dyu) > g.w_y || abs(dzu) > g.w_z) continue;
         for (int izd = w.iz_lo; izd <= w.iz_hi; ++izd) {
           const uint32_t da = bs_d[izd * g.ny + w.iy_lo], db = bs_d[izd * g.ny + w.iy_hi + 1];
-          for (uint32_t d = da; d < db; ++d) try_pair(g, dyu, dzu, cu.z, srt[d], yh, zh, best_cost, best_u, best_d);
+          for (uint32_t d = da; d < db; ++d) try_pair(g, srt, dyu, dzu, cu.z, u, srt[d], d, yh, zh, b);
         }
       }
     }
@@ -119,9 +113,10 @@ __device__ __forceinline__ void pair_search_nested(const DevGeom& g, const int4*
 
 template <bool FINE>
 __global__ void __launch_bounds__(A2_THREADS)
-a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int4* __restrict__ srt,
+a2_neighbours_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, const uint32_t* __restrict__ ro, const int4* __restrict__ srt,
                      const uint32_t* __restrict__ sec_key, const uint32_t* __restrict__ bin_start,
-                     int32_t* __restrict__ link_up, int32_t* __restrict__ link_dn, uint32_t* __restrict__ owner) {
+                     int32_t* __restrict__ link_up, int32_t* __restrict__ link_dn) {
+  if (ctl->bad_offsets) return;
   const int sr = blockIdx.x;
   const int r = sr % g.n_rows;
   const uint32_t a = ro[sr], b = ro[sr + 1];
@@ -134,17 +129,15 @@ a2_neighbours_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int
   }
   for (uint32_t j = a + threadIdx.x; j < b; j += A2_THREADS) {
     const int4 ch = srt[j];
-    const int yh = ch.x, zh = ch.y, hid = ch.z;
-    int best_u = -1, best_d = -1;
+    const int yh = ch.x, zh = ch.y;
+    Best b = {INT32_MAX, -1, -1};
     if (inner) {
       const Window w = window_bins(g, yh, zh, org_z);
-      int best_cost = INT32_MAX;
-      pair_search_nested<FINE>(g, srt, w, bs_u, bs_d, yh, zh, best_cost, best_u, best_d);
-      if (best_u < 0 || best_cost > g.c_max) best_u = best_d = -1;   // P10
+      pair_search_nested<FINE>(g, srt, w, bs_u, bs_d, yh, zh, b);
+      if (b.pu < 0 || b.cost > g.c_max) b.pu = b.pd = -1;   // P10
     }
-    link_up[hid] = best_u;
-    link_dn[hid] = best_d;
-    owner[hid] = 0u;   // a5 ownership words start empty
+    link_up[j] = b.pu;
+    link_dn[j] = b.pd;
   }
 }
 
@@ -180,11 +173,12 @@ __device__ __forceinline__ uint32_t side_mask(const DevGeom& g, const int4* __re
   return m;
 }
 
-__global__ void __launch_bounds__(A2_THREADS)
-a2_neighbours_mask_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int4* __restrict__ srt,
+// 16 CTAs of 128 threads per SM (32 registers): the kernel hides its gathers with resident warps
+__global__ void __launch_bounds__(A2_THREADS, 16)
+a2_neighbours_mask_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, const uint32_t* __restrict__ ro, const int4* __restrict__ srt,
                           const uint32_t* __restrict__ sec_key, const uint32_t* __restrict__ bin_start,
-                          int32_t* __restrict__ link_up, int32_t* __restrict__ link_dn,
-                          uint32_t* __restrict__ owner) {
+                          int32_t* __restrict__ link_up, int32_t* __restrict__ link_dn) {
+  if (ctl->bad_offsets) return;
   const int sr = blockIdx.x;
   const int r = sr % g.n_rows;
   const uint32_t a = ro[sr], b = ro[sr + 1];
@@ -197,42 +191,41 @@ a2_neighbours_mask_kernel(const DevGeom g, const uint32_t* __restrict__ ro, cons
   }
   for (uint32_t j = a + threadIdx.x; j < b; j += A2_THREADS) {
     const int4 ch = srt[j];
-    const int yh = ch.x, zh = ch.y, hid = ch.z;
-    int best_u = -1, best_d = -1;
+    const int yh = ch.x, zh = ch.y;
+    Best b = {INT32_MAX, -1, -1};
     if (inner) {
       const Window w = window_bins(g, yh, zh, org_z);
-      int best_cost = INT32_MAX;
       const Ranges qu = load_ranges(g, w, bs_u), qd = load_ranges(g, w, bs_d);
       const uint32_t nu0 = qu.b0 - qu.a0, nu = nu0 + (qu.b1 - qu.a1);
       const uint32_t nd0 = qd.b0 - qd.a0, nd = nd0 + (qd.b1 - qd.a1);
       if (nu > 32u || nd > 32u) {
-        pair_search_nested<false>(g, srt, w, bs_u, bs_d, yh, zh, best_cost, best_u, best_d);
+        pair_search_nested<false>(g, srt, w, bs_u, bs_d, yh, zh, b);
       } else if (nu && nd) {
         const uint32_t mu = side_mask(g, srt, qu, nu0, nu, yh, zh);
         const uint32_t md = mu ? side_mask(g, srt, qd, nd0, nd, yh, zh) : 0u;
         if (md) {
           for (uint32_t bu = mu; bu; bu &= bu - 1u) {
-            const int4 cu = srt[range_at(qu, nu0, (uint32_t)__ffs((int)bu) - 1u)];
+            const uint32_t pu = range_at(qu, nu0, (uint32_t)__ffs((int)bu) - 1u);
+            const int4 cu = srt[pu];
             const int dyu = cu.x - yh, dzu = cu.y - zh, idu = cu.z;
             for (uint32_t bd = md; bd; bd &= bd - 1u) {
-              const int4 cd = srt[range_at(qd, nd0, (uint32_t)__ffs((int)bd) - 1u)];
+              const uint32_t pd = range_at(qd, nd0, (uint32_t)__ffs((int)bd) - 1u);
+              const int4 cd = srt[pd];
               const int ddy = dyu + (cd.x - yh), ddz = dzu + (cd.y - zh);
               const int cost = g.cost_wy * ddy * ddy + g.cost_wz * ddz * ddz;   // P8
-              const int idd = cd.z;
-              if (cost < best_cost || (cost == best_cost && (idu < best_u || (idu == best_u && idd < best_d)))) {   // P9
-                best_cost = cost;
-                best_u = idu;
-                best_d = idd;
+              if (cost < b.cost || (cost == b.cost && tie_wins(srt, b, idu, cd.z))) {   // P9
+                b.cost = cost;
+                b.pu = (int)pu;
+                b.pd = (int)pd;
               }
             }
           }
         }
       }
-      if (best_u < 0 || best_cost > g.c_max) best_u = best_d = -1;   // P10
+      if (b.pu < 0 || b.cost > g.c_max) b.pu = b.pd = -1;   // P10
     }
-    link_up[hid] = best_u;
-    link_dn[hid] = best_d;
-    owner[hid] = 0u;   // a5 ownership words start empty
+    link_up[j] = b.pu;
+    link_dn[j] = b.pd;
   }
 }
 
@@ -246,7 +239,7 @@ constexpr int A2_KEEP = 12;
 
 __device__ __forceinline__ int filter_side(const DevGeom& g, const int4* __restrict__ srt, const Window& w,
                                            const uint32_t* __restrict__ bs, int yh, int zh,
-                                           int* __restrict__ col /* [A2_KEEP][3][A2_THREADS] column */) {
+                                           int* __restrict__ col /* [A2_KEEP][3][A2_THREADS] column: dy, dz, sorted position */) {
   int cnt = 0;
   for (int iz = w.iz_lo; iz <= w.iz_hi; ++iz) {   // one contiguous sorted range per z-bin row of the window
     const uint32_t ra = bs[iz * g.ny + w.iy_lo], rb = bs[iz * g.ny + w.iy_hi + 1];
@@ -261,7 +254,7 @@ __device__ __forceinline__ int filter_side(const DevGeom& g, const int4* __restr
           int* e = col + cnt * 3 * A2_THREADS;
           e[0] = dy;
           e[A2_THREADS] = dz;
-          e[2 * A2_THREADS] = c.z;
+          e[2 * A2_THREADS] = (int)t;   // sorted position; ids are only needed on cost ties (P9)
         }
         ++cnt;
       }
@@ -272,11 +265,11 @@ __device__ __forceinline__ int filter_side(const DevGeom& g, const int4* __restr
 
 template <bool FINE>
 __global__ void __launch_bounds__(A2_THREADS)
-a2_neighbours_dense_kernel(const DevGeom g, const uint32_t* __restrict__ ro, const int4* __restrict__ srt,
+a2_neighbours_dense_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, const uint32_t* __restrict__ ro, const int4* __restrict__ srt,
                            const uint32_t* __restrict__ sec_key, const uint32_t* __restrict__ bin_start,
-                           int32_t* __restrict__ link_up, int32_t* __restrict__ link_dn,
-                           uint32_t* __restrict__ owner) {
-  __shared__ int cand[2][A2_KEEP][3][A2_THREADS];   // [side][slot][dy, dz, id][thread]: a thread reads only its column
+                           int32_t* __restrict__ link_up, int32_t* __restrict__ link_dn) {
+  __shared__ int cand[2][A2_KEEP][3][A2_THREADS];   // [side][slot][dy, dz, position][thread]: a thread reads only its column
+  if (ctl->bad_offsets) return;
   const int sr = blockIdx.x;
   const int r = sr % g.n_rows;
   const uint32_t a = ro[sr], b = ro[sr + 1];
@@ -292,15 +285,14 @@ a2_neighbours_dense_kernel(const DevGeom g, const uint32_t* __restrict__ ro, con
   // gridDim.y CTAs share a row (dense rows hold thousands of clusters)
   for (uint32_t j = a + blockIdx.y * A2_THREADS + threadIdx.x; j < b; j += gridDim.y * A2_THREADS) {
     const int4 ch = srt[j];
-    const int yh = ch.x, zh = ch.y, hid = ch.z;
-    int best_u = -1, best_d = -1;
+    const int yh = ch.x, zh = ch.y;
+    Best b = {INT32_MAX, -1, -1};
     if (inner) {
       const Window w = window_bins(g, yh, zh, org_z);
-      int best_cost = INT32_MAX;
       const int nu = filter_side(g, srt, w, bs_u, yh, zh, col_u);
       const int nd = nu > 0 ? filter_side(g, srt, w, bs_d, yh, zh, col_d) : 0;
       if (nu > A2_KEEP || nd > A2_KEEP) {
-        pair_search_nested<FINE>(g, srt, w, bs_u, bs_d, yh, zh, best_cost, best_u, best_d);
+        pair_search_nested<FINE>(g, srt, w, bs_u, bs_d, yh, zh, b);
       } else {
         const int np = nu * nd;   // one flat loop over the pairs
         int iu = 0, id = 0;
@@ -309,20 +301,19 @@ a2_neighbours_dense_kernel(const DevGeom g, const uint32_t* __restrict__ ro, con
           const int* ed = col_d + id * 3 * A2_THREADS;
           const int ddy = eu[0] + ed[0], ddz = eu[A2_THREADS] + ed[A2_THREADS];
           const int cost = g.cost_wy * ddy * ddy + g.cost_wz * ddz * ddz;   // P8
-          const int idu = eu[2 * A2_THREADS], idd = ed[2 * A2_THREADS];
-          if (cost < best_cost || (cost == best_cost && (idu < best_u || (idu == best_u && idd < best_d)))) {   // P9
-            best_cost = cost;
-            best_u = idu;
-            best_d = idd;
+          const int pu = eu[2 * A2_THREADS], pd = ed[2 * A2_THREADS];
+          if (cost < b.cost || (cost == b.cost && tie_wins(srt, b, srt[pu].z, srt[pd].z))) {   // P9
+            b.cost = cost;
+            b.pu = pu;
+            b.pd = pd;
           }
           if (++id == nd) { id = 0; ++iu; }
         }
       }
-      if (best_u < 0 || best_cost > g.c_max) best_u = best_d = -1;   // P10
+      if (b.pu < 0 || b.cost > g.c_max) b.pu = b.pd = -1;   // P10
     }
-    link_up[hid] = best_u;
-    link_dn[hid] = best_d;
-    owner[hid] = 0u;   // a5 ownership words start empty
+    link_up[j] = b.pu;
+    link_dn[j] = b.pd;
   }
 }
 
@@ -335,7 +326,7 @@ cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64
   // z-bins narrower than the window
   const bool dense = (double)n > 0.75 * (double)R * (double)(t->g.ny * t->g.nz);
   const bool fine = t->g.shift_z < t->base_shift_z;
-#define A2_ARGS t->g, ro, t->s.srt, t->s.sec_key, t->s.bin_start, t->s.link_up, t->s.link_dn, t->s.owner
+#define A2_ARGS t->g, t->s.ctl, ro, t->s.srt, t->s.sec_key, t->s.bin_start, t->s.link_up, t->s.link_dn
   // dense rows: CTAs per row from the average row length (a longer row just loops)
   int64_t per_row = (n / R + A2_THREADS - 1) / A2_THREADS;
   per_row = per_row < 1 ? 1 : (per_row > 64 ? 64 : per_row);

@@ -32,16 +32,13 @@ enum : int { PH_IDLE = 0, PH_INIT, PH_A, PH_B, PH_CS, PH_CD, PH_FIN, PH_DONE };
 enum : int { M_NONE = 0, M_LINK, M_TABLE, M_SEARCH };
 
 constexpr int A4_THREADS = 128;   // warps never synchronise with each other after the geometry tables are loaded
-#ifndef TPC_A4_MIN_BLOCKS
-#define TPC_A4_MIN_BLOCKS 4   // 16 warps per SM: registers capped at 128 per thread (5 and 6 measured slower)
-#endif
-constexpr int A4_MIN_BLOCKS = TPC_A4_MIN_BLOCKS;
+constexpr int A4_MIN_BLOCKS = 4;   // 16 warps per SM: registers capped at 128 per thread (5 and 6 measured slower)
 
 __global__ void __launch_bounds__(A4_THREADS, A4_MIN_BLOCKS)
-a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restrict__ rec,
-                 const int4* __restrict__ srt, const uint32_t* __restrict__ sec_key,
-                 const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ seed_start,
-                 const int32_t* __restrict__ seed_sr, float4* __restrict__ tl_rec, int32_t* __restrict__ tl_hits,
+a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restrict__ srt,
+                 const uint32_t* __restrict__ sec_key, const uint32_t* __restrict__ bin_start,
+                 const int32_t* __restrict__ seed_pos, const int32_t* __restrict__ seed_sr,
+                 float4* __restrict__ tl_rec, int32_t* __restrict__ tl_hits, int2* __restrict__ tl_yz,
                  uint32_t* __restrict__ owner) {
   extern __shared__ double smem_a4[];
   const unsigned FULL = 0xffffffffu;
@@ -63,20 +60,21 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
 
   int phase = PH_IDLE;
   bool exhausted = false;
-  int i = -1, h = -1, y0 = 0, z0 = 0, sec_base = 0, r0 = 0, row = 0, nh = 0, miss = 0, lowest = 0, rmin = 0, rmax = 0;
+  int i = -1, sec_base = 0, r0 = 0, row = 0, nh = 0, miss = 0, lowest = 0, rmin = 0, rmax = 0;
+  bool more = false;   // the chain has a further hit (its record is in rcn)
   int org_z = 0;
   bool fail_dn = false;
   float chi2 = 0.f;
-  int32_t* tab = tl_hits;   // this tracklet's row -> hit table
+  int32_t* tab = tl_hits;   // this tracklet's row -> hit id table
+  int2* yz = tl_yz;         // and its row -> (y, z) stream for the downward refit
   State p;
   Cov C;
   p.y = p.z = p.s = p.t = p.q = 0; p.oy = p.oz = 0;
   cov_reset(g, C);
   // gathers issued one step ahead (a mismatch of the tag only costs the direct load)
-  int rcn_id = -1;                 // record of cluster rcn_id
-  Rec3 rcn = {0, 0, -1};
-  int t1_row = -1, t1_val = -1;    // table entries of the next two rows on the way down
-  int t2_row = -1, t2_val = -1;
+  Rec rcn = {0, 0, -1, -1};        // srt record of the next chain hit
+  int s1_row = -1, s1_y = YZ_NONE, s1_z = 0;   // stream entries of the next two rows on the way down
+  int s2_row = -1, s2_y = YZ_NONE, s2_z = 0;
   uint32_t pk_y = 0xFFFFFFFFu, pk_z = 0xFFFFFFFFu;   // bin ranges of the window keyed (pk_y, pk_z)
   BinRanges pq = {0, 0, 0, 0};
 
@@ -95,19 +93,19 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
       if (want && k < n_seeds) {
         // P19: state from the first two chain hits; the INIT step resets C and updates with the first hit
         i = (int)k;
-        h = seed_start[k];
+        const int h = seed_pos[k];
         const int sr = seed_sr[k];
         const int sec = sr / nr;
         sec_base = sec * nr;
         r0 = sr - sec_base;
         org_z = zmin_from_key(sec_key[sec]);
         tab = tl_hits + (size_t)k * nr;
-        const int4 c0 = rec[h];
-        const int4 c1 = rec[c0.z];
-        rcn_id = h;
-        rcn.y = c0.x; rcn.z = c0.y; rcn.up = c0.z;
-        y0 = c0.x;
-        z0 = c0.y;
+        yz = tl_yz + (size_t)k * ((nr + 3) & ~3);   // groups of four rows are 32-byte aligned (a4_phases.cu)
+        const int4 c0 = srt[h];
+        const int4 c1 = srt[c0.w];
+        rcn.y = c0.x; rcn.z = c0.y; rcn.id = c0.z; rcn.up = c0.w;
+        more = true;
+        const int y0 = c0.x, z0 = c0.y;
         const float dxr = s_row_dx[r0];
         const float dy = (float)(c1.x - y0) * g.inv_units, dz = (float)(c1.y - z0) * g.inv_units;
         const float ichord = rsqrtf(fmaf(dxr, dxr, dy * dy));
@@ -115,7 +113,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
         p.oy = y0; p.oz = z0;
         row = rmin = rmax = lowest = r0;
         nh = 0; miss = 0; chi2 = 0.f; fail_dn = false;
-        t1_row = t2_row = -1;
+        s1_row = s2_row = -1;
         pk_y = pk_z = 0xFFFFFFFFu;
         phase = PH_INIT;
       }
@@ -123,7 +121,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
     if (!__any_sync(FULL, phase != PH_IDLE)) break;
 
     // ---- phase transitions that need no work ----
-    if (phase == PH_A && h < 0) phase = PH_B;                                                      // chain ended
+    if (phase == PH_A && !more) phase = PH_B;                                                      // chain ended
     if (phase == PH_B && !(row + 1 < nr && miss < g.max_miss)) phase = PH_CS;                      // P20
     if (phase == PH_CD && (row == 0 || (row - 1 < r0 && miss >= g.max_miss))) phase = PH_FIN;      // P20
     const int ph = phase;
@@ -148,35 +146,28 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
     }
 
     // ---- hit known before the transport (chain link or recorded hit) ----
-    int hid = -1;
-    if (mode == M_LINK) hid = h;
-    int nid = -1;   // hit whose record the next step will want
-    if (mode == M_TABLE) {
-      // rolling two-deep pipeline over the table on the way down: t1 = entry of this row, t2 = of the next
-      if (t1_row != trow) {
-        t1_val = -1;
-        ld_cg_s32_if(t1_val, tab + trow, true);
-      }
-      hid = t1_val;
-      const int n1 = trow - 1, n2 = trow - 2;
-      const bool have1 = t2_row == n1;
-      t1_val = t2_val;
-      t1_row = n1;
-      if (have1) nid = t1_val;   // loaded in an earlier step: safe to consume without waiting
-      ld_cg_s32_if(t1_val, tab + n1, !have1 && n1 >= r0);
-      if (n1 < r0) t1_row = -1;
-      t2_row = n2 >= r0 ? n2 : -1;
-      ld_cg_s32_if(t2_val, tab + n2, n2 >= r0);
+    int hid = -1, hy = YZ_NONE, hz = 0;
+    const Rec rc = rcn;
+    if (mode == M_LINK) {
+      hid = rc.id;
+      hy = rc.y;
+      hz = rc.z;
     }
-    Rec3 rc = rcn;
-    if (hid < 0) { rc.y = y0; rc.z = z0; rc.up = -1; }
-    ld_rec_if(rc, rec + hid, hid >= 0 && hid != rcn_id);
-    // next step's record: the chain's next hit, or the recorded hit of the next row down
-    if (mode == M_LINK) nid = rc.up;
-    {
-      const bool fetch = nid >= 0 && nid != rcn_id;
-      if (fetch) rcn_id = nid;
-      ld_rec_if(rcn, rec + nid, fetch);
+    ld_rec_if(rcn, srt + rc.up, mode == M_LINK && rc.up >= 0);   // the next chain hit, one step ahead
+    if (mode == M_TABLE) {
+      // rolling two-deep pipeline over the tracklet's (y, z) stream on the way down
+      ld_cg_yz_if(s1_y, s1_z, yz + trow, s1_row != trow);
+      hy = s1_y;
+      hz = s1_z;
+      hid = hy != YZ_NONE ? 0 : -1;   // the id is not needed on the way down
+      const int n1 = trow - 1, n2 = trow - 2;
+      const bool have1 = s2_row == n1;
+      s1_y = s2_y;
+      s1_z = s2_z;
+      s1_row = n1 >= r0 ? n1 : -1;
+      ld_cg_yz_if(s1_y, s1_z, yz + n1, !have1 && n1 >= r0);
+      s2_row = n2 >= r0 ? n2 : -1;
+      ld_cg_yz_if(s2_y, s2_z, yz + n2, n2 >= r0);
     }
     // candidates of this step's search: their bin ranges were loaded during the last step; touch them now
     const uint32_t* bs = bin_start + (size_t)(sec_base + trow) * g.nb_stride;
@@ -209,13 +200,14 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
     if (ok && tr) ok = transport<true>(g, dx, p, C);
     if (ok) {
       row = trow;
-      float ym = resid_y(g, p, rc.y), zm = resid_z(g, p, rc.z);   // residuals of the hit, cm
+      float ym = resid_y(g, p, hy), zm = resid_z(g, p, hz);   // residuals of the hit, cm
       if (mode == M_SEARCH) {
         const float vy = C.var_y() + g.sy2, vz = C.var_z() + g.sz2;
         const Window w = search_window(g, p.y, p.z, vy, vz, p.oy, p.oz, org_z);
         Found f;
         f.id = -1;
         f.ry = f.rz = 0.f;
+        f.hy = f.hz = 0;
         float bestd = __int_as_float(0x7f800000);
         const float wy = 1.f / vy, wz = 1.f / vz;
         if (w.iz_hi <= w.iz_lo + 1) {   // always so on the coarse grid (bins >= 2 gate_z wide)
@@ -237,6 +229,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
         ym = f.ry;
         zm = f.rz;
         tab[row] = hid;
+        if (ph == PH_B) yz[row] = make_int2(hid >= 0 ? f.hy : YZ_NONE, f.hz);
         rmin = min(rmin, row);
         rmax = max(rmax, row);
         if (hid >= 0) {
@@ -248,9 +241,10 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
         }
       } else if (mode == M_LINK) {
         tab[row] = hid;
+        yz[row] = make_int2(hy, hz);
         rmax = row;
         ++nh;
-        h = rc.up;
+        more = rc.up >= 0;
       }
       if (mode != M_NONE && hid >= 0) chi2 += update(g, p, C, ym, zm);
       if (ph == PH_INIT) phase = PH_A;
@@ -330,7 +324,7 @@ cudaError_t setup_a4_attributes(tpc_tracker* t) {
 cudaError_t launch_a4_follow(const tpc_tracker* t, int64_t n, cudaStream_t st) {
   if (n == 0 || t->s_cap == 0) return cudaSuccess;
   a4_follow_kernel<<<t->a4_blocks, A4_THREADS, a4_smem_bytes(t->g), st>>>(
-      t->g, t->s.ctl, t->s.rec, t->s.srt, t->s.sec_key, t->s.bin_start, t->s.seed_start, t->s.seed_sr, t->s.tl_rec,
-      t->s.tl_hits, t->s.owner);
+      t->g, t->s.ctl, t->s.srt, t->s.sec_key, t->s.bin_start, t->s.seed_pos, t->s.seed_sr, t->s.tl_rec, t->s.tl_hits,
+      t->s.tl_yz, t->s.owner);
   return cudaGetLastError();
 }

@@ -13,51 +13,53 @@
 namespace {
 
 constexpr int AP_THREADS = 128;
-#ifndef TPC_A4_REFILL_MIN
-#define TPC_A4_REFILL_MIN 8
-#endif
-constexpr int A4_REFILL_MIN = TPC_A4_REFILL_MIN;
+constexpr int A4_REFILL_MIN = 8;   // free lanes a warp collects before it refills (4: +2 % a4 time, 16: equal)
 enum : int { Q_B = 0, Q_C = 1, Q_D = 2 };
 
 struct Env {   // everything a warp needs that does not change during a kernel
   DevGeom g;
   DevCtl* ctl;
-  const int4* rec;
   const int4* srt;
   const uint32_t* sec_key;
   const uint32_t* bin_start;
-  const int32_t* seed_start;
+  const int32_t* seed_pos;
   const int32_t* seed_sr;
   float4* tl_rec;
   int32_t* tl_hits;
+  int2* tl_yz;
   int4* tl_state;
   uint32_t* q_items;
   uint32_t* tl_span;
   const double* s_row_x;   // shared-memory copies
   const float* s_row_dx;
+  int2* s_yz;              // this lane's staging column for the (y, z) stream: slot k at s_yz[k * AP_THREADS]
+  int yz_stride;           // entries per tracklet in tl_yz: n_rows rounded up to a multiple of 4 (32-byte groups)
   uint32_t n_seeds, s_cap;
   int lane, lanes_used;
 };
 
 struct Trk {   // per-tracklet constants, recomputed from the seed rank when a lane picks the tracklet up
-  int i, h0, y0, z0, up0, sec_base, r0, org_z;   // (y0, z0): the first cluster, the state's origin at pick-up
-  int32_t* tab;   // its row -> hit table = its final hit list
+  int i, id0, y0, z0, up0, sec_base, r0, org_z;   // (y0, z0, id0, up0): the seed's first cluster (its srt record)
+  int32_t* tab;   // its row -> hit id table = its final hit list
+  int2* yz;       // its row -> (y, z) of the recorded hit: what the downward refit streams
 };
 
 __device__ __forceinline__ Trk trk_of(const Env& e, int i) {
   Trk t;
   t.i = i;
-  t.h0 = e.seed_start[i];
+  const int h0 = e.seed_pos[i];
   const int sr = e.seed_sr[i];
   const int sec = sr / e.g.n_rows;
   t.sec_base = sec * e.g.n_rows;
   t.r0 = sr - t.sec_base;
   t.org_z = zmin_from_key(e.sec_key[sec]);
   t.tab = e.tl_hits + (size_t)i * e.g.n_rows;
-  const int4 c0 = e.rec[t.h0];
+  t.yz = e.tl_yz + (size_t)i * e.yz_stride;
+  const int4 c0 = e.srt[h0];
   t.y0 = c0.x;
   t.z0 = c0.y;
-  t.up0 = c0.z;
+  t.id0 = c0.z;
+  t.up0 = c0.w;
   return t;
 }
 
@@ -91,7 +93,8 @@ __device__ __forceinline__ void state_load(const Env& e, int i, Trk& t, State& p
   t.r0 = o.z - t.sec_base;
   t.org_z = o.w;
   t.tab = e.tl_hits + (size_t)i * e.g.n_rows;
-  t.h0 = t.up0 = -1;
+  t.yz = e.tl_yz + (size_t)i * e.yz_stride;
+  t.id0 = t.up0 = -1;
   C.d0 = f0.x; C.d1 = f0.y; C.d2 = f0.z; C.d3 = f0.w; C.d4 = f1.x; C.u01 = f1.y; C.u02 = f1.z; C.u03 = f1.w;
   C.u04 = f2.x; C.u12 = f2.y; C.u13 = f2.z; C.u14 = f2.w; C.u23 = f3.x; C.u24 = f3.y; C.u34 = f3.z;
   p.y = f3.w; p.z = f4.x; p.s = f4.y; p.t = f4.z; p.q = f4.w;
@@ -152,6 +155,27 @@ __device__ __forceinline__ int queue_pop(const Env& e, int q, unsigned want, boo
   return i;
 }
 
+// The (y, z) stream of a tracklet (tl_yz) is written through a four-row staging column in shared memory, one
+// aligned 32-byte group per store: single 8-byte stores made the two upward phases ~25 % slower, because every
+// partially written sector is first filled from DRAM (measured: +9 B of DRAM reads per step).  A group may carry
+// stale slots for rows the phase did not visit: rows below the seed's first row and above the last visited row
+// are never read (phase C runs from the last visited row down to the seed's first row).
+__device__ __forceinline__ void yz_stage(const Env& e, int row, int y, int z) {
+  e.s_yz[(row & 3) * AP_THREADS] = make_int2(y, z);
+}
+// rows [first, row] of the group of `row` are staged; rows below `first` belong to an earlier phase and must stay
+__device__ __forceinline__ void yz_flush(const Env& e, const Trk& t, int row, int first) {
+  const int base = row & ~3;
+  if (base >= first) {
+    const int2 v0 = e.s_yz[0], v1 = e.s_yz[AP_THREADS], v2 = e.s_yz[2 * AP_THREADS], v3 = e.s_yz[3 * AP_THREADS];
+    int4* dst = (int4*)(t.yz + base);
+    dst[0] = make_int4(v0.x, v0.y, v1.x, v1.y);
+    dst[1] = make_int4(v2.x, v2.y, v3.x, v3.y);
+  } else {
+    for (int r = first; r <= row; ++r) t.yz[r] = e.s_yz[(r & 3) * AP_THREADS];
+  }
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 // Phase A: P19 initial state + fit up the seed chain, no gate.  Items = seed ranks from ctl->next_seed.
 // ---------------------------------------------------------------------------------------------------------------
@@ -165,8 +189,9 @@ __device__ __forceinline__ void phase_a(const Env& e) {
   Cov C;
   p.y = p.z = p.s = p.t = p.q = 0; p.oy = p.oz = 0;
   cov_reset(g, C);
-  int h = -1;
-  Rec3 rcn = {0, 0, -1};
+  Rec rcn = {0, 0, -1, -1};   // the chain hit of the next step (requested one step ahead)
+  bool more = false;          // rcn holds a chain hit
+  bool dirty = false;         // the staging column holds rows that are not in tl_yz yet
   while (true) {
     const bool want = !live && e.lane < e.lanes_used && !exhausted;
     const unsigned idle = __ballot_sync(FULL, want);
@@ -179,9 +204,9 @@ __device__ __forceinline__ void phase_a(const Env& e) {
       const uint32_t k = base + (uint32_t)__popc(idle & ((1u << e.lane) - 1u));
       if (want && k < e.n_seeds) {
         t = trk_of(e, (int)k);
-        h = t.h0;
-        const int4 c1 = e.rec[t.up0];
-        rcn.y = t.y0; rcn.z = t.z0; rcn.up = t.up0;
+        const int4 c1 = e.srt[t.up0];
+        rcn.y = t.y0; rcn.z = t.z0; rcn.id = t.id0; rcn.up = t.up0;
+        more = true;
         const float dxr = e.s_row_dx[t.r0];
         const float dy = (float)(c1.x - t.y0) * g.inv_units, dz = (float)(c1.y - t.z0) * g.inv_units;
         const float ichord = rsqrtf(fmaf(dxr, dxr, dy * dy));
@@ -199,22 +224,27 @@ __device__ __forceinline__ void phase_a(const Env& e) {
     const bool tr = live && !first;
     const int trow = b.row + (tr ? 1 : 0);
     const float dx = e.s_row_dx[b.row];
-    const int hid = h;
-    const Rec3 rc = rcn;
-    ld_rec_if(rcn, e.rec + rc.up, live && rc.up >= 0);   // the next chain hit, one step ahead
+    const Rec rc = rcn;
+    ld_rec_if(rcn, e.srt + rc.up, live && rc.up >= 0);   // the next chain hit, one step ahead
     bool ok = live;
     if (tr) ok = transport<true>(g, dx, p, C);
     if (ok) {
       b.row = trow;
       update(g, p, C, resid_y(g, p, rc.y), resid_z(g, p, rc.z));
-      t.tab[trow] = hid;
+      t.tab[trow] = rc.id;
+      yz_stage(e, trow, rc.y, rc.z);
+      dirty = true;
       b.rmax = trow;
       ++b.nh;
-      h = rc.up;
+      more = rc.up >= 0;
       first = false;
     }
     // the chain ended, or the transport failed (P18; then phase B is skipped)
-    const bool leave = live && (!ok || h < 0);
+    const bool leave = live && (!ok || !more);
+    if (dirty && ((b.row & 3) == 3 || leave)) {
+      yz_flush(e, t, b.row, 0);   // rows of the group below the seed's first row are never read: whole groups
+      dirty = false;
+    }
     if (leave) state_save(e, t, p, C, b);
     const bool to_b = leave && ok && b.row + 1 < g.n_rows;
     queue_push(e, Q_B, len_bucket(g.n_rows - 1 - b.row, g.n_rows), t.i, to_b);
@@ -234,6 +264,7 @@ __device__ __forceinline__ Found search_step(const Env& e, const Trk& t, const S
   Found f;
   f.id = -1;
   f.ry = f.rz = 0.f;
+  f.hy = f.hz = 0;
   float bestd = __int_as_float(0x7f800000);
   const float wy = 1.f / vy, wz = 1.f / vz;
   if (w.iz_hi <= w.iz_lo + 1) {   // always so on the coarse grid
@@ -288,6 +319,8 @@ __device__ __forceinline__ void phase_b(const Env& e) {
   cov_reset(g, C);
   uint32_t pk_y = 0xFFFFFFFFu, pk_z = 0xFFFFFFFFu;
   BinRanges pq = {0, 0, 0, 0};
+  int fr = 0;           // first row this phase visits for the tracklet (the rows below are phase A's)
+  bool dirty = false;   // the staging column holds rows that are not in tl_yz yet
   while (true) {
     const bool want = !live && e.lane < e.lanes_used && !dry;
     const unsigned idle = __ballot_sync(FULL, want);
@@ -297,6 +330,7 @@ __device__ __forceinline__ void phase_b(const Env& e) {
       if (i >= 0) {
         state_load(e, i, t, p, C, b);
         pk_y = pk_z = 0xFFFFFFFFu;
+        fr = b.row + 1;
         live = true;
       }
     }
@@ -317,6 +351,8 @@ __device__ __forceinline__ void phase_b(const Env& e) {
       b.row = trow;
       const Found f = search_step(e, t, p, C, trow, pk_y, pk_z, pq);
       t.tab[trow] = f.id;
+      yz_stage(e, trow, f.id >= 0 ? f.hy : YZ_NONE, f.hz);
+      dirty = true;
       b.rmax = trow;
       if (f.id >= 0) {
         update(g, p, C, f.ry, f.rz);
@@ -330,6 +366,10 @@ __device__ __forceinline__ void phase_b(const Env& e) {
     pk_z = nk_z;
     pq = nq;
     const bool leave = live && (!ok || !(b.row + 1 < g.n_rows && b.miss < g.max_miss));   // P18, P20
+    if (dirty && ((b.row & 3) == 3 || leave)) {
+      yz_flush(e, t, b.row, fr);
+      dirty = false;
+    }
     if (leave) state_save(e, t, p, C, b);
     queue_push(e, Q_C, len_bucket(b.row - t.r0, g.n_rows), t.i, leave);
     if (leave) live = false;
@@ -338,8 +378,9 @@ __device__ __forceinline__ void phase_b(const Env& e) {
 
 // ---------------------------------------------------------------------------------------------------------------
 // Phase C: covariance reset (P22), then refit down over the recorded hits to the seed's first row.  The first step
-// of a tracklet (reset + update with the top row's hit) has no transport.  Table entries of the next two rows and
-// the record of the next hit are requested one step ahead.
+// of a tracklet (reset + update with the top row's hit) has no transport.  The hits come from the tracklet's own
+// (y, z) stream, written row by row on the way up: one sequential 8-byte load per step, requested two rows ahead --
+// no gather by cluster id, no table look-up.
 // ---------------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void phase_c(const Env& e) {
   const unsigned FULL = 0xffffffffu;
@@ -352,9 +393,8 @@ __device__ __forceinline__ void phase_c(const Env& e) {
   Cov C;
   p.y = p.z = p.s = p.t = p.q = 0; p.oy = p.oz = 0;
   cov_reset(g, C);
-  int t1_row = -1, t1_val = -1, t2_row = -1, t2_val = -1;   // table entries of this step's row and the one below
-  int rcn_id = -1;
-  Rec3 rcn = {0, 0, -1};
+  int s1_row = -1, s1_y = YZ_NONE, s1_z = 0;   // stream entries of this step's row and of the one below
+  int s2_row = -1, s2_y = YZ_NONE, s2_z = 0;
   while (true) {
     const bool want = !live && e.lane < e.lanes_used && !dry;
     const unsigned idle = __ballot_sync(FULL, want);
@@ -363,8 +403,7 @@ __device__ __forceinline__ void phase_c(const Env& e) {
       const int i = queue_pop(e, Q_C, idle, want, &bk, &dry);
       if (i >= 0) {
         state_load(e, i, t, p, C, b);
-        t1_row = t2_row = -1;
-        rcn_id = -1;
+        s1_row = s2_row = -1;
         first = true;
         live = true;
       }
@@ -380,36 +419,25 @@ __device__ __forceinline__ void phase_c(const Env& e) {
     const bool tr = live && !first;
     const int trow = b.row - (tr ? 1 : 0);
     const float dx = -e.s_row_dx[max(b.row - 1, 0)];
-    int hid = -1, nid = -1;
-    if (live) {   // rolling two-deep pipeline over the table on the way down
-      if (t1_row != trow) {
-        t1_val = -1;
-        ld_cg_s32_if(t1_val, t.tab + trow, true);
-      }
-      hid = t1_val;
+    int hy = YZ_NONE, hz = 0;
+    if (live) {   // rolling two-deep pipeline over the stream on the way down
+      ld_cg_yz_if(s1_y, s1_z, t.yz + trow, s1_row != trow);
+      hy = s1_y;
+      hz = s1_z;
       const int n1 = trow - 1, n2 = trow - 2;
-      const bool have1 = t2_row == n1;
-      t1_val = t2_val;
-      t1_row = n1;
-      if (have1) nid = t1_val;   // loaded in an earlier step: safe to consume without waiting
-      ld_cg_s32_if(t1_val, t.tab + n1, !have1 && n1 >= t.r0);
-      if (n1 < t.r0) t1_row = -1;
-      t2_row = n2 >= t.r0 ? n2 : -1;
-      ld_cg_s32_if(t2_val, t.tab + n2, n2 >= t.r0);
-    }
-    Rec3 rc = rcn;
-    if (hid < 0) { rc.y = t.y0; rc.z = t.z0; rc.up = -1; }
-    ld_rec_if(rc, e.rec + hid, hid >= 0 && hid != rcn_id);
-    {
-      const bool fetch = nid >= 0 && nid != rcn_id;
-      if (fetch) rcn_id = nid;
-      ld_rec_if(rcn, e.rec + nid, fetch);
+      const bool have1 = s2_row == n1;
+      s1_y = s2_y;
+      s1_z = s2_z;
+      s1_row = n1 >= t.r0 ? n1 : -1;
+      ld_cg_yz_if(s1_y, s1_z, t.yz + n1, !have1 && n1 >= t.r0);
+      s2_row = n2 >= t.r0 ? n2 : -1;
+      ld_cg_yz_if(s2_y, s2_z, t.yz + n2, n2 >= t.r0);
     }
     bool ok = live;
     if (tr) ok = transport<true>(g, dx, p, C);
     if (ok) {
       b.row = trow;
-      if (hid >= 0) b.chi2 += update(g, p, C, resid_y(g, p, rc.y), resid_z(g, p, rc.z));
+      if (hy != YZ_NONE) b.chi2 += update(g, p, C, resid_y(g, p, hy), resid_z(g, p, hz));
       first = false;
     } else if (live) {
       b.fail_dn = true;   // P18: the state stays at the row where it stopped
@@ -542,18 +570,20 @@ a4_votes_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, const float4* _
   }
 }
 
-// Resident CTAs per SM: the refit phase fits 96 registers without spilling, so it runs at 20 warps per SM; the
-// other three need the full 128 (16 warps).
-constexpr int ap_min_blocks(int ph) { return ph == 2 ? 5 : 4; }
+// Resident CTAs per SM (measured, profiles/r02_a4_occupancy.md): the three phases that gather clusters run best at
+// 16 warps per SM -- at 20 or 24 they are slower, at 12 equal, at 8 slower: they sit between gather latency and the
+// DRAM's random-sector rate -- while the refit phase streams its measurements and gains up to 28 warps.
+constexpr int ap_min_blocks(int ph) { return ph == 2 ? 7 : 4; }
 
 template <int PH>
 __global__ void __launch_bounds__(AP_THREADS, ap_min_blocks(PH))
-a4_phase_kernel(const DevGeom g, uint32_t s_cap, DevCtl* __restrict__ ctl, const int4* __restrict__ rec,
-                const int4* __restrict__ srt, const uint32_t* __restrict__ sec_key,
-                const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ seed_start,
-                const int32_t* __restrict__ seed_sr, float4* __restrict__ tl_rec, int32_t* __restrict__ tl_hits,
+a4_phase_kernel(const DevGeom g, uint32_t s_cap, DevCtl* __restrict__ ctl, const int4* __restrict__ srt,
+                const uint32_t* __restrict__ sec_key, const uint32_t* __restrict__ bin_start,
+                const int32_t* __restrict__ seed_pos, const int32_t* __restrict__ seed_sr,
+                float4* __restrict__ tl_rec, int32_t* __restrict__ tl_hits, int2* __restrict__ tl_yz,
                 int4* __restrict__ tl_state, uint32_t* __restrict__ q_items, uint32_t* __restrict__ tl_span) {
   extern __shared__ double smem_ap[];
+  __shared__ int2 s_yz[4][AP_THREADS];
   const int nr = g.n_rows;
   const uint32_t n_seeds = ctl->n_seeds;
   if (n_seeds == 0) return;
@@ -566,10 +596,13 @@ a4_phase_kernel(const DevGeom g, uint32_t s_cap, DevCtl* __restrict__ ctl, const
   __syncthreads();
   Env e;
   e.g = g;
-  e.ctl = ctl; e.rec = rec; e.srt = srt; e.sec_key = sec_key; e.bin_start = bin_start;
-  e.seed_start = seed_start; e.seed_sr = seed_sr; e.tl_rec = tl_rec; e.tl_hits = tl_hits; e.tl_state = tl_state;
+  e.ctl = ctl; e.srt = srt; e.sec_key = sec_key; e.bin_start = bin_start;
+  e.seed_pos = seed_pos; e.seed_sr = seed_sr; e.tl_rec = tl_rec; e.tl_hits = tl_hits; e.tl_yz = tl_yz;
+  e.tl_state = tl_state;
   e.q_items = q_items; e.tl_span = tl_span; e.s_row_x = s_row_x; e.s_row_dx = s_row_dx;
   e.n_seeds = n_seeds; e.s_cap = s_cap;
+  e.s_yz = &s_yz[0][threadIdx.x];
+  e.yz_stride = (nr + 3) & ~3;
   e.lane = threadIdx.x & 31;
   // few seeds (one small event): spread them over all warps instead of filling the first warps' 32 lanes
   const uint32_t n_warps = gridDim.x * (blockDim.x >> 5);
@@ -587,13 +620,13 @@ cudaError_t launch_a4_phases(const tpc_tracker* t, int64_t n, cudaStream_t st) {
   const size_t smem = (size_t)t->g.n_rows * (8 + 4);
 #define AP_LAUNCH(PH)                                                                                         \
   a4_phase_kernel<PH><<<t->a4_sms * ap_min_blocks(PH), AP_THREADS, smem, st>>>(                                                \
-      t->g, (uint32_t)t->s_cap, t->s.ctl, t->s.rec, t->s.srt, t->s.sec_key, t->s.bin_start, t->s.seed_start, \
-      t->s.seed_sr, t->s.tl_rec, t->s.tl_hits, t->s.tl_state, t->s.q_items, t->s.tl_span)
+      t->g, (uint32_t)t->s_cap, t->s.ctl, t->s.srt, t->s.sec_key, t->s.bin_start, t->s.seed_pos, t->s.seed_sr, \
+      t->s.tl_rec, t->s.tl_hits, t->s.tl_yz, t->s.tl_state, t->s.q_items, t->s.tl_span)
   AP_LAUNCH(0);
   AP_LAUNCH(1);
   AP_LAUNCH(2);
   AP_LAUNCH(3);
 #undef AP_LAUNCH
-  a4_votes_kernel<<<148 * 64, 256, 0, st>>>(t->g, t->s.ctl, t->s.tl_rec, t->s.tl_span, t->s.tl_hits, t->s.owner);
+  a4_votes_kernel<<<t->a4_sms * 64, 256, 0, st>>>(t->g, t->s.ctl, t->s.tl_rec, t->s.tl_span, t->s.tl_hits, t->s.owner);
   return cudaGetLastError();
 }

@@ -10,6 +10,7 @@ __device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? l
 
 struct Found {
   int id;
+  int hy, hz;     // its fixed-point coordinates
   float ry, rz;   // residuals (hit - state) of the accepted hit, cm
 };
 
@@ -66,13 +67,18 @@ __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefe
 // for the load right there -- which would turn every gather that is issued one step ahead into a blocking one.
 // (y, z, up link) of a cluster record as three scalar loads: a predicated 128-bit load needs an aligned register
 // quad, which ptxas then copies out of right behind the load (and so waits for it); scalars land in place.
-struct Rec3 {
-  int y, z, up;
+struct Rec {   // an srt record: (y, z, cluster id, cleaned up link as a sorted position)
+  int y, z, id, up;
 };
-__device__ __forceinline__ void ld_rec_if(Rec3& v, const int4* p, bool pred) {
-  asm volatile("{ .reg .pred q; setp.ne.s32 q, %3, 0; @q ld.global.nc.s32 %0, [%4]; @q ld.global.nc.s32 %1, [%4+4];"
-               " @q ld.global.nc.s32 %2, [%4+8]; }"
-               : "+r"(v.y), "+r"(v.z), "+r"(v.up) : "r"((int)pred), "l"(p));
+__device__ __forceinline__ void ld_rec_if(Rec& v, const int4* p, bool pred) {
+  asm volatile("{ .reg .pred q; setp.ne.s32 q, %4, 0; @q ld.global.nc.s32 %0, [%5]; @q ld.global.nc.s32 %1, [%5+4];"
+               " @q ld.global.nc.s32 %2, [%5+8]; @q ld.global.nc.s32 %3, [%5+12]; }"
+               : "+r"(v.y), "+r"(v.z), "+r"(v.id), "+r"(v.up) : "r"((int)pred), "l"(p));
+}
+// (y, z) of a recorded hit out of the tracklet's own stream (written by this call's upward pass: read through L2)
+__device__ __forceinline__ void ld_cg_yz_if(int& y, int& z, const int2* p, bool pred) {
+  asm volatile("{ .reg .pred q; setp.ne.s32 q, %2, 0; @q ld.global.cg.v2.s32 {%0, %1}, [%3]; }"
+               : "+r"(y), "+r"(z) : "r"((int)pred), "l"(p) : "memory");
 }
 __device__ __forceinline__ void ld_u32_if(uint32_t& v, const uint32_t* p, bool pred) {
   asm volatile("{ .reg .pred q; setp.ne.s32 q, %1, 0; @q ld.global.nc.u32 %0, [%2]; }" : "+r"(v) : "r"((int)pred), "l"(p));
@@ -110,6 +116,8 @@ __device__ __forceinline__ void search_ranges(const DevGeom& g, const BinRanges&
       if (d < bestd || (d == bestd && c.z < f.id)) {
         bestd = d;
         f.id = c.z;
+        f.hy = c.x;
+        f.hz = c.y;
         f.ry = dy;
         f.rz = dz;
       }

@@ -35,11 +35,13 @@ a5_select_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int32_t* __res
   const unsigned FULL = 0xffffffffu;
   const uint32_t n_seeds = ctl->n_seeds;
   const uint32_t n_tiles = (n_seeds + A5_TILE - 1) / A5_TILE;
+  const uint32_t seed_flags = (ctl->n_seeds_found > n_seeds ? TPC_FLAG_SEED_OVERFLOW : 0u) |
+                              (ctl->bad_offsets ? TPC_FLAG_BAD_OFFSETS : 0u);
   if (n_seeds == 0) {
     if (blockIdx.x == 0 && threadIdx.x == 0) {
       counts[0] = 0;
       counts[1] = 0;
-      counts[2] = 0;
+      counts[2] = (int32_t)seed_flags;
       counts[3] = 0;
     }
     return;
@@ -156,9 +158,9 @@ a5_select_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int32_t* __res
     const uint32_t nt = excl[0] + tot_k, nhits = excl[1] + tot_h;
     counts[0] = (int32_t)nt;
     counts[1] = (int32_t)nhits;
-    counts[2] = (nt > (uint32_t)track_capacity ? TPC_FLAG_TRACK_OVERFLOW : 0u) |
-                (nhits > (uint32_t)hit_capacity ? TPC_FLAG_HIT_OVERFLOW : 0u);
-    counts[3] = (int32_t)n_seeds;
+    counts[2] = (int32_t)((nt > (uint32_t)track_capacity ? TPC_FLAG_TRACK_OVERFLOW : 0u) |
+                          (nhits > (uint32_t)hit_capacity ? TPC_FLAG_HIT_OVERFLOW : 0u) | seed_flags);
+    counts[3] = (int32_t)ctl->n_seeds_found;
   }
 }
 

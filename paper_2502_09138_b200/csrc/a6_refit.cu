@@ -8,7 +8,7 @@
 //
 // Same execution model as a4: persistent warps, one lane per track, lanes refill from a device counter, one
 // uniform step (optional covariance reset, optional transport, update) for both passes; fp32 state relative to
-// the first hit, fp32 U D U^T covariance (kalman.cuh).  The hit's (y, z) comes from the a3 records of the same call (rec[id]), requested
+// the first hit, fp32 U D U^T covariance (kalman.cuh).  The hit's (y, z) comes from the caller's cluster arrays (y[id], z[id]), requested
 // one step ahead; its row from the row list a5 wrote next to the hit list.
 #include "tpc_internal.cuh"
 #include "kalman.cuh"
@@ -20,14 +20,14 @@ constexpr int A6_THREADS = 128;
 enum : int { R_IDLE = 0, R_FIRST, R_UP, R_TOP, R_DOWN };
 
 // Predicated loads straight into their destination registers (see a4_follow.cu for why they are PTX).
-__device__ __forceinline__ void ld_yz_if(int& y, int& z, const int4* p, bool pred) {
-  asm volatile("{ .reg .pred q; setp.ne.s32 q, %2, 0; @q ld.global.nc.s32 %0, [%3]; @q ld.global.nc.s32 %1, [%3+4]; }"
-               : "+r"(y), "+r"(z) : "r"((int)pred), "l"(p));
+__device__ __forceinline__ void ld_yz_if(int& y, int& z, const int32_t* py, const int32_t* pz, bool pred) {
+  asm volatile("{ .reg .pred q; setp.ne.s32 q, %2, 0; @q ld.global.nc.s32 %0, [%3]; @q ld.global.nc.s32 %1, [%4]; }"
+               : "+r"(y), "+r"(z) : "r"((int)pred), "l"(py), "l"(pz));
 }
 
 __global__ void __launch_bounds__(A6_THREADS, 4)
-a6_refit_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restrict__ rec,
-                const uint8_t* __restrict__ hit_row, const tpc_track_rec_t* __restrict__ tracks,
+a6_refit_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int32_t* __restrict__ cy_in,
+                const int32_t* __restrict__ cz_in, const uint8_t* __restrict__ hit_row, const tpc_track_rec_t* __restrict__ tracks,
                 int32_t track_capacity, const int32_t* __restrict__ hit_ids, int32_t hit_capacity,
                 const int32_t* __restrict__ counts, tpc_track_rec_t* __restrict__ out) {
   extern __shared__ double s_row_x[];
@@ -69,16 +69,15 @@ a6_refit_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restric
         hl = hit_ids + t->hit_offset;
         hr = hit_row + t->hit_offset;
         row = hr[0];
-        const int4 c0 = rec[hl[0]];
-        y0 = c0.x;
-        z0 = c0.y;
+        y0 = cy_in[hl[0]];
+        z0 = cz_in[hl[0]];
         pf_j = 0; pf_y = y0; pf_z = z0;
         p.y = 0; p.z = 0; p.s = 0; p.t = 0; p.q = 0;
         p.oy = y0; p.oz = z0;
         if (m >= 2) {   // P19 with the gap to the second owned hit
-          const int4 c1 = rec[hl[1]];
+          const int y1 = cy_in[hl[1]], z1 = cz_in[hl[1]];
           const float dxr = (float)(s_row_x[hr[1]] - s_row_x[row]);
-          const float dy = (float)(c1.x - y0) * g.inv_units, dz = (float)(c1.y - z0) * g.inv_units;
+          const float dy = (float)(y1 - y0) * g.inv_units, dz = (float)(z1 - z0) * g.inv_units;
           const float ichord = rsqrtf(fmaf(dxr, dxr, dy * dy));
           p.s = dy * ichord;
           p.t = dz * ichord;
@@ -99,7 +98,7 @@ a6_refit_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restric
     int trow = row, cy = pf_y, cz = pf_z;
     if (active) {
       trow = hr[j];
-      ld_yz_if(cy, cz, rec + hl[j], pf_j != j);   // not requested ahead (after a pass ended early): load now
+      ld_yz_if(cy, cz, cy_in + hl[j], cz_in + hl[j], pf_j != j);   // not requested ahead (after a pass ended early): load now
     }
     // the hit of the next step: its record is requested now and used then
     {
@@ -111,7 +110,7 @@ a6_refit_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restric
       int hn = 0;
       if (fetch) hn = hl[jn];
       if (fetch) pf_j = jn;
-      ld_yz_if(pf_y, pf_z, rec + hn, fetch);
+      ld_yz_if(pf_y, pf_z, cy_in + hn, cz_in + hn, fetch);
     }
     if (active && reset) cov_reset(g, C);
     if (ph == R_TOP) { chi2 = 0.f; used = 0; }
@@ -151,13 +150,13 @@ a6_refit_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restric
 
 }  // namespace
 
-cudaError_t launch_a6_refit(const tpc_tracker* t, const uint32_t* ro, const tpc_tracks_out_t* tracks,
+cudaError_t launch_a6_refit(const tpc_tracker* t, const int32_t* y, const int32_t* z, const tpc_tracks_out_t* tracks,
                             tpc_track_rec_t* refit_out, cudaStream_t st) {
   if (t->last_n == 0 || t->a4_blocks == 0 || tracks->track_capacity == 0) return cudaSuccess;
   cudaError_t e = cudaMemsetAsync(&t->s.ctl->next_track, 0, sizeof(uint32_t), st);
   if (e != cudaSuccess) return e;
   a6_refit_kernel<<<t->a4_blocks, A6_THREADS, (size_t)t->g.n_rows * sizeof(double), st>>>(
-      t->g, t->s.ctl, t->s.rec, t->s.hit_row, tracks->tracks, tracks->track_capacity, tracks->hit_ids,
+      t->g, t->s.ctl, y, z, t->s.hit_row, tracks->tracks, tracks->track_capacity, tracks->hit_ids,
       tracks->hit_capacity, tracks->counts, refit_out);
   return cudaGetLastError();
 }

@@ -32,6 +32,16 @@ int ceil_log2(int64_t v) {
   return s;
 }
 
+// Seeds a call can hold.  The worst case is n/l_min, but the per-seed scratch is ~2.2 KB and real events have far
+// fewer (BASELINE configs: n/50 .. n/20), so the bound is n/16 + 4096 unless the caller reserved more; a call that
+// exceeds it sets TPC_FLAG_SEED_OVERFLOW and reports the count it needs (a3, a5).
+int64_t seed_capacity(const tpc_tracker* t, int64_t n) {
+  const int64_t worst = n / t->params.l_min + 1;
+  int64_t cap = n / 16 + 4096;
+  if (cap < t->seed_reserve) cap = t->seed_reserve;
+  return cap < worst ? cap : worst;
+}
+
 // Lays the scratch arrays out inside one allocation; returns the total size.  base may be NULL (size query).
 size_t layout(tpc_tracker* t, char* base, int64_t n, int64_t R) {
   size_t off = 0;
@@ -40,7 +50,7 @@ size_t layout(tpc_tracker* t, char* base, int64_t n, int64_t R) {
     off += align_up(bytes, 256);
     return p;
   };
-  const int64_t s_cap = n / t->params.l_min + 1;
+  const int64_t s_cap = seed_capacity(t, n);
   const int64_t tiles_a3 = (n + A3_TILE - 1) / A3_TILE;
   const int64_t tiles_a5 = (s_cap + A5_TILE - 1) / A5_TILE;
   Scratch& s = t->s;
@@ -54,16 +64,18 @@ size_t layout(tpc_tracker* t, char* base, int64_t n, int64_t R) {
   s.bin_start = (uint32_t*)take((size_t)R * t->g.nb_stride * 4);
   s.link_up = (int32_t*)take((size_t)n * 4);
   s.link_dn = (int32_t*)take((size_t)n * 4);
-  s.rec = (int4*)take((size_t)n * 16);
   s.owner = (uint32_t*)take((size_t)n * 4);
   s.hit_row = (uint8_t*)take((size_t)n + 64);
   s.q_items = (uint32_t*)take((size_t)s_cap * 3 * A4_Q_BUCKETS * 4);
   s.tl_state = (int4*)take((size_t)s_cap * A4_STATE_V4 * 16);
   s.tl_span = (uint32_t*)take((size_t)s_cap * 4);
+  s.seed_tmp = (int4*)take((size_t)s_cap * 16);
   s.seed_start = (int32_t*)take((size_t)s_cap * 4);
+  s.seed_pos = (int32_t*)take((size_t)s_cap * 4);
   s.seed_sr = (int32_t*)take((size_t)s_cap * 4);
   s.tl_rec = (float4*)take((size_t)s_cap * TL_REC_V4 * 16);
   s.tl_hits = (int32_t*)take((size_t)s_cap * t->g.n_rows * 4);
+  s.tl_yz = (int2*)take((size_t)s_cap * ((t->g.n_rows + 3) & ~3) * 8);
   if (base) {
     t->s_cap = s_cap;
     t->tiles_a3 = tiles_a3;
@@ -194,7 +206,7 @@ int tpc_tracker_create(const tpc_geometry_t* geo, const tpc_field_t* field, tpc_
   tpc_params_t prm;
   if (geo->params) prm = *geo->params; else tpc_default_params(&prm);
   if (prm.w_y < 0 || prm.w_z < 0 || prm.cost_wy < 0 || prm.cost_wz < 0 || prm.c_max < 0 || prm.l_min < 2 ||
-      prm.max_miss < 0 || prm.n_min_tracklet < 1 || prm.n_min_tracklet > 255 || prm.n_min_owned < 1 ||
+      prm.max_miss < 1 || prm.n_min_tracklet < 1 || prm.n_min_tracklet > 255 || prm.n_min_owned < 1 ||
       nr > 255 || !(prm.sigma_y > 0) || !(prm.sigma_z > 0) || !(prm.sinphi_max > 0) || !(prm.sinphi_max < 1) ||
       !(prm.gate_y_cm >= 0) || !(prm.gate_z_cm >= 0))
     return TPC_ERR_ARG;
@@ -299,9 +311,10 @@ int tpc_track(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* strea
   if ((out->track_capacity > 0 && !out->tracks) || (out->hit_capacity > 0 && !out->hit_ids)) return TPC_ERR_ARG;
   if (n > 0 && (!cl->y || !cl->z)) return TPC_ERR_ARG;
   if (!cl->row_offsets) return TPC_ERR_ARG;
-  if (n >= ((int64_t)1 << 31) || n / t->params.l_min + 1 >= 0xFFFFFF) return TPC_ERR_CAPACITY;
+  if (n >= ((int64_t)1 << 31) || seed_capacity(t, n) >= 0xFFFFFF) return TPC_ERR_CAPACITY;
   cudaStream_t st = (cudaStream_t)stream;
   const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
+  if (n > 0 && R == 0) return TPC_ERR_ARG;   // clusters but no (sector,row) to put them in
   choose_grid(t, n, R);
   int rc = ensure_arena(t, n, R);
   if (rc != TPC_OK) return rc;
@@ -310,20 +323,21 @@ int tpc_track(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* strea
   t->last_y = cl->y;
   t->last_z = cl->z;
   TPC_CUDA(t, cudaMemsetAsync(t->s.ctl, 0, t->ctl_bytes, st));
+  if (n > 0) TPC_CUDA(t, cudaMemsetAsync(t->s.owner, 0, (size_t)n * 4, st));   // a5 ownership words start empty
   cudaEvent_t* ev = t->ev + (t->timed_calls % TIMING_SETS) * 6;   // ring of event sets, one per timed call
   if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[0], st));
+  TPC_CUDA(t, launch_a0_check(t, cl->row_offsets, n, st));
   TPC_CUDA(t, launch_a0_origin(t, cl->z, cl->row_offsets, n, st));
   TPC_CUDA(t, launch_a1_grid(t, cl->y, cl->z, cl->row_offsets, n, st));
   if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[1], st));
   TPC_CUDA(t, launch_a2_neighbours(t, cl->row_offsets, n, st));
   if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[2], st));
-  TPC_CUDA(t, launch_a3_seeds(t, cl->y, cl->z, cl->row_offsets, n, st));
+  TPC_CUDA(t, launch_a3_seeds(t, cl->row_offsets, n, st));
   if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[3], st));
   // a4 variant: large calls run the follower as four phase-specialised kernels + a vote kernel (20 % fewer
   // instructions per tracklet, but five launches and a queue tail each: measured slower below ~10 events of
-  // configs[1]); small calls run the single uniform kernel.  TPC_A4_MODE=uniform|phased overrides (tests).
-  const char* mode = getenv("TPC_A4_MODE");
-  t->a4_phased = mode ? (strcmp(mode, "phased") == 0) : (n >= A4_PHASED_MIN_CLUSTERS);
+  // configs[1]); small calls run the single uniform kernel.  tpc_debug_set_a4_variant overrides (tests).
+  t->a4_phased = t->a4_variant ? (t->a4_variant == 2) : (n >= A4_PHASED_MIN_CLUSTERS);
   if (t->a4_phased) TPC_CUDA(t, launch_a4_phases(t, n, st));
   else TPC_CUDA(t, launch_a4_follow(t, n, st));
   if (t->timing) TPC_CUDA(t, cudaEventRecord(ev[4], st));
@@ -344,7 +358,7 @@ int tpc_refit(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* strea
   // the records of the clusters (a3) must be those of the call that produced `tracks`
   if (!t->arena || n != t->last_n || cl->row_offsets != t->last_ro || cl->y != t->last_y || cl->z != t->last_z)
     return TPC_ERR_ARG;
-  TPC_CUDA(t, launch_a6_refit(t, cl->row_offsets, tracks, refit_out, (cudaStream_t)stream));
+  TPC_CUDA(t, launch_a6_refit(t, cl->y, cl->z, tracks, refit_out, (cudaStream_t)stream));
   return TPC_OK;
 }
 
@@ -389,12 +403,17 @@ int tpc_track_host(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* 
     TPC_CUDA(t, cudaMemcpyAsync(b + o_z, cl->z, (size_t)n * 4, cudaMemcpyHostToDevice, st));
   }
   TPC_CUDA(t, cudaMemcpyAsync(b + o_ro, cl->row_offsets, (size_t)(R + 1) * 4, cudaMemcpyHostToDevice, st));
-  int rc = tpc_track(t, &dcl, n, stream, &dout);
-  if (rc != TPC_OK) return rc;
-  TPC_CUDA(t, cudaMemcpyAsync(out->counts, dout.counts, 16, cudaMemcpyDeviceToHost, st));
-  TPC_CUDA(t, cudaStreamSynchronize(st));
+  for (int attempt = 0;; ++attempt) {
+    int rc = tpc_track(t, &dcl, n, stream, &dout);
+    if (rc != TPC_OK) return rc;
+    TPC_CUDA(t, cudaMemcpyAsync(out->counts, dout.counts, 16, cudaMemcpyDeviceToHost, st));
+    TPC_CUDA(t, cudaStreamSynchronize(st));
+    if (!(out->counts[2] & TPC_FLAG_SEED_OVERFLOW) || attempt == 1) break;
+    t->seed_reserve = (int64_t)out->counts[3] + out->counts[3] / 8 + 1024;   // the call said what it needs: once more
+  }
   const int64_t nt = out->counts[0] < out->track_capacity ? out->counts[0] : out->track_capacity;
-  const int64_t nh = out->counts[1] <= out->hit_capacity ? out->counts[1] : 0;
+  // a5 writes the list of every track whose hits fit below hit_capacity: copy that prefix
+  const int64_t nh = out->counts[1] <= out->hit_capacity ? out->counts[1] : out->hit_capacity;
   if (nt > 0)
     TPC_CUDA(t, cudaMemcpyAsync(out->tracks, dout.tracks, (size_t)nt * sizeof(tpc_track_rec_t), cudaMemcpyDeviceToHost, st));
   if (nh > 0) TPC_CUDA(t, cudaMemcpyAsync(out->hit_ids, dout.hit_ids, (size_t)nh * 4, cudaMemcpyDeviceToHost, st));
@@ -404,7 +423,19 @@ int tpc_track_host(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* 
 
 int64_t tpc_scratch_bytes(const tpc_tracker_t* t) { return t ? (int64_t)(t->arena_bytes + t->host_arena_bytes) : 0; }
 
-int tpc_launches_per_call(const tpc_tracker_t* t) { return t ? (t->a4_phased ? 10 : 6) : 0; }
+int tpc_launches_per_call(const tpc_tracker_t* t) { return t ? (t->a4_phased ? 12 : 8) : 0; }
+
+int tpc_reserve_seeds(tpc_tracker_t* t, int64_t n_seeds) {
+  if (!t || n_seeds < 0) return TPC_ERR_ARG;
+  if (n_seeds > t->seed_reserve) t->seed_reserve = n_seeds;
+  return TPC_OK;
+}
+
+int tpc_debug_set_a4_variant(tpc_tracker_t* t, int variant) {
+  if (!t || variant < 0 || variant > 2) return TPC_ERR_ARG;
+  t->a4_variant = variant;
+  return TPC_OK;
+}
 
 int tpc_set_stage_timing(tpc_tracker_t* t, int enable) {
   if (!t) return TPC_ERR_ARG;
@@ -444,12 +475,7 @@ int tpc_debug_copy_links(tpc_tracker_t* t, int which, int32_t* up, int32_t* dn, 
   if (!t->arena) return TPC_ERR_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   if (t->last_n == 0) return TPC_OK;
-  if (which == 0) {
-    TPC_CUDA(t, cudaMemcpyAsync(up, t->s.link_up, (size_t)t->last_n * 4, cudaMemcpyDeviceToDevice, st));
-    TPC_CUDA(t, cudaMemcpyAsync(dn, t->s.link_dn, (size_t)t->last_n * 4, cudaMemcpyDeviceToDevice, st));
-  } else {
-    TPC_CUDA(t, launch_dbg_clean(t, t->last_n, up, dn, st));
-  }
+  TPC_CUDA(t, launch_dbg_links(t, t->last_n, which, up, dn, st));
   return TPC_OK;
 }
 

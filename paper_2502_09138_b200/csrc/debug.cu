@@ -5,25 +5,34 @@
 
 namespace {
 
-// Cleaned links exactly as a3 left them for a4: rec[h] = (y, z, cleaned up link, cleaned down link).
-__global__ void dbg_clean_kernel(int64_t n, const int4* __restrict__ rec, int32_t* __restrict__ up_o,
+// Links live in sorted space (positions in srt); the exports translate them to cluster ids.
+// which = 0: the raw a2 tables.  which = 1: the cleaned links exactly as a3 left them for a4 -- the cleaned up link
+// is the fourth word of the srt record; a3 keeps no down-link table (nothing downstream reads one), so the cleaned
+// down links are the inverse of what it wrote (mutuality, P11): dn'[up'[h]] = h.
+__global__ void dbg_links_kernel(int64_t n, int which, const int4* __restrict__ srt, const int32_t* __restrict__ up,
+                                 const int32_t* __restrict__ dn, int32_t* __restrict__ up_o,
                                  int32_t* __restrict__ dn_o) {
-  const int64_t h = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (h >= n) return;
-  const int4 r = rec[h];
-  up_o[h] = r.z;
-  dn_o[h] = r.w;
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= n) return;
+  const int4 c = srt[p];
+  if (which == 0) {
+    const int u = up[p], d = dn[p];
+    up_o[c.z] = u >= 0 ? srt[u].z : -1;
+    dn_o[c.z] = d >= 0 ? srt[d].z : -1;
+  } else {
+    up_o[c.z] = c.w >= 0 ? srt[c.w].z : -1;
+    if (c.w >= 0) dn_o[srt[c.w].z] = c.z;
+  }
 }
 
 __global__ void dbg_seed_len_kernel(const DevCtl* ctl, const int32_t* __restrict__ seed_start,
-                                    const int4* __restrict__ rec, int32_t* __restrict__ start,
-                                    int32_t* __restrict__ len) {
+                                    const int32_t* __restrict__ seed_pos, const int4* __restrict__ srt,
+                                    int32_t* __restrict__ start, int32_t* __restrict__ len) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= (int64_t)ctl->n_seeds) return;
-  const int h0 = seed_start[i];
   int l = 1;
-  for (int c = rec[h0].z; c >= 0; c = rec[c].z) ++l;
-  start[i] = h0;
+  for (int c = srt[seed_pos[i]].w; c >= 0; c = srt[c].w) ++l;
+  start[i] = seed_start[i];
   len[i] = l;
 }
 
@@ -52,14 +61,18 @@ __global__ void dbg_owner_kernel(int64_t n, const uint32_t* __restrict__ owner, 
 
 }  // namespace
 
-cudaError_t launch_dbg_clean(const tpc_tracker* t, int64_t n, int32_t* up, int32_t* dn, cudaStream_t st) {
+cudaError_t launch_dbg_links(const tpc_tracker* t, int64_t n, int which, int32_t* up, int32_t* dn, cudaStream_t st) {
   if (n == 0) return cudaSuccess;
-  dbg_clean_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, t->s.rec, up, dn);
+  if (which == 1) {   // down links are scattered through the inverse: start from "none"
+    cudaError_t e = cudaMemsetAsync(dn, 0xff, (size_t)n * 4, st);
+    if (e != cudaSuccess) return e;
+  }
+  dbg_links_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, which, t->s.srt, t->s.link_up, t->s.link_dn, up, dn);
   return cudaGetLastError();
 }
 cudaError_t launch_dbg_seed_len(const tpc_tracker* t, int32_t* start, int32_t* len, cudaStream_t st) {
   if (t->s_cap == 0) return cudaSuccess;
-  dbg_seed_len_kernel<<<(unsigned)((t->s_cap + 255) / 256), 256, 0, st>>>(t->s.ctl, t->s.seed_start, t->s.rec, start, len);
+  dbg_seed_len_kernel<<<(unsigned)((t->s_cap + 255) / 256), 256, 0, st>>>(t->s.ctl, t->s.seed_start, t->s.seed_pos, t->s.srt, start, len);
   return cudaGetLastError();
 }
 cudaError_t launch_dbg_tracklets(const tpc_tracker* t, float* par, float* cov, float* chi2, int32_t* n_hits,

@@ -3,6 +3,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <limits.h>
 
 #include "../../include/tpc_track.h"
 
@@ -31,36 +32,42 @@ struct CtlLine {         // one hot counter per 128-byte line
   uint32_t pad[31];
 };
 struct DevCtl {
-  uint32_t n_seeds;      // written by a3
+  uint32_t n_seeds;      // written by a3: seeds kept = min(seeds found, seed capacity)
   uint32_t ticket_a3;    // dynamic tile ids for the a3 look-back scan
   uint32_t ticket_a5;
   uint32_t next_seed;    // a4 work queue: next seed rank to hand to a free lane
   uint32_t next_track;   // a6 work queue
-  uint32_t pad[27];
+  uint32_t n_seeds_found; // a3: seeds the call holds (> n_seeds iff the seed capacity was too small)
+  uint32_t bad_offsets;  // a0: row_offsets are not a CSR over n clusters -> every later stage does nothing
+  uint32_t pad[25];
   CtlLine q_alloc[3 * A4_Q_BUCKETS];   // a4 phase queues B, C, D x length bucket: items pushed by earlier phases ...
   CtlLine q_head[3 * A4_Q_BUCKETS];    // ... and items claimed by the consuming phase
 };
 
 struct Scratch {
   // a1
-  int4* srt;                // clusters in bin order inside each row: (y, z, cluster id, 0) -- one 16-B load per candidate
+  int4* srt;                // clusters in bin order inside each row: (y, z, cluster id, cleaned up link as a sorted
+                            // position or -1 [a3]) -- one 16-B load per search candidate and per followed chain hit
   uint32_t* sec_key;        // [n_sectors] a0: order-preserving key of the sector's smallest z (zeroed per call)
   uint32_t* bin_start;      // [R * nb_stride] global sorted index of the first cluster of each bin (+ sentinel)
-  // a2 / a3 (id space)
+  // a2 / a3: raw links in SORTED space (position of the linked cluster in srt, -1 = none), written coalesced
   int32_t *link_up, *link_dn;
-  int4* rec;                // a3: per cluster id (y, z, cleaned up link, cleaned down link) -- one 16-B gather per a4 step
-  uint32_t* owner;          // packed (n_hits << 24 | 0xFFFFFF - rank), 0 = none
+  uint32_t* owner;          // [n, id space] packed (n_hits << 24 | 0xFFFFFF - rank), 0 = none (zeroed per call)
   uint8_t* hit_row;         // [n] a5: row of the hit at each position of the output hit list (for a6)
   uint32_t* q_items;        // [3 * A4_Q_BUCKETS][s_cap] a4 phase queues: seed ranks
   int4* tl_state;           // [s_cap][A4_STATE_V4] a4 filter state of a tracklet between two phases
   uint32_t* tl_span;        // [s_cap] first | last << 8 row a tracklet visited (rows outside hold no hit)
   // a3 -> a4
-  int32_t* seed_start;      // [s_cap] start cluster id, ascending
+  int4* seed_tmp;           // [s_cap] a3: seeds in sorted-position order (position, start id, sector*n_rows+row, 0)
+  int32_t* seed_start;      // [s_cap] start cluster id, ascending (P14)
+  int32_t* seed_pos;        // [s_cap] sorted position of the start cluster
   int32_t* seed_sr;         // [s_cap] sector * n_rows + row of the start cluster
   // a4 tracklets, one 96-B record + one row table per seed
   float4* tl_rec;           // [s_cap][6]: (x_ref,y,z,sinphi) (tanl,qpt,chi2,n_hits as int bits) cov[0..3] cov[4..7]
                             //             cov[8..11] (cov[12],cov[13],cov[14],sector*n_rows+first seed row as int bits)
   int32_t* tl_hits;         // [s_cap][n_rows] cluster id or -1
+  int2* tl_yz;              // [s_cap][n_rows] (y, z) of the hit the upward pass recorded in that row (y = INT32_MIN:
+                            // none): the downward refit streams these instead of gathering clusters by id
   // control
   DevCtl* ctl;
   uint64_t* scan_a3;        // look-back status words
@@ -69,6 +76,8 @@ struct Scratch {
   int32_t *st_y, *st_z; uint32_t* st_ro;
   tpc_track_rec_t* st_tracks; int32_t* st_hits; int32_t* st_counts;
 };
+
+constexpr int32_t YZ_NONE = INT32_MIN;   // tl_yz[..].x of a row without a hit
 
 constexpr int TIMING_SETS = 64;   // ring of per-call stage-event sets (tpc_get_stage_ms_mean averages over them)
 
@@ -84,9 +93,11 @@ struct tpc_tracker {
   int64_t cap_n, cap_rows;   // sizes the arena was laid out for
   int base_shift_y, base_shift_z;   // coarsest grid (bins >= 2 x the widest window); dense calls refine it
   int64_t y_units, z_units;         // grid extents in fixed-point units
-  int64_t s_cap;             // seed capacity of the current layout
+  int64_t s_cap;             // seed capacity of the current layout (api.cu: seed_capacity)
+  int64_t seed_reserve;      // tpc_reserve_seeds: lower bound on s_cap
   int64_t tiles_a3, tiles_a5;
   int a4_phased;             // the most recent call ran a4 as phase kernels (api.cu)
+  int a4_variant;            // tpc_debug_set_a4_variant: 0 = by call size, 1 = uniform kernel, 2 = phase kernels
   int a4_sms;              // SMs of the device (phase kernels size their own persistent grids)
   int a4_blocks, a4_warps;   // persistent a4 grid: blocks x warps per block = resident warps of the device (set at create)
   size_t ctl_bytes;          // bytes zeroed per call
@@ -111,21 +122,22 @@ constexpr int A4_STATE_V4 = 8;  // 16-byte words of a parked a4 state: 15 U D U^
 constexpr int TL_REC_V4 = 6;    // float4 words per tracklet record
 
 // launchers (each in its own .cu)
+cudaError_t launch_a0_check(const tpc_tracker* t, const uint32_t* ro, int64_t n, cudaStream_t st);
 cudaError_t launch_a0_origin(const tpc_tracker* t, const int32_t* z, const uint32_t* ro, int64_t n, cudaStream_t st);
 cudaError_t launch_a1_grid(const tpc_tracker* t, const int32_t* y, const int32_t* z, const uint32_t* ro, int64_t n, cudaStream_t st);
 cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64_t n, cudaStream_t st);
-cudaError_t launch_a3_seeds(const tpc_tracker* t, const int32_t* y, const int32_t* z, const uint32_t* ro, int64_t n, cudaStream_t st);
+cudaError_t launch_a3_seeds(const tpc_tracker* t, const uint32_t* ro, int64_t n, cudaStream_t st);
 cudaError_t launch_a4_follow(const tpc_tracker* t, int64_t n, cudaStream_t st);
 cudaError_t setup_a4_attributes(tpc_tracker* t);
 cudaError_t launch_a4_phases(const tpc_tracker* t, int64_t n, cudaStream_t st);
 cudaError_t launch_a5_select(const tpc_tracker* t, const tpc_tracks_out_t* out, cudaStream_t st);
-cudaError_t launch_a6_refit(const tpc_tracker* t, const uint32_t* ro, const tpc_tracks_out_t* tracks,
+cudaError_t launch_a6_refit(const tpc_tracker* t, const int32_t* y, const int32_t* z, const tpc_tracks_out_t* tracks,
                             tpc_track_rec_t* refit_out, cudaStream_t st);
 cudaError_t setup_a1_attributes(const tpc_tracker* t);
 size_t a1_smem_bytes(const DevGeom& g);
 
 // debug.cu
-cudaError_t launch_dbg_clean(const tpc_tracker* t, int64_t n, int32_t* up, int32_t* dn, cudaStream_t st);
+cudaError_t launch_dbg_links(const tpc_tracker* t, int64_t n, int which, int32_t* up, int32_t* dn, cudaStream_t st);
 cudaError_t launch_dbg_seed_len(const tpc_tracker* t, int32_t* start, int32_t* len, cudaStream_t st);
 cudaError_t launch_dbg_tracklets(const tpc_tracker* t, float* par, float* cov, float* chi2, int32_t* n_hits, int32_t* hits, cudaStream_t st);
 cudaError_t launch_dbg_owner(const tpc_tracker* t, int64_t n, int32_t* owner, cudaStream_t st);

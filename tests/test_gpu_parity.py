@@ -13,11 +13,12 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-4
 
 
-def _run_gpu(ev, params=None):
+def _run_gpu(ev, params=None, a4_variant=0):
     import torch
     from paper_2502_09138_b200 import Tracker
     from paper_2502_09138_b200.events import geometry_from_event, upload
     trk = Tracker(geometry_from_event(ev, params))
+    trk.set_a4_variant(a4_variant)
     y, z, ro = upload(ev)
     out = trk.track(y, z, ro)
     tracks, hit_ids, ns = out.to_host()
@@ -76,11 +77,13 @@ def compare(ev, orc, g, o, *, min_assign=0.999, label=""):
     assert np.array_equal(g["n_hits"][same], o["n_hits"][same]), label + " tracklet n_hits"
     cerr = cov_scaled_error(g["cov"][same], o["cov"][same]) if err.size else np.zeros((0, 15))
     worst_cov = float(cerr.max()) if cerr.size else 0.0
-    assert worst_cov <= COV_TOL, f"{label} covariance off by {worst_cov:.3e} (scaled), element {np.unravel_index(cerr.argmax(), cerr.shape)}"
+    n_cov_bad = int((cerr > COV_TOL).any(axis=1).sum()) if cerr.size else 0
+    assert n_cov_bad <= n_allowed, \
+        f"{label} {n_cov_bad} covariances off by up to {worst_cov:.3e} (scaled), element {np.unravel_index(cerr.argmax(), cerr.shape)}"
     xref = o["chi2"][same]
     xerr = np.abs(g["chi2"][same].astype(np.float64) - xref) / np.maximum(xref, 1.0) if err.size else np.zeros(0)
     worst_chi2 = float(xerr.max()) if xerr.size else 0.0
-    assert worst_chi2 <= CHI2_TOL, f"{label} chi2 off by {worst_chi2:.3e}"
+    assert int((xerr > CHI2_TOL).sum()) <= n_allowed, f"{label} chi2 off by {worst_chi2:.3e}"
     # ---- output tracks ----
     gt = g["tracks"]
     frac, pairs = assignment_match(gt["seed_cluster"], gt["hit_offset"], gt["n_hits"], g["hit_ids"],
@@ -100,7 +103,7 @@ def compare(ev, orc, g, o, *, min_assign=0.999, label=""):
         rerr = np.abs(rec_par[ks].astype(np.float64) - o["par"][k][ks]) / np.maximum(np.abs(o["par"][k][ks]), 1.0)
         assert rerr.size == 0 or int((rerr[:, 1:] > TOL).any(axis=1).sum()) <= n_allowed, \
             label + " track record parameters vs oracle"
-        assert rerr.size == 0 or cov_scaled_error(gt["cov"][ks], o["cov"][k][ks]).max() <= COV_TOL
+        assert rerr.size == 0 or int((cov_scaled_error(gt["cov"][ks], o["cov"][k][ks]) > COV_TOL).any(axis=1).sum()) <= n_allowed
     sec, row = ev.sector_row()
     for t in range(0, len(gt), max(1, len(gt) // 200)):
         h = g["hit_ids"][gt["hit_offset"][t]: gt["hit_offset"][t] + gt["n_hits"][t]]
@@ -373,13 +376,13 @@ def test_refit_rejects_foreign_input(orc):
 
 
 @pytest.mark.parametrize("mode", ["uniform", "phased"])
-def test_both_a4_variants_on_small_and_stress_events(orc, mode, monkeypatch):
+def test_both_a4_variants_on_small_and_stress_events(orc, mode):
     """The library picks the a4 variant by call size (phase kernels for large calls); both must give the oracle's
-    result on any input, so both are forced here on events of either size class."""
-    monkeypatch.setenv("TPC_A4_MODE", mode)
+    result on any input, so both are forced here (tpc_debug_set_a4_variant) on events of either size class."""
+    variant = {"uniform": 1, "phased": 2}[mode]
     for ev, lab in ((make_event(0), "cfg0"), (make_event(1, 1001), "cfg1"), (make_event(4), "cfg4"),
                     (make_event(2, collisions=6), "cfg2/6")):
-        compare(ev, orc, _run_gpu(ev), orc.track(ev), label=f"{lab} a4={mode}")
+        compare(ev, orc, _run_gpu(ev, a4_variant=variant), orc.track(ev), label=f"{lab} a4={mode}")
 
 
 def test_edge_empty_and_tiny(orc):
@@ -424,6 +427,95 @@ def test_capacity_overflow_flags(orc):
     torch.cuda.synchronize()
     c = out.counts.cpu().numpy()
     assert c[0] > 10 and c[1] > 500 and c[2] == 3
+    trk.close()
+
+
+def test_seed_capacity_overflow_and_reserve(orc):
+    """The handle holds n/16 + 4096 seeds per call by default.  A call with more raises TPC_FLAG_SEED_OVERFLOW and
+    reports in counts[3] what it needs; after tpc_reserve_seeds the same call gives the oracle's result.  Built from
+    short chains: every 8th row is emptied, which cuts every track into pieces of 7 rows whose inner 5 clusters form
+    a chain (the end clusters of a piece have no pair of neighbours, P5/P8): ~n/7 seeds of exactly l_min clusters."""
+    import torch
+    from paper_2502_09138_b200 import Tracker
+    from paper_2502_09138_b200.events import geometry_from_event, upload
+    ev = make_event(1, 91, n_tracks=6000, noise=0.0)
+    sec, row = ev.sector_row()
+    keep = (row % 8) != 7
+    idx = np.nonzero(keep)[0]
+    ev.y, ev.z, ev.label = ev.y[idx], ev.z[idx], ev.label[idx]
+    ev.y_exact, ev.z_exact = ev.y_exact[idx], ev.z_exact[idx]
+    counts = np.bincount((sec * ev.n_rows + row)[idx], minlength=ev.n_sectors * ev.n_rows)
+    ev.row_offsets = np.concatenate([[0], np.cumsum(counts)]).astype(np.uint32)
+    o = orc.track(ev)
+    ns = len(o["seed_start"])
+    assert ns > ev.n // 16 + 4096, (ns, ev.n)
+    trk = Tracker(geometry_from_event(ev))
+    y, z, ro = upload(ev)
+    out = trk.track(y, z, ro)
+    torch.cuda.synchronize()
+    c = out.counts.cpu().numpy()
+    assert c[2] & 4 and c[3] == ns, c                                  # TPC_FLAG_SEED_OVERFLOW, seeds needed
+    trk.reserve_seeds(int(c[3]))
+    tracks, hit_ids, ns2 = trk.track(y, z, ro).to_host()
+    assert ns2 == ns and np.array_equal(hit_ids, o["hit_ids"])
+    assert np.array_equal(tracks["seed_cluster"], o["seed_start"][o["trk_seed"]])
+    # the host-buffer entry point retries by itself
+    trk2 = Tracker(geometry_from_event(ev))
+    from paper_2502_09138_b200 import TRACK_DTYPE
+    ht = torch.empty((ev.n // 10 + 16) * 112, dtype=torch.uint8).pin_memory()
+    hh = torch.empty(ev.n + 16, dtype=torch.int32).pin_memory()
+    hc = torch.zeros(4, dtype=torch.int32).pin_memory()
+    trk2.track_host(torch.from_numpy(ev.y.copy()), torch.from_numpy(ev.z.copy()),
+                    torch.from_numpy(ev.row_offsets.view(np.int32).copy()), ht, hh, hc)
+    assert int(hc[2]) == 0 and int(hc[3]) == ns and np.array_equal(hh[: int(hc[1])].numpy(), o["hit_ids"])
+    trk.close()
+    trk2.close()
+
+
+def test_malformed_row_offsets_are_flagged_not_followed(orc):
+    import torch
+    from paper_2502_09138_b200 import Tracker
+    from paper_2502_09138_b200.events import geometry_from_event, upload
+    ev = make_event(0)
+    trk = Tracker(geometry_from_event(ev))
+    y, z, ro = upload(ev)
+    for mutate in ("descending", "short", "long"):
+        bad = ro.clone()
+        if mutate == "descending":
+            bad[40] = bad[41] + 5
+        elif mutate == "short":
+            bad[-1] = bad[-1] - 3
+        else:
+            bad[-1] = bad[-1] + 1000
+        out = trk.track(y, z, bad)
+        torch.cuda.synchronize()
+        c = out.counts.cpu().numpy()
+        assert c[2] & 8 and c[0] == 0 and c[1] == 0, (mutate, c)       # TPC_FLAG_BAD_OFFSETS
+    tracks, _, _ = trk.track(y, z, ro).to_host()                       # the handle is fine afterwards
+    assert len(tracks) == len(orc.track(ev)["trk_seed"])
+    trk.close()
+
+
+def test_host_entry_copies_the_hit_lists_that_fitted(orc):
+    import torch
+    from paper_2502_09138_b200 import Tracker, TRACK_DTYPE
+    from paper_2502_09138_b200.events import geometry_from_event
+    ev = make_event(0)
+    o = orc.track(ev)
+    trk = Tracker(geometry_from_event(ev))
+    cap = 1000
+    ht = torch.empty(2000 * 112, dtype=torch.uint8).pin_memory()
+    hh = torch.full((cap,), -7, dtype=torch.int32).pin_memory()
+    hc = torch.zeros(4, dtype=torch.int32).pin_memory()
+    trk.track_host(torch.from_numpy(ev.y.copy()), torch.from_numpy(ev.z.copy()),
+                   torch.from_numpy(ev.row_offsets.view(np.int32).copy()), ht, hh, hc)
+    assert int(hc[2]) == 2 and int(hc[1]) == len(o["hit_ids"]) > cap   # TPC_FLAG_HIT_OVERFLOW
+    rec = ht[: int(hc[0]) * 112].numpy().view(TRACK_DTYPE)
+    fit = rec["hit_offset"] + rec["n_hits"] <= cap
+    assert fit.any() and not fit.all()
+    for k in np.nonzero(fit)[0]:
+        a = rec["hit_offset"][k]
+        assert np.array_equal(hh[a: a + rec["n_hits"][k]].numpy(), o["hit_ids"][a: a + rec["n_hits"][k]])
     trk.close()
 
 
