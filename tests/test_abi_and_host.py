@@ -103,43 +103,35 @@ def test_product_never_imports_the_oracle():
             assert "libtpctrack" not in src, fn
 
 
-_WORKER = r"""
-import os, sys
-sys.path.insert(0, {root!r})
-import torch.distributed as dist
-import bench
-dist.init_process_group("gloo")
-r, w = dist.get_rank(), dist.get_world_size()
-seeds = bench.shard_seeds(r, w, 4)
-ms, units = bench.aggregate(10.0 + 5.0 * r, 100.0 * (r + 1), dist, None)
-gathered = [None] * w
-dist.all_gather_object(gathered, seeds)
-if r == 0:
-    flat = [s for g in gathered for s in g]
-    assert len(set(flat)) == len(flat) == 4 * w, flat
-    assert ms == 15.0 and units == 300.0, (ms, units)
-    print("GLOO_OK")
-dist.destroy_process_group()
-"""
+def test_bench_gpus_flag_starts_replica_ranks_gloo_world2():
+    """`bench.py --gpus 2` outside torchrun starts two replica ranks itself (torchrun's environment, rendezvous on
+    127.0.0.1).  N > 1: ranks are replicas on their own events (weak scaling, no data-path collective); rank 0 reports
+    the max-over-ranks time and the sum of units.  Run on the CPU over gloo through the launcher."""
+    import json
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--selftest-ranks",
+                          "--batch-events", "4"], capture_output=True, text=True, timeout=300, env=env)
+    assert out.returncode == 0, out.stderr
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    assert line == {"selftest": "ranks", "n_gpus": 2, "ms_max": 15.0, "units_sum": 300.0, "seeds_distinct": True}
 
 
-def test_multi_rank_bookkeeping_gloo_world2(tmp_path):
-    """N > 1: ranks are replicas on their own events (weak scaling, no data-path collective); rank 0 reports
-    max-over-ranks time and the sum of units."""
+def test_bench_under_torchrun_environment_does_not_spawn_again():
+    """With torchrun's variables already set, --gpus N is only a label: the process is one rank of the job."""
+    import json
     with socket.socket() as s:
         s.bind(("127.0.0.1", 0))
         port = s.getsockname()[1]
-    script = tmp_path / "w.py"
-    script.write_text(_WORKER.format(root=ROOT))
     procs = []
     for r in range(2):
         env = dict(os.environ, RANK=str(r), WORLD_SIZE="2", LOCAL_RANK=str(r), MASTER_ADDR="127.0.0.1",
                    MASTER_PORT=str(port))
-        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE,
-                                      stderr=subprocess.STDOUT, text=True))
+        procs.append(subprocess.Popen([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--selftest-ranks"],
+                                      env=env, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True))
     outs = [p.communicate(timeout=240)[0] for p in procs]
     assert all(p.returncode == 0 for p in procs), outs
-    assert "GLOO_OK" in outs[0]
+    line = json.loads([l for l in outs[0].splitlines() if l.startswith("{")][-1])
+    assert line["n_gpus"] == 2 and line["seeds_distinct"] and line["units_sum"] == 300.0
 
 
 def test_bench_reference_arm_prints_contract_line():
