@@ -49,6 +49,9 @@ def lib():
         _lib.orc_update.restype = C.c_double
         _lib.orc_transport.restype = C.c_int
         _lib.orc_num_threads.restype = C.c_int
+        _lib.orc_rotate.restype = C.c_int
+        _lib.orc_match_chi2.restype = C.c_double
+        _lib.orc_merge.restype = C.c_int64
     return _lib
 
 
@@ -174,6 +177,59 @@ def refit(y_cm, z_cm, row_offsets, n_sectors, n_rows, row_x, bz, trk_hit_offset,
                     _i32(np.ascontiguousarray(trk_n_owned, np.int32)), _i32(np.ascontiguousarray(hit_ids, np.int32)),
                     _f64(par), _f64(cov), _f64(chi2), _i32(n_used))
     return par, cov, chi2, n_used
+
+
+MERGE_GAP_MAX = 25        # P43: rows between the last hit of a segment and the first hit of its continuation
+MERGE_CHI2_MAX = 50.0     # P44: 5-parameter chi2 of the extrapolated state against the continuation's state
+
+
+def rotate(x, state, cov, alpha, cq, sinphi_max=0.95):
+    """orc_rotate: (ok, x', state', cov') in the frame turned by alpha."""
+    xx = C.c_double(float(x))
+    st = np.array(state, dtype=np.float64)
+    cv = None if cov is None else np.array(cov, dtype=np.float64).reshape(25)
+    ok = lib().orc_rotate(C.c_double(cq), C.c_double(sinphi_max), C.c_double(alpha), C.byref(xx), _f64(st),
+                          _f64(cv) if cv is not None else None)
+    return bool(ok), xx.value, st, (None if cv is None else cv.reshape(5, 5))
+
+
+def match_chi2(par_a, cov_a, par_b, cov_b, alpha, cq, sinphi_max=0.95):
+    pa, ca = np.ascontiguousarray(par_a, np.float64), np.ascontiguousarray(cov_a, np.float64)
+    pb, cb = np.ascontiguousarray(par_b, np.float64), np.ascontiguousarray(cov_b, np.float64)
+    return float(lib().orc_match_chi2(C.c_double(cq), C.c_double(sinphi_max), C.c_double(alpha), _f64(pa), _f64(ca),
+                                      _f64(pb), _f64(cb)))
+
+
+def merge(par, cov, sector, first_row, last_row, bz, params=None, n_per_side=18, sector_angle=np.deg2rad(20.0),
+          gap_max=MERGE_GAP_MAX, chi2_max=MERGE_CHI2_MAX):
+    """orc_merge over track records (par [nt, 6], cov [nt, 15]); returns (succ, pred, link_chi2, n_links)."""
+    p = params or default_params()
+    nt = int(np.asarray(sector).shape[0])
+    par = np.ascontiguousarray(par, np.float64).reshape(nt, 6)
+    cov = np.ascontiguousarray(cov, np.float64).reshape(nt, 15)
+    sector = np.ascontiguousarray(sector, np.int32)
+    first_row = np.ascontiguousarray(first_row, np.int32)
+    last_row = np.ascontiguousarray(last_row, np.int32)
+    succ = np.full(nt, -1, np.int32)
+    pred = np.full(nt, -1, np.int32)
+    chi2 = np.full(nt, -1.0, np.float64)
+    nl = lib().orc_merge(C.c_double(p.cq_per_tesla * bz), C.c_double(p.sinphi_max), C.c_int32(n_per_side),
+                         C.c_double(sector_angle), C.c_int32(gap_max), C.c_double(chi2_max), C.c_int64(nt), _f64(par),
+                         _f64(cov), _i32(sector), _i32(first_row), _i32(last_row), _i32(succ), _i32(pred), _f64(chi2))
+    return succ, pred, chi2, int(nl)
+
+
+def track_records(ev, o):
+    """(sector, first_row, last_row) of the oracle's output tracks, from their owned hit lists."""
+    sec, row = ev.sector_row()
+    nt = len(o["trk_seed"])
+    s = np.zeros(nt, np.int32)
+    f = np.zeros(nt, np.int32)
+    l = np.zeros(nt, np.int32)
+    for t in range(nt):
+        h = o["hit_ids"][o["trk_hit_offset"][t]: o["trk_hit_offset"][t] + o["trk_n_owned"][t]]
+        s[t], f[t], l[t] = sec[h[0]], row[h[0]], row[h[-1]]
+    return s, f, l
 
 
 def track(ev, params=None, *, brute=False, search_mode=1, exact_coords=False, timings=None):

@@ -584,3 +584,156 @@ extern "C" void orc_refit(const orc_params_t* p, double bz, int32_t n_sectors, i
     n_used[t] = used;
   }
 }
+
+// ------------------------------------------------------------------------------------------------
+// NEXT-1: merging of sector tracks across sector edges, the central membrane and inside a sector.
+// Readings P42..P46.  Geometry: the frame of sector s' = s + 1 is the frame of s turned by +20 degrees.
+// ------------------------------------------------------------------------------------------------
+// P42.  Point (x, y) and direction phi in the old frame; in the frame turned by alpha:
+//   x' = x cos a + y sin a,  y' = -x sin a + y cos a,  phi' = phi - a,  z, tan lambda, q/pT unchanged.
+// The state is "at the plane x = const", so a variation of y moves the point off the new plane x'; bringing it back
+// along the track (dy'/dx' = tan phi', dz/dx' = tan lambda / cos phi', d sin phi'/dx' = k) gives the Jacobian
+//   dy'/dy = cos phi / cos phi',  dz'/dy = -sin a tan lambda / cos phi',  dsin phi'/dy = -k sin a,
+//   dsin phi'/dsin phi = cos phi' / cos phi,  all other entries as the identity.
+extern "C" int orc_rotate(double cq, double smax, double alpha, double* x, double* st, double* C) {
+  const double ca = std::cos(alpha), sa = std::sin(alpha);
+  const double s = st[2];
+  if (!(std::fabs(s) < 1.0)) return 0;
+  const double c = std::sqrt(1.0 - s * s);
+  const double s1 = s * ca - c * sa, c1 = c * ca + s * sa;
+  if (!(c1 > 0.0) || !(std::fabs(s1) < smax)) return 0;
+  if (C) {
+    double R[25];
+    for (int i = 0; i < 25; ++i) R[i] = 0.0;
+    for (int i = 0; i < 5; ++i) R[i * 5 + i] = 1.0;
+    R[0 * 5 + 0] = c / c1;
+    R[1 * 5 + 0] = -sa * st[3] / c1;
+    R[2 * 5 + 0] = -sa * cq * st[4];
+    R[2 * 5 + 2] = c1 / c;
+    double RC[25];
+    for (int i = 0; i < 5; ++i)
+      for (int j = 0; j < 5; ++j) {
+        double a = 0.0;
+        for (int l = 0; l < 5; ++l) a += R[i * 5 + l] * C[l * 5 + j];
+        RC[i * 5 + j] = a;
+      }
+    for (int i = 0; i < 5; ++i)
+      for (int j = 0; j < 5; ++j) {
+        double a = 0.0;
+        for (int l = 0; l < 5; ++l) a += RC[i * 5 + l] * R[j * 5 + l];
+        C[i * 5 + j] = a;
+      }
+  }
+  const double x0 = *x, y0 = st[0];
+  *x = x0 * ca + y0 * sa;
+  st[0] = -x0 * sa + y0 * ca;
+  st[2] = s1;
+  return 1;
+}
+
+static void unpack_cov(const double* c15, double* C) {
+  int q = 0;
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j <= i; ++j) {
+      C[i * 5 + j] = c15[q];
+      C[j * 5 + i] = c15[q];
+      ++q;
+    }
+}
+
+// P44.  chi2 = D^T S^-1 D by Cholesky S = L L^T (S is the sum of two covariances).
+extern "C" double orc_match_chi2(double cq, double smax, double alpha, const double* pa, const double* ca15,
+                                 const double* pb, const double* cb15) {
+  double x = pa[0], st[5], Ca[25], Cb[25];
+  for (int i = 0; i < 5; ++i) st[i] = pa[1 + i];
+  unpack_cov(ca15, Ca);
+  unpack_cov(cb15, Cb);
+  if (alpha != 0.0 && !orc_rotate(cq, smax, alpha, &x, st, Ca)) return -1.0;
+  if (!orc_transport(cq, smax, pb[0] - x, st, Ca)) return -1.0;
+  double S[25], D[5], L[25];
+  for (int i = 0; i < 25; ++i) S[i] = Ca[i] + Cb[i];
+  for (int i = 0; i < 5; ++i) D[i] = pb[1 + i] - st[i];
+  for (int i = 0; i < 25; ++i) L[i] = 0.0;
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j <= i; ++j) {
+      double a = S[i * 5 + j];
+      for (int l = 0; l < j; ++l) a -= L[i * 5 + l] * L[j * 5 + l];
+      if (i == j) {
+        if (!(a > 0.0)) return -1.0;
+        L[i * 5 + i] = std::sqrt(a);
+      } else {
+        L[i * 5 + j] = a / L[j * 5 + j];
+      }
+    }
+  double chi2 = 0.0, w[5];
+  for (int i = 0; i < 5; ++i) {   // forward substitution L w = D; chi2 = |w|^2
+    double a = D[i];
+    for (int l = 0; l < i; ++l) a -= L[i * 5 + l] * w[l];
+    w[i] = a / L[i * 5 + i];
+    chi2 += w[i] * w[i];
+  }
+  return chi2;
+}
+
+// P43: is a -> b a candidate, and by which rotation?
+static bool merge_candidate(int32_t n_per_side, double sector_angle, int32_t gap_max, int32_t sa, int32_t sb,
+                            int32_t last_a, int32_t first_b, double* alpha) {
+  const int32_t g = first_b - last_a;
+  if (g < 1 || g > gap_max) return false;
+  if (sa == sb) {
+    *alpha = 0.0;
+    return true;
+  }
+  const int32_t side_a = sa / n_per_side, side_b = sb / n_per_side;
+  const int32_t ia = sa % n_per_side, ib = sb % n_per_side;
+  if (side_a == side_b) {
+    const int32_t d = ((ib - ia) % n_per_side + n_per_side) % n_per_side;
+    if (d == 1) { *alpha = sector_angle; return true; }
+    if (d == n_per_side - 1) { *alpha = -sector_angle; return true; }
+    return false;
+  }
+  if (ia == ib) {   // across the central membrane: same azimuth, other side
+    *alpha = 0.0;
+    return true;
+  }
+  return false;
+}
+
+extern "C" int64_t orc_merge(double cq, double smax, int32_t n_per_side, double sector_angle, int32_t gap_max,
+                             double chi2_max, int64_t nt, const double* par, const double* cov, const int32_t* sector,
+                             const int32_t* first_row, const int32_t* last_row, int32_t* succ, int32_t* pred,
+                             double* link_chi2) {
+  std::vector<int32_t> best_s(nt, -1), best_p(nt, -1);
+  std::vector<double> chi_s(nt, std::numeric_limits<double>::infinity()), chi_p(nt, std::numeric_limits<double>::infinity());
+  // plain all-pairs scan; ascending b (a) with a strict "<" keeps the smaller index on ties (P45)
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t a = 0; a < nt; ++a)
+    for (int64_t b = 0; b < nt; ++b) {
+      double alpha;
+      if (a == b || !merge_candidate(n_per_side, sector_angle, gap_max, sector[a], sector[b], last_row[a], first_row[b], &alpha)) continue;
+      const double c = orc_match_chi2(cq, smax, alpha, par + a * 6, cov + a * 15, par + b * 6, cov + b * 15);
+      if (c < 0.0 || !(c < chi2_max)) continue;
+      if (c < chi_s[a]) { chi_s[a] = c; best_s[a] = (int32_t)b; }
+    }
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t b = 0; b < nt; ++b)
+    for (int64_t a = 0; a < nt; ++a) {
+      double alpha;
+      if (a == b || !merge_candidate(n_per_side, sector_angle, gap_max, sector[a], sector[b], last_row[a], first_row[b], &alpha)) continue;
+      const double c = orc_match_chi2(cq, smax, alpha, par + a * 6, cov + a * 15, par + b * 6, cov + b * 15);
+      if (c < 0.0 || !(c < chi2_max)) continue;
+      if (c < chi_p[b]) { chi_p[b] = c; best_p[b] = (int32_t)a; }
+    }
+  int64_t links = 0;
+  for (int64_t t = 0; t < nt; ++t) { succ[t] = -1; pred[t] = -1; link_chi2[t] = -1.0; }
+  for (int64_t a = 0; a < nt; ++a) {
+    const int32_t b = best_s[a];
+    if (b >= 0 && best_p[b] == (int32_t)a) {
+      succ[a] = b;
+      pred[b] = (int32_t)a;
+      link_chi2[a] = chi_s[a];
+      ++links;
+    }
+  }
+  return links;
+}

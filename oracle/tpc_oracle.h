@@ -93,6 +93,28 @@ void orc_refit(const orc_params_t* p, double bz, int32_t n_sectors, int32_t n_ro
                const int32_t* trk_hit_offset, const int32_t* trk_n_owned, const int32_t* hit_ids, double* par,
                double* cov, double* chi2, int32_t* n_used);
 
+/* ---- NEXT-1: merging of sector tracks (readings P42..P46) ----
+ * orc_rotate: state (y, z, sin phi, tan lambda, q/pT) at the plane x of a sector frame -> the frame turned by alpha
+ * (radians, positive = towards larger azimuth): *x and state are replaced by the same point and direction in the new
+ * frame, cov (full 5x5 row-major, may be NULL) by R C R^T for the state taken at the new plane x = *x.  Returns 0
+ * (nothing changed) iff the track does not move along +x' in the new frame or |sin phi'| >= sinphi_max. */
+int orc_rotate(double cq, double sinphi_max, double alpha, double* x, double* state, double* cov);
+/* chi2 of "track a continues as track b": a's record (x_ref, state, packed covariance) is rotated by alpha into b's
+ * frame, transported to b's x_ref, D = p_b - p_a', S = C_b + C_a', chi2 = D^T S^-1 D.  Negative iff the rotation or
+ * the transport fails. */
+double orc_match_chi2(double cq, double sinphi_max, double alpha, const double* par_a, const double* cov_a,
+                      const double* par_b, const double* cov_b);
+/* Links between the n_tracks records (par[t*6..] = x_ref + state, cov[t*15..] packed lower triangle, sector,
+ * first_row, last_row of the owned hits).  Candidate a -> b (P43): 1 <= first_row[b] - last_row[a] <= gap_max and the
+ * sectors are the same, azimuthal neighbours on the same side ((s' - s) mod n_per_side in {1, n_per_side - 1},
+ * alpha = +-sector_angle), or face each other across the central membrane (s' = s +- n_per_side, alpha = 0).
+ * succ[a] = candidate b minimising (chi2, b) among those with 0 <= chi2 < chi2_max; pred[b] likewise over a; a link
+ * a -> b stands iff succ[a] == b and pred[b] == a (P45).  Outputs: succ, pred (-1 = none, only standing links),
+ * link_chi2[a] of a's standing link (else -1).  Returns the number of links. */
+int64_t orc_merge(double cq, double sinphi_max, int32_t n_per_side, double sector_angle, int32_t gap_max,
+                  double chi2_max, int64_t n_tracks, const double* par, const double* cov, const int32_t* sector,
+                  const int32_t* first_row, const int32_t* last_row, int32_t* succ, int32_t* pred, double* link_chi2);
+
 int orc_num_threads(void);
 
 #ifdef __cplusplus
