@@ -52,7 +52,7 @@ typedef struct {
   int32_t cost_wy, cost_wz;  /* a2 cost = cost_wy*(y_u+y_d-2y_h)^2 + cost_wz*(z_u+z_d-2z_h)^2 (P8): 9, 4 */
   int32_t c_max;             /* a2 accept iff cost <= c_max (P10): 3538944 */
   int32_t l_min;             /* a3 seed iff chain length >= l_min clusters (P13): 5 */
-  int32_t max_miss;          /* a4 stop after this many consecutive rows without a hit (P20): 5 */
+  int32_t max_miss;          /* a4 stop after this many consecutive rows without a hit (P20): 5; >= 1 */
   int32_t n_min_tracklet;    /* a4/a5 tracklets with fewer hits are discarded (P24): 10 */
   int32_t n_min_owned;       /* a5 output iff owned hits >= this (P27): 10 */
   int32_t reserved;          /* must be 0 */
@@ -145,6 +145,29 @@ int tpc_track_host(tpc_tracker_t* t, const tpc_clusters_t* clusters_host, int64_
  * Errors: TPC_ERR_ARG (also when `clusters` is not the input of the handle's last call), TPC_ERR_CUDA. */
 int tpc_refit(tpc_tracker_t* t, const tpc_clusters_t* clusters, int64_t n, void* stream, const tpc_tracks_out_t* tracks,
               tpc_track_rec_t* refit_out);
+
+/* NEXT-1 (readings P42..P46 in DESIGN.md): links between sector tracks that are pieces of one particle
+ * -- across a sector edge, across the central membrane, or inside one sector.  a -> b is a candidate iff b's first row
+ * lies 1..gap_max rows above a's last row and the sectors are equal, azimuthal neighbours on one z side, or face each
+ * other across the membrane (sectors come in groups of 2*n_per_side = one event; side = (s / n_per_side) % 2).
+ * a's record is rotated into b's frame, transported to b's x, and chi2 = D^T (C_a' + C_b)^-1 D over the five
+ * parameters; succ(a) / pred(b) = candidate of smallest (chi2, index) with chi2 < chi2_max; a link stands iff
+ * succ(a) == b and pred(b) == a. */
+typedef struct {
+  int32_t gap_max;      /* P43: 25 rows */
+  int32_t n_per_side;   /* sectors per z side: 18 */
+  double chi2_max;      /* P44: 50 */
+  double sector_angle;  /* radians between the frames of neighbouring sectors: 20 degrees */
+} tpc_merge_params_t;
+void tpc_default_merge_params(tpc_merge_params_t* p);
+/* tracks: [device] records as written by tpc_track or tpc_refit (ascending sector), counts: [device] the int32[4] of
+ * that call (counts[0] tracks), track_capacity: records readable.  params: [host], NULL = defaults.
+ * Outputs, all [device]: succ[track_capacity], pred[track_capacity] (track index or -1), link_chi2[track_capacity]
+ * (chi2 of a's link, -1 without), merge_counts int32[4]: [0] links, [1] merged tracks (= tracks - links), [2] tracks.
+ * Asynchronous on `stream`.  Errors: TPC_ERR_ARG, TPC_ERR_NOMEM, TPC_ERR_CUDA. */
+int tpc_merge(tpc_tracker_t* t, const tpc_track_rec_t* tracks, const int32_t* counts, int32_t track_capacity,
+              const tpc_merge_params_t* params, void* stream, int32_t* succ, int32_t* pred, float* link_chi2,
+              int32_t* merge_counts);
 
 int tpc_tracker_destroy(tpc_tracker_t* t);
 

@@ -692,7 +692,9 @@ static bool merge_candidate(int32_t n_per_side, double sector_angle, int32_t gap
     if (d == n_per_side - 1) { *alpha = -sector_angle; return true; }
     return false;
   }
-  if (ia == ib) {   // across the central membrane: same azimuth, other side
+  // across the central membrane: same azimuth, other side of the same event (a batch of events is laid out as
+  // groups of 2 n_per_side sectors)
+  if (ia == ib && sa / (2 * n_per_side) == sb / (2 * n_per_side)) {
     *alpha = 0.0;
     return true;
   }

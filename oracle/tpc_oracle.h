@@ -107,7 +107,8 @@ double orc_match_chi2(double cq, double sinphi_max, double alpha, const double* 
 /* Links between the n_tracks records (par[t*6..] = x_ref + state, cov[t*15..] packed lower triangle, sector,
  * first_row, last_row of the owned hits).  Candidate a -> b (P43): 1 <= first_row[b] - last_row[a] <= gap_max and the
  * sectors are the same, azimuthal neighbours on the same side ((s' - s) mod n_per_side in {1, n_per_side - 1},
- * alpha = +-sector_angle), or face each other across the central membrane (s' = s +- n_per_side, alpha = 0).
+ * alpha = +-sector_angle), or face each other across the central membrane (s' = s +- n_per_side inside one group of
+ * 2 n_per_side sectors -- a batch of events is laid out as such groups --, alpha = 0).
  * succ[a] = candidate b minimising (chi2, b) among those with 0 <= chi2 < chi2_max; pred[b] likewise over a; a link
  * a -> b stands iff succ[a] == b and pred[b] == a (P45).  Outputs: succ, pred (-1 = none, only standing links),
  * link_chi2[a] of a's standing link (else -1).  Returns the number of links. */

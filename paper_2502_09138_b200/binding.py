@@ -65,6 +65,12 @@ TRACK_DTYPE = np.dtype([
 assert TRACK_DTYPE.itemsize == C.sizeof(TrackRec) == 112
 
 
+class MergeParams(C.Structure):
+    """tpc_merge_params_t"""
+    _fields_ = [("gap_max", C.c_int32), ("n_per_side", C.c_int32), ("chi2_max", C.c_double),
+                ("sector_angle", C.c_double)]
+
+
 class _TracksOut(C.Structure):
     _fields_ = [("tracks", C.c_void_p), ("track_capacity", C.c_int32), ("hit_capacity", C.c_int32),
                 ("hit_ids", C.c_void_p), ("counts", C.c_void_p)]
@@ -97,6 +103,10 @@ def load_library():
     lib.tpc_track_host.argtypes = lib.tpc_track.argtypes
     lib.tpc_refit.argtypes = [C.c_void_p, C.POINTER(_Clusters), C.c_int64, C.c_void_p, C.POINTER(_TracksOut),
                               C.c_void_p]
+    lib.tpc_default_merge_params.argtypes = [C.POINTER(MergeParams)]
+    lib.tpc_default_merge_params.restype = None
+    lib.tpc_merge.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(MergeParams), C.c_void_p,
+                              C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.tpc_tracker_destroy.argtypes = [C.c_void_p]
     lib.tpc_status_string.argtypes = [C.c_int]
     lib.tpc_status_string.restype = C.c_char_p
@@ -253,6 +263,20 @@ class Tracker:
         self._check(self._lib.tpc_refit(self._h, C.byref(cl), C.c_int64(n), self._stream_ptr(stream), C.byref(o),
                                         _ptr(ref)))
         return ref
+
+    def merge(self, tracks, counts, params: "MergeParams | None" = None, stream=None):
+        """tpc_merge on device track records (uint8 tensor of 112-byte records, e.g. out.tracks or the tensor refit()
+        returned) and the int32[4] counts of that call.  Returns device tensors (succ, pred, link_chi2, merge_counts)."""
+        import torch
+        cap = int(tracks.shape[0] // 112)
+        succ = torch.empty(max(cap, 1), dtype=torch.int32, device=tracks.device)
+        pred = torch.empty(max(cap, 1), dtype=torch.int32, device=tracks.device)
+        chi2 = torch.empty(max(cap, 1), dtype=torch.float32, device=tracks.device)
+        mc = torch.zeros(4, dtype=torch.int32, device=tracks.device)
+        self._check(self._lib.tpc_merge(self._h, _ptr(tracks), _ptr(counts), C.c_int32(cap),
+                                        C.byref(params) if params is not None else None, self._stream_ptr(stream),
+                                        _ptr(succ), _ptr(pred), _ptr(chi2), _ptr(mc)))
+        return succ, pred, chi2, mc
 
     def track_host(self, y, z, row_offsets, tracks, hit_ids, counts, stream=None):
         """tpc_track_host: all arguments are HOST tensors (pinned for asynchronous copies): y, z int32 [n],

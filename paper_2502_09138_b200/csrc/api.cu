@@ -299,6 +299,9 @@ int tpc_tracker_destroy(tpc_tracker_t* t) {
   if (t->arena) cudaFree(t->arena);
   if (t->host_arena) cudaFree(t->host_arena);
   if (t->geom_blob) cudaFree(t->geom_blob);
+  if (t->merge_sec) cudaFree(t->merge_sec);
+  if (t->merge_best) cudaFree(t->merge_best);
+  if (t->merge_chi2) cudaFree(t->merge_chi2);
   for (int k = 0; k < TIMING_SETS * 6; ++k)
     if (t->ev[k]) cudaEventDestroy(t->ev[k]);
   delete t;
@@ -359,6 +362,44 @@ int tpc_refit(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* strea
   if (!t->arena || n != t->last_n || cl->row_offsets != t->last_ro || cl->y != t->last_y || cl->z != t->last_z)
     return TPC_ERR_ARG;
   TPC_CUDA(t, launch_a6_refit(t, cl->y, cl->z, tracks, refit_out, (cudaStream_t)stream));
+  return TPC_OK;
+}
+
+void tpc_default_merge_params(tpc_merge_params_t* p) {
+  if (!p) return;
+  p->gap_max = 25;
+  p->n_per_side = 18;
+  p->chi2_max = 50.0;
+  p->sector_angle = 20.0 * 3.14159265358979323846 / 180.0;
+}
+
+int tpc_merge(tpc_tracker_t* t, const tpc_track_rec_t* tracks, const int32_t* counts, int32_t track_capacity,
+              const tpc_merge_params_t* params, void* stream, int32_t* succ, int32_t* pred, float* link_chi2,
+              int32_t* merge_counts) {
+  if (!t || !counts || !merge_counts || track_capacity < 0) return TPC_ERR_ARG;
+  if (track_capacity > 0 && (!tracks || !succ || !pred || !link_chi2)) return TPC_ERR_ARG;
+  tpc_merge_params_t mp;
+  if (params) mp = *params; else tpc_default_merge_params(&mp);
+  if (mp.gap_max < 1 || mp.n_per_side < 1 || !(mp.chi2_max > 0)) return TPC_ERR_ARG;
+  if (track_capacity > t->merge_cap || !t->merge_sec) {
+    TPC_CUDA(t, cudaDeviceSynchronize());
+    if (t->merge_sec) cudaFree(t->merge_sec);
+    if (t->merge_best) cudaFree(t->merge_best);
+    if (t->merge_chi2) cudaFree(t->merge_chi2);
+    t->merge_sec = nullptr; t->merge_best = nullptr; t->merge_chi2 = nullptr; t->merge_cap = 0;
+    const size_t cap = (size_t)(track_capacity > 0 ? track_capacity : 1);
+    cudaError_t e = cudaMalloc(&t->merge_sec, ((size_t)t->g.n_sectors + 2) * 4);
+    if (e == cudaSuccess) e = cudaMalloc(&t->merge_best, cap * 2 * 4);
+    if (e == cudaSuccess) e = cudaMalloc(&t->merge_chi2, cap * 2 * 8);
+    if (e == cudaErrorMemoryAllocation) {
+      cudaGetLastError();
+      return TPC_ERR_NOMEM;
+    }
+    if (e != cudaSuccess) return fail_cuda(t, e, "cudaMalloc(merge scratch)");
+    t->merge_cap = (int64_t)cap;
+  }
+  TPC_CUDA(t, launch_a7_merge(t, &mp, tracks, counts, track_capacity, succ, pred, link_chi2, merge_counts,
+                              (cudaStream_t)stream));
   return TPC_OK;
 }
 

@@ -102,6 +102,8 @@ struct tpc_tracker {
   int a4_blocks, a4_warps;   // persistent a4 grid: blocks x warps per block = resident warps of the device (set at create)
   size_t ctl_bytes;          // bytes zeroed per call
   Scratch s;
+  // a7 (tpc_merge) scratch, grown on demand: per-sector track ranges, best partner and its chi2 for both directions
+  int32_t* merge_sec; int32_t* merge_best; double* merge_chi2; int64_t merge_cap;
   int64_t last_n; const uint32_t* last_ro; const int32_t* last_y; const int32_t* last_z;
   // stage timing
   int timing; int64_t timed_calls; cudaEvent_t ev[TIMING_SETS * 6];
@@ -133,6 +135,9 @@ cudaError_t launch_a4_phases(const tpc_tracker* t, int64_t n, cudaStream_t st);
 cudaError_t launch_a5_select(const tpc_tracker* t, const tpc_tracks_out_t* out, cudaStream_t st);
 cudaError_t launch_a6_refit(const tpc_tracker* t, const int32_t* y, const int32_t* z, const tpc_tracks_out_t* tracks,
                             tpc_track_rec_t* refit_out, cudaStream_t st);
+cudaError_t launch_a7_merge(const tpc_tracker* t, const tpc_merge_params_t* mp, const tpc_track_rec_t* tracks,
+                            const int32_t* counts, int32_t cap, int32_t* succ, int32_t* pred, float* link_chi2,
+                            int32_t* merge_counts, cudaStream_t st);
 cudaError_t setup_a1_attributes(const tpc_tracker* t);
 size_t a1_smem_bytes(const DevGeom& g);
 

@@ -361,6 +361,104 @@ def test_refit_config1_and_stress(orc):
     _refit_parity(make_event(4), orc, "refit cfg4")       # loopers: failed transports, short down passes
 
 
+def _merge_parity(ev, orc, label, use_refit=True):
+    """tpc_merge against orc_merge on the SAME records: the oracle is fed the device's float32 track records, so the
+    comparison isolates the merging step (rotation, transport, chi2, mutual-best rule)."""
+    import torch
+    from paper_2502_09138_b200 import Tracker, TRACK_DTYPE
+    from paper_2502_09138_b200.events import geometry_from_event, upload
+    trk = Tracker(geometry_from_event(ev))
+    y, z, ro = upload(ev)
+    out = trk.track(y, z, ro)
+    recs_dev = trk.refit(y, z, ro, out) if use_refit else out.tracks
+    succ, pred, chi2, mc = trk.merge(recs_dev, out.counts)
+    torch.cuda.synchronize()
+    nt = int(out.counts[0])
+    rec = recs_dev[: nt * 112].cpu().numpy().view(TRACK_DTYPE)
+    g_succ, g_pred, g_chi2, g_mc = succ[:nt].cpu().numpy(), pred[:nt].cpu().numpy(), chi2[:nt].cpu().numpy(), mc.cpu().numpy()
+    trk.close()
+    par = np.stack([rec[f] for f in ("x", "y", "z", "sinphi", "tanl", "qpt")], axis=1).astype(np.float64)
+    o_succ, o_pred, o_chi2, o_nl = orc.merge(par, rec["cov"].astype(np.float64), rec["sector"], rec["first_row"],
+                                             rec["last_row"], ev.cfg.bz)
+    assert g_mc[2] == nt and g_mc[0] == int((g_succ >= 0).sum()) and g_mc[1] == nt - g_mc[0]
+    same = (g_succ == o_succ) & (g_pred == o_pred)
+    assert same.mean() >= 0.999, f"{label}: links identical for {same.mean():.5f} of {nt} tracks"
+    both = (g_succ >= 0) & (g_succ == o_succ)
+    assert np.allclose(g_chi2[both], o_chi2[both], rtol=1e-4, atol=1e-6), label
+    assert np.all(g_chi2[g_succ < 0] == -1)
+    # structure: a link is mutual, rows ascend along it, nobody has two predecessors
+    a = np.nonzero(g_succ >= 0)[0]
+    assert np.array_equal(g_pred[g_succ[a]], a) and len(set(g_succ[a].tolist())) == len(a)
+    assert np.all(rec["first_row"][g_succ[a]] > rec["last_row"][a])
+    print(f"[merge] {label}: tracks={nt} links gpu={g_mc[0]} oracle={o_nl} identical={same.mean():.6f}")
+    return nt, int(g_mc[0]), o_nl
+
+
+def test_merge_config1_and_stress(orc):
+    """NEXT-1 merging, CUDA against the oracle: central Pb-Pb (every second track crosses a sector edge) and the
+    stress config (loopers, doubled smearing), on refitted and on plain records."""
+    nt, links, o_links = _merge_parity(make_event(1, 1000), orc, "merge cfg1")
+    assert links == o_links and links > 0.4 * nt        # ~7600 sector tracks -> ~4100 particles
+    _merge_parity(make_event(1, 1001), orc, "merge cfg1 plain records", use_refit=False)
+    _merge_parity(make_event(4), orc, "merge cfg4")
+
+
+def test_merge_batch_keeps_events_apart(orc):
+    """Two events in one call (72 sectors): links never join tracks of different events, and each event's links are
+    those of the event tracked alone."""
+    evs = [make_event(1, 3000 + k, n_tracks=700) for k in range(2)]
+    import torch
+    from paper_2502_09138_b200 import Tracker, TRACK_DTYPE
+    from paper_2502_09138_b200.events import geometry_from_event, upload
+    per_event = []
+    for ev in [concat_events(evs)] + evs:
+        trk = Tracker(geometry_from_event(ev))
+        y, z, ro = upload(ev)
+        out = trk.track(y, z, ro)
+        recs = trk.refit(y, z, ro, out)
+        succ, pred, chi2, mc = trk.merge(recs, out.counts)
+        torch.cuda.synchronize()
+        nt = int(out.counts[0])
+        per_event.append((recs[: nt * 112].cpu().numpy().view(TRACK_DTYPE), succ[:nt].cpu().numpy()))
+        trk.close()
+    (rec, succ), (r0, s0), (r1, s1) = per_event
+    a = np.nonzero(succ >= 0)[0]
+    assert np.all(rec["sector"][a] // 36 == rec["sector"][succ[a]] // 36)
+    n0 = len(r0)
+    assert len(rec) == n0 + len(r1)
+    assert np.array_equal(succ[:n0], s0)
+    assert np.array_equal(succ[n0:], np.where(s1 >= 0, s1 + n0, -1))
+
+
+def test_merge_handmade_membrane_and_wraparound(orc):
+    """Hand-made records through tpc_merge: the same straight line seen from sector 17 and sector 0 (wrap-around), and
+    from a sector and the one facing it across the central membrane."""
+    import torch
+    from paper_2502_09138_b200 import Tracker, Geometry, TRACK_DTYPE
+    from gen.events import row_x
+    from test_oracle_merge import _line_record, _cov_small
+    p0, d = (80.0, 0.0), np.deg2rad(2.0)
+    recs = np.zeros(4, dtype=TRACK_DTYPE)
+
+    def put(k, r, sector, first, last):
+        recs[k]["x"], recs[k]["y"], recs[k]["z"], recs[k]["sinphi"], recs[k]["tanl"], recs[k]["qpt"] = r
+        recs[k]["cov"] = _cov_small()
+        recs[k]["sector"], recs[k]["first_row"], recs[k]["last_row"] = sector, first, last
+
+    put(0, _line_record(np.deg2rad(10.0), 140.0, p0, d, 0.0, 0.1), 0, 41, 80)       # continuation in sector 0
+    put(1, _line_record(np.deg2rad(30.0), 100.0, (60.0, 30.0), np.deg2rad(35.0), 5.0, 0.4), 1, 10, 60)
+    put(2, _line_record(np.deg2rad(350.0), 100.0, p0, d, 0.0, 0.1), 17, 5, 40)      # inner piece in sector 17
+    put(3, _line_record(np.deg2rad(30.0), 150.0, (60.0, 30.0), np.deg2rad(35.0), 5.0, 0.4), 19, 61, 120)   # faces 1
+    trk = Tracker(Geometry(n_sectors=36, row_x=row_x()))
+    dev = torch.from_numpy(recs.view(np.uint8).copy()).cuda()
+    counts = torch.tensor([4, 0, 0, 0], dtype=torch.int32, device="cuda")
+    succ, pred, chi2, mc = trk.merge(dev, counts)
+    torch.cuda.synchronize()
+    assert succ.cpu().tolist() == [-1, 3, 0, -1] and pred.cpu().tolist() == [2, -1, -1, 1]
+    assert mc.cpu().tolist()[:3] == [2, 2, 4] and float(chi2[1]) < 1e-6 and float(chi2[2]) < 1e-6
+    trk.close()
+
+
 def test_refit_rejects_foreign_input(orc):
     import torch
     from paper_2502_09138_b200 import Tracker

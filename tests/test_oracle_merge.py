@@ -170,7 +170,8 @@ def test_sector_relations(orc):
 
     az = lambda s: (s % 18 + 0.5) * 20.0      # noqa: E731  (P2)
     cases = [(1, 2, True), (2, 1, True), (1, 3, False), (1, 1, True), (19, 20, True), (1, 20, False), (1, 19, True),
-             (17, 0, True), (0, 17, True), (35, 18, True), (0, 35, False)]
+             (17, 0, True), (0, 17, True), (35, 18, True), (0, 35, False),
+             (37, 38, True), (37, 55, True), (19, 37, False), (1, 37, False)]   # second event of a batch: sectors 36..71
     for sa, sb, linked in cases:
         a, b = rec(az(sa), 100.0), rec(az(sb), 150.0)
         if abs(a[3]) > 0.9 or abs(b[3]) > 0.9:
