@@ -183,12 +183,25 @@ def run_ours(args):
     y, z, ro = upload(ev, dev)
     main = torch.cuda.current_stream()
     sweep = [args.streams] if args.streams > 0 else [1, 2, 3, 4]   # K handles/streams, best reported
+    if args.profile:
+        sweep = [1]
     handles = []
     for k in range(max(sweep)):
         t = Tracker(geometry_from_event(ev))
+        t.set_a2_variant(args.a2_variant)
         handles.append({"trk": t, "stream": main if k == 0 else torch.cuda.Stream(dev), "y": y, "z": z, "ro": ro,
                         "out": t.alloc_out(n, track_capacity=n // 40 + 1024, hit_capacity=n + 1024)})
     trk, out = handles[0]["trk"], handles[0]["out"]
+
+    if args.profile:   # for ncu: W warm-up calls + K calls on one stream, nothing else (see profiles/*.md)
+        for _ in range(args.warmup + args.steps):
+            trk.track(y, z, ro, out, main)
+        torch.cuda.synchronize()
+        print(json.dumps({"profile_run": True, "calls": args.warmup + args.steps, "launches_per_call": trk.launches_per_call(),
+                          "clusters_per_call": n, "batch_events": B}))
+        for h in handles:
+            h["trk"].close()
+        return
 
     # ---- device-resident arm: no stage events, no host work inside the timed region ------------------------
     for h in handles:
@@ -489,6 +502,8 @@ def main():
     ap.add_argument("--streams", type=int, default=0, help="handles/streams of the device arm; 0 = sweep 1..4")
     ap.add_argument("--e2e-threads", type=int, default=3, help="host threads (handles, streams) of the e2e arm")
     ap.add_argument("--selftest-ranks", action="store_true", help="CPU check of the multi-rank plumbing (gloo)")
+    ap.add_argument("--a2-variant", type=int, default=0, help="0 = direct a2 (default), 1 = TMA-staged rows (evidence run)")
+    ap.add_argument("--profile", action="store_true", help="only W + K tpc_track calls on one stream (for ncu)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:   # not under torchrun: start the replica ranks here

@@ -191,6 +191,9 @@ int tpc_get_stage_ms_mean(tpc_tracker_t* t, float ms[5], int32_t* n_calls);
 /* ---- test-only: a4 has two variants that compute the same thing (phase kernels for large calls, one uniform
  * kernel for small ones).  0 = choose by call size (default), 1 = uniform, 2 = phased. */
 int tpc_debug_set_a4_variant(tpc_tracker_t* t, int variant);
+/* a2 on sparse calls: 0 = rows read through L1/L2 (default), 1 = rows staged in shared memory by TMA bulk copies, a
+ * CTA sliding a three-row window over 19 rows (north_star's sketch; same links; profiles/r02_a2_staged.md). */
+int tpc_debug_set_a2_variant(tpc_tracker_t* t, int variant);
 
 /* ---- test-only exports: intermediate results of the most recent tpc_track call on this handle ----
  * All outputs are [device] buffers in id space (-1 = none), written asynchronously on `stream`. */

@@ -117,6 +117,7 @@ def load_library():
     lib.tpc_launches_per_call.argtypes = [C.c_void_p]
     lib.tpc_reserve_seeds.argtypes = [C.c_void_p, C.c_int64]
     lib.tpc_debug_set_a4_variant.argtypes = [C.c_void_p, C.c_int]
+    lib.tpc_debug_set_a2_variant.argtypes = [C.c_void_p, C.c_int]
     lib.tpc_set_stage_timing.argtypes = [C.c_void_p, C.c_int]
     lib.tpc_get_stage_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
     lib.tpc_get_stage_ms_mean.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_int32)]
@@ -325,6 +326,10 @@ class Tracker:
     def set_a4_variant(self, variant: int):
         """tpc_debug_set_a4_variant: 0 = by call size, 1 = uniform kernel, 2 = phase kernels (tests)."""
         self._check(self._lib.tpc_debug_set_a4_variant(self._h, C.c_int(int(variant))))
+
+    def set_a2_variant(self, variant: int):
+        """tpc_debug_set_a2_variant: 0 = direct, 1 = rows staged in shared memory by TMA bulk copies."""
+        self._check(self._lib.tpc_debug_set_a2_variant(self._h, C.c_int(int(variant))))
 
     def debug_seeds(self, n: int, n_seeds: int):
         import torch

@@ -173,6 +173,46 @@ __device__ __forceinline__ uint32_t side_mask(const DevGeom& g, const int4* __re
   return m;
 }
 
+// Best pair of one cluster through the window masks.  su / sd: where the up / down row's records are read from,
+// indexed by GLOBAL sorted position (the direct kernel passes srt for both; the staged kernel passes shared-memory
+// copies of the two rows, biased by the rows' first positions); srt: the global array (rare paths: ids on cost ties,
+// more than 32 range clusters on a side).
+__device__ __forceinline__ Best mask_best_pair(const DevGeom& g, const int4* __restrict__ srt, const int4* su,
+                                               const int4* sd, const uint32_t* bs_u, const uint32_t* bs_d, int yh,
+                                               int zh, int org_z) {
+  Best b = {INT32_MAX, -1, -1};
+  const Window w = window_bins(g, yh, zh, org_z);
+  const Ranges qu = load_ranges(g, w, bs_u), qd = load_ranges(g, w, bs_d);
+  const uint32_t nu0 = qu.b0 - qu.a0, nu = nu0 + (qu.b1 - qu.a1);
+  const uint32_t nd0 = qd.b0 - qd.a0, nd = nd0 + (qd.b1 - qd.a1);
+  if (nu > 32u || nd > 32u) {
+    pair_search_nested<false>(g, srt, w, bs_u, bs_d, yh, zh, b);
+  } else if (nu && nd) {
+    const uint32_t mu = side_mask(g, su, qu, nu0, nu, yh, zh);
+    const uint32_t md = mu ? side_mask(g, sd, qd, nd0, nd, yh, zh) : 0u;
+    if (md) {
+      for (uint32_t bu = mu; bu; bu &= bu - 1u) {
+        const uint32_t pu = range_at(qu, nu0, (uint32_t)__ffs((int)bu) - 1u);
+        const int4 cu = su[pu];
+        const int dyu = cu.x - yh, dzu = cu.y - zh, idu = cu.z;
+        for (uint32_t bd = md; bd; bd &= bd - 1u) {
+          const uint32_t pd = range_at(qd, nd0, (uint32_t)__ffs((int)bd) - 1u);
+          const int4 cd = sd[pd];
+          const int ddy = dyu + (cd.x - yh), ddz = dzu + (cd.y - zh);
+          const int cost = g.cost_wy * ddy * ddy + g.cost_wz * ddz * ddz;   // P8
+          if (cost < b.cost || (cost == b.cost && tie_wins(srt, b, idu, cd.z))) {   // P9
+            b.cost = cost;
+            b.pu = (int)pu;
+            b.pd = (int)pd;
+          }
+        }
+      }
+    }
+  }
+  if (b.pu < 0 || b.cost > g.c_max) b.pu = b.pd = -1;   // P10
+  return b;
+}
+
 // 16 CTAs of 128 threads per SM (32 registers): the kernel hides its gathers with resident warps
 __global__ void __launch_bounds__(A2_THREADS, 16)
 a2_neighbours_mask_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, const uint32_t* __restrict__ ro, const int4* __restrict__ srt,
@@ -191,41 +231,134 @@ a2_neighbours_mask_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, const
   }
   for (uint32_t j = a + threadIdx.x; j < b; j += A2_THREADS) {
     const int4 ch = srt[j];
-    const int yh = ch.x, zh = ch.y;
-    Best b = {INT32_MAX, -1, -1};
-    if (inner) {
-      const Window w = window_bins(g, yh, zh, org_z);
-      const Ranges qu = load_ranges(g, w, bs_u), qd = load_ranges(g, w, bs_d);
-      const uint32_t nu0 = qu.b0 - qu.a0, nu = nu0 + (qu.b1 - qu.a1);
-      const uint32_t nd0 = qd.b0 - qd.a0, nd = nd0 + (qd.b1 - qd.a1);
-      if (nu > 32u || nd > 32u) {
-        pair_search_nested<false>(g, srt, w, bs_u, bs_d, yh, zh, b);
-      } else if (nu && nd) {
-        const uint32_t mu = side_mask(g, srt, qu, nu0, nu, yh, zh);
-        const uint32_t md = mu ? side_mask(g, srt, qd, nd0, nd, yh, zh) : 0u;
-        if (md) {
-          for (uint32_t bu = mu; bu; bu &= bu - 1u) {
-            const uint32_t pu = range_at(qu, nu0, (uint32_t)__ffs((int)bu) - 1u);
-            const int4 cu = srt[pu];
-            const int dyu = cu.x - yh, dzu = cu.y - zh, idu = cu.z;
-            for (uint32_t bd = md; bd; bd &= bd - 1u) {
-              const uint32_t pd = range_at(qd, nd0, (uint32_t)__ffs((int)bd) - 1u);
-              const int4 cd = srt[pd];
-              const int ddy = dyu + (cd.x - yh), ddz = dzu + (cd.y - zh);
-              const int cost = g.cost_wy * ddy * ddy + g.cost_wz * ddz * ddz;   // P8
-              if (cost < b.cost || (cost == b.cost && tie_wins(srt, b, idu, cd.z))) {   // P9
-                b.cost = cost;
-                b.pu = (int)pu;
-                b.pd = (int)pd;
-              }
-            }
-          }
-        }
-      }
-      if (b.pu < 0 || b.cost > g.c_max) b.pu = b.pd = -1;   // P10
+    Best bp = {INT32_MAX, -1, -1};
+    if (inner) bp = mask_best_pair(g, srt, srt, srt, bs_u, bs_d, ch.x, ch.y, org_z);
+    link_up[j] = bp.pu;
+    link_dn[j] = bp.pd;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// north_star's a2: "stages the r-1 / r+1 row grids in shared memory via TMA".  A CTA owns A2S_ROWS consecutive rows of
+// one sector and slides a three-row window over them: every row's cluster records and bin starts are copied into a
+// four-slot shared-memory ring ONCE, by 1-D bulk copies (cp.async.bulk, completion on an mbarrier), two rows ahead
+// of their use, and serve as down row, own row and up row in turn.  Rows that do not fit a slot are read from global
+// memory through the same pointers.  Same arithmetic (mask_best_pair), same links; which of the two kernels a call
+// runs is decided in launch_a2_neighbours from the measurement in profiles/r02_a2_staged.md.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int A2S_ROWS = 19;       // rows per CTA (152 = 8 x 19); two extra rows are staged per CTA
+constexpr int A2S_RING = 4;
+constexpr int A2S_ROWCAP = 320;    // records per slot (5 KB); longer rows stay in global memory
+constexpr int A2S_BINCAP = 1024;   // bin starts per slot (4 KB)
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase) {
+  asm volatile(
+      "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n"
+      " bra WAIT_%=;\n DONE_%=:\n}" ::"r"(smem_u32(bar)), "r"(phase) : "memory");
+}
+// 1-D bulk copy global -> shared (TMA without a tensor map): 16-byte aligned addresses, size a multiple of 16
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+__global__ void __launch_bounds__(A2_THREADS)
+a2_neighbours_staged_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, const uint32_t* __restrict__ ro,
+                            const int4* __restrict__ srt, const uint32_t* __restrict__ sec_key,
+                            const uint32_t* __restrict__ bin_start, int32_t* __restrict__ link_up,
+                            int32_t* __restrict__ link_dn) {
+  __shared__ __align__(128) int4 s_rec[A2S_RING][A2S_ROWCAP];
+  __shared__ __align__(128) uint32_t s_bin[A2S_RING][A2S_BINCAP];
+  __shared__ __align__(8) uint64_t s_bar[A2S_RING];
+  __shared__ uint32_t s_a[A2S_RING], s_b[A2S_RING];      // position range of the row in each slot
+  __shared__ int s_staged[A2S_RING];                      // the slot holds a copy (else: read global memory)
+  __shared__ uint32_t s_uses[A2S_RING], s_phase[A2S_RING];   // copies issued into the slot so far; parity to wait for
+  if (ctl->bad_offsets) return;
+  const int nr = g.n_rows;
+  const int chunks = (nr + A2S_ROWS - 1) / A2S_ROWS;
+  const int sec = blockIdx.x / chunks, chunk = blockIdx.x % chunks;
+  const int r_lo = chunk * A2S_ROWS, r_hi = min(r_lo + A2S_ROWS, nr);   // rows [r_lo, r_hi)
+  const int org_z = zmin_from_key(sec_key[sec]);
+  const int64_t sr0 = (int64_t)sec * nr;
+  const bool bins_fit = g.nb_stride <= A2S_BINCAP;
+  if (threadIdx.x == 0) {
+    for (int k = 0; k < A2S_RING; ++k) {
+      mbar_init(&s_bar[k], 1);
+      s_uses[k] = 0;
     }
-    link_up[j] = b.pu;
-    link_dn[j] = b.pd;
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  // thread 0 stages row `row` (any row of the sector, or nothing outside it) into slot row & 3
+  auto stage = [&](int row) {
+    const int slot = row & (A2S_RING - 1);
+    if (row < 0 || row >= nr) {
+      s_staged[slot] = 0;
+      s_a[slot] = s_b[slot] = 0;
+      return;
+    }
+    const uint32_t a = ro[sr0 + row], b = ro[sr0 + row + 1];
+    s_a[slot] = a;
+    s_b[slot] = b;
+    const bool fit = bins_fit && b - a <= (uint32_t)A2S_ROWCAP;
+    s_staged[slot] = fit ? 1 : 0;
+    if (fit) {
+      const uint32_t bytes_rec = (b - a) * 16u, bytes_bin = (uint32_t)g.nb_stride * 4u;
+      s_phase[slot] = s_uses[slot] & 1u;   // the mbarrier's phase flips once per completed copy into this slot
+      ++s_uses[slot];
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier reads of the slot precede the copy
+      mbar_expect_tx(&s_bar[slot], bytes_rec + bytes_bin);
+      if (bytes_rec) bulk_g2s(&s_rec[slot][0], srt + a, bytes_rec, &s_bar[slot]);
+      bulk_g2s(&s_bin[slot][0], bin_start + (size_t)(sr0 + row) * g.nb_stride, bytes_bin, &s_bar[slot]);
+    }
+  };
+  if (threadIdx.x == 0) {
+    stage(r_lo - 1);
+    stage(r_lo);
+    stage(r_lo + 1);
+  }
+  __syncthreads();
+  for (int r = r_lo; r < r_hi; ++r) {
+    if (threadIdx.x == 0 && r + 2 <= r_hi) stage(r + 2);   // two rows ahead; its slot was the down row of row r - 1
+    __syncthreads();                                        // s_a / s_b / s_staged of the new slot are visible
+    const int sc = r & 3, su_ = (r + 1) & 3, sd_ = (r - 1) & 3;
+    const bool inner = r >= 1 && r <= nr - 2;               // P5
+    const uint32_t a = s_a[sc], b = s_b[sc];
+    auto wait_slot = [&](int row) {
+      const int slot = row & 3;
+      if (row >= 0 && row < nr && s_staged[slot]) mbar_wait(&s_bar[slot], s_phase[slot]);
+    };
+    wait_slot(r - 1);
+    wait_slot(r);
+    wait_slot(r + 1);
+    // pointers indexed by global sorted position: the shared copy biased by the row's first position, or srt itself
+    const int4* pc = s_staged[sc] ? &s_rec[sc][0] - a : srt;
+    const int4* pu = srt;
+    const int4* pd = srt;
+    const uint32_t *bs_u = nullptr, *bs_d = nullptr;
+    if (inner) {
+      pu = s_staged[su_] ? &s_rec[su_][0] - s_a[su_] : srt;
+      pd = s_staged[sd_] ? &s_rec[sd_][0] - s_a[sd_] : srt;
+      bs_u = s_staged[su_] ? &s_bin[su_][0] : bin_start + (size_t)(sr0 + r + 1) * g.nb_stride;
+      bs_d = s_staged[sd_] ? &s_bin[sd_][0] : bin_start + (size_t)(sr0 + r - 1) * g.nb_stride;
+    }
+    for (uint32_t j = a + threadIdx.x; j < b; j += A2_THREADS) {
+      const int4 ch = pc[j];
+      Best bp = {INT32_MAX, -1, -1};
+      if (inner) bp = mask_best_pair(g, srt, pu, pd, bs_u, bs_d, ch.x, ch.y, org_z);
+      link_up[j] = bp.pu;
+      link_dn[j] = bp.pd;
+    }
+    __syncthreads();   // everybody is done with the down row's slot before it is staged again
   }
 }
 
@@ -334,7 +467,10 @@ cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64
   if (dense && fine) a2_neighbours_dense_kernel<true><<<grid2, A2_THREADS, 0, st>>>(A2_ARGS);
   else if (dense) a2_neighbours_dense_kernel<false><<<grid2, A2_THREADS, 0, st>>>(A2_ARGS);
   else if (fine) a2_neighbours_kernel<true><<<(unsigned)R, A2_THREADS, 0, st>>>(A2_ARGS);
-  else a2_neighbours_mask_kernel<<<(unsigned)R, A2_THREADS, 0, st>>>(A2_ARGS);
+  else if (t->a2_variant == 1) {
+    const int chunks = (t->g.n_rows + A2S_ROWS - 1) / A2S_ROWS;
+    a2_neighbours_staged_kernel<<<(unsigned)(t->g.n_sectors * chunks), A2_THREADS, 0, st>>>(A2_ARGS);
+  } else a2_neighbours_mask_kernel<<<(unsigned)R, A2_THREADS, 0, st>>>(A2_ARGS);
 #undef A2_ARGS
   return cudaGetLastError();
 }

@@ -472,6 +472,12 @@ int tpc_reserve_seeds(tpc_tracker_t* t, int64_t n_seeds) {
   return TPC_OK;
 }
 
+int tpc_debug_set_a2_variant(tpc_tracker_t* t, int variant) {
+  if (!t || variant < 0 || variant > 1) return TPC_ERR_ARG;
+  t->a2_variant = variant;
+  return TPC_OK;
+}
+
 int tpc_debug_set_a4_variant(tpc_tracker_t* t, int variant) {
   if (!t || variant < 0 || variant > 2) return TPC_ERR_ARG;
   t->a4_variant = variant;

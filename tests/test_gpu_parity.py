@@ -13,12 +13,13 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-4
 
 
-def _run_gpu(ev, params=None, a4_variant=0):
+def _run_gpu(ev, params=None, a4_variant=0, a2_variant=0):
     import torch
     from paper_2502_09138_b200 import Tracker
     from paper_2502_09138_b200.events import geometry_from_event, upload
     trk = Tracker(geometry_from_event(ev, params))
     trk.set_a4_variant(a4_variant)
+    trk.set_a2_variant(a2_variant)
     y, z, ro = upload(ev)
     out = trk.track(y, z, ro)
     tracks, hit_ids, ns = out.to_host()
@@ -481,6 +482,23 @@ def test_both_a4_variants_on_small_and_stress_events(orc, mode):
     for ev, lab in ((make_event(0), "cfg0"), (make_event(1, 1001), "cfg1"), (make_event(4), "cfg4"),
                     (make_event(2, collisions=6), "cfg2/6")):
         compare(ev, orc, _run_gpu(ev, a4_variant=variant), orc.track(ev), label=f"{lab} a4={mode}")
+
+
+def test_a2_staged_variant_gives_the_same_links(orc):
+    """a2 with the neighbour rows staged in shared memory by TMA bulk copies (north_star's sketch): bit-exact links on a
+    sparse event, on a 40-row geometry (chunks of 19 rows with a ragged tail), on rows longer than a staging slot
+    (those fall back to global memory) and on an event with empty rows."""
+    from gen.events import Config
+    ev = make_event(1, 1002)
+    compare(ev, orc, _run_gpu(ev, a2_variant=1), orc.track(ev), label="a2 staged cfg1")
+    cfg = Config("one_sector_40_rows", n_sectors=1, open_sector=True, tracks_per_collision=1500, pt_min=0.3,
+                 noise=0.05, n_rows=40)
+    ev = make_event(cfg, seed=7)                      # ~1500 clusters per row: no row fits a slot
+    compare(ev, orc, _run_gpu(ev, a2_variant=1), orc.track(ev), label="a2 staged long rows")
+    ev = make_event(0)
+    compare(ev, orc, _run_gpu(ev, a2_variant=1), orc.track(ev), label="a2 staged cfg0")
+    ev = make_event(1, 77, n_tracks=40)               # very sparse: many empty rows
+    compare(ev, orc, _run_gpu(ev, a2_variant=1), orc.track(ev), label="a2 staged empty rows")
 
 
 def test_edge_empty_and_tiny(orc):
