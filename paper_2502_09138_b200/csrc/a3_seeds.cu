@@ -114,11 +114,14 @@ a3_seeds_kernel(const DevGeom g, int64_t n, const uint32_t* __restrict__ ro, con
 // P14: seed rank = ascending start id.  seed_tmp is in position order; the seeds of one (sector,row) are adjacent in
 // it and fill the same rank range in both orders.
 __global__ void __launch_bounds__(256)
-a3_rank_kernel(const DevCtl* __restrict__ ctl, const int4* __restrict__ seed_tmp, int32_t* __restrict__ seed_start,
-               int32_t* __restrict__ seed_pos, int32_t* __restrict__ seed_sr) {
+a3_rank_kernel(const DevCtl* __restrict__ ctl, const int4* __restrict__ seed_tmp, const int4* __restrict__ srt,
+               int32_t* __restrict__ seed_start, int32_t* __restrict__ seed_pos, int32_t* __restrict__ seed_sr,
+               int4* __restrict__ seed_rec) {
   const int64_t ns = ctl->n_seeds;
   for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < ns; k += (int64_t)gridDim.x * blockDim.x) {
     const int4 me = seed_tmp[k];
+    const int4 c0 = srt[me.x];     // the seed's first cluster and (requested before the counting loops) its second
+    const int4 c1 = srt[c0.w];
     int64_t left = 0, smaller = 0;
     for (int64_t j = k - 1; j >= 0; --j) {
       const int4 o = seed_tmp[j];
@@ -135,6 +138,9 @@ a3_rank_kernel(const DevCtl* __restrict__ ctl, const int4* __restrict__ seed_tmp
     seed_start[rank] = me.y;
     seed_pos[rank] = me.x;
     seed_sr[rank] = me.z;
+    // everything a4 needs to start the tracklet, in one 32-byte record: (sr, y0, z0, id0) (up0, y1, z1, -)
+    seed_rec[2 * rank] = make_int4(me.z, c0.x, c0.y, c0.z);
+    seed_rec[2 * rank + 1] = make_int4(c0.w, c1.x, c1.y, 0);
   }
 }
 
@@ -148,6 +154,7 @@ cudaError_t launch_a3_seeds(const tpc_tracker* t, const uint32_t* ro, int64_t n,
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   // the seed count stays on the device: a grid-stride kernel sized for the device, not for the capacity
-  a3_rank_kernel<<<t->a4_sms * 4, 256, 0, st>>>(t->s.ctl, t->s.seed_tmp, t->s.seed_start, t->s.seed_pos, t->s.seed_sr);
+  a3_rank_kernel<<<t->a4_sms * 8, 256, 0, st>>>(t->s.ctl, t->s.seed_tmp, t->s.srt, t->s.seed_start, t->s.seed_pos,
+                                               t->s.seed_sr, t->s.seed_rec);
   return cudaGetLastError();
 }

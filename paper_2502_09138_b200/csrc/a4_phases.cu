@@ -22,8 +22,7 @@ struct Env {   // everything a warp needs that does not change during a kernel
   const int4* srt;
   const uint32_t* sec_key;
   const uint32_t* bin_start;
-  const int32_t* seed_pos;
-  const int32_t* seed_sr;
+  const int4* seed_rec;
   float4* tl_rec;
   int32_t* tl_hits;
   int2* tl_yz;
@@ -40,6 +39,7 @@ struct Env {   // everything a warp needs that does not change during a kernel
 
 struct Trk {   // per-tracklet constants, recomputed from the seed rank when a lane picks the tracklet up
   int i, id0, y0, z0, up0, sec_base, r0, org_z;   // (y0, z0, id0, up0): the seed's first cluster (its srt record)
+  int y1, z1;     // the seed's second cluster (P19 initial direction); valid in phase A only
   int32_t* tab;   // its row -> hit id table = its final hit list
   int2* yz;       // its row -> (y, z) of the recorded hit: what the downward refit streams
 };
@@ -47,19 +47,20 @@ struct Trk {   // per-tracklet constants, recomputed from the seed rank when a l
 __device__ __forceinline__ Trk trk_of(const Env& e, int i) {
   Trk t;
   t.i = i;
-  const int h0 = e.seed_pos[i];
-  const int sr = e.seed_sr[i];
+  const int4 q0 = e.seed_rec[2 * i], q1 = e.seed_rec[2 * i + 1];   // one 32-byte sector (a3_rank_kernel)
+  const int sr = q0.x;
   const int sec = sr / e.g.n_rows;
   t.sec_base = sec * e.g.n_rows;
   t.r0 = sr - t.sec_base;
   t.org_z = zmin_from_key(e.sec_key[sec]);
   t.tab = e.tl_hits + (size_t)i * e.g.n_rows;
   t.yz = e.tl_yz + (size_t)i * e.yz_stride;
-  const int4 c0 = e.srt[h0];
-  t.y0 = c0.x;
-  t.z0 = c0.y;
-  t.id0 = c0.z;
-  t.up0 = c0.w;
+  t.y0 = q0.y;
+  t.z0 = q0.z;
+  t.id0 = q0.w;
+  t.up0 = q1.x;
+  t.y1 = q1.y;
+  t.z1 = q1.z;
   return t;
 }
 
@@ -95,6 +96,7 @@ __device__ __forceinline__ void state_load(const Env& e, int i, Trk& t, State& p
   t.tab = e.tl_hits + (size_t)i * e.g.n_rows;
   t.yz = e.tl_yz + (size_t)i * e.yz_stride;
   t.id0 = t.up0 = -1;
+  t.y1 = t.z1 = 0;
   C.d0 = f0.x; C.d1 = f0.y; C.d2 = f0.z; C.d3 = f0.w; C.d4 = f1.x; C.u01 = f1.y; C.u02 = f1.z; C.u03 = f1.w;
   C.u04 = f2.x; C.u12 = f2.y; C.u13 = f2.z; C.u14 = f2.w; C.u23 = f3.x; C.u24 = f3.y; C.u34 = f3.z;
   p.y = f3.w; p.z = f4.x; p.s = f4.y; p.t = f4.z; p.q = f4.w;
@@ -204,11 +206,10 @@ __device__ __forceinline__ void phase_a(const Env& e) {
       const uint32_t k = base + (uint32_t)__popc(idle & ((1u << e.lane) - 1u));
       if (want && k < e.n_seeds) {
         t = trk_of(e, (int)k);
-        const int4 c1 = e.srt[t.up0];
         rcn.y = t.y0; rcn.z = t.z0; rcn.id = t.id0; rcn.up = t.up0;
         more = true;
         const float dxr = e.s_row_dx[t.r0];
-        const float dy = (float)(c1.x - t.y0) * g.inv_units, dz = (float)(c1.y - t.z0) * g.inv_units;
+        const float dy = (float)(t.y1 - t.y0) * g.inv_units, dz = (float)(t.z1 - t.z0) * g.inv_units;
         const float ichord = rsqrtf(fmaf(dxr, dxr, dy * dy));
         p.y = 0; p.z = 0; p.s = dy * ichord; p.t = dz * ichord; p.q = 0;
         p.oy = t.y0; p.oz = t.z0;
@@ -579,8 +580,7 @@ template <int PH>
 __global__ void __launch_bounds__(AP_THREADS, ap_min_blocks(PH))
 a4_phase_kernel(const DevGeom g, uint32_t s_cap, DevCtl* __restrict__ ctl, const int4* __restrict__ srt,
                 const uint32_t* __restrict__ sec_key, const uint32_t* __restrict__ bin_start,
-                const int32_t* __restrict__ seed_pos, const int32_t* __restrict__ seed_sr,
-                float4* __restrict__ tl_rec, int32_t* __restrict__ tl_hits, int2* __restrict__ tl_yz,
+                const int4* __restrict__ seed_rec, float4* __restrict__ tl_rec, int32_t* __restrict__ tl_hits, int2* __restrict__ tl_yz,
                 int4* __restrict__ tl_state, uint32_t* __restrict__ q_items, uint32_t* __restrict__ tl_span) {
   extern __shared__ double smem_ap[];
   __shared__ int2 s_yz[4][AP_THREADS];
@@ -597,7 +597,7 @@ a4_phase_kernel(const DevGeom g, uint32_t s_cap, DevCtl* __restrict__ ctl, const
   Env e;
   e.g = g;
   e.ctl = ctl; e.srt = srt; e.sec_key = sec_key; e.bin_start = bin_start;
-  e.seed_pos = seed_pos; e.seed_sr = seed_sr; e.tl_rec = tl_rec; e.tl_hits = tl_hits; e.tl_yz = tl_yz;
+  e.seed_rec = seed_rec; e.tl_rec = tl_rec; e.tl_hits = tl_hits; e.tl_yz = tl_yz;
   e.tl_state = tl_state;
   e.q_items = q_items; e.tl_span = tl_span; e.s_row_x = s_row_x; e.s_row_dx = s_row_dx;
   e.n_seeds = n_seeds; e.s_cap = s_cap;
@@ -620,7 +620,7 @@ cudaError_t launch_a4_phases(const tpc_tracker* t, int64_t n, cudaStream_t st) {
   const size_t smem = (size_t)t->g.n_rows * (8 + 4);
 #define AP_LAUNCH(PH)                                                                                         \
   a4_phase_kernel<PH><<<t->a4_sms * ap_min_blocks(PH), AP_THREADS, smem, st>>>(                                                \
-      t->g, (uint32_t)t->s_cap, t->s.ctl, t->s.srt, t->s.sec_key, t->s.bin_start, t->s.seed_pos, t->s.seed_sr, \
+      t->g, (uint32_t)t->s_cap, t->s.ctl, t->s.srt, t->s.sec_key, t->s.bin_start, t->s.seed_rec,              \
       t->s.tl_rec, t->s.tl_hits, t->s.tl_yz, t->s.tl_state, t->s.q_items, t->s.tl_span)
   AP_LAUNCH(0);
   AP_LAUNCH(1);

@@ -73,6 +73,7 @@ size_t layout(tpc_tracker* t, char* base, int64_t n, int64_t R) {
   s.seed_start = (int32_t*)take((size_t)s_cap * 4);
   s.seed_pos = (int32_t*)take((size_t)s_cap * 4);
   s.seed_sr = (int32_t*)take((size_t)s_cap * 4);
+  s.seed_rec = (int4*)take((size_t)s_cap * 32);
   s.tl_rec = (float4*)take((size_t)s_cap * TL_REC_V4 * 16);
   s.tl_hits = (int32_t*)take((size_t)s_cap * t->g.n_rows * 4);
   s.tl_yz = (int2*)take((size_t)s_cap * ((t->g.n_rows + 3) & ~3) * 8);

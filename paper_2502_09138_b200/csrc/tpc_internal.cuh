@@ -62,6 +62,7 @@ struct Scratch {
   int32_t* seed_start;      // [s_cap] start cluster id, ascending (P14)
   int32_t* seed_pos;        // [s_cap] sorted position of the start cluster
   int32_t* seed_sr;         // [s_cap] sector * n_rows + row of the start cluster
+  int4* seed_rec;           // [s_cap][2] (sr, y0, z0, id0) (up0, y1, z1, -): a tracklet's start in one 32-byte load
   // a4 tracklets, one 96-B record + one row table per seed
   float4* tl_rec;           // [s_cap][6]: (x_ref,y,z,sinphi) (tanl,qpt,chi2,n_hits as int bits) cov[0..3] cov[4..7]
                             //             cov[8..11] (cov[12],cov[13],cov[14],sector*n_rows+first seed row as int bits)
