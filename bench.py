@@ -453,6 +453,49 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def run_config(args):
+    """`--config C`: one event of BASELINE.json configs[C] (30 = the 2 M-cluster reading 3b) per tpc_track call, on one
+    stream: the per-config rows of BASELINE.md section 5.  Not the headline (that is configs[1] x 32 events)."""
+    import torch
+    from gen.events import make_event
+    from paper_2502_09138_b200 import Tracker
+    from paper_2502_09138_b200.events import geometry_from_event, upload
+    ev = make_event(args.config)
+    trk = Tracker(geometry_from_event(ev))
+    y, z, ro = upload(ev)
+    out = trk.alloc_out(ev.n)
+    st = torch.cuda.current_stream()
+    for _ in range(args.warmup):
+        trk.track(y, z, ro, out, st)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(st)
+    for _ in range(args.steps):
+        trk.track(y, z, ro, out, st)
+    e1.record(st)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    trk.set_stage_timing(True)
+    for _ in range(min(args.steps, 8)):
+        trk.track(y, z, ro, out, st)
+    torch.cuda.synchronize()
+    stage_ms, _ = trk.stage_ms_mean()
+    tracks, hit_ids, n_seeds = out.to_host()
+    _, _, _, nh, _ = trk.debug_tracklets(n_seeds)
+    grid = trk.debug_grid(ev.n)
+    sb = stage_bytes(float(ev.n), float(grid["stride"]) * trk.n_sectors * trk.n_rows, float(nh.sum()), float(n_seeds))
+    hbm_peak, peak_kind, _ = read_peaks()
+    gbs = sum(sb.values()) / (ms * 1e-3) / 1e9
+    print(json.dumps({"metric": METRIC, "config": {"workload": f"one event of configs[{args.config}] ({ev.cfg.name}) per call"},
+                      "value": ev.n / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms, "steps": args.steps,
+                      "clusters": ev.n, "seeds": int(n_seeds), "tracks": len(tracks), "tracks_per_s": len(tracks) / (ms * 1e-3),
+                      "alg_bytes_per_cluster": sum(sb.values()) / ev.n, "hbm_gbs": gbs, "hbm_frac_measured": gbs / hbm_peak,
+                      "hbm_frac_8TBs": gbs / 8000.0, "stage_ms": dict(zip(["a1", "a2", "a3", "a4", "a5"], stage_ms)),
+                      "a4_variant": "phases" if trk.launches_per_call() == 12 else "uniform",
+                      "scratch_gb": trk.scratch_bytes() / 1e9}))
+    trk.close()
+
+
 def launch_replicas(args):
     """`python bench.py --gpus N` outside torchrun: start N replica ranks of this script (one per GPU, torchrun's
     environment variables, rendezvous on 127.0.0.1) and pass rank 0's JSON line through."""
@@ -503,6 +546,8 @@ def main():
     ap.add_argument("--e2e-threads", type=int, default=3, help="host threads (handles, streams) of the e2e arm")
     ap.add_argument("--selftest-ranks", action="store_true", help="CPU check of the multi-rank plumbing (gloo)")
     ap.add_argument("--a2-variant", type=int, default=0, help="0 = direct a2 (default), 1 = TMA-staged rows (evidence run)")
+    ap.add_argument("--config", type=int, default=None, choices=[0, 1, 2, 3, 30, 4],
+                    help="time one event of that config per call instead of the headline batch (BASELINE.md section 5)")
     ap.add_argument("--profile", action="store_true", help="only W + K tpc_track calls on one stream (for ncu)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -512,6 +557,8 @@ def main():
         run_selftest_ranks(args)
     elif args.impl == "reference":
         run_reference(args)
+    elif args.config is not None:
+        run_config(args)
     else:
         run_ours(args)
 

@@ -201,6 +201,14 @@ a7_best_kernel(const MergeCfg c, const tpc_track_rec_t* __restrict__ tracks, con
       const tpc_track_rec_t* r = tracks + o;
       const int gap = FORWARD ? r->first_row - my_last : my_first - r->last_row;
       if (gap < 1 || gap > c.gap_max) continue;
+      // exact prefilter: tan lambda and q/pT (and their variances) change neither in the rotation nor along the
+      // helix, and D^T S^-1 D >= D_i^2 / S_ii for a positive definite S, so a pair that fails on one of them alone
+      // cannot pass the full chi2
+      {
+        const double dt = (double)r->tanl - m.t, dq = (double)r->qpt - m.q;
+        if (dt * dt >= c.chi2_max * ((double)r->cov[9] + m.C[9]) || dq * dq >= c.chi2_max * ((double)r->cov[14] + m.C[14]))
+          continue;
+      }
       MState other;
       load_state(r, other);
       // rotation goes from the inner segment's frame to the outer one's
