@@ -219,6 +219,26 @@ def merge(par, cov, sector, first_row, last_row, bz, params=None, n_per_side=18,
     return succ, pred, chi2, int(nl)
 
 
+def refit_merged(y_cm, z_cm, row_offsets, n_sectors, n_rows, row_x, bz, trk_hit_offset, trk_n_owned, hit_ids, succ, pred,
+                 params=None, n_per_side=18, sector_angle=np.deg2rad(20.0)):
+    """orc_refit_merged (P47): refit over the hits of every chain of linked tracks; heads only (n_used > 0)."""
+    p = params or default_params()
+    nt = trk_n_owned.shape[0]
+    par = np.zeros((nt, 6), dtype=np.float64)
+    cov = np.zeros((nt, 15), dtype=np.float64)
+    chi2 = np.zeros(nt, dtype=np.float64)
+    n_used = np.zeros(nt, dtype=np.int32)
+    out_sector = np.full(nt, -1, dtype=np.int32)
+    lib().orc_refit_merged(C.byref(p), C.c_double(bz), C.c_int32(n_sectors), C.c_int32(n_rows),
+                           _f64(np.ascontiguousarray(row_x, np.float64)), _f64(np.ascontiguousarray(y_cm, np.float64)),
+                           _f64(np.ascontiguousarray(z_cm, np.float64)), _u32(row_offsets), C.c_int32(n_per_side),
+                           C.c_double(sector_angle), C.c_int64(nt), _i32(np.ascontiguousarray(trk_hit_offset, np.int32)),
+                           _i32(np.ascontiguousarray(trk_n_owned, np.int32)), _i32(np.ascontiguousarray(hit_ids, np.int32)),
+                           _i32(np.ascontiguousarray(succ, np.int32)), _i32(np.ascontiguousarray(pred, np.int32)),
+                           _f64(par), _f64(cov), _f64(chi2), _i32(n_used), _i32(out_sector))
+    return par, cov, chi2, n_used, out_sector
+
+
 def track_records(ev, o):
     """(sector, first_row, last_row) of the oracle's output tracks, from their owned hit lists."""
     sec, row = ev.sector_row()

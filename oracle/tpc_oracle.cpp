@@ -739,3 +739,92 @@ extern "C" int64_t orc_merge(double cq, double smax, int32_t n_per_side, double 
   }
   return links;
 }
+
+// ------------------------------------------------------------------------------------------------
+// P47: refit over a chain of linked tracks (the "global refit" of SURVEY 8(f) NEXT-1).
+// ------------------------------------------------------------------------------------------------
+// angle by which the frame of sector sb is turned against the frame of sa (P42); the pair must be related (P43)
+static double frame_angle(int32_t n_per_side, double sector_angle, int32_t sa, int32_t sb) {
+  if (sa == sb) return 0.0;
+  if (sa / n_per_side != sb / n_per_side) return 0.0;   // across the membrane: same frame
+  const int32_t d = ((sb % n_per_side - sa % n_per_side) % n_per_side + n_per_side) % n_per_side;
+  return d == 1 ? sector_angle : -sector_angle;
+}
+
+extern "C" void orc_refit_merged(const orc_params_t* p, double bz, int32_t n_sectors, int32_t n_rows,
+                                 const double* row_x, const double* y, const double* z, const uint32_t* ro,
+                                 int32_t n_per_side, double sector_angle, int64_t n_tracks,
+                                 const int32_t* trk_hit_offset, const int32_t* trk_n_owned, const int32_t* hit_ids,
+                                 const int32_t* succ, const int32_t* pred, double* par, double* cov, double* chi2_out,
+                                 int32_t* n_used, int32_t* out_sector) {
+  const double cq = p->cq_per_tesla * bz;
+  const double sy2 = p->sigma_y * p->sigma_y, sz2 = p->sigma_z * p->sigma_z;
+  const int64_t n_sr = (int64_t)n_sectors * n_rows;
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t t = 0; t < n_tracks; ++t) {
+    n_used[t] = 0;
+    if (pred[t] >= 0) continue;
+    // the chain's hits with their row x and sector
+    std::vector<int32_t> h;
+    for (int64_t c = t; c >= 0; c = succ[c])
+      for (int32_t j = 0; j < trk_n_owned[c]; ++j) h.push_back(hit_ids[trk_hit_offset[c] + j]);
+    const int32_t m = (int32_t)h.size();
+    std::vector<double> xs(m);
+    std::vector<int32_t> sec(m);
+    for (int32_t j = 0; j < m; ++j) {
+      int64_t lo = 0, hi = n_sr;
+      while (hi - lo > 1) {
+        int64_t mid = (lo + hi) / 2;
+        if (ro[mid] <= (uint32_t)h[j]) lo = mid; else hi = mid;
+      }
+      xs[j] = row_x[lo % n_rows];
+      sec[j] = (int32_t)(lo / n_rows);
+    }
+    if (m == 0) continue;
+    double st[5] = {y[h[0]], z[h[0]], 0.0, 0.0, 0.0};
+    double C[25];
+    reset_cov(p, C);
+    double x = xs[0], chi2 = 0.0;
+    int32_t cur = sec[0], used = 0;
+    if (m >= 2 && sec[1] == sec[0]) {   // a chain's first track owns >= n_min_owned hits of one sector
+      const double dx01 = xs[1] - xs[0], dy = y[h[1]] - y[h[0]], dz = z[h[1]] - z[h[0]];
+      const double chord = std::sqrt(dx01 * dx01 + dy * dy);
+      st[2] = dy / chord;
+      st[3] = dz / chord;
+    }
+    // move the state to hit j: rotate into its sector's frame if needed, then transport to its row
+    auto move_to = [&](int32_t j) -> bool {
+      if (sec[j] != cur) {
+        const double a = frame_angle(n_per_side, sector_angle, cur, sec[j]);
+        if (a != 0.0 && !orc_rotate(cq, p->sinphi_max, a, &x, st, C)) return false;
+        cur = sec[j];
+      }
+      if (!orc_transport(cq, p->sinphi_max, xs[j] - x, st, C)) return false;
+      x = xs[j];
+      return true;
+    };
+    orc_update(st, C, y[h[0]], z[h[0]], sy2, sz2);
+    int32_t last = 0;
+    for (int32_t j = 1; j < m; ++j) {   // up
+      if (!move_to(j)) break;
+      orc_update(st, C, y[h[j]], z[h[j]], sy2, sz2);
+      last = j;
+    }
+    reset_cov(p, C);
+    chi2 += orc_update(st, C, y[h[last]], z[h[last]], sy2, sz2);
+    used = 1;
+    for (int32_t j = last - 1; j >= 0; --j) {   // down
+      if (!move_to(j)) break;
+      chi2 += orc_update(st, C, y[h[j]], z[h[j]], sy2, sz2);
+      ++used;
+    }
+    par[t * 6] = x;
+    for (int i = 0; i < 5; ++i) par[t * 6 + 1 + i] = st[i];
+    int q = 0;
+    for (int i = 0; i < 5; ++i)
+      for (int j = 0; j <= i; ++j) cov[t * 15 + q++] = C[i * 5 + j];
+    chi2_out[t] = chi2;
+    n_used[t] = used;
+    out_sector[t] = cur;
+  }
+}

@@ -116,6 +116,19 @@ int64_t orc_merge(double cq, double sinphi_max, int32_t n_per_side, double secto
                   double chi2_max, int64_t n_tracks, const double* par, const double* cov, const int32_t* sector,
                   const int32_t* first_row, const int32_t* last_row, int32_t* succ, int32_t* pred, double* link_chi2);
 
+/* P47: refit over the hits of a whole chain of linked tracks.  For every chain head a (pred[a] < 0): hits = owned hits
+ * of a, succ[a], succ[succ[a]], ... in that order (rows ascend along a chain, P43); the P41 schedule runs over that
+ * list, the state living in the frame of the sector of the hit it was last moved to: before a transport to a hit of
+ * another sector the state and covariance are rotated into that sector's frame (P42; a failed rotation ends the pass
+ * like a failed transport).  Outputs per track index: heads get (x_ref, state) at the row where the down pass ended
+ * in the frame of that hit's sector (out_sector), packed covariance, chi2 and the hits used on the way down; tracks
+ * that are not heads get n_used = 0 and nothing else. */
+void orc_refit_merged(const orc_params_t* p, double bz, int32_t n_sectors, int32_t n_rows, const double* row_x,
+                      const double* y_cm, const double* z_cm, const uint32_t* row_offsets, int32_t n_per_side,
+                      double sector_angle, int64_t n_tracks, const int32_t* trk_hit_offset,
+                      const int32_t* trk_n_owned, const int32_t* hit_ids, const int32_t* succ, const int32_t* pred,
+                      double* par, double* cov, double* chi2, int32_t* n_used, int32_t* out_sector);
+
 int orc_num_threads(void);
 
 #ifdef __cplusplus

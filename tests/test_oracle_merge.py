@@ -243,3 +243,109 @@ def test_exact_helices_crossing_sector_edges_are_linked_and_only_those(orc):
     assert want > 400 and got >= 0.99 * want, (got, want)
     # chains never branch and never loop
     assert len(set(succ[a].tolist())) == len(a)
+
+
+# ------------------------------------------------------------------------------------------ P47: refit over chains
+def _merged(orc, ev, o, exact=False):
+    s, f, l = orc.track_records(ev, o)
+    succ, pred, chi2, nl = orc.merge(o["refit_par"], o["refit_cov"], s, f, l, ev.cfg.bz)
+    y, z = (ev.y_exact, ev.z_exact) if exact else (ev.y / 640.0, ev.z / 640.0)
+    r = orc.refit_merged(y, z, ev.row_offsets, ev.n_sectors, ev.n_rows, ev.row_x, ev.cfg.bz, o["trk_hit_offset"],
+                         o["trk_n_owned"], o["hit_ids"], succ, pred)
+    return s, succ, pred, r
+
+
+def test_merged_refit_of_unlinked_tracks_is_the_plain_refit(orc):
+    ev = make_event(1, 21, n_tracks=600)
+    o = orc.track(ev)
+    s, succ, pred, (par, cov, chi2, used, osec) = _merged(orc, ev, o)
+    alone = (succ < 0) & (pred < 0)
+    assert alone.sum() > 100
+    assert np.array_equal(par[alone], o["refit_par"][alone]) and np.array_equal(cov[alone], o["refit_cov"][alone])
+    assert np.array_equal(used[alone], o["refit_used"][alone]) and np.array_equal(osec[alone], s[alone])
+    assert np.all(used[pred >= 0] == 0)                               # only chain heads carry a result
+
+
+def test_merged_refit_reaches_generator_truth_across_sector_edges(orc):
+    """Exact helices: the fit over both pieces of a particle that crosses a sector edge uses every hit of both, and
+    gives the generator's truth parameters at the first hit in the first piece's frame -- so the state was rotated by
+    the right angle, in the right direction, with the right reference-plane bookkeeping, on the way up AND back."""
+    ev = make_event(1, 11, n_tracks=1500, noise=0.0, sigma_scale=0.0)
+    o = orc.track(ev, exact_coords=True)
+    s, succ, pred, (par, cov, chi2, used, osec) = _merged(orc, ev, o, exact=True)
+    heads = np.nonzero((pred < 0) & (succ >= 0))[0]
+    assert len(heads) > 300
+    n_hits_chain = np.array([sum(o["trk_n_owned"][c] for c in _chain(succ, a)) for a in heads])
+    full = used[heads] == n_hits_chain
+    assert full.mean() > 0.9                                          # the rest stop at |sin phi| >= 0.95 in a turned frame
+    worst, n_pure = 0.0, 0
+    for a in heads[full]:
+        hits = np.concatenate([o["hit_ids"][o["trk_hit_offset"][c]: o["trk_hit_offset"][c] + o["trk_n_owned"][c]]
+                               for c in _chain(succ, a)])
+        lab = ev.label[hits] // 64
+        if not np.all(lab == lab[0]):
+            continue                       # a track that crosses another may own one of its clusters
+        n_pure += 1
+        tp = truth_params_at(ev, lab[0], int(s[a]), par[a, 0])
+        worst = max(worst, float((np.abs(par[a, 1:] - tp) / np.maximum(np.abs(tp), 1.0)).max()))
+        assert osec[a] == s[a]
+    assert n_pure > 0.95 * full.sum() and worst < 5e-5, (n_pure, worst)
+
+
+def _chain(succ, a):
+    while a >= 0:
+        yield a
+        a = succ[a]
+
+
+def test_merged_refit_tightens_the_fit_and_keeps_chi2_per_dof_at_one(orc):
+    """Smeared central event: joining two pieces roughly doubles the lever arm, so the q/pT variance of the merged fit is
+    well below that of the head alone; and chi2 per degree of freedom stays ~1 -- a rotation that moved the state off
+    the track would cost chi2 of the order of (shift / 0.1 cm)^2 per hit."""
+    ev = make_event(1, 1000)
+    o = orc.track(ev)
+    s, succ, pred, (par, cov, chi2, used, osec) = _merged(orc, ev, o)
+    heads = np.nonzero((pred < 0) & (succ >= 0))[0]
+    assert len(heads) > 2500
+    ratio = cov[heads, 14] / o["refit_cov"][heads, 14]
+    assert np.median(ratio) < 0.5
+    ndf = 2 * used[heads] - 5
+    ok = ndf > 40
+    assert 0.85 < np.median(chi2[heads][ok] / ndf[ok]) < 1.15
+
+
+def test_merged_refit_handmade_line_through_two_sectors(orc):
+    """A straight line (Bz = 0) with hits placed by plane geometry in sector 1 (rows 20..39) and sector 2 (rows 40..59):
+    every residual is zero in the right frames, so the fit returns the line exactly and uses all 40 hits."""
+    n_rows = 80
+    xr = 85.0 + (160.0 / 151.0) * np.arange(n_rows)
+    p0, d = np.array([70.0, 38.0]), np.deg2rad(48.0)
+    az = lambda sct: np.deg2rad((sct % 18 + 0.5) * 20.0)      # noqa: E731
+
+    def local_hit(sct, row):
+        ca, sa = np.cos(az(sct)), np.sin(az(sct))
+        px, py = p0[0] * ca + p0[1] * sa, -p0[0] * sa + p0[1] * ca
+        phi = d - az(sct)
+        t = (xr[row] - px) / np.cos(phi)
+        return py + t * np.sin(phi), 3.0 + 0.25 * t, phi
+
+    ys, zs, counts = [], [], np.zeros(36 * n_rows, dtype=np.int64)
+    for sct, rows in ((1, range(20, 40)), (2, range(40, 60))):
+        for r in rows:
+            yy, zz, _ = local_hit(sct, r)
+            ys.append(yy)
+            zs.append(zz)
+            counts[sct * n_rows + r] += 1
+    ro = np.concatenate([[0], np.cumsum(counts)]).astype(np.uint32)
+    y, z = np.array(ys), np.array(zs)
+    off, cnt, ids = np.array([0, 20], np.int32), np.array([20, 20], np.int32), np.arange(40, dtype=np.int32)
+    succ, pred = np.array([1, -1], np.int32), np.array([-1, 0], np.int32)
+    par, cov, chi2, used, osec = orc.refit_merged(y, z, ro, 36, n_rows, xr, 0.0, off, cnt, ids, succ, pred)
+    y0, z0, phi0 = local_hit(1, 20)
+    assert used.tolist() == [40, 0] and osec[0] == 1 and par[0, 0] == xr[20]
+    assert abs(par[0, 1] - y0) < 1e-9 and abs(par[0, 2] - z0) < 1e-9
+    assert abs(par[0, 3] - np.sin(phi0)) < 1e-11 and abs(par[0, 4] - 0.25) < 1e-11 and chi2[0] < 1e-16
+    # the other direction of rotation: the same line entered as sector 2 -> sector 1 must NOT fit (wrong frames)
+    ys2 = [local_hit(2, r)[0] for r in range(20, 40)] + [local_hit(1, r)[0] for r in range(40, 60)]
+    par2, _, chi2_2, used2, _ = orc.refit_merged(np.array(ys2), z, ro, 36, n_rows, xr, 0.0, off, cnt, ids, succ, pred)
+    assert chi2_2[0] > 1e3 or used2[0] < 40
