@@ -260,6 +260,15 @@ def run_ours(args):
     torch.cuda.synchronize()
     merge_ms = r0e.elapsed_time(r1e) / 5
     merge_counts = mres[3].cpu().numpy()
+    for _ in range(2):
+        trk.refit_merged(y, z, ro, out, mres[0], mres[1], None, stream)
+    torch.cuda.synchronize()
+    r0e.record(stream)
+    for _ in range(5):
+        trk.refit_merged(y, z, ro, out, mres[0], mres[1], None, stream)
+    r1e.record(stream)
+    torch.cuda.synchronize()
+    refit_merged_ms = r0e.elapsed_time(r1e) / 5
 
     # ---- single-event latency (B = 1), for context -------------------------------------------------------
     ev1 = evs[0]
@@ -394,9 +403,9 @@ def run_ours(args):
                              f"> 126 MB L2; no explicit flush"},
             "tracks_per_s": len(tracks) * world * args.steps / (ms_max * 1e-3),
             "single_event_latency_ms": latency_ms,
-            "next": {"a6_refit_ms": refit_ms, "tracks_refitted": len(tracks), "a7_merge_ms": merge_ms,
+            "next": {"a6_refit_ms": refit_ms, "tracks_refitted": len(tracks), "a7_merge_ms": merge_ms, "a6_refit_merged_ms": refit_merged_ms,
                      "merge_links": int(merge_counts[0]), "merged_tracks": int(merge_counts[1]),
-                     "note": "tpc_refit and tpc_merge over the step's output tracks; outside the timed step"},
+                     "note": "tpc_refit, tpc_merge and tpc_refit_merged over the step's output tracks; outside the timed step"},
             "e2e": {"value": e2e_units / (e2e_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "steps": e2e_steps, "ms_per_step": e2e_max / e2e_steps,
                     "host_threads": T},

@@ -169,6 +169,17 @@ int tpc_merge(tpc_tracker_t* t, const tpc_track_rec_t* tracks, const int32_t* co
               const tpc_merge_params_t* params, void* stream, int32_t* succ, int32_t* pred, float* link_chi2,
               int32_t* merge_counts);
 
+/* P47: refit over the hits of every chain of linked tracks.  `clusters`, `n`, `tracks` as for tpc_refit
+ * (the tpc_track output of the handle's last call, whose hit lists are used); succ / pred: [device] links from
+ * tpc_merge.  For every chain head (pred < 0) the P41 schedule runs over the owned hits of the head, its successor,
+ * ...; before a hit of another sector the state is rotated into that sector's frame (P42).  refit_out: [device]
+ * track_capacity records: heads get x .. chi2 at the row where the downward pass ended, `sector` = the frame of that
+ * state, n_hits = hits used on the way down; other tracks get n_hits = 0; the remaining fields are copied.
+ * Asynchronous on `stream`.  Errors: TPC_ERR_ARG, TPC_ERR_CUDA. */
+int tpc_refit_merged(tpc_tracker_t* t, const tpc_clusters_t* clusters, int64_t n, void* stream,
+                     const tpc_tracks_out_t* tracks, const int32_t* succ, const int32_t* pred,
+                     const tpc_merge_params_t* params, tpc_track_rec_t* refit_out);
+
 int tpc_tracker_destroy(tpc_tracker_t* t);
 
 const char* tpc_status_string(int status);

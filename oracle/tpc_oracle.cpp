@@ -793,11 +793,20 @@ extern "C" void orc_refit_merged(const orc_params_t* p, double bz, int32_t n_sec
       st[3] = dz / chord;
     }
     // move the state to hit j: rotate into its sector's frame if needed, then transport to its row
+    // (all or nothing: if the rotation works but the transport fails, the state stays in the old frame)
     auto move_to = [&](int32_t j) -> bool {
       if (sec[j] != cur) {
+        double x2 = x, st2[5], C2[25];
+        for (int i = 0; i < 5; ++i) st2[i] = st[i];
+        for (int i = 0; i < 25; ++i) C2[i] = C[i];
         const double a = frame_angle(n_per_side, sector_angle, cur, sec[j]);
-        if (a != 0.0 && !orc_rotate(cq, p->sinphi_max, a, &x, st, C)) return false;
+        if (a != 0.0 && !orc_rotate(cq, p->sinphi_max, a, &x2, st2, C2)) return false;
+        if (!orc_transport(cq, p->sinphi_max, xs[j] - x2, st2, C2)) return false;
+        for (int i = 0; i < 5; ++i) st[i] = st2[i];
+        for (int i = 0; i < 25; ++i) C[i] = C2[i];
         cur = sec[j];
+        x = xs[j];
+        return true;
       }
       if (!orc_transport(cq, p->sinphi_max, xs[j] - x, st, C)) return false;
       x = xs[j];

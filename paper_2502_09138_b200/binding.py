@@ -107,6 +107,8 @@ def load_library():
     lib.tpc_default_merge_params.restype = None
     lib.tpc_merge.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(MergeParams), C.c_void_p,
                               C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.tpc_refit_merged.argtypes = [C.c_void_p, C.POINTER(_Clusters), C.c_int64, C.c_void_p, C.POINTER(_TracksOut),
+                                     C.c_void_p, C.c_void_p, C.POINTER(MergeParams), C.c_void_p]
     lib.tpc_tracker_destroy.argtypes = [C.c_void_p]
     lib.tpc_status_string.argtypes = [C.c_int]
     lib.tpc_status_string.restype = C.c_char_p
@@ -278,6 +280,21 @@ class Tracker:
                                         C.byref(params) if params is not None else None, self._stream_ptr(stream),
                                         _ptr(succ), _ptr(pred), _ptr(chi2), _ptr(mc)))
         return succ, pred, chi2, mc
+
+    def refit_merged(self, y, z, row_offsets, out: "TracksOut", succ, pred, params: "MergeParams | None" = None,
+                     stream=None):
+        """tpc_refit_merged: refit over every chain of linked tracks (succ / pred from merge()); returns a device uint8
+        tensor of track records (heads carry the result, other tracks n_hits = 0)."""
+        import torch
+        n = int(y.shape[0])
+        cl = _Clusters(_ptr(y), _ptr(z), _ptr(row_offsets))
+        o = _TracksOut(_ptr(out.tracks), int(out.tracks.shape[0] // 112), int(out.hit_ids.shape[0]), _ptr(out.hit_ids),
+                       _ptr(out.counts))
+        ref = torch.zeros_like(out.tracks)
+        self._check(self._lib.tpc_refit_merged(self._h, C.byref(cl), C.c_int64(n), self._stream_ptr(stream), C.byref(o),
+                                               _ptr(succ), _ptr(pred),
+                                               C.byref(params) if params is not None else None, _ptr(ref)))
+        return ref
 
     def track_host(self, y, z, row_offsets, tracks, hit_ids, counts, stream=None):
         """tpc_track_host: all arguments are HOST tensors (pinned for asynchronous copies): y, z int32 [n],

@@ -404,6 +404,23 @@ int tpc_merge(tpc_tracker_t* t, const tpc_track_rec_t* tracks, const int32_t* co
   return TPC_OK;
 }
 
+int tpc_refit_merged(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* stream, const tpc_tracks_out_t* tracks,
+                     const int32_t* succ, const int32_t* pred, const tpc_merge_params_t* params,
+                     tpc_track_rec_t* refit_out) {
+  if (!t || !cl || !tracks || n < 0) return TPC_ERR_ARG;
+  if (!tracks->counts || tracks->track_capacity < 0 || tracks->hit_capacity < 0) return TPC_ERR_ARG;
+  if (tracks->track_capacity > 0 && (!tracks->tracks || !refit_out || !succ || !pred)) return TPC_ERR_ARG;
+  if (tracks->hit_capacity > 0 && !tracks->hit_ids) return TPC_ERR_ARG;
+  // the row list of the output hits (a5) must be that of the call that produced `tracks`
+  if (!t->arena || n != t->last_n || cl->row_offsets != t->last_ro || cl->y != t->last_y || cl->z != t->last_z)
+    return TPC_ERR_ARG;
+  tpc_merge_params_t mp;
+  if (params) mp = *params; else tpc_default_merge_params(&mp);
+  if (mp.n_per_side < 1) return TPC_ERR_ARG;
+  TPC_CUDA(t, launch_a6_refit_merged(t, &mp, cl->y, cl->z, tracks, succ, pred, refit_out, (cudaStream_t)stream));
+  return TPC_OK;
+}
+
 int tpc_track_host(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* stream, tpc_tracks_out_t* out) {
   if (!t || !cl || !out || n < 0) return TPC_ERR_ARG;
   if (!out->counts || out->track_capacity < 0 || out->hit_capacity < 0) return TPC_ERR_ARG;

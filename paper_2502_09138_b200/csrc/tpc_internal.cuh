@@ -137,6 +137,9 @@ cudaError_t launch_a4_phases(const tpc_tracker* t, int64_t n, cudaStream_t st);
 cudaError_t launch_a5_select(const tpc_tracker* t, const tpc_tracks_out_t* out, cudaStream_t st);
 cudaError_t launch_a6_refit(const tpc_tracker* t, const int32_t* y, const int32_t* z, const tpc_tracks_out_t* tracks,
                             tpc_track_rec_t* refit_out, cudaStream_t st);
+cudaError_t launch_a6_refit_merged(const tpc_tracker* t, const tpc_merge_params_t* mp, const int32_t* y,
+                                   const int32_t* z, const tpc_tracks_out_t* tracks, const int32_t* succ,
+                                   const int32_t* pred, tpc_track_rec_t* refit_out, cudaStream_t st);
 cudaError_t launch_a7_merge(const tpc_tracker* t, const tpc_merge_params_t* mp, const tpc_track_rec_t* tracks,
                             const int32_t* counts, int32_t cap, int32_t* succ, int32_t* pred, float* link_chi2,
                             int32_t* merge_counts, cudaStream_t st);

@@ -404,6 +404,58 @@ def test_merge_config1_and_stress(orc):
     _merge_parity(make_event(4), orc, "merge cfg4")
 
 
+def test_refit_merged_against_the_oracle(orc):
+    """P47 through the C ABI: tpc_track -> tpc_refit -> tpc_merge -> tpc_refit_merged against orc_refit_merged run on
+    the oracle's own tracks and links.  Compared on chains whose head and hit lists are the same on both sides:
+    x_ref, frame sector and hits used equal; parameters within 1e-4; chi2 within 1e-3."""
+    import torch
+    from paper_2502_09138_b200 import Tracker, TRACK_DTYPE
+    from paper_2502_09138_b200.events import geometry_from_event, upload
+    for ev, label in ((make_event(1, 1000), "cfg1"), (make_event(4, n_tracks=1500), "cfg4/1500")):
+        trk = Tracker(geometry_from_event(ev))
+        y, z, ro = upload(ev)
+        out = trk.track(y, z, ro)
+        recs = trk.refit(y, z, ro, out)
+        succ, pred, _, mc = trk.merge(recs, out.counts)
+        mr = trk.refit_merged(y, z, ro, out, succ, pred)
+        tracks, hit_ids, _ = out.to_host()
+        nt = len(tracks)
+        g = mr[: nt * 112].cpu().numpy().view(TRACK_DTYPE)
+        g_succ, g_pred = succ[:nt].cpu().numpy(), pred[:nt].cpu().numpy()
+        trk.close()
+        o = orc.track(ev)
+        assert np.array_equal(hit_ids, o["hit_ids"]) and nt == len(o["trk_seed"]), label   # same tracks on both sides
+        s, f, l = orc.track_records(ev, o)
+        o_succ, o_pred, _, _ = orc.merge(o["refit_par"], o["refit_cov"], s, f, l, ev.cfg.bz)
+        assert (g_succ == o_succ).mean() >= 0.999, label          # links from fp32 records against fp64 records
+        par, cov, chi2, used, osec = orc.refit_merged(ev.y / 640.0, ev.z / 640.0, ev.row_offsets, ev.n_sectors, ev.n_rows,
+                                                      ev.row_x, ev.cfg.bz, o["trk_hit_offset"], o["trk_n_owned"],
+                                                      o["hit_ids"], o_succ, o_pred)
+        same_chain = np.ones(nt, bool)                             # the whole chain of a head is linked identically
+        for a in range(nt):
+            c, d = a, a
+            while c >= 0 or d >= 0:
+                if c != d:
+                    same_chain[a] = False
+                    break
+                c, d = g_succ[c], o_succ[d]
+        heads = np.nonzero((o_pred < 0) & (g_pred < 0) & same_chain)[0]
+        assert len(heads) >= 0.995 * int((o_pred < 0).sum())
+        assert np.all(g["n_hits"][g_pred >= 0] == 0)
+        assert np.array_equal(g["n_hits"][heads], used[heads]), label
+        assert np.array_equal(g["sector"][heads], osec[heads]) and np.array_equal(g["x"][heads], par[heads, 0].astype(np.float32))
+        gp = np.stack([g[k][heads] for k in ("y", "z", "sinphi", "tanl", "qpt")], axis=1).astype(np.float64)
+        err = np.abs(gp - par[heads, 1:]) / np.maximum(np.abs(par[heads, 1:]), 1.0)
+        n_bad = int((err > TOL).any(axis=1).sum())
+        assert n_bad <= 1e-3 * len(heads), f"{label}: {n_bad} merged refits beyond 1e-4, worst {err.max(axis=0)}"
+        xerr = np.abs(g["chi2"][heads] - chi2[heads]) / np.maximum(chi2[heads], 1.0)
+        assert (xerr > 1e-3).sum() <= 1e-3 * len(heads), label
+        linked = heads[o_succ[heads] >= 0]
+        print(f"[refit_merged] {label}: heads={len(heads)} of which chains={len(linked)} beyond_1e-4={n_bad} "
+              f"worst={err.max():.2e} worst_on_chains={err[o_succ[heads] >= 0].max():.2e}")
+        assert len(linked) > 100
+
+
 def test_merge_batch_keeps_events_apart(orc):
     """Two events in one call (72 sectors): links never join tracks of different events, and each event's links are
     those of the event tracked alone."""
