@@ -54,6 +54,7 @@ class Config:
     noise: float = 0.05
     bz: float = 0.5
     n_rows: int = N_ROWS
+    row_pitches: tuple = ()         # ((n_gaps, pitch_cm), ...) from row 0 at x = 85 cm; empty = equidistant 85..245 cm
 
 
 CONFIGS = {
@@ -195,7 +196,12 @@ def make_event(cfg_id: int | Config, seed: int | None = None, *, sigma_scale: fl
     if time_mode is not None:
         cfg.time_mode = time_mode
     rng = Rng(seed)
-    xr = row_x(cfg.n_rows)
+    if cfg.row_pitches:             # pad rows in regions of different pitch (NEXT-4, P48)
+        gaps = np.concatenate([np.full(k, float(p)) for k, p in cfg.row_pitches])
+        assert gaps.size == cfg.n_rows - 1
+        xr = X_FIRST + np.concatenate([[0.0], np.cumsum(gaps)])
+    else:
+        xr = row_x(cfg.n_rows)
     n_az = 1 if cfg.n_sectors == 1 else 18
     alphas = np.zeros(1) if n_az == 1 else (np.arange(18) + 0.5) * np.deg2rad(20.0)
 

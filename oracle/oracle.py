@@ -77,13 +77,21 @@ def _f64(a):
     return _p(a, C.c_double)
 
 
-def neighbours(y, z, row_offsets, n_sectors, n_rows, params=None, brute=False):
+def pitch_weights(row_x):
+    """P48: integer weight of every gap between consecutive rows, nearbyint(64 * pitch in cm); None when all weights
+    are equal (then the cost is the plain second difference of P8)."""
+    w = np.rint(64.0 * np.diff(np.asarray(row_x, dtype=np.float64))).astype(np.int32)
+    return None if np.all(w == w[0]) else np.ascontiguousarray(w)
+
+
+def neighbours(y, z, row_offsets, n_sectors, n_rows, params=None, brute=False, gap_w=None):
     p = params or default_params()
     n = y.shape[0]
     up = np.empty(n, dtype=np.int32)
     dn = np.empty(n, dtype=np.int32)
-    f = lib().orc_neighbours_brute if brute else lib().orc_neighbours_pruned
-    f(C.byref(p), C.c_int32(n_sectors), C.c_int32(n_rows), _i32(y), _i32(z), _u32(row_offsets), _i32(up), _i32(dn))
+    f = lib().orc_neighbours_brute_w if brute else lib().orc_neighbours_pruned_w
+    f(C.byref(p), C.c_int32(n_sectors), C.c_int32(n_rows), _i32(gap_w) if gap_w is not None else None, _i32(y), _i32(z),
+      _u32(row_offsets), _i32(up), _i32(dn))
     return up, dn
 
 
@@ -259,7 +267,8 @@ def track(ev, params=None, *, brute=False, search_mode=1, exact_coords=False, ti
     int/units_per_cm: the oracle-internal entry that bypasses quantisation (SURVEY 8c pin table)."""
     p = params or default_params()
     t = [time.perf_counter()]
-    up, dn = neighbours(ev.y, ev.z, ev.row_offsets, ev.n_sectors, ev.n_rows, p, brute=brute)
+    up, dn = neighbours(ev.y, ev.z, ev.row_offsets, ev.n_sectors, ev.n_rows, p, brute=brute,
+                        gap_w=pitch_weights(ev.row_x))
     t.append(time.perf_counter())
     upc, dnc = clean_links(up, dn)
     ss, sl = find_seeds(upc, dnc, p)

@@ -63,20 +63,23 @@ static inline bool in_window(const orc_params_t* p, int32_t yh, int32_t zh, int3
   return std::llabs(dy) <= p->w_y && std::llabs(dz) <= p->w_z;
 }
 
-static inline int64_t pair_cost(const orc_params_t* p, int32_t yh, int32_t zh, int32_t yu, int32_t zu, int32_t yd,
-                                int32_t zd) {
-  int64_t ddy = (int64_t)yu + yd - 2 * (int64_t)yh;
-  int64_t ddz = (int64_t)zu + zd - 2 * (int64_t)zh;
+// P8 for any row pitches (P48): the straight line through d and u, evaluated at the row of h, misses h by
+// (wa y_u + wb y_d - (wa + wb) y_h) / (wa + wb) with wa, wb the integer pitch weights of the gaps below and above h.
+// The cost is that numerator squared and weighted; for equal pitches (wa == wb == 1) it is the plain second difference.
+static inline int64_t pair_cost(const orc_params_t* p, int64_t wa, int64_t wb, int32_t yh, int32_t zh, int32_t yu,
+                                int32_t zu, int32_t yd, int32_t zd) {
+  int64_t ddy = wa * yu + wb * yd - (wa + wb) * (int64_t)yh;
+  int64_t ddz = wa * zu + wb * zd - (wa + wb) * (int64_t)zh;
   return p->cost_wy * ddy * ddy + p->cost_wz * ddz * ddz;
 }
 
-static void best_pair(const orc_params_t* p, const int32_t* y, const int32_t* z, int32_t h,
+static void best_pair(const orc_params_t* p, int64_t wa, int64_t wb, const int32_t* y, const int32_t* z, int32_t h,
                       const std::vector<int32_t>& U, const std::vector<int32_t>& D, int32_t* up, int32_t* dn) {
   int64_t best_cost = std::numeric_limits<int64_t>::max();
   int32_t bu = -1, bd = -1;
   for (int32_t u : U)
     for (int32_t d : D) {
-      int64_t c = pair_cost(p, y[h], z[h], y[u], z[u], y[d], z[d]);
+      int64_t c = pair_cost(p, wa, wb, y[h], z[h], y[u], z[u], y[d], z[d]);
       bool better = c < best_cost || (c == best_cost && (u < bu || (u == bu && d < bd)));
       if (better) {
         best_cost = c;
@@ -84,7 +87,8 @@ static void best_pair(const orc_params_t* p, const int32_t* y, const int32_t* z,
         bd = d;
       }
     }
-  if (bu >= 0 && best_cost <= p->c_max) {
+  // P10 with the pitch weights: cost / ((wa + wb) / 2)^2 <= c_max
+  if (bu >= 0 && 4 * best_cost <= (int64_t)p->c_max * (wa + wb) * (wa + wb)) {
     *up = bu;
     *dn = bd;
   } else {
@@ -93,8 +97,9 @@ static void best_pair(const orc_params_t* p, const int32_t* y, const int32_t* z,
   }
 }
 
-extern "C" void orc_neighbours_brute(const orc_params_t* p, int32_t n_sectors, int32_t n_rows, const int32_t* y,
-                                     const int32_t* z, const uint32_t* ro, int32_t* link_up, int32_t* link_dn) {
+extern "C" void orc_neighbours_brute_w(const orc_params_t* p, int32_t n_sectors, int32_t n_rows, const int32_t* gap_w,
+                                       const int32_t* y, const int32_t* z, const uint32_t* ro, int32_t* link_up,
+                                       int32_t* link_dn) {
 #pragma omp parallel for schedule(dynamic, 1)
   for (int32_t s = 0; s < n_sectors; ++s) {
     std::vector<int32_t> U, D;
@@ -110,10 +115,15 @@ extern "C" void orc_neighbours_brute(const orc_params_t* p, int32_t n_sectors, i
           if (in_window(p, y[h], z[h], y[c], z[c])) U.push_back((int32_t)c);
         for (uint32_t c = o[-1]; c < o[0]; ++c)
           if (in_window(p, y[h], z[h], y[c], z[c])) D.push_back((int32_t)c);
-        best_pair(p, y, z, (int32_t)h, U, D, &link_up[h], &link_dn[h]);
+        best_pair(p, gap_w ? gap_w[r - 1] : 1, gap_w ? gap_w[r] : 1, y, z, (int32_t)h, U, D, &link_up[h], &link_dn[h]);
       }
     }
   }
+}
+
+extern "C" void orc_neighbours_brute(const orc_params_t* p, int32_t n_sectors, int32_t n_rows, const int32_t* y,
+                                     const int32_t* z, const uint32_t* ro, int32_t* link_up, int32_t* link_dn) {
+  orc_neighbours_brute_w(p, n_sectors, n_rows, nullptr, y, z, ro, link_up, link_dn);
 }
 
 // z-sorted index per row: the oracle's own pruning structure (not the GPU's (y,z) bin grid).
@@ -128,8 +138,9 @@ static void build_zorder(int64_t n_sr, const uint32_t* ro, const T* z, std::vect
   }
 }
 
-extern "C" void orc_neighbours_pruned(const orc_params_t* p, int32_t n_sectors, int32_t n_rows, const int32_t* y,
-                                      const int32_t* z, const uint32_t* ro, int32_t* link_up, int32_t* link_dn) {
+extern "C" void orc_neighbours_pruned_w(const orc_params_t* p, int32_t n_sectors, int32_t n_rows, const int32_t* gap_w,
+                                        const int32_t* y, const int32_t* z, const uint32_t* ro, int32_t* link_up,
+                                        int32_t* link_dn) {
   std::vector<int32_t> zo;
   build_zorder<int32_t>((int64_t)n_sectors * n_rows, ro, z, zo);
   auto collect = [&](uint32_t a, uint32_t b, int32_t yh, int32_t zh, std::vector<int32_t>& out) {
@@ -153,10 +164,15 @@ extern "C" void orc_neighbours_pruned(const orc_params_t* p, int32_t n_sectors, 
         if (r < 1 || r > n_rows - 2) continue;
         collect(o[1], o[2], y[h], z[h], U);
         collect(o[-1], o[0], y[h], z[h], D);
-        best_pair(p, y, z, (int32_t)h, U, D, &link_up[h], &link_dn[h]);
+        best_pair(p, gap_w ? gap_w[r - 1] : 1, gap_w ? gap_w[r] : 1, y, z, (int32_t)h, U, D, &link_up[h], &link_dn[h]);
       }
     }
   }
+}
+
+extern "C" void orc_neighbours_pruned(const orc_params_t* p, int32_t n_sectors, int32_t n_rows, const int32_t* y,
+                                      const int32_t* z, const uint32_t* ro, int32_t* link_up, int32_t* link_dn) {
+  orc_neighbours_pruned_w(p, n_sectors, n_rows, nullptr, y, z, ro, link_up, link_dn);
 }
 
 // ------------------------------------------------------------------------------------------------

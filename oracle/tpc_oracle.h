@@ -49,6 +49,17 @@ void orc_neighbours_brute(const orc_params_t* p, int32_t n_sectors, int32_t n_ro
 void orc_neighbours_pruned(const orc_params_t* p, int32_t n_sectors, int32_t n_rows, const int32_t* y,
                            const int32_t* z, const uint32_t* row_offsets, int32_t* link_up, int32_t* link_dn);
 
+/* P48 (NEXT-4: rows that are not equidistant).  gap_w[r], r = 0..n_rows-2: integer pitch weight of the gap between
+ * rows r and r+1 (nearbyint(64 * pitch in cm), oracle.py: pitch_weights); NULL = all equal.  For cluster h in row r
+ * with wa = gap_w[r-1], wb = gap_w[r]: cost = cost_wy*(wa y_u + wb y_d - (wa+wb) y_h)^2 + cost_wz*(...z...)^2,
+ * minimised as before, accepted iff 4 cost <= c_max (wa + wb)^2.  With equal weights this is P8 / P10 exactly. */
+void orc_neighbours_brute_w(const orc_params_t* p, int32_t n_sectors, int32_t n_rows, const int32_t* gap_w,
+                            const int32_t* y, const int32_t* z, const uint32_t* row_offsets, int32_t* link_up,
+                            int32_t* link_dn);
+void orc_neighbours_pruned_w(const orc_params_t* p, int32_t n_sectors, int32_t n_rows, const int32_t* gap_w,
+                             const int32_t* y, const int32_t* z, const uint32_t* row_offsets, int32_t* link_up,
+                             int32_t* link_dn);
+
 /* ---- stage 3: cleaner, chains, seeds (integer, bit-exact) -- SURVEY 8(c) "Stage 3" ---- */
 void orc_clean_links(int64_t n, const int32_t* up, const int32_t* dn, int32_t* up_c, int32_t* dn_c);
 /* returns number of seeds; seeds ascend by start id; seed_start/seed_len need capacity n / l_min + 1 */

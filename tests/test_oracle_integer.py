@@ -187,3 +187,81 @@ def test_zero_smearing_one_pure_chain_per_track(orc):
             c = upc[c]
         assert len(labs) == 1
     assert len({int(ev.label[s]) for s in ss}) == 100
+
+
+# ---- NEXT-4 / P48: rows that are not equidistant (pitch-weighted straightness) ----
+PADPLANE = ((62, 0.75), (33, 1.0), (29, 1.2), (27, 1.5))      # 152 rows in four regions of different pitch
+
+
+def test_weighted_cost_prefers_the_straight_line_through_unequal_gaps(orc):
+    """Row 0 -> row 1 is 1 cm, row 1 -> row 2 is 2 cm (weights 64, 128).  The straight continuation of d -> h lies twice
+    as far from h as d does; the unweighted second difference would pick the mirror image of d instead."""
+    w = np.array([64, 128], dtype=np.int32)
+    y, z, off = _rows([[(-100, -50)], [(0, 0)], [(100, 50), (200, 100)]])      # ids: d = 0, h = 1, u = 2 (mirror), 3 (line)
+    up, dn = orc.neighbours(y, z, off, 1, 3, brute=True, gap_w=w)
+    assert up[1] == 3 and dn[1] == 0
+    up0, _ = orc.neighbours(y, z, off, 1, 3, brute=True)
+    assert up0[1] == 2                                          # what P8 for equal pitches gives on the same clusters
+    up2, dn2 = orc.neighbours(y, z, off, 1, 3, brute=False, gap_w=w)
+    assert up2[1] == 3 and dn2[1] == 0
+
+
+def test_weighted_cost_value_and_threshold(orc):
+    """D_y = wa y_u + wb y_d - (wa + wb) y_h = 64 * 10 = 640 -> cost = 9 * 640^2 = 3 686 400; accepted iff
+    4 cost <= c_max (wa + wb)^2 = c_max * 36 864, i.e. iff c_max >= 400."""
+    w = np.array([64, 128], dtype=np.int32)
+    y, z, off = _rows([[(0, 0)], [(0, 0)], [(10, 0)]])
+    p = orc.default_params()
+    p.c_max = 400
+    assert orc.neighbours(y, z, off, 1, 3, p, brute=True, gap_w=w)[0][1] == 2
+    p.c_max = 399
+    assert orc.neighbours(y, z, off, 1, 3, p, brute=True, gap_w=w)[0][1] == -1
+
+
+def test_equal_weights_are_the_unweighted_reading(orc):
+    ev = make_event(1, 9, n_tracks=300)
+    a = orc.neighbours(ev.y, ev.z, ev.row_offsets, ev.n_sectors, ev.n_rows)
+    b = orc.neighbours(ev.y, ev.z, ev.row_offsets, ev.n_sectors, ev.n_rows, gap_w=np.full(ev.n_rows - 1, 68, np.int32))
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+    assert orc.pitch_weights(ev.row_x) is None                  # 160/151 cm everywhere -> one weight, 68
+
+
+def _padplane_event(seed, **kw):
+    from gen.events import Config
+    cfg = Config("padplane_4_regions", n_sectors=36, tracks_per_collision=400, row_pitches=PADPLANE, **kw)
+    return make_event(cfg, seed=seed)
+
+
+def test_weighted_pruned_equals_bruteforce_on_a_four_region_geometry(orc):
+    ev = _padplane_event(3)
+    w = orc.pitch_weights(ev.row_x)
+    assert w is not None and sorted(set(w.tolist())) == [48, 64, 77, 96]
+    a = orc.neighbours(ev.y, ev.z, ev.row_offsets, ev.n_sectors, ev.n_rows, brute=True, gap_w=w)
+    b = orc.neighbours(ev.y, ev.z, ev.row_offsets, ev.n_sectors, ev.n_rows, brute=False, gap_w=w)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+def test_exact_helices_on_unequal_pitches_give_one_pure_chain_per_track(orc):
+    """The zero-smearing pin of the chain finder on the four-region geometry: with the weighted cost a helix stays
+    'straight' across the pitch changes (rows 62, 95, 124), so no chain breaks there; with the unweighted cost the
+    kink at a pitch change costs 9 * (0.25 * slope * 640)^2 and chains of inclined tracks break."""
+    from gen.events import Config
+    cfg = Config("padplane_open_sector", n_sectors=1, open_sector=True, tracks_per_collision=100, pt_min=0.2, noise=0.0,
+                 row_pitches=PADPLANE)
+    ev = make_event(cfg, seed=5, sigma_scale=0.0)
+    w = orc.pitch_weights(ev.row_x)
+    up, dn = orc.neighbours(ev.y, ev.z, ev.row_offsets, 1, ev.n_rows, gap_w=w)
+    upc, dnc = orc.clean_links(up, dn)
+    ss, sl = orc.find_seeds(upc, dnc)
+    sec, row = ev.sector_row()
+    n_tracks = len(set((ev.label[ev.label >= 0] // 64).tolist()))
+    assert len(ss) == n_tracks
+    for s0 in ss:                                               # every chain is one particle from end to end
+        labs, c = [], s0
+        while c >= 0:
+            labs.append(ev.label[c] // 64)
+            c = upc[c]
+        assert len(set(labs)) == 1
+    up0, dn0 = orc.neighbours(ev.y, ev.z, ev.row_offsets, 1, ev.n_rows)      # unweighted on the same clusters
+    ss0, _ = orc.find_seeds(*orc.clean_links(up0, dn0))
+    assert len(ss0) > n_tracks                                   # chains break at the pitch changes
