@@ -32,7 +32,7 @@ extern "C" {
 
 #define TPC_OK 0
 #define TPC_ERR_ARG (-1)       /* NULL pointer, negative size, parameter out of range */
-#define TPC_ERR_GEOMETRY (-2)  /* n_rows < 3, rows not equidistant (P6), non-positive extents */
+#define TPC_ERR_GEOMETRY (-2)  /* n_rows < 3, rows not ascending, pitch outside 1/64 .. 512 cm, non-positive extents */
 #define TPC_ERR_CUDA (-3)      /* a CUDA runtime call failed (tpc_last_cuda_error() tells which) */
 #define TPC_ERR_NOMEM (-4)     /* scratch allocation failed */
 #define TPC_ERR_CAPACITY (-5)  /* n too large for the packed ownership word (n/l_min >= 2^24) */
@@ -67,7 +67,7 @@ typedef struct {
 typedef struct {
   int32_t n_sectors;       /* independent sectors in one call (36; 1 for configs[0]; B*36 for a batch of B events) */
   int32_t n_rows;          /* pad rows per sector (152), >= 3 */
-  const double* row_x;     /* [host] n_rows local x of the pad rows in cm, ascending, equidistant (P6) */
+  const double* row_x;     /* [host] n_rows local x of the pad rows in cm, ascending; pitches may differ (P48) */
   double units_per_cm;     /* fixed-point scale (640) */
   double y_half_tan;       /* |y| <= row_x[r]*y_half_tan (tan 10 deg); used for grid sizing only */
   double y_half_cm;        /* if > 0: |y| extent in cm for every row instead (open sector, configs[0]); grid sizing only */

@@ -450,6 +450,70 @@ a2_neighbours_dense_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, cons
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// P48 (NEXT-4): rows that are not equidistant.  The straightness of (d, h, u) is the pitch-weighted second difference
+// wa c_u + wb c_d - (wa + wb) c_h with the integer weights of the gaps below (wa) and above (wb) the row of h; its
+// square needs 64 bits, and the acceptance is 4 cost <= c_max (wa + wb)^2.  One plain kernel for every grid shape
+// (the definition's nested scan over the window's bin rows); geometries with equal pitches never come here, their
+// cost is the same up to the common factor wa^2 and stays in the 32-bit kernels above.
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(A2_THREADS)
+a2_neighbours_weighted_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, const uint32_t* __restrict__ ro,
+                              const int4* __restrict__ srt, const uint32_t* __restrict__ sec_key,
+                              const uint32_t* __restrict__ bin_start, int32_t* __restrict__ link_up,
+                              int32_t* __restrict__ link_dn) {
+  if (ctl->bad_offsets) return;
+  const int sr = blockIdx.x;
+  const int r = sr % g.n_rows;
+  const uint32_t a = ro[sr], b = ro[sr + 1];
+  const bool inner = r >= 1 && r <= g.n_rows - 2;   // P5
+  const int org_z = zmin_from_key(sec_key[sr / g.n_rows]);
+  const uint32_t *bs_u = nullptr, *bs_d = nullptr;
+  long long wa = 1, wb = 1;
+  if (inner) {
+    bs_u = bin_start + (size_t)(sr + 1) * g.nb_stride;
+    bs_d = bin_start + (size_t)(sr - 1) * g.nb_stride;
+    wa = g.gap_w[r - 1];
+    wb = g.gap_w[r];
+  }
+  const long long wab = wa + wb;
+  for (uint32_t j = a + blockIdx.y * A2_THREADS + threadIdx.x; j < b; j += gridDim.y * A2_THREADS) {
+    const int4 ch = srt[j];
+    const int yh = ch.x, zh = ch.y;
+    long long best_cost = LLONG_MAX;
+    int best_u = -1, best_d = -1, pu_best = -1, pd_best = -1;
+    if (inner) {
+      const Window w = window_bins(g, yh, zh, org_z);
+      for (int izu = w.iz_lo; izu <= w.iz_hi; ++izu) {
+        const uint32_t ua = bs_u[izu * g.ny + w.iy_lo], ub = bs_u[izu * g.ny + w.iy_hi + 1];
+        for (uint32_t u = ua; u < ub; ++u) {
+          const int4 cu = srt[u];
+          if (abs(cu.x - yh) > g.w_y || abs(cu.y - zh) > g.w_z) continue;   // P7
+          for (int izd = w.iz_lo; izd <= w.iz_hi; ++izd) {
+            const uint32_t da = bs_d[izd * g.ny + w.iy_lo], db = bs_d[izd * g.ny + w.iy_hi + 1];
+            for (uint32_t d = da; d < db; ++d) {
+              const int4 cd = srt[d];
+              if (abs(cd.x - yh) > g.w_y || abs(cd.y - zh) > g.w_z) continue;
+              const long long ddy = wa * cu.x + wb * cd.x - wab * yh, ddz = wa * cu.y + wb * cd.y - wab * zh;
+              const long long cost = (long long)g.cost_wy * ddy * ddy + (long long)g.cost_wz * ddz * ddz;
+              if (cost < best_cost || (cost == best_cost && (cu.z < best_u || (cu.z == best_u && cd.z < best_d)))) {   // P9
+                best_cost = cost;
+                best_u = cu.z;
+                best_d = cd.z;
+                pu_best = (int)u;
+                pd_best = (int)d;
+              }
+            }
+          }
+        }
+      }
+      if (pu_best < 0 || 4 * best_cost > (long long)g.c_max * wab * wab) pu_best = pd_best = -1;   // P10 (P48)
+    }
+    link_up[j] = pu_best;
+    link_dn[j] = pd_best;
+  }
+}
+
 }  // namespace
 
 cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64_t n, cudaStream_t st) {
@@ -464,7 +528,8 @@ cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64
   int64_t per_row = (n / R + A2_THREADS - 1) / A2_THREADS;
   per_row = per_row < 1 ? 1 : (per_row > 64 ? 64 : per_row);
   const dim3 grid2((unsigned)R, (unsigned)per_row);
-  if (dense && fine) a2_neighbours_dense_kernel<true><<<grid2, A2_THREADS, 0, st>>>(A2_ARGS);
+  if (t->g.gap_w) a2_neighbours_weighted_kernel<<<grid2, A2_THREADS, 0, st>>>(A2_ARGS);
+  else if (dense && fine) a2_neighbours_dense_kernel<true><<<grid2, A2_THREADS, 0, st>>>(A2_ARGS);
   else if (dense) a2_neighbours_dense_kernel<false><<<grid2, A2_THREADS, 0, st>>>(A2_ARGS);
   else if (fine) a2_neighbours_kernel<true><<<(unsigned)R, A2_THREADS, 0, st>>>(A2_ARGS);
   else if (t->a2_variant == 1) {

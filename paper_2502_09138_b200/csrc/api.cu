@@ -182,7 +182,7 @@ const char* tpc_status_string(int status) {
   switch (status) {
     case TPC_OK: return "ok";
     case TPC_ERR_ARG: return "bad argument";
-    case TPC_ERR_GEOMETRY: return "bad geometry (n_rows < 3, rows not equidistant or extents not positive)";
+    case TPC_ERR_GEOMETRY: return "bad geometry (n_rows < 3, rows not ascending or extents not positive)";
     case TPC_ERR_CUDA: return "CUDA runtime error";
     case TPC_ERR_NOMEM: return "out of device memory";
     case TPC_ERR_CAPACITY: return "too many clusters for one call";
@@ -199,10 +199,16 @@ int tpc_tracker_create(const tpc_geometry_t* geo, const tpc_field_t* field, tpc_
   if (geo->n_rows < 3 || !(geo->units_per_cm > 0) || !(geo->z_extent_cm > 0)) return TPC_ERR_GEOMETRY;
   if (!(geo->y_half_cm > 0) && !(geo->y_half_tan > 0)) return TPC_ERR_GEOMETRY;
   const int nr = geo->n_rows;
-  const double pitch = (geo->row_x[nr - 1] - geo->row_x[0]) / (nr - 1);
-  if (!(pitch > 0)) return TPC_ERR_GEOMETRY;
-  for (int r = 0; r + 1 < nr; ++r)   // P6: the a2 cost is a second difference, valid for equidistant rows only
-    if (fabs((geo->row_x[r + 1] - geo->row_x[r]) - pitch) > 1e-6 * pitch) return TPC_ERR_GEOMETRY;
+  // P48: rows need not be equidistant; the a2 cost weights the two gaps of a triplet by their integer pitch weights
+  // nearbyint(64 * pitch / cm) (1..2^15: pitches between 1/64 cm and 512 cm).  Equal weights = P8 as written.
+  bool equal_w = true;
+  for (int r = 0; r + 1 < nr; ++r) {
+    const double pitch = geo->row_x[r + 1] - geo->row_x[r];
+    if (!(pitch > 0)) return TPC_ERR_GEOMETRY;
+    const double w = nearbyint(64.0 * pitch);
+    if (w < 1 || w > 32768) return TPC_ERR_GEOMETRY;
+    if (w != nearbyint(64.0 * (geo->row_x[1] - geo->row_x[0]))) equal_w = false;
+  }
 
   tpc_params_t prm;
   if (geo->params) prm = *geo->params; else tpc_default_params(&prm);
@@ -211,7 +217,7 @@ int tpc_tracker_create(const tpc_geometry_t* geo, const tpc_field_t* field, tpc_
       nr > 255 || !(prm.sigma_y > 0) || !(prm.sigma_z > 0) || !(prm.sinphi_max > 0) || !(prm.sinphi_max < 1) ||
       !(prm.gate_y_cm >= 0) || !(prm.gate_z_cm >= 0))
     return TPC_ERR_ARG;
-  // the a2 cost must fit int32: |ddy| <= 2 w_y, |ddz| <= 2 w_z
+  // the a2 cost must fit int32 (equal pitches; the weighted cost is 64-bit): |ddy| <= 2 w_y, |ddz| <= 2 w_z
   {
     const double cmaxv = (double)prm.cost_wy * 4.0 * prm.w_y * prm.w_y + (double)prm.cost_wz * 4.0 * prm.w_z * prm.w_z;
     if (cmaxv >= 2147483647.0) return TPC_ERR_ARG;
@@ -271,16 +277,28 @@ int tpc_tracker_create(const tpc_geometry_t* geo, const tpc_field_t* field, tpc_
   g.cq = (float)(prm.cq_per_tesla * field->bz_tesla);
   for (int k = 0; k < 5; ++k) g.c_reset[k] = (float)prm.c_reset[k];
 
-  // geometry tables in one small device blob: row_x (double) | row_dx (float)
+  // geometry tables in one small device blob: row_x (double) | row_dx (float) | gap_w (int32)
   const size_t o_dx = align_up((size_t)nr * 8, 256);
-  const size_t blob = o_dx + align_up((size_t)nr * 4, 256);
+  const size_t o_w = o_dx + align_up((size_t)nr * 4, 256);
+  const size_t blob = o_w + align_up((size_t)nr * 4, 256);
+  int32_t* w_host = new (std::nothrow) int32_t[nr];
+  if (!w_host) {
+    delete[] dx_host;
+    delete t;
+    return TPC_ERR_NOMEM;
+  }
+  for (int r = 0; r + 1 < nr; ++r) w_host[r] = (int32_t)nearbyint(64.0 * (geo->row_x[r + 1] - geo->row_x[r]));
+  w_host[nr - 1] = 0;
   int rc = TPC_OK;
   e = cudaMalloc(&t->geom_blob, blob);
   if (e == cudaSuccess) e = cudaMemcpy(t->geom_blob, geo->row_x, (size_t)nr * 8, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy((char*)t->geom_blob + o_dx, dx_host, (size_t)nr * 4, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy((char*)t->geom_blob + o_w, w_host, (size_t)nr * 4, cudaMemcpyHostToDevice);
   delete[] dx_host;
+  delete[] w_host;
   g.row_x = (const double*)t->geom_blob;
   g.row_dx = (const float*)((char*)t->geom_blob + o_dx);
+  g.gap_w = equal_w ? nullptr : (const int32_t*)((char*)t->geom_blob + o_w);
   if (e == cudaSuccess) e = setup_a1_attributes(t);
   if (e == cudaSuccess) e = setup_a4_attributes(t);
   for (int k = 0; k < TIMING_SETS * 6 && e == cudaSuccess; ++k) e = cudaEventCreate(&t->ev[k]);

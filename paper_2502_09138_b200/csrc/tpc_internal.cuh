@@ -16,6 +16,7 @@ struct DevGeom {
   int32_t shift_y, shift_z, ny, nz, nb_stride, org_y;
   const double* row_x;     // [n_rows] cm
   const float* row_dx;     // [n_rows] row_x[r+1] - row_x[r], rounded once from double (last entry repeats)
+  const int32_t* gap_w;    // [n_rows - 1] P48 pitch weights nearbyint(64 * pitch / cm), or NULL when all are equal
   // a2 / a3
   int32_t w_y, w_z, cost_wy, cost_wz, c_max, l_min;
   // a4 / a5

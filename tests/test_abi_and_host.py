@@ -64,9 +64,10 @@ def test_host_only_entry_points(lib):
 
 
 def test_geometry_is_validated_before_cuda(lib):
-    """P6: non-equidistant rows and n_rows < 3 are rejected (TPC_ERR_GEOMETRY) without needing a device."""
+    """Rows that do not ascend and n_rows < 3 are rejected (TPC_ERR_GEOMETRY) without needing a device.  (Rows of
+    unequal pitch are accepted since round 2: P48.)"""
     from paper_2502_09138_b200.binding import _Geometry, _Field
-    rx = np.array([85.0, 86.0, 88.5, 89.0])
+    rx = np.array([85.0, 86.0, 85.5, 89.0])
     g = _Geometry(1, 4, rx.ctypes.data_as(C.POINTER(C.c_double)), 640.0, 0.176, 0.0, 250.0, None)
     f = _Field(0.5)
     h = C.c_void_p()

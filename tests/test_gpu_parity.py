@@ -211,6 +211,22 @@ def test_small_geometry_40_rows(orc):
     compare(ev, orc, g, o, label="40 rows")
 
 
+def test_rows_of_unequal_pitch(orc):
+    """NEXT-4 / P48: a pad plane with four regions of different row pitch (0.75 / 1.0 / 1.2 / 1.5 cm).  a2 weights the
+    two gaps of every triplet; everything downstream takes the row positions from the geometry.  Full comparison."""
+    from gen.events import Config
+    pads = ((62, 0.75), (33, 1.0), (29, 1.2), (27, 1.5))
+    ev = make_event(Config("padplane_4_regions", n_sectors=36, tracks_per_collision=2500, row_pitches=pads), seed=3)
+    g, o = _run_gpu(ev), orc.track(ev)
+    assert len(o["seed_start"]) > 5000 and len(o["trk_seed"]) > 3000
+    compare(ev, orc, g, o, label="unequal pitches")
+    ev = make_event(Config("padplane_open", n_sectors=1, open_sector=True, tracks_per_collision=100, pt_min=0.2,
+                           noise=0.0, row_pitches=pads), seed=5, sigma_scale=0.0)
+    g = _run_gpu(ev)
+    compare(ev, orc, g, orc.track(ev), label="unequal pitches, exact helices")
+    assert len(g["tracks"]) == 100
+
+
 def test_non_default_parameters(orc):
     """tpc_params_t reaches every stage: narrower windows, shorter seeds, fewer allowed misses, tighter gate."""
     from paper_2502_09138_b200.binding import default_params
