@@ -247,6 +247,51 @@ def refit_merged(y_cm, z_cm, row_offsets, n_sectors, n_rows, row_x, bz, trk_hit_
     return par, cov, chi2, n_used, out_sector
 
 
+def compress(ev, o):
+    """orc_compress on the oracle's output tracks: (drow uint8, ry int32, rz int32) in hit-list order (P50)."""
+    nh = len(o["hit_ids"])
+    drow = np.zeros(max(nh, 1), np.uint8)
+    ry = np.zeros(max(nh, 1), np.int32)
+    rz = np.zeros(max(nh, 1), np.int32)
+    lib().orc_compress(C.c_int32(ev.n_rows), _i32(ev.y), _i32(ev.z), _u32(ev.row_offsets),
+                       C.c_int64(ev.n_sectors * ev.n_rows), C.c_int64(len(o["trk_seed"])),
+                       _i32(np.ascontiguousarray(o["trk_hit_offset"], np.int32)),
+                       _i32(np.ascontiguousarray(o["trk_n_owned"], np.int32)),
+                       _i32(np.ascontiguousarray(o["hit_ids"], np.int32)), _p(drow, C.c_uint8), _i32(ry), _i32(rz))
+    return drow[:nh], ry[:nh], rz[:nh]
+
+
+def decompress(trk_hit_offset, trk_n_owned, drow, ry, rz):
+    """orc_decompress: (row, y, z) of every hit from the residual streams (P51)."""
+    nh = int(len(drow))
+    row = np.zeros(max(nh, 1), np.int32)
+    y = np.zeros(max(nh, 1), np.int32)
+    z = np.zeros(max(nh, 1), np.int32)
+    lib().orc_decompress(C.c_int64(len(trk_n_owned)), _i32(np.ascontiguousarray(trk_hit_offset, np.int32)),
+                         _i32(np.ascontiguousarray(trk_n_owned, np.int32)),
+                         _p(np.ascontiguousarray(drow, np.uint8), C.c_uint8), _i32(np.ascontiguousarray(ry, np.int32)),
+                         _i32(np.ascontiguousarray(rz, np.int32)), _i32(row), _i32(y), _i32(z))
+    return row[:nh], y[:nh], z[:nh]
+
+
+def residual_histogram(trk_hit_offset, trk_n_owned, res, j_min=2):
+    hist = np.zeros(65536, np.int64)
+    lib().orc_residual_histogram(C.c_int64(len(trk_n_owned)), _i32(np.ascontiguousarray(trk_hit_offset, np.int32)),
+                                 _i32(np.ascontiguousarray(trk_n_owned, np.int32)),
+                                 _i32(np.ascontiguousarray(res, np.int32)), C.c_int32(j_min), _p(hist, C.c_int64))
+    return hist
+
+
+def entropy_bits(hist):
+    """Empirical entropy in bits per symbol of a histogram: what an ideal entropy coder (the paper's rANS stage) needs."""
+    h = np.asarray(hist, dtype=np.float64)
+    n = h.sum()
+    if n == 0:
+        return 0.0
+    p = h[h > 0] / n
+    return float(-(p * np.log2(p)).sum())
+
+
 def track_records(ev, o):
     """(sector, first_row, last_row) of the oracle's output tracks, from their owned hit lists."""
     sec, row = ev.sector_row()

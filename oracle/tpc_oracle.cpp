@@ -853,3 +853,97 @@ extern "C" void orc_refit_merged(const orc_params_t* p, double bz, int32_t n_sec
     out_sector[t] = cur;
   }
 }
+
+// ------------------------------------------------------------------------------------------------
+// NEXT-3: track-model residual transform.  Readings P50..P52.
+// ------------------------------------------------------------------------------------------------
+static inline int64_t floor_div(int64_t a, int64_t b) {   // b > 0
+  int64_t q = a / b;
+  if ((a % b != 0) && (a < 0)) --q;
+  return q;
+}
+
+// P50 predictor for hit j >= 2 from the previous hits' rows r[] and coordinates c[] (j indexes the current hit)
+static inline int64_t predict(const int32_t* r, const int32_t* c, int32_t j) {
+  const bool four = j >= 4 && r[j] - r[j - 1] == 1 && r[j - 1] - r[j - 2] == 1 && r[j - 2] - r[j - 3] == 1 &&
+                    r[j - 3] - r[j - 4] == 1;
+  if (four) return floor_div(2 * (int64_t)c[j - 1] + c[j - 2] - c[j - 4], 2);
+  const int64_t g1 = r[j - 1] - r[j - 2], g2 = r[j] - r[j - 1];
+  return (int64_t)c[j - 1] + floor_div(((int64_t)c[j - 1] - c[j - 2]) * g2, g1);
+}
+
+extern "C" void orc_compress(int32_t n_rows, const int32_t* y, const int32_t* z, const uint32_t* ro, int64_t n_sr,
+                             int64_t n_tracks, const int32_t* off, const int32_t* cnt, const int32_t* hit_ids,
+                             uint8_t* drow, int32_t* ry, int32_t* rz) {
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t t = 0; t < n_tracks; ++t) {
+    const int32_t m = cnt[t];
+    std::vector<int32_t> r(m), cy(m), cz(m);
+    for (int32_t j = 0; j < m; ++j) {
+      const int32_t h = hit_ids[off[t] + j];
+      int64_t lo = 0, hi = n_sr;
+      while (hi - lo > 1) {
+        int64_t mid = (lo + hi) / 2;
+        if (ro[mid] <= (uint32_t)h) lo = mid; else hi = mid;
+      }
+      r[j] = (int32_t)(lo % n_rows);
+      cy[j] = y[h];
+      cz[j] = z[h];
+    }
+    for (int32_t j = 0; j < m; ++j) {
+      const int64_t k = off[t] + j;
+      if (j == 0) {
+        drow[k] = (uint8_t)r[0];
+        ry[k] = cy[0];
+        rz[k] = cz[0];
+      } else if (j == 1) {
+        drow[k] = (uint8_t)(r[1] - r[0]);
+        ry[k] = cy[1] - cy[0];
+        rz[k] = cz[1] - cz[0];
+      } else {
+        drow[k] = (uint8_t)(r[j] - r[j - 1]);
+        ry[k] = (int32_t)(cy[j] - predict(r.data(), cy.data(), j));
+        rz[k] = (int32_t)(cz[j] - predict(r.data(), cz.data(), j));
+      }
+    }
+  }
+}
+
+extern "C" void orc_decompress(int64_t n_tracks, const int32_t* off, const int32_t* cnt, const uint8_t* drow,
+                               const int32_t* ry, const int32_t* rz, int32_t* row, int32_t* y, int32_t* z) {
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t t = 0; t < n_tracks; ++t) {
+    const int32_t m = cnt[t];
+    int32_t* r = row + off[t];
+    int32_t* cy = y + off[t];
+    int32_t* cz = z + off[t];
+    for (int32_t j = 0; j < m; ++j) {
+      const int64_t k = off[t] + j;
+      if (j == 0) {
+        r[0] = drow[k];
+        cy[0] = ry[k];
+        cz[0] = rz[k];
+      } else if (j == 1) {
+        r[1] = r[0] + drow[k];
+        cy[1] = cy[0] + ry[k];
+        cz[1] = cz[0] + rz[k];
+      } else {
+        r[j] = r[j - 1] + drow[k];
+        cy[j] = (int32_t)(predict(r, cy, j) + ry[k]);
+        cz[j] = (int32_t)(predict(r, cz, j) + rz[k]);
+      }
+    }
+  }
+}
+
+extern "C" void orc_residual_histogram(int64_t n_tracks, const int32_t* off, const int32_t* cnt, const int32_t* res,
+                                       int32_t j_min, int64_t* hist) {
+  for (int i = 0; i < 65536; ++i) hist[i] = 0;
+  for (int64_t t = 0; t < n_tracks; ++t)
+    for (int32_t j = j_min; j < cnt[t]; ++j) {
+      int64_t v = (int64_t)res[off[t] + j] + 32768;
+      if (v < 0) v = 0;
+      if (v > 65535) v = 65535;
+      ++hist[v];
+    }
+}

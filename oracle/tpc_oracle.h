@@ -140,6 +140,27 @@ void orc_refit_merged(const orc_params_t* p, double bz, int32_t n_sectors, int32
                       const int32_t* trk_n_owned, const int32_t* hit_ids, const int32_t* succ, const int32_t* pred,
                       double* par, double* cov, double* chi2, int32_t* n_used, int32_t* out_sector);
 
+/* ---- NEXT-3: track-model cluster compression, the residual transform (readings P50..P52) ----
+ * Lossless integer transform of the clusters an output track owns into small residuals against a predictor built
+ * from the track's previous hits (the entropy coder that follows is a separate 0.10 % line of the paper's Table 1).
+ * For track t with hits h_0..h_{m-1} (ascending rows r_j), for coordinate c in {y, z} (fixed-point ints), P50:
+ *   j = 0: drow = r_0, residual = c_0 (absolute);  j = 1: drow = r_1 - r_0, residual = c_1 - c_0;
+ *   j >= 2, the four previous hits in four consecutive rows and r_j = r_{j-1} + 1 (least-squares line through the last
+ *           four hits, extrapolated one row): pred = floor((2 c_{j-1} + c_{j-2} - c_{j-4}) / 2);
+ *   j >= 2 otherwise (two-point line with the row gaps g1 = r_{j-1} - r_{j-2}, g2 = r_j - r_{j-1}):
+ *           pred = c_{j-1} + floor((c_{j-1} - c_{j-2}) * g2 / g1);   residual = c_j - pred, drow = g2.
+ * floor = rounding towards minus infinity.  Outputs in hit-list order: drow[k], ry[k], rz[k], k = hit_offset + j. */
+void orc_compress(int32_t n_rows, const int32_t* y, const int32_t* z, const uint32_t* row_offsets, int64_t n_sr,
+                  int64_t n_tracks, const int32_t* trk_hit_offset, const int32_t* trk_n_owned, const int32_t* hit_ids,
+                  uint8_t* drow, int32_t* ry, int32_t* rz);
+/* Inverse (P51): rebuilds row, y, z of every hit from the residual streams, track by track. */
+void orc_decompress(int64_t n_tracks, const int32_t* trk_hit_offset, const int32_t* trk_n_owned, const uint8_t* drow,
+                    const int32_t* ry, const int32_t* rz, int32_t* row, int32_t* y, int32_t* z);
+/* P52: histogram of the residuals of the hits with j >= `j_min` of every track, clamped to [-32768, 32767]
+ * (bin = residual + 32768; the two edge bins collect everything beyond), 65536 bins. */
+void orc_residual_histogram(int64_t n_tracks, const int32_t* trk_hit_offset, const int32_t* trk_n_owned,
+                            const int32_t* res, int32_t j_min, int64_t* hist);
+
 int orc_num_threads(void);
 
 #ifdef __cplusplus
