@@ -269,6 +269,23 @@ def run_ours(args):
     r1e.record(stream)
     torch.cuda.synchronize()
     refit_merged_ms = r0e.elapsed_time(r1e) / 5
+    # NEXT-3: residual transform of the owned clusters + the entropy an ideal coder would reach on its histograms
+    for _ in range(2):
+        comp = trk.compress(y, z, ro, out, stream)
+    torch.cuda.synchronize()
+    r0e.record(stream)
+    for _ in range(5):
+        comp = trk.compress(y, z, ro, out, stream)
+    r1e.record(stream)
+    torch.cuda.synchronize()
+    compress_ms = r0e.elapsed_time(r1e) / 5
+
+    def _entropy(h):
+        h = h.cpu().numpy().astype(np.float64)
+        p = h[h > 0] / max(h.sum(), 1.0)
+        return float(-(p * np.log2(p)).sum())
+
+    comp_bits = {"ry": _entropy(comp["hist_ry"]), "rz": _entropy(comp["hist_rz"]), "drow": _entropy(comp["hist_drow"])}
 
     # ---- single-event latency (B = 1), for context -------------------------------------------------------
     ev1 = evs[0]
@@ -403,9 +420,11 @@ def run_ours(args):
                              f"> 126 MB L2; no explicit flush"},
             "tracks_per_s": len(tracks) * world * args.steps / (ms_max * 1e-3),
             "single_event_latency_ms": latency_ms,
-            "next": {"a6_refit_ms": refit_ms, "tracks_refitted": len(tracks), "a7_merge_ms": merge_ms, "a6_refit_merged_ms": refit_merged_ms,
+            "next": {"a6_refit_ms": refit_ms, "tracks_refitted": len(tracks), "a7_merge_ms": merge_ms, "a6_refit_merged_ms": refit_merged_ms, "a8_compress_ms": compress_ms,
+                     "compress_entropy_bits_per_symbol": comp_bits, "owned_clusters": int(len(hit_ids)),
+                     "compress_bits_per_owned_cluster": comp_bits["ry"] + comp_bits["rz"] + comp_bits["drow"],
                      "merge_links": int(merge_counts[0]), "merged_tracks": int(merge_counts[1]),
-                     "note": "tpc_refit, tpc_merge and tpc_refit_merged over the step's output tracks; outside the timed step"},
+                     "note": "tpc_refit, tpc_merge, tpc_refit_merged and tpc_compress over the step's output; outside the timed step"},
             "e2e": {"value": e2e_units / (e2e_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "steps": e2e_steps, "ms_per_step": e2e_max / e2e_steps,
                     "host_threads": T},

@@ -180,6 +180,31 @@ int tpc_refit_merged(tpc_tracker_t* t, const tpc_clusters_t* clusters, int64_t n
                      const tpc_tracks_out_t* tracks, const int32_t* succ, const int32_t* pred,
                      const tpc_merge_params_t* params, tpc_track_rec_t* refit_out);
 
+/* NEXT-3 (readings P50..P52 in DESIGN.md): track-model cluster compression, the residual transform.
+ * Every hit an output track owns is replaced by (row step, y residual, z residual) against an integer predictor
+ * built from the track's previous hits: j = 0 absolute; j = 1 first difference; j >= 2 the least-squares line
+ * through the last four hits when those and the hit sit in five consecutive rows, pred = floor((2 c1 + c2 - c4) / 2),
+ * else the two-point line with the row gaps, pred = c1 + floor((c1 - c2) g2 / g1).  Integer, lossless.
+ * All pointers [device]; drow, ry, rz: hit_capacity entries in hit-list order; hist_ry / hist_rz: 65536 uint32 bins of
+ * the residuals of the hits with j >= 2 (bin = residual + 32768, edge bins collect the rest), hist_drow: 256 bins of
+ * the row steps of the hits with j >= 1.  The histograms are what an entropy coder (the paper's rANS stage) needs. */
+typedef struct {
+  uint8_t* drow;
+  int32_t* ry;
+  int32_t* rz;
+  uint32_t* hist_ry;
+  uint32_t* hist_rz;
+  uint32_t* hist_drow;
+} tpc_compressed_t;
+/* clusters / n / tracks: the input and output of the handle's most recent tpc_track call (as for tpc_refit).
+ * Asynchronous on `stream`.  Errors: TPC_ERR_ARG, TPC_ERR_CUDA. */
+int tpc_compress(tpc_tracker_t* t, const tpc_clusters_t* clusters, int64_t n, void* stream,
+                 const tpc_tracks_out_t* tracks, const tpc_compressed_t* out);
+/* The inverse: row, y, z ([device], hit_capacity int32 each, hit-list order) from the residual streams and the tracks'
+ * hit_offset / n_hits.  Needs no cluster input. */
+int tpc_decompress(tpc_tracker_t* t, void* stream, const tpc_tracks_out_t* tracks, const tpc_compressed_t* in,
+                   int32_t* row, int32_t* y, int32_t* z);
+
 int tpc_tracker_destroy(tpc_tracker_t* t);
 
 const char* tpc_status_string(int status);

@@ -71,6 +71,12 @@ class MergeParams(C.Structure):
                 ("sector_angle", C.c_double)]
 
 
+class _Compressed(C.Structure):
+    """tpc_compressed_t"""
+    _fields_ = [("drow", C.c_void_p), ("ry", C.c_void_p), ("rz", C.c_void_p), ("hist_ry", C.c_void_p),
+                ("hist_rz", C.c_void_p), ("hist_drow", C.c_void_p)]
+
+
 class _TracksOut(C.Structure):
     _fields_ = [("tracks", C.c_void_p), ("track_capacity", C.c_int32), ("hit_capacity", C.c_int32),
                 ("hit_ids", C.c_void_p), ("counts", C.c_void_p)]
@@ -109,6 +115,10 @@ def load_library():
                               C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.tpc_refit_merged.argtypes = [C.c_void_p, C.POINTER(_Clusters), C.c_int64, C.c_void_p, C.POINTER(_TracksOut),
                                      C.c_void_p, C.c_void_p, C.POINTER(MergeParams), C.c_void_p]
+    lib.tpc_compress.argtypes = [C.c_void_p, C.POINTER(_Clusters), C.c_int64, C.c_void_p, C.POINTER(_TracksOut),
+                                 C.POINTER(_Compressed)]
+    lib.tpc_decompress.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_TracksOut), C.POINTER(_Compressed), C.c_void_p,
+                                   C.c_void_p, C.c_void_p]
     lib.tpc_tracker_destroy.argtypes = [C.c_void_p]
     lib.tpc_status_string.argtypes = [C.c_int]
     lib.tpc_status_string.restype = C.c_char_p
@@ -295,6 +305,37 @@ class Tracker:
                                                _ptr(succ), _ptr(pred),
                                                C.byref(params) if params is not None else None, _ptr(ref)))
         return ref
+
+    def compress(self, y, z, row_offsets, out: "TracksOut", stream=None):
+        """tpc_compress on the output of the last track() call: dict of device tensors drow (uint8), ry, rz (int32) in
+        hit-list order and the histograms hist_ry, hist_rz (65536), hist_drow (256)."""
+        import torch
+        dev = out.hit_ids.device
+        hc = int(out.hit_ids.shape[0])
+        c = dict(drow=torch.zeros(max(hc, 1), dtype=torch.uint8, device=dev),
+                 ry=torch.zeros(max(hc, 1), dtype=torch.int32, device=dev),
+                 rz=torch.zeros(max(hc, 1), dtype=torch.int32, device=dev),
+                 hist_ry=torch.zeros(65536, dtype=torch.int32, device=dev),
+                 hist_rz=torch.zeros(65536, dtype=torch.int32, device=dev),
+                 hist_drow=torch.zeros(256, dtype=torch.int32, device=dev))
+        cl = _Clusters(_ptr(y), _ptr(z), _ptr(row_offsets))
+        o = _TracksOut(_ptr(out.tracks), int(out.tracks.shape[0] // 112), hc, _ptr(out.hit_ids), _ptr(out.counts))
+        cs = _Compressed(*[_ptr(c[k]) for k in ("drow", "ry", "rz", "hist_ry", "hist_rz", "hist_drow")])
+        self._check(self._lib.tpc_compress(self._h, C.byref(cl), C.c_int64(int(y.shape[0])), self._stream_ptr(stream),
+                                           C.byref(o), C.byref(cs)))
+        return c
+
+    def decompress(self, out: "TracksOut", comp: dict, stream=None):
+        """tpc_decompress: (row, y, z) int32 device tensors in hit-list order from the residual streams."""
+        import torch
+        dev = out.hit_ids.device
+        hc = int(out.hit_ids.shape[0])
+        row, yy, zz = (torch.zeros(max(hc, 1), dtype=torch.int32, device=dev) for _ in range(3))
+        o = _TracksOut(_ptr(out.tracks), int(out.tracks.shape[0] // 112), hc, _ptr(out.hit_ids), _ptr(out.counts))
+        cs = _Compressed(*[_ptr(comp[k]) for k in ("drow", "ry", "rz", "hist_ry", "hist_rz", "hist_drow")])
+        self._check(self._lib.tpc_decompress(self._h, self._stream_ptr(stream), C.byref(o), C.byref(cs), _ptr(row),
+                                             _ptr(yy), _ptr(zz)))
+        return row, yy, zz
 
     def track_host(self, y, z, row_offsets, tracks, hit_ids, counts, stream=None):
         """tpc_track_host: all arguments are HOST tensors (pinned for asynchronous copies): y, z int32 [n],

@@ -439,6 +439,29 @@ int tpc_refit_merged(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void
   return TPC_OK;
 }
 
+int tpc_compress(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* stream, const tpc_tracks_out_t* tracks,
+                 const tpc_compressed_t* out) {
+  if (!t || !cl || !tracks || !out || n < 0) return TPC_ERR_ARG;
+  if (!tracks->counts || tracks->track_capacity < 0 || tracks->hit_capacity < 0) return TPC_ERR_ARG;
+  if (!out->hist_ry || !out->hist_rz || !out->hist_drow) return TPC_ERR_ARG;
+  if (tracks->hit_capacity > 0 && (!tracks->hit_ids || !out->drow || !out->ry || !out->rz)) return TPC_ERR_ARG;
+  if (tracks->track_capacity > 0 && !tracks->tracks) return TPC_ERR_ARG;
+  // the row list of the output hits (a5) must be that of the call that produced `tracks`
+  if (!t->arena || n != t->last_n || cl->row_offsets != t->last_ro || cl->y != t->last_y || cl->z != t->last_z)
+    return TPC_ERR_ARG;
+  TPC_CUDA(t, launch_a8_compress(t, cl->y, cl->z, tracks, out, (cudaStream_t)stream));
+  return TPC_OK;
+}
+
+int tpc_decompress(tpc_tracker_t* t, void* stream, const tpc_tracks_out_t* tracks, const tpc_compressed_t* in,
+                   int32_t* row, int32_t* y, int32_t* z) {
+  if (!t || !tracks || !in || !tracks->counts || tracks->track_capacity < 0 || tracks->hit_capacity < 0) return TPC_ERR_ARG;
+  if (tracks->hit_capacity > 0 && (!in->drow || !in->ry || !in->rz || !row || !y || !z)) return TPC_ERR_ARG;
+  if (tracks->track_capacity > 0 && !tracks->tracks) return TPC_ERR_ARG;
+  TPC_CUDA(t, launch_a8_decompress(t, tracks, in, row, y, z, (cudaStream_t)stream));
+  return TPC_OK;
+}
+
 int tpc_track_host(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* stream, tpc_tracks_out_t* out) {
   if (!t || !cl || !out || n < 0) return TPC_ERR_ARG;
   if (!out->counts || out->track_capacity < 0 || out->hit_capacity < 0) return TPC_ERR_ARG;

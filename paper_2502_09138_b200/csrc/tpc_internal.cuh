@@ -141,6 +141,10 @@ cudaError_t launch_a6_refit(const tpc_tracker* t, const int32_t* y, const int32_
 cudaError_t launch_a6_refit_merged(const tpc_tracker* t, const tpc_merge_params_t* mp, const int32_t* y,
                                    const int32_t* z, const tpc_tracks_out_t* tracks, const int32_t* succ,
                                    const int32_t* pred, tpc_track_rec_t* refit_out, cudaStream_t st);
+cudaError_t launch_a8_compress(const tpc_tracker* t, const int32_t* y, const int32_t* z, const tpc_tracks_out_t* tracks,
+                               const tpc_compressed_t* c, cudaStream_t st);
+cudaError_t launch_a8_decompress(const tpc_tracker* t, const tpc_tracks_out_t* tracks, const tpc_compressed_t* c,
+                                 int32_t* row, int32_t* y, int32_t* z, cudaStream_t st);
 cudaError_t launch_a7_merge(const tpc_tracker* t, const tpc_merge_params_t* mp, const tpc_track_rec_t* tracks,
                             const int32_t* counts, int32_t cap, int32_t* succ, int32_t* pred, float* link_chi2,
                             int32_t* merge_counts, cudaStream_t st);

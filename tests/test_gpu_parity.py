@@ -528,6 +528,44 @@ def test_merge_handmade_membrane_and_wraparound(orc):
     trk.close()
 
 
+def test_compress_residual_streams_bit_exact_and_lossless(orc):
+    """NEXT-3 through the C ABI: tpc_compress against orc_compress (integer -> bit-exact streams and histograms) and
+    tpc_decompress back to the owned clusters, on a central event, the stress config (row gaps, short tracks) and a
+    40-row geometry; tracks longer than one 32-hit chunk exercise the carried predecessors."""
+    import torch
+    from gen.events import Config
+    from paper_2502_09138_b200 import Tracker
+    from paper_2502_09138_b200.events import geometry_from_event, upload
+    cfg40 = Config("one_sector_40_rows", n_sectors=1, open_sector=True, tracks_per_collision=300, pt_min=0.3, noise=0.05,
+                   n_rows=40)
+    for ev, label in ((make_event(1, 1000), "cfg1"), (make_event(4), "cfg4"), (make_event(cfg40, seed=7), "40 rows")):
+        trk = Tracker(geometry_from_event(ev))
+        y, z, ro = upload(ev)
+        out = trk.track(y, z, ro)
+        comp = trk.compress(y, z, ro, out)
+        row_d, y_d, z_d = trk.decompress(out, comp)
+        tracks, hit_ids, _ = out.to_host()
+        nh = len(hit_ids)
+        # the oracle transforms the device's own tracks: the comparison isolates the transform
+        o = dict(trk_seed=np.arange(len(tracks)), trk_hit_offset=tracks["hit_offset"].astype(np.int32),
+                 trk_n_owned=tracks["n_hits"].astype(np.int32), hit_ids=hit_ids)
+        drow, ry, rz = orc.compress(ev, o)
+        assert np.array_equal(comp["drow"][:nh].cpu().numpy(), drow), label
+        assert np.array_equal(comp["ry"][:nh].cpu().numpy(), ry) and np.array_equal(comp["rz"][:nh].cpu().numpy(), rz), label
+        for key, res in (("hist_ry", ry), ("hist_rz", rz)):
+            ref = orc.residual_histogram(o["trk_hit_offset"], o["trk_n_owned"], res, 2)
+            assert np.array_equal(comp[key].cpu().numpy().astype(np.int64), ref), (label, key)
+        first = np.ones(nh, bool)
+        first[o["trk_hit_offset"]] = False
+        assert np.array_equal(comp["hist_drow"].cpu().numpy(), np.bincount(drow[first], minlength=256)), label
+        sec, rw = ev.sector_row()
+        assert np.array_equal(row_d[:nh].cpu().numpy(), rw[hit_ids]), label
+        assert np.array_equal(y_d[:nh].cpu().numpy(), ev.y[hit_ids]) and np.array_equal(z_d[:nh].cpu().numpy(), ev.z[hit_ids])
+        hy, hz = orc.entropy_bits(comp["hist_ry"].cpu().numpy()), orc.entropy_bits(comp["hist_rz"].cpu().numpy())
+        print(f"[compress] {label}: {nh} owned hits of {ev.n} clusters, residual entropy y {hy:.2f} z {hz:.2f} bits")
+        trk.close()
+
+
 def test_refit_rejects_foreign_input(orc):
     import torch
     from paper_2502_09138_b200 import Tracker
