@@ -52,6 +52,7 @@ def lib():
         _lib.orc_rotate.restype = C.c_int
         _lib.orc_match_chi2.restype = C.c_double
         _lib.orc_merge.restype = C.c_int64
+        _lib.orc_clusterize.restype = C.c_int64
     return _lib
 
 
@@ -290,6 +291,26 @@ def entropy_bits(hist):
         return 0.0
     p = h[h > 0] / n
     return float(-(p * np.log2(p)).sum())
+
+
+CLUSTER_Q_PEAK_MIN = 6     # P53: smallest ADC value of a peak
+
+
+def clusterize(d, n_per_side=18, pad_units=256, time_units=330, q_peak_min=CLUSTER_Q_PEAK_MIN):
+    """orc_clusterize on gen.digits.Digits (duck-typed: n_sectors, n_rows, n_pads, n_time, pad, time, adc, offsets).
+    Returns dict(y, z, qtot, qmax, row_offsets)."""
+    cap = max(int(d.pad.shape[0]), 1)
+    y = np.zeros(cap, np.int32)
+    z = np.zeros(cap, np.int32)
+    qt = np.zeros(cap, np.int32)
+    qm = np.zeros(cap, np.int32)
+    ro = np.zeros(d.n_sectors * d.n_rows + 1, np.uint32)
+    u16 = lambda a: _p(np.ascontiguousarray(a, np.uint16), C.c_uint16)      # noqa: E731
+    nc = lib().orc_clusterize(C.c_int32(d.n_sectors), C.c_int32(d.n_rows), C.c_int32(n_per_side), C.c_int32(d.n_pads),
+                              C.c_int32(d.n_time), C.c_int32(pad_units), C.c_int32(time_units), C.c_int32(q_peak_min),
+                              u16(d.pad), u16(d.time), u16(d.adc), _u32(np.ascontiguousarray(d.offsets, np.uint32)),
+                              _i32(y), _i32(z), _i32(qt), _i32(qm), _u32(ro))
+    return dict(y=y[:nc].copy(), z=z[:nc].copy(), qtot=qt[:nc].copy(), qmax=qm[:nc].copy(), row_offsets=ro)
 
 
 def track_records(ev, o):

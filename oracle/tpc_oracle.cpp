@@ -947,3 +947,58 @@ extern "C" void orc_residual_histogram(int64_t n_tracks, const int32_t* off, con
       ++hist[v];
     }
 }
+
+// ------------------------------------------------------------------------------------------------
+// NEXT-2: clusterizer.  Readings P53..P56.  A dense (time x pad) image per row.
+// ------------------------------------------------------------------------------------------------
+static inline int64_t rdiv(int64_t a, int64_t b) {   // floor((2a + b) / (2b)), b > 0: round to nearest, halves up
+  const int64_t n = 2 * a + b, d = 2 * b;
+  int64_t q = n / d;
+  if ((n % d != 0) && (n < 0)) --q;
+  return q;
+}
+
+extern "C" int64_t orc_clusterize(int32_t n_sectors, int32_t n_rows, int32_t n_per_side, int32_t n_pads,
+                                  int32_t n_time, int32_t pad_units, int32_t time_units, int32_t q_peak_min,
+                                  const uint16_t* pad, const uint16_t* time, const uint16_t* adc,
+                                  const uint32_t* doff, int32_t* y, int32_t* z, int32_t* qtot, int32_t* qmax,
+                                  uint32_t* row_offsets) {
+  const int64_t n_sr = (int64_t)n_sectors * n_rows;
+  const int64_t W = n_pads + 2, H = n_time + 2;   // one empty cell of margin all around
+  std::vector<int32_t> img((size_t)(W * H), 0);
+  const int64_t y_off = ((int64_t)(n_pads - 1) * pad_units) / 2;   // non-negative: floor
+  int64_t nc = 0;
+  row_offsets[0] = 0;
+  for (int64_t sr = 0; sr < n_sr; ++sr) {
+    const int32_t side = (int32_t)((sr / n_rows) / n_per_side) % 2;
+    for (uint32_t i = doff[sr]; i < doff[sr + 1]; ++i) img[(size_t)((time[i] + 1) * W + pad[i] + 1)] = adc[i];
+    for (uint32_t i = doff[sr]; i < doff[sr + 1]; ++i) {   // digits ascend by (time, pad): so do the peaks (P55)
+      const int32_t a = adc[i];
+      if (a < q_peak_min) continue;
+      const int64_t c = (int64_t)(time[i] + 1) * W + pad[i] + 1;
+      bool peak = true;
+      int64_t Q = 0, Sy = 0, St = 0;
+      for (int dt = -1; dt <= 1; ++dt)
+        for (int dp = -1; dp <= 1; ++dp) {
+          const int32_t v = img[(size_t)(c + dt * W + dp)];
+          Q += v;
+          Sy += (int64_t)v * dp;
+          St += (int64_t)v * dt;
+          if (dt == 0 && dp == 0) continue;
+          const bool before = dt < 0 || (dt == 0 && dp < 0);   // precedes (t, p) in (time, pad) order
+          if (before ? !(a > v) : !(a >= v)) peak = false;
+        }
+      if (!peak) continue;
+      const int64_t yy = (int64_t)pad[i] * pad_units - y_off + rdiv((int64_t)pad_units * Sy, Q);
+      const int64_t zz = (int64_t)time[i] * time_units + rdiv((int64_t)time_units * St, Q);
+      y[nc] = (int32_t)yy;
+      z[nc] = (int32_t)(side ? -zz : zz);
+      qtot[nc] = (int32_t)Q;
+      qmax[nc] = a;
+      ++nc;
+    }
+    for (uint32_t i = doff[sr]; i < doff[sr + 1]; ++i) img[(size_t)((time[i] + 1) * W + pad[i] + 1)] = 0;
+    row_offsets[sr + 1] = (uint32_t)nc;
+  }
+  return nc;
+}

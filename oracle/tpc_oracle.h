@@ -161,6 +161,22 @@ void orc_decompress(int64_t n_tracks, const int32_t* trk_hit_offset, const int32
 void orc_residual_histogram(int64_t n_tracks, const int32_t* trk_hit_offset, const int32_t* trk_n_owned,
                             const int32_t* res, int32_t j_min, int64_t* hist);
 
+/* ---- NEXT-2: clusterizer, digits -> clusters (readings P53..P56) ----
+ * Digits of a (sector,row): cells (pad, time bin) with an ADC value >= 1, unique, ascending by (time, pad) (P56).
+ * P53 peak: a digit with adc >= q_peak_min that is greater than each of its 8 neighbours preceding it in (time, pad)
+ *   order and greater than or equal to each of the others (absent cells count 0): a plateau yields its first cell.
+ * P54 cluster of a peak at (p, t): over its 3 x 3 block Q = sum a, Sy = sum a dp, St = sum a dt;
+ *   y = p * pad_units - floor((n_pads - 1) * pad_units / 2) + rdiv(pad_units * Sy, Q),
+ *   |z| = t * time_units + rdiv(time_units * St, Q), z < 0 on the C side (side = (sector / n_per_side) % 2),
+ *   rdiv(a, b) = floor((2 a + b) / (2 b)); qtot = Q, qmax = the peak's adc.  A digit may belong to several blocks.
+ * P55 order: the clusters of a (sector,row) ascend by (time, pad) of their peak.
+ * Outputs y, z, qtot, qmax (capacity = number of digits suffices), row_offsets[n_sectors * n_rows + 1].
+ * Returns the number of clusters. */
+int64_t orc_clusterize(int32_t n_sectors, int32_t n_rows, int32_t n_per_side, int32_t n_pads, int32_t n_time,
+                       int32_t pad_units, int32_t time_units, int32_t q_peak_min, const uint16_t* pad,
+                       const uint16_t* time, const uint16_t* adc, const uint32_t* digit_offsets, int32_t* y,
+                       int32_t* z, int32_t* qtot, int32_t* qmax, uint32_t* row_offsets);
+
 int orc_num_threads(void);
 
 #ifdef __cplusplus
