@@ -286,6 +286,24 @@ def run_ours(args):
         return float(-(p * np.log2(p)).sum())
 
     comp_bits = {"ry": _entropy(comp["hist_ry"]), "rz": _entropy(comp["hist_rz"]), "drow": _entropy(comp["hist_drow"])}
+    # NEXT-2: clusterizer on the synthetic digits of ONE configs[1] event (gen/digits.py)
+    from gen.digits import make_digits
+    dg = make_digits(evs[0])
+    trk_c = Tracker(geometry_from_event(evs[0]))
+    u16 = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.int16)).to(dev).view(torch.uint16)   # noqa: E731
+    d_pad, d_time, d_adc = u16(dg.pad), u16(dg.time), u16(dg.adc)
+    d_off = torch.from_numpy(dg.offsets.view(np.int32).copy()).to(dev)
+    for _ in range(2):
+        cl_out = trk_c.clusterize(d_pad, d_time, d_adc, d_off, dg.n_pads, stream=stream)
+    torch.cuda.synchronize()
+    r0e.record(stream)
+    for _ in range(5):
+        cl_out = trk_c.clusterize(d_pad, d_time, d_adc, d_off, dg.n_pads, stream=stream)
+    r1e.record(stream)
+    torch.cuda.synchronize()
+    clusterize_ms = r0e.elapsed_time(r1e) / 5
+    n_found = int(cl_out["counts"][0])
+    trk_c.close()
 
     # ---- single-event latency (B = 1), for context -------------------------------------------------------
     ev1 = evs[0]
@@ -420,11 +438,13 @@ def run_ours(args):
                              f"> 126 MB L2; no explicit flush"},
             "tracks_per_s": len(tracks) * world * args.steps / (ms_max * 1e-3),
             "single_event_latency_ms": latency_ms,
-            "next": {"a6_refit_ms": refit_ms, "tracks_refitted": len(tracks), "a7_merge_ms": merge_ms, "a6_refit_merged_ms": refit_merged_ms, "a8_compress_ms": compress_ms,
+            "next": {"a6_refit_ms": refit_ms, "tracks_refitted": len(tracks), "a7_merge_ms": merge_ms, "a6_refit_merged_ms": refit_merged_ms, "a8_compress_ms": compress_ms, "a9_clusterize_ms_one_event": clusterize_ms,
+                     "clusterize_digits": int(dg.n), "clusterize_clusters": n_found,
+                     "clusterize_digits_per_s": dg.n / (clusterize_ms * 1e-3),
                      "compress_entropy_bits_per_symbol": comp_bits, "owned_clusters": int(len(hit_ids)),
                      "compress_bits_per_owned_cluster": comp_bits["ry"] + comp_bits["rz"] + comp_bits["drow"],
                      "merge_links": int(merge_counts[0]), "merged_tracks": int(merge_counts[1]),
-                     "note": "tpc_refit, tpc_merge, tpc_refit_merged and tpc_compress over the step's output; outside the timed step"},
+                     "note": "tpc_refit, tpc_merge, tpc_refit_merged, tpc_compress over the step's output and tpc_clusterize on one event's digits; outside the timed step"},
             "e2e": {"value": e2e_units / (e2e_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "steps": e2e_steps, "ms_per_step": e2e_max / e2e_steps,
                     "host_threads": T},

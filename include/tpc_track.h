@@ -205,6 +205,42 @@ int tpc_compress(tpc_tracker_t* t, const tpc_clusters_t* clusters, int64_t n, vo
 int tpc_decompress(tpc_tracker_t* t, void* stream, const tpc_tracks_out_t* tracks, const tpc_compressed_t* in,
                    int32_t* row, int32_t* y, int32_t* z);
 
+/* NEXT-2 (readings P53..P56 in DESIGN.md): clusterizer in front of the path, digits -> clusters.
+ * Digits of a (sector,row): cells (pad, time bin) with an ADC value >= 1, unique, ascending by (time, pad).
+ * Peak (P53): adc >= q_peak_min, greater than each of its 8 neighbours that precede it in (time, pad) order and
+ * greater or equal to the others (absent cells count 0).  Cluster (P54): over the peak's 3 x 3 block Q = sum a,
+ * Sy = sum a dp, St = sum a dt; y = p * pad_units - floor((n_pads - 1) * pad_units / 2) + rdiv(pad_units * Sy, Q),
+ * |z| = t * time_units + rdiv(time_units * St, Q), negative on the C side ((sector / n_per_side) % 2 == 1),
+ * rdiv(a, b) = floor((2a + b) / (2b)).  Clusters of a (sector,row) ascend by (time, pad) of their peak (P55). */
+typedef struct {
+  const uint16_t* pad;       /* [device] n_digits */
+  const uint16_t* time;      /* [device] n_digits */
+  const uint16_t* adc;       /* [device] n_digits, 1..1023 */
+  const uint32_t* offsets;   /* [device] n_sectors*n_rows + 1 CSR offsets into the digit arrays */
+} tpc_digits_t;
+typedef struct {
+  int32_t n_pads;            /* pads per row (<= 32768); pad p is y = (p - (n_pads-1)/2) * pad pitch */
+  int32_t n_per_side;        /* sectors per z side: 18 */
+  int32_t pad_units;         /* pad pitch in fixed-point units: 256 = 0.4 cm */
+  int32_t time_units;        /* time-bin width in fixed-point units of z: 330 */
+  int32_t q_peak_min;        /* P53: 6 */
+} tpc_cluster_params_t;
+void tpc_default_cluster_params(tpc_cluster_params_t* p);
+typedef struct {
+  int32_t* y;                /* [device] capacity; with z and row_offsets the input format of tpc_track */
+  int32_t* z;
+  int32_t* qtot;             /* [device] capacity: charge of the 3 x 3 block */
+  int32_t* qmax;             /* [device] capacity: ADC value of the peak */
+  uint32_t* row_offsets;     /* [device] n_sectors*n_rows + 1 */
+  int32_t* counts;           /* [device] int32[2]: [0] clusters found, [1] 1 iff that exceeds capacity (the excess is
+                                not written; row_offsets still describe the full result) */
+  int32_t capacity;
+} tpc_clusters_out_t;
+/* Geometry (n_sectors, n_rows) from the handle.  Asynchronous on `stream`.  Errors: TPC_ERR_ARG, TPC_ERR_NOMEM,
+ * TPC_ERR_CUDA. */
+int tpc_clusterize(tpc_tracker_t* t, const tpc_digits_t* digits, int64_t n_digits, const tpc_cluster_params_t* params,
+                   void* stream, const tpc_clusters_out_t* out);
+
 int tpc_tracker_destroy(tpc_tracker_t* t);
 
 const char* tpc_status_string(int status);

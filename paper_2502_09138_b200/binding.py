@@ -77,6 +77,21 @@ class _Compressed(C.Structure):
                 ("hist_rz", C.c_void_p), ("hist_drow", C.c_void_p)]
 
 
+class ClusterParams(C.Structure):
+    """tpc_cluster_params_t"""
+    _fields_ = [("n_pads", C.c_int32), ("n_per_side", C.c_int32), ("pad_units", C.c_int32), ("time_units", C.c_int32),
+                ("q_peak_min", C.c_int32)]
+
+
+class _Digits(C.Structure):
+    _fields_ = [("pad", C.c_void_p), ("time", C.c_void_p), ("adc", C.c_void_p), ("offsets", C.c_void_p)]
+
+
+class _ClustersOut(C.Structure):
+    _fields_ = [("y", C.c_void_p), ("z", C.c_void_p), ("qtot", C.c_void_p), ("qmax", C.c_void_p),
+                ("row_offsets", C.c_void_p), ("counts", C.c_void_p), ("capacity", C.c_int32)]
+
+
 class _TracksOut(C.Structure):
     _fields_ = [("tracks", C.c_void_p), ("track_capacity", C.c_int32), ("hit_capacity", C.c_int32),
                 ("hit_ids", C.c_void_p), ("counts", C.c_void_p)]
@@ -119,6 +134,10 @@ def load_library():
                                  C.POINTER(_Compressed)]
     lib.tpc_decompress.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_TracksOut), C.POINTER(_Compressed), C.c_void_p,
                                    C.c_void_p, C.c_void_p]
+    lib.tpc_default_cluster_params.argtypes = [C.POINTER(ClusterParams)]
+    lib.tpc_default_cluster_params.restype = None
+    lib.tpc_clusterize.argtypes = [C.c_void_p, C.POINTER(_Digits), C.c_int64, C.POINTER(ClusterParams), C.c_void_p,
+                                   C.POINTER(_ClustersOut)]
     lib.tpc_tracker_destroy.argtypes = [C.c_void_p]
     lib.tpc_status_string.argtypes = [C.c_int]
     lib.tpc_status_string.restype = C.c_char_p
@@ -336,6 +355,29 @@ class Tracker:
         self._check(self._lib.tpc_decompress(self._h, self._stream_ptr(stream), C.byref(o), C.byref(cs), _ptr(row),
                                              _ptr(yy), _ptr(zz)))
         return row, yy, zz
+
+    def clusterize(self, pad, time, adc, offsets, n_pads: int, params: "ClusterParams | None" = None, capacity=None,
+                   stream=None):
+        """tpc_clusterize: digits (uint16 CUDA tensors pad, time, adc; int32 CSR offsets) -> dict of device tensors
+        y, z, qtot, qmax (int32), row_offsets (int32 bits of uint32), counts (int32[2])."""
+        import torch
+        nd = int(pad.shape[0])
+        cap = int(capacity if capacity is not None else max(nd // 3, 16))
+        dev = offsets.device
+        out = dict(y=torch.zeros(cap, dtype=torch.int32, device=dev), z=torch.zeros(cap, dtype=torch.int32, device=dev),
+                   qtot=torch.zeros(cap, dtype=torch.int32, device=dev), qmax=torch.zeros(cap, dtype=torch.int32, device=dev),
+                   row_offsets=torch.zeros(self.n_sectors * self.n_rows + 1, dtype=torch.int32, device=dev),
+                   counts=torch.zeros(2, dtype=torch.int32, device=dev))
+        if params is None:
+            params = ClusterParams()
+            self._lib.tpc_default_cluster_params(C.byref(params))
+        params.n_pads = int(n_pads)
+        d = _Digits(_ptr(pad), _ptr(time), _ptr(adc), _ptr(offsets))
+        o = _ClustersOut(_ptr(out["y"]), _ptr(out["z"]), _ptr(out["qtot"]), _ptr(out["qmax"]), _ptr(out["row_offsets"]),
+                         _ptr(out["counts"]), cap)
+        self._check(self._lib.tpc_clusterize(self._h, C.byref(d), C.c_int64(nd), C.byref(params),
+                                             self._stream_ptr(stream), C.byref(o)))
+        return out
 
     def track_host(self, y, z, row_offsets, tracks, hit_ids, counts, stream=None):
         """tpc_track_host: all arguments are HOST tensors (pinned for asynchronous copies): y, z int32 [n],

@@ -301,6 +301,7 @@ int tpc_tracker_create(const tpc_geometry_t* geo, const tpc_field_t* field, tpc_
   g.gap_w = equal_w ? nullptr : (const int32_t*)((char*)t->geom_blob + o_w);
   if (e == cudaSuccess) e = setup_a1_attributes(t);
   if (e == cudaSuccess) e = setup_a4_attributes(t);
+  if (e == cudaSuccess) e = setup_a9_attributes();
   for (int k = 0; k < TIMING_SETS * 6 && e == cudaSuccess; ++k) e = cudaEventCreate(&t->ev[k]);
   if (e != cudaSuccess) {
     rc = e == cudaErrorMemoryAllocation ? TPC_ERR_NOMEM : TPC_ERR_CUDA;
@@ -318,6 +319,10 @@ int tpc_tracker_destroy(tpc_tracker_t* t) {
   if (t->arena) cudaFree(t->arena);
   if (t->host_arena) cudaFree(t->host_arena);
   if (t->geom_blob) cudaFree(t->geom_blob);
+  if (t->cl_keys) cudaFree(t->cl_keys);
+  if (t->cl_flag) cudaFree(t->cl_flag);
+  if (t->cl_parked) cudaFree(t->cl_parked);
+  if (t->cl_row_count) cudaFree(t->cl_row_count);
   if (t->merge_sec) cudaFree(t->merge_sec);
   if (t->merge_best) cudaFree(t->merge_best);
   if (t->merge_chi2) cudaFree(t->merge_chi2);
@@ -459,6 +464,48 @@ int tpc_decompress(tpc_tracker_t* t, void* stream, const tpc_tracks_out_t* track
   if (tracks->hit_capacity > 0 && (!in->drow || !in->ry || !in->rz || !row || !y || !z)) return TPC_ERR_ARG;
   if (tracks->track_capacity > 0 && !tracks->tracks) return TPC_ERR_ARG;
   TPC_CUDA(t, launch_a8_decompress(t, tracks, in, row, y, z, (cudaStream_t)stream));
+  return TPC_OK;
+}
+
+void tpc_default_cluster_params(tpc_cluster_params_t* p) {
+  if (!p) return;
+  p->n_pads = 223;
+  p->n_per_side = 18;
+  p->pad_units = 256;
+  p->time_units = 330;
+  p->q_peak_min = 6;
+}
+
+int tpc_clusterize(tpc_tracker_t* t, const tpc_digits_t* d, int64_t n_digits, const tpc_cluster_params_t* params,
+                   void* stream, const tpc_clusters_out_t* out) {
+  if (!t || !d || !out || !params || n_digits < 0 || n_digits >= ((int64_t)1 << 31)) return TPC_ERR_ARG;
+  if (!d->offsets || !out->row_offsets || !out->counts || out->capacity < 0) return TPC_ERR_ARG;
+  if (n_digits > 0 && (!d->pad || !d->time || !d->adc)) return TPC_ERR_ARG;
+  if (out->capacity > 0 && (!out->y || !out->z || !out->qtot || !out->qmax)) return TPC_ERR_ARG;
+  if (params->n_pads < 1 || params->n_pads > 32768 || params->n_per_side < 1 || params->pad_units < 1 ||
+      params->time_units < 1 || params->q_peak_min < 1)
+    return TPC_ERR_ARG;
+  const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
+  if (n_digits > t->cl_cap || !t->cl_row_count) {
+    TPC_CUDA(t, cudaDeviceSynchronize());
+    if (t->cl_keys) cudaFree(t->cl_keys);
+    if (t->cl_flag) cudaFree(t->cl_flag);
+    if (t->cl_parked) cudaFree(t->cl_parked);
+    if (t->cl_row_count) cudaFree(t->cl_row_count);
+    t->cl_keys = nullptr; t->cl_flag = nullptr; t->cl_parked = nullptr; t->cl_row_count = nullptr; t->cl_cap = 0;
+    const size_t cap = (size_t)(n_digits > 0 ? n_digits + n_digits / 8 : 1);
+    cudaError_t e = cudaMalloc(&t->cl_keys, cap * 4);
+    if (e == cudaSuccess) e = cudaMalloc(&t->cl_flag, cap);
+    if (e == cudaSuccess) e = cudaMalloc(&t->cl_parked, cap * 16);
+    if (e == cudaSuccess) e = cudaMalloc(&t->cl_row_count, (size_t)(R + 1) * 4);
+    if (e == cudaErrorMemoryAllocation) {
+      cudaGetLastError();
+      return TPC_ERR_NOMEM;
+    }
+    if (e != cudaSuccess) return fail_cuda(t, e, "cudaMalloc(clusterizer scratch)");
+    t->cl_cap = (int64_t)cap;
+  }
+  TPC_CUDA(t, launch_a9_clusterize(t, params, d, n_digits, out, (cudaStream_t)stream));
   return TPC_OK;
 }
 

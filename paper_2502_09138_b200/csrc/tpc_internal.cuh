@@ -107,6 +107,9 @@ struct tpc_tracker {
   Scratch s;
   // a7 (tpc_merge) scratch, grown on demand: per-sector track ranges, best partner and its chi2 for both directions
   int32_t* merge_sec; int32_t* merge_best; double* merge_chi2; int64_t merge_cap;
+  // a9 (tpc_clusterize) scratch, grown on demand: sorted keys of rows too long for shared memory, peak flags and
+  // parked clusters per digit, clusters per row
+  uint32_t* cl_keys; uint8_t* cl_flag; int4* cl_parked; uint32_t* cl_row_count; int64_t cl_cap;
   int64_t last_n; const uint32_t* last_ro; const int32_t* last_y; const int32_t* last_z;
   // stage timing
   int timing; int64_t timed_calls; cudaEvent_t ev[TIMING_SETS * 6];
@@ -145,6 +148,9 @@ cudaError_t launch_a8_compress(const tpc_tracker* t, const int32_t* y, const int
                                const tpc_compressed_t* c, cudaStream_t st);
 cudaError_t launch_a8_decompress(const tpc_tracker* t, const tpc_tracks_out_t* tracks, const tpc_compressed_t* c,
                                  int32_t* row, int32_t* y, int32_t* z, cudaStream_t st);
+cudaError_t setup_a9_attributes();
+cudaError_t launch_a9_clusterize(const tpc_tracker* t, const tpc_cluster_params_t* cp, const tpc_digits_t* d,
+                                 int64_t n_digits, const tpc_clusters_out_t* out, cudaStream_t st);
 cudaError_t launch_a7_merge(const tpc_tracker* t, const tpc_merge_params_t* mp, const tpc_track_rec_t* tracks,
                             const int32_t* counts, int32_t cap, int32_t* succ, int32_t* pred, float* link_chi2,
                             int32_t* merge_counts, cudaStream_t st);

@@ -566,6 +566,62 @@ def test_compress_residual_streams_bit_exact_and_lossless(orc):
         trk.close()
 
 
+def _upload_digits(d):
+    import torch
+    f = lambda a, t: torch.from_numpy(np.ascontiguousarray(a).view(t)).cuda()      # noqa: E731
+    return (f(d.pad, np.int16).view(torch.uint16) if hasattr(torch, "uint16") else f(d.pad, np.int16),
+            f(d.time, np.int16).view(torch.uint16) if hasattr(torch, "uint16") else f(d.time, np.int16),
+            f(d.adc, np.int16).view(torch.uint16) if hasattr(torch, "uint16") else f(d.adc, np.int16),
+            f(d.offsets, np.int32))
+
+
+def test_clusterizer_bit_exact_and_feeds_the_tracker(orc):
+    """NEXT-2 through the C ABI: tpc_clusterize against orc_clusterize (integer -> bit-exact y, z, charges and CSR
+    offsets, in order) on a central event, on rows longer than the shared-memory staging (global-memory path) and on an
+    event with empty rows; then digits -> clusters -> tracks entirely on the device equals tracking the oracle's
+    clusters."""
+    import torch
+    from types import SimpleNamespace
+    from gen.digits import make_digits
+    from gen.events import Config
+    from paper_2502_09138_b200 import Tracker
+    from paper_2502_09138_b200.events import geometry_from_event
+    dense = Config("one_sector_dense", n_sectors=1, open_sector=True, tracks_per_collision=2500, pt_min=0.3, noise=0.05)
+    for ev, label in ((make_event(1, 1000), "cfg1"), (make_event(dense, seed=3), "long rows"),
+                      (make_event(1, 77, n_tracks=40), "empty rows")):
+        d = make_digits(ev)
+        c = orc.clusterize(d)
+        trk = Tracker(geometry_from_event(ev))
+        pad, time, adc, off = _upload_digits(d)
+        out = trk.clusterize(pad, time, adc, off, d.n_pads)
+        torch.cuda.synchronize()
+        nc = int(out["counts"][0])
+        assert int(out["counts"][1]) == 0 and nc == len(c["y"]), (label, nc, len(c["y"]))
+        assert np.array_equal(out["row_offsets"].cpu().numpy().view(np.uint32), c["row_offsets"]), label
+        for k in ("y", "z", "qtot", "qmax"):
+            assert np.array_equal(out[k][:nc].cpu().numpy(), c[k]), (label, k)
+        if label == "long rows":
+            assert np.diff(d.offsets.astype(np.int64)).max() > 12 * 1024        # the global-memory path ran
+        print(f"[clusterize] {label}: {d.n} digits -> {nc} clusters for {ev.n} deposited")
+        if label == "cfg1":
+            # the device's clusters straight into tpc_track; the oracle tracks its own (identical) clusters
+            res = trk.track(out["y"][:nc].contiguous(), out["z"][:nc].contiguous(), out["row_offsets"])
+            tracks, hit_ids, ns = res.to_host()
+            ev2 = SimpleNamespace(y=c["y"], z=c["z"], row_offsets=c["row_offsets"], n_sectors=ev.n_sectors, n_rows=ev.n_rows,
+                                  row_x=ev.row_x, cfg=ev.cfg, n=nc)
+            o = orc.track(ev2)
+            assert np.array_equal(hit_ids, o["hit_ids"]) and len(tracks) == len(o["trk_seed"]) > 6000
+        trk.close()
+    # capacity overflow: flagged, nothing written beyond
+    ev = make_event(0)
+    d = make_digits(ev)
+    trk = Tracker(geometry_from_event(ev))
+    out = trk.clusterize(*_upload_digits(d), d.n_pads, capacity=100)
+    torch.cuda.synchronize()
+    assert int(out["counts"][1]) == 1 and int(out["counts"][0]) > 100
+    trk.close()
+
+
 def test_refit_rejects_foreign_input(orc):
     import torch
     from paper_2502_09138_b200 import Tracker
