@@ -368,7 +368,8 @@ a2_neighbours_staged_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, con
 // memory and the pair loop runs over |U| x |D| window candidates only (a few, against hundreds of range pairs).
 // A cluster with more than A2_KEEP candidates on a side falls back to the nested scan.
 // ---------------------------------------------------------------------------------------------------------------
-constexpr int A2_KEEP = 12;
+constexpr int A2_KEEP = 20;   // in-window candidates kept per side (60 KB of lists per CTA); configs[3] literal: 12 -> 13.1 ms,
+                              // 20 -> 8.2 ms, 32 -> 10.9 ms, 48 -> 21.0 ms (fewer fallbacks against fewer resident CTAs)
 
 __device__ __forceinline__ int filter_side(const DevGeom& g, const int4* __restrict__ srt, const Window& w,
                                            const uint32_t* __restrict__ bs, int yh, int zh,
@@ -401,7 +402,7 @@ __global__ void __launch_bounds__(A2_THREADS)
 a2_neighbours_dense_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, const uint32_t* __restrict__ ro, const int4* __restrict__ srt,
                            const uint32_t* __restrict__ sec_key, const uint32_t* __restrict__ bin_start,
                            int32_t* __restrict__ link_up, int32_t* __restrict__ link_dn) {
-  __shared__ int cand[2][A2_KEEP][3][A2_THREADS];   // [side][slot][dy, dz, position][thread]: a thread reads only its column
+  extern __shared__ int cand[];   // [side][slot][dy, dz, position][thread]: a thread reads only its column
   if (ctl->bad_offsets) return;
   const int sr = blockIdx.x;
   const int r = sr % g.n_rows;
@@ -413,8 +414,8 @@ a2_neighbours_dense_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, cons
     bs_u = bin_start + (size_t)(sr + 1) * g.nb_stride;
     bs_d = bin_start + (size_t)(sr - 1) * g.nb_stride;
   }
-  int* const col_u = &cand[0][0][0][threadIdx.x];
-  int* const col_d = &cand[1][0][0][threadIdx.x];
+  int* const col_u = cand + threadIdx.x;
+  int* const col_d = cand + A2_KEEP * 3 * A2_THREADS + threadIdx.x;
   // gridDim.y CTAs share a row (dense rows hold thousands of clusters)
   for (uint32_t j = a + blockIdx.y * A2_THREADS + threadIdx.x; j < b; j += gridDim.y * A2_THREADS) {
     const int4 ch = srt[j];
@@ -516,6 +517,13 @@ a2_neighbours_weighted_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, c
 
 }  // namespace
 
+cudaError_t setup_a2_attributes() {
+  const int bytes = 2 * A2_KEEP * 3 * A2_THREADS * (int)sizeof(int);
+  cudaError_t e = cudaFuncSetAttribute(a2_neighbours_dense_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(a2_neighbours_dense_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
 cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64_t n, cudaStream_t st) {
   const int64_t R = (int64_t)t->g.n_sectors * t->g.n_rows;
   if (R == 0) return cudaSuccess;
@@ -528,9 +536,10 @@ cudaError_t launch_a2_neighbours(const tpc_tracker* t, const uint32_t* ro, int64
   int64_t per_row = (n / R + A2_THREADS - 1) / A2_THREADS;
   per_row = per_row < 1 ? 1 : (per_row > 64 ? 64 : per_row);
   const dim3 grid2((unsigned)R, (unsigned)per_row);
+  const size_t dense_smem = (size_t)2 * A2_KEEP * 3 * A2_THREADS * sizeof(int);
   if (t->g.gap_w) a2_neighbours_weighted_kernel<<<grid2, A2_THREADS, 0, st>>>(A2_ARGS);
-  else if (dense && fine) a2_neighbours_dense_kernel<true><<<grid2, A2_THREADS, 0, st>>>(A2_ARGS);
-  else if (dense) a2_neighbours_dense_kernel<false><<<grid2, A2_THREADS, 0, st>>>(A2_ARGS);
+  else if (dense && fine) a2_neighbours_dense_kernel<true><<<grid2, A2_THREADS, dense_smem, st>>>(A2_ARGS);
+  else if (dense) a2_neighbours_dense_kernel<false><<<grid2, A2_THREADS, dense_smem, st>>>(A2_ARGS);
   else if (fine) a2_neighbours_kernel<true><<<(unsigned)R, A2_THREADS, 0, st>>>(A2_ARGS);
   else if (t->a2_variant == 1) {
     const int chunks = (t->g.n_rows + A2S_ROWS - 1) / A2S_ROWS;

@@ -302,6 +302,7 @@ int tpc_tracker_create(const tpc_geometry_t* geo, const tpc_field_t* field, tpc_
   if (e == cudaSuccess) e = setup_a1_attributes(t);
   if (e == cudaSuccess) e = setup_a4_attributes(t);
   if (e == cudaSuccess) e = setup_a9_attributes();
+  if (e == cudaSuccess) e = setup_a2_attributes();
   for (int k = 0; k < TIMING_SETS * 6 && e == cudaSuccess; ++k) e = cudaEventCreate(&t->ev[k]);
   if (e != cudaSuccess) {
     rc = e == cudaErrorMemoryAllocation ? TPC_ERR_NOMEM : TPC_ERR_CUDA;

@@ -149,6 +149,7 @@ cudaError_t launch_a8_compress(const tpc_tracker* t, const int32_t* y, const int
 cudaError_t launch_a8_decompress(const tpc_tracker* t, const tpc_tracks_out_t* tracks, const tpc_compressed_t* c,
                                  int32_t* row, int32_t* y, int32_t* z, cudaStream_t st);
 cudaError_t setup_a9_attributes();
+cudaError_t setup_a2_attributes();
 cudaError_t launch_a9_clusterize(const tpc_tracker* t, const tpc_cluster_params_t* cp, const tpc_digits_t* d,
                                  int64_t n_digits, const tpc_clusters_out_t* out, cudaStream_t st);
 cudaError_t launch_a7_merge(const tpc_tracker* t, const tpc_merge_params_t* mp, const tpc_track_rec_t* tracks,
