@@ -3,11 +3,18 @@
 // (PAPER.md:29, :40 name the task only; BASELINE.json north_star names the five stages).
 // Independent of the CUDA path: no shared code, headers, tables or constants.
 //
-// Pins (tests/test_oracle_*.py): grid == brute force; mutual links; chain partition invariants;
-// transport == closed-form circle/helix and reversibility; Jacobian == central finite differences and
-// == long-double closed form; straight-line limit == weighted least squares (numpy lstsq); exact helices
-// reconstructed to 1e-4; <=1 owner per hit.  Unpinned by the paper: the free constants of orc_params_t and
-// the efficiency / fake-rate values themselves ("parity unpinned" beyond the 100 % zero-smearing case).
+// Pins (tests/test_oracle_*.py, all -m "not gpu"; the table is in DESIGN.md section 3): grid == brute force; mutual
+// links; chain partition invariants; transport == closed-form circle/helix and reversibility; Jacobian == central finite
+// differences and == long-double closed form; update == information form and, for Bz -> 0, weighted least squares
+// (numpy lstsq); the follower's rules (row search and gate, miss/stop logic, initial state, final transport) and the
+// selection filters on hand-made straight tracks with closed-form line-fit variances (test_oracle_follower_rules.py);
+// exact helices reconstructed to 1e-4; <= 1 owner per hit; refit == generator truth; rotation == plane geometry, the
+// generator's helix in the next sector and finite differences; merge rules on hand-made records; pitch-weighted cost on
+// hand-made unequal gaps; residual transform values, exactness on lines / parabolas and the lossless round trip;
+// clusterizer centroids, plateau and threshold rules worked out by hand and resolution against the digit generator.
+// No function is left "parity unpinned".  Unpinned by the paper: the free constants of orc_params_t (and of the merge,
+// compression and clusterizer readings) and the efficiency / fake-rate values themselves beyond the 100 % zero-
+// smearing case -- they are whatever this written algorithm yields.
 #include "tpc_oracle.h"
 
 #include <algorithm>
