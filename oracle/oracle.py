@@ -283,6 +283,49 @@ def residual_histogram(trk_hit_offset, trk_n_owned, res, j_min=2):
     return hist
 
 
+def rans_symbol(v, alphabet_bits):
+    return int(lib().orc_rans_symbol(C.c_int32(int(v)), C.c_int32(alphabet_bits)))
+
+
+def rans_normalise(counts):
+    """P58: normalised frequencies (sum 65536) of a histogram over the alphabet."""
+    counts = np.ascontiguousarray(counts, np.int64)
+    freq = np.zeros(len(counts), np.uint32)
+    lib().orc_rans_normalise(C.c_int32(len(counts)), _p(counts, C.c_int64), _u32(freq))
+    return freq
+
+
+def rans_encode(values, alphabet_bits=12, chunk=512):
+    """P57..P60: dict(freq, chunk_off, esc_off, payload, escapes) of an int32 stream."""
+    values = np.ascontiguousarray(values, np.int32)
+    n = int(len(values))
+    n_chunks = (n + chunk - 1) // chunk
+    freq = np.zeros(1 << alphabet_bits, np.uint32)
+    chunk_off = np.zeros(n_chunks + 1, np.uint32)
+    esc_off = np.zeros(n_chunks + 1, np.uint32)
+    payload = np.zeros(max(n_chunks * 4 + 2 * n, 1), np.uint8)
+    escapes = np.zeros(max(n, 1), np.int32)
+    lib().orc_rans_encode.restype = C.c_int64
+    nbytes = lib().orc_rans_encode(_i32(values), C.c_int64(n), C.c_int32(alphabet_bits), C.c_int32(chunk), _u32(freq),
+                                   _u32(chunk_off), _u32(esc_off), _p(payload, C.c_uint8), _i32(escapes))
+    return dict(n=n, alphabet_bits=alphabet_bits, chunk=chunk, freq=freq, chunk_off=chunk_off, esc_off=esc_off,
+                payload=payload[:nbytes].copy(), escapes=escapes[:int(esc_off[-1])].copy())
+
+
+def rans_decode(enc):
+    """The inverse of rans_encode."""
+    n = enc["n"]
+    values = np.zeros(max(n, 1), np.int32)
+    payload = np.ascontiguousarray(np.concatenate([enc["payload"], np.zeros(2, np.uint8)]))
+    escapes = np.ascontiguousarray(np.concatenate([enc["escapes"], np.zeros(1, np.int32)]))
+    lib().orc_rans_decode(C.c_int64(n), C.c_int32(enc["alphabet_bits"]), C.c_int32(enc["chunk"]),
+                          _u32(np.ascontiguousarray(enc["freq"], np.uint32)),
+                          _u32(np.ascontiguousarray(enc["chunk_off"], np.uint32)),
+                          _u32(np.ascontiguousarray(enc["esc_off"], np.uint32)), _p(payload, C.c_uint8), _i32(escapes),
+                          _i32(values))
+    return values[:n]
+
+
 def entropy_bits(hist):
     """Empirical entropy in bits per symbol of a histogram: what an ideal entropy coder (the paper's rANS stage) needs."""
     h = np.asarray(hist, dtype=np.float64)

@@ -11,7 +11,9 @@
 // exact helices reconstructed to 1e-4; <= 1 owner per hit; refit == generator truth; rotation == plane geometry, the
 // generator's helix in the next sector and finite differences; merge rules on hand-made records; pitch-weighted cost on
 // hand-made unequal gaps; residual transform values, exactness on lines / parabolas and the lossless round trip;
-// clusterizer centroids, plateau and threshold rules worked out by hand and resolution against the digit generator.
+// clusterizer centroids, plateau and threshold rules worked out by hand and resolution against the digit generator;
+// rANS stage: frequency tables and chunk bytes worked out by hand (with and without an emission, x = f 2^16), a
+// certain symbol costs 0 bits, a symbol of probability 1/16 exactly 4, size against the Shannon bound, round trip.
 // No function is left "parity unpinned".  Unpinned by the paper: the free constants of orc_params_t (and of the merge,
 // compression and clusterizer readings) and the efficiency / fake-rate values themselves beyond the 100 % zero-
 // smearing case -- they are whatever this written algorithm yields.
@@ -953,6 +955,103 @@ extern "C" void orc_residual_histogram(int64_t n_tracks, const int32_t* off, con
       if (v > 65535) v = 65535;
       ++hist[v];
     }
+}
+
+// ------------------------------------------------------------------------------------------------
+// NEXT-3, entropy stage: static rANS over chunks.  Readings P57..P60 (tpc_oracle.h).
+// ------------------------------------------------------------------------------------------------
+static const uint64_t RANS_M = 65536;   // probabilities in units of 1/M; also the lower bound of the state
+
+extern "C" int32_t orc_rans_symbol(int32_t v, int32_t alphabet_bits) {   // P57
+  const int64_t half = (int64_t)1 << (alphabet_bits - 1);
+  return ((int64_t)v > -half && (int64_t)v < half) ? (int32_t)(v + half) : 0;
+}
+
+extern "C" void orc_rans_normalise(int32_t alphabet, const int64_t* counts, uint32_t* freq) {   // P58
+  int64_t N = 0, K = 0;
+  for (int32_t s = 0; s < alphabet; ++s) {
+    N += counts[s];
+    if (counts[s] > 0) ++K;
+    freq[s] = 0;
+  }
+  if (N == 0) return;
+  int64_t sum = 0;
+  int32_t top = 0;
+  for (int32_t s = 0; s < alphabet; ++s) {
+    if (counts[s] == 0) continue;
+    freq[s] = (uint32_t)(1 + (counts[s] * ((int64_t)RANS_M - K)) / N);
+    sum += freq[s];
+    if (counts[s] > counts[top]) top = s;   // the first of the most frequent
+  }
+  freq[top] += (uint32_t)((int64_t)RANS_M - sum);
+}
+
+extern "C" int64_t orc_rans_encode(const int32_t* values, int64_t n, int32_t alphabet_bits, int32_t chunk,
+                                   uint32_t* freq, uint32_t* chunk_off, uint32_t* esc_off, uint8_t* payload,
+                                   int32_t* escapes) {
+  const int32_t A = 1 << alphabet_bits;
+  std::vector<int64_t> counts((size_t)A, 0);
+  for (int64_t i = 0; i < n; ++i) ++counts[orc_rans_symbol(values[i], alphabet_bits)];
+  orc_rans_normalise(A, counts.data(), freq);
+  std::vector<uint64_t> cum((size_t)A + 1, 0);
+  for (int32_t s = 0; s < A; ++s) cum[s + 1] = cum[s] + freq[s];
+  const int64_t n_chunks = (n + chunk - 1) / chunk;
+  int64_t bytes = 0, n_esc = 0;
+  chunk_off[0] = 0;
+  esc_off[0] = 0;
+  for (int64_t c = 0; c < n_chunks; ++c) {
+    const int64_t i0 = c * chunk, i1 = std::min<int64_t>(n, i0 + chunk);
+    for (int64_t i = i0; i < i1; ++i)   // escapes in stream order
+      if (orc_rans_symbol(values[i], alphabet_bits) == 0) escapes[n_esc++] = values[i];
+    std::vector<uint16_t> words;   // in emission order
+    uint64_t x = RANS_M;
+    for (int64_t i = i1 - 1; i >= i0; --i) {
+      const int32_t s = orc_rans_symbol(values[i], alphabet_bits);
+      const uint64_t f = freq[s];
+      if (x >= f * 65536) {
+        words.push_back((uint16_t)(x & 0xFFFF));
+        x >>= 16;
+      }
+      x = (x / f) * RANS_M + (x % f) + cum[s];
+    }
+    for (int b = 0; b < 4; ++b) payload[bytes++] = (uint8_t)((x >> (8 * b)) & 0xFF);
+    for (size_t k = words.size(); k-- > 0;) {   // the decoder reads the last emitted word first
+      payload[bytes++] = (uint8_t)(words[k] & 0xFF);
+      payload[bytes++] = (uint8_t)(words[k] >> 8);
+    }
+    chunk_off[c + 1] = (uint32_t)bytes;
+    esc_off[c + 1] = (uint32_t)n_esc;
+  }
+  return bytes;
+}
+
+extern "C" void orc_rans_decode(int64_t n, int32_t alphabet_bits, int32_t chunk, const uint32_t* freq,
+                                const uint32_t* chunk_off, const uint32_t* esc_off, const uint8_t* payload,
+                                const int32_t* escapes, int32_t* values) {
+  const int32_t A = 1 << alphabet_bits;
+  const int64_t half = (int64_t)A / 2;
+  std::vector<uint64_t> cum((size_t)A + 1, 0);
+  for (int32_t s = 0; s < A; ++s) cum[s + 1] = cum[s] + freq[s];
+  const int64_t n_chunks = (n + chunk - 1) / chunk;
+  for (int64_t c = 0; c < n_chunks; ++c) {
+    const int64_t i0 = c * chunk, i1 = std::min<int64_t>(n, i0 + chunk);
+    const uint8_t* in = payload + chunk_off[c];
+    uint64_t x = 0;
+    for (int b = 0; b < 4; ++b) x |= (uint64_t)(*in++) << (8 * b);
+    int64_t e = esc_off[c];
+    for (int64_t i = i0; i < i1; ++i) {
+      const uint64_t slot = x % RANS_M;
+      // the symbol whose interval [c_s, c_s + f_s) holds the slot (binary search over the cumulative table)
+      const int32_t s = (int32_t)(std::upper_bound(cum.begin(), cum.end(), slot) - cum.begin()) - 1;
+      x = (uint64_t)freq[s] * (x / RANS_M) + slot - cum[s];
+      if (x < RANS_M) {
+        const uint64_t w = (uint64_t)in[0] | ((uint64_t)in[1] << 8);
+        in += 2;
+        x = x * 65536 + w;
+      }
+      values[i] = s == 0 ? escapes[e++] : (int32_t)(s - half);
+    }
+  }
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -161,6 +161,30 @@ void orc_decompress(int64_t n_tracks, const int32_t* trk_hit_offset, const int32
 void orc_residual_histogram(int64_t n_tracks, const int32_t* trk_hit_offset, const int32_t* trk_n_owned,
                             const int32_t* res, int32_t j_min, int64_t* hist);
 
+/* ---- NEXT-3, entropy stage (the paper's "TPC rANS Encoding"; readings P57..P60) ----
+ * Static range-variant asymmetric numeral system (Duda 2013) over independent chunks of a symbol stream, state
+ * in [2^16, 2^32), 16-bit renormalisation, probabilities in units of 1/M, M = 2^16.
+ * P57 symbols: alphabet A = 2^alphabet_bits; a value v with -A/2 < v < A/2 is the symbol v + A/2; any other value is
+ *   the escape symbol 0 and goes, as it is, to the escape list (stream order).
+ * P58 frequencies: n_s = occurrences of s, N = their sum, K = symbols that occur; f_s = 0 if n_s = 0, else
+ *   f_s = 1 + floor(n_s (M - K) / N); the remainder M - sum f_s (0 <= . < K) goes to the most frequent symbol (the
+ *   smallest one among equals).  c_s = sum_{u<s} f_u.  N = 0: all f_s = 0.
+ * P59 coding of a chunk (symbols i0 .. i1-1 of the stream, `chunk` symbols, the last chunk shorter): x = 2^16; for
+ *   i = i1-1 down to i0, s = symbol i: if x >= f_s 2^16, the low 16 bits of x are emitted and x >>= 16; then
+ *   x = floor(x / f_s) 2^16 + (x mod f_s) + c_s.  Decoding runs forwards: slot = x mod 2^16, s = the symbol with
+ *   c_s <= slot < c_s + f_s, x = f_s floor(x / 2^16) + slot - c_s; if x < 2^16, x = x 2^16 + the next 16-bit word.
+ * P60 layout: the bytes of a chunk are the final x (uint32, little endian) followed by the emitted words in the order
+ *   the decoder consumes them (the last emitted first; uint16, little endian); chunk c occupies
+ *   payload[chunk_off[c] .. chunk_off[c+1]), its escapes escapes[esc_off[c] .. esc_off[c+1]).
+ * Capacities the caller provides: freq[A], chunk_off / esc_off[n_chunks + 1] with n_chunks = ceil(n / chunk),
+ * payload[n_chunks * 4 + 2 n], escapes[n].  orc_rans_encode returns the payload size in bytes. */
+int32_t orc_rans_symbol(int32_t v, int32_t alphabet_bits);
+void orc_rans_normalise(int32_t alphabet, const int64_t* counts, uint32_t* freq);
+int64_t orc_rans_encode(const int32_t* values, int64_t n, int32_t alphabet_bits, int32_t chunk, uint32_t* freq,
+                        uint32_t* chunk_off, uint32_t* esc_off, uint8_t* payload, int32_t* escapes);
+void orc_rans_decode(int64_t n, int32_t alphabet_bits, int32_t chunk, const uint32_t* freq, const uint32_t* chunk_off,
+                     const uint32_t* esc_off, const uint8_t* payload, const int32_t* escapes, int32_t* values);
+
 /* ---- NEXT-2: clusterizer, digits -> clusters (readings P53..P56) ----
  * Digits of a (sector,row): cells (pad, time bin) with an ADC value >= 1, unique, ascending by (time, pad) (P56).
  * P53 peak: a digit with adc >= q_peak_min that is greater than each of its 8 neighbours preceding it in (time, pad)
