@@ -286,6 +286,33 @@ def run_ours(args):
         return float(-(p * np.log2(p)).sum())
 
     comp_bits = {"ry": _entropy(comp["hist_ry"]), "rz": _entropy(comp["hist_rz"]), "drow": _entropy(comp["hist_drow"])}
+    # NEXT-3, entropy stage: the three residual streams through tpc_rans_encode / tpc_rans_decode (chunks of 512)
+    nh_owned = int(out.counts.cpu().numpy()[1])
+    streams3 = [(comp["ry"][:nh_owned].contiguous(), 12), (comp["rz"][:nh_owned].contiguous(), 12),
+                (comp["drow"][:nh_owned].contiguous(), 8)]
+    encs = [trk.rans_encode(v, alphabet_bits=b, chunk=512, stream=stream) for v, b in streams3]
+    torch.cuda.synchronize()
+    r0e.record(stream)
+    for _ in range(5):
+        for (v, b), enc in zip(streams3, encs):
+            trk.rans_encode(v, alphabet_bits=b, chunk=512, stream=stream, into=enc)
+    r1e.record(stream)
+    torch.cuda.synchronize()
+    rans_encode_ms = r0e.elapsed_time(r1e) / 5
+    decs = [trk.rans_decode(enc, stream=stream) for enc in encs]
+    torch.cuda.synchronize()
+    r0e.record(stream)
+    for _ in range(5):
+        for enc in encs:
+            trk.rans_decode(enc, stream=stream)
+    r1e.record(stream)
+    torch.cuda.synchronize()
+    rans_decode_ms = r0e.elapsed_time(r1e) / 5
+    rans_lossless = all(bool(torch.equal(d, v)) for d, (v, _) in zip(decs, streams3))
+    rans_bytes = 0
+    for enc in encs:   # payload + raw escapes + two 32-bit offsets per chunk + the frequency table
+        c = enc["counts"].cpu().numpy()
+        rans_bytes += int(c[0]) + 4 * int(c[1]) + 8 * int(c[2]) + 4 * int(enc["freq"].shape[0])
     # NEXT-2: clusterizer on the synthetic digits of ONE configs[1] event (gen/digits.py)
     from gen.digits import make_digits
     dg = make_digits(evs[0])
@@ -443,8 +470,11 @@ def run_ours(args):
                      "clusterize_digits_per_s": dg.n / (clusterize_ms * 1e-3),
                      "compress_entropy_bits_per_symbol": comp_bits, "owned_clusters": int(len(hit_ids)),
                      "compress_bits_per_owned_cluster": comp_bits["ry"] + comp_bits["rz"] + comp_bits["drow"],
+                     "a10_rans_encode_ms": rans_encode_ms, "a10_rans_decode_ms": rans_decode_ms,
+                     "rans_bytes": rans_bytes, "rans_bits_per_owned_cluster": 8.0 * rans_bytes / max(nh_owned, 1),
+                     "rans_raw_bits_per_owned_cluster": 72, "rans_lossless": rans_lossless,
                      "merge_links": int(merge_counts[0]), "merged_tracks": int(merge_counts[1]),
-                     "note": "tpc_refit, tpc_merge, tpc_refit_merged, tpc_compress over the step's output and tpc_clusterize on one event's digits; outside the timed step"},
+                     "note": "tpc_refit, tpc_merge, tpc_refit_merged, tpc_compress, tpc_rans_encode / _decode over the step's output and tpc_clusterize on one event's digits; outside the timed step"},
             "e2e": {"value": e2e_units / (e2e_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "steps": e2e_steps, "ms_per_step": e2e_max / e2e_steps,
                     "host_threads": T},

@@ -205,6 +205,39 @@ int tpc_compress(tpc_tracker_t* t, const tpc_clusters_t* clusters, int64_t n, vo
 int tpc_decompress(tpc_tracker_t* t, void* stream, const tpc_tracks_out_t* tracks, const tpc_compressed_t* in,
                    int32_t* row, int32_t* y, int32_t* z);
 
+/* NEXT-3, the entropy stage ("TPC rANS Encoding"; readings P57..P60 in DESIGN.md): static range-variant
+ * asymmetric numeral system over independent chunks of a value stream.  State in [2^16, 2^32), 16-bit words,
+ * probabilities in units of 1/65536.
+ * P57: alphabet A = 2^alphabet_bits; a value v with -A/2 < v < A/2 is the symbol v + A/2, any other value is the
+ *      escape symbol 0 and is kept as it is in the escape list (stream order).
+ * P58: frequencies from the stream's own histogram n_s (N values, K symbols occur): f_s = 1 + floor(n_s (65536 - K) / N)
+ *      for the symbols that occur, the remainder 65536 - sum f_s goes to the most frequent (smallest among equals).
+ * P59: a chunk (`chunk` consecutive values, the last one shorter) is coded backwards from x = 2^16: if x >= f_s 2^16
+ *      the low 16 bits of x are emitted and x >>= 16; x = floor(x / f_s) 2^16 + x mod f_s + c_s (c_s = sum of f below s).
+ * P60: chunk c is payload[chunk_off[c] .. chunk_off[c+1]): the final x (uint32, little endian), then the emitted
+ *      words, last emitted first (uint16, little endian); its escapes are escapes[esc_off[c] .. esc_off[c+1]).
+ * All pointers [device] and caller-owned.  counts: int64[4] = payload bytes, escapes, chunks, flags (bit 0: the
+ * payload did not fit payload_capacity, bit 1: the escapes did not fit; nothing is written out of bounds, the sizes
+ * reported are the needed ones).  payload_capacity >= 4 * n_chunks + 2 * n and escape_capacity >= n always fit. */
+typedef struct {
+  uint32_t* freq;        /* 2^alphabet_bits normalised frequencies */
+  uint32_t* chunk_off;   /* n_chunks + 1 byte offsets, n_chunks = ceil(n / chunk) */
+  uint32_t* esc_off;     /* n_chunks + 1 */
+  uint8_t* payload;      /* payload_capacity bytes, 2-byte aligned */
+  int32_t* escapes;      /* escape_capacity values */
+  int64_t* counts;       /* int64[4] */
+  int64_t payload_capacity;
+  int64_t escape_capacity;
+} tpc_rans_stream_t;
+/* values: [device] n values of value_bytes = 4 (int32) or 1 (uint8, e.g. the row steps); 1 <= alphabet_bits <= 12,
+ * 1 <= chunk <= 65535 (512 is what bench.py uses).  Asynchronous on `stream` (the handle's scratch grows on demand,
+ * which synchronises once).  Errors: TPC_ERR_ARG, TPC_ERR_NOMEM, TPC_ERR_CUDA. */
+int tpc_rans_encode(tpc_tracker_t* t, const void* values, int32_t value_bytes, int64_t n, int32_t alphabet_bits,
+                    int32_t chunk, void* stream, const tpc_rans_stream_t* out);
+/* The inverse: n values from a stream written with the same alphabet_bits and chunk. */
+int tpc_rans_decode(tpc_tracker_t* t, const tpc_rans_stream_t* in, int64_t n, int32_t alphabet_bits, int32_t chunk,
+                    void* stream, void* values, int32_t value_bytes);
+
 /* NEXT-2 (readings P53..P56 in DESIGN.md): clusterizer in front of the path, digits -> clusters.
  * Digits of a (sector,row): cells (pad, time bin) with an ADC value >= 1, unique, ascending by (time, pad).
  * Peak (P53): adc >= q_peak_min, greater than each of its 8 neighbours that precede it in (time, pad) order and

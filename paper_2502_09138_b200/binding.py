@@ -77,6 +77,13 @@ class _Compressed(C.Structure):
                 ("hist_rz", C.c_void_p), ("hist_drow", C.c_void_p)]
 
 
+class _RansStream(C.Structure):
+    """tpc_rans_stream_t"""
+    _fields_ = [("freq", C.c_void_p), ("chunk_off", C.c_void_p), ("esc_off", C.c_void_p), ("payload", C.c_void_p),
+                ("escapes", C.c_void_p), ("counts", C.c_void_p), ("payload_capacity", C.c_int64),
+                ("escape_capacity", C.c_int64)]
+
+
 class ClusterParams(C.Structure):
     """tpc_cluster_params_t"""
     _fields_ = [("n_pads", C.c_int32), ("n_per_side", C.c_int32), ("pad_units", C.c_int32), ("time_units", C.c_int32),
@@ -134,6 +141,10 @@ def load_library():
                                  C.POINTER(_Compressed)]
     lib.tpc_decompress.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_TracksOut), C.POINTER(_Compressed), C.c_void_p,
                                    C.c_void_p, C.c_void_p]
+    lib.tpc_rans_encode.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int64, C.c_int32, C.c_int32, C.c_void_p,
+                                    C.POINTER(_RansStream)]
+    lib.tpc_rans_decode.argtypes = [C.c_void_p, C.POINTER(_RansStream), C.c_int64, C.c_int32, C.c_int32, C.c_void_p,
+                                    C.c_void_p, C.c_int32]
     lib.tpc_default_cluster_params.argtypes = [C.POINTER(ClusterParams)]
     lib.tpc_default_cluster_params.restype = None
     lib.tpc_clusterize.argtypes = [C.c_void_p, C.POINTER(_Digits), C.c_int64, C.POINTER(ClusterParams), C.c_void_p,
@@ -355,6 +366,53 @@ class Tracker:
         self._check(self._lib.tpc_decompress(self._h, self._stream_ptr(stream), C.byref(o), C.byref(cs), _ptr(row),
                                              _ptr(yy), _ptr(zz)))
         return row, yy, zz
+
+    @staticmethod
+    def _rans_struct(enc: dict) -> "_RansStream":
+        return _RansStream(_ptr(enc["freq"]), _ptr(enc["chunk_off"]), _ptr(enc["esc_off"]), _ptr(enc["payload"]),
+                           _ptr(enc["escapes"]), _ptr(enc["counts"]), int(enc["payload"].shape[0]),
+                           int(enc["escapes"].shape[0]))
+
+    def rans_encode(self, values, alphabet_bits: int = 12, chunk: int = 512, payload_capacity=None,
+                    escape_capacity=None, stream=None, into: "dict | None" = None):
+        """tpc_rans_encode of an int32 or uint8 CUDA tensor: dict of device tensors freq, chunk_off, esc_off (uint32
+        bits in int32), payload (uint8), escapes (int32), counts (int64[4]: payload bytes, escapes, chunks, flags).
+        Default capacities hold any input; `into` reuses the buffers of an earlier call of the same shape."""
+        import torch
+        n = int(values.shape[0])
+        vb = {torch.int32: 4, torch.uint8: 1}[values.dtype]
+        n_chunks = (n + chunk - 1) // chunk
+        dev = values.device
+        enc = into
+        if enc is None:
+            pc = int(payload_capacity if payload_capacity is not None else 4 * n_chunks + 2 * n)
+            ec = int(escape_capacity if escape_capacity is not None else n)
+            enc = dict(freq=torch.zeros(1 << alphabet_bits, dtype=torch.int32, device=dev),
+                       chunk_off=torch.zeros(n_chunks + 1, dtype=torch.int32, device=dev),
+                       esc_off=torch.zeros(n_chunks + 1, dtype=torch.int32, device=dev),
+                       payload=torch.zeros(max(pc, 2), dtype=torch.uint8, device=dev),
+                       escapes=torch.zeros(max(ec, 1), dtype=torch.int32, device=dev),
+                       counts=torch.zeros(4, dtype=torch.int64, device=dev),
+                       n=n, alphabet_bits=alphabet_bits, chunk=chunk, value_bytes=vb)
+            if payload_capacity is not None:
+                enc["payload"] = enc["payload"][:pc] if pc >= 2 else enc["payload"][:0]
+            if escape_capacity is not None:
+                enc["escapes"] = enc["escapes"][:ec]
+        rs = self._rans_struct(enc)
+        self._check(self._lib.tpc_rans_encode(self._h, C.c_void_p(_ptr(values)), vb, C.c_int64(n), alphabet_bits, chunk,
+                                              self._stream_ptr(stream), C.byref(rs)))
+        return enc
+
+    def rans_decode(self, enc: dict, stream=None):
+        """tpc_rans_decode: the values of an encoded stream (same dtype as the input of rans_encode)."""
+        import torch
+        n = enc["n"]
+        vb = enc["value_bytes"]
+        values = torch.zeros(max(n, 1), dtype=torch.int32 if vb == 4 else torch.uint8, device=enc["freq"].device)
+        rs = self._rans_struct(enc)
+        self._check(self._lib.tpc_rans_decode(self._h, C.byref(rs), C.c_int64(n), enc["alphabet_bits"], enc["chunk"],
+                                              self._stream_ptr(stream), C.c_void_p(_ptr(values)), vb))
+        return values[:n]
 
     def clusterize(self, pad, time, adc, offsets, n_pads: int, params: "ClusterParams | None" = None, capacity=None,
                    stream=None):

@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "libtpctrack.so")
 SOURCES = ["api.cu", "a1_grid.cu", "a2_neighbours.cu", "a3_seeds.cu", "a4_follow.cu", "a4_phases.cu", "a5_select.cu", "a6_refit.cu",
-           "a7_merge.cu", "a8_compress.cu", "a9_cluster.cu", "debug.cu"]
+           "a7_merge.cu", "a8_compress.cu", "a9_cluster.cu", "a10_rans.cu", "debug.cu"]
 HEADERS = [os.path.join(CSRC, "tpc_internal.cuh"), os.path.join(CSRC, "kalman.cuh"), os.path.join(CSRC, "a4_search.cuh"), os.path.join(os.path.dirname(_HERE), "include", "tpc_track.h")]
 # a4 only: fp32 division / sqrt / rsqrt as MUFU + one correction (2 ulp), denormals flushed.  Measured against
 # the fp64 oracle on configs 0, 1, 2, 4: worst parameter error 9e-6 (bar 1e-4), hit tables unchanged; a4 -5 %.

@@ -324,6 +324,7 @@ int tpc_tracker_destroy(tpc_tracker_t* t) {
   if (t->cl_flag) cudaFree(t->cl_flag);
   if (t->cl_parked) cudaFree(t->cl_parked);
   if (t->cl_row_count) cudaFree(t->cl_row_count);
+  if (t->rans_scratch) cudaFree(t->rans_scratch);
   if (t->merge_sec) cudaFree(t->merge_sec);
   if (t->merge_best) cudaFree(t->merge_best);
   if (t->merge_chi2) cudaFree(t->merge_chi2);
@@ -465,6 +466,41 @@ int tpc_decompress(tpc_tracker_t* t, void* stream, const tpc_tracks_out_t* track
   if (tracks->hit_capacity > 0 && (!in->drow || !in->ry || !in->rz || !row || !y || !z)) return TPC_ERR_ARG;
   if (tracks->track_capacity > 0 && !tracks->tracks) return TPC_ERR_ARG;
   TPC_CUDA(t, launch_a8_decompress(t, tracks, in, row, y, z, (cudaStream_t)stream));
+  return TPC_OK;
+}
+
+int tpc_rans_encode(tpc_tracker_t* t, const void* values, int32_t value_bytes, int64_t n, int32_t alphabet_bits,
+                    int32_t chunk, void* stream, const tpc_rans_stream_t* out) {
+  if (!t || !out || n < 0 || n >= ((int64_t)1 << 31) || (value_bytes != 1 && value_bytes != 4)) return TPC_ERR_ARG;
+  if (alphabet_bits < 1 || alphabet_bits > 12 || chunk < 1 || chunk > 65535) return TPC_ERR_ARG;
+  if (!out->freq || !out->chunk_off || !out->esc_off || !out->counts || out->payload_capacity < 0 ||
+      out->escape_capacity < 0)
+    return TPC_ERR_ARG;
+  if (n > 0 && (!values || (out->payload_capacity > 0 && !out->payload) || (out->escape_capacity > 0 && !out->escapes)))
+    return TPC_ERR_ARG;
+  const size_t need = rans_scratch_bytes(n, chunk, alphabet_bits);
+  if (need > t->rans_scratch_cap) {
+    TPC_CUDA(t, cudaDeviceSynchronize());
+    if (t->rans_scratch) cudaFree(t->rans_scratch);
+    t->rans_scratch = nullptr;
+    t->rans_scratch_cap = 0;
+    if (cudaMalloc(&t->rans_scratch, need) != cudaSuccess) {
+      cudaGetLastError();
+      return TPC_ERR_NOMEM;
+    }
+    t->rans_scratch_cap = need;
+  }
+  TPC_CUDA(t, launch_a10_rans_encode(t, values, value_bytes, n, alphabet_bits, chunk, out, (cudaStream_t)stream));
+  return TPC_OK;
+}
+
+int tpc_rans_decode(tpc_tracker_t* t, const tpc_rans_stream_t* in, int64_t n, int32_t alphabet_bits, int32_t chunk,
+                    void* stream, void* values, int32_t value_bytes) {
+  if (!t || !in || n < 0 || n >= ((int64_t)1 << 31) || (value_bytes != 1 && value_bytes != 4)) return TPC_ERR_ARG;
+  if (alphabet_bits < 1 || alphabet_bits > 12 || chunk < 1 || chunk > 65535) return TPC_ERR_ARG;
+  if (!in->freq || !in->chunk_off || !in->esc_off) return TPC_ERR_ARG;
+  if (n > 0 && (!values || !in->payload)) return TPC_ERR_ARG;
+  TPC_CUDA(t, launch_a10_rans_decode(t, in, n, alphabet_bits, chunk, values, value_bytes, (cudaStream_t)stream));
   return TPC_OK;
 }
 

@@ -110,6 +110,8 @@ struct tpc_tracker {
   // a9 (tpc_clusterize) scratch, grown on demand: sorted keys of rows too long for shared memory, peak flags and
   // parked clusters per digit, clusters per row
   uint32_t* cl_keys; uint8_t* cl_flag; int4* cl_parked; uint32_t* cl_row_count; int64_t cl_cap;
+  // a10 (tpc_rans_encode) scratch, grown on demand: chunk slots, histogram, cumulative table, per-chunk counts
+  void* rans_scratch; size_t rans_scratch_cap;
   int64_t last_n; const uint32_t* last_ro; const int32_t* last_y; const int32_t* last_z;
   // stage timing
   int timing; int64_t timed_calls; cudaEvent_t ev[TIMING_SETS * 6];
@@ -150,6 +152,11 @@ cudaError_t launch_a8_decompress(const tpc_tracker* t, const tpc_tracks_out_t* t
                                  int32_t* row, int32_t* y, int32_t* z, cudaStream_t st);
 cudaError_t setup_a9_attributes();
 cudaError_t setup_a2_attributes();
+size_t rans_scratch_bytes(int64_t n, int32_t chunk, int32_t bits);
+cudaError_t launch_a10_rans_encode(const tpc_tracker* t, const void* values, int32_t value_bytes, int64_t n,
+                                   int32_t bits, int32_t chunk, const tpc_rans_stream_t* out, cudaStream_t st);
+cudaError_t launch_a10_rans_decode(const tpc_tracker* t, const tpc_rans_stream_t* in, int64_t n, int32_t bits,
+                                   int32_t chunk, void* values, int32_t value_bytes, cudaStream_t st);
 cudaError_t launch_a9_clusterize(const tpc_tracker* t, const tpc_cluster_params_t* cp, const tpc_digits_t* d,
                                  int64_t n_digits, const tpc_clusters_out_t* out, cudaStream_t st);
 cudaError_t launch_a7_merge(const tpc_tracker* t, const tpc_merge_params_t* mp, const tpc_track_rec_t* tracks,

@@ -566,6 +566,97 @@ def test_compress_residual_streams_bit_exact_and_lossless(orc):
         trk.close()
 
 
+def _rans_equal(enc, ref, label):
+    nb, ne = int(ref["chunk_off"][-1]), int(ref["esc_off"][-1])
+    c = enc["counts"].cpu().numpy()
+    assert c.tolist() == [nb, ne, len(ref["chunk_off"]) - 1, 0], (label, c)
+    assert np.array_equal(enc["freq"].cpu().numpy().view(np.uint32), ref["freq"]), label
+    assert np.array_equal(enc["chunk_off"].cpu().numpy().view(np.uint32), ref["chunk_off"]), label
+    assert np.array_equal(enc["esc_off"].cpu().numpy().view(np.uint32), ref["esc_off"]), label
+    assert np.array_equal(enc["payload"][:nb].cpu().numpy(), ref["payload"]), label
+    assert np.array_equal(enc["escapes"][:ne].cpu().numpy(), ref["escapes"]), label
+
+
+def test_rans_stage_bit_exact_and_lossless(orc):
+    """NEXT-3 entropy stage through the C ABI: tpc_rans_encode against orc_rans_encode (bytes, tables and offsets
+    bit-exact) and tpc_rans_decode back to the input: hand-sized streams (alphabets, chunk sizes, escapes, a ragged last
+    chunk, one value, none), then the three residual streams of a central event (int32 y / z residuals in a 4096-symbol
+    alphabet, uint8 row steps in a 256-symbol one) in the chunking bench.py uses."""
+    import torch
+    from paper_2502_09138_b200 import Tracker
+    from paper_2502_09138_b200.events import geometry_from_event, upload
+    ev = make_event(1, 1000)
+    trk = Tracker(geometry_from_event(ev))
+    rng = np.random.default_rng(3)
+    for n, chunk, bits in ((0, 16, 8), (1, 16, 8), (16, 16, 8), (17, 16, 8), (1000, 1, 4), (5000, 512, 12), (4097, 4096, 12),
+                           (70001, 333, 6), (300000, 65535, 1), (200000, 512, 12)):
+        v = np.rint(rng.normal(0, (1 << bits) / 6.0, n)).astype(np.int32)
+        if n > 10:
+            v[rng.integers(0, n, 5)] = rng.integers(-2**31, 2**31 - 1, 5, dtype=np.int64).astype(np.int32)
+            v[rng.integers(0, n, 2)] = -(1 << (bits - 1))                      # the boundary value escapes
+        if n == 70001:
+            v[:] = 0
+            v[-1] = 1                                                          # x = f 2^16 exactly at a chunk's end
+        d = torch.from_numpy(v).cuda()
+        enc = trk.rans_encode(d, alphabet_bits=bits, chunk=chunk)
+        _rans_equal(enc, orc.rans_encode(v, bits, chunk), (n, chunk, bits))
+        assert np.array_equal(trk.rans_decode(enc).cpu().numpy(), v), (n, chunk, bits)
+    # uint8 input
+    v8 = rng.integers(0, 256, 50000).astype(np.uint8)
+    enc = trk.rans_encode(torch.from_numpy(v8).cuda(), alphabet_bits=8, chunk=100)
+    _rans_equal(enc, orc.rans_encode(v8.astype(np.int32), 8, 100), "uint8")
+    assert np.array_equal(trk.rans_decode(enc).cpu().numpy(), v8)
+    # the residual streams of an event
+    y, z, ro = upload(ev)
+    out = trk.track(y, z, ro)
+    comp = trk.compress(y, z, ro, out)
+    _, hit_ids, _ = out.to_host()
+    nh = len(hit_ids)
+    total = 0
+    for key, bits in (("ry", 12), ("rz", 12), ("drow", 8)):
+        d = comp[key][:nh].contiguous()
+        enc = trk.rans_encode(d, alphabet_bits=bits, chunk=512)
+        ref = orc.rans_encode(d.cpu().numpy().astype(np.int32), bits, 512)
+        _rans_equal(enc, ref, key)
+        assert torch.equal(trk.rans_decode(enc), d), key
+        size = len(ref["payload"]) + 4 * len(ref["escapes"]) + 8 * (len(ref["chunk_off"]) - 1)
+        total += size
+        print(f"[rans] {key}: {nh} values -> {size} bytes = {8.0 * size / nh:.2f} bits per hit "
+              f"({len(ref['escapes'])} escapes)")
+    print(f"[rans] {8.0 * total / nh:.2f} bits per owned hit against 72 raw (row, y, z)")
+    trk.close()
+
+
+def test_rans_capacity_overflow_is_flagged_not_written(orc):
+    """Payload and escape buffers that are too small: counts report the sizes needed and both flags, whole chunks that
+    fit are written, and nothing lands beyond the capacities (guard bytes behind both buffers stay untouched)."""
+    import torch
+    from paper_2502_09138_b200 import Tracker
+    from paper_2502_09138_b200.events import geometry_from_event
+    trk = Tracker(geometry_from_event(make_event(0)))
+    rng = np.random.default_rng(8)
+    v = np.rint(rng.normal(0, 300, 40000)).astype(np.int32)
+    v[::100] = 1 << 20
+    ref = orc.rans_encode(v, 12, 512)
+    nb, ne = len(ref["payload"]), len(ref["escapes"])
+    d = torch.from_numpy(v).cuda()
+    enc = trk.rans_encode(d, 12, 512)                                           # full-size buffers: the dict to reuse
+    _rans_equal(enc, ref, "full")
+    cap_p, cap_e = (nb // 2) & ~1, ne // 2
+    big_p = torch.full((nb + 64,), 0xEE, dtype=torch.uint8, device="cuda")
+    big_e = torch.full((ne + 64,), -77, dtype=torch.int32, device="cuda")
+    small = dict(enc, payload=big_p[:cap_p], escapes=big_e[:cap_e], counts=torch.zeros(4, dtype=torch.int64, device="cuda"))
+    trk.rans_encode(d, 12, 512, into=small)
+    c = small["counts"].cpu().numpy().tolist()
+    assert c == [nb, ne, len(ref["chunk_off"]) - 1, 3], c
+    assert bool((big_p[cap_p:] == 0xEE).all()) and bool((big_e[cap_e:] == -77).all())
+    full = np.asarray(ref["chunk_off"], np.int64)
+    fit = int(full[full <= cap_p].max())
+    assert np.array_equal(big_p[:fit].cpu().numpy(), ref["payload"][:fit])
+    assert np.array_equal(big_e[:cap_e].cpu().numpy(), ref["escapes"][:cap_e])
+    trk.close()
+
+
 def _upload_digits(d):
     import torch
     f = lambda a, t: torch.from_numpy(np.ascontiguousarray(a).view(t)).cuda()      # noqa: E731
