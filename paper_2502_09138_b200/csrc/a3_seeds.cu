@@ -5,9 +5,8 @@
 // array of a1), at position p.  One synchronous cleaning step from the raw tables: up'[p] = up[p] if dn[up[p]] == p
 // else -1 (dn' likewise).  Chain start: dn'[p] < 0 and up'[p] >= 0; a chain is a seed iff it has >= l_min clusters,
 // which a walk of at most l_min - 1 steps decides.
-// Thread per sorted position: loads and stores of the link tables and of srt are coalesced, and the cleaned up link
-// goes into the free fourth word of the cluster's srt record, so that a4 follows a chain with one 16-byte gather per
-// hit out of the same array its row searches read (no second per-cluster record array).
+// Thread per sorted position: loads and stores of the link tables are coalesced; the cleaned up links go to a table of
+// their own (clean_up, whole sectors per warp), which a4 reads next to the srt record of every chain hit it follows.
 // Seeds come out in sorted-position order (block scan + single-pass look-back scan); P14 ranks them by ascending
 // start *id*.  Positions and ids of a (sector,row) fill the same index range, so the two orders differ only inside
 // a row: a3_rank_kernel moves every seed to its id-order rank by counting, among the seeds of its own row (which
@@ -22,7 +21,8 @@ constexpr int A3_ITEMS = A3_TILE / A3_THREADS;
 // Latency-bound (gathers, look-back): full occupancy (8 CTAs, 32 registers) beats 6 CTAs at 40 registers.
 __global__ void __launch_bounds__(A3_THREADS, 8)
 a3_seeds_kernel(const DevGeom g, int64_t n, const uint32_t* __restrict__ ro, const int32_t* __restrict__ up,
-                const int32_t* __restrict__ dn, int4* __restrict__ srt, int4* __restrict__ seed_tmp,
+                const int32_t* __restrict__ dn, int32_t* __restrict__ clean_up, const int4* __restrict__ srt,
+                int4* __restrict__ seed_tmp,
                 DevCtl* __restrict__ ctl, uint64_t* __restrict__ status, uint32_t n_tiles, uint32_t s_cap) {
   __shared__ uint32_t wsum[33];
   __shared__ uint32_t sh_tile;
@@ -57,17 +57,26 @@ a3_seeds_kernel(const DevGeom g, int64_t n, const uint32_t* __restrict__ ro, con
     du[k] = u[k] >= 0 ? dn[u[k]] : -1;
     ud[k] = d[k] >= 0 ? up[d[k]] : -1;
   }
-  int c[A3_ITEMS], len[A3_ITEMS];
+  int c[A3_ITEMS], len[A3_ITEMS], cl[A3_ITEMS];
   bool walk[A3_ITEMS];
 #pragma unroll
   for (int k = 0; k < A3_ITEMS; ++k) {
     const int p = (int)(p0 + k);
     const int uc = (u[k] >= 0 && du[k] == p) ? u[k] : -1;   // P11
     const int dc = (d[k] >= 0 && ud[k] == p) ? d[k] : -1;
-    if (p0 + k < n) srt[p0 + k].w = uc;   // the four 4-byte stores of a thread fill two 32-byte sectors' w words
+    cl[k] = uc;
     walk[k] = dc < 0 && uc >= 0;   // P12 chain start; the walk uses raw links + the mutual test (= cleaned links)
     c[k] = uc;
     len[k] = 2;
+  }
+  // the cleaned up links go to a table of their own, 16 bytes per thread, whole sectors per warp (as the fourth word
+  // of the srt records every 4-byte store dirtied a sector that DRAM had to fill first: 0.6 GB of traffic per step)
+  if (vec) {
+    *(int4*)(clean_up + p0) = make_int4(cl[0], cl[1], cl[2], cl[3]);
+  } else {
+#pragma unroll
+    for (int k = 0; k < A3_ITEMS; ++k)
+      if (p0 + k < n) clean_up[p0 + k] = cl[k];
   }
   for (int step = 2; step < g.l_min; ++step) {   // all walks of the thread advance together
     int nx[A3_ITEMS], back[A3_ITEMS];
@@ -115,13 +124,15 @@ a3_seeds_kernel(const DevGeom g, int64_t n, const uint32_t* __restrict__ ro, con
 // it and fill the same rank range in both orders.
 __global__ void __launch_bounds__(256)
 a3_rank_kernel(const DevCtl* __restrict__ ctl, const int4* __restrict__ seed_tmp, const int4* __restrict__ srt,
+               const int32_t* __restrict__ clean_up,
                int32_t* __restrict__ seed_start, int32_t* __restrict__ seed_pos, int32_t* __restrict__ seed_sr,
                int4* __restrict__ seed_rec) {
   const int64_t ns = ctl->n_seeds;
   for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < ns; k += (int64_t)gridDim.x * blockDim.x) {
     const int4 me = seed_tmp[k];
+    const int up0 = clean_up[me.x];
     const int4 c0 = srt[me.x];     // the seed's first cluster and (requested before the counting loops) its second
-    const int4 c1 = srt[c0.w];
+    const int4 c1 = srt[up0];
     int64_t left = 0, smaller = 0;
     for (int64_t j = k - 1; j >= 0; --j) {
       const int4 o = seed_tmp[j];
@@ -140,7 +151,7 @@ a3_rank_kernel(const DevCtl* __restrict__ ctl, const int4* __restrict__ seed_tmp
     seed_sr[rank] = me.z;
     // everything a4 needs to start the tracklet, in one 32-byte record: (sr, y0, z0, id0) (up0, y1, z1, -)
     seed_rec[2 * rank] = make_int4(me.z, c0.x, c0.y, c0.z);
-    seed_rec[2 * rank + 1] = make_int4(c0.w, c1.x, c1.y, 0);
+    seed_rec[2 * rank + 1] = make_int4(up0, c1.x, c1.y, 0);
   }
 }
 
@@ -149,12 +160,12 @@ a3_rank_kernel(const DevCtl* __restrict__ ctl, const int4* __restrict__ seed_tmp
 cudaError_t launch_a3_seeds(const tpc_tracker* t, const uint32_t* ro, int64_t n, cudaStream_t st) {
   if (t->tiles_a3 == 0 || n == 0) return cudaSuccess;
   const uint32_t tiles = (uint32_t)((n + A3_TILE - 1) / A3_TILE);
-  a3_seeds_kernel<<<tiles, A3_THREADS, 0, st>>>(t->g, n, ro, t->s.link_up, t->s.link_dn, t->s.srt, t->s.seed_tmp,
+  a3_seeds_kernel<<<tiles, A3_THREADS, 0, st>>>(t->g, n, ro, t->s.link_up, t->s.link_dn, t->s.clean_up, t->s.srt, t->s.seed_tmp,
                                                t->s.ctl, t->s.scan_a3, tiles, (uint32_t)t->s_cap);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   // the seed count stays on the device: a grid-stride kernel sized for the device, not for the capacity
-  a3_rank_kernel<<<t->a4_sms * 8, 256, 0, st>>>(t->s.ctl, t->s.seed_tmp, t->s.srt, t->s.seed_start, t->s.seed_pos,
+  a3_rank_kernel<<<t->a4_sms * 8, 256, 0, st>>>(t->s.ctl, t->s.seed_tmp, t->s.srt, t->s.clean_up, t->s.seed_start, t->s.seed_pos,
                                                t->s.seed_sr, t->s.seed_rec);
   return cudaGetLastError();
 }

@@ -36,6 +36,7 @@ constexpr int A4_MIN_BLOCKS = 4;   // 16 warps per SM: registers capped at 128 p
 
 __global__ void __launch_bounds__(A4_THREADS, A4_MIN_BLOCKS)
 a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restrict__ srt,
+                 const int32_t* __restrict__ clean_up,
                  const uint32_t* __restrict__ sec_key, const uint32_t* __restrict__ bin_start,
                  const int32_t* __restrict__ seed_pos, const int32_t* __restrict__ seed_sr,
                  float4* __restrict__ tl_rec, int32_t* __restrict__ tl_hits, int2* __restrict__ tl_yz,
@@ -101,9 +102,10 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
         org_z = zmin_from_key(sec_key[sec]);
         tab = tl_hits + (size_t)k * nr;
         yz = tl_yz + (size_t)k * ((nr + 3) & ~3);   // groups of four rows are 32-byte aligned (a4_phases.cu)
+        const int up0 = clean_up[h];
         const int4 c0 = srt[h];
-        const int4 c1 = srt[c0.w];
-        rcn.y = c0.x; rcn.z = c0.y; rcn.id = c0.z; rcn.up = c0.w;
+        const int4 c1 = srt[up0];
+        rcn.y = c0.x; rcn.z = c0.y; rcn.id = c0.z; rcn.up = up0;
         more = true;
         const int y0 = c0.x, z0 = c0.y;
         const float dxr = s_row_dx[r0];
@@ -153,7 +155,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
       hy = rc.y;
       hz = rc.z;
     }
-    ld_rec_if(rcn, srt + rc.up, mode == M_LINK && rc.up >= 0);   // the next chain hit, one step ahead
+    ld_rec_if(rcn, srt + rc.up, clean_up + rc.up, mode == M_LINK && rc.up >= 0);   // the next chain hit, one step ahead
     if (mode == M_TABLE) {
       // rolling two-deep pipeline over the tracklet's (y, z) stream on the way down
       ld_cg_yz_if(s1_y, s1_z, yz + trow, s1_row != trow);
@@ -324,7 +326,7 @@ cudaError_t setup_a4_attributes(tpc_tracker* t) {
 cudaError_t launch_a4_follow(const tpc_tracker* t, int64_t n, cudaStream_t st) {
   if (n == 0 || t->s_cap == 0) return cudaSuccess;
   a4_follow_kernel<<<t->a4_blocks, A4_THREADS, a4_smem_bytes(t->g), st>>>(
-      t->g, t->s.ctl, t->s.srt, t->s.sec_key, t->s.bin_start, t->s.seed_pos, t->s.seed_sr, t->s.tl_rec, t->s.tl_hits,
+      t->g, t->s.ctl, t->s.srt, t->s.clean_up, t->s.sec_key, t->s.bin_start, t->s.seed_pos, t->s.seed_sr, t->s.tl_rec, t->s.tl_hits,
       t->s.tl_yz, t->s.owner);
   return cudaGetLastError();
 }

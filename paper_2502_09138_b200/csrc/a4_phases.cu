@@ -20,6 +20,7 @@ struct Env {   // everything a warp needs that does not change during a kernel
   DevGeom g;
   DevCtl* ctl;
   const int4* srt;
+  const int32_t* clean_up;   // a3: cleaned up link of every sorted position
   const uint32_t* sec_key;
   const uint32_t* bin_start;
   const int4* seed_rec;
@@ -191,7 +192,7 @@ __device__ __forceinline__ void phase_a(const Env& e) {
   Cov C;
   p.y = p.z = p.s = p.t = p.q = 0; p.oy = p.oz = 0;
   cov_reset(g, C);
-  Rec rcn = {0, 0, -1, -1};   // the chain hit of the next step (requested one step ahead)
+  Rec rcn = {0, 0, -1, -1};   // the chain hit of the next step (requested one step ahead: its record and its link)
   bool more = false;          // rcn holds a chain hit
   bool dirty = false;         // the staging column holds rows that are not in tl_yz yet
   while (true) {
@@ -226,7 +227,7 @@ __device__ __forceinline__ void phase_a(const Env& e) {
     const int trow = b.row + (tr ? 1 : 0);
     const float dx = e.s_row_dx[b.row];
     const Rec rc = rcn;
-    ld_rec_if(rcn, e.srt + rc.up, live && rc.up >= 0);   // the next chain hit, one step ahead
+    ld_rec_if(rcn, e.srt + rc.up, e.clean_up + rc.up, live && rc.up >= 0);   // the next chain hit, one step ahead
     bool ok = live;
     if (tr) ok = transport<true>(g, dx, p, C);
     if (ok) {
@@ -579,6 +580,7 @@ constexpr int ap_min_blocks(int ph) { return ph == 2 ? 7 : 4; }
 template <int PH>
 __global__ void __launch_bounds__(AP_THREADS, ap_min_blocks(PH))
 a4_phase_kernel(const DevGeom g, uint32_t s_cap, DevCtl* __restrict__ ctl, const int4* __restrict__ srt,
+                const int32_t* __restrict__ clean_up,
                 const uint32_t* __restrict__ sec_key, const uint32_t* __restrict__ bin_start,
                 const int4* __restrict__ seed_rec, float4* __restrict__ tl_rec, int32_t* __restrict__ tl_hits, int2* __restrict__ tl_yz,
                 int4* __restrict__ tl_state, uint32_t* __restrict__ q_items, uint32_t* __restrict__ tl_span) {
@@ -596,7 +598,7 @@ a4_phase_kernel(const DevGeom g, uint32_t s_cap, DevCtl* __restrict__ ctl, const
   __syncthreads();
   Env e;
   e.g = g;
-  e.ctl = ctl; e.srt = srt; e.sec_key = sec_key; e.bin_start = bin_start;
+  e.ctl = ctl; e.srt = srt; e.clean_up = clean_up; e.sec_key = sec_key; e.bin_start = bin_start;
   e.seed_rec = seed_rec; e.tl_rec = tl_rec; e.tl_hits = tl_hits; e.tl_yz = tl_yz;
   e.tl_state = tl_state;
   e.q_items = q_items; e.tl_span = tl_span; e.s_row_x = s_row_x; e.s_row_dx = s_row_dx;
@@ -620,7 +622,7 @@ cudaError_t launch_a4_phases(const tpc_tracker* t, int64_t n, cudaStream_t st) {
   const size_t smem = (size_t)t->g.n_rows * (8 + 4);
 #define AP_LAUNCH(PH)                                                                                         \
   a4_phase_kernel<PH><<<t->a4_sms * ap_min_blocks(PH), AP_THREADS, smem, st>>>(                                                \
-      t->g, (uint32_t)t->s_cap, t->s.ctl, t->s.srt, t->s.sec_key, t->s.bin_start, t->s.seed_rec,              \
+      t->g, (uint32_t)t->s_cap, t->s.ctl, t->s.srt, t->s.clean_up, t->s.sec_key, t->s.bin_start, t->s.seed_rec, \
       t->s.tl_rec, t->s.tl_hits, t->s.tl_yz, t->s.tl_state, t->s.q_items, t->s.tl_span)
   AP_LAUNCH(0);
   AP_LAUNCH(1);

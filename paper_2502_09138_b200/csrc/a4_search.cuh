@@ -67,13 +67,13 @@ __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefe
 // for the load right there -- which would turn every gather that is issued one step ahead into a blocking one.
 // (y, z, up link) of a cluster record as three scalar loads: a predicated 128-bit load needs an aligned register
 // quad, which ptxas then copies out of right behind the load (and so waits for it); scalars land in place.
-struct Rec {   // an srt record: (y, z, cluster id, cleaned up link as a sorted position)
+struct Rec {   // a chain hit: its srt record (y, z, cluster id) and its cleaned up link (a sorted position, a3's table)
   int y, z, id, up;
 };
-__device__ __forceinline__ void ld_rec_if(Rec& v, const int4* p, bool pred) {
+__device__ __forceinline__ void ld_rec_if(Rec& v, const int4* p, const int32_t* link, bool pred) {
   asm volatile("{ .reg .pred q; setp.ne.s32 q, %4, 0; @q ld.global.nc.s32 %0, [%5]; @q ld.global.nc.s32 %1, [%5+4];"
-               " @q ld.global.nc.s32 %2, [%5+8]; @q ld.global.nc.s32 %3, [%5+12]; }"
-               : "+r"(v.y), "+r"(v.z), "+r"(v.id), "+r"(v.up) : "r"((int)pred), "l"(p));
+               " @q ld.global.nc.s32 %2, [%5+8]; @q ld.global.nc.s32 %3, [%6]; }"
+               : "+r"(v.y), "+r"(v.z), "+r"(v.id), "+r"(v.up) : "r"((int)pred), "l"(p), "l"(link));
 }
 // (y, z) of a recorded hit out of the tracklet's own stream (written by this call's upward pass: read through L2)
 __device__ __forceinline__ void ld_cg_yz_if(int& y, int& z, const int2* p, bool pred) {

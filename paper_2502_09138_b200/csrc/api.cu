@@ -64,6 +64,7 @@ size_t layout(tpc_tracker* t, char* base, int64_t n, int64_t R) {
   s.bin_start = (uint32_t*)take((size_t)R * t->g.nb_stride * 4);
   s.link_up = (int32_t*)take((size_t)n * 4);
   s.link_dn = (int32_t*)take((size_t)n * 4);
+  s.clean_up = (int32_t*)take((size_t)n * 4);
   s.owner = (uint32_t*)take((size_t)n * 4);
   s.hit_row = (uint8_t*)take((size_t)n + 64);
   s.q_items = (uint32_t*)take((size_t)s_cap * 3 * A4_Q_BUCKETS * 4);

@@ -6,11 +6,12 @@
 namespace {
 
 // Links live in sorted space (positions in srt); the exports translate them to cluster ids.
-// which = 0: the raw a2 tables.  which = 1: the cleaned links exactly as a3 left them for a4 -- the cleaned up link
-// is the fourth word of the srt record; a3 keeps no down-link table (nothing downstream reads one), so the cleaned
+// which = 0: the raw a2 tables.  which = 1: the cleaned links exactly as a3 left them for a4 -- the cleaned up links
+// are a3's clean_up table; a3 keeps no down-link table (nothing downstream reads one), so the cleaned
 // down links are the inverse of what it wrote (mutuality, P11): dn'[up'[h]] = h.
 __global__ void dbg_links_kernel(int64_t n, int which, const int4* __restrict__ srt, const int32_t* __restrict__ up,
-                                 const int32_t* __restrict__ dn, int32_t* __restrict__ up_o,
+                                 const int32_t* __restrict__ dn, const int32_t* __restrict__ clean_up,
+                                 int32_t* __restrict__ up_o,
                                  int32_t* __restrict__ dn_o) {
   const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= n) return;
@@ -20,18 +21,19 @@ __global__ void dbg_links_kernel(int64_t n, int which, const int4* __restrict__ 
     up_o[c.z] = u >= 0 ? srt[u].z : -1;
     dn_o[c.z] = d >= 0 ? srt[d].z : -1;
   } else {
-    up_o[c.z] = c.w >= 0 ? srt[c.w].z : -1;
-    if (c.w >= 0) dn_o[srt[c.w].z] = c.z;
+    const int cu = clean_up[p];
+    up_o[c.z] = cu >= 0 ? srt[cu].z : -1;
+    if (cu >= 0) dn_o[srt[cu].z] = c.z;
   }
 }
 
 __global__ void dbg_seed_len_kernel(const DevCtl* ctl, const int32_t* __restrict__ seed_start,
-                                    const int32_t* __restrict__ seed_pos, const int4* __restrict__ srt,
+                                    const int32_t* __restrict__ seed_pos, const int32_t* __restrict__ clean_up,
                                     int32_t* __restrict__ start, int32_t* __restrict__ len) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= (int64_t)ctl->n_seeds) return;
   int l = 1;
-  for (int c = srt[seed_pos[i]].w; c >= 0; c = srt[c].w) ++l;
+  for (int c = clean_up[seed_pos[i]]; c >= 0; c = clean_up[c]) ++l;
   start[i] = seed_start[i];
   len[i] = l;
 }
@@ -67,12 +69,12 @@ cudaError_t launch_dbg_links(const tpc_tracker* t, int64_t n, int which, int32_t
     cudaError_t e = cudaMemsetAsync(dn, 0xff, (size_t)n * 4, st);
     if (e != cudaSuccess) return e;
   }
-  dbg_links_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, which, t->s.srt, t->s.link_up, t->s.link_dn, up, dn);
+  dbg_links_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, which, t->s.srt, t->s.link_up, t->s.link_dn, t->s.clean_up, up, dn);
   return cudaGetLastError();
 }
 cudaError_t launch_dbg_seed_len(const tpc_tracker* t, int32_t* start, int32_t* len, cudaStream_t st) {
   if (t->s_cap == 0) return cudaSuccess;
-  dbg_seed_len_kernel<<<(unsigned)((t->s_cap + 255) / 256), 256, 0, st>>>(t->s.ctl, t->s.seed_start, t->s.seed_pos, t->s.srt, start, len);
+  dbg_seed_len_kernel<<<(unsigned)((t->s_cap + 255) / 256), 256, 0, st>>>(t->s.ctl, t->s.seed_start, t->s.seed_pos, t->s.clean_up, start, len);
   return cudaGetLastError();
 }
 cudaError_t launch_dbg_tracklets(const tpc_tracker* t, float* par, float* cov, float* chi2, int32_t* n_hits,

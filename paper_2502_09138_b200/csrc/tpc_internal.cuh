@@ -47,12 +47,13 @@ struct DevCtl {
 
 struct Scratch {
   // a1
-  int4* srt;                // clusters in bin order inside each row: (y, z, cluster id, cleaned up link as a sorted
-                            // position or -1 [a3]) -- one 16-B load per search candidate and per followed chain hit
+  int4* srt;                // clusters in bin order inside each row: (y, z, cluster id, 0) -- one 16-B load per search
+                            // candidate and per followed chain hit
   uint32_t* sec_key;        // [n_sectors] a0: order-preserving key of the sector's smallest z (zeroed per call)
   uint32_t* bin_start;      // [R * nb_stride] global sorted index of the first cluster of each bin (+ sentinel)
   // a2 / a3: raw links in SORTED space (position of the linked cluster in srt, -1 = none), written coalesced
   int32_t *link_up, *link_dn;
+  int32_t* clean_up;        // [n, sorted space] a3: the cleaned up link (P11: the raw one where it is mutual, else -1)
   uint32_t* owner;          // [n, id space] packed (n_hits << 24 | 0xFFFFFF - rank), 0 = none (zeroed per call)
   uint8_t* hit_row;         // [n] a5: row of the hit at each position of the output hit list (for a6)
   uint32_t* q_items;        // [3 * A4_Q_BUCKETS][s_cap] a4 phase queues: seed ranks
