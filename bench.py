@@ -347,6 +347,20 @@ def run_ours(args):
     l1.record(stream)
     torch.cuda.synchronize()
     latency_ms = l0.elapsed_time(l1) / 10
+    # the same call captured once into a CUDA graph and replayed (14 launches become one)
+    cg = torch.cuda.CUDAGraph()
+    gs = torch.cuda.Stream(device=dev)
+    with torch.cuda.graph(cg, stream=gs):
+        trk1.track(y1, z1, ro1, out1, torch.cuda.current_stream())
+    for _ in range(3):
+        cg.replay()
+    torch.cuda.synchronize()
+    l0.record()
+    for _ in range(10):
+        cg.replay()
+    l1.record()
+    torch.cuda.synchronize()
+    latency_graph_ms = l0.elapsed_time(l1) / 10
     trk1.close()
 
     # ---- end to end through the host-buffer entry point --------------------------------------------------
@@ -464,7 +478,7 @@ def run_ours(args):
                        "l2": f"working set {trk.scratch_bytes() / 1e6:.0f} MB scratch + {8 * n / 1e6:.0f} MB input "
                              f"> 126 MB L2; no explicit flush"},
             "tracks_per_s": len(tracks) * world * args.steps / (ms_max * 1e-3),
-            "single_event_latency_ms": latency_ms,
+            "single_event_latency_ms": latency_ms, "single_event_latency_cuda_graph_ms": latency_graph_ms,
             "next": {"a6_refit_ms": refit_ms, "tracks_refitted": len(tracks), "a7_merge_ms": merge_ms, "a6_refit_merged_ms": refit_merged_ms, "a8_compress_ms": compress_ms, "a9_clusterize_ms_one_event": clusterize_ms,
                      "clusterize_digits": int(dg.n), "clusterize_clusters": n_found,
                      "clusterize_digits_per_s": dg.n / (clusterize_ms * 1e-3),

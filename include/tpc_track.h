@@ -119,6 +119,9 @@ int tpc_tracker_create(const tpc_geometry_t* geometry, const tpc_field_t* field,
 
 /* Runs a1..a5 on n clusters, enqueued on `stream`; no host synchronisation unless scratch must grow.
  * clusters and out are [host] structs holding [device] pointers.  n may be 0.
+ * The call only enqueues memsets and kernels whose launch parameters depend on (n, the handle) alone: once an earlier
+ * call of at least this size has sized the scratch (and with stage timing off) it can be captured into a CUDA graph
+ * (stream capture on `stream`) and replayed on new data in the same buffers.
  * Errors: TPC_ERR_ARG, TPC_ERR_CAPACITY, TPC_ERR_NOMEM, TPC_ERR_CUDA. */
 int tpc_track(tpc_tracker_t* t, const tpc_clusters_t* clusters, int64_t n, void* stream, tpc_tracks_out_t* out);
 

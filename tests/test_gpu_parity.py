@@ -566,6 +566,43 @@ def test_compress_residual_streams_bit_exact_and_lossless(orc):
         trk.close()
 
 
+def test_track_call_replays_from_a_cuda_graph():
+    """tpc_track only enqueues work whose launch parameters depend on (n, handle): captured once into a CUDA graph it
+    replays on new clusters written into the same buffers and gives that event's own result."""
+    import torch
+    from paper_2502_09138_b200 import Tracker
+    from paper_2502_09138_b200.events import geometry_from_event, upload
+    ev_a, ev_b = make_event(1, 1000), make_event(1, 1001)
+    n = max(ev_a.n, ev_b.n)
+    trk = Tracker(geometry_from_event(ev_a))
+
+    def padded(ev):   # same n for both events: the extra clusters go to the last (sector,row), far outside the volume
+        y = np.concatenate([ev.y, np.full(n - ev.n, 0, np.int32)])
+        z = np.concatenate([ev.z, np.full(n - ev.n, ev.z.max(), np.int32)])
+        ro = ev.row_offsets.copy()
+        ro[-1] = n
+        return y, z, ro
+
+    ya, za, roa = padded(ev_a)
+    y, z, ro = (torch.from_numpy(a.view(np.int32) if a.dtype == np.uint32 else a).cuda() for a in (ya, za, roa))
+    ref_a = trk.track(y, z, ro).to_host()
+    out = trk.alloc_out(n)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=torch.cuda.Stream()):
+        trk.track(y, z, ro, out, stream=torch.cuda.current_stream())
+    g.replay()
+    got_a = out.to_host()
+    assert np.array_equal(got_a[1], ref_a[1]) and np.array_equal(got_a[0]["n_hits"], ref_a[0]["n_hits"])
+    yb, zb, rob = padded(ev_b)
+    y.copy_(torch.from_numpy(yb)); z.copy_(torch.from_numpy(zb)); ro.copy_(torch.from_numpy(rob.view(np.int32)))
+    g.replay()
+    got_b = out.to_host()
+    ref_b = trk.track(y, z, ro).to_host()
+    assert len(got_b[0]) == len(ref_b[0]) and len(got_b[0]) != len(got_a[0])
+    assert np.array_equal(got_b[1], ref_b[1]) and np.array_equal(got_b[0]["hit_offset"], ref_b[0]["hit_offset"])
+    trk.close()
+
+
 def _rans_equal(enc, ref, label):
     nb, ne = int(ref["chunk_off"][-1]), int(ref["esc_off"][-1])
     c = enc["counts"].cpu().numpy()
