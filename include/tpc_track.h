@@ -36,6 +36,7 @@ extern "C" {
 #define TPC_ERR_CUDA (-3)      /* a CUDA runtime call failed (tpc_last_cuda_error() tells which) */
 #define TPC_ERR_NOMEM (-4)     /* scratch allocation failed */
 #define TPC_ERR_CAPACITY (-5)  /* n too large for the packed ownership word (n/l_min >= 2^24) */
+#define TPC_ERR_STATIC_SCRATCH (-6) /* tpc_rans_encode_static: the input needs more than its fixed scratch array */
 
 /* device-side flags OR-ed into counts[2] */
 #define TPC_FLAG_TRACK_OVERFLOW 1u /* more output tracks than track_capacity: tracks beyond it not written */
@@ -240,6 +241,25 @@ int tpc_rans_encode(tpc_tracker_t* t, const void* values, int32_t value_bytes, i
 /* The inverse: n values from a stream written with the same alphabet_bits and chunk. */
 int tpc_rans_decode(tpc_tracker_t* t, const tpc_rans_stream_t* in, int64_t n, int32_t alphabet_bits, int32_t chunk,
                     void* stream, void* values, int32_t value_bytes);
+
+/* tpc_rans_encode for callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that
+ * forbid cudaMalloc): the same kernels, the same stream layout and bytes as tpc_rans_encode, but the scratch (chunk
+ * slots, histogram, cumulative table, per-chunk counts) is a fixed array in device memory that belongs to the library
+ * image, not to a handle -- TPC_RANS_STATIC_SCRATCH_BYTES on every GPU that loads the library, until the process
+ * exits.  No handle; the call makes no cudaMalloc / cudaFree and calls no allocating library routine (the first call
+ * on a device looks the array's address up once, cudaGetSymbolAddress, with that device current).
+ * Limit: the scratch a call needs is
+ *     ceil(n / chunk) * (4 + 2 * chunk)  +  4 * 2^alphabet_bits  +  4 * (2^alphabet_bits + 1)  +  8 * (ceil(n / chunk) + 1)
+ * bytes (each of the four parts rounded up to 16); an input that needs more than TPC_RANS_STATIC_SCRATCH_BYTES is
+ * rejected with TPC_ERR_STATIC_SCRATCH before anything is enqueued.  2 000 000 values at chunk = 512, alphabet_bits = 12
+ * fit (one central Pb-Pb event has ~560 000 owned clusters per residual stream).
+ * All calls on a device share the one array and it keeps the last call's contents: every call clears what must start
+ * at zero itself, but two calls that overlap on the GPU (different streams, or graphs replayed concurrently) race --
+ * serialise them.  Arguments, outputs and the other errors as for tpc_rans_encode; after TPC_ERR_CUDA there is no handle
+ * whose tpc_last_cuda_error could be asked. */
+#define TPC_RANS_STATIC_SCRATCH_BYTES (4u << 20)
+int tpc_rans_encode_static(const void* values, int32_t value_bytes, int64_t n, int32_t alphabet_bits, int32_t chunk,
+                           void* stream, const tpc_rans_stream_t* out);
 
 /* NEXT-2 (readings P53..P56 in DESIGN.md): clusterizer in front of the path, digits -> clusters.
  * Digits of a (sector,row): cells (pad, time bin) with an ADC value >= 1, unique, ascending by (time, pad).

@@ -5,4 +5,4 @@ Argument marshalling only: every step of the path runs in the library's kernels.
 importing the binding without the built library, or calling it without a CUDA device, raises.
 """
 from .binding import (Geometry, Params, Tracker, TrackRec, TracksOut, TRACK_DTYPE, lib_path, load_library,  # noqa: F401
-                      declared_symbols)
+                      declared_symbols, rans_alloc, rans_encode_static, RANS_STATIC_SCRATCH_BYTES)

@@ -145,6 +145,8 @@ def load_library():
                                     C.POINTER(_RansStream)]
     lib.tpc_rans_decode.argtypes = [C.c_void_p, C.POINTER(_RansStream), C.c_int64, C.c_int32, C.c_int32, C.c_void_p,
                                     C.c_void_p, C.c_int32]
+    lib.tpc_rans_encode_static.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int32, C.c_int32, C.c_void_p,
+                                           C.POINTER(_RansStream)]
     lib.tpc_default_cluster_params.argtypes = [C.POINTER(ClusterParams)]
     lib.tpc_default_cluster_params.restype = None
     lib.tpc_clusterize.argtypes = [C.c_void_p, C.POINTER(_Digits), C.c_int64, C.POINTER(ClusterParams), C.c_void_p,
@@ -534,3 +536,39 @@ class Tracker:
         self._check(self._lib.tpc_debug_copy_grid(self._h, _ptr(ids), _ptr(bs), self._stream_ptr(None)))
         return dict(stride=stride, nz=nz, shift_y=sy, shift_z=sz, ids=ids.cpu().numpy(),
                     bin_start=bs.cpu().numpy().view(np.uint32).reshape(self.n_sectors * self.n_rows, stride))
+
+
+RANS_STATIC_SCRATCH_BYTES = 4 << 20     # TPC_RANS_STATIC_SCRATCH_BYTES
+
+
+def rans_encode_static(values, enc: dict, stream=None) -> dict:
+    """tpc_rans_encode_static: the encoder that allocates nothing (its scratch is a fixed array inside the library, at
+    most RANS_STATIC_SCRATCH_BYTES per call; all calls share it, so calls must not overlap on the GPU).  `enc` holds
+    the caller's output tensors, laid out as Tracker.rans_encode returns them (freq, chunk_off, esc_off, payload,
+    escapes, counts and n, alphabet_bits, chunk, value_bytes); it is written and returned.  Needs no Tracker."""
+    import torch
+    n = int(values.shape[0])
+    vb = {torch.int32: 4, torch.uint8: 1}[values.dtype]
+    if n != enc["n"] or vb != enc["value_bytes"]:
+        raise ValueError("enc was laid out for another input")
+    rs = Tracker._rans_struct(enc)
+    s = stream if stream is not None else torch.cuda.current_stream()
+    rc = load_library().tpc_rans_encode_static(C.c_void_p(_ptr(values)), vb, C.c_int64(n), enc["alphabet_bits"],
+                                               enc["chunk"], C.c_void_p(int(s.cuda_stream)), C.byref(rs))
+    if rc != 0:
+        raise TpcError(rc)
+    return enc
+
+
+def rans_alloc(n: int, alphabet_bits: int = 12, chunk: int = 512, value_bytes: int = 4, device="cuda") -> dict:
+    """Output tensors of an encode call for n values, sized so that any input fits (what Tracker.rans_encode makes)."""
+    import torch
+    n_chunks = (n + chunk - 1) // chunk
+    return dict(freq=torch.zeros(1 << alphabet_bits, dtype=torch.int32, device=device),
+                chunk_off=torch.zeros(n_chunks + 1, dtype=torch.int32, device=device),
+                esc_off=torch.zeros(n_chunks + 1, dtype=torch.int32, device=device),
+                payload=torch.zeros(max(4 * n_chunks + 2 * n, 2), dtype=torch.uint8, device=device),
+                escapes=torch.zeros(max(n, 1), dtype=torch.int32, device=device),
+                counts=torch.zeros(4, dtype=torch.int64, device=device),
+                n=n, alphabet_bits=alphabet_bits, chunk=chunk, value_bytes=value_bytes)
+

@@ -14,6 +14,8 @@
 //   encode : thread per chunk -> scratch slots, sizes; escapes to their place
 //   pack   : warp per chunk, slot -> payload
 //   decode : thread per chunk, symbol by binary search over the cumulative table
+#include <mutex>
+
 #include "tpc_internal.cuh"
 
 namespace {
@@ -283,3 +285,109 @@ cudaError_t launch_a10_rans_decode(const tpc_tracker* t, const tpc_rans_stream_t
                                                                    in->esc_off, in->payload, in->escapes, values);
   return cudaGetLastError();
 }
+
+// ---------------------------------------------------------------------------------------------------------------
+// tpc_rans_encode_static (include/tpc_track.h): the encoder for callers that must not allocate.  Same kernels, same
+// scratch layout; the scratch is this array, part of the library image on every GPU that loads it.  In host code the
+// name g_rans_static_scratch is only a stand-in for the symbol: the device address comes from cudaGetSymbolAddress,
+// once per device, with that device current, and that pointer is what the kernels get.
+// ---------------------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_rans_static_scratch[TPC_RANS_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mutex;
+void* g_static_ptr[STATIC_MAX_DEVICES];   // device address of the array, per device ordinal (NULL: not looked up yet)
+int g_static_sms[STATIC_MAX_DEVICES];
+
+// the launch sequence of launch_a10_rans_encode on a scratch pointer of the caller's
+cudaError_t enqueue_rans_encode(char* scratch, int sms, const void* values, int32_t value_bytes, int64_t n, int32_t bits,
+                                int32_t chunk, const tpc_rans_stream_t* out, cudaStream_t st) {
+  const int A = 1 << bits;
+  const int64_t n_chunks = (n + chunk - 1) / chunk;
+  char* p = scratch;
+  uint8_t* slots = (uint8_t*)p;        p += align_up((size_t)n_chunks * (4 + 2 * (size_t)chunk), 16);
+  uint32_t* hist = (uint32_t*)p;       p += align_up((size_t)A * 4, 16);
+  uint32_t* cum = (uint32_t*)p;        p += align_up(((size_t)A + 1) * 4, 16);
+  uint32_t* esc_cnt = (uint32_t*)p;    p += align_up((size_t)(n_chunks + 1) * 4, 16);
+  uint32_t* size = (uint32_t*)p;
+  // the array holds the previous call's contents: the histogram and the escape counts are accumulated into, so they
+  // start at zero; cum, size and the slots are written before they are read
+  cudaError_t e = cudaMemsetAsync(hist, 0, (size_t)A * 4, st);
+  if (e != cudaSuccess) return e;
+  e = cudaMemsetAsync(esc_cnt, 0, (size_t)(n_chunks + 1) * 4, st);
+  if (e != cudaSuccess) return e;
+  e = cudaMemsetAsync(out->counts, 0, 4 * sizeof(int64_t), st);
+  if (e != cudaSuccess) return e;
+  const int grid_el = (int)std::min<int64_t>((n + RANS_THREADS - 1) / RANS_THREADS, (int64_t)sms * 8);
+  const int grid_ch = (int)((n_chunks + RANS_THREADS - 1) / RANS_THREADS);
+  if (n > 0) {
+    if (value_bytes == 1)
+      rans_count_kernel<uint8_t><<<grid_el, RANS_THREADS, 0, st>>>(values, n, bits, chunk, hist, esc_cnt);
+    else
+      rans_count_kernel<int32_t><<<grid_el, RANS_THREADS, 0, st>>>(values, n, bits, chunk, hist, esc_cnt);
+  }
+  rans_table_kernel<<<1, 1024, 0, st>>>(bits, n, hist, out->freq, cum);
+  rans_scan_kernel<<<1, 1024, 0, st>>>(esc_cnt, n_chunks, out->esc_off, out->counts + 1);
+  if (n > 0) {
+    if (value_bytes == 1)
+      rans_encode_kernel<uint8_t><<<grid_ch, RANS_THREADS, 0, st>>>(values, n, bits, chunk, n_chunks, out->freq, cum,
+                                                                     out->esc_off, out->escape_capacity, slots, size,
+                                                                     out->escapes);
+    else
+      rans_encode_kernel<int32_t><<<grid_ch, RANS_THREADS, 0, st>>>(values, n, bits, chunk, n_chunks, out->freq, cum,
+                                                                     out->esc_off, out->escape_capacity, slots, size,
+                                                                     out->escapes);
+  }
+  rans_scan_kernel<<<1, 1024, 0, st>>>(size, n_chunks, out->chunk_off, out->counts);
+  if (n > 0)
+    rans_pack_kernel<<<sms * 8, RANS_THREADS, 0, st>>>(chunk, n_chunks, slots, out->chunk_off, out->payload_capacity,
+                                                       out->payload);
+  rans_counts_kernel<<<1, 1, 0, st>>>(n_chunks, out->payload_capacity, out->escape_capacity, out->counts);
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+
+extern "C" {
+#pragma GCC visibility push(default)
+
+int tpc_rans_encode_static(const void* values, int32_t value_bytes, int64_t n, int32_t alphabet_bits, int32_t chunk,
+                           void* stream, const tpc_rans_stream_t* out) {
+  if (!out || n < 0 || n >= ((int64_t)1 << 31) || (value_bytes != 1 && value_bytes != 4)) return TPC_ERR_ARG;
+  if (alphabet_bits < 1 || alphabet_bits > RANS_MAX_BITS || chunk < 1 || chunk > 65535) return TPC_ERR_ARG;
+  if (!out->freq || !out->chunk_off || !out->esc_off || !out->counts || out->payload_capacity < 0 ||
+      out->escape_capacity < 0)
+    return TPC_ERR_ARG;
+  if (n > 0 && (!values || (out->payload_capacity > 0 && !out->payload) || (out->escape_capacity > 0 && !out->escapes)))
+    return TPC_ERR_ARG;
+  if (rans_scratch_bytes(n, chunk, alphabet_bits) > (size_t)TPC_RANS_STATIC_SCRATCH_BYTES) return TPC_ERR_STATIC_SCRATCH;
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return TPC_ERR_CUDA;
+  if (dev < 0 || dev >= STATIC_MAX_DEVICES) return TPC_ERR_ARG;
+  char* scratch = nullptr;
+  int sms = 0;
+  {
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {   // once per device, with that device current
+      void* p = nullptr;
+      if (cudaGetSymbolAddress(&p, g_rans_static_scratch) != cudaSuccess || !p) return TPC_ERR_CUDA;
+      int count = 0;
+      if (cudaDeviceGetAttribute(&count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || count <= 0)
+        return TPC_ERR_CUDA;
+      g_static_sms[dev] = count;
+      g_static_ptr[dev] = p;
+    }
+    scratch = (char*)g_static_ptr[dev];
+    sms = g_static_sms[dev];
+  }
+  if (enqueue_rans_encode(scratch, sms, values, value_bytes, n, alphabet_bits, chunk, out, (cudaStream_t)stream) !=
+      cudaSuccess)
+    return TPC_ERR_CUDA;
+  return TPC_OK;
+}
+
+#pragma GCC visibility pop
+}  // extern "C"

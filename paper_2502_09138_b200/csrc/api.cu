@@ -187,6 +187,7 @@ const char* tpc_status_string(int status) {
     case TPC_ERR_CUDA: return "CUDA runtime error";
     case TPC_ERR_NOMEM: return "out of device memory";
     case TPC_ERR_CAPACITY: return "too many clusters for one call";
+    case TPC_ERR_STATIC_SCRATCH: return "input needs more scratch than the static array of tpc_rans_encode_static holds";
     default: return "unknown status";
   }
 }
