@@ -33,6 +33,8 @@ struct Env {   // everything a warp needs that does not change during a kernel
   const double* s_row_x;   // shared-memory copies
   const float* s_row_dx;
   int2* s_yz;              // this lane's staging column for the (y, z) stream: slot k at s_yz[k * AP_THREADS]
+  int* s_tab;              // likewise for the hit table: eight rows = one 32-byte group
+  bool tab_groups;         // n_rows is a multiple of 8: every aligned group of eight rows lies inside the tracklet's table
   int yz_stride;           // entries per tracklet in tl_yz: n_rows rounded up to a multiple of 4 (32-byte groups)
   uint32_t n_seeds, s_cap;
   int lane, lanes_used;
@@ -179,6 +181,36 @@ __device__ __forceinline__ void yz_flush(const Env& e, const Trk& t, int row, in
   }
 }
 
+// The hit table (4-byte entries) goes through an eight-row staging column in the same way, for the same reason.
+// Stale slots of a group land in rows the phase did not visit: a later phase that visits them rewrites them (it
+// stores row by row inside a group it shares with an earlier phase), and rows no phase visits lie outside
+// [rmin, rmax] and are padded with -1 by the votes kernel.
+__device__ __forceinline__ void tab_stage(const Env& e, int row, int id) { e.s_tab[(row & 7) * AP_THREADS] = id; }
+__device__ __forceinline__ void tab_store_group(const Env& e, const Trk& t, int base) {
+  const int* c = e.s_tab;
+  int4* dst = (int4*)(t.tab + base);
+  dst[0] = make_int4(c[0], c[AP_THREADS], c[2 * AP_THREADS], c[3 * AP_THREADS]);
+  dst[1] = make_int4(c[4 * AP_THREADS], c[5 * AP_THREADS], c[6 * AP_THREADS], c[7 * AP_THREADS]);
+}
+// upward phases: rows [first, row] of the group of `row` are staged; rows below `first` are an earlier phase's
+__device__ __forceinline__ void tab_flush_up(const Env& e, const Trk& t, int row, int first) {
+  const int base = row & ~7;
+  if (e.tab_groups && base >= first) {
+    tab_store_group(e, t, base);
+  } else {
+    for (int r = max(first, base); r <= row; ++r) t.tab[r] = e.s_tab[(r & 7) * AP_THREADS];
+  }
+}
+// downward phase: rows [row, last] of the group of `row` are staged; rows above `last` are an earlier phase's
+__device__ __forceinline__ void tab_flush_down(const Env& e, const Trk& t, int row, int last) {
+  const int base = row & ~7;
+  if (e.tab_groups && base + 7 <= last) {
+    tab_store_group(e, t, base);
+  } else {
+    for (int r = row; r <= min(last, base + 7); ++r) t.tab[r] = e.s_tab[(r & 7) * AP_THREADS];
+  }
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 // Phase A: P19 initial state + fit up the seed chain, no gate.  Items = seed ranks from ctl->next_seed.
 // ---------------------------------------------------------------------------------------------------------------
@@ -195,6 +227,7 @@ __device__ __forceinline__ void phase_a(const Env& e) {
   Rec rcn = {0, 0, -1, -1};   // the chain hit of the next step (requested one step ahead: its record and its link)
   bool more = false;          // rcn holds a chain hit
   bool dirty = false;         // the staging column holds rows that are not in tl_yz yet
+  bool dirty_t = false;       // likewise for the hit table
   while (true) {
     const bool want = !live && e.lane < e.lanes_used && !exhausted;
     const unsigned idle = __ballot_sync(FULL, want);
@@ -233,9 +266,10 @@ __device__ __forceinline__ void phase_a(const Env& e) {
     if (ok) {
       b.row = trow;
       update(g, p, C, resid_y(g, p, rc.y), resid_z(g, p, rc.z));
-      t.tab[trow] = rc.id;
+      tab_stage(e, trow, rc.id);
       yz_stage(e, trow, rc.y, rc.z);
       dirty = true;
+      dirty_t = true;
       b.rmax = trow;
       ++b.nh;
       more = rc.up >= 0;
@@ -246,6 +280,10 @@ __device__ __forceinline__ void phase_a(const Env& e) {
     if (dirty && ((b.row & 3) == 3 || leave)) {
       yz_flush(e, t, b.row, 0);   // rows of the group below the seed's first row are never read: whole groups
       dirty = false;
+    }
+    if (dirty_t && ((b.row & 7) == 7 || leave)) {
+      tab_flush_up(e, t, b.row, 0);
+      dirty_t = false;
     }
     if (leave) state_save(e, t, p, C, b);
     const bool to_b = leave && ok && b.row + 1 < g.n_rows;
@@ -323,6 +361,7 @@ __device__ __forceinline__ void phase_b(const Env& e) {
   BinRanges pq = {0, 0, 0, 0};
   int fr = 0;           // first row this phase visits for the tracklet (the rows below are phase A's)
   bool dirty = false;   // the staging column holds rows that are not in tl_yz yet
+  bool dirty_t = false; // likewise for the hit table
   while (true) {
     const bool want = !live && e.lane < e.lanes_used && !dry;
     const unsigned idle = __ballot_sync(FULL, want);
@@ -352,9 +391,10 @@ __device__ __forceinline__ void phase_b(const Env& e) {
     if (ok) {
       b.row = trow;
       const Found f = search_step(e, t, p, C, trow, pk_y, pk_z, pq);
-      t.tab[trow] = f.id;
+      tab_stage(e, trow, f.id);
       yz_stage(e, trow, f.id >= 0 ? f.hy : YZ_NONE, f.hz);
       dirty = true;
+      dirty_t = true;
       b.rmax = trow;
       if (f.id >= 0) {
         update(g, p, C, f.ry, f.rz);
@@ -371,6 +411,10 @@ __device__ __forceinline__ void phase_b(const Env& e) {
     if (dirty && ((b.row & 3) == 3 || leave)) {
       yz_flush(e, t, b.row, fr);
       dirty = false;
+    }
+    if (dirty_t && ((b.row & 7) == 7 || leave)) {
+      tab_flush_up(e, t, b.row, fr);
+      dirty_t = false;
     }
     if (leave) state_save(e, t, p, C, b);
     queue_push(e, Q_C, len_bucket(b.row - t.r0, g.n_rows), t.i, leave);
@@ -470,6 +514,8 @@ __device__ __forceinline__ void phase_d(const Env& e) {
   cov_reset(g, C);
   uint32_t pk_y = 0xFFFFFFFFu, pk_z = 0xFFFFFFFFu;
   BinRanges pq = {0, 0, 0, 0};
+  int d_last = 0;         // first (= highest) row this phase visits for the tracklet; the rows above are earlier phases'
+  bool dirty_t = false;   // the staging column holds hit-table rows that are not in tl_hits yet
   while (true) {
     const bool want = !live && e.lane < e.lanes_used && !dry;
     const unsigned idle = __ballot_sync(FULL, want);
@@ -479,6 +525,7 @@ __device__ __forceinline__ void phase_d(const Env& e) {
       if (i >= 0) {
         state_load(e, i, t, p, C, b);
         pk_y = pk_z = 0xFFFFFFFFu;
+        d_last = b.row - 1;
         live = true;
       }
     }
@@ -508,7 +555,12 @@ __device__ __forceinline__ void phase_d(const Env& e) {
     if (srch) {
       if (ok) {
         const Found f = search_step(e, t, p, C, trow, pk_y, pk_z, pq);
-        t.tab[trow] = f.id;
+        tab_stage(e, trow, f.id);
+        dirty_t = true;
+        if ((trow & 7) == 0) {
+          tab_flush_down(e, t, trow, d_last);
+          dirty_t = false;
+        }
         b.rmin = min(b.rmin, trow);
         if (f.id >= 0) {
           b.chi2 += update(g, p, C, f.ry, f.rz);
@@ -529,6 +581,10 @@ __device__ __forceinline__ void phase_d(const Env& e) {
     // ---- tracklets that ended: record, padding of the hit table and ownership votes ----
     const unsigned done = __ballot_sync(FULL, fin);
     if (done) {
+      if (fin && dirty_t) {   // b.rmin is the lowest row this phase wrote
+        tab_flush_down(e, t, b.rmin, d_last);
+        dirty_t = false;
+      }
       if (fin) {
         float4* o = e.tl_rec + (size_t)t.i * TL_REC_V4;
         o[0] = make_float4((float)e.s_row_x[b.row], (float)(((double)p.y + (double)p.oy) * g.inv_units_d),
@@ -586,6 +642,7 @@ a4_phase_kernel(const DevGeom g, uint32_t s_cap, DevCtl* __restrict__ ctl, const
                 int4* __restrict__ tl_state, uint32_t* __restrict__ q_items, uint32_t* __restrict__ tl_span) {
   extern __shared__ double smem_ap[];
   __shared__ int2 s_yz[4][AP_THREADS];
+  __shared__ int s_tab[8][AP_THREADS];
   const int nr = g.n_rows;
   const uint32_t n_seeds = ctl->n_seeds;
   if (n_seeds == 0) return;
@@ -604,6 +661,8 @@ a4_phase_kernel(const DevGeom g, uint32_t s_cap, DevCtl* __restrict__ ctl, const
   e.q_items = q_items; e.tl_span = tl_span; e.s_row_x = s_row_x; e.s_row_dx = s_row_dx;
   e.n_seeds = n_seeds; e.s_cap = s_cap;
   e.s_yz = &s_yz[0][threadIdx.x];
+  e.s_tab = &s_tab[0][threadIdx.x];
+  e.tab_groups = (nr & 7) == 0;
   e.yz_stride = (nr + 3) & ~3;
   e.lane = threadIdx.x & 31;
   // few seeds (one small event): spread them over all warps instead of filling the first warps' 32 lanes
