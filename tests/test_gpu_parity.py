@@ -774,6 +774,19 @@ def test_both_a4_variants_on_small_and_stress_events(orc, mode):
         compare(ev, orc, _run_gpu(ev, a4_variant=variant), orc.track(ev), label=f"{lab} a4={mode}")
 
 
+def test_phase_kernels_on_row_counts_that_are_no_multiple_of_eight(orc):
+    """The phase kernels write their hit tables in aligned groups of eight rows when n_rows allows it and row by row
+    otherwise: 43 rows (odd: no aligned group fits every tracklet's table) and 40 rows, both with the phase kernels
+    forced, must give the oracle's tracks."""
+    from gen.events import Config
+    for nr in (43, 40):
+        cfg = Config(f"one_sector_{nr}_rows", n_sectors=1, open_sector=True, tracks_per_collision=800, pt_min=0.3,
+                     noise=0.05, n_rows=nr)
+        ev = make_event(cfg, seed=11)
+        assert ev.n_rows == nr
+        compare(ev, orc, _run_gpu(ev, a4_variant=2), orc.track(ev), label=f"{nr} rows, phase kernels")
+
+
 def test_a2_staged_variant_gives_the_same_links(orc):
     """a2 with the neighbour rows staged in shared memory by TMA bulk copies (north_star's sketch): bit-exact links on a
     sparse event, on a 40-row geometry (chunks of 19 rows with a ragged tail), on rows longer than a staging slot
