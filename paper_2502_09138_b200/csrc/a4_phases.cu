@@ -35,6 +35,7 @@ struct Env {   // everything a warp needs that does not change during a kernel
   int2* s_yz;              // this lane's staging column for the (y, z) stream: slot k at s_yz[k * AP_THREADS]
   int* s_tab;              // likewise for the hit table: eight rows = one 32-byte group
   bool tab_groups;         // n_rows is a multiple of 8: every aligned group of eight rows lies inside the tracklet's table
+  float bucket_scale;      // A4_Q_BUCKETS / n_rows
   int yz_stride;           // entries per tracklet in tl_yz: n_rows rounded up to a multiple of 4 (32-byte groups)
   uint32_t n_seeds, s_cap;
   int lane, lanes_used;
@@ -116,8 +117,9 @@ __device__ __forceinline__ void state_load(const Env& e, int i, Trk& t, State& p
 
 // Length bucket of a tracklet entering a phase: the rows it has left to cover.  Longest first (bucket 0), so that
 // the tail of each phase kernel consists of short tracklets.
-__device__ __forceinline__ int len_bucket(int rows_left, int n_rows) {
-  const int b = (A4_Q_BUCKETS - 1) - min(max(rows_left, 0), n_rows - 1) * A4_Q_BUCKETS / n_rows;
+__device__ __forceinline__ int len_bucket(const Env& e, int rows_left) {
+  // evaluated by every lane in every step: a multiplication, not an integer division (the bucket only orders the work)
+  const int b = (A4_Q_BUCKETS - 1) - __float2int_rz((float)min(max(rows_left, 0), e.g.n_rows - 1) * e.bucket_scale);
   return b < 0 ? 0 : b;
 }
 
@@ -287,8 +289,8 @@ __device__ __forceinline__ void phase_a(const Env& e) {
     }
     if (leave) state_save(e, t, p, C, b);
     const bool to_b = leave && ok && b.row + 1 < g.n_rows;
-    queue_push(e, Q_B, len_bucket(g.n_rows - 1 - b.row, g.n_rows), t.i, to_b);
-    queue_push(e, Q_C, len_bucket(b.row - t.r0, g.n_rows), t.i, leave && !to_b);
+    queue_push(e, Q_B, len_bucket(e, g.n_rows - 1 - b.row), t.i, to_b);
+    queue_push(e, Q_C, len_bucket(e, b.row - t.r0), t.i, leave && !to_b);
     if (leave) live = false;
   }
 }
@@ -417,7 +419,7 @@ __device__ __forceinline__ void phase_b(const Env& e) {
       dirty_t = false;
     }
     if (leave) state_save(e, t, p, C, b);
-    queue_push(e, Q_C, len_bucket(b.row - t.r0, g.n_rows), t.i, leave);
+    queue_push(e, Q_C, len_bucket(e, b.row - t.r0), t.i, leave);
     if (leave) live = false;
   }
 }
@@ -490,7 +492,7 @@ __device__ __forceinline__ void phase_c(const Env& e) {
     }
     const bool leave = live && (!ok || b.row <= t.r0);   // below the seed's first row phase D searches
     if (leave) state_save(e, t, p, C, b);
-    queue_push(e, Q_D, len_bucket(b.row, g.n_rows), t.i, leave);
+    queue_push(e, Q_D, len_bucket(e, b.row), t.i, leave);
     if (leave) live = false;
   }
 }
@@ -664,6 +666,7 @@ a4_phase_kernel(const DevGeom g, uint32_t s_cap, DevCtl* __restrict__ ctl, const
   e.s_tab = &s_tab[0][threadIdx.x];
   e.tab_groups = (nr & 7) == 0;
   e.yz_stride = (nr + 3) & ~3;
+  e.bucket_scale = (float)A4_Q_BUCKETS / (float)nr;
   e.lane = threadIdx.x & 31;
   // few seeds (one small event): spread them over all warps instead of filling the first warps' 32 lanes
   const uint32_t n_warps = gridDim.x * (blockDim.x >> 5);
