@@ -40,7 +40,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
                  const uint32_t* __restrict__ sec_key, const uint32_t* __restrict__ bin_start,
                  const int32_t* __restrict__ seed_pos, const int32_t* __restrict__ seed_sr,
                  float4* __restrict__ tl_rec, int32_t* __restrict__ tl_hits, int2* __restrict__ tl_yz,
-                 uint32_t* __restrict__ owner) {
+                 uint32_t* __restrict__ tl_span, uint32_t* __restrict__ owner) {
   extern __shared__ double smem_a4[];
   const unsigned FULL = 0xffffffffu;
   const int lane = threadIdx.x & 31;
@@ -263,7 +263,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
     pk_z = nk_z;
     pq = npq;
 
-    // ---- tracklets that ended: record, padding of the hit table and ownership votes ----
+    // ---- tracklets that ended: record, visited span and ownership votes ----
     const unsigned done = __ballot_sync(FULL, phase == PH_DONE);
     if (done) {
       if (phase == PH_DONE) {
@@ -277,6 +277,7 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
         o[3] = make_float4(cv[4], cv[5], cv[6], cv[7]);
         o[4] = make_float4(cv[8], cv[9], cv[10], cv[11]);
         o[5] = make_float4(cv[12], cv[13], cv[14], __int_as_float(sec_base + r0));
+        tl_span[i] = (uint32_t)rmin | ((uint32_t)rmax << 8);   // the rows outside hold nothing: a5 masks by the span
       }
       __syncwarp();   // the table entries of the ending lanes are visible to the whole warp
       unsigned dm = done;
@@ -298,7 +299,6 @@ a4_follow_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int4* __restri
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
           const int r = k * 32 + lane;
-          if (r < nr && (r < smin || r > smax)) out[r] = -1;
           if (word && v[k] >= 0) atomicMax(&owner[v[k]], word);
         }
       }
@@ -327,6 +327,6 @@ cudaError_t launch_a4_follow(const tpc_tracker* t, int64_t n, cudaStream_t st) {
   if (n == 0 || t->s_cap == 0) return cudaSuccess;
   a4_follow_kernel<<<t->a4_blocks, A4_THREADS, a4_smem_bytes(t->g), st>>>(
       t->g, t->s.ctl, t->s.srt, t->s.clean_up, t->s.sec_key, t->s.bin_start, t->s.seed_pos, t->s.seed_sr, t->s.tl_rec, t->s.tl_hits,
-      t->s.tl_yz, t->s.owner);
+      t->s.tl_yz, t->s.tl_span, t->s.owner);
   return cudaGetLastError();
 }

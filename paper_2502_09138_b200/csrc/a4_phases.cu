@@ -605,11 +605,13 @@ __device__ __forceinline__ void phase_d(const Env& e) {
   }
 }
 
-// P24, P26: owner(h) = surviving tracklet with the most hits, ties -> smallest rank; rows a tracklet never visited
-// get -1.  One warp per tracklet, grid-stride.
+// P24, P26: owner(h) = surviving tracklet with the most hits, ties -> smallest rank.  Only the rows the tracklet
+// visited (tl_span) hold entries; the rest of its table is never written and never read (a5 masks by the span too).
+// One warp per tracklet, grid-stride.
 __global__ void __launch_bounds__(256)
 a4_votes_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, const float4* __restrict__ tl_rec,
-                const uint32_t* __restrict__ tl_span, int32_t* __restrict__ tl_hits, uint32_t* __restrict__ owner) {
+                const uint32_t* __restrict__ tl_span, const int32_t* __restrict__ tl_hits,
+                uint32_t* __restrict__ owner) {
   const int nr = g.n_rows, lane = threadIdx.x & 31;
   const uint32_t n_seeds = ctl->n_seeds;
   const uint32_t warps = gridDim.x * (blockDim.x >> 5);
@@ -618,13 +620,12 @@ a4_votes_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, const float4* _
     const uint32_t span = tl_span[i];
     const int smin = span & 0xff, smax = (span >> 8) & 0xff;
     const uint32_t word = nh >= g.n_min_tracklet ? (((uint32_t)nh << 24) | (0xFFFFFFu - i)) : 0u;
-    int32_t* out = tl_hits + (size_t)i * nr;
-    for (int r = lane; r < nr; r += 32) {
-      if (r >= smin && r <= smax) {
+    if (!word) continue;   // P24: a discarded tracklet casts no vote
+    const int32_t* out = tl_hits + (size_t)i * nr;
+    for (int r = (smin & ~7) + lane; r <= smax; r += 32) {   // from the 32-byte group that holds the first row
+      if (r >= smin) {
         const int v = out[r];
-        if (word && v >= 0) atomicMax(&owner[v], word);
-      } else {
-        out[r] = -1;
+        if (v >= 0) atomicMax(&owner[v], word);
       }
     }
   }

@@ -22,7 +22,7 @@ constexpr int A5_UNROLL = 8;       // tracklets whose loads one warp keeps in fl
 __global__ void __launch_bounds__(256, 2)
 a5_select_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int32_t* __restrict__ seed_start,
                  const float4* __restrict__ tl_rec, const int32_t* __restrict__ tl_hits,
-                 const uint32_t* __restrict__ owner, uint64_t* __restrict__ status,
+                 const uint32_t* __restrict__ tl_span, const uint32_t* __restrict__ owner, uint64_t* __restrict__ status,
                  uint8_t* __restrict__ hit_row, tpc_track_rec_t* __restrict__ tracks, int32_t track_capacity,
                  int32_t* __restrict__ hit_ids,
                  int32_t hit_capacity, int32_t* __restrict__ counts) {
@@ -31,6 +31,7 @@ a5_select_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int32_t* __res
   __shared__ uint64_t sh_excl;
   __shared__ uint32_t own_mask[A5_TILE][A5_MASK_WORDS];
   __shared__ uint32_t s_word[A5_TILE];   // packed vote word of a surviving tracklet, 0 = discarded (P24)
+  __shared__ uint32_t s_span[A5_TILE];   // first | last << 8 row the tracklet visited: only those table entries exist
   __shared__ uint32_t sh_off[A5_TILE];   // output hit offset of a kept tracklet, 0xFFFFFFFF = no hit list to write
   const unsigned FULL = 0xffffffffu;
   const uint32_t n_seeds = ctl->n_seeds;
@@ -58,12 +59,16 @@ a5_select_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int32_t* __res
   const int64_t i = t0 + threadIdx.x;   // this thread's tracklet in the scans and the record
 
   if (threadIdx.x < A5_TILE) {
-    uint32_t w = 0;
+    uint32_t w = 0, sp = 1u;   // span 1 .. 0: empty
     if (threadIdx.x < n_here) {
       const int nh = __float_as_int(tl_rec[i * TL_REC_V4 + 1].w);
-      if (nh >= g.n_min_tracklet) w = ((uint32_t)nh << 24) | (0xFFFFFFu - (uint32_t)i);
+      if (nh >= g.n_min_tracklet) {   // a discarded tracklet owns nothing: none of its table is read
+        w = ((uint32_t)nh << 24) | (0xFFFFFFu - (uint32_t)i);
+        sp = tl_span[i];
+      }
     }
     s_word[threadIdx.x] = w;
+    s_span[threadIdx.x] = sp;
   }
   __syncthreads();
 
@@ -76,7 +81,11 @@ a5_select_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int32_t* __res
       int h[A5_UNROLL];
       uint32_t ow[A5_UNROLL];
 #pragma unroll
-      for (int u = 0; u < A5_UNROLL; ++u) h[u] = (in_row && tb + u < n_here) ? col[(int64_t)(tb + u) * nr] : -1;
+      for (int u = 0; u < A5_UNROLL; ++u) {
+        const uint32_t sp = s_span[min(tb + u, A5_TILE - 1)];
+        const bool in_span = in_row && tb + u < n_here && r >= (int)(sp & 0xffu) && r <= (int)((sp >> 8) & 0xffu);
+        h[u] = in_span ? col[(int64_t)(tb + u) * nr] : -1;
+      }
 #pragma unroll
       for (int u = 0; u < A5_UNROLL; ++u) ow[u] = h[u] >= 0 ? owner[h[u]] : 0u;
 #pragma unroll
@@ -177,7 +186,7 @@ cudaError_t launch_a5_select(const tpc_tracker* t, const tpc_tracks_out_t* out, 
   }
   const unsigned blocks = (unsigned)((t->s_cap + A5_TILE - 1) / A5_TILE);
   const int row_threads = 32 * ((t->g.n_rows + 31) / 32);
-  a5_select_kernel<<<blocks, row_threads > A5_TILE ? row_threads : A5_TILE, 0, st>>>(t->g, t->s.ctl, t->s.seed_start, t->s.tl_rec, t->s.tl_hits, t->s.owner,
+  a5_select_kernel<<<blocks, row_threads > A5_TILE ? row_threads : A5_TILE, 0, st>>>(t->g, t->s.ctl, t->s.seed_start, t->s.tl_rec, t->s.tl_hits, t->s.tl_span, t->s.owner,
                                               t->s.scan_a5, t->s.hit_row, out->tracks, out->track_capacity, out->hit_ids,
                                               out->hit_capacity, out->counts);
   return cudaGetLastError();

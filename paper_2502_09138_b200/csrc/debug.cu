@@ -39,7 +39,8 @@ __global__ void dbg_seed_len_kernel(const DevCtl* ctl, const int32_t* __restrict
 }
 
 __global__ void dbg_tracklets_kernel(const DevCtl* ctl, int n_rows, const float4* __restrict__ tl_rec,
-                                     const int32_t* __restrict__ tl_hits, float* par, float* cov, float* chi2,
+                                     const int32_t* __restrict__ tl_hits, const uint32_t* __restrict__ tl_span,
+                                     float* par, float* cov, float* chi2,
                                      int32_t* n_hits, int32_t* hits) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= (int64_t)ctl->n_seeds) return;
@@ -51,7 +52,10 @@ __global__ void dbg_tracklets_kernel(const DevCtl* ctl, int n_rows, const float4
   if (chi2) chi2[i] = q[6];
   if (n_hits) n_hits[i] = __float_as_int(q[7]);
   if (hits)
-    for (int r = 0; r < n_rows; ++r) hits[i * n_rows + r] = tl_hits[i * n_rows + r];
+    for (int r = 0; r < n_rows; ++r) {   // only the rows of the visited span hold entries
+      const int smin = tl_span[i] & 0xff, smax = (tl_span[i] >> 8) & 0xff;
+      hits[i * n_rows + r] = (r >= smin && r <= smax) ? tl_hits[i * n_rows + r] : -1;
+    }
 }
 
 __global__ void dbg_owner_kernel(int64_t n, const uint32_t* __restrict__ owner, int32_t* __restrict__ out) {
@@ -81,7 +85,7 @@ cudaError_t launch_dbg_tracklets(const tpc_tracker* t, float* par, float* cov, f
                                  int32_t* hits, cudaStream_t st) {
   if (t->s_cap == 0) return cudaSuccess;
   dbg_tracklets_kernel<<<(unsigned)((t->s_cap + 127) / 128), 128, 0, st>>>(
-      t->s.ctl, t->g.n_rows, t->s.tl_rec, t->s.tl_hits, par, cov, chi2, n_hits, hits);
+      t->s.ctl, t->g.n_rows, t->s.tl_rec, t->s.tl_hits, t->s.tl_span, par, cov, chi2, n_hits, hits);
   return cudaGetLastError();
 }
 cudaError_t launch_dbg_owner(const tpc_tracker* t, int64_t n, int32_t* owner, cudaStream_t st) {
