@@ -77,17 +77,25 @@ a5_select_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int32_t* __res
     const int r = wid * 32 + lane;
     const bool in_row = r < nr;
     const int32_t* col = tl_hits + t0 * nr + r;
-    for (int tb = 0; tb < n_here; tb += A5_UNROLL) {
-      int h[A5_UNROLL];
-      uint32_t ow[A5_UNROLL];
+    // the table entries of the next batch are requested while the owner words of this one are in flight
+    auto load_batch = [&](int tb, int* h) {
 #pragma unroll
-      for (int u = 0; u < A5_UNROLL; ++u) {
+      for (int u = 0; u < A5_UNROLL; ++u) {   // rows outside the tracklet's span hold nothing
         const uint32_t sp = s_span[min(tb + u, A5_TILE - 1)];
         const bool in_span = in_row && tb + u < n_here && r >= (int)(sp & 0xffu) && r <= (int)((sp >> 8) & 0xffu);
         h[u] = in_span ? col[(int64_t)(tb + u) * nr] : -1;
       }
+    };
+    int hn[A5_UNROLL];
+    load_batch(0, hn);
+    for (int tb = 0; tb < n_here; tb += A5_UNROLL) {
+      int h[A5_UNROLL];
+      uint32_t ow[A5_UNROLL];
+#pragma unroll
+      for (int u = 0; u < A5_UNROLL; ++u) h[u] = hn[u];
 #pragma unroll
       for (int u = 0; u < A5_UNROLL; ++u) ow[u] = h[u] >= 0 ? owner[h[u]] : 0u;
+      load_batch(tb + A5_UNROLL, hn);   // beyond the tile: all -1, no loads
 #pragma unroll
       for (int u = 0; u < A5_UNROLL; ++u) {
         if (tb + u < n_here) {   // warp-uniform
