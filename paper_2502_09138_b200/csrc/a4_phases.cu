@@ -469,7 +469,7 @@ __device__ __forceinline__ void phase_c(const Env& e) {
     const float dx = -e.s_row_dx[max(b.row - 1, 0)];
     int hy = YZ_NONE, hz = 0;
     if (live) {   // rolling two-deep pipeline over the stream on the way down
-      ld_cg_yz_if(s1_y, s1_z, t.yz + trow, s1_row != trow);
+      ld_ca_yz_if(s1_y, s1_z, t.yz + trow, s1_row != trow);
       hy = s1_y;
       hz = s1_z;
       const int n1 = trow - 1, n2 = trow - 2;
@@ -477,9 +477,9 @@ __device__ __forceinline__ void phase_c(const Env& e) {
       s1_y = s2_y;
       s1_z = s2_z;
       s1_row = n1 >= t.r0 ? n1 : -1;
-      ld_cg_yz_if(s1_y, s1_z, t.yz + n1, !have1 && n1 >= t.r0);
+      ld_ca_yz_if(s1_y, s1_z, t.yz + n1, !have1 && n1 >= t.r0);
       s2_row = n2 >= t.r0 ? n2 : -1;
-      ld_cg_yz_if(s2_y, s2_z, t.yz + n2, n2 >= t.r0);
+      ld_ca_yz_if(s2_y, s2_z, t.yz + n2, n2 >= t.r0);
     }
     bool ok = live;
     if (tr) ok = transport<true>(g, dx, p, C);

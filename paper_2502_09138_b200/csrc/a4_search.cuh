@@ -80,6 +80,12 @@ __device__ __forceinline__ void ld_cg_yz_if(int& y, int& z, const int2* p, bool 
   asm volatile("{ .reg .pred q; setp.ne.s32 q, %2, 0; @q ld.global.cg.v2.s32 {%0, %1}, [%3]; }"
                : "+r"(y), "+r"(z) : "r"((int)pred), "l"(p) : "memory");
 }
+// the same in a kernel that only reads the stream (phase C: written by earlier launches): through L1, where the other
+// three entries of the 32-byte group are found when their rows come up
+__device__ __forceinline__ void ld_ca_yz_if(int& y, int& z, const int2* p, bool pred) {
+  asm volatile("{ .reg .pred q; setp.ne.s32 q, %2, 0; @q ld.global.ca.v2.s32 {%0, %1}, [%3]; }"
+               : "+r"(y), "+r"(z) : "r"((int)pred), "l"(p) : "memory");
+}
 __device__ __forceinline__ void ld_u32_if(uint32_t& v, const uint32_t* p, bool pred) {
   asm volatile("{ .reg .pred q; setp.ne.s32 q, %1, 0; @q ld.global.nc.u32 %0, [%2]; }" : "+r"(v) : "r"((int)pred), "l"(p));
 }
