@@ -22,7 +22,7 @@ constexpr int A3_ITEMS = A3_TILE / A3_THREADS;
 __global__ void __launch_bounds__(A3_THREADS, 8)
 a3_seeds_kernel(const DevGeom g, int64_t n, const uint32_t* __restrict__ ro, const int32_t* __restrict__ up,
                 const int32_t* __restrict__ dn, int32_t* __restrict__ clean_up, const int4* __restrict__ srt,
-                int4* __restrict__ seed_tmp,
+                int4* __restrict__ seed_tmp, uint32_t* __restrict__ seed_mask,
                 DevCtl* __restrict__ ctl, uint64_t* __restrict__ status, uint32_t n_tiles, uint32_t s_cap) {
   __shared__ uint32_t wsum[33];
   __shared__ uint32_t sh_tile;
@@ -110,7 +110,11 @@ a3_seeds_kernel(const DevGeom g, int64_t n, const uint32_t* __restrict__ ro, con
         const int mid = (lo + hi) >> 1;
         if (ro[mid] <= p) lo = mid; else hi = mid;
       }
-      if (excl + pos < s_cap) seed_tmp[excl + pos] = make_int4((int)p, srt[p].z, lo, 0);
+      if (excl + pos < s_cap) {
+        const int id = srt[p].z;
+        seed_tmp[excl + pos] = make_int4((int)p, id, lo, 0);
+        atomicOr(&seed_mask[id >> 5], 1u << (id & 31));   // for a3_rank_kernel's long rows
+      }
       ++pos;
     }
   if (tile == n_tiles - 1 && threadIdx.x == 0) {
@@ -121,9 +125,16 @@ a3_seeds_kernel(const DevGeom g, int64_t n, const uint32_t* __restrict__ ro, con
 }
 
 // P14: seed rank = ascending start id.  seed_tmp is in position order; the seeds of one (sector,row) are adjacent in
-// it and fill the same rank range in both orders.
+// it and fill the same rank range in both orders: rank = seeds of earlier rows + seeds of the own row with a smaller
+// id.  Rows with a few seeds (central events: two per row): both counts by walking the neighbours in seed_tmp.  A
+// walk that does not reach the row's ends within A3_RANK_WALK seeds (pile-up: a thousand seeds in a row, and the walk
+// is quadratic) is replaced by a binary search for the row's first seed and a population count over the row's part
+// of the seed bit mask (bit = cluster id).  Both give the same number.
+constexpr int A3_RANK_WALK = 24;
+
 __global__ void __launch_bounds__(256)
-a3_rank_kernel(const DevCtl* __restrict__ ctl, const int4* __restrict__ seed_tmp, const int4* __restrict__ srt,
+a3_rank_kernel(const DevCtl* __restrict__ ctl, const uint32_t* __restrict__ ro, const int4* __restrict__ seed_tmp,
+               const uint32_t* __restrict__ seed_mask, const int4* __restrict__ srt,
                const int32_t* __restrict__ clean_up,
                int32_t* __restrict__ seed_start, int32_t* __restrict__ seed_pos, int32_t* __restrict__ seed_sr,
                int4* __restrict__ seed_rec) {
@@ -134,18 +145,41 @@ a3_rank_kernel(const DevCtl* __restrict__ ctl, const int4* __restrict__ seed_tmp
     const int4 c0 = srt[me.x];     // the seed's first cluster and (requested before the counting loops) its second
     const int4 c1 = srt[up0];
     int64_t left = 0, smaller = 0;
+    bool whole = true;   // both walks reached the ends of the row
     for (int64_t j = k - 1; j >= 0; --j) {
       const int4 o = seed_tmp[j];
       if (o.z != me.z) break;
+      if (left == A3_RANK_WALK) { whole = false; break; }
       ++left;
       smaller += o.y < me.y;
     }
-    for (int64_t j = k + 1; j < ns; ++j) {
-      const int4 o = seed_tmp[j];
-      if (o.z != me.z) break;
-      smaller += o.y < me.y;
+    if (whole) {
+      int steps = 0;
+      for (int64_t j = k + 1; j < ns; ++j) {
+        const int4 o = seed_tmp[j];
+        if (o.z != me.z) break;
+        if (steps == A3_RANK_WALK) { whole = false; break; }
+        ++steps;
+        smaller += o.y < me.y;
+      }
     }
-    const int64_t rank = k - left + smaller;
+    int64_t rank = k - left + smaller;
+    if (!whole) {
+      int64_t lo = -1, hi = k;   // first seed of the row: smallest index whose (sector,row) is this one
+      while (hi - lo > 1) {
+        const int64_t mid = (lo + hi) >> 1;
+        if (seed_tmp[mid].z < me.z) lo = mid; else hi = mid;
+      }
+      const uint32_t a = ro[me.z], id = (uint32_t)me.y;   // ids of the row: a .. ; seeds with an id in [a, id)
+      uint32_t cnt = 0;
+      for (uint32_t w = a >> 5; w <= id >> 5; ++w) {
+        uint32_t m = seed_mask[w];
+        if (w == a >> 5) m &= ~0u << (a & 31);
+        if (w == id >> 5) m &= (1u << (id & 31)) - 1u;
+        cnt += __popc(m);
+      }
+      rank = hi + cnt;
+    }
     seed_start[rank] = me.y;
     seed_pos[rank] = me.x;
     seed_sr[rank] = me.z;
@@ -160,12 +194,12 @@ a3_rank_kernel(const DevCtl* __restrict__ ctl, const int4* __restrict__ seed_tmp
 cudaError_t launch_a3_seeds(const tpc_tracker* t, const uint32_t* ro, int64_t n, cudaStream_t st) {
   if (t->tiles_a3 == 0 || n == 0) return cudaSuccess;
   const uint32_t tiles = (uint32_t)((n + A3_TILE - 1) / A3_TILE);
-  a3_seeds_kernel<<<tiles, A3_THREADS, 0, st>>>(t->g, n, ro, t->s.link_up, t->s.link_dn, t->s.clean_up, t->s.srt, t->s.seed_tmp,
+  a3_seeds_kernel<<<tiles, A3_THREADS, 0, st>>>(t->g, n, ro, t->s.link_up, t->s.link_dn, t->s.clean_up, t->s.srt, t->s.seed_tmp, t->s.seed_mask,
                                                t->s.ctl, t->s.scan_a3, tiles, (uint32_t)t->s_cap);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   // the seed count stays on the device: a grid-stride kernel sized for the device, not for the capacity
-  a3_rank_kernel<<<t->a4_sms * 8, 256, 0, st>>>(t->s.ctl, t->s.seed_tmp, t->s.srt, t->s.clean_up, t->s.seed_start, t->s.seed_pos,
+  a3_rank_kernel<<<t->a4_sms * 8, 256, 0, st>>>(t->s.ctl, ro, t->s.seed_tmp, t->s.seed_mask, t->s.srt, t->s.clean_up, t->s.seed_start, t->s.seed_pos,
                                                t->s.seed_sr, t->s.seed_rec);
   return cudaGetLastError();
 }

@@ -59,6 +59,7 @@ size_t layout(tpc_tracker* t, char* base, int64_t n, int64_t R) {
   s.scan_a3 = (uint64_t*)take((size_t)tiles_a3 * 8);
   s.scan_a5 = (uint64_t*)take((size_t)tiles_a5 * 8);
   s.sec_key = (uint32_t*)take((size_t)(t->g.n_sectors > 0 ? t->g.n_sectors : 1) * 4);
+  s.seed_mask = (uint32_t*)take((size_t)(n / 32 + 1) * 4);
   const size_t ctl_bytes = off;
   s.srt = (int4*)take((size_t)n * 16 + 64);
   s.bin_start = (uint32_t*)take((size_t)R * t->g.nb_stride * 4);

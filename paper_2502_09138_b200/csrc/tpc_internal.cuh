@@ -73,6 +73,7 @@ struct Scratch {
                             // none): the downward refit streams these instead of gathering clusters by id
   // control
   DevCtl* ctl;
+  uint32_t* seed_mask;      // [n/32 + 1] a3: bit id set iff cluster id starts a kept seed (zeroed per call)
   uint64_t* scan_a3;        // look-back status words
   uint64_t* scan_a5;        // two channels per tile
   // host-buffer path staging
