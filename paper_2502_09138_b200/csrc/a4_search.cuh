@@ -107,26 +107,38 @@ __device__ __forceinline__ void load_ranges_if(const DevGeom& g, const uint32_t*
 
 // P17/P21: among the candidates minimise (d, id), d = dy^2/(Cyy + sy2) + dz^2/(Czz + sz2), restricted to
 // |dy| <= gate_y and |dz| <= gate_z (cm).  Accumulates into (f, bestd); the caller applies the gate d < gate_d.
+__device__ __forceinline__ void search_take(const DevGeom& g, const int4& c, const State& p, float wy, float wz,
+                                            Found& f, float& bestd) {
+  const float dy = resid_y(g, p, c.x), dz = resid_z(g, p, c.y);
+  if (fabsf(dy) > g.gate_y || fabsf(dz) > g.gate_z) return;
+  const float d = dy * dy * wy + dz * dz * wz;
+  if (d < bestd || (d == bestd && c.z < f.id)) {
+    bestd = d;
+    f.id = c.z;
+    f.hy = c.x;
+    f.hz = c.y;
+    f.ry = dy;
+    f.rz = dz;
+  }
+}
+
 __device__ __forceinline__ void search_ranges(const DevGeom& g, const BinRanges& q, const State& p, float wy, float wz,
                                               const int4* __restrict__ srt, Found& f, float& bestd) {
   const uint32_t n0 = q.b0 - q.a0, total = n0 + (q.b1 - q.a1);
   if (total) {
-    int4 nx = srt[n0 ? q.a0 : q.a1];
-    for (uint32_t t = 0; t < total; ++t) {   // one flat loop over both z-bins
+    // a search has 1.8 candidates on average: the first two are requested together and tested in line, the flat loop
+    // over both z-bins takes over from the third (an index beyond the last re-reads the last: never tested)
+    auto at = [&](uint32_t t) { t = min(t, total - 1); return t < n0 ? q.a0 + t : q.a1 + (t - n0); };
+    const int4 c0 = srt[at(0)], c1 = srt[at(1)], c2 = srt[at(2)], c3 = srt[at(3)];
+    int4 nx = srt[at(4)];
+    search_take(g, c0, p, wy, wz, f, bestd);
+    if (total > 1) search_take(g, c1, p, wy, wz, f, bestd);
+    if (total > 2) search_take(g, c2, p, wy, wz, f, bestd);
+    if (total > 3) search_take(g, c3, p, wy, wz, f, bestd);
+    for (uint32_t t = 4; t < total; ++t) {
       const int4 c = nx;
-      const uint32_t tn = min(t + 1, total - 1);   // next one in flight (the last iteration re-reads itself)
-      nx = srt[tn < n0 ? q.a0 + tn : q.a1 + (tn - n0)];
-      const float dy = resid_y(g, p, c.x), dz = resid_z(g, p, c.y);
-      if (fabsf(dy) > g.gate_y || fabsf(dz) > g.gate_z) continue;
-      const float d = dy * dy * wy + dz * dz * wz;
-      if (d < bestd || (d == bestd && c.z < f.id)) {
-        bestd = d;
-        f.id = c.z;
-        f.hy = c.x;
-        f.hz = c.y;
-        f.ry = dy;
-        f.rz = dz;
-      }
+      nx = srt[at(t + 1)];   // next one in flight
+      search_take(g, c, p, wy, wz, f, bestd);
     }
   }
 }
