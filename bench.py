@@ -635,7 +635,7 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--streams", type=int, default=0, help="handles/streams of the device arm; 0 = sweep 1..4")
-    ap.add_argument("--e2e-threads", type=int, default=6, help="host threads (handles, streams) of the e2e arm")
+    ap.add_argument("--e2e-threads", type=int, default=8, help="host threads (handles, streams) of the e2e arm")
     ap.add_argument("--selftest-ranks", action="store_true", help="CPU check of the multi-rank plumbing (gloo)")
     ap.add_argument("--a2-variant", type=int, default=0, help="0 = direct a2 (default), 1 = TMA-staged rows (evidence run)")
     ap.add_argument("--config", type=int, default=None, choices=[0, 1, 2, 3, 30, 4],
