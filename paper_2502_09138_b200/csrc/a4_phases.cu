@@ -34,6 +34,8 @@ struct Env {   // everything a warp needs that does not change during a kernel
   const float* s_row_dx;
   int2* s_yz;              // this lane's staging column for the (y, z) stream: slot k at s_yz[k * AP_THREADS]
   int* s_tab;              // likewise for the hit table: eight rows = one 32-byte group
+  uint32_t* q_buf;         // this warp's collected queue items [2 slots][A4_Q_BUCKETS][A4_Q_BATCH] and their counts
+  int* q_cnt;
   bool tab_groups;         // n_rows is a multiple of 8: every aligned group of eight rows lies inside the tracklet's table
   float bucket_scale;      // A4_Q_BUCKETS / n_rows
   int yz_stride;           // entries per tracklet in tl_yz: n_rows rounded up to a multiple of 4 (32-byte groups)
@@ -123,20 +125,54 @@ __device__ __forceinline__ int len_bucket(const Env& e, int rows_left) {
   return b < 0 ? 0 : b;
 }
 
-// Producer side (lanes with pred, after state_save): one atomic per warp and bucket.
-__device__ __forceinline__ void queue_push(const Env& e, int q, int bucket, int i, bool pred) {
+// Producer side (lanes with pred, after state_save).  A warp collects the items it produces per (queue, bucket) in
+// shared memory and hands them over A4_Q_BATCH at a time: the fetch-add that claims their place in the queue -- a
+// round trip the warp waits for -- is paid once per batch instead of in every step in which a lane leaves.
+constexpr int A4_Q_BATCH = 16;
+
+__device__ __forceinline__ void queue_flush(const Env& e, int q, int slot, int bk) {
+  const int n = e.q_cnt[slot * A4_Q_BUCKETS + bk];
+  if (n == 0) return;   // warp-uniform
+  const int qq = q * A4_Q_BUCKETS + bk;
+  uint32_t base = 0;
+  if (e.lane == 0) base = atomicAdd(&e.ctl->q_alloc[qq].v, (uint32_t)n);
+  base = __shfl_sync(0xffffffffu, base, 0);
+  if (e.lane < n)
+    e.q_items[(size_t)qq * e.s_cap + base + e.lane] = e.q_buf[(slot * A4_Q_BUCKETS + bk) * A4_Q_BATCH + e.lane];
+  __syncwarp();
+  if (e.lane == 0) e.q_cnt[slot * A4_Q_BUCKETS + bk] = 0;
+  __syncwarp();
+}
+
+// slot: which of the phase's destination queues (0, or 1 for phase A's second one)
+__device__ __forceinline__ void queue_push(const Env& e, int q, int slot, int bucket, int i, bool pred) {
   unsigned todo = __ballot_sync(0xffffffffu, pred);
   while (todo) {   // one round per distinct bucket among the leaving lanes (usually one or two)
     const int bk = __shfl_sync(0xffffffffu, bucket, __ffs(todo) - 1);
     const bool mine = pred && bucket == bk;
     const unsigned m = __ballot_sync(0xffffffffu, mine);
-    const int qq = q * A4_Q_BUCKETS + bk;
-    const int leader = __ffs(m) - 1;
-    uint32_t base = 0;
-    if (e.lane == leader) base = atomicAdd(&e.ctl->q_alloc[qq].v, (uint32_t)__popc(m));
-    base = __shfl_sync(0xffffffffu, base, leader);
-    if (mine) e.q_items[(size_t)qq * e.s_cap + base + __popc(m & ((1u << e.lane) - 1u))] = (uint32_t)i;
+    const int cell = slot * A4_Q_BUCKETS + bk;
+    int done = 0;   // items of this round already stored
+    const int total = __popc(m), rank = __popc(m & ((1u << e.lane) - 1u));
+    while (done < total) {   // at most three rounds (32 lanes, batches of 16)
+      const int have = e.q_cnt[cell];
+      const int take = min(total - done, A4_Q_BATCH - have);
+      if (mine && rank >= done && rank < done + take) e.q_buf[cell * A4_Q_BATCH + have + rank - done] = (uint32_t)i;
+      __syncwarp();
+      if (e.lane == 0) e.q_cnt[cell] = have + take;
+      __syncwarp();
+      done += take;
+      if (have + take == A4_Q_BATCH) queue_flush(e, q, slot, bk);
+    }
     todo &= ~m;
+  }
+}
+
+// before a warp leaves a phase kernel: everything it still holds
+__device__ __forceinline__ void queue_flush_all(const Env& e, int q0, int q1) {
+  for (int bk = 0; bk < A4_Q_BUCKETS; ++bk) {
+    queue_flush(e, q0, 0, bk);
+    if (q1 >= 0) queue_flush(e, q1, 1, bk);
   }
 }
 
@@ -255,7 +291,10 @@ __device__ __forceinline__ void phase_a(const Env& e) {
         live = true;
       }
     }
-    if (!__any_sync(FULL, live)) return;
+    if (!__any_sync(FULL, live)) {
+      queue_flush_all(e, Q_B, Q_C);
+      return;
+    }
 
     if (live && first) cov_reset(g, C);   // P19
     const bool tr = live && !first;
@@ -289,8 +328,8 @@ __device__ __forceinline__ void phase_a(const Env& e) {
     }
     if (leave) state_save(e, t, p, C, b);
     const bool to_b = leave && ok && b.row + 1 < g.n_rows;
-    queue_push(e, Q_B, len_bucket(e, g.n_rows - 1 - b.row), t.i, to_b);
-    queue_push(e, Q_C, len_bucket(e, b.row - t.r0), t.i, leave && !to_b);
+    queue_push(e, Q_B, 0, len_bucket(e, g.n_rows - 1 - b.row), t.i, to_b);
+    queue_push(e, Q_C, 1, len_bucket(e, b.row - t.r0), t.i, leave && !to_b);
     if (leave) live = false;
   }
 }
@@ -377,7 +416,10 @@ __device__ __forceinline__ void phase_b(const Env& e) {
         live = true;
       }
     }
-    if (!__any_sync(FULL, live)) return;
+    if (!__any_sync(FULL, live)) {
+      queue_flush_all(e, Q_C, -1);
+      return;
+    }
 
     const int trow = b.row + 1;   // a live lane always has a row above and fewer than max_miss misses
     const float dx = e.s_row_dx[b.row];
@@ -419,7 +461,7 @@ __device__ __forceinline__ void phase_b(const Env& e) {
       dirty_t = false;
     }
     if (leave) state_save(e, t, p, C, b);
-    queue_push(e, Q_C, len_bucket(e, b.row - t.r0), t.i, leave);
+    queue_push(e, Q_C, 0, len_bucket(e, b.row - t.r0), t.i, leave);
     if (leave) live = false;
   }
 }
@@ -456,7 +498,10 @@ __device__ __forceinline__ void phase_c(const Env& e) {
         live = true;
       }
     }
-    if (!__any_sync(FULL, live)) return;
+    if (!__any_sync(FULL, live)) {
+      queue_flush_all(e, Q_D, -1);
+      return;
+    }
 
     if (live && first) {   // P22
       cov_reset(g, C);
@@ -492,7 +537,7 @@ __device__ __forceinline__ void phase_c(const Env& e) {
     }
     const bool leave = live && (!ok || b.row <= t.r0);   // below the seed's first row phase D searches
     if (leave) state_save(e, t, p, C, b);
-    queue_push(e, Q_D, len_bucket(e, b.row), t.i, leave);
+    queue_push(e, Q_D, 0, len_bucket(e, b.row), t.i, leave);
     if (leave) live = false;
   }
 }
@@ -646,6 +691,8 @@ a4_phase_kernel(const DevGeom g, uint32_t s_cap, DevCtl* __restrict__ ctl, const
   extern __shared__ double smem_ap[];
   __shared__ int2 s_yz[4][AP_THREADS];
   __shared__ int s_tab[8][AP_THREADS];
+  __shared__ uint32_t s_qbuf[AP_THREADS / 32][2 * A4_Q_BUCKETS * A4_Q_BATCH];
+  __shared__ int s_qcnt[AP_THREADS / 32][2 * A4_Q_BUCKETS];
   const int nr = g.n_rows;
   const uint32_t n_seeds = ctl->n_seeds;
   if (n_seeds == 0) return;
@@ -665,6 +712,10 @@ a4_phase_kernel(const DevGeom g, uint32_t s_cap, DevCtl* __restrict__ ctl, const
   e.n_seeds = n_seeds; e.s_cap = s_cap;
   e.s_yz = &s_yz[0][threadIdx.x];
   e.s_tab = &s_tab[0][threadIdx.x];
+  e.q_buf = &s_qbuf[threadIdx.x >> 5][0];
+  e.q_cnt = &s_qcnt[threadIdx.x >> 5][0];
+  if ((threadIdx.x & 31) < 2 * A4_Q_BUCKETS) s_qcnt[threadIdx.x >> 5][threadIdx.x & 31] = 0;
+  __syncwarp();
   e.tab_groups = (nr & 7) == 0;
   e.yz_stride = (nr + 3) & ~3;
   e.bucket_scale = (float)A4_Q_BUCKETS / (float)nr;
