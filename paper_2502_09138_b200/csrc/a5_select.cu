@@ -161,14 +161,21 @@ a5_select_kernel(const DevGeom g, DevCtl* __restrict__ ctl, const int32_t* __res
     uint32_t w = sh_off[t];
     if (w == 0xFFFFFFFFu) continue;
     const int32_t* src = tl_hits + (t0 + t) * nr;
-    for (int k = 0; k < n_words; ++k) {
-      const unsigned m = own_mask[t][k];
-      if ((m >> lane) & 1u) {
-        const uint32_t at = w + __popc(m & ((1u << lane) - 1u));
-        hit_ids[at] = src[k * 32 + lane];
+    int v[A5_MASK_WORDS];   // all loads of the tracklet first, then the stores
+    unsigned mk[A5_MASK_WORDS];
+#pragma unroll
+    for (int k = 0; k < A5_MASK_WORDS; ++k) {
+      mk[k] = k < n_words ? own_mask[t][k] : 0u;
+      v[k] = ((mk[k] >> lane) & 1u) ? src[k * 32 + lane] : -1;
+    }
+#pragma unroll
+    for (int k = 0; k < A5_MASK_WORDS; ++k) {
+      if ((mk[k] >> lane) & 1u) {
+        const uint32_t at = w + __popc(mk[k] & ((1u << lane) - 1u));
+        hit_ids[at] = v[k];
         hit_row[at] = (uint8_t)(k * 32 + lane);   // for a6 (tpc_refit): the row of every output hit
       }
-      w += __popc(m);
+      w += __popc(mk[k]);
     }
   }
   if (tile == n_tiles - 1 && threadIdx.x == 0) {
