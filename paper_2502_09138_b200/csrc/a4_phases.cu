@@ -676,10 +676,10 @@ a4_votes_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, const float4* _
   }
 }
 
-// Resident CTAs per SM (measured, profiles/r02_a4_occupancy.md): the three phases that gather clusters run best at
-// 16 warps per SM -- at 20 or 24 they are slower, at 12 equal, at 8 slower: they sit between gather latency and the
-// DRAM's random-sector rate -- while the refit phase streams its measurements and gains up to 28 warps.
-constexpr int ap_min_blocks(int ph) { return ph == 2 ? 7 : 4; }
+// Resident CTAs per SM (measured per phase, profiles/r02_summary.md): the two phases that search run best at 16 warps
+// per SM (5 CTAs: B +0.06, D +0.03 ms; 3: slower too), the chain fit at 20 (4: +0.01, 6: +0.03 ms), the refit phase,
+// which streams its measurements, at 28 (6 or 8 CTAs: +0.01 / +0.03 ms).
+constexpr int ap_min_blocks(int ph) { return ph == 2 ? 7 : (ph == 0 ? 5 : 4); }
 
 template <int PH>
 __global__ void __launch_bounds__(AP_THREADS, ap_min_blocks(PH))
