@@ -677,9 +677,10 @@ a4_votes_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, const float4* _
 }
 
 // Resident CTAs per SM (measured per phase, profiles/r02_summary.md): the two phases that search run best at 16 warps
-// per SM (5 CTAs: B +0.06, D +0.03 ms; 3: slower too), the chain fit at 20 (4: +0.01, 6: +0.03 ms), the refit phase,
-// which streams its measurements, at 28 (6 or 8 CTAs: +0.01 / +0.03 ms).
-constexpr int ap_min_blocks(int ph) { return ph == 2 ? 7 : (ph == 0 ? 5 : 4); }
+// per SM (5 CTAs: B +0.06, D +0.03 ms; 3: slower too), the refit phase, which streams its measurements, at 28 (6 or
+// 8 CTAs: +0.01 / +0.03 ms).  The chain fit alone on the GPU is 0.01 ms faster at 20 warps than at 16 (24: +0.03),
+// but with a second call on a second stream the step is 0.7 % slower then: 16.
+constexpr int ap_min_blocks(int ph) { return ph == 2 ? 7 : 4; }
 
 template <int PH>
 __global__ void __launch_bounds__(AP_THREADS, ap_min_blocks(PH))
