@@ -213,6 +213,8 @@ def run_ours(args):
         for K in sweep:
             if world > 1:
                 dist.barrier()
+            for h in handles[:K]:   # the caller says how many calls it keeps in flight (sizes a4's persistent grids)
+                h["trk"].set_concurrency(K)
             ms_k = timed_round_robin(handles[:K], args.steps, main)
             ms_k, units_k = aggregate(ms_k, float(n) * args.steps, dist if world > 1 else None, dev)
             results[K] = (ms_k, units_k)
@@ -222,6 +224,8 @@ def run_ours(args):
     ms_max, units = results[best_k]
     value = units / (ms_max * 1e-3)
 
+    for h in handles:
+        h["trk"].set_concurrency(1)
     # ---- stage times: a separate pass on one stream with CUDA events between the stages ---------------------
     trk.set_stage_timing(True)
     for _ in range(min(args.steps, 16)):
@@ -379,6 +383,7 @@ def run_ours(args):
              "tr": torch.empty(out.tracks.shape[0], dtype=torch.uint8).pin_memory(),
              "hi": torch.empty(out.hit_ids.shape[0], dtype=torch.int32).pin_memory(),
              "cn": torch.zeros(4, dtype=torch.int32).pin_memory()}
+        w["trk"].set_concurrency(T)
         workers.append(w)
 
     def run_host(w, n_calls):

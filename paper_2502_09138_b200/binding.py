@@ -160,6 +160,7 @@ def load_library():
     lib.tpc_scratch_bytes.restype = C.c_int64
     lib.tpc_launches_per_call.argtypes = [C.c_void_p]
     lib.tpc_reserve_seeds.argtypes = [C.c_void_p, C.c_int64]
+    lib.tpc_set_concurrency.argtypes = [C.c_void_p, C.c_int32]
     lib.tpc_debug_set_a4_variant.argtypes = [C.c_void_p, C.c_int]
     lib.tpc_debug_set_a2_variant.argtypes = [C.c_void_p, C.c_int]
     lib.tpc_set_stage_timing.argtypes = [C.c_void_p, C.c_int]
@@ -478,6 +479,10 @@ class Tracker:
         dn = torch.empty(n, dtype=torch.int32, device="cuda")
         self._check(self._lib.tpc_debug_copy_links(self._h, 1 if cleaned else 0, _ptr(up), _ptr(dn), self._stream_ptr(None)))
         return up.cpu().numpy(), dn.cpu().numpy()
+
+    def set_concurrency(self, k: int):
+        """tpc_set_concurrency: how many tpc_track calls the caller keeps in flight on the device at the same time."""
+        self._check(self._lib.tpc_set_concurrency(self._h, int(k)))
 
     def reserve_seeds(self, n_seeds: int):
         """tpc_reserve_seeds: raise the handle's seed capacity (after TPC_FLAG_SEED_OVERFLOW)."""

@@ -681,6 +681,10 @@ a4_votes_kernel(const DevGeom g, const DevCtl* __restrict__ ctl, const float4* _
 // 8 CTAs: +0.01 / +0.03 ms).  The chain fit alone on the GPU is 0.01 ms faster at 20 warps than at 16 (24: +0.03),
 // but with a second call on a second stream the step is 0.7 % slower then: 16.
 constexpr int ap_min_blocks(int ph) { return ph == 2 ? 7 : 4; }
+// CTAs per SM actually launched.  A call that shares the GPU with other calls (K handles on K streams) leaves CTA
+// slots to them: with three streams 3 / 4 (C) per SM give 6.42 G clusters/s against 6.21 at 4 / 7, alone 5.32 against
+// 5.64 (profiles/r02_summary.md).
+constexpr int ap_grid_blocks(int ph, bool shared) { return shared ? (ph == 2 ? 4 : 3) : ap_min_blocks(ph); }
 
 template <int PH>
 __global__ void __launch_bounds__(AP_THREADS, ap_min_blocks(PH))
@@ -735,8 +739,9 @@ a4_phase_kernel(const DevGeom g, uint32_t s_cap, DevCtl* __restrict__ ctl, const
 cudaError_t launch_a4_phases(const tpc_tracker* t, int64_t n, cudaStream_t st) {
   if (n == 0 || t->s_cap == 0) return cudaSuccess;
   const size_t smem = (size_t)t->g.n_rows * (8 + 4);
+  const bool shared = t->concurrency >= 2;   // tpc_set_concurrency: other calls run next to this one
 #define AP_LAUNCH(PH)                                                                                         \
-  a4_phase_kernel<PH><<<t->a4_sms * ap_min_blocks(PH), AP_THREADS, smem, st>>>(                                                \
+  a4_phase_kernel<PH><<<t->a4_sms * ap_grid_blocks(PH, shared), AP_THREADS, smem, st>>>(                                                \
       t->g, (uint32_t)t->s_cap, t->s.ctl, t->s.srt, t->s.clean_up, t->s.sec_key, t->s.bin_start, t->s.seed_rec, \
       t->s.tl_rec, t->s.tl_hits, t->s.tl_yz, t->s.tl_state, t->s.q_items, t->s.tl_span)
   AP_LAUNCH(0);

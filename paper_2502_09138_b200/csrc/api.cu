@@ -612,6 +612,12 @@ int64_t tpc_scratch_bytes(const tpc_tracker_t* t) { return t ? (int64_t)(t->aren
 
 int tpc_launches_per_call(const tpc_tracker_t* t) { return t ? (t->a4_phased ? 12 : 8) : 0; }
 
+int tpc_set_concurrency(tpc_tracker_t* t, int32_t k) {
+  if (!t || k < 1) return TPC_ERR_ARG;
+  t->concurrency = k;
+  return TPC_OK;
+}
+
 int tpc_reserve_seeds(tpc_tracker_t* t, int64_t n_seeds) {
   if (!t || n_seeds < 0) return TPC_ERR_ARG;
   if (n_seeds > t->seed_reserve) t->seed_reserve = n_seeds;

@@ -101,6 +101,7 @@ struct tpc_tracker {
   int64_t seed_reserve;      // tpc_reserve_seeds: lower bound on s_cap
   int64_t tiles_a3, tiles_a5;
   int a4_phased;             // the most recent call ran a4 as phase kernels (api.cu)
+  int concurrency;           // tpc_set_concurrency: calls the caller keeps in flight on the device (0 / 1: this one alone)
   int a2_variant;            // tpc_debug_set_a2_variant: 0 = direct kernels, 1 = shared-memory staged rows (sparse calls)
   int a4_variant;            // tpc_debug_set_a4_variant: 0 = by call size, 1 = uniform kernel, 2 = phase kernels
   int a4_sms;              // SMs of the device (phase kernels size their own persistent grids)

@@ -938,6 +938,30 @@ def test_host_entry_copies_the_hit_lists_that_fitted(orc):
     trk.close()
 
 
+def test_concurrency_hint_changes_no_result():
+    """tpc_set_concurrency only sizes a4's persistent grids: the output of a call is byte for byte the same."""
+    import torch
+    from paper_2502_09138_b200 import Tracker
+    from paper_2502_09138_b200.binding import TpcError
+    from paper_2502_09138_b200.events import geometry_from_event, upload
+    ev = make_event(1, 1003)
+    trk = Tracker(geometry_from_event(ev))
+    trk.set_a4_variant(2)              # the phase kernels are the ones the hint acts on
+    y, z, ro = upload(ev)
+    ref = trk.track(y, z, ro)
+    ref_tracks, ref_hits = ref.tracks.clone(), ref.hit_ids.clone()
+    ref_counts = ref.counts.cpu().tolist()
+    for k in (3, 8, 1):
+        trk.set_concurrency(k)
+        out = trk.track(y, z, ro)
+        assert out.counts.cpu().tolist() == ref_counts, k
+        nt, nh = ref_counts[0], ref_counts[1]
+        assert torch.equal(out.tracks[: nt * 112], ref_tracks[: nt * 112]) and torch.equal(out.hit_ids[:nh], ref_hits[:nh]), k
+    with pytest.raises(TpcError):
+        trk.set_concurrency(0)
+    trk.close()
+
+
 def test_deterministic_run_to_run(orc):
     ev = make_event(4, n_tracks=800)
     a = _run_gpu(ev)
